@@ -1,0 +1,120 @@
+"""Adjoint (vector-Jacobian) right-hand side and adjoint-state driver (oracle, fp64).
+
+Test infrastructure only; see oracle/__init__.py.
+
+PAPER.md:210-228, Eqs. (27)-(30): after the forward solve, the system
+    dm/dt = f(t, m),           m(T) = m_output
+    da/dt = -(df/dm)^T a,      a(T) = grad_y L
+    du/dt = -(df/dtheta)^T a,  u(T) = 0
+is integrated backwards in time and u(0) = grad_theta L.  (Eq. 29 prints the products without
+the transpose; the adjoint variable multiplies the Jacobian from the left, as in the cited
+neural-ODE reference 26.)  The paper delegates both products to framework autodiff
+(PAPER.md:288); C7 of SURVEY.md §8(c) writes them out for theta = Ms (cell-wise):
+
+  H = Hlin(m) + H_zeeman,  Hlin = exchange + anisotropy + demag (linear in m),
+  f = -g' m x H - alpha g' m x (m x H),  g' = gamma/(1+alpha^2)
+
+  b = (df/dH)^T a       = g' m x a - alpha g' m x (m x a)
+  d = (df/dm|_H)^T a    = -g' H x a - alpha g' [(m.H) a + (a.m) H - 2 (a.H) m]
+  (df/dm)^T a           = d + Hlin^T b,   Hlin^T b = L o Hlin(b / L)     (L Hlin is symmetric)
+  (df/dMs_c)^T a        = - S^T[ b.H / (S Ms) ]_c
+                          + sum_i b_{c+i} . mu0 (M Hext_loc)_i / L_{c+i}
+                          + (S^T q)_c . Hcell_c + mbar_c . Y_c
+     q = b / (S Ms),  mbar = S^T m / 8,  Hcell = -N * (Ms mbar),  Y = -N * (Ms o S^T q)
+"""
+import numpy as np
+
+from . import demag as _demag
+from . import llg as _llg
+from .mesh import (LOCAL, MU0, element_matrices, gather_nodes_to_cells, node_view,
+                   scatter_cells_to_nodes)
+
+
+def _safe_div(num, den):
+    out = np.zeros_like(num)
+    ok = den > 0
+    out[..., ok] = num[..., ok] / den[ok]
+    return out
+
+
+def adjoint_rhs(p, t, m, a, zeeman=None):
+    """Returns (f, dadt, dudt_Ms) = (f(t,m), -(df/dm)^T a, -(df/dMs)^T a)."""
+    gp = p.gamma / (1.0 + p.alpha ** 2)
+    al = p.alpha
+    L = p.L
+    SMs = scatter_cells_to_nodes(p.Ms)
+    h_ext = zeeman(t) if zeeman is not None else None
+    if h_ext is not None:
+        h_ext = np.asarray(h_ext, dtype=np.float64)
+        if h_ext.ndim == 1:
+            h_ext = np.broadcast_to(h_ext[:, None, None, None], m.shape)
+    H = _llg.effective_field(p, m, h_ext)
+    f = _llg.llg_from_field(p, m, H)
+
+    cross = _llg.cross
+    dot = lambda x, y: x[0] * y[0] + x[1] * y[1] + x[2] * y[2]
+    mxa = cross(m, a)
+    b = gp * mxa - al * gp * cross(m, mxa)
+    d = -gp * cross(H, a) - al * gp * (dot(m, H) * a + dot(a, m) * H - 2.0 * dot(a, H) * m)
+
+    # Hlin^T b = L o Hlin(b / L): the same field operators, without the Zeeman term
+    p_lin = _llg.Problem(p.n_cells, p.dx, p.Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha,
+                         p.terms & ~_llg.TERM_ZEEMAN, p._Nt)
+    HTb = L * _llg.effective_field(p_lin, _safe_div(b, L), None)
+    dadt = -(d + HTb)
+
+    # -(df/dMs)^T a
+    grad = -gather_nodes_to_cells(_safe_div(dot(b, H), SMs))
+    if (p.terms & _llg.TERM_ZEEMAN) and h_ext is not None:
+        _, M = element_matrices(p.dx)
+        bL = _safe_div(b, L)
+        for i in LOCAL:
+            for ip in LOCAL:
+                grad = grad + MU0 * M[i + ip] * np.sum(node_view(bL, i) * node_view(h_ext, ip), axis=0)
+    if p.terms & _llg.TERM_DEMAG:
+        q = _safe_div(b, SMs)
+        STq = gather_nodes_to_cells(q)
+        mbar = gather_nodes_to_cells(m) / 8.0
+        Hcell = _demag.demag_field_cells_fft(p.Ms * mbar, p.Nt)
+        Y = _demag.demag_field_cells_fft(p.Ms * STq, p.Nt)
+        grad = grad + np.sum(STq * Hcell, axis=0) + np.sum(mbar * Y, axis=0)
+    return f, dadt, -grad
+
+
+def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
+    """Fixed-step RK4 with renormalisation; returns (m_T, {step index: m}) (C8)."""
+    m = m0.copy()
+    ckpt = {}
+    for s in range(n_steps):
+        if checkpoint_every and s % checkpoint_every == 0:
+            ckpt[s] = m.copy()
+        m = _llg.rk4_step(p, t0 + s * dt, dt, m, zeeman, renormalise=True)
+    return m, ckpt
+
+
+def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0):
+    """Integrate Eq. (29) from T = t0 + n_steps dt back to t0 with RK4 steps of -dt.
+
+    State (m, a, u); m is renormalised after every step and replaced by the stored forward
+    value whenever a checkpoint index is reached (reading C8).  Returns (m0, a0, u0);
+    u0 = dJ/dMs per cell (Eq. 30).
+    """
+    m, a = mT.copy(), aT.copy()
+    u = np.zeros(p.n_cells)
+    h = -dt
+
+    def F(t, m_, a_):
+        return adjoint_rhs(p, t, m_, a_, zeeman)
+
+    for s in range(n_steps, 0, -1):
+        t = t0 + s * dt
+        k1 = F(t, m, a)
+        k2 = F(t + 0.5 * h, m + 0.5 * h * k1[0], a + 0.5 * h * k1[1])
+        k3 = F(t + 0.5 * h, m + 0.5 * h * k2[0], a + 0.5 * h * k2[1])
+        k4 = F(t + h, m + h * k3[0], a + h * k3[1])
+        m = _llg.normalise(m + h / 6.0 * (k1[0] + 2 * k2[0] + 2 * k3[0] + k4[0]))
+        a = a + h / 6.0 * (k1[1] + 2 * k2[1] + 2 * k3[1] + k4[1])
+        u = u + h / 6.0 * (k1[2] + 2 * k2[2] + 2 * k3[2] + k4[2])
+        if checkpoints is not None and (s - 1) in checkpoints:
+            m = checkpoints[s - 1].copy()
+    return m, a, u

@@ -1,0 +1,152 @@
+"""Pins for oracle/adjoint.py (C7, C8 of SURVEY.md §8(c); Eqs. 27-30)."""
+import numpy as np
+import pytest
+
+from oracle import adjoint, llg, mesh
+from oracle.llg import Problem, TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN
+
+ALL = TERM_EXCHANGE | TERM_DEMAG | TERM_ANISO | TERM_ZEEMAN
+
+
+def rand_unit(shape, seed):
+    v = np.random.default_rng(seed).standard_normal((3,) + tuple(shape))
+    return v / np.sqrt(np.sum(v * v, axis=0))
+
+
+def make(n=(3, 2, 2), alpha=0.1, terms=ALL, seed=0):
+    rng = np.random.default_rng(seed)
+    dx = (3e-9, 2.5e-9, 3.5e-9)
+    p = Problem(n, dx, rng.uniform(4e5, 8e5, n), rng.uniform(0.8e-11, 1.3e-11, n),
+                rng.uniform(1e5, 5e5, n), ku_axis=(0.0, 0.6, 0.8), alpha=alpha, terms=terms)
+    hext = rng.standard_normal((3,) + p.node_shape) * 3e4
+    return p, (lambda t: hext)
+
+
+def with_Ms(p, Ms):
+    return Problem(p.n_cells, p.dx, Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha, p.terms, p._Nt)
+
+
+@pytest.mark.parametrize("terms", [ALL, TERM_EXCHANGE | TERM_DEMAG, TERM_DEMAG, TERM_EXCHANGE | TERM_ANISO | TERM_ZEEMAN])
+def test_dense_jacobians_by_finite_differences(terms):
+    """Explicit dense Jacobians of the oracle's own forward RHS by central differences on a
+    3x2x2-cell mesh; both vector-Jacobian products must equal a^T J."""
+    p, zee = make(terms=terms)
+    p.Nt  # build tensor once
+    rng = np.random.default_rng(1)
+    m = rand_unit(p.node_shape, 2) * (1 + 0.05 * rng.standard_normal(p.node_shape))   # |m| != 1 on purpose
+    a = rng.standard_normal(m.shape)
+    f, dadt, dudt = adjoint.adjoint_rhs(p, 0.0, m, a, zee)
+    assert np.allclose(f, llg.llg_rhs(p, 0.0, m, zee), rtol=1e-14)
+    # J_m
+    Jm_T_a = np.zeros(m.size)
+    fl = m.ravel()
+    for k in range(m.size):
+        h = 1e-6
+        mp_, mm_ = fl.copy(), fl.copy()
+        mp_[k] += h
+        mm_[k] -= h
+        col = (llg.llg_rhs(p, 0.0, mp_.reshape(m.shape), zee) - llg.llg_rhs(p, 0.0, mm_.reshape(m.shape), zee)) / (2 * h)
+        Jm_T_a[k] = np.sum(a * col)
+    assert np.allclose(-dadt.ravel(), Jm_T_a, rtol=1e-7, atol=1e-8 * np.abs(Jm_T_a).max())
+    # J_Ms
+    JMs_T_a = np.zeros(p.Ms.size)
+    for k in range(p.Ms.size):
+        h = 1e-4 * p.Ms.ravel()[k]
+        Mp, Mm = p.Ms.ravel().copy(), p.Ms.ravel().copy()
+        Mp[k] += h
+        Mm[k] -= h
+        col = (llg.llg_rhs(with_Ms(p, Mp.reshape(p.n_cells)), 0.0, m, zee)
+               - llg.llg_rhs(with_Ms(p, Mm.reshape(p.n_cells)), 0.0, m, zee)) / (2 * h)
+        JMs_T_a[k] = np.sum(a * col)
+    assert np.allclose(-dudt.ravel(), JMs_T_a, rtol=1e-6, atol=1e-7 * np.abs(JMs_T_a).max())
+
+
+def test_dot_product_test_larger_mesh():
+    """<a, J v> = <J^T a, v> with J v by central differences (6x5x3 cells, all terms)."""
+    p, zee = make(n=(6, 5, 3), seed=3)
+    rng = np.random.default_rng(4)
+    m = rand_unit(p.node_shape, 5)
+    a = rng.standard_normal(m.shape)
+    v = rng.standard_normal(m.shape)
+    w = rng.standard_normal(p.n_cells) * 1e5
+    _, dadt, dudt = adjoint.adjoint_rhs(p, 0.0, m, a, zee)
+    h = 1e-6
+    Jv = (llg.llg_rhs(p, 0.0, m + h * v, zee) - llg.llg_rhs(p, 0.0, m - h * v, zee)) / (2 * h)
+    lhs, rhs = np.sum(a * Jv), np.sum(-dadt * v)
+    assert abs(lhs - rhs) < 1e-8 * abs(lhs)
+    h = 1e-5
+    Jw = (llg.llg_rhs(with_Ms(p, p.Ms + h * w), 0.0, m, zee) - llg.llg_rhs(with_Ms(p, p.Ms - h * w), 0.0, m, zee)) / (2 * h)
+    lhs, rhs = np.sum(a * Jw), np.sum(-dudt * w)
+    assert abs(lhs - rhs) < 1e-6 * abs(lhs)
+
+
+def test_transpose_field_operator_is_L_H_Linv():
+    """H^T b = L o H(b/L) equals the explicit transpose of the dense field matrix."""
+    p, _ = make(terms=TERM_EXCHANGE | TERM_DEMAG | TERM_ANISO)
+    nn = int(np.prod((3,) + p.node_shape))
+    Hmat = np.zeros((nn, nn))
+    for k in range(nn):
+        e = np.zeros(nn)
+        e[k] = 1.0
+        Hmat[:, k] = llg.effective_field(p, e.reshape((3,) + p.node_shape)).ravel()
+    b = np.random.default_rng(6).standard_normal((3,) + p.node_shape)
+    L = p.L
+    got = L * llg.effective_field(p, b / L)
+    assert np.allclose(got.ravel(), Hmat.T @ b.ravel(), rtol=1e-12, atol=1e-12 * np.abs(got).max())
+
+
+def objective_and_grad(p, m0, zee, dt, nst, w, ckpt_every):
+    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=ckpt_every)
+    J = float(np.sum(w * mT))
+    _, _, u0 = adjoint.backward_rk4(p, mT, w, dt, nst, zee, checkpoints=ck if ckpt_every else None)
+    return J, u0, mT
+
+
+def test_adjoint_state_gradient_against_finite_differences():
+    """C8 on an 8x3x1 film, 300 RK4 steps: dJ/dMs from Eq. (29)-(30) vs central differences."""
+    rng = np.random.default_rng(7)
+    n, dx = (8, 3, 1), (4e-9, 4e-9, 5e-9)
+    p = Problem(n, dx, rng.uniform(1e5, 1.5e5, n), np.full(n, 3.65e-12), np.zeros(n), alpha=1e-2,
+                terms=TERM_EXCHANGE | TERM_DEMAG | TERM_ZEEMAN)
+    p.Nt
+    zee = lambda t: np.array([0.0, 2e3, 0.0])
+    m0 = 0.1 * rng.standard_normal((3,) + p.node_shape)
+    m0[0] += 1
+    m0 /= np.sqrt(np.sum(m0 * m0, axis=0))
+    w = np.zeros_like(m0)
+    w[1, -3:] = 1.0 / w[1, -3:].size
+    dt, nst = 5e-14, 300
+    J, u0, _ = objective_and_grad(p, m0, zee, dt, nst, w, 50)
+    _, u0_nock, _ = objective_and_grad(p, m0, zee, dt, nst, w, 0)
+    cells = [(0, 0, 0), (3, 1, 0), (7, 2, 0), (5, 0, 0)]
+    for c in cells:
+        h = 1e-4 * p.Ms[c]
+        Mp, Mm = p.Ms.copy(), p.Ms.copy()
+        Mp[c] += h
+        Mm[c] -= h
+        Jp = float(np.sum(w * adjoint.forward_rk4(with_Ms(p, Mp), m0, dt, nst, zee)[0]))
+        Jm = float(np.sum(w * adjoint.forward_rk4(with_Ms(p, Mm), m0, dt, nst, zee)[0]))
+        fd = (Jp - Jm) / (2 * h)
+        assert abs(u0[c] - fd) < 1e-3 * abs(fd), (c, u0[c], fd)
+        assert abs(u0_nock[c] - fd) < 1e-3 * abs(fd)
+    # invariance under the checkpoint interval (same tolerance)
+    _, u0_b, _ = objective_and_grad(p, m0, zee, dt, nst, w, 100)
+    assert np.abs(u0_b - u0).max() < 1e-3 * np.abs(u0).max()
+
+
+def test_adjoint_driver_zero_and_linearity():
+    rng = np.random.default_rng(8)
+    n, dx = (4, 2, 1), (4e-9, 4e-9, 5e-9)
+    p = Problem(n, dx, rng.uniform(1e5, 1.5e5, n), np.full(n, 3.65e-12), np.zeros(n), alpha=1e-2,
+                terms=TERM_EXCHANGE | TERM_DEMAG)
+    m0 = rand_unit(p.node_shape, 9)
+    mT, ck = adjoint.forward_rk4(p, m0, 5e-14, 20, checkpoint_every=10)
+    a1 = rng.standard_normal(m0.shape)
+    a2 = rng.standard_normal(m0.shape)
+    run = lambda a: adjoint.backward_rk4(p, mT, a, 5e-14, 20, checkpoints=ck)[2]
+    assert np.all(run(np.zeros_like(a1)) == 0.0)
+    u1, u2, u12 = run(a1), run(a2), run(2.0 * a1 - 0.5 * a2)
+    assert np.allclose(u12, 2.0 * u1 - 0.5 * u2, rtol=1e-10, atol=1e-12 * np.abs(u1).max())
+    # checkpoints put m back exactly on the forward trajectory
+    mb = adjoint.backward_rk4(p, mT, a1, 5e-14, 20, checkpoints=ck)[0]
+    assert np.array_equal(mb, m0)

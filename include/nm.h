@@ -1,0 +1,170 @@
+/* nm.h — C-ABI of the B200-native nodal finite-difference LLG right-hand side.
+ *
+ * The method is the hot path of NeuralMag (arxiv 2411.11725; citations are lines of
+ * /root/reference/PAPER.md): the Landau-Lifshitz-Gilbert right-hand side, Eq. (1),
+ * on a nodal finite-difference mesh (magnetisation m on the (N1+1)(N2+1)(N3+1) vertices, material
+ * parameters on the N1 N2 N3 cells; Eqs. 8-16) with
+ *   - exchange, uniaxial-anisotropy and Zeeman fields from the mass-lumped weak form
+ *     (Eqs. 17-22),
+ *   - the demagnetisation field as a zero-padded FFT convolution over cells with node<->cell
+ *     averaging before and after (Sec. III B),
+ *   - explicit Runge-Kutta steps (RK4, Dormand-Prince),
+ *   - the adjoint (vector-Jacobian) right-hand side of the adjoint-state system, Eq. (29)
+ *     (PAPER.md:219-228).
+ * Where the paper is silent the readings C1..C8 of DESIGN.md apply.
+ *
+ * Conventions
+ *   Precision    every array of one mesh has the mesh's dtype (NM_F32: float, NM_F64: double).
+ *   Memory       every `const void*` / `void*` array argument is DEVICE memory on `desc.device`
+ *                unless the name ends in `_host`.  The caller owns all of it, including the
+ *                workspace block handed to nm_mesh_create; the library allocates no device
+ *                memory after nm_mesh_create returns and frees none that it did not allocate.
+ *   Layout       nodal vector fields are structure-of-arrays [3][N3+1][N2+1][N1+1], x (index 1 of
+ *                the paper's multi-index) fastest, contiguous.  Nodal scalars [N3+1][N2+1][N1+1].
+ *                Cell scalars [N3][N2][N1], cell vectors [3][N3][N2][N1].
+ *   Units        SI: H and Ms in A/m, A in J/m, Ku in J/m^3, gamma in m/(A s), t in s
+ *                (PAPER.md:37).  mu0 = 4 pi 1e-7 exactly.
+ *   Streams      `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All
+ *                work is enqueued on it and the call returns without synchronising, except where
+ *                stated.  Calls on one mesh must not overlap (they share the workspace).
+ *   Errors       every entry point returns nm_status; nothing throws across the ABI;
+ *                nm_last_error() returns a thread-local message for the last failure.
+ *                NaN/Inf in inputs are not checked.  Nodes all of whose adjacent cells have
+ *                Ms = 0 get H = 0 (reading C3(iii)).
+ */
+#ifndef NM_H
+#define NM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nm_mesh nm_mesh; /* opaque, library-owned host object */
+
+typedef enum { NM_F32 = 0, NM_F64 = 1 } nm_dtype;
+
+typedef enum {
+    NM_OK = 0,
+    NM_EINVAL = -1,       /* bad argument (null pointer, non-positive size, ...) */
+    NM_EUNSUPPORTED = -2, /* valid request this build cannot serve (see nm_mesh_create) */
+    NM_ECUDA = -3,        /* a CUDA runtime call or kernel launch failed */
+    NM_ENOMEM = -4        /* workspace too small / host allocation failed */
+} nm_status;
+
+/* field terms, OR-ed into nm_mesh_desc.terms */
+enum { NM_TERM_EXCHANGE = 1, NM_TERM_DEMAG = 2, NM_TERM_ANISO = 4, NM_TERM_ZEEMAN = 8 };
+
+typedef enum { NM_RK4 = 0, NM_DOPRI5 = 1 } nm_scheme;
+
+/* Statement of the problem: regular grid, nodal m, cell-wise materials. */
+typedef struct {
+    int n_cells[3];       /* N1, N2, N3 >= 1.  With NM_TERM_DEMAG every N_d > 1 must be
+                             2^a 3^b (FFT radices 2,3,4,8), else NM_EUNSUPPORTED. */
+    double cell_size[3];  /* metres, > 0 */
+    nm_dtype dtype;
+    int device;           /* CUDA device ordinal */
+    unsigned terms;       /* OR of NM_TERM_* */
+    double gamma;         /* reduced gyromagnetic ratio, m/(A s) */
+    double alpha;         /* Gilbert damping, scalar */
+    double ku_axis[3];    /* anisotropy axis k, unit vector, global (reading C3(i)) */
+    const void *Ms, *A, *Ku; /* device, cell-wise [N3][N2][N1], copied at create; NULL => scalar below */
+    double Ms_scalar, A_scalar, Ku_scalar;
+    long long node_pitch[3]; /* reserved for padded layouts; must be all 0 (contiguous) */
+} nm_mesh_desc;
+
+/* Bytes of device workspace nm_mesh_create needs for this description (spectrum buffers, demag
+ * tensor, lumped mass, Runge-Kutta and adjoint scratch).  Host-only call. */
+nm_status nm_mesh_query_workspace(const nm_mesh_desc *desc, size_t *bytes_out);
+
+/* Build a mesh object inside the caller's workspace (256-byte aligned device block of at least the
+ * queried size).  Computes the demag tensor of uniformly magnetised cuboids (reading C4: Newell
+ * closed form in __float128 near the origin, 6-D Gauss quadrature of the dipole kernel beyond
+ * 8 cell sizes; both agree with the closed form to < 1e-15), its real, symmetric spectrum with
+ * 1/(P1 P2 P3) folded in, S Ms and the FFT tables.  Synchronous; not part of the hot path. */
+nm_status nm_mesh_create(nm_mesh **out, const nm_mesh_desc *desc, void *workspace, size_t bytes);
+
+/* Replace the cell-wise saturation magnetisation (device array) and recompute S Ms. */
+nm_status nm_mesh_set_Ms(nm_mesh *mesh, const void *Ms, void *stream);
+
+/* Frees the host object only (the workspace stays the caller's). */
+nm_status nm_mesh_destroy(nm_mesh *mesh);
+
+/* Thread-local message describing the last non-NM_OK status returned on this thread. */
+const char *nm_last_error(void);
+
+/* External (Zeeman) field  H_ext(t, n) = h_uniform + h_static[n] + amp(t) * h_pulse[n]
+ * (nodal field through the weak form, Eq. 21; reading C3(ii)). */
+typedef struct {
+    const void *h_static, *h_pulse; /* device nodal 3-vector fields or NULL */
+    double h_uniform[3];            /* A/m, added at every node */
+    double (*amp)(double t, void *user); /* host callback, called once per field evaluation
+                                            (per RK stage) on the calling thread; NULL => 1 */
+    void *user;
+} nm_zeeman;
+
+/* a1-a8: H_out = H_ex + H_an + H_zeeman + H_demag at the nodes (terms selected at create).
+ * `zeeman` may be NULL (no external field). */
+nm_status nm_heff(nm_mesh *mesh, double t, const void *m, const nm_zeeman *zeeman, void *H_out,
+                  void *stream);
+
+/* a1-a9: dmdt_out = -g' m x H - alpha g' m x (m x H), g' = gamma/(1+alpha^2)  (Eq. 1). */
+nm_status nm_llg_rhs(nm_mesh *mesh, double t, const void *m, const nm_zeeman *zeeman,
+                     void *dmdt_out, void *stream);
+
+/* a10: one explicit Runge-Kutta step of size dt on m_inout (in place).
+ *   NM_RK4     classical tableau, 4 right-hand sides; err_norm_host must be NULL or is set to 0.
+ *   NM_DOPRI5  Dormand-Prince 5(4), 7 right-hand sides; the scaled RMS error
+ *              err = sqrt(mean(((y5-y4)/(atol + rtol max(|y0|,|y5|)))^2)) over all 3*nodes
+ *              components is computed on the device; the step is committed iff err <= 1,
+ *              otherwise m_inout is left unchanged.  If err_norm_host != NULL the stream is
+ *              synchronised once and *err_norm_host = err (the caller adapts dt).
+ *   renormalise != 0: m_n <- m_n/|m_n| once per committed step (reading C6); stages see the
+ *              un-normalised intermediate states. */
+nm_status nm_rk_step(nm_mesh *mesh, nm_scheme scheme, double t, double dt, void *m_inout,
+                     const nm_zeeman *zeeman, int renormalise, double rtol, double atol,
+                     double *err_norm_host, void *stream);
+
+/* a11: right-hand sides of the adjoint-state system Eq. (29) for theta = Ms (cell-wise):
+ *   dmdt_out    = f(t, m)                         (may be NULL)
+ *   dadt_out    = -(df/dm)^T a                    (nodal 3-vector)
+ *   dudt_Ms_out = -(df/dMs)^T a                   (cell scalar, may be NULL)
+ * with the explicit transposed operators of reading C7 (two demag convolutions). */
+nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, const void *a,
+                             const nm_zeeman *zeeman, void *dmdt_out, void *dadt_out,
+                             void *dudt_Ms_out, void *stream);
+
+/* One RK4 step of size -dt of the augmented system (m, a, u) of Eq. (29), integrating backwards
+ * from t to t - dt (reading C8); m is renormalised after the step if renormalise != 0.
+ * u_inout is the cell-wise accumulator whose value at t = 0 is grad_Ms of the objective (Eq. 30). */
+nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                              void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream);
+
+/* Debug / test getters (not hot path).  Copy the real-space demag tensor N[6][N3][N2][N1]
+ * (components xx,yy,zz,xy,xz,yz; non-negative cell offsets; fp64) to a HOST buffer, and the
+ * cell-wise demag field [3][N3][N2][N1] of the last nm_heff/nm_llg_rhs call (mesh dtype) to a
+ * DEVICE buffer. */
+nm_status nm_debug_get_tensor(nm_mesh *mesh, double *N_host);
+nm_status nm_debug_get_cell_field(nm_mesh *mesh, void *Hc_out, void *stream);
+
+/* Number of kernel launches this library has issued on this mesh since create (for bench). */
+long long nm_launch_count(const nm_mesh *mesh);
+
+/* Per-kernel timing for the roofline line of bench.py.  Between
+ * nm_profile_begin and nm_profile_end every kernel launch on this mesh is bracketed by a pair of
+ * CUDA events on the launching stream (at most 4096 launches are recorded; later ones are only
+ * counted by nm_launch_count).  nm_profile_end synchronises `stream` and writes, for each of the
+ * nm_profile_class_count() kernel classes, the summed device time in milliseconds and the number
+ * of recorded launches to the two HOST arrays (each of nm_profile_class_count() entries).
+ * nm_profile_class_name(i) names class i ("x_fwd", "y_fwd", "mid", "y_inv", "x_inv", "node",
+ * "adj_cell", "lincomb", "other"). */
+int nm_profile_class_count(void);
+const char *nm_profile_class_name(int cls);
+nm_status nm_profile_begin(nm_mesh *mesh);
+nm_status nm_profile_end(nm_mesh *mesh, void *stream, double *ms_host, long long *count_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NM_H */

@@ -1,0 +1,759 @@
+// C-ABI entry points of libnm.so (include/nm.h): mesh setup, field / right-hand-side evaluation,
+// Runge-Kutta steps and the adjoint right-hand side.  Host orchestration only: every step of the
+// path runs in the kernels of nm_local.cu and nm_demag.cu.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "nm_internal.h"
+#include "nm_local.cuh"
+
+// ---- errors ------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+void nm_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+extern "C" const char *nm_last_error(void) { return g_err; }
+
+namespace {
+
+// ---- geometry, FFT plans -----------------------------------------------------------------------
+bool smooth23(int n)
+{
+    while (n % 2 == 0) n /= 2;
+    while (n % 3 == 0) n /= 3;
+    return n == 1;
+}
+
+void make_plan(int L, NmFftPlan *p)
+{
+    p->L = L;
+    p->n_stages = 0;
+    int n = L;
+    // factors of three first (largest blocks), then 8s, then what is left of the power of two
+    while (n % 3 == 0) { p->radix[p->n_stages++] = 3; n /= 3; }
+    while (n % 8 == 0) { p->radix[p->n_stages++] = 8; n /= 8; }
+    if (n % 4 == 0) { p->radix[p->n_stages++] = 4; n /= 4; }
+    if (n % 2 == 0) { p->radix[p->n_stages++] = 2; n /= 2; }
+}
+
+// Position <-> frequency of the decimation-in-frequency stages (nm_fft.cuh): a stage with block
+// length n and radix R leaves the outputs k = t (mod R) in sub-block t.
+void make_maps(const NmFftPlan &p, std::vector<int> &kmap, std::vector<int> &pos)
+{
+    kmap.assign(p.L, 0);
+    pos.assign(p.L, 0);
+    for (int q = 0; q < p.L; ++q) {
+        int rem = q, m = p.L, k = 0, w = 1;
+        for (int s = 0; s < p.n_stages; ++s) {
+            m /= p.radix[s];
+            const int t = rem / m;
+            rem -= t * m;
+            k += t * w;
+            w *= p.radix[s];
+        }
+        kmap[q] = k;
+        pos[k] = q;
+    }
+}
+
+nm_status validate(const nm_mesh_desc *d)
+{
+    if (!d) { nm_set_error("desc is NULL"); return NM_EINVAL; }
+    for (int i = 0; i < 3; ++i) {
+        if (d->n_cells[i] < 1) { nm_set_error("n_cells[%d] = %d < 1", i, d->n_cells[i]); return NM_EINVAL; }
+        if (!(d->cell_size[i] > 0)) { nm_set_error("cell_size[%d] must be > 0", i); return NM_EINVAL; }
+        if (d->node_pitch[i] != 0) { nm_set_error("node_pitch must be 0 (contiguous layout)"); return NM_EINVAL; }
+    }
+    if (d->dtype != NM_F32 && d->dtype != NM_F64) { nm_set_error("bad dtype"); return NM_EINVAL; }
+    if (d->terms == 0 || (d->terms & ~15u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
+    if (!(d->gamma == d->gamma) || !(d->alpha == d->alpha)) { nm_set_error("gamma / alpha is NaN"); return NM_EINVAL; }
+    if (d->terms & NM_TERM_ANISO) {
+        const double *k = d->ku_axis;
+        const double n2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+        if (std::fabs(n2 - 1.0) > 1e-9) { nm_set_error("ku_axis must be a unit vector"); return NM_EINVAL; }
+    }
+    if (d->terms & NM_TERM_DEMAG) {
+        for (int i = 0; i < 3; ++i)
+            if (d->n_cells[i] > 1 && !smooth23(d->n_cells[i])) {
+                nm_set_error("n_cells[%d] = %d is not of the form 2^a 3^b (demag FFT radices)", i, d->n_cells[i]);
+                return NM_EUNSUPPORTED;
+            }
+        const size_t cx = d->dtype == NM_F64 ? 16 : 8;
+        if ((size_t)12 * d->n_cells[0] * cx > 200 * 1024) {
+            nm_set_error("n_cells[0] = %d too long for the x pass", d->n_cells[0]);
+            return NM_EUNSUPPORTED;
+        }
+    }
+    return NM_OK;
+}
+
+void make_geom(const nm_mesh_desc *d, NmGeom *g)
+{
+    g->N1 = d->n_cells[0]; g->N2 = d->n_cells[1]; g->N3 = d->n_cells[2];
+    g->n1 = g->N1 + 1; g->n2 = g->N2 + 1; g->n3 = g->N3 + 1;
+    g->P1 = g->N1 > 1 ? 2 * g->N1 : 1;
+    g->P2 = g->N2 > 1 ? 2 * g->N2 : 1;
+    g->P3 = g->N3 > 1 ? 2 * g->N3 : 1;
+    g->C1 = g->N1 > 1 ? g->N1 + 1 : 1;
+    g->C1p = (g->C1 + 3) & ~3;
+    g->K2 = g->N2 > 1 ? g->N2 + 1 : 1;
+    g->K3 = g->N3 > 1 ? g->N3 + 1 : 1;
+    g->Lx = g->N1;
+    g->cells = (long long)g->N1 * g->N2 * g->N3;
+    g->nodes = (long long)g->n1 * g->n2 * g->n3;
+}
+
+// Bump allocator over the caller's workspace; with base == nullptr it only measures.
+struct Carver {
+    char *base;
+    size_t off;
+    void *take(size_t bytes)
+    {
+        off = (off + 255) & ~(size_t)255;
+        void *p = base ? base + off : nullptr;
+        off += bytes;
+        return p;
+    }
+};
+
+size_t carve(nm_mesh *m, char *base)
+{
+    const NmGeom &g = m->g;
+    const size_t e = m->esz, cx = 2 * m->esz;
+    const bool demag = (m->desc.terms & NM_TERM_DEMAG) != 0;
+    Carver c{base, 0};
+    m->Ms = c.take(g.cells * e);
+    m->A = c.take(g.cells * e);
+    m->Ku = c.take(g.cells * e);
+    m->sMs = c.take(g.nodes * e);
+    m->n_partials = nm_node_blocks(g.nodes);
+    m->partials = (double *)c.take(((size_t)m->n_partials + 1) * sizeof(double));
+    // Runge-Kutta / adjoint scratch; doubles as fp64 scratch of the tensor setup
+    const size_t vec = (size_t)3 * g.nodes * e;
+    size_t rk = 9 * vec;
+    if (demag) {
+        const size_t need = (size_t)2 * 6 * g.C1 * g.K2 * g.K3 * sizeof(double);
+        if (need > rk) rk = need;
+    }
+    char *r = (char *)c.take(rk);
+    for (int i = 0; i < 7; ++i) m->K[i] = r ? r + i * vec : nullptr;
+    for (int i = 0; i < 2; ++i) m->Y[i] = r ? r + (7 + i) * vec : nullptr;
+    m->Q = c.take(vec);
+    m->W = c.take(g.nodes * e);
+    m->Uc[0] = c.take(g.cells * e);
+    m->Uc[1] = c.take(g.cells * e);
+    m->Hc1 = m->Hc2 = nullptr;
+    m->Nreal = nullptr;
+    m->Nhat = m->tw_x = m->tw_x2 = m->tw_y = m->tw_z = m->bufA = m->bufB = nullptr;
+    m->kmap_x = m->pos_x = m->kmap_y = m->pos_y = m->kmap_z = m->pos_z = nullptr;
+    if (demag) {
+        m->Hc1 = c.take(3 * g.cells * e);
+        m->Hc2 = c.take(3 * g.cells * e);
+        m->Nreal = (double *)c.take(6 * g.cells * sizeof(double));
+        m->Nhat = c.take((size_t)6 * g.K3 * g.K2 * g.C1p * e);
+        m->tw_x = c.take((size_t)g.Lx * cx);
+        m->tw_x2 = c.take((size_t)g.C1 * cx);
+        m->tw_y = c.take((size_t)g.P2 * cx);
+        m->tw_z = c.take((size_t)g.P3 * cx);
+        m->kmap_x = (int *)c.take(g.Lx * sizeof(int));
+        m->pos_x = (int *)c.take(g.Lx * sizeof(int));
+        m->kmap_y = (int *)c.take(g.P2 * sizeof(int));
+        m->pos_y = (int *)c.take(g.P2 * sizeof(int));
+        m->kmap_z = (int *)c.take(g.P3 * sizeof(int));
+        m->pos_z = (int *)c.take(g.P3 * sizeof(int));
+        m->bufA = c.take((size_t)3 * g.N3 * g.N2 * g.C1p * cx);
+        if (g.N3 > 1) m->bufB = c.take((size_t)3 * g.N3 * g.P2 * g.C1p * cx);
+    }
+    return (c.off + 255) & ~(size_t)255;
+}
+
+void init_host(nm_mesh *m, const nm_mesh_desc *d)
+{
+    m->desc = *d;
+    make_geom(d, &m->g);
+    m->f64 = d->dtype == NM_F64;
+    m->esz = m->f64 ? 8 : 4;
+    m->launches = 0;
+    m->hc1_valid = false;
+    m->prof_on = false;
+    m->prof_n = 0;
+    m->prof_ev_made = 0;
+    make_plan(m->g.Lx, &m->plan_x);
+    make_plan(m->g.P2, &m->plan_y);
+    make_plan(m->g.P3, &m->plan_z);
+}
+
+template <typename T> __global__ void k_fill(T *p, long long n, T v)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = v;
+}
+
+template <typename T>
+nm_status set_material(nm_mesh *m, void *dst, const void *src, double scalar, cudaStream_t st)
+{
+    const long long n = m->g.cells;
+    if (src) {
+        NM_CUDA_TRY(cudaMemcpyAsync(dst, src, n * sizeof(T), cudaMemcpyDeviceToDevice, st));
+    } else {
+        {
+            NmLaunchScope sc(m, NM_K_OTHER, st);
+            k_fill<T><<<(unsigned)((n + 255) / 256), 256, 0, st>>>((T *)dst, n, (T)scalar);
+        }
+        NM_CUDA_TRY(cudaGetLastError());
+    }
+    return NM_OK;
+}
+
+// exp(-2 pi i q / L), q = 0..count-1, evaluated in fp64 and rounded to the mesh dtype
+template <typename T>
+nm_status upload_twiddles(void *dst, int L, int count, cudaStream_t st)
+{
+    typedef typename NmVec2<T>::type V;
+    std::vector<V> h(count);
+    for (int q = 0; q < count; ++q) {
+        // exact octant reduction keeps cos/sin at multiples of pi/2 exact
+        const double x = 2.0 * (double)q / (double)L;   // angle / pi
+        double c, s;
+        const long long q8 = (long long)q * 8;
+        if (q8 % L == 0 && (q8 / L) % 2 == 0) {
+            const int oct = (int)((q8 / L) / 2) & 3;     // multiples of pi/2
+            const double cc[4] = {1, 0, -1, 0}, ss[4] = {0, 1, 0, -1};
+            c = cc[oct]; s = ss[oct];
+        } else {
+            c = std::cos(M_PI * x);
+            s = std::sin(M_PI * x);
+        }
+        h[q].x = (T)c;
+        h[q].y = (T)(-s);
+    }
+    NM_CUDA_TRY(cudaMemcpyAsync(dst, h.data(), count * sizeof(V), cudaMemcpyHostToDevice, st));
+    NM_CUDA_TRY(cudaStreamSynchronize(st));
+    return NM_OK;
+}
+
+nm_status upload_ints(int *dst, const std::vector<int> &v, cudaStream_t st)
+{
+    NM_CUDA_TRY(cudaMemcpyAsync(dst, v.data(), v.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+    NM_CUDA_TRY(cudaStreamSynchronize(st));
+    return NM_OK;
+}
+
+template <typename T> nm_status setup_tables(nm_mesh *m, cudaStream_t st)
+{
+    const NmGeom &g = m->g;
+    NM_TRY(upload_twiddles<T>(m->tw_x, g.Lx, g.Lx, st));
+    NM_TRY(upload_twiddles<T>(m->tw_x2, g.P1, g.C1, st));
+    NM_TRY(upload_twiddles<T>(m->tw_y, g.P2, g.P2, st));
+    NM_TRY(upload_twiddles<T>(m->tw_z, g.P3, g.P3, st));
+    std::vector<int> km, ps;
+    make_maps(m->plan_x, km, ps);
+    NM_TRY(upload_ints(m->kmap_x, km, st));
+    NM_TRY(upload_ints(m->pos_x, ps, st));
+    make_maps(m->plan_y, km, ps);
+    NM_TRY(upload_ints(m->kmap_y, km, st));
+    NM_TRY(upload_ints(m->pos_y, ps, st));
+    make_maps(m->plan_z, km, ps);
+    NM_TRY(upload_ints(m->kmap_z, km, st));
+    NM_TRY(upload_ints(m->pos_z, ps, st));
+    return NM_OK;
+}
+
+} // namespace
+
+// ---- mesh life cycle ---------------------------------------------------------------------------
+extern "C" nm_status nm_mesh_query_workspace(const nm_mesh_desc *desc, size_t *bytes_out)
+{
+    NM_TRY(validate(desc));
+    if (!bytes_out) { nm_set_error("bytes_out is NULL"); return NM_EINVAL; }
+    nm_mesh tmp;
+    init_host(&tmp, desc);
+    *bytes_out = carve(&tmp, nullptr);
+    return NM_OK;
+}
+
+extern "C" nm_status nm_mesh_set_Ms(nm_mesh *mesh, const void *Ms, void *stream)
+{
+    if (!mesh || !Ms) { nm_set_error("NULL argument"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    NM_CUDA_TRY(cudaSetDevice(mesh->desc.device));
+    NM_CUDA_TRY(cudaMemcpyAsync(mesh->Ms, Ms, mesh->g.cells * mesh->esz, cudaMemcpyDeviceToDevice, st));
+    mesh->hc1_valid = false;
+    return nm_compute_sMs(mesh, st);
+}
+
+extern "C" nm_status nm_mesh_create(nm_mesh **out, const nm_mesh_desc *desc, void *workspace, size_t bytes)
+{
+    if (!out) { nm_set_error("out is NULL"); return NM_EINVAL; }
+    *out = nullptr;
+    NM_TRY(validate(desc));
+    if (!workspace || ((uintptr_t)workspace & 255)) {
+        nm_set_error("workspace must be a 256-byte aligned device pointer");
+        return NM_EINVAL;
+    }
+    nm_mesh *m = new (std::nothrow) nm_mesh;
+    if (!m) { nm_set_error("host allocation failed"); return NM_ENOMEM; }
+    init_host(m, desc);
+    const size_t need = carve(m, (char *)workspace);
+    if (bytes < need) {
+        nm_set_error("workspace of %zu bytes is smaller than the %zu required", bytes, need);
+        delete m;
+        return NM_ENOMEM;
+    }
+    m->ws = (char *)workspace;
+    m->ws_bytes = bytes;
+    nm_status s = NM_OK;
+    cudaStream_t st = 0;
+    do {
+        cudaError_t e = cudaSetDevice(desc->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, desc->device);
+        if (e == cudaSuccess) e = cudaMemsetAsync(workspace, 0, need, st);
+        if (e != cudaSuccess) {
+            nm_set_error("device setup failed: %s", cudaGetErrorString(e));
+            s = NM_ECUDA;
+            break;
+        }
+        if (m->f64) {
+            if ((s = set_material<double>(m, m->Ms, desc->Ms, desc->Ms_scalar, st)) != NM_OK) break;
+            if ((s = set_material<double>(m, m->A, desc->A, desc->A_scalar, st)) != NM_OK) break;
+            if ((s = set_material<double>(m, m->Ku, desc->Ku, desc->Ku_scalar, st)) != NM_OK) break;
+        } else {
+            if ((s = set_material<float>(m, m->Ms, desc->Ms, desc->Ms_scalar, st)) != NM_OK) break;
+            if ((s = set_material<float>(m, m->A, desc->A, desc->A_scalar, st)) != NM_OK) break;
+            if ((s = set_material<float>(m, m->Ku, desc->Ku, desc->Ku_scalar, st)) != NM_OK) break;
+        }
+        if ((s = nm_compute_sMs(m, st)) != NM_OK) break;
+        if (desc->terms & NM_TERM_DEMAG) {
+            s = m->f64 ? setup_tables<double>(m, st) : setup_tables<float>(m, st);
+            if (s != NM_OK) break;
+            if ((s = nm_build_tensor(m, st)) != NM_OK) break;
+            // the tensor setup used the Runge-Kutta region as scratch
+            if (cudaMemsetAsync(m->K[0], 0, (char *)m->Q - (char *)m->K[0], st) != cudaSuccess) {
+                nm_set_error("cudaMemsetAsync failed");
+                s = NM_ECUDA;
+                break;
+            }
+        }
+        if (cudaStreamSynchronize(st) != cudaSuccess) {
+            nm_set_error("nm_mesh_create: %s", cudaGetErrorString(cudaGetLastError()));
+            s = NM_ECUDA;
+        }
+    } while (0);
+    if (s != NM_OK) {
+        delete m;
+        return s;
+    }
+    // the pointers in desc are not kept
+    m->desc.Ms = m->desc.A = m->desc.Ku = nullptr;
+    *out = m;
+    return NM_OK;
+}
+
+extern "C" nm_status nm_mesh_destroy(nm_mesh *mesh)
+{
+    if (mesh) {
+        for (int i = 0; i < mesh->prof_ev_made; ++i) {
+            cudaEventDestroy(mesh->prof_ev[i][0]);
+            cudaEventDestroy(mesh->prof_ev[i][1]);
+        }
+    }
+    delete mesh;
+    return NM_OK;
+}
+
+static const char *const kClassNames[NM_K_COUNT] = {"x_fwd", "y_fwd", "mid", "y_inv", "x_inv",
+                                                    "node", "adj_cell", "lincomb", "other"};
+
+extern "C" int nm_profile_class_count(void) { return NM_K_COUNT; }
+
+extern "C" const char *nm_profile_class_name(int cls)
+{
+    return cls >= 0 && cls < NM_K_COUNT ? kClassNames[cls] : "";
+}
+
+extern "C" nm_status nm_profile_begin(nm_mesh *mesh)
+{
+    if (!mesh) { nm_set_error("NULL argument"); return NM_EINVAL; }
+    mesh->prof_on = true;
+    mesh->prof_n = 0;
+    return NM_OK;
+}
+
+extern "C" nm_status nm_profile_end(nm_mesh *mesh, void *stream, double *ms_host, long long *count_host)
+{
+    if (!mesh || !ms_host || !count_host) { nm_set_error("NULL argument"); return NM_EINVAL; }
+    mesh->prof_on = false;
+    NM_CUDA_TRY(cudaSetDevice(mesh->desc.device));
+    NM_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    for (int c = 0; c < NM_K_COUNT; ++c) { ms_host[c] = 0.0; count_host[c] = 0; }
+    for (int i = 0; i < mesh->prof_n; ++i) {
+        float ms = 0.f;
+        NM_CUDA_TRY(cudaEventElapsedTime(&ms, mesh->prof_ev[i][0], mesh->prof_ev[i][1]));
+        ms_host[mesh->prof_cls[i]] += ms;
+        count_host[mesh->prof_cls[i]]++;
+    }
+    mesh->prof_n = 0;
+    return NM_OK;
+}
+
+extern "C" long long nm_launch_count(const nm_mesh *mesh) { return mesh ? mesh->launches : 0; }
+
+extern "C" nm_status nm_debug_get_tensor(nm_mesh *mesh, double *N_host)
+{
+    if (!mesh || !N_host) { nm_set_error("NULL argument"); return NM_EINVAL; }
+    if (!mesh->Nreal) { nm_set_error("mesh has no demag term"); return NM_EINVAL; }
+    NM_CUDA_TRY(cudaSetDevice(mesh->desc.device));
+    NM_CUDA_TRY(cudaMemcpy(N_host, mesh->Nreal, 6 * mesh->g.cells * sizeof(double), cudaMemcpyDeviceToHost));
+    return NM_OK;
+}
+
+extern "C" nm_status nm_debug_get_cell_field(nm_mesh *mesh, void *Hc_out, void *stream)
+{
+    if (!mesh || !Hc_out) { nm_set_error("NULL argument"); return NM_EINVAL; }
+    if (!mesh->Hc1 || !mesh->hc1_valid) { nm_set_error("no cell demag field has been computed"); return NM_EINVAL; }
+    NM_CUDA_TRY(cudaSetDevice(mesh->desc.device));
+    NM_CUDA_TRY(cudaMemcpyAsync(Hc_out, mesh->Hc1, 3 * mesh->g.cells * mesh->esz, cudaMemcpyDeviceToDevice,
+                                (cudaStream_t)stream));
+    return NM_OK;
+}
+
+// ---- field evaluation --------------------------------------------------------------------------
+namespace {
+
+// Constant part of the node-kernel arguments for this mesh at time t.
+template <typename T>
+void base_args(const nm_mesh *m, double t, const nm_zeeman *z, unsigned terms, NmLocalArgs<T> *a)
+{
+    memset(a, 0, sizeof(*a));
+    a->g = m->g;
+    a->Ms = (const T *)m->Ms;
+    a->A = (const T *)m->A;
+    a->Ku = (const T *)m->Ku;
+    a->sMs = (const T *)m->sMs;
+    a->terms = terms;
+    const double *dx = m->desc.cell_size;
+    const double V = dx[0] * dx[1] * dx[2];
+    for (int e = 0; e < 8; ++e) {
+        // vertices differ along axis d iff bit d of e is set: 1-D entries K1 = +-1, M1 = 1/3 or 1/6
+        double wm = V, wk = 0.0;
+        for (int d = 0; d < 3; ++d) wm *= ((e >> d) & 1) ? 1.0 / 6.0 : 1.0 / 3.0;
+        for (int d = 0; d < 3; ++d) {
+            double term = (((e >> d) & 1) ? -1.0 : 1.0) / (dx[d] * dx[d]);
+            for (int f = 0; f < 3; ++f)
+                if (f != d) term *= ((e >> f) & 1) ? 1.0 / 6.0 : 1.0 / 3.0;
+            wk += term;
+        }
+        a->wK[e] = (T)(V * wk);
+        a->wM[e] = (T)wm;
+    }
+    for (int j = 0; j < 3; ++j) a->kax[j] = (T)m->desc.ku_axis[j];
+    a->mu0 = (T)NM_MU0;
+    a->mu0V8 = (T)(NM_MU0 * V / 8.0);
+    if ((terms & NM_TERM_ZEEMAN) && z) {
+        a->h_static = (const T *)z->h_static;
+        a->h_pulse = (const T *)z->h_pulse;
+        a->amp = (T)(z->amp ? z->amp(t, z->user) : 1.0);
+        for (int j = 0; j < 3; ++j) a->hu[j] = (T)z->h_uniform[j];
+    }
+    const double gp = m->desc.gamma / (1.0 + m->desc.alpha * m->desc.alpha);
+    a->gp = (T)gp;
+    a->agp = (T)(m->desc.alpha * gp);
+}
+
+// Demag convolution of `fld` into Hc (if the term is on) and the matching pointer for the node kernel.
+template <typename T>
+nm_status demag_part(nm_mesh *m, const T *fld, T *Hc, const T **Hc_arg, cudaStream_t st)
+{
+    *Hc_arg = nullptr;
+    if (m->desc.terms & NM_TERM_DEMAG) {
+        NM_TRY(nm_demag_conv<T>(m, fld, Hc, st));
+        *Hc_arg = Hc;
+    }
+    return NM_OK;
+}
+
+template <typename T>
+nm_status eval_simple(nm_mesh *m, double t, const T *fld, const nm_zeeman *z, T *out, int mode,
+                      cudaStream_t st)
+{
+    NmLocalArgs<T> a;
+    base_args<T>(m, t, z, m->desc.terms, &a);
+    a.fld = fld;
+    NM_TRY(demag_part<T>(m, fld, (T *)m->Hc1, &a.Hc, st));
+    m->hc1_valid = a.Hc != nullptr;
+    a.mode = mode;
+    a.out = out;
+    return nm_launch_node<T>(m, a, st);
+}
+
+// One Runge-Kutta stage: k = f(t, fld) with the stage combination fused into the node kernel.
+template <typename T>
+nm_status eval_stage(nm_mesh *m, double t, const T *fld, const nm_zeeman *z, const NmRkArgs<T> &rk,
+                     cudaStream_t st)
+{
+    NmLocalArgs<T> a;
+    base_args<T>(m, t, z, m->desc.terms, &a);
+    a.fld = fld;
+    NM_TRY(demag_part<T>(m, fld, (T *)m->Hc1, &a.Hc, st));
+    m->hc1_valid = a.Hc != nullptr;
+    a.mode = NM_MODE_RK;
+    a.rk = rk;
+    return nm_launch_node<T>(m, a, st);
+}
+
+template <typename T>
+nm_status rk4_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z, int renorm, cudaStream_t st)
+{
+    T *K0 = (T *)m->K[0], *K1 = (T *)m->K[1], *K2 = (T *)m->K[2];
+    T *Y0 = (T *)m->Y[0], *Y1 = (T *)m->Y[1];
+    NmRkArgs<T> r;
+    memset(&r, 0, sizeof(r));
+    r.y0 = y;
+    r.dt = (T)dt;
+    // k1 = f(t, y);  Y0 = y + dt/2 k1
+    r.kstore = K0; r.nprev = 0; r.cself = (T)0.5; r.ynext = Y0;
+    NM_TRY(eval_stage<T>(m, t, y, z, r, st));
+    // k2 = f(t + dt/2, Y0);  Y1 = y + dt/2 k2
+    r.kstore = K1; r.ynext = Y1;
+    NM_TRY(eval_stage<T>(m, t + 0.5 * dt, Y0, z, r, st));
+    // k3 = f(t + dt/2, Y1);  Y0 = y + dt k3
+    r.kstore = K2; r.cself = (T)1; r.ynext = Y0;
+    NM_TRY(eval_stage<T>(m, t + 0.5 * dt, Y1, z, r, st));
+    // k4 = f(t + dt, Y0);  y <- y + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised
+    r.kstore = nullptr;
+    r.nprev = 3;
+    r.kprev[0] = K0; r.kprev[1] = K1; r.kprev[2] = K2;
+    r.cprev[0] = (T)(1.0 / 6.0); r.cprev[1] = (T)(2.0 / 6.0); r.cprev[2] = (T)(2.0 / 6.0);
+    r.cself = (T)(1.0 / 6.0);
+    r.ynext = y;
+    r.renorm = renorm;
+    return eval_stage<T>(m, t + dt, Y0, z, r, st);
+}
+
+// Dormand-Prince 5(4) (Dormand & Prince 1980; "Dormand-Prince method")
+const double DP_C[7] = {0.0, 1.0 / 5, 3.0 / 10, 4.0 / 5, 8.0 / 9, 1.0, 1.0};
+const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5, 0, 0, 0, 0, 0},
+    {3.0 / 40, 9.0 / 40, 0, 0, 0, 0},
+    {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0},
+    {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0},
+    {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0},
+    {35.0 / 384, 0.0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}};
+const double DP_B5[7] = {35.0 / 384, 0.0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84, 0.0};
+const double DP_B4[7] = {5179.0 / 57600, 0.0, 7571.0 / 16695, 393.0 / 640, -92097.0 / 339200,
+                         187.0 / 2100, 1.0 / 40};
+
+template <typename T>
+nm_status dopri5_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z, int renorm,
+                      double rtol, double atol, double *err_host, cudaStream_t st)
+{
+    T *Yb[2] = {(T *)m->Y[0], (T *)m->Y[1]};
+    const T *fld = y;
+    for (int s = 0; s < 7; ++s) {
+        NmRkArgs<T> r;
+        memset(&r, 0, sizeof(r));
+        r.y0 = y;
+        r.dt = (T)dt;
+        r.kstore = s < 6 ? (T *)m->K[s] : nullptr;
+        r.nprev = s;
+        for (int j = 0; j < s; ++j) r.kprev[j] = (const T *)m->K[j];
+        if (s < 6) {
+            // next stage state (s < 5) or the fifth-order solution y5 (s = 5: row 6 of A equals b5)
+            for (int j = 0; j < s; ++j) r.cprev[j] = (T)DP_A[s + 1][j];
+            r.cself = (T)DP_A[s + 1][s];
+            r.ynext = Yb[s & 1];
+        } else {
+            for (int j = 0; j < 6; ++j) r.eprev[j] = (T)(DP_B5[j] - DP_B4[j]);
+            r.eself = (T)(DP_B5[6] - DP_B4[6]);
+            r.want_err = 1;
+            r.rtol = (T)rtol;
+            r.atol = (T)atol;
+            r.partials = m->partials;
+        }
+        NM_TRY(eval_stage<T>(m, t + DP_C[s] * dt, fld, z, r, st));
+        if (s < 6) fld = Yb[s & 1];
+    }
+    NM_TRY(nm_launch_err_final(m, m->n_partials, 3.0 * (double)m->g.nodes, st));
+    // y5 lives in Yb[5 & 1]
+    NM_TRY(nm_launch_commit<T>(m, y, Yb[1], m->partials + m->n_partials, renorm, st));
+    if (err_host) {
+        NM_CUDA_TRY(cudaMemcpyAsync(err_host, m->partials + m->n_partials, sizeof(double),
+                                    cudaMemcpyDeviceToHost, st));
+        NM_CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    return NM_OK;
+}
+
+// (f, -(df/dm)^T a, -(df/dMs)^T a): reading C7, two demag convolutions and two node passes.
+template <typename T>
+nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_zeeman *z, T *f_out,
+                       T *dadt, T *dudt, cudaStream_t st)
+{
+    NmLocalArgs<T> a;
+    base_args<T>(m, t, z, m->desc.terms, &a);
+    a.fld = mm;
+    NM_TRY(demag_part<T>(m, mm, (T *)m->Hc1, &a.Hc, st));
+    m->hc1_valid = a.Hc != nullptr;
+    a.mode = NM_MODE_ADJ1;
+    a.out = f_out;
+    a.adj = av;
+    a.Q = (T *)m->Q;
+    a.W = (T *)m->W;
+    a.dadt = dadt;
+    NM_TRY(nm_launch_node<T>(m, a, st));
+    // Hlin^T b = (S Ms) o Hlin(q): same operators on q = b / (S Ms), no Zeeman term
+    NmLocalArgs<T> b;
+    base_args<T>(m, t, nullptr, m->desc.terms & ~(unsigned)NM_TERM_ZEEMAN, &b);
+    b.fld = (const T *)m->Q;
+    NM_TRY(demag_part<T>(m, (const T *)m->Q, (T *)m->Hc2, &b.Hc, st));
+    b.mode = NM_MODE_ADJ2;
+    b.dadt = dadt;
+    NM_TRY(nm_launch_node<T>(m, b, st));
+    if (dudt) {
+        NmAdjCellArgs<T> c;
+        memset(&c, 0, sizeof(c));
+        c.g = m->g;
+        c.m = mm;
+        c.Q = (const T *)m->Q;
+        c.W = (const T *)m->W;
+        c.Hc1 = a.Hc;
+        c.Hc2 = b.Hc;
+        c.h_static = a.h_static;
+        c.h_pulse = a.h_pulse;
+        c.amp = a.amp;
+        for (int j = 0; j < 3; ++j) c.hu[j] = a.hu[j];
+        for (int e = 0; e < 8; ++e) {
+            double wm = 8.0;   // (8/V) * V prod_d M1
+            for (int d = 0; d < 3; ++d) wm *= ((e >> d) & 1) ? 1.0 / 6.0 : 1.0 / 3.0;
+            c.wM8V[e] = (T)wm;
+        }
+        c.terms = (m->desc.terms & NM_TERM_ZEEMAN) && z ? m->desc.terms : (m->desc.terms & ~(unsigned)NM_TERM_ZEEMAN);
+        c.dudt = dudt;
+        NM_TRY(nm_launch_adj_cell<T>(m, c, st));
+    }
+    return NM_OK;
+}
+
+template <typename T>
+nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, const nm_zeeman *z,
+                      int renorm, cudaStream_t st)
+{
+    const long long nv = 3 * m->g.nodes, nc = m->g.cells, nn = m->g.nodes;
+    T *F = (T *)m->K[0], *DA = (T *)m->K[1], *AM = (T *)m->K[2], *AA = (T *)m->K[3];
+    T *Ym = (T *)m->Y[0], *Ya = (T *)m->Y[1];
+    T *DU = (T *)m->Uc[0], *AU = (T *)m->Uc[1];
+    const double h = -dt;
+    const double w[4] = {h / 6, h / 3, h / 3, h / 6};
+    const double cn[3] = {0.5 * h, 0.5 * h, h};     // next stage state = y + cn * k
+    const double ts[4] = {t, t + 0.5 * h, t + 0.5 * h, t + h};
+    const T *sm = mm, *sa = av;
+    for (int s = 0; s < 4; ++s) {
+        NM_TRY(adjoint_eval<T>(m, ts[s], sm, sa, z, F, DA, DU, st));
+        const T ws = (T)w[s];
+        const T *srcF[1] = {F}, *srcA[1] = {DA}, *srcU[1] = {DU};
+        if (s < 3) {
+            // accumulators (first stage starts them from the state)
+            NM_TRY(nm_lincomb<T>(m, AM, s == 0 ? mm : AM, 1, srcF, &ws, nv, 0, st));
+            NM_TRY(nm_lincomb<T>(m, AA, s == 0 ? av : AA, 1, srcA, &ws, nv, 0, st));
+            NM_TRY(nm_lincomb<T>(m, AU, s == 0 ? u : AU, 1, srcU, &ws, nc, 0, st));
+            const T c = (T)cn[s];
+            NM_TRY(nm_lincomb<T>(m, Ym, mm, 1, srcF, &c, nv, 0, st));
+            NM_TRY(nm_lincomb<T>(m, Ya, av, 1, srcA, &c, nv, 0, st));
+            sm = Ym;
+            sa = Ya;
+        } else {
+            NM_TRY(nm_lincomb<T>(m, mm, AM, 1, srcF, &ws, nv, renorm ? nn : 0, st));
+            NM_TRY(nm_lincomb<T>(m, av, AA, 1, srcA, &ws, nv, 0, st));
+            NM_TRY(nm_lincomb<T>(m, u, AU, 1, srcU, &ws, nc, 0, st));
+        }
+    }
+    return NM_OK;
+}
+
+nm_status check_call(nm_mesh *mesh, const void *p0, const void *p1)
+{
+    if (!mesh || !p0 || !p1) { nm_set_error("NULL argument"); return NM_EINVAL; }
+    NM_CUDA_TRY(cudaSetDevice(mesh->desc.device));
+    return NM_OK;
+}
+
+} // namespace
+
+extern "C" nm_status nm_heff(nm_mesh *mesh, double t, const void *m, const nm_zeeman *zeeman, void *H_out,
+                             void *stream)
+{
+    NM_TRY(check_call(mesh, m, H_out));
+    cudaStream_t st = (cudaStream_t)stream;
+    return mesh->f64 ? eval_simple<double>(mesh, t, (const double *)m, zeeman, (double *)H_out, NM_MODE_H, st)
+                     : eval_simple<float>(mesh, t, (const float *)m, zeeman, (float *)H_out, NM_MODE_H, st);
+}
+
+extern "C" nm_status nm_llg_rhs(nm_mesh *mesh, double t, const void *m, const nm_zeeman *zeeman,
+                                void *dmdt_out, void *stream)
+{
+    NM_TRY(check_call(mesh, m, dmdt_out));
+    cudaStream_t st = (cudaStream_t)stream;
+    return mesh->f64 ? eval_simple<double>(mesh, t, (const double *)m, zeeman, (double *)dmdt_out, NM_MODE_RHS, st)
+                     : eval_simple<float>(mesh, t, (const float *)m, zeeman, (float *)dmdt_out, NM_MODE_RHS, st);
+}
+
+extern "C" nm_status nm_rk_step(nm_mesh *mesh, nm_scheme scheme, double t, double dt, void *m_inout,
+                                const nm_zeeman *zeeman, int renormalise, double rtol, double atol,
+                                double *err_norm_host, void *stream)
+{
+    NM_TRY(check_call(mesh, m_inout, m_inout));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (scheme == NM_RK4) {
+        if (err_norm_host) *err_norm_host = 0.0;
+        return mesh->f64 ? rk4_step<double>(mesh, t, dt, (double *)m_inout, zeeman, renormalise, st)
+                         : rk4_step<float>(mesh, t, dt, (float *)m_inout, zeeman, renormalise, st);
+    }
+    if (scheme == NM_DOPRI5) {
+        if (!(rtol >= 0) || !(atol >= 0) || (rtol == 0 && atol == 0)) {
+            nm_set_error("rtol / atol must be non-negative and not both zero");
+            return NM_EINVAL;
+        }
+        return mesh->f64 ? dopri5_step<double>(mesh, t, dt, (double *)m_inout, zeeman, renormalise, rtol,
+                                               atol, err_norm_host, st)
+                         : dopri5_step<float>(mesh, t, dt, (float *)m_inout, zeeman, renormalise, rtol,
+                                              atol, err_norm_host, st);
+    }
+    nm_set_error("unknown scheme %d", (int)scheme);
+    return NM_EINVAL;
+}
+
+extern "C" nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, const void *a,
+                                        const nm_zeeman *zeeman, void *dmdt_out, void *dadt_out,
+                                        void *dudt_Ms_out, void *stream)
+{
+    NM_TRY(check_call(mesh, m, a));
+    if (!dadt_out) { nm_set_error("dadt_out is NULL"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return mesh->f64 ? adjoint_eval<double>(mesh, t, (const double *)m, (const double *)a, zeeman,
+                                            (double *)dmdt_out, (double *)dadt_out, (double *)dudt_Ms_out, st)
+                     : adjoint_eval<float>(mesh, t, (const float *)m, (const float *)a, zeeman,
+                                           (float *)dmdt_out, (float *)dadt_out, (float *)dudt_Ms_out, st);
+}
+
+extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                                         void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
+{
+    NM_TRY(check_call(mesh, m_inout, a_inout));
+    if (!u_inout) { nm_set_error("u_inout is NULL"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return mesh->f64 ? adjoint_rk4<double>(mesh, t, dt, (double *)m_inout, (double *)a_inout,
+                                           (double *)u_inout, zeeman, renormalise, st)
+                     : adjoint_rk4<float>(mesh, t, dt, (float *)m_inout, (float *)a_inout,
+                                          (float *)u_inout, zeeman, renormalise, st);
+}

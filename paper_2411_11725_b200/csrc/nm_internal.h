@@ -1,0 +1,136 @@
+// Internal definitions shared by the translation units of libnm.so (not part of the ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+#include <string>
+
+#include "../../include/nm.h"
+
+#define NM_MAX_STAGES 20
+#define NM_PROF_MAX 4096
+
+// kernel classes reported by nm_profile_end (order = NM_PROF_* of include/nm.h)
+enum NmKernelClass {
+    NM_K_X_FWD = 0, NM_K_Y_FWD, NM_K_MID, NM_K_Y_INV, NM_K_X_INV, NM_K_NODE, NM_K_ADJ_CELL,
+    NM_K_LINCOMB, NM_K_OTHER, NM_K_COUNT
+};
+#define NM_MU0 (4.0e-7 * 3.14159265358979323846264338327950288)
+
+// ------------------------------------------------------------------------------------------------
+// FFT plan for one axis: complex transform of length L as a product of radix-{8,4,2,3} stages.
+// Forward = decimation in frequency (natural order in, digit-reversed out), inverse = the
+// adjoint stages in reverse order (digit-reversed in, natural out), so a convolution needs no
+// reordering pass: the spectrum lives in digit-reversed ("position") order everywhere and
+// kmap[pos] gives the frequency index of a position, pos[k] its inverse.
+struct NmFftPlan {
+    int L;
+    int n_stages;
+    int radix[NM_MAX_STAGES];
+};
+
+template <typename T> struct NmVec2;
+template <> struct NmVec2<float> { typedef float2 type; };
+template <> struct NmVec2<double> { typedef double2 type; };
+
+// Geometry and workspace pointers handed to kernels by value.
+struct NmGeom {
+    int N1, N2, N3;    // cells
+    int n1, n2, n3;    // nodes = cells + 1
+    int P1, P2, P3;    // padded FFT lengths (2 N_d, or 1 if N_d == 1)
+    int C1;            // complex outputs of the x transform: N1 + 1 (or 1)
+    int C1p;           // row pitch of spectrum buffers, complex elements
+    int K2, K3;        // folded frequency counts along y, z: N_d + 1 (or 1)
+    int Lx;            // complex length of the packed x transform: N1 (P1/2)
+    long long cells, nodes;
+};
+
+struct nm_mesh {
+    nm_mesh_desc desc;
+    NmGeom g;
+    bool f64;
+    size_t esz;        // sizeof(real)
+    int sm_count;
+    long long launches;
+    // FFT plans
+    NmFftPlan plan_x, plan_y, plan_z;
+    // device pointers inside the caller's workspace
+    char *ws;
+    size_t ws_bytes;
+    void *Ms, *A, *Ku;      // cell scalars (real)
+    void *sMs;              // nodal S Ms (real)
+    double *Nreal;          // [6][N3][N2][N1] fp64 real-space tensor
+    void *Nhat;             // [6][K3][K2][C1p] real spectrum, scaled by 1/(P1 P2 P3)
+    void *tw_x, *tw_x2, *tw_y, *tw_z;   // complex twiddle tables
+    int *kmap_x, *pos_x, *kmap_y, *pos_y, *kmap_z, *pos_z;
+    void *bufA, *bufB;      // spectrum buffers (complex)
+    void *Hc1, *Hc2;        // cell demag fields [3][cells]
+    void *Q, *W;            // adjoint scratch: nodal vector, nodal scalar
+    void *K[7];             // RK stage derivatives (nodal vectors)
+    void *Y[2];             // RK stage states
+    void *Uc[2];            // cell scalars (adjoint RK)
+    double *partials;       // reduction scratch [node blocks + 1]
+    int n_partials;
+    bool hc1_valid;
+    // per-launch timing (nm_profile_begin / nm_profile_end)
+    bool prof_on;
+    int prof_n;
+    int prof_cls[NM_PROF_MAX];
+    cudaEvent_t prof_ev[NM_PROF_MAX][2];
+    int prof_ev_made;       // events created so far (created lazily, destroyed with the mesh)
+};
+
+// Brackets one kernel launch with an event pair when profiling is on, and counts it.
+struct NmLaunchScope {
+    nm_mesh *m;
+    cudaStream_t st;
+    int slot;
+    NmLaunchScope(nm_mesh *mesh, int cls, cudaStream_t stream) : m(mesh), st(stream), slot(-1)
+    {
+        m->launches++;
+        if (m->prof_on && m->prof_n < NM_PROF_MAX) {
+            slot = m->prof_n++;
+            if (slot >= m->prof_ev_made) {
+                cudaEventCreate(&m->prof_ev[slot][0]);
+                cudaEventCreate(&m->prof_ev[slot][1]);
+                m->prof_ev_made = slot + 1;
+            }
+            m->prof_cls[slot] = cls;
+            cudaEventRecord(m->prof_ev[slot][0], st);
+        }
+    }
+    ~NmLaunchScope()
+    {
+        if (slot >= 0) cudaEventRecord(m->prof_ev[slot][1], st);
+    }
+};
+
+void nm_set_error(const char *fmt, ...);
+
+#define NM_CUDA_TRY(expr)                                                                       \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            nm_set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__,     \
+                         __LINE__);                                                             \
+            return NM_ECUDA;                                                                    \
+        }                                                                                       \
+    } while (0)
+
+#define NM_TRY(expr)                                                                            \
+    do {                                                                                        \
+        nm_status s_ = (expr);                                                                  \
+        if (s_ != NM_OK) return s_;                                                             \
+    } while (0)
+
+// nm_tensor.cu
+nm_status nm_build_tensor(nm_mesh *mesh, cudaStream_t st);
+// nm_demag.cu
+template <typename T>
+nm_status nm_demag_conv(nm_mesh *mesh, const T *field_nodes, T *Hc_out, cudaStream_t st);
+// nm_local.cu
+nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st);
+
+extern "C" int nm_newell_near_box(const int *box, const double *dx, double *out, int n_threads);

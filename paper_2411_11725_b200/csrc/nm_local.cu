@@ -1,0 +1,457 @@
+// Node and cell kernels: a5-a11 of the hot path.
+//
+// One thread per node evaluates, in one pass over the 27-node neighbourhood and the 8 adjacent
+// cells,
+//   exchange    H = -(1/L_n) sum_{c∋n} 2 A_c sum_i' K[i,i'] m_{c+i'}        (Eqs. 3, 17-22; C3)
+//   anisotropy  H = +(1/L_n) sum_{c∋n} 2 Ku_c sum_i' M[i,i'] (m_{c+i'}.k) k  (reading C3(i))
+//   Zeeman      H = (mu0/L_n) sum_{c∋n} Ms_c sum_i' M[i,i'] Hext_{c+i'}      (Eq. 21; C3(ii))
+//   demag       H = sum_{c∋n} Ms_c Hcell_c / sum_{c∋n} Ms_c                  (C5)
+// with L_n = mu0 (V/8) sum_{c∋n} Ms_c (Eq. 22), then the LLG cross products of Eq. (1) and the
+// Runge-Kutta stage combination (a10) or the adjoint products of reading C7 (a11).
+//
+// The element matrices only depend on which coordinates of the two vertices differ, so the
+// cell loop of Eqs. (19)-(20) is regrouped by neighbour offset delta in {-1,0,1}^3: the weight of
+// m_{n+delta} is K[e(delta)] times the sum of 2 A_c over the cells that contain both nodes.  The
+// exchange term is accumulated in difference form sum w (m_{n+delta} - m_n) (rows of K sum to
+// zero), which keeps fp32 exact for smooth m.
+#include "nm_local.cuh"
+
+namespace {
+
+constexpr int kBlock = 256;
+
+template <typename T> __device__ __forceinline__ T rsqrt_t(T v);
+template <> __device__ __forceinline__ float rsqrt_t<float>(float v) { return 1.0f / sqrtf(v); }
+template <> __device__ __forceinline__ double rsqrt_t<double>(double v) { return 1.0 / sqrt(v); }
+
+template <typename T> __device__ __forceinline__ T abs_t(T v) { return v < 0 ? -v : v; }
+template <typename T> __device__ __forceinline__ T max_t(T a, T b) { return a > b ? a : b; }
+
+template <typename T>
+__device__ __forceinline__ void cross3(const T *a, const T *b, T *c)
+{
+    c[0] = a[1] * b[2] - a[2] * b[1];
+    c[1] = a[2] * b[0] - a[0] * b[2];
+    c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double red[32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) red[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (w == 0) {
+        r = l < (blockDim.x + 31) / 32 ? red[l] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+    }
+    return r;   // valid in thread 0
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
+{
+    const NmGeom &g = a.g;
+    const long long n = (long long)blockIdx.x * kBlock + threadIdx.x;
+    const bool live = n < g.nodes;
+    double err2 = 0.0;
+    if (live) {
+        const int i1 = (int)(n % g.n1);
+        const int i2 = (int)((n / g.n1) % g.n2);
+        const int i3 = (int)(n / ((long long)g.n1 * g.n2));
+        const long long nn = g.nodes;
+
+        // the 8 adjacent cells: 2A, 2Ku, Ms (0 where the cell does not exist) and sum Ms Hcell
+        T cA[8], cK[8], cM[8];
+        T hd[3] = {0, 0, 0};
+        T sms = 0;
+#pragma unroll
+        for (int oz = 0; oz < 2; ++oz)
+#pragma unroll
+            for (int oy = 0; oy < 2; ++oy)
+#pragma unroll
+                for (int ox = 0; ox < 2; ++ox) {
+                    const int c1 = i1 + ox - 1, c2 = i2 + oy - 1, c3 = i3 + oz - 1;
+                    const int ci = ox + 2 * oy + 4 * oz;
+                    const bool ok = c1 >= 0 && c1 < g.N1 && c2 >= 0 && c2 < g.N2 && c3 >= 0 && c3 < g.N3;
+                    T ms = 0, aa = 0, kk = 0;
+                    if (ok) {
+                        const long long c = ((long long)c3 * g.N2 + c2) * g.N1 + c1;
+                        ms = a.Ms[c];
+                        if (a.terms & NM_TERM_EXCHANGE) aa = (T)2 * a.A[c];
+                        if (a.terms & NM_TERM_ANISO) kk = (T)2 * a.Ku[c];
+                        if (a.Hc) {
+                            hd[0] += ms * a.Hc[c];
+                            hd[1] += ms * a.Hc[g.cells + c];
+                            hd[2] += ms * a.Hc[2 * g.cells + c];
+                        }
+                    }
+                    cM[ci] = ms; cA[ci] = aa; cK[ci] = kk;
+                    sms += ms;
+                }
+
+        const T mc[3] = {a.fld[n], a.fld[nn + n], a.fld[2 * nn + n]};
+        const bool zee_on = (a.terms & NM_TERM_ZEEMAN) != 0;
+        const bool zee_nodal = zee_on && (a.h_static || a.h_pulse);
+        T ex[3] = {0, 0, 0}, ze[3] = {0, 0, 0};
+        T an = 0;
+#pragma unroll
+        for (int dz = -1; dz <= 1; ++dz)
+#pragma unroll
+            for (int dy = -1; dy <= 1; ++dy)
+#pragma unroll
+                for (int dx = -1; dx <= 1; ++dx) {
+                    const int e = (dx != 0) | ((dy != 0) << 1) | ((dz != 0) << 2);
+                    // cells that contain both n and n + delta
+                    T sA = 0, sK = 0, sM = 0;
+#pragma unroll
+                    for (int oz = 0; oz < 2; ++oz)
+#pragma unroll
+                        for (int oy = 0; oy < 2; ++oy)
+#pragma unroll
+                            for (int ox = 0; ox < 2; ++ox) {
+                                const bool in = (dx == 0 || ox == (dx + 1) / 2) &&
+                                                (dy == 0 || oy == (dy + 1) / 2) &&
+                                                (dz == 0 || oz == (dz + 1) / 2);
+                                if (in) {
+                                    const int ci = ox + 2 * oy + 4 * oz;
+                                    sA += cA[ci]; sK += cK[ci]; sM += cM[ci];
+                                }
+                            }
+                    const int j1 = i1 + dx, j2 = i2 + dy, j3 = i3 + dz;
+                    const bool inb = j1 >= 0 && j1 < g.n1 && j2 >= 0 && j2 < g.n2 && j3 >= 0 && j3 < g.n3;
+                    if (!inb) continue;
+                    const long long nb = n + dx + (long long)dy * g.n1 + (long long)dz * g.n1 * g.n2;
+                    T mb[3];
+                    if (e == 0) {
+                        mb[0] = mc[0]; mb[1] = mc[1]; mb[2] = mc[2];
+                    } else {
+                        mb[0] = a.fld[nb]; mb[1] = a.fld[nn + nb]; mb[2] = a.fld[2 * nn + nb];
+                        const T w = a.wK[e] * sA;
+                        ex[0] += w * (mb[0] - mc[0]);
+                        ex[1] += w * (mb[1] - mc[1]);
+                        ex[2] += w * (mb[2] - mc[2]);
+                    }
+                    an += a.wM[e] * sK * (mb[0] * a.kax[0] + mb[1] * a.kax[1] + mb[2] * a.kax[2]);
+                    if (zee_nodal) {
+                        const T w = a.wM[e] * sM;
+#pragma unroll
+                        for (int j = 0; j < 3; ++j) {
+                            T h = 0;
+                            if (a.h_static) h += a.h_static[j * nn + nb];
+                            if (a.h_pulse) h += a.amp * a.h_pulse[j * nn + nb];
+                            ze[j] += w * h;
+                        }
+                    }
+                }
+
+        T H[3] = {0, 0, 0};
+        if (sms > 0) {
+            const T invL = (T)1 / (a.mu0V8 * sms);
+            const T invS = (T)1 / sms;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                T h = (a.kax[j] * an - ex[j]) * invL + hd[j] * invS;
+                if (zee_on) h += a.hu[j];
+                if (zee_nodal) h += a.mu0 * ze[j] * invL;
+                H[j] = h;
+            }
+        }
+
+        if (a.mode == NM_MODE_H) {
+            a.out[n] = H[0]; a.out[nn + n] = H[1]; a.out[2 * nn + n] = H[2];
+        } else if (a.mode == NM_MODE_ADJ2) {
+            // dadt = -(d + (S Ms) Hlin(q));  fld = q, H = Hlin(q)
+#pragma unroll
+            for (int j = 0; j < 3; ++j) a.dadt[j * nn + n] = -(a.dadt[j * nn + n] + sms * H[j]);
+        } else {
+            T mxH[3], mxmxH[3], f[3];
+            cross3(mc, H, mxH);
+            cross3(mc, mxH, mxmxH);
+#pragma unroll
+            for (int j = 0; j < 3; ++j) f[j] = -a.gp * mxH[j] - a.agp * mxmxH[j];
+            if (a.mode == NM_MODE_RHS) {
+                a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
+            } else if (a.mode == NM_MODE_RK) {
+                const NmRkArgs<T> &r = a.rk;
+                if (r.kstore) {
+                    r.kstore[n] = f[0]; r.kstore[nn + n] = f[1]; r.kstore[2 * nn + n] = f[2];
+                }
+                T y0[3], y[3], er[3];
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    y0[j] = r.y0[j * nn + n];
+                    T acc = r.cself * f[j];
+                    T ea = r.eself * f[j];
+                    for (int p = 0; p < r.nprev; ++p) {
+                        const T kp = r.kprev[p][j * nn + n];
+                        acc += r.cprev[p] * kp;
+                        ea += r.eprev[p] * kp;
+                    }
+                    y[j] = y0[j] + r.dt * acc;
+                    er[j] = r.dt * ea;
+                }
+                if (r.ynext) {
+                    if (r.renorm) {
+                        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+                        y[0] *= inv; y[1] *= inv; y[2] *= inv;
+                    }
+                    r.ynext[n] = y[0]; r.ynext[nn + n] = y[1]; r.ynext[2 * nn + n] = y[2];
+                }
+                if (r.want_err) {
+                    // last Dormand-Prince stage: fld = y5 (un-normalised), y0 = start of step
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) {
+                        const T sc = r.atol + r.rtol * max_t(abs_t(y0[j]), abs_t(mc[j]));
+                        const double q = (double)(er[j] / sc);
+                        err2 += q * q;
+                    }
+                }
+            } else {   // NM_MODE_ADJ1
+                if (a.out) {
+                    a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
+                }
+                const T av[3] = {a.adj[n], a.adj[nn + n], a.adj[2 * nn + n]};
+                T mxa[3], mxmxa[3], Hxa[3], b[3];
+                cross3(mc, av, mxa);
+                cross3(mc, mxa, mxmxa);
+                cross3(H, av, Hxa);
+                const T mH = mc[0] * H[0] + mc[1] * H[1] + mc[2] * H[2];
+                const T am = av[0] * mc[0] + av[1] * mc[1] + av[2] * mc[2];
+                const T aH = av[0] * H[0] + av[1] * H[1] + av[2] * H[2];
+                const T invS = sms > 0 ? (T)1 / sms : (T)0;
+                T bH = 0;
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    b[j] = a.gp * mxa[j] - a.agp * mxmxa[j];
+                    const T d = -a.gp * Hxa[j] - a.agp * (mH * av[j] + am * H[j] - (T)2 * aH * mc[j]);
+                    a.dadt[j * nn + n] = d;
+                    a.Q[j * nn + n] = b[j] * invS;
+                    bH += b[j] * H[j];
+                }
+                a.W[n] = bH * invS;
+            }
+        }
+    }
+    if (a.mode == NM_MODE_RK && a.rk.want_err) {
+        const double s = block_sum(err2);
+        if (threadIdx.x == 0) a.rk.partials[blockIdx.x] = s;
+    }
+}
+
+// partials[0..n) -> partials[n] = sqrt(sum / count), fixed summation order
+__global__ void k_err_final(double *partials, int n, double count)
+{
+    double v = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) v += partials[i];
+    const double s = block_sum(v);
+    if (threadIdx.x == 0) partials[n] = sqrt(s / count);
+}
+
+// Dormand-Prince commit: m <- (normalised) y5 iff err <= 1
+template <typename T>
+__global__ void k_commit(T *__restrict__ m, const T *__restrict__ y5, long long nodes,
+                         const double *__restrict__ err, int renorm)
+{
+    if (!(*err <= 1.0)) return;
+    const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= nodes) return;
+    T y[3] = {y5[n], y5[nodes + n], y5[2 * nodes + n]};
+    if (renorm) {
+        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+        y[0] *= inv; y[1] *= inv; y[2] *= inv;
+    }
+    m[n] = y[0]; m[nodes + n] = y[1]; m[2 * nodes + n] = y[2];
+}
+
+template <typename T>
+__global__ void k_sMs(const T *__restrict__ Ms, T *__restrict__ sMs, NmGeom g)
+{
+    const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= g.nodes) return;
+    const int i1 = (int)(n % g.n1), i2 = (int)((n / g.n1) % g.n2), i3 = (int)(n / ((long long)g.n1 * g.n2));
+    T s = 0;
+    for (int oz = 0; oz < 2; ++oz)
+        for (int oy = 0; oy < 2; ++oy)
+            for (int ox = 0; ox < 2; ++ox) {
+                const int c1 = i1 + ox - 1, c2 = i2 + oy - 1, c3 = i3 + oz - 1;
+                if (c1 >= 0 && c1 < g.N1 && c2 >= 0 && c2 < g.N2 && c3 >= 0 && c3 < g.N3)
+                    s += Ms[((long long)c3 * g.N2 + c2) * g.N1 + c1];
+            }
+    sMs[n] = s;
+}
+
+// a11, Ms gradient per cell (reading C7):
+//   dudt_c = -[ -(S^T w)_c + zeeman piece + (S^T q)_c . Hcell_c + mbar_c . Y_c ],  Y = 8 Hc2
+template <typename T>
+__global__ void k_adj_cell(const NmAdjCellArgs<T> a)
+{
+    const NmGeom &g = a.g;
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= g.cells) return;
+    const int c1 = (int)(c % g.N1), c2 = (int)((c / g.N1) % g.N2), c3 = (int)(c / ((long long)g.N1 * g.N2));
+    const long long nn = g.nodes;
+    T sw = 0, sq[3] = {0, 0, 0}, sm[3] = {0, 0, 0}, zee = 0;
+    const bool zee_on = (a.terms & NM_TERM_ZEEMAN) != 0;
+    const bool zee_nodal = zee_on && (a.h_static || a.h_pulse);
+    long long nd[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        nd[i] = ((long long)(c3 + (i >> 2)) * g.n2 + (c2 + ((i >> 1) & 1))) * g.n1 + (c1 + (i & 1));
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        sw += a.W[nd[i]];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            sq[j] += a.Q[j * nn + nd[i]];
+            sm[j] += a.m[j * nn + nd[i]];
+        }
+    }
+    if (zee_nodal) {
+        for (int ip = 0; ip < 8; ++ip) {
+            T h[3];
+            for (int j = 0; j < 3; ++j) {
+                T v = 0;
+                if (a.h_static) v += a.h_static[j * nn + nd[ip]];
+                if (a.h_pulse) v += a.amp * a.h_pulse[j * nn + nd[ip]];
+                h[j] = v;
+            }
+            for (int i = 0; i < 8; ++i) {
+                const T w = a.wM8V[i ^ ip];
+                zee += w * (a.Q[nd[i]] * h[0] + a.Q[nn + nd[i]] * h[1] + a.Q[2 * nn + nd[i]] * h[2]);
+            }
+        }
+    }
+    if (zee_on) zee += sq[0] * a.hu[0] + sq[1] * a.hu[1] + sq[2] * a.hu[2];
+    T grad = -sw + zee;
+    if (a.Hc1) {
+        for (int j = 0; j < 3; ++j)
+            grad += sq[j] * a.Hc1[j * g.cells + c] + sm[j] * a.Hc2[j * g.cells + c];   // mbar.Y = (sm/8).(8 Hc2)
+    }
+    a.dudt[c] = -grad;
+}
+
+// out = base + sum_j coef_j src_j  (optionally normalised as 3-vectors over `vec_n` nodes)
+template <typename T> struct LinArgs {
+    T *out;
+    const T *base;
+    const T *src[4];
+    T coef[4];
+    int nsrc;
+    long long n;        // elements
+    long long vec_n;    // > 0: arrays are [3][vec_n] and the result is normalised per node
+};
+
+template <typename T> __global__ void k_lincomb(const LinArgs<T> a)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a.vec_n > 0) {
+        if (i >= a.vec_n) return;
+        T y[3];
+        for (int j = 0; j < 3; ++j) {
+            T v = a.base[j * a.vec_n + i];
+            for (int s = 0; s < a.nsrc; ++s) v += a.coef[s] * a.src[s][j * a.vec_n + i];
+            y[j] = v;
+        }
+        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+        for (int j = 0; j < 3; ++j) a.out[j * a.vec_n + i] = y[j] * inv;
+    } else {
+        if (i >= a.n) return;
+        T v = a.base[i];
+        for (int s = 0; s < a.nsrc; ++s) v += a.coef[s] * a.src[s][i];
+        a.out[i] = v;
+    }
+}
+
+inline unsigned nblk(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+} // namespace
+
+// ---- host launchers used by nm_api.cu -----------------------------------------------------------
+template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
+{
+    {
+        NmLaunchScope sc(mesh, NM_K_NODE, st);
+        k_node<T><<<nblk(a.g.nodes, kBlock), kBlock, 0, st>>>(a);
+    }
+
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+int nm_node_blocks(long long nodes) { return (int)nblk(nodes, kBlock); }
+
+nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st)
+{
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        k_err_final<<<1, 1024, 0, st>>>(mesh->partials, n_partials, count);
+    }
+
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+template <typename T>
+nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st)
+{
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        k_commit<T><<<nblk(mesh->g.nodes, 256), 256, 0, st>>>(m, y5, mesh->g.nodes, err, renorm);
+    }
+
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+template <typename T> nm_status nm_launch_adj_cell(nm_mesh *mesh, const NmAdjCellArgs<T> &a, cudaStream_t st)
+{
+    {
+        NmLaunchScope sc(mesh, NM_K_ADJ_CELL, st);
+        k_adj_cell<T><<<nblk(a.g.cells, 128), 128, 0, st>>>(a);
+    }
+
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+template <typename T>
+nm_status nm_lincomb(nm_mesh *mesh, T *out, const T *base, int nsrc, const T *const *src, const T *coef,
+                     long long n, long long vec_n, cudaStream_t st)
+{
+    LinArgs<T> a;
+    a.out = out; a.base = base; a.nsrc = nsrc; a.n = n; a.vec_n = vec_n;
+    for (int s = 0; s < 4; ++s) {
+        a.src[s] = s < nsrc ? src[s] : nullptr;
+        a.coef[s] = s < nsrc ? coef[s] : (T)0;
+    }
+    {
+        NmLaunchScope sc(mesh, NM_K_LINCOMB, st);
+        k_lincomb<T><<<nblk(vec_n > 0 ? vec_n : n, 256), 256, 0, st>>>(a);
+    }
+
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st)
+{
+    NmLaunchScope sc(mesh, NM_K_OTHER, st);
+    if (mesh->f64)
+        k_sMs<double><<<nblk(mesh->g.nodes, 256), 256, 0, st>>>((const double *)mesh->Ms, (double *)mesh->sMs, mesh->g);
+    else
+        k_sMs<float><<<nblk(mesh->g.nodes, 256), 256, 0, st>>>((const float *)mesh->Ms, (float *)mesh->sMs, mesh->g);
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+#define NM_INST(T)                                                                                       \
+    template nm_status nm_launch_node<T>(nm_mesh *, const NmLocalArgs<T> &, cudaStream_t);              \
+    template nm_status nm_launch_commit<T>(nm_mesh *, T *, const T *, const double *, int, cudaStream_t); \
+    template nm_status nm_launch_adj_cell<T>(nm_mesh *, const NmAdjCellArgs<T> &, cudaStream_t);        \
+    template nm_status nm_lincomb<T>(nm_mesh *, T *, const T *, int, const T *const *, const T *,       \
+                                     long long, long long, cudaStream_t);
+NM_INST(float)
+NM_INST(double)

@@ -1,0 +1,74 @@
+// Argument blocks of the node / cell kernels in nm_local.cu (internal).
+#pragma once
+
+#include "nm_internal.h"
+
+enum NmLocalMode {
+    NM_MODE_H = 0,      // out = H_eff
+    NM_MODE_RHS = 1,    // out = f(m, H)                                  (Eq. 1)
+    NM_MODE_RK = 2,     // Runge-Kutta stage epilogue (a10)
+    NM_MODE_ADJ1 = 3,   // adjoint pass 1: f, b, d, q = b/(S Ms), w = b.H/(S Ms)
+    NM_MODE_ADJ2 = 4    // adjoint pass 2: dadt = -(d + (S Ms) Hlin(q))
+};
+
+template <typename T> struct NmRkArgs {
+    const T *y0;        // state at the start of the step
+    T *kstore;          // where to keep this stage's derivative (or null)
+    const T *kprev[6];  // earlier stage derivatives
+    T cprev[6];         // their weights in the next stage state / final update
+    T eprev[6];         // their weights in the embedded error (last Dormand-Prince stage)
+    int nprev;
+    T cself, eself;
+    T *ynext;           // y0 + dt (sum cprev kprev + cself f), or null
+    T dt;
+    int renorm;         // normalise ynext (final RK4 update written to m in place)
+    int want_err;       // accumulate the scaled squared error into partials[blockIdx.x]
+    T rtol, atol;
+    double *partials;
+};
+
+template <typename T> struct NmLocalArgs {
+    NmGeom g;
+    const T *fld;       // nodal field the linear operators act on (m, or q in NM_MODE_ADJ2)
+    const T *Ms, *A, *Ku, *sMs;
+    const T *Hc;        // cell demag field [3][cells] or null
+    unsigned terms;
+    T wK[8], wM[8];     // element matrix entries by offset pattern e (bit d: vertices differ along d)
+    T kax[3];
+    T mu0V8;            // mu0 V / 8
+    T mu0;
+    // Zeeman: H_ext = hu + h_static + amp * h_pulse
+    const T *h_static, *h_pulse;
+    T amp;
+    T hu[3];
+    // LLG
+    T gp, agp;          // gamma' = gamma/(1+alpha^2), alpha gamma'
+    int mode;
+    T *out;             // H (MODE_H), f (MODE_RHS / ADJ1, may be null), dadt (ADJ1: d, ADJ2: final)
+    // adjoint
+    const T *adj;       // a
+    T *Q, *W, *dadt;
+    NmRkArgs<T> rk;
+};
+
+template <typename T> struct NmAdjCellArgs {
+    NmGeom g;
+    const T *m, *Q, *W, *Hc1, *Hc2;
+    const T *h_static, *h_pulse;
+    T amp;
+    T hu[3];
+    T wM8V[8];          // (8/V) * mass matrix entry by offset pattern
+    unsigned terms;
+    T *dudt;
+};
+
+// host launchers defined in nm_local.cu
+template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st);
+int nm_node_blocks(long long nodes);
+nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st);
+template <typename T>
+nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st);
+template <typename T> nm_status nm_launch_adj_cell(nm_mesh *mesh, const NmAdjCellArgs<T> &a, cudaStream_t st);
+template <typename T>
+nm_status nm_lincomb(nm_mesh *mesh, T *out, const T *base, int nsrc, const T *const *src, const T *coef,
+                     long long n, long long vec_n, cudaStream_t st);

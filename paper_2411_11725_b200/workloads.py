@@ -162,3 +162,24 @@ def fd_cells(w, k=8, seed=6):
     rng = np.random.default_rng(seed)
     flat = rng.choice(int(np.prod(w.n_cells)), size=k, replace=False)
     return [tuple(int(v) for v in np.unravel_index(f, w.n_cells)) for f in flat]
+
+
+def varied_case(n_cells, dx=(2e-9, 3e-9, 2.5e-9), seed=11, vacuum=False, alpha=0.05):
+    """Ragged parity case: every term on, cell-wise random Ms, A, Ku (optionally a vacuum corner
+    block with Ms = 0), a tilted anisotropy axis, smoothed random m and a nodal static field.
+    Returns (workload, h_static)."""
+    n = tuple(int(v) for v in n_cells)
+    rng = np.random.default_rng(seed)
+    w = Workload("varied_%dx%dx%d" % n, n, tuple(dx), None, None, alpha=alpha,
+                 terms=TERM_EXCHANGE | TERM_DEMAG | TERM_ANISO | TERM_ZEEMAN, seed=seed,
+                 h_uniform=(1e4, -2e4, 3e4), dt=2e-14)
+    w.Ms = rng.uniform(4e5, 9e5, size=n)
+    w.A = rng.uniform(0.8e-11, 1.5e-11, size=n)
+    w.Ku = rng.uniform(1e5, 5e5, size=n)
+    if vacuum:
+        w.Ms[: max(1, n[0] // 3), : max(1, n[1] // 2), :] = 0.0
+    k = np.array([1.0, 2.0, 2.0])
+    w.ku_axis = tuple(k / np.sqrt(np.sum(k * k)))
+    w.m0 = _unit(box_filter3(random_unit_field(w.node_shape, seed + 1)))
+    h_static = 5e4 * rng.standard_normal((3,) + w.node_shape)
+    return w, h_static

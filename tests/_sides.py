@@ -1,0 +1,81 @@
+"""Build the two sides of a parity test from one seeded Workload (tests only).
+
+`oracle_problem` feeds the rounded inputs to the fp64 CPU oracle, `gpu_mesh` feeds the same
+rounded inputs to libnm.so through the ctypes binding.  Nothing here does any of the method's
+arithmetic.
+"""
+import numpy as np
+
+from paper_2411_11725_b200 import workloads as wl
+
+
+def rel_l2(x, ref):
+    x = np.asarray(x, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    den = np.sqrt(np.sum(ref * ref))
+    num = np.sqrt(np.sum((x - ref) ** 2))
+    return num / den if den > 0 else num
+
+
+def np_dtype(torch_dtype):
+    import torch
+    return np.float64 if torch_dtype == torch.float64 else np.float32
+
+
+def oracle_problem(w, dtype=np.float64):
+    """oracle.llg.Problem with the materials rounded to the build precision."""
+    from oracle import llg
+    r = lambda v: wl.round_to(w.cell_array(v), dtype)
+    return llg.Problem(tuple(w.n_cells), tuple(float(v) for v in w.dx), r(w.Ms), r(w.A), r(w.Ku),
+                       tuple(w.ku_axis), float(w.gamma), float(w.alpha), int(w.terms))
+
+
+def oracle_zeeman(w, dtype=np.float64, h_static=None):
+    """Callable t -> nodal H_ext (paper index order) matching gpu_zeeman, or None."""
+    if not (w.terms & wl.TERM_ZEEMAN):
+        return None
+    hu = wl.round_to(np.asarray(w.h_uniform, dtype=np.float64), dtype)
+    hp = wl.round_to(w.h_pulse, dtype) if w.h_pulse is not None else None
+    hs = wl.round_to(h_static, dtype) if h_static is not None else None
+    shape = (3,) + w.node_shape
+
+    def z(t):
+        h = np.broadcast_to(hu[:, None, None, None], shape).copy()
+        if hs is not None:
+            h += hs
+        if hp is not None:
+            amp = float(np.asarray(wl.sinc_pulse(t, **w.pulse) if w.pulse else 1.0).astype(dtype))
+            h += amp * hp
+        return h
+    return z
+
+
+def dev(a, torch_dtype, device=0):
+    """Paper-order numpy array -> ABI-order device tensor of the mesh dtype."""
+    import torch
+    return torch.from_numpy(wl.to_abi(a)).to(device="cuda:%d" % device, dtype=torch_dtype).contiguous()
+
+
+def host(t):
+    """ABI-order device tensor -> paper-order fp64 numpy array."""
+    return wl.from_abi(t.detach().cpu().double().numpy())
+
+
+def gpu_mesh(w, torch_dtype, device=0):
+    from paper_2411_11725_b200 import binding as nm
+    mat = {}
+    for name in ("Ms", "A", "Ku"):
+        v = getattr(w, name)
+        mat[name] = float(v) if np.isscalar(v) else dev(v, torch_dtype, device)
+    return nm.Mesh(w.n_cells, w.dx, dtype=torch_dtype, device=device, terms=w.terms, gamma=w.gamma,
+                   alpha=w.alpha, ku_axis=w.ku_axis, **mat)
+
+
+def gpu_zeeman(w, torch_dtype, device=0, h_static=None):
+    from paper_2411_11725_b200 import binding as nm
+    if not (w.terms & wl.TERM_ZEEMAN):
+        return None
+    hp = dev(w.h_pulse, torch_dtype, device) if w.h_pulse is not None else None
+    hs = dev(h_static, torch_dtype, device) if h_static is not None else None
+    amp = (lambda t: wl.sinc_pulse(t, **w.pulse)) if (w.pulse and hp is not None) else None
+    return nm.Zeeman(h_uniform=w.h_uniform, h_static=hs, h_pulse=hp, amp=amp)

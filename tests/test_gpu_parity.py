@@ -1,0 +1,290 @@
+"""GPU parity: libnm.so (through the C-ABI binding) against the fp64 CPU oracle, element by element
+on the same seeded inputs.  Tolerances are north_star's: relative L2 <= 1e-5 (fp32), 1e-11 (fp64).
+"""
+import numpy as np
+import pytest
+
+from paper_2411_11725_b200 import workloads as wl
+
+from _sides import (dev, gpu_mesh, gpu_zeeman, host, np_dtype, oracle_problem, oracle_zeeman,
+                    rel_l2)
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+TOL = {"f32": 1e-5, "f64": 1e-11}
+DT = {"f32": torch.float32, "f64": torch.float64}
+
+
+def _m0(w, td):
+    return wl.round_to(w.m0, np_dtype(td))
+
+
+# ---- demag tensor (reading C4): library setup vs the oracle's __float128 closed form -------------
+@pytest.mark.parametrize("n,dx", [((12, 8, 6), (2e-9, 3e-9, 2.5e-9)),
+                                  ((32, 8, 1), (3.125e-9, 3.125e-9, 3e-9)),
+                                  ((48, 48, 48), (2e-9, 2e-9, 2e-9)),
+                                  ((1, 1, 1), (1e-9, 2e-9, 0.5e-9)),
+                                  ((64, 2, 1), (1e-9, 4e-9, 8e-9))])
+def test_tensor_matches_oracle(n, dx):
+    from oracle import demag
+    from paper_2411_11725_b200 import binding as nm
+    mesh = nm.Mesh(n, dx, dtype=torch.float64, terms=wl.TERM_DEMAG, Ms=1.0, A=0.0, Ku=0.0)
+    got = mesh.nm_debug_get_tensor()            # [6][N3][N2][N1]
+    ref = wl.to_abi(demag.demag_tensor(n, dx))  # oracle [6][N1][N2][N3] -> ABI order
+    assert got.shape == ref.shape
+    assert np.max(np.abs(got - ref)) <= 1e-13
+
+
+# ---- H_eff ---------------------------------------------------------------------------------------
+def _heff_case(w, prec, h_static=None):
+    td = DT[prec]
+    nd = np_dtype(td)
+    p = oracle_problem(w, nd)
+    m = _m0(w, td)
+    z = oracle_zeeman(w, nd, h_static)
+    from oracle import llg
+    ref = llg.effective_field(p, m, z(0.0) if z else None)
+    mesh = gpu_mesh(w, td)
+    got = host(mesh.nm_heff(0.0, dev(m, td), gpu_zeeman(w, td, h_static=h_static)))
+    return got, ref, mesh, p, m
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_heff_config1_tiny_film(prec):
+    got, ref, *_ = _heff_case(wl.config1_tiny_film(), prec)
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_heff_config2_cube64(prec):
+    got, ref, *_ = _heff_case(wl.config2_cube(64), prec)
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(24, 12, 6), (6, 18, 48), (16, 1, 1), (1, 16, 4), (1, 1, 1),
+                               (2, 2, 2), (96, 4, 3), (9, 27, 2)])
+def test_heff_ragged_all_terms(n, prec):
+    w, hs = wl.varied_case(n, vacuum=(n[0] >= 6))
+    got, ref, *_ = _heff_case(w, prec, hs)
+    assert rel_l2(got, ref) <= TOL[prec]
+    # vacuum nodes (S Ms = 0) get exactly H = 0 (reading C3(iii))
+    from oracle.mesh import scatter_cells_to_nodes
+    vac = scatter_cells_to_nodes(w.cell_array(w.Ms)) == 0
+    assert np.all(got[:, vac] == 0)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_heff_term_by_term(prec):
+    """Each term alone against the oracle's part (a dropped or mis-signed term cannot hide)."""
+    from oracle import llg
+    td = DT[prec]
+    nd = np_dtype(td)
+    base, hs = wl.varied_case((12, 6, 4))
+    for term in (wl.TERM_EXCHANGE, wl.TERM_DEMAG, wl.TERM_ANISO, wl.TERM_ZEEMAN):
+        w, _ = wl.varied_case((12, 6, 4))
+        w.terms = term
+        p = oracle_problem(w, nd)
+        m = _m0(w, td)
+        z = oracle_zeeman(w, nd, hs)
+        ref = llg.effective_field(p, m, z(0.0) if z else None)
+        got = host(gpu_mesh(w, td).nm_heff(0.0, dev(m, td), gpu_zeeman(w, td, h_static=hs)))
+        assert rel_l2(got, ref) <= TOL[prec], term
+
+
+def test_cell_demag_field_matches_direct_sum():
+    """Cell field from the FFT passes vs the oracle's brute-force O(N^2) sum (no FFT on that side)."""
+    from oracle import demag
+    w, _ = wl.varied_case((6, 4, 3))
+    w.terms = wl.TERM_DEMAG
+    td = torch.float64
+    p = oracle_problem(w)
+    m = _m0(w, td)
+    mesh = gpu_mesh(w, td)
+    mesh.nm_heff(0.0, dev(m, td))
+    got = host(mesh.nm_debug_get_cell_field())
+    ref = demag.demag_field_cells_direct(demag.cell_magnetization(m, p.Ms), p.Nt)
+    assert rel_l2(got, ref) <= 1e-12
+
+
+# ---- LLG right-hand side and Runge-Kutta ---------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_llg_rhs(prec):
+    from oracle import llg
+    td = DT[prec]
+    nd = np_dtype(td)
+    w, hs = wl.varied_case((12, 6, 4), vacuum=True)
+    p = oracle_problem(w, nd)
+    m = _m0(w, td)
+    ref = llg.llg_rhs(p, 0.0, m, oracle_zeeman(w, nd, hs))
+    got = host(gpu_mesh(w, td).nm_llg_rhs(0.0, dev(m, td), gpu_zeeman(w, td, h_static=hs)))
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+def test_rk4_trajectory_config1_fp64():
+    """Config 1: 200 fixed RK4 steps of 1e-13 s in fp64, whole trajectory end state."""
+    from oracle import llg
+    w = wl.config1_tiny_film()
+    td = torch.float64
+    p = oracle_problem(w)
+    m = _m0(w, td)
+    mesh = gpu_mesh(w, td)
+    y = dev(m, td)
+    ref = m.copy()
+    worst = 0.0
+    for s in range(w.n_steps):
+        ref = llg.rk4_step(p, s * w.dt, w.dt, ref)
+        mesh.nm_rk_step(0, s * w.dt, w.dt, y)
+        if s % 50 == 49:
+            worst = max(worst, rel_l2(host(y), ref))
+    assert worst <= 1e-11
+    assert np.max(np.abs(np.sqrt(np.sum(host(y) ** 2, axis=0)) - 1.0)) < 1e-14
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_rk4_steps_all_terms(prec):
+    from oracle import llg
+    td = DT[prec]
+    nd = np_dtype(td)
+    w, hs = wl.varied_case((12, 6, 4))
+    p = oracle_problem(w, nd)
+    z = oracle_zeeman(w, nd, hs)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td, h_static=hs)
+    ref = _m0(w, td)
+    y = dev(ref, td)
+    for s in range(5):
+        ref = llg.rk4_step(p, s * w.dt, w.dt, ref, z)
+        mesh.nm_rk_step(0, s * w.dt, w.dt, y, gz)
+    assert rel_l2(host(y), ref) <= TOL[prec]
+    # without renormalisation
+    ref2 = llg.rk4_step(p, 0.0, w.dt, _m0(w, td), z, renormalise=False)
+    y2 = dev(_m0(w, td), td)
+    mesh.nm_rk_step(0, 0.0, w.dt, y2, gz, renormalise=False)
+    assert rel_l2(host(y2), ref2) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_dopri5_step_accept_and_reject(prec):
+    from oracle import llg
+    td = DT[prec]
+    nd = np_dtype(td)
+    w, hs = wl.varied_case((12, 6, 4))
+    p = oracle_problem(w, nd)
+    z = oracle_zeeman(w, nd, hs)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td, h_static=hs)
+    m = _m0(w, td)
+    for dt, expect in ((2e-14, True), (2e-12, False)):
+        ref, err_ref, acc = llg.dopri5_step(p, 0.0, dt, m, z, rtol=1e-5, atol=1e-5)
+        assert acc == expect
+        y = dev(m, td)
+        err = mesh.nm_rk_step(1, 0.0, dt, y, gz, rtol=1e-5, atol=1e-5, want_err=True)
+        # fp32: the embedded error is a cancelling sum of stage derivatives, so its rounding floor
+        # (~1e-5 of the scaled norm) is absolute, not relative
+        assert abs(err - err_ref) <= (1e-8 * err_ref if prec == "f64" else 2e-2 * err_ref + 1e-4)
+        assert rel_l2(host(y), ref) <= TOL[prec]
+        if not expect:
+            assert np.array_equal(host(y), m)      # rejected step leaves m untouched
+
+
+def test_dopri5_replay_config3_small_fp32():
+    """Config 3's recipe on a 64x64x1 film: the GPU runs the adaptive controller in fp32, the
+    oracle replays the GPU's accepted/rejected dt sequence in fp64."""
+    from oracle import llg
+    w = wl.config3_thin_film(64)
+    td = torch.float32
+    p = oracle_problem(w, np.float32)
+    z = oracle_zeeman(w, np.float32)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    ref = _m0(w, td)
+    y = dev(ref, td)
+    t, dt = 0.0, 1e-13
+    accepted = 0
+    for _ in range(60):
+        err = mesh.nm_rk_step(1, t, dt, y, gz, rtol=1e-5, atol=1e-5, want_err=True)
+        out, err_ref, acc = llg.dopri5_step(p, t, dt, ref, z, rtol=1e-5, atol=1e-5)
+        if err <= 1.0:
+            assert acc or abs(err_ref - 1.0) < 1e-2
+            ref = out if acc else ref
+            t += dt
+            accepted += 1
+        dt = llg.dopri5_next_dt(dt, err)
+        if accepted >= 25:
+            break
+    assert accepted >= 10
+    assert rel_l2(host(y), ref) <= 1e-5
+
+
+# ---- adjoint -------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("nodal_zeeman", [False, True])
+def test_adjoint_rhs(prec, nodal_zeeman):
+    from oracle import adjoint
+    td = DT[prec]
+    nd = np_dtype(td)
+    w, hs = wl.varied_case((12, 6, 4))
+    if not nodal_zeeman:
+        hs = None
+    p = oracle_problem(w, nd)
+    z = oracle_zeeman(w, nd, hs)
+    m = _m0(w, td)
+    a = wl.round_to(np.random.default_rng(77).standard_normal(m.shape), nd)
+    f_ref, da_ref, du_ref = adjoint.adjoint_rhs(p, 0.0, m, a, z)
+    mesh = gpu_mesh(w, td)
+    f, da, du = mesh.nm_llg_adjoint_rhs(0.0, dev(m, td), dev(a, td), gpu_zeeman(w, td, h_static=hs))
+    assert rel_l2(host(f), f_ref) <= TOL[prec]
+    assert rel_l2(host(da), da_ref) <= TOL[prec]
+    # the Ms gradient is a sum of cancelling pieces: fp32 gets a looser bound
+    assert rel_l2(host(du), du_ref) <= (1e-11 if prec == "f64" else 2e-4)
+
+
+def test_adjoint_rk4_backward_small_config5_fp64():
+    """Config 5's recipe on a 32x8x1 film, 40 steps, checkpoints every 10: u(0) = dJ/dMs."""
+    from oracle import adjoint
+    w = wl.config5_inverse((32, 8, 1), n_steps=40)
+    td = torch.float64
+    p = oracle_problem(w)
+    z = oracle_zeeman(w)
+    gz = gpu_zeeman(w, td)
+    m0 = _m0(w, td)
+    mT_ref, ck = adjoint.forward_rk4(p, m0, w.dt, w.n_steps, z, checkpoint_every=10)
+    aT = wl.objective_weights(w)
+    _, a0_ref, u0_ref = adjoint.backward_rk4(p, mT_ref, aT, w.dt, w.n_steps, z, checkpoints=ck)
+
+    mesh = gpu_mesh(w, td)
+    y = dev(m0, td)
+    gck = {}
+    for s in range(w.n_steps):
+        if s % 10 == 0:
+            gck[s] = y.clone()
+        mesh.nm_rk_step(0, s * w.dt, w.dt, y, gz)
+    assert rel_l2(host(y), mT_ref) <= 1e-11
+    a = dev(aT, td)
+    u = torch.zeros(mesh.cell_shape_abi, dtype=td, device="cuda:0")
+    for s in range(w.n_steps, 0, -1):
+        mesh.nm_adjoint_rk4_step(s * w.dt, w.dt, y, a, u, gz)
+        if (s - 1) in gck:
+            y.copy_(gck[s - 1])
+    assert rel_l2(host(a), a0_ref) <= 1e-11
+    assert rel_l2(wl.from_abi(u.cpu().numpy()), u0_ref) <= 1e-11
+
+
+# ---- boundary behaviour --------------------------------------------------------------------------
+def test_errors_are_statuses_not_crashes():
+    from paper_2411_11725_b200 import binding as nm
+    with pytest.raises(nm.NmError) as e:
+        nm.Mesh((5, 4, 4), (1e-9,) * 3, terms=wl.TERM_DEMAG, Ms=1.0, A=0.0, Ku=0.0)
+    assert e.value.status == nm.NM_EUNSUPPORTED
+    with pytest.raises(nm.NmError) as e:
+        nm.Mesh((0, 4, 4), (1e-9,) * 3, terms=1, Ms=1.0, A=1.0, Ku=0.0)
+    assert e.value.status == nm.NM_EINVAL
+    # exchange-only meshes accept any size
+    mesh = nm.Mesh((5, 7, 3), (1e-9,) * 3, dtype=torch.float64, terms=1, Ms=8e5, A=1.3e-11, Ku=0.0)
+    m = torch.zeros(mesh.node_shape_abi, dtype=torch.float64, device="cuda:0")
+    m[0] = 1.0
+    assert float(mesh.nm_heff(0.0, m).abs().max()) == 0.0   # uniform m: exchange field vanishes
+    assert mesh.nm_launch_count() > 0

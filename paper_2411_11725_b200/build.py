@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnm.so")
-CU = ["nm_api.cu", "nm_local.cu", "nm_demag.cu", "nm_tensor.cu"]
+CU = ["nm_api.cu", "nm_local.cu", "nm_demag.cu", "nm_demag_fast.cu", "nm_tensor.cu"]
 CPP = ["nm_newell_host.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
@@ -58,7 +58,7 @@ def build(force=False, verbose=False):
         if p.wait() != 0:
             raise RuntimeError("build failed: " + " ".join(cmd))
     tmp = LIB + ".%d.tmp" % os.getpid()
-    cmd = [_nvcc(), "-shared", "-o", tmp] + objs + ["-lquadmath", "-lpthread", "-lcudart"]
+    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs + ["-lquadmath", "-lpthread", "-lcudart"]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

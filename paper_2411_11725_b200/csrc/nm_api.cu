@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -154,13 +155,19 @@ size_t carve(nm_mesh *m, char *base)
     m->Uc[1] = c.take(g.cells * e);
     m->Hc1 = m->Hc2 = nullptr;
     m->Nreal = nullptr;
+    m->fast.Tn = m->fast.wPx = nullptr;
     m->Nhat = m->tw_x = m->tw_x2 = m->tw_y = m->tw_z = m->bufA = m->bufB = nullptr;
     m->kmap_x = m->pos_x = m->kmap_y = m->pos_y = m->kmap_z = m->pos_z = nullptr;
     if (demag) {
         m->Hc1 = c.take(3 * g.cells * e);
         m->Hc2 = c.take(3 * g.cells * e);
         m->Nreal = (double *)c.take(6 * g.cells * sizeof(double));
-        m->Nhat = c.take((size_t)6 * g.K3 * g.K2 * g.C1p * e);
+        if (m->fast.on) {
+            m->fast.Tn = c.take(nm_fast_tensor_elems(g, m->fast) * e);
+            m->fast.wPx = c.take((size_t)g.P1 * cx);
+        } else {
+            m->Nhat = c.take((size_t)6 * g.K3 * g.K2 * g.C1p * e);
+        }
         m->tw_x = c.take((size_t)g.Lx * cx);
         m->tw_x2 = c.take((size_t)g.C1 * cx);
         m->tw_y = c.take((size_t)g.P2 * cx);
@@ -171,8 +178,13 @@ size_t carve(nm_mesh *m, char *base)
         m->pos_y = (int *)c.take(g.P2 * sizeof(int));
         m->kmap_z = (int *)c.take(g.P3 * sizeof(int));
         m->pos_z = (int *)c.take(g.P3 * sizeof(int));
-        m->bufA = c.take((size_t)3 * g.N3 * g.N2 * g.C1p * cx);
-        if (g.N3 > 1) m->bufB = c.take((size_t)3 * g.N3 * g.P2 * g.C1p * cx);
+        if (m->fast.on) {
+            m->bufA = c.take(nm_fast_bufA_elems(g, m->fast) * cx);
+            m->bufB = c.take(nm_fast_bufB_elems(g, m->fast) * cx);
+        } else {
+            m->bufA = c.take((size_t)3 * g.N3 * g.N2 * g.C1p * cx);
+            if (g.N3 > 1) m->bufB = c.take((size_t)3 * g.N3 * g.P2 * g.C1p * cx);
+        }
     }
     return (c.off + 255) & ~(size_t)255;
 }
@@ -188,6 +200,13 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
     m->prof_on = false;
     m->prof_n = 0;
     m->prof_ev_made = 0;
+    nm_fast_plan(d, m->g, &m->fast);
+    {
+        const char *env = getenv("NM_DEMAG_PATH");      // "generic" forces the general-size kernels
+        if (env && strcmp(env, "generic") == 0) m->fast.on = false;
+        const char *ch = getenv("NM_KT_CHUNK");
+        m->fast.kt_chunk = ch ? atoi(ch) : 0;
+    }
     make_plan(m->g.Lx, &m->plan_x);
     make_plan(m->g.P2, &m->plan_y);
     make_plan(m->g.P3, &m->plan_z);
@@ -256,6 +275,7 @@ template <typename T> nm_status setup_tables(nm_mesh *m, cudaStream_t st)
     NM_TRY(upload_twiddles<T>(m->tw_x2, g.P1, g.C1, st));
     NM_TRY(upload_twiddles<T>(m->tw_y, g.P2, g.P2, st));
     NM_TRY(upload_twiddles<T>(m->tw_z, g.P3, g.P3, st));
+    if (m->fast.on) NM_TRY(upload_twiddles<T>(m->fast.wPx, g.P1, g.P1, st));
     std::vector<int> km, ps;
     make_maps(m->plan_x, km, ps);
     NM_TRY(upload_ints(m->kmap_x, km, st));

@@ -271,6 +271,7 @@ static const size_t kSmemCap = 200 * 1024;
 template <typename T>
 nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
 {
+    if (mesh->fast.on) return nm_demag_conv_fast<T>(mesh, fld, Hc_out, st);
     typedef typename Cx<T>::V V;
     const NmGeom &g = mesh->g;
     V *A = (V *)mesh->bufA, *B = (V *)mesh->bufB;

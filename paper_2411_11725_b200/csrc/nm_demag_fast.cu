@@ -1,0 +1,526 @@
+// Fast demagnetisation path: a1-a4 of the hot path for grids with N_d = 16 M_d, M_d in {1,2,4,8,16}
+// (DESIGN.md "Fast demag path").  Same mathematics as nm_demag.cu (reading C5):
+//   M_c = Ms_c (1/8) sum_i m_{c+i},   H_c = - sum_c' N(c - c') M_c',   P_d = 2 N_d,
+// organised for B200:
+//   * every transform is the register-resident radix-16 x radix-M kernel of nm_fft16.cuh; padded
+//     transforms never touch their zero half,
+//   * the x transform packs two real cell rows (c2, c2+1) into one complex line,
+//   * spectra live in k1-blocked layouts (8 complex = 64 B per row) so that every pass moves
+//     contiguous blocks:  A[kt][comp][c3][c2][8],  B[kt][ky][comp][c3][8],
+//     with the 8 columns of a row XOR-swizzled by the row index of the *consuming* pass
+//     (slot = k1 ^ (row & 7)) so that its strided shared-memory reads are conflict-free,
+//   * the tensor is stored as T[kt][|ky|][6][k1][|kz|] and read coalesced along kz.
+// Passes: k_fx_fwd (avg * Ms, x R2C) -> k_fy_fwd -> k_fz_mid (z fwd, H^ = -N^ M^, z inv) ->
+// k_fy_inv -> k_fx_inv (C2R, crop) -> Hc[3][N3][N2][N1] for the node kernel.
+#include "nm_fft16.cuh"
+#include "nm_internal.h"
+
+using namespace nmf;
+
+namespace {
+
+constexpr int kWarps = 8;
+constexpr int kThreadsF = 32 * kWarps;
+constexpr int TW = 8;   // complex columns (k1) per blocked row
+
+template <typename V> __device__ __forceinline__ void copy_in(V *dst, const V *__restrict__ src, int n)
+{
+    // n complex elements, both 16-byte aligned, n even
+    const int4 *s4 = reinterpret_cast<const int4 *>(src);
+    int4 *d4 = reinterpret_cast<int4 *>(dst);
+    const int n4 = n * (int)sizeof(V) / 16;
+    for (int i = threadIdx.x; i < n4; i += blockDim.x) d4[i] = s4[i];
+}
+
+// -------------------------------------------------------------------------------------------------
+// y forward.  CTA = LT consecutive c3 of one (kt, comp); 8 warps x LT lines.
+//   in : A[kt][comp][c3][c2][8]           (rows swizzled by c2)
+//   out: B[kt][ky][comp][c3][8]           (rows swizzled by c3), ky natural 0..P2-1
+template <typename T, int M>
+__global__ void __launch_bounds__(kThreadsF)
+k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict__ B, int N3, int kt0,
+         const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    constexpr int OUT_PITCH = LT * TW + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V *s_io = reinterpret_cast<V *>(smem_raw);              // in: LT*N*8, out: P*OUT_PITCH
+    V *s_scr = s_io + P * OUT_PITCH;                        // 2*kWarps teams
+    const int c3_0 = blockIdx.x * LT;
+    const int comp = blockIdx.y;
+    const int kt = kt0 + blockIdx.z;
+    const int ktl = blockIdx.z;                             // B is indexed relative to kt0
+    const V *src = A + ((((long long)kt * 3 + comp) * N3 + c3_0) * N) * TW;
+    copy_in(s_io, src, LT * N * TW);
+    __syncthreads();
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l, sub = line / TW, k1 = line % TW;
+    V tw[16];
+    load_twiddles2<T, M>(tw, wP, j);
+    V a[16];
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+        const int e = j + M * t;
+        V v = s_io[(sub * N + e) * TW + (k1 ^ (e & 7))];
+        if (h) v = cmul(v, wP[e]);
+        a[t] = v;
+    }
+    __syncthreads();   // the input tile is dead; s_io becomes the output tile
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    fft_fwd<T, M>(a, tw, scr, i);
+    const int sl = k1 ^ ((c3_0 + sub) & 7);
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int ky = 2 * slot_freq<M>(j, s) + h;
+        s_io[ky * OUT_PITCH + sub * TW + sl] = a[s];
+    }
+    __syncthreads();
+    // rows of LT*8 complex, one per ky
+    V *dst = B + ((long long)ktl * P * 3 + comp) * N3 * TW + (long long)c3_0 * TW;
+    for (int idx = threadIdx.x; idx < P * LT * TW; idx += blockDim.x) {
+        const int ky = idx / (LT * TW), r = idx % (LT * TW);
+        dst[(long long)ky * 3 * N3 * TW + r] = s_io[ky * OUT_PITCH + r];
+    }
+}
+
+// y inverse, cropped to N2.  in: B (as above), out: A layout (rows swizzled by c2).
+template <typename T, int M>
+__global__ void __launch_bounds__(kThreadsF)
+k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict__ A, int N3, int kt0,
+         const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    constexpr int PITCH = LT * TW + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V *s_io = reinterpret_cast<V *>(smem_raw);              // in: P*PITCH, out: LT*N*8
+    V *s_scr = s_io + P * PITCH;
+    const int c3_0 = blockIdx.x * LT;
+    const int comp = blockIdx.y;
+    const int kt = kt0 + blockIdx.z;
+    const int ktl = blockIdx.z;
+    const V *src = B + ((long long)ktl * P * 3 + comp) * N3 * TW + (long long)c3_0 * TW;
+    for (int idx = threadIdx.x; idx < P * LT * TW; idx += blockDim.x) {
+        const int ky = idx / (LT * TW), r = idx % (LT * TW);
+        s_io[ky * PITCH + r] = src[(long long)ky * 3 * N3 * TW + r];
+    }
+    __syncthreads();
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l, sub = line / TW, k1 = line % TW;
+    V tw[16];
+    load_twiddles2<T, M>(tw, wP, j);
+    V a[16];
+    const int sl = k1 ^ ((c3_0 + sub) & 7);
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int ky = 2 * slot_freq<M>(j, s) + h;
+        a[s] = s_io[ky * PITCH + sub * TW + sl];
+    }
+    __syncthreads();
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    fft_inv<T, M>(a, tw, scr, i);
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+        const int e = j + M * t;
+        V v = a[t];
+        if (h) v = cmulc(v, wP[e]);
+        // sum of the even and odd halves: partner lane = lane ^ 1
+        v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
+        v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+        if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ (e & 7))] = v;
+    }
+    __syncthreads();
+    V *dst = A + ((((long long)kt * 3 + comp) * N3 + c3_0) * N) * TW;
+    copy_in(dst, s_io, LT * N * TW);
+}
+
+// -------------------------------------------------------------------------------------------------
+// z forward, tensor multiply, z inverse, in place on B.  CTA = LT consecutive ky of one kt.
+//   Tn[kt][|ky|][6][k1][|kz|] (pitch Kzp), components xx,yy,zz,xy,xz,yz, scaled by 1/(P1 P2 P3);
+//   off-diagonal components are odd in their two axes: sign -1 per folded axis (ky > N2, kz > N3).
+template <typename T, int M>
+__global__ void __launch_bounds__(kThreadsF)
+k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, int kt0, int Kzp,
+         const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V *s_io = reinterpret_cast<V *>(smem_raw);              // LT*3*N*8
+    V *s_scr = s_io + LT * 3 * N * TW;
+    const int P2 = 2 * N2;
+    int ky0;
+    if (LT == 1) {
+        // +ky and -ky in neighbouring CTAs: they read the same folded tensor rows
+        const int it = blockIdx.x;
+        ky0 = (it & 1) ? P2 - ((it + 1) >> 1) : (it >> 1);
+    } else {
+        ky0 = blockIdx.x * LT;
+    }
+    const int ktl = blockIdx.y, kt = kt0 + ktl;
+    V *tile = B + (((long long)ktl * P2 + ky0) * 3 * N) * TW;
+    copy_in(s_io, tile, LT * 3 * N * TW);
+    __syncthreads();
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l, sub = line / TW, k1 = line % TW;
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V tw[16];
+    load_twiddles2<T, M>(tw, wP, j);
+    V a[3][16];
+    V *my = s_io + (sub * 3) * N * TW;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            const int e = j + M * t;
+            V v = my[(c * N + e) * TW + (k1 ^ (e & 7))];
+            if (h) v = cmul(v, wP[e]);
+            a[c][t] = v;
+        }
+        fft_fwd<T, M>(a[c], tw, scr, i);
+    }
+    // H^ = -N^ M^
+    const int ky = ky0 + sub;
+    const int kyf = ky <= N2 ? ky : P2 - ky;
+    const T sy = ky <= N2 ? (T)1 : (T)-1;
+    const long long cstride = (long long)TW * Kzp;
+    const T *trow = Tn + ((((long long)kt * (N2 + 1) + kyf) * 6) * TW + k1) * Kzp;
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int kz = 2 * slot_freq<M>(j, s) + h;
+        const int kzf = kz <= N ? kz : P - kz;
+        const T sz = kz <= N ? (T)1 : (T)-1;
+        const T *tp = trow + kzf;
+        const T nxx = tp[0], nyy = tp[cstride], nzz = tp[2 * cstride];
+        const T nxy = sy * tp[3 * cstride], nxz = sz * tp[4 * cstride], nyz = sy * sz * tp[5 * cstride];
+        const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
+        a[0][s] = mk<T>(-(nxx * mx.x + nxy * my_.x + nxz * mz.x), -(nxx * mx.y + nxy * my_.y + nxz * mz.y));
+        a[1][s] = mk<T>(-(nxy * mx.x + nyy * my_.x + nyz * mz.x), -(nxy * mx.y + nyy * my_.y + nyz * mz.y));
+        a[2][s] = mk<T>(-(nxz * mx.x + nyz * my_.x + nzz * mz.x), -(nxz * mx.y + nyz * my_.y + nzz * mz.y));
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        fft_inv<T, M>(a[c], tw, scr, i);
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            const int e = j + M * t;
+            V v = a[c][t];
+            if (h) v = cmulc(v, wP[e]);
+            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
+            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            if ((t >> 3) == h) my[(c * N + e) * TW + (k1 ^ (e & 7))] = v;
+        }
+    }
+    __syncthreads();
+    copy_in(tile, s_io, LT * 3 * N * TW);
+}
+
+// -------------------------------------------------------------------------------------------------
+// x forward: node -> cell average times Ms (a1), two real cell rows (c2, c2+1) per complex line,
+// padded transform, untangle, blocked store.  CTA = R = 2 LT W cell rows of one c3, all components.
+template <typename T, int M>
+__global__ void __launch_bounds__(kThreadsF)
+k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V *__restrict__ A, NmGeom g,
+         int NKT, const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    const int W = blockDim.x >> 5;
+    const int R = 2 * LT * W;
+    constexpr int CP = N + 1;                               // cell row pitch (reals)
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V *s_z = reinterpret_cast<V *>(smem_raw);               // W*LT lines x P
+    V *s_scr = s_z + W * LT * P;                            // 2 W teams
+    T *s_cell = reinterpret_cast<T *>(s_scr + 2 * W * Team<M>::SCRATCH);   // R x CP
+    const int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l;
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V tw[16];
+    load_twiddles2<T, M>(tw, wP, j);
+    const long long plane = (long long)g.n1 * g.n2;
+    for (int comp = 0; comp < 3; ++comp) {
+        // a1: M_c = Ms_c (1/8) sum of the 8 vertices
+        const T *base = fld + (long long)comp * g.nodes + (long long)c3 * plane;
+        for (int idx = threadIdx.x; idx < R * N; idx += blockDim.x) {
+            const int r = idx / N, c1 = idx % N;
+            const int c2 = r0 + r;
+            const T *p = base + (long long)c2 * g.n1 + c1;
+            const T sum = ((p[0] + p[1]) + (p[g.n1] + p[g.n1 + 1])) +
+                          ((p[plane] + p[plane + 1]) + (p[plane + g.n1] + p[plane + g.n1 + 1]));
+            s_cell[r * CP + c1] = Ms[((long long)c3 * g.N2 + c2) * g.N1 + c1] * (T)0.125 * sum;
+        }
+        __syncthreads();
+        V a[16];
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            const int e = j + M * t;
+            V v = mk<T>(s_cell[(2 * line) * CP + e], s_cell[(2 * line + 1) * CP + e]);
+            if (h) v = cmul(v, wP[e]);
+            a[t] = v;
+        }
+        fft_fwd<T, M>(a, tw, scr, i);
+#pragma unroll
+        for (int s = 0; s < 16; ++s) s_z[line * P + 2 * slot_freq<M>(j, s) + h] = a[s];
+        __syncthreads();
+        // untangle the two real rows of each line and store blocked, swizzled by c2
+        for (int idx = threadIdx.x; idx < NKT * R * TW; idx += blockDim.x) {
+            const int kt = idx / (R * TW), rem = idx % (R * TW);
+            const int r = rem / TW, slot = rem % TW;
+            const int c2 = r0 + r;
+            const int k = kt * TW + (slot ^ (c2 & 7));
+            V out = mk<T>((T)0, (T)0);
+            if (k <= N) {
+                const V zk = s_z[(r >> 1) * P + k];
+                const V zm = s_z[(r >> 1) * P + ((P - k) & (P - 1))];
+                if (r & 1) out = mk<T>((T)0.5 * (zk.y + zm.y), (T)-0.5 * (zk.x - zm.x));
+                else out = mk<T>((T)0.5 * (zk.x + zm.x), (T)0.5 * (zk.y - zm.y));
+            }
+            A[((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW + rem] = out;
+        }
+        __syncthreads();
+    }
+}
+
+// x inverse: rebuild the packed spectrum of two real rows from their half spectra, inverse
+// transform cropped to N1, write the cell field Hc[comp][c3][c2][c1].
+template <typename T, int M>
+__global__ void __launch_bounds__(kThreadsF)
+k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, int NKT,
+         const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    const int W = blockDim.x >> 5;
+    const int R = 2 * LT * W;
+    const int XP = NKT * TW + 1;                            // row pitch of s_x (complex)
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V *s_x = reinterpret_cast<V *>(smem_raw);               // R x XP
+    V *s_scr = s_x + R * XP;
+    const int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l;
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V tw[16];
+    load_twiddles2<T, M>(tw, wP, j);
+    for (int comp = 0; comp < 3; ++comp) {
+        for (int idx = threadIdx.x; idx < NKT * R * TW; idx += blockDim.x) {
+            const int kt = idx / (R * TW), rem = idx % (R * TW);
+            const int r = rem / TW, slot = rem % TW;
+            const int c2 = r0 + r;
+            s_x[r * XP + kt * TW + (slot ^ (c2 & 7))] =
+                A[((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW + rem];
+        }
+        __syncthreads();
+        V a[16];
+        const V *xa = s_x + (2 * line) * XP, *xb = xa + XP;
+#pragma unroll
+        for (int s = 0; s < 16; ++s) {
+            const int k = 2 * slot_freq<M>(j, s) + h;
+            if (k <= N) {
+                const V u = xa[k], v = xb[k];
+                a[s] = mk<T>(u.x - v.y, u.y + v.x);          // Xa + i Xb
+            } else {
+                const V u = xa[P - k], v = xb[P - k];
+                a[s] = mk<T>(u.x + v.y, v.x - u.y);          // conj(Xa) + i conj(Xb)
+            }
+        }
+        fft_inv<T, M>(a, tw, scr, i);
+        T *ha = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0 + 2 * line) * g.N1;
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            const int e = j + M * t;
+            V v = a[t];
+            if (h) v = cmulc(v, wP[e]);
+            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
+            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            if ((t >> 3) == h) {
+                ha[e] = v.x;
+                ha[g.N1 + e] = v.y;
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <typename K> nm_status set_smem_f(K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024)
+        NM_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return NM_OK;
+}
+
+template <typename T> size_t scratch_bytes(int warps)
+{
+    return (size_t)2 * warps * 272 * sizeof(typename VT<T>::V);
+}
+
+// ---- per-axis launchers (M is a template parameter of the kernels) ----
+template <typename T, int M>
+nm_status launch_x(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_t st)
+{
+    typedef typename VT<T>::V V;
+    const NmGeom &g = mesh->g;
+    const NmFast &f = mesh->fast;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    const int W = f.Wx, R = 2 * LT * W;
+    const dim3 grid(g.N2 / R, g.N3);
+    if (!inverse) {
+        const size_t sm = (size_t)W * LT * P * sizeof(V) + scratch_bytes<T>(W) + (size_t)R * (N + 1) * sizeof(T);
+        NM_TRY(set_smem_f(k_fx_fwd<T, M>, sm));
+        NmLaunchScope sc(mesh, NM_K_X_FWD, st);
+        k_fx_fwd<T, M><<<grid, 32 * W, sm, st>>>(fld, (const T *)mesh->Ms, (V *)mesh->bufA, g, f.NKT,
+                                                 (const V *)f.wPx);
+    } else {
+        const size_t sm = (size_t)R * (f.NKT * TW + 1) * sizeof(V) + scratch_bytes<T>(W);
+        NM_TRY(set_smem_f(k_fx_inv<T, M>, sm));
+        NmLaunchScope sc(mesh, NM_K_X_INV, st);
+        k_fx_inv<T, M><<<grid, 32 * W, sm, st>>>((const V *)mesh->bufA, Hc, g, f.NKT, (const V *)f.wPx);
+    }
+    return NM_OK;
+}
+
+template <typename T, int M>
+nm_status launch_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st)
+{
+    typedef typename VT<T>::V V;
+    const NmGeom &g = mesh->g;
+    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    const size_t sm = (size_t)P * (LT * TW + 1) * sizeof(V) + scratch_bytes<T>(kWarps);
+    const dim3 grid(g.N3 / LT, 3, nkt);
+    if (!inverse) {
+        NM_TRY(set_smem_f(k_fy_fwd<T, M>, sm));
+        NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
+        k_fy_fwd<T, M><<<grid, kThreadsF, sm, st>>>((const V *)mesh->bufA, (V *)mesh->bufB, g.N3, kt0,
+                                                    (const V *)mesh->tw_y);
+    } else {
+        NM_TRY(set_smem_f(k_fy_inv<T, M>, sm));
+        NmLaunchScope sc(mesh, NM_K_Y_INV, st);
+        k_fy_inv<T, M><<<grid, kThreadsF, sm, st>>>((const V *)mesh->bufB, (V *)mesh->bufA, g.N3, kt0,
+                                                    (const V *)mesh->tw_y);
+    }
+    return NM_OK;
+}
+
+template <typename T, int M>
+nm_status launch_z(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
+{
+    typedef typename VT<T>::V V;
+    const NmGeom &g = mesh->g;
+    constexpr int N = 16 * M, LT = 16 / M;
+    const size_t sm = (size_t)LT * 3 * N * TW * sizeof(V) + scratch_bytes<T>(kWarps);
+    NM_TRY(set_smem_f(k_fz_mid<T, M>, sm));
+    const dim3 grid(g.P2 / LT, nkt);
+    NmLaunchScope sc(mesh, NM_K_MID, st);
+    k_fz_mid<T, M><<<grid, kThreadsF, sm, st>>>((V *)mesh->bufB, (const T *)mesh->fast.Tn, g.N2, kt0,
+                                                mesh->fast.Kzp, (const V *)mesh->tw_z);
+    return NM_OK;
+}
+
+#define NM_SWITCH_M(Mv, CALL)                                                                          \
+    switch (Mv) {                                                                                      \
+    case 1: { constexpr int MM = 1; NM_TRY(CALL); } break;                                             \
+    case 2: { constexpr int MM = 2; NM_TRY(CALL); } break;                                             \
+    case 4: { constexpr int MM = 4; NM_TRY(CALL); } break;                                             \
+    case 8: { constexpr int MM = 8; NM_TRY(CALL); } break;                                             \
+    default: { constexpr int MM = 16; NM_TRY(CALL); } break;                                           \
+    }
+
+// tensor in the fast layout from the folded fp64 octant in[6][K3][K2][K1]
+template <typename T>
+__global__ void k_tensor_store_fast(const double *__restrict__ in, T *__restrict__ Tn, int K1, int K2,
+                                    int K3, int NKT, int Kzp, double scale)
+{
+    const long long total = (long long)NKT * K2 * 6 * TW * Kzp;
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total) return;
+    long long r = idx;
+    const int kz = (int)(r % Kzp); r /= Kzp;
+    const int k1 = (int)(r % TW); r /= TW;
+    const int a = (int)(r % 6); r /= 6;
+    const int ky = (int)(r % K2);
+    const int kt = (int)(r / K2);
+    const int kx = kt * TW + k1;
+    double v = 0.0;
+    if (kx < K1 && kz < K3) {
+        v = in[(((long long)a * K3 + kz) * K2 + ky) * K1 + kx] * scale;
+        if (a >= 3) v = -v;   // (-i)^2 from the two odd axes
+    }
+    Tn[idx] = (T)v;
+}
+
+} // namespace
+
+// Which grids the fast path serves, and its sizes.  Host only.
+void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
+{
+    f->on = false;
+    if (!(d->terms & NM_TERM_DEMAG)) return;
+    int M[3];
+    const int N[3] = {g.N1, g.N2, g.N3};
+    for (int a = 0; a < 3; ++a) {
+        if (N[a] != 16 && N[a] != 32 && N[a] != 64 && N[a] != 128 && N[a] != 256) return;
+        M[a] = N[a] / 16;
+    }
+    const int LTx = 16 / M[0];
+    int W = kWarps;
+    while (W >= 1 && (g.N2 % (2 * LTx * W)) != 0) W >>= 1;
+    if (W < 1) return;
+    f->M1 = M[0]; f->M2 = M[1]; f->M3 = M[2];
+    f->Wx = W;
+    f->NKT = (g.C1 + TW - 1) / TW;
+    f->Kzp = (g.N3 + 1 + 3) & ~3;
+    f->on = true;
+}
+
+size_t nm_fast_tensor_elems(const NmGeom &g, const NmFast &f)
+{
+    return (size_t)f.NKT * (g.N2 + 1) * 6 * TW * f.Kzp;
+}
+size_t nm_fast_bufA_elems(const NmGeom &g, const NmFast &f) { return (size_t)f.NKT * 3 * g.N3 * g.N2 * TW; }
+size_t nm_fast_bufB_elems(const NmGeom &g, const NmFast &f) { return (size_t)f.NKT * g.P2 * 3 * g.N3 * TW; }
+
+nm_status nm_fast_store_tensor(nm_mesh *mesh, const double *octant, double scale, cudaStream_t st)
+{
+    const NmGeom &g = mesh->g;
+    const NmFast &f = mesh->fast;
+    const long long total = (long long)nm_fast_tensor_elems(g, f);
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    if (mesh->f64)
+        k_tensor_store_fast<double><<<blocks, 256, 0, st>>>(octant, (double *)f.Tn, g.C1, g.K2, g.K3, f.NKT, f.Kzp, scale);
+    else
+        k_tensor_store_fast<float><<<blocks, 256, 0, st>>>(octant, (float *)f.Tn, g.C1, g.K2, g.K3, f.NKT, f.Kzp, scale);
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+template <typename T>
+nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
+{
+    const NmFast &f = mesh->fast;
+    NM_SWITCH_M(f.M1, (launch_x<T, MM>(mesh, false, fld, Hc_out, st)));
+    const int chunk = f.kt_chunk > 0 && f.kt_chunk < f.NKT ? f.kt_chunk : f.NKT;
+    for (int kt0 = 0; kt0 < f.NKT; kt0 += chunk) {
+        const int nkt = kt0 + chunk <= f.NKT ? chunk : f.NKT - kt0;
+        NM_SWITCH_M(f.M2, (launch_y<T, MM>(mesh, false, kt0, nkt, st)));
+        NM_SWITCH_M(f.M3, (launch_z<T, MM>(mesh, kt0, nkt, st)));
+        NM_SWITCH_M(f.M2, (launch_y<T, MM>(mesh, true, kt0, nkt, st)));
+    }
+    NM_SWITCH_M(f.M1, (launch_x<T, MM>(mesh, true, fld, Hc_out, st)));
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+template nm_status nm_demag_conv_fast<float>(nm_mesh *, const float *, float *, cudaStream_t);
+template nm_status nm_demag_conv_fast<double>(nm_mesh *, const double *, double *, cudaStream_t);

@@ -1,0 +1,295 @@
+// Register-resident FFT core of the fast demag path (device code).
+//
+// a2/a4 of the hot path: zero-padded transforms of the demag convolution
+// (PAPER.md:175-181).  A padded transform of length P = 2N whose upper input half is zero splits
+// exactly into two N-point transforms,
+//     X[2k]   = FFT_N(x)[k],            X[2k+1] = FFT_N(x[n] w_P^n)[k],         w_P = exp(-2 pi i/P)
+// and the cropped inverse into
+//     y[n]    = IFFT_N(X_even)[n] + conj(w_P^n) IFFT_N(X_odd)[n],   n < N,
+// so no thread ever touches the zero half.  N = 16 M, M in {1,2,4,8,16}.  A *team* of 16 threads
+// holds 16 complex values each and transforms 16/M lines at once:
+//     stage 1   radix-16 butterfly over the register index t (elements j + M t of a line)
+//     twiddle   w_N^(j t')
+//     exchange  through a team-private, conflict-free shared-memory scratch (warp-synchronous)
+//     stage 2   radix-M butterflies
+// The spectrum stays in the scrambled register order stage 2 leaves it in (slot_freq below); the
+// inverse runs the same steps backwards, so no reordering pass exists.  Two teams share a warp:
+// lane = 2 i + h, team h = 0 takes the even outputs, h = 1 the odd ones.
+#pragma once
+
+#include "nm_internal.h"
+
+namespace nmf {
+
+template <typename T> struct VT { typedef typename NmVec2<T>::type V; };
+
+template <typename T> __device__ __forceinline__ typename VT<T>::V mk(T a, T b)
+{
+    typename VT<T>::V v;
+    v.x = a;
+    v.y = b;
+    return v;
+}
+template <typename V> __device__ __forceinline__ V cadd(V a, V b) { a.x += b.x; a.y += b.y; return a; }
+template <typename V> __device__ __forceinline__ V csub(V a, V b) { a.x -= b.x; a.y -= b.y; return a; }
+template <typename V> __device__ __forceinline__ V cmul(V a, V b)
+{
+    V r;
+    r.x = a.x * b.x - a.y * b.y;
+    r.y = a.x * b.y + a.y * b.x;
+    return r;
+}
+template <typename V> __device__ __forceinline__ V cmulc(V a, V b)   // a * conj(b)
+{
+    V r;
+    r.x = a.x * b.x + a.y * b.y;
+    r.y = a.y * b.x - a.x * b.y;
+    return r;
+}
+// a * w (INV = false) or a * conj(w) (INV = true)
+template <bool INV, typename V> __device__ __forceinline__ V ctw(V a, V w)
+{
+    return INV ? cmulc(a, w) : cmul(a, w);
+}
+// multiply by -i (forward) / +i (inverse)
+template <bool INV, typename V> __device__ __forceinline__ V rot90(V a)
+{
+    V r;
+    if (INV) { r.x = -a.y; r.y = a.x; }
+    else { r.x = a.y; r.y = -a.x; }
+    return r;
+}
+
+// 4-point DFT, natural order in and out; sign -1 (forward) or +1 (INV).
+template <bool INV, typename V> __device__ __forceinline__ void dft4(V &a0, V &a1, V &a2, V &a3)
+{
+    const V s02 = cadd(a0, a2), d02 = csub(a0, a2);
+    const V s13 = cadd(a1, a3), d13 = rot90<INV>(csub(a1, a3));
+    a0 = cadd(s02, s13);
+    a2 = csub(s02, s13);
+    a1 = cadd(d02, d13);
+    a3 = csub(d02, d13);
+}
+
+template <typename V> __device__ __forceinline__ void dft2(V &a0, V &a1)
+{
+    const V s = cadd(a0, a1), d = csub(a0, a1);
+    a0 = s;
+    a1 = d;
+}
+
+// exp(-+ 2 pi i q/16) as compile-time constants
+template <typename T, bool INV, int Q> __device__ __forceinline__ typename VT<T>::V mul_w16(typename VT<T>::V a)
+{
+    typedef typename VT<T>::V V;
+    constexpr int q = ((Q % 16) + 16) % 16;
+    const T c1 = (T)0.92387953251128675612818318939679;   // cos(pi/8)
+    const T s1 = (T)0.38268343236508977172845998403040;   // sin(pi/8)
+    const T h = (T)0.70710678118654752440084436210485;
+    if (q == 0) return a;
+    if (q == 4) return rot90<INV>(a);
+    if (q == 8) return mk<T>(-a.x, -a.y);
+    if (q == 12) return rot90<!INV>(a);
+    if (q == 2) {   // h (1 -+ i)
+        return INV ? mk<T>(h * (a.x - a.y), h * (a.x + a.y)) : mk<T>(h * (a.x + a.y), h * (a.y - a.x));
+    }
+    if (q == 6) {   // h (-1 -+ i)
+        return INV ? mk<T>(-h * (a.x + a.y), h * (a.x - a.y)) : mk<T>(h * (a.y - a.x), -h * (a.x + a.y));
+    }
+    T c, s;   // w = c - i s (forward)
+    if (q == 1) { c = c1; s = s1; }
+    else if (q == 3) { c = s1; s = c1; }
+    else if (q == 5) { c = -s1; s = c1; }
+    else if (q == 7) { c = -c1; s = s1; }
+    else if (q == 9) { c = -c1; s = -s1; }
+    else if (q == 10) { c = -h; s = -h; }
+    else if (q == 11) { c = -s1; s = -c1; }
+    else if (q == 13) { c = s1; s = -c1; }
+    else if (q == 14) { c = h; s = -h; }
+    else { c = c1; s = -s1; }   // 15
+    const V w = mk<T>(c, -s);
+    return ctw<INV>(a, w);
+}
+
+// Position <-> frequency of the in-register butterflies (DIF leaves digit-reversed order).
+__host__ __device__ constexpr int rev16(int p) { return 4 * (p & 3) + (p >> 2); }
+__host__ __device__ constexpr int rev8(int p) { return 4 * (p & 1) + (p >> 1); }
+__host__ __device__ constexpr int revM(int M, int p)
+{
+    return M == 16 ? rev16(p) : M == 8 ? rev8(p) : p;   // dft4 / dft2 / identity are natural
+}
+
+// 16-point DFT.  Forward: natural in, position p holds frequency rev16(p).  Inverse (INV): the
+// exact reverse (input in that order, natural out, unscaled).
+template <typename T, bool INV> __device__ __forceinline__ void dft16(typename VT<T>::V *a)
+{
+    if (!INV) {
+#pragma unroll
+        for (int n1 = 0; n1 < 4; ++n1) dft4<false>(a[n1], a[n1 + 4], a[n1 + 8], a[n1 + 12]);
+        a[5] = mul_w16<T, false, 1>(a[5]);
+        a[9] = mul_w16<T, false, 2>(a[9]);
+        a[13] = mul_w16<T, false, 3>(a[13]);
+        a[6] = mul_w16<T, false, 2>(a[6]);
+        a[10] = mul_w16<T, false, 4>(a[10]);
+        a[14] = mul_w16<T, false, 6>(a[14]);
+        a[7] = mul_w16<T, false, 3>(a[7]);
+        a[11] = mul_w16<T, false, 6>(a[11]);
+        a[15] = mul_w16<T, false, 9>(a[15]);
+#pragma unroll
+        for (int k2 = 0; k2 < 4; ++k2) dft4<false>(a[4 * k2], a[4 * k2 + 1], a[4 * k2 + 2], a[4 * k2 + 3]);
+    } else {
+#pragma unroll
+        for (int k2 = 0; k2 < 4; ++k2) dft4<true>(a[4 * k2], a[4 * k2 + 1], a[4 * k2 + 2], a[4 * k2 + 3]);
+        a[5] = mul_w16<T, true, 1>(a[5]);
+        a[9] = mul_w16<T, true, 2>(a[9]);
+        a[13] = mul_w16<T, true, 3>(a[13]);
+        a[6] = mul_w16<T, true, 2>(a[6]);
+        a[10] = mul_w16<T, true, 4>(a[10]);
+        a[14] = mul_w16<T, true, 6>(a[14]);
+        a[7] = mul_w16<T, true, 3>(a[7]);
+        a[11] = mul_w16<T, true, 6>(a[11]);
+        a[15] = mul_w16<T, true, 9>(a[15]);
+#pragma unroll
+        for (int n1 = 0; n1 < 4; ++n1) dft4<true>(a[n1], a[n1 + 4], a[n1 + 8], a[n1 + 12]);
+    }
+}
+
+// 8-point DFT on a[0..7] with stride 1: forward natural in, position p holds rev8(p).
+template <typename T, bool INV> __device__ __forceinline__ void dft8(typename VT<T>::V *a)
+{
+    if (!INV) {
+        dft4<false>(a[0], a[2], a[4], a[6]);
+        dft4<false>(a[1], a[3], a[5], a[7]);
+        a[3] = mul_w16<T, false, 2>(a[3]);
+        a[5] = mul_w16<T, false, 4>(a[5]);
+        a[7] = mul_w16<T, false, 6>(a[7]);
+        dft2(a[0], a[1]);
+        dft2(a[2], a[3]);
+        dft2(a[4], a[5]);
+        dft2(a[6], a[7]);
+    } else {
+        dft2(a[0], a[1]);
+        dft2(a[2], a[3]);
+        dft2(a[4], a[5]);
+        dft2(a[6], a[7]);
+        a[3] = mul_w16<T, true, 2>(a[3]);
+        a[5] = mul_w16<T, true, 4>(a[5]);
+        a[7] = mul_w16<T, true, 6>(a[7]);
+        dft4<true>(a[0], a[2], a[4], a[6]);
+        dft4<true>(a[1], a[3], a[5], a[7]);
+    }
+}
+
+// Stage 2: 16/M butterflies of radix M on slots [u*M, u*M + M).
+template <typename T, bool INV, int M> __device__ __forceinline__ void dftM(typename VT<T>::V *a)
+{
+    if (M == 16) dft16<T, INV>(a);
+    else if (M == 8) { dft8<T, INV>(a); dft8<T, INV>(a + 8); }
+    else if (M == 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) dft4<INV>(a[4 * u], a[4 * u + 1], a[4 * u + 2], a[4 * u + 3]);
+    } else if (M == 2) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) dft2(a[2 * u], a[2 * u + 1]);
+    }
+}
+
+// Team geometry for N = 16 M.  Thread i of the team (0..15): stage 1 works on line l1 = i / M with
+// elements j + M t (j = i % M); stage 2 on line l1 again with sub-transforms t' = q U + u (q = i % M).
+template <int M> struct Team {
+    static constexpr int N = 16 * M;
+    static constexpr int U = 16 / M;        // radix-M butterflies per thread in stage 2
+    static constexpr int LINES = 16 / M;    // lines per team
+    static constexpr int SCRATCH = 256 + 16;   // complex elements of exchange scratch per team
+};
+
+// frequency (0..N-1) of the N-point transform held in slot s = u*M + p of team thread with q = i % M
+template <int M> __device__ __forceinline__ int slot_freq(int q, int s)
+{
+    const int u = s / M, p = s % M;
+    return q * (16 / M) + u + 16 * revM(M, p);
+}
+
+__device__ __forceinline__ int skew(int lin) { return lin + (lin >> 4); }
+
+// Twiddles of one team thread: tw[t'] = w_N^(j t') = w_P^(2 j t'), t' = 1..15 (tw[0] unused), from
+// the table wP[q] = exp(-2 pi i q / P), P = 2N = 32 M.
+template <typename T, int M>
+__device__ __forceinline__ void load_twiddles2(typename VT<T>::V *tw, const typename VT<T>::V *__restrict__ wP, int j)
+{
+#pragma unroll
+    for (int t = 1; t < 16; ++t) tw[t] = wP[(2 * j * t) & (32 * M - 1)];
+}
+
+// Forward N-point transform of the team's lines.  a[t] = x[j + M t] on entry (natural), on exit
+// slot s holds frequency slot_freq<M>(q, s).  `scr` = this team's scratch, i = team thread index.
+template <typename T, int M>
+__device__ __forceinline__ void fft_fwd(typename VT<T>::V *a, const typename VT<T>::V *tw,
+                                        typename VT<T>::V *scr, int i)
+{
+    typedef typename VT<T>::V V;
+    dft16<T, false>(a);
+    if (M == 1) {
+        // positions hold rev16 order; bring to slot order u = t' (U = 16)
+        V b[16];
+#pragma unroll
+        for (int p = 0; p < 16; ++p) b[rev16(p)] = a[p];
+#pragma unroll
+        for (int p = 0; p < 16; ++p) a[p] = b[p];
+        return;
+    }
+    const int l = i / M, j = i % M;
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+        const int tp = rev16(p);
+        V v = a[p];
+        if (tp != 0) v = cmul(v, tw[tp]);
+        scr[skew((l * 16 + tp) * M + j)] = v;
+    }
+    __syncwarp();
+    constexpr int U = 16 / M;
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int u = s / M, jj = s % M;
+        a[s] = scr[skew((l * 16 + j * U + u) * M + jj)];
+    }
+    dftM<T, false, M>(a);
+}
+
+// Inverse: slot order in, a[t] = N * x[j + M t] out (unscaled).
+template <typename T, int M>
+__device__ __forceinline__ void fft_inv(typename VT<T>::V *a, const typename VT<T>::V *tw,
+                                        typename VT<T>::V *scr, int i)
+{
+    typedef typename VT<T>::V V;
+    if (M == 1) {
+        V b[16];
+#pragma unroll
+        for (int p = 0; p < 16; ++p) b[p] = a[rev16(p)];
+#pragma unroll
+        for (int p = 0; p < 16; ++p) a[p] = b[p];
+        dft16<T, true>(a);
+        return;
+    }
+    dftM<T, true, M>(a);
+    const int l = i / M, j = i % M;
+    constexpr int U = 16 / M;
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int u = s / M, jj = s % M;
+        scr[skew((l * 16 + j * U + u) * M + jj)] = a[s];
+    }
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+        const int tp = rev16(p);
+        V v = scr[skew((l * 16 + tp) * M + j)];
+        if (tp != 0) v = cmulc(v, tw[tp]);
+        a[p] = v;
+    }
+    dft16<T, true>(a);
+}
+
+} // namespace nmf

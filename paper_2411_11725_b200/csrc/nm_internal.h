@@ -47,9 +47,22 @@ struct NmGeom {
     long long cells, nodes;
 };
 
+// Fast demag path (nm_demag_fast.cu): sizes 16 M_d per axis, blocked spectrum layouts.
+struct NmFast {
+    bool on;
+    int M1, M2, M3;    // N_d / 16
+    int Wx;            // warps per CTA of the x passes
+    int NKT;           // k1 tiles of 8 columns
+    int Kzp;           // pitch of the |kz| axis of the tensor
+    int kt_chunk;      // k1 tiles per y/z/y launch group (0 = all)
+    void *Tn;          // tensor [NKT][N2+1][6][8][Kzp] (real)
+    void *wPx;         // exp(-2 pi i q / P1), q < P1
+};
+
 struct nm_mesh {
     nm_mesh_desc desc;
     NmGeom g;
+    NmFast fast;
     bool f64;
     size_t esz;        // sizeof(real)
     int sm_count;
@@ -130,6 +143,14 @@ nm_status nm_build_tensor(nm_mesh *mesh, cudaStream_t st);
 // nm_demag.cu
 template <typename T>
 nm_status nm_demag_conv(nm_mesh *mesh, const T *field_nodes, T *Hc_out, cudaStream_t st);
+// nm_demag_fast.cu
+void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f);
+size_t nm_fast_tensor_elems(const NmGeom &g, const NmFast &f);
+size_t nm_fast_bufA_elems(const NmGeom &g, const NmFast &f);
+size_t nm_fast_bufB_elems(const NmGeom &g, const NmFast &f);
+nm_status nm_fast_store_tensor(nm_mesh *mesh, const double *octant, double scale, cudaStream_t st);
+template <typename T>
+nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *field_nodes, T *Hc_out, cudaStream_t st);
 // nm_local.cu
 nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st);
 

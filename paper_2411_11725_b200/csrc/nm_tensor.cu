@@ -197,7 +197,9 @@ nm_status nm_build_tensor(nm_mesh *mesh, cudaStream_t st)
                                                                    K2 * K1, g.P3, 2);
     const double scale = 1.0 / ((double)g.P1 * g.P2 * g.P3);
     const long long tot = 6LL * K3 * K2 * g.C1p;
-    if (mesh->f64)
+    if (mesh->fast.on) {
+        NM_TRY(nm_fast_store_tensor(mesh, s0, scale, st));
+    } else if (mesh->f64)
         k_tensor_store<double><<<blocks_for(tot, 256), 256, 0, st>>>(s0, (double *)mesh->Nhat,
                                                                     (int)K1, (int)K2, (int)K3,
                                                                     g.C1p, scale);

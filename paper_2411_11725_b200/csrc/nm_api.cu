@@ -137,7 +137,7 @@ size_t carve(nm_mesh *m, char *base)
     m->A = c.take(g.cells * e);
     m->Ku = c.take(g.cells * e);
     m->sMs = c.take(g.nodes * e);
-    m->n_partials = nm_node_blocks(g.nodes);
+    m->n_partials = nm_node_blocks(g);
     m->partials = (double *)c.take(((size_t)m->n_partials + 1) * sizeof(double));
     // Runge-Kutta / adjoint scratch; doubles as fp64 scratch of the tensor setup
     const size_t vec = (size_t)3 * g.nodes * e;

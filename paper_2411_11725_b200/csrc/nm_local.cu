@@ -50,51 +50,55 @@ __device__ __forceinline__ double block_sum(double v)
     return r;   // valid in thread 0
 }
 
-template <typename T>
+// EXTRA = false: exchange + demag + uniform Zeeman only (no anisotropy, no nodal Zeeman arrays).
+// Grid: x = blocks of kBlock nodes of one z plane (flattened i2*n1 + i1), y = i3.
+// A neighbour or cell that does not exist is read at a clamped (valid) address and only ever
+// multiplied by a zero coefficient, so the kernel has no per-neighbour branches.
+template <typename T, bool EXTRA>
 __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
 {
     const NmGeom &g = a.g;
-    const long long n = (long long)blockIdx.x * kBlock + threadIdx.x;
-    const bool live = n < g.nodes;
+    const int pl = g.n1 * g.n2;
+    const int p = blockIdx.x * kBlock + threadIdx.x;
+    const int i3 = blockIdx.y;
+    const bool live = p < pl;
     double err2 = 0.0;
     if (live) {
-        const int i1 = (int)(n % g.n1);
-        const int i2 = (int)((n / g.n1) % g.n2);
-        const int i3 = (int)(n / ((long long)g.n1 * g.n2));
+        const int i2 = p / g.n1, i1 = p - i2 * g.n1;
         const long long nn = g.nodes;
-
-        // the 8 adjacent cells: 2A, 2Ku, Ms (0 where the cell does not exist) and sum Ms Hcell
+        const long long n = (long long)i3 * pl + p;
+        const int ox[3] = {i1 > 0 ? -1 : 0, 0, i1 < g.N1 ? 1 : 0};
+        const int oy[3] = {i2 > 0 ? -g.n1 : 0, 0, i2 < g.N2 ? g.n1 : 0};
+        const int oz[3] = {i3 > 0 ? -pl : 0, 0, i3 < g.N3 ? pl : 0};
+        // the 8 adjacent cells (bit 0: x, 1: y, 2: z; 0 = lower side)
+        const bool vx[2] = {i1 > 0, i1 < g.N1}, vy[2] = {i2 > 0, i2 < g.N2}, vz[2] = {i3 > 0, i3 < g.N3};
+        const int cx[2] = {i1 > 0 ? i1 - 1 : 0, i1 < g.N1 ? i1 : g.N1 - 1};
+        const int cy[2] = {i2 > 0 ? i2 - 1 : 0, i2 < g.N2 ? i2 : g.N2 - 1};
+        const int cz[2] = {i3 > 0 ? i3 - 1 : 0, i3 < g.N3 ? i3 : g.N3 - 1};
+        const bool ex_on = (a.terms & NM_TERM_EXCHANGE) != 0;
         T cA[8], cK[8], cM[8];
         T hd[3] = {0, 0, 0};
         T sms = 0;
 #pragma unroll
-        for (int oz = 0; oz < 2; ++oz)
-#pragma unroll
-            for (int oy = 0; oy < 2; ++oy)
-#pragma unroll
-                for (int ox = 0; ox < 2; ++ox) {
-                    const int c1 = i1 + ox - 1, c2 = i2 + oy - 1, c3 = i3 + oz - 1;
-                    const int ci = ox + 2 * oy + 4 * oz;
-                    const bool ok = c1 >= 0 && c1 < g.N1 && c2 >= 0 && c2 < g.N2 && c3 >= 0 && c3 < g.N3;
-                    T ms = 0, aa = 0, kk = 0;
-                    if (ok) {
-                        const long long c = ((long long)c3 * g.N2 + c2) * g.N1 + c1;
-                        ms = a.Ms[c];
-                        if (a.terms & NM_TERM_EXCHANGE) aa = (T)2 * a.A[c];
-                        if (a.terms & NM_TERM_ANISO) kk = (T)2 * a.Ku[c];
-                        if (a.Hc) {
-                            hd[0] += ms * a.Hc[c];
-                            hd[1] += ms * a.Hc[g.cells + c];
-                            hd[2] += ms * a.Hc[2 * g.cells + c];
-                        }
-                    }
-                    cM[ci] = ms; cA[ci] = aa; cK[ci] = kk;
-                    sms += ms;
-                }
-
-        const T mc[3] = {a.fld[n], a.fld[nn + n], a.fld[2 * nn + n]};
+        for (int ci = 0; ci < 8; ++ci) {
+            const int bx = ci & 1, by = (ci >> 1) & 1, bz = ci >> 2;
+            const long long c = ((long long)cz[bz] * g.N2 + cy[by]) * g.N1 + cx[bx];
+            const bool ok = vx[bx] && vy[by] && vz[bz];
+            const T ms = ok ? a.Ms[c] : (T)0;
+            cM[ci] = ms;
+            cA[ci] = (ok && ex_on) ? (T)2 * a.A[c] : (T)0;
+            if (EXTRA) cK[ci] = (ok && (a.terms & NM_TERM_ANISO)) ? (T)2 * a.Ku[c] : (T)0;
+            if (a.Hc) {
+                hd[0] += ms * a.Hc[c];
+                hd[1] += ms * a.Hc[g.cells + c];
+                hd[2] += ms * a.Hc[2 * g.cells + c];
+            }
+            sms += ms;
+        }
+        const T *f0 = a.fld + n, *f1 = f0 + nn, *f2 = f1 + nn;
+        const T mc[3] = {f0[0], f1[0], f2[0]};
         const bool zee_on = (a.terms & NM_TERM_ZEEMAN) != 0;
-        const bool zee_nodal = zee_on && (a.h_static || a.h_pulse);
+        const bool zee_nodal = EXTRA && zee_on && (a.h_static || a.h_pulse);
         T ex[3] = {0, 0, 0}, ze[3] = {0, 0, 0};
         T an = 0;
 #pragma unroll
@@ -104,45 +108,41 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
 #pragma unroll
                 for (int dx = -1; dx <= 1; ++dx) {
                     const int e = (dx != 0) | ((dy != 0) << 1) | ((dz != 0) << 2);
+                    if (e == 0 && !EXTRA) continue;
                     // cells that contain both n and n + delta
                     T sA = 0, sK = 0, sM = 0;
 #pragma unroll
-                    for (int oz = 0; oz < 2; ++oz)
-#pragma unroll
-                        for (int oy = 0; oy < 2; ++oy)
-#pragma unroll
-                            for (int ox = 0; ox < 2; ++ox) {
-                                const bool in = (dx == 0 || ox == (dx + 1) / 2) &&
-                                                (dy == 0 || oy == (dy + 1) / 2) &&
-                                                (dz == 0 || oz == (dz + 1) / 2);
-                                if (in) {
-                                    const int ci = ox + 2 * oy + 4 * oz;
-                                    sA += cA[ci]; sK += cK[ci]; sM += cM[ci];
-                                }
-                            }
-                    const int j1 = i1 + dx, j2 = i2 + dy, j3 = i3 + dz;
-                    const bool inb = j1 >= 0 && j1 < g.n1 && j2 >= 0 && j2 < g.n2 && j3 >= 0 && j3 < g.n3;
-                    if (!inb) continue;
-                    const long long nb = n + dx + (long long)dy * g.n1 + (long long)dz * g.n1 * g.n2;
+                    for (int ci = 0; ci < 8; ++ci) {
+                        const int bx = ci & 1, by = (ci >> 1) & 1, bz = ci >> 2;
+                        const bool in = (dx == 0 || bx == (dx + 1) / 2) && (dy == 0 || by == (dy + 1) / 2) &&
+                                        (dz == 0 || bz == (dz + 1) / 2);
+                        if (in) {
+                            sA += cA[ci];
+                            if (EXTRA) { sK += cK[ci]; sM += cM[ci]; }
+                        }
+                    }
+                    const int off = ox[dx + 1] + oy[dy + 1] + oz[dz + 1];
                     T mb[3];
                     if (e == 0) {
                         mb[0] = mc[0]; mb[1] = mc[1]; mb[2] = mc[2];
                     } else {
-                        mb[0] = a.fld[nb]; mb[1] = a.fld[nn + nb]; mb[2] = a.fld[2 * nn + nb];
+                        mb[0] = f0[off]; mb[1] = f1[off]; mb[2] = f2[off];
                         const T w = a.wK[e] * sA;
                         ex[0] += w * (mb[0] - mc[0]);
                         ex[1] += w * (mb[1] - mc[1]);
                         ex[2] += w * (mb[2] - mc[2]);
                     }
-                    an += a.wM[e] * sK * (mb[0] * a.kax[0] + mb[1] * a.kax[1] + mb[2] * a.kax[2]);
-                    if (zee_nodal) {
-                        const T w = a.wM[e] * sM;
+                    if (EXTRA) {
+                        an += a.wM[e] * sK * (mb[0] * a.kax[0] + mb[1] * a.kax[1] + mb[2] * a.kax[2]);
+                        if (zee_nodal) {
+                            const T w = a.wM[e] * sM;
 #pragma unroll
-                        for (int j = 0; j < 3; ++j) {
-                            T h = 0;
-                            if (a.h_static) h += a.h_static[j * nn + nb];
-                            if (a.h_pulse) h += a.amp * a.h_pulse[j * nn + nb];
-                            ze[j] += w * h;
+                            for (int j = 0; j < 3; ++j) {
+                                T hv = 0;
+                                if (a.h_static) hv += a.h_static[j * nn + n + off];
+                                if (a.h_pulse) hv += a.amp * a.h_pulse[j * nn + n + off];
+                                ze[j] += w * hv;
+                            }
                         }
                     }
                 }
@@ -153,10 +153,10 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
             const T invS = (T)1 / sms;
 #pragma unroll
             for (int j = 0; j < 3; ++j) {
-                T h = (a.kax[j] * an - ex[j]) * invL + hd[j] * invS;
-                if (zee_on) h += a.hu[j];
-                if (zee_nodal) h += a.mu0 * ze[j] * invL;
-                H[j] = h;
+                T hv = (a.kax[j] * an - ex[j]) * invL + hd[j] * invS;
+                if (zee_on) hv += a.hu[j];
+                if (zee_nodal) hv += a.mu0 * ze[j] * invL;
+                H[j] = hv;
             }
         }
 
@@ -185,10 +185,10 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
                     y0[j] = r.y0[j * nn + n];
                     T acc = r.cself * f[j];
                     T ea = r.eself * f[j];
-                    for (int p = 0; p < r.nprev; ++p) {
-                        const T kp = r.kprev[p][j * nn + n];
-                        acc += r.cprev[p] * kp;
-                        ea += r.eprev[p] * kp;
+                    for (int q = 0; q < r.nprev; ++q) {
+                        const T kp = r.kprev[q][j * nn + n];
+                        acc += r.cprev[q] * kp;
+                        ea += r.eprev[q] * kp;
                     }
                     y[j] = y0[j] + r.dt * acc;
                     er[j] = r.dt * ea;
@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
     }
     if (a.mode == NM_MODE_RK && a.rk.want_err) {
         const double s = block_sum(err2);
-        if (threadIdx.x == 0) a.rk.partials[blockIdx.x] = s;
+        if (threadIdx.x == 0) a.rk.partials[blockIdx.y * gridDim.x + blockIdx.x] = s;
     }
 }
 
@@ -374,14 +374,17 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
 {
     {
         NmLaunchScope sc(mesh, NM_K_NODE, st);
-        k_node<T><<<nblk(a.g.nodes, kBlock), kBlock, 0, st>>>(a);
+        const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
+        const bool extra = (a.terms & NM_TERM_ANISO) || ((a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse));
+        if (extra) k_node<T, true><<<grid, kBlock, 0, st>>>(a);
+        else k_node<T, false><<<grid, kBlock, 0, st>>>(a);
     }
 
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;
 }
 
-int nm_node_blocks(long long nodes) { return (int)nblk(nodes, kBlock); }
+int nm_node_blocks(const NmGeom &g) { return (int)(nblk((long long)g.n1 * g.n2, kBlock) * g.n3); }
 
 nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st)
 {

@@ -64,7 +64,7 @@ template <typename T> struct NmAdjCellArgs {
 
 // host launchers defined in nm_local.cu
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st);
-int nm_node_blocks(long long nodes);
+int nm_node_blocks(const NmGeom &g);
 nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st);
 template <typename T>
 nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st);

@@ -206,12 +206,11 @@ def run_b200(args):
     import torch.distributed as dist
 
     from paper_2411_11725_b200 import binding as nm
+    from paper_2411_11725_b200 import replicas
     from paper_2411_11725_b200 import workloads as wl
 
     nm.lib()                                 # fails loudly if libnm.so is missing (no fallback)
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.rank_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -225,7 +224,7 @@ def run_b200(args):
     # seeded synthetic input, config 4's recipe (replica r uses seed 4 + N + r)
     w = wl.config4_sweep(N)
     if rank:
-        w.m0 = wl.random_unit_field(w.node_shape, 4 + N + rank)
+        w.m0 = wl.random_unit_field(w.node_shape, replicas.replica_seed(N, rank))
     m_host = torch.from_numpy(wl.to_abi(w.m0)).to(td).pin_memory()
     a_host = torch.from_numpy(wl.to_abi(
         np.random.default_rng(99 + rank).standard_normal((3,) + w.node_shape))).to(td).pin_memory()
@@ -264,11 +263,7 @@ def run_b200(args):
         return e0.elapsed_time(e1) * 1e-3
 
     def over_ranks(sec):
-        if world > 1:
-            t = torch.tensor([sec], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            return float(t.item())
-        return sec
+        return replicas.max_over_ranks(sec, dev)
 
     for _ in range(args.warmup):
         step()
@@ -286,7 +281,7 @@ def run_b200(args):
     sec_plain = over_ranks(timed(step, args.steps))
 
     cells = N ** 3
-    value = world * EVALS_PER_STEP * cells * args.steps / sec / 1e6
+    value = replicas.job_value(world, EVALS_PER_STEP, cells, args.steps, sec)
 
     # ---- breakdown: the three calls of BASELINE.json's metric, timed alone ----
     H = torch.empty_like(m)
@@ -316,7 +311,7 @@ def run_b200(args):
     sec_e2e = over_ranks(timed(step_e2e, args.steps))
     h2d = 2 * m_host.numel() * s
     d2h = (2 * m_host.numel() + du_back.numel()) * s
-    e2e_value = world * EVALS_PER_STEP * cells * args.steps / sec_e2e / 1e6
+    e2e_value = replicas.job_value(world, EVALS_PER_STEP, cells, args.steps, sec_e2e)
 
     if rank != 0:
         if world > 1:

@@ -49,6 +49,9 @@ def _lib():
         _LIB.newell_tensor_quad.restype = ctypes.c_int
         _LIB.newell_tensor_quad.argtypes = [ctypes.POINTER(ctypes.c_int),
                                             ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]
+        _LIB.newell_tensor_quad_at.restype = ctypes.c_int
+        _LIB.newell_tensor_quad_at.argtypes = [ctypes.c_void_p, ctypes.c_long,
+                                               ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]
     return _LIB
 
 
@@ -60,6 +63,18 @@ def demag_tensor(n_cells, dx):
     rc = _lib().newell_tensor_quad(n, d, out.ctypes.data_as(ctypes.c_void_p))
     if rc != 0:
         raise MemoryError("newell_tensor_quad")
+    return out
+
+
+def demag_tensor_at(offsets, dx):
+    """N[k, a] at the signed cell offsets offsets[k] = (p1, p2, p3), a in COMPONENTS order: the
+    same closed form as demag_tensor, evaluated offset by offset (for sampled checks on grids
+    whose full table would take minutes)."""
+    p = np.ascontiguousarray(np.asarray(offsets, dtype=np.int32).reshape(-1, 3))
+    d = (ctypes.c_double * 3)(*[float(v) for v in dx])
+    out = np.empty((p.shape[0], 6), dtype=np.float64)
+    _lib().newell_tensor_quad_at(p.ctypes.data_as(ctypes.c_void_p), p.shape[0], d,
+                                 out.ctypes.data_as(ctypes.c_void_p))
     return out
 
 

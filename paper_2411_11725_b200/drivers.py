@@ -1,0 +1,63 @@
+"""Host-side drivers around the C-ABI: the adaptive step controller of config 3 and the
+adjoint-state gradient loop of config 5.  They hold loop control only — which step to take next,
+when to store or restore a checkpoint — and call `nm_rk_step` / `nm_adjoint_rk4_step` for every
+piece of arithmetic on the fields (readings C6 and C8).
+"""
+import torch
+
+
+def dopri5_next_dt(dt, err_norm, safety=0.9, lo=0.2, hi=5.0):
+    """Reading C6: dt_new = dt * clip(0.9 * err^(-1/5), 0.2, 5)."""
+    if not (err_norm > 0.0):
+        return dt * hi
+    return dt * min(hi, max(lo, safety * err_norm ** (-0.2)))
+
+
+def integrate_dopri5(mesh, m, t0, t1, dt0, zeeman=None, rtol=1e-5, atol=1e-5, renormalise=True,
+                     max_steps=10 ** 9, on_step=None):
+    """Advance m in place from t0 to t1 with Dormand-Prince 5(4).  The device takes
+    the accept/reject decision (nm_rk_step leaves m untouched on a rejected step) and returns the
+    scalar error norm; this loop only adapts dt.  Returns (t, dt, accepted, rejected)."""
+    t, dt = float(t0), float(dt0)
+    acc = rej = 0
+    while t < t1 and acc + rej < max_steps:
+        h = min(dt, t1 - t)
+        err = mesh.nm_rk_step(1, t, h, m, zeeman, renormalise=renormalise, rtol=rtol, atol=atol,
+                              want_err=True)
+        if err <= 1.0:
+            t += h
+            acc += 1
+            if on_step is not None:
+                on_step(t, h, err)
+        else:
+            rej += 1
+        dt = dopri5_next_dt(h, err)
+    return t, dt, acc, rej
+
+
+def forward_rk4(mesh, m, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
+    """n_steps fixed RK4 steps in place; returns {step index: clone of m before that step}."""
+    ck = {}
+    for s in range(n_steps):
+        if checkpoint_every and s % checkpoint_every == 0:
+            ck[s] = m.clone()
+        mesh.nm_rk_step(0, t0 + s * dt, dt, m, zeeman)
+    return ck
+
+
+def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_every=100, t0=0.0):
+    """Adjoint-state gradient dJ/dMs (Eqs. 27-30; reading C8).
+
+    Forward RK4 from m0 with checkpoints, a(T) = aT_of_mT(m(T)) (the caller's dJ/dm(T)), then the
+    backward RK4 of (m, a, u) with step -dt, m replaced by the stored checkpoint whenever one is
+    reached.  Returns (m(T), a(0), u(0) = dJ/dMs per cell)."""
+    m = m0.clone()
+    ck = forward_rk4(mesh, m, dt, n_steps, zeeman, checkpoint_every, t0)
+    mT = m.clone()
+    a = aT_of_mT(mT).clone()
+    u = torch.zeros(mesh.cell_shape_abi, dtype=m.dtype, device=m.device)
+    for s in range(n_steps, 0, -1):
+        mesh.nm_adjoint_rk4_step(t0 + s * dt, dt, m, a, u, zeeman)
+        if (s - 1) in ck:
+            m.copy_(ck[s - 1])
+    return mT, a, u

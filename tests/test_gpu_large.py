@@ -1,0 +1,156 @@
+"""GPU parity at bench-sized grids, through the C-ABI.
+
+The fp64 oracle cannot evaluate a dense 256^3 field in test time (its __float128 tensor table
+alone takes minutes), so the 256^3 checks use what it *can* compute one output at a time:
+  * a sparse source field (the operators are linear): H^cell at sampled cells is a direct sum
+    over the few non-zero source cells with the oracle tensor evaluated offset by offset, and
+    the exchange field at a sampled node only needs the 3x3x3-cell block around it;
+  * a closed form that holds at any size: the magnetometric demag factor -1/3 of a uniformly
+    magnetised cube.
+Both run in the launch configuration bench.py times (config 4, 256^3, fp32, exchange + demag,
+scalar materials: fast demag path, k_node<EXTRA = false>).  The 128^3 / 96^3 cases are dense
+element-by-element parity on grids that span many tiles of every pass.
+"""
+import numpy as np
+import pytest
+
+from paper_2411_11725_b200 import workloads as wl
+
+from _sides import dev, gpu_mesh, host, oracle_problem, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.mark.parametrize("N", [128, 96])
+def test_heff_dense_parity_fp32(N):
+    """Config 4 at 128^3 (fast path) and 96^3 (generic radix-2/3 path), fp32, every node."""
+    from oracle import llg
+    w = wl.config4_sweep(N)
+    p = oracle_problem(w, np.float32)
+    m = wl.round_to(w.m0, np.float32)
+    ref = llg.effective_field(p, m)
+    mesh = gpu_mesh(w, torch.float32)
+    H = host(mesh.nm_heff(0.0, dev(m, torch.float32)))
+    assert rel_l2(H, ref) <= 1e-5
+    f = host(mesh.nm_llg_rhs(0.0, dev(m, torch.float32)))
+    assert rel_l2(f, llg.llg_from_field(p, m, ref)) <= 1e-5
+
+
+def _sparse_field(node_shape, k, seed):
+    """m = 0 except at k seeded nodes (random vectors of length ~1), some on faces and corners."""
+    rng = np.random.default_rng(seed)
+    m = np.zeros((3,) + tuple(node_shape))
+    pts = [tuple(int(rng.integers(0, s)) for s in node_shape) for _ in range(k - 4)]
+    hi = tuple(s - 1 for s in node_shape)
+    pts += [(0, 0, 0), hi, (0, hi[1] // 2, hi[2]), (hi[0], 3, 0)]
+    for q in pts:
+        m[(slice(None),) + q] = rng.standard_normal(3)
+    return m, pts
+
+
+def _oracle_cell_field_at(cells, src_idx, src_M, dx):
+    """H_c = - sum_c' N(c - c') M_c' for the listed cells, sources given as (index, vector)."""
+    from oracle import demag
+    out = np.zeros((len(cells), 3))
+    for k, c in enumerate(cells):
+        offs = np.asarray(c)[None, :] - src_idx                   # (S, 3)
+        T = demag.demag_tensor_at(offs, dx)                       # (S, 6)
+        for a, (r, s) in enumerate(demag.COMPONENTS):
+            out[k, r] -= np.sum(T[:, a] * src_M[:, s])
+            if r != s:
+                out[k, s] -= np.sum(T[:, a] * src_M[:, r])
+    return out
+
+
+def _oracle_exchange_at(node, m, w, dtype):
+    """Exchange field at one node from the oracle run on the block of cells within 2 of it."""
+    from oracle import llg
+    lo = [max(0, q - 2) for q in node]
+    hi = [min(n, q + 2) for q, n in zip(node, w.n_cells)]         # cell range [lo, hi)
+    nc = tuple(h - l for l, h in zip(lo, hi))
+    sub = m[:, lo[0]:hi[0] + 1, lo[1]:hi[1] + 1, lo[2]:hi[2] + 1]
+    r = lambda v: wl.round_to(np.full(nc, float(v)), dtype)
+    p = llg.Problem(nc, tuple(float(v) for v in w.dx), r(w.Ms), r(w.A), r(0.0), (0.0, 0.0, 1.0),
+                    float(w.gamma), float(w.alpha), wl.TERM_EXCHANGE)
+    H = llg.effective_field(p, np.ascontiguousarray(sub))
+    q = tuple(a - b for a, b in zip(node, lo))
+    # the block must contain every cell adjacent to the node that exists in the full mesh
+    for d in range(3):
+        assert (node[d] == 0 or q[d] >= 1) and (node[d] == w.n_cells[d] or q[d] <= nc[d] - 1)
+    return H[(slice(None),) + q]
+
+
+def test_heff_256_sparse_sources_sampled_fp32():
+    """Bench configuration (256^3, fp32, exchange + demag): sampled H^cell and nodal H_eff."""
+    from oracle import demag, mesh as omesh
+    N = 256
+    w = wl.config4_sweep(N)
+    nd = np.float32
+    m, pts = _sparse_field(w.node_shape, 120, seed=2561)
+    m = wl.round_to(m, nd)
+    msh = gpu_mesh(w, torch.float32)
+    H = host(msh.nm_heff(0.0, dev(m, torch.float32)))
+    Hc = host(msh.nm_debug_get_cell_field())
+
+    # source cells: the <= 8 cells around every non-zero node, M_c = Ms (1/8) sum of vertices
+    Ms = float(np.float32(w.Ms))
+    src = {}
+    for q in pts:
+        for o in np.ndindex(2, 2, 2):
+            c = tuple(a - b for a, b in zip(q, o))
+            if all(0 <= v < N for v in c):
+                src[c] = None
+    src_idx = np.array(sorted(src))
+    src_M = np.zeros((len(src_idx), 3))
+    for k, c in enumerate(src_idx):
+        blk = m[:, c[0]:c[0] + 2, c[1]:c[1] + 2, c[2]:c[2] + 2]
+        src_M[k] = Ms * blk.reshape(3, 8).sum(axis=1) / 8.0       # C5
+
+    rng = np.random.default_rng(2562)
+    cells = [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(40)]
+    cells += [tuple(int(v) for v in src_idx[i]) for i in rng.integers(0, len(src_idx), 20)]
+    cells += [(0, 0, 0), (N - 1, N - 1, N - 1), (N - 1, 0, 17), (128, 128, 128), (127, 128, 255)]
+    ref_c = _oracle_cell_field_at(cells, src_idx, src_M, w.dx)
+    got_c = np.array([Hc[(slice(None),) + c] for c in cells])
+    peak = np.abs(Hc).max()
+    assert rel_l2(got_c, ref_c) <= 1e-5
+    assert np.abs(got_c - ref_c).max() <= 1e-5 * peak
+
+    # nodal H_eff at sampled nodes: exchange from the local block + Ms-weighted mean of the
+    # adjacent cell fields (uniform Ms: plain mean over the cells that exist; C5)
+    nodes = [pts[i] for i in (0, 1, 2, 3, 4)] + [pts[-1], pts[-2], pts[-3], pts[-4]]
+    nodes += [tuple(min(N, v + 1) for v in pts[5]), tuple(max(0, v - 1) for v in pts[6])]
+    ref_n, got_n = [], []
+    for q in nodes:
+        adj = [tuple(a - b for a, b in zip(q, o)) for o in np.ndindex(2, 2, 2)]
+        adj = [c for c in adj if all(0 <= v < N for v in c)]
+        hd = _oracle_cell_field_at(adj, src_idx, src_M, w.dx).mean(axis=0)
+        ref_n.append(_oracle_exchange_at(q, m, w, nd) + hd)
+        got_n.append(H[(slice(None),) + q])
+    assert rel_l2(np.array(got_n), np.array(ref_n)) <= 1e-5
+
+
+def test_uniform_cube_256_demag_factor_fp32():
+    """Uniformly magnetised 256^3 cube: the L-weighted mean nodal demag field is -Ms/3 along m
+    (magnetometric factor of a cube, exact for the discrete operator: oracle pin
+    test_uniform_cube_magnetometric_factor), zero across, and the exchange field vanishes."""
+    N = 256
+    w = wl.config4_sweep(N)
+    msh = gpu_mesh(w, torch.float32)
+    m = torch.zeros(msh.node_shape_abi, dtype=torch.float32, device="cuda:0")
+    m[2] = 1.0
+    H = msh.nm_heff(0.0, m).double()
+    # L_n is proportional to the number of adjacent cells: 8, 4, 2, 1 by position
+    wgt = torch.ones(N + 1, dtype=torch.float64, device="cuda:0")
+    wgt[0] = wgt[-1] = 0.5
+    L = wgt[:, None, None] * wgt[None, :, None] * wgt[None, None, :]
+    mean = [float((H[j] * L).sum() / L.sum()) for j in range(3)]
+    Ms = float(np.float32(w.Ms))
+    assert abs(mean[2] + Ms / 3.0) <= 1e-5 * Ms / 3.0
+    assert abs(mean[0]) <= 1e-5 * Ms and abs(mean[1]) <= 1e-5 * Ms
+    # mirror symmetry of H_z about the mid-planes
+    Hz = H[2]
+    assert float((Hz - Hz.flip(0)).abs().max()) <= 2e-5 * Ms
+    assert float((Hz - Hz.flip(2)).abs().max()) <= 2e-5 * Ms

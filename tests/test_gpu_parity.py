@@ -204,6 +204,7 @@ def test_dopri5_replay_config3_small_fp32():
     """Config 3's recipe on a 64x64x1 film: the GPU runs the adaptive controller in fp32, the
     oracle replays the GPU's accepted/rejected dt sequence in fp64."""
     from oracle import llg
+    from paper_2411_11725_b200 import drivers
     w = wl.config3_thin_film(64)
     td = torch.float32
     p = oracle_problem(w, np.float32)
@@ -222,7 +223,7 @@ def test_dopri5_replay_config3_small_fp32():
             ref = out if acc else ref
             t += dt
             accepted += 1
-        dt = llg.dopri5_next_dt(dt, err)
+        dt = drivers.dopri5_next_dt(dt, err)
         if accepted >= 25:
             break
     assert accepted >= 10
@@ -281,6 +282,35 @@ def test_adjoint_rk4_backward_small_config5_fp64():
             y.copy_(gck[s - 1])
     assert rel_l2(host(a), a0_ref) <= 1e-11
     assert rel_l2(wl.from_abi(u.cpu().numpy()), u0_ref) <= 1e-11
+
+
+def test_adjoint_gradient_driver_vs_finite_differences_config5_small_fp64():
+    """Config 5's check on a 32x8x1 film, 40 steps: dJ/dMs from drivers.adjoint_gradient against
+    central finite differences of J (GPU forward solves with Ms_c +- h) on 8 seeded cells
+    (C8: <= 1e-3 relative; the adjoint-state gradient is the continuous problem's)."""
+    from paper_2411_11725_b200 import drivers
+    w = wl.config5_inverse((32, 8, 1), n_steps=40)
+    td = torch.float64
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    m0 = dev(_m0(w, td), td)
+    g = dev(wl.objective_weights(w), td)
+    _, _, u0 = drivers.adjoint_gradient(mesh, m0, lambda mT: g, w.dt, w.n_steps, gz, checkpoint_every=10)
+    grad = wl.from_abi(u0.cpu().numpy())
+
+    def J(Ms):
+        mesh.nm_mesh_set_Ms(dev(Ms, td))
+        y = m0.clone()
+        drivers.forward_rk4(mesh, y, w.dt, w.n_steps, gz)
+        return float((g * y).sum())
+
+    for c in wl.fd_cells(w, 8, 6):
+        h = 1e-4 * w.Ms[c]
+        Mp, Mm = w.Ms.copy(), w.Ms.copy()
+        Mp[c] += h
+        Mm[c] -= h
+        fd = (J(Mp) - J(Mm)) / (2 * h)
+        assert abs(grad[c] - fd) <= 1e-3 * abs(fd), (c, grad[c], fd)
 
 
 # ---- boundary behaviour --------------------------------------------------------------------------

@@ -269,3 +269,24 @@ def test_L_weighted_self_adjointness_and_positive_energy():
     b = np.sum(L * np.sum(v * effective_field(pd, u), axis=0))
     assert abs(a - b) < 1e-13 * max(abs(a), abs(b))
     assert -0.5 * np.sum(L * np.sum(u * effective_field(pd, u), axis=0)) > 0   # demag energy >= 0
+
+
+def test_tensor_at_listed_offsets_matches_table_and_dipole_limit():
+    """demag_tensor_at (offset-by-offset evaluation used by the full-size sampled GPU checks)
+    equals the table with the parity rules of tensor_at, and at a separation far outside any
+    table it tends to the point-dipole tensor (independent of the table code path)."""
+    dx = (2.0, 3.0, 2.5)
+    Nt = demag.demag_tensor((6, 5, 7), dx)
+    offs = [(0, 0, 0), (1, 0, 0), (-1, 2, -3), (5, -4, 6), (-5, -4, -6), (0, 3, -2)]
+    T = demag.demag_tensor_at(offs, dx)
+    for k, p in enumerate(offs):
+        for a in range(6):
+            assert abs(T[k, a] - demag.tensor_at(Nt, a, p)) <= 1e-16   # summation order only
+    p = (300, -170, 410)
+    T = demag.demag_tensor_at([p], dx)[0]
+    D = dipole_tensor(np.array(p) * np.array(dx), np.prod(dx))
+    A = np.zeros((3, 3))
+    for a, (r, s) in enumerate(demag.COMPONENTS):
+        A[r, s] = A[s, r] = T[a]
+    assert np.abs(A - D).max() <= 1e-4 * np.abs(D).max()
+    assert abs(np.trace(A)) <= 1e-9 * np.abs(D).max()

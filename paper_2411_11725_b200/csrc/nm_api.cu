@@ -196,6 +196,10 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
     m->f64 = d->dtype == NM_F64;
     m->esz = m->f64 ? 8 : 4;
     m->launches = 0;
+    m->last_partials = 0;
+    m->uni_A = d->A == nullptr;
+    m->uni_Ku = d->Ku == nullptr;
+    m->uni_Ms = d->Ms == nullptr;
     m->hc1_valid = false;
     m->prof_on = false;
     m->prof_n = 0;
@@ -309,6 +313,7 @@ extern "C" nm_status nm_mesh_set_Ms(nm_mesh *mesh, const void *Ms, void *stream)
     NM_CUDA_TRY(cudaSetDevice(mesh->desc.device));
     NM_CUDA_TRY(cudaMemcpyAsync(mesh->Ms, Ms, mesh->g.cells * mesh->esz, cudaMemcpyDeviceToDevice, st));
     mesh->hc1_valid = false;
+    mesh->uni_Ms = false;
     return nm_compute_sMs(mesh, st);
 }
 
@@ -485,6 +490,17 @@ void base_args(const nm_mesh *m, double t, const nm_zeeman *z, unsigned terms, N
         a->amp = (T)(z->amp ? z->amp(t, z->user) : 1.0);
         for (int j = 0; j < 3; ++j) a->hu[j] = (T)z->h_uniform[j];
     }
+    // separable kernel: uniform A and Ku (anisotropy off counts as uniform)
+    const bool an_on = (terms & NM_TERM_ANISO) != 0;
+    a->sep = (m->uni_A && (m->uni_Ku || !an_on)) ? 1 : 0;
+    {
+        const char *env = getenv("NM_NODE_PATH");        // "generic" forces the 27-point kernel
+        if (env && strcmp(env, "generic") == 0) a->sep = 0;
+    }
+    a->cex = (terms & NM_TERM_EXCHANGE) ? (T)(16.0 * m->desc.A_scalar / NM_MU0) : (T)0;
+    a->cku = an_on ? (T)(16.0 * m->desc.Ku_scalar / NM_MU0) : (T)0;
+    for (int d = 0; d < 3; ++d) a->idx2[d] = (T)(1.0 / (dx[d] * dx[d]));
+    a->ms_uni = m->uni_Ms ? (T)m->desc.Ms_scalar : (T)0;
     const double gp = m->desc.gamma / (1.0 + m->desc.alpha * m->desc.alpha);
     a->gp = (T)gp;
     a->agp = (T)(m->desc.alpha * gp);
@@ -604,11 +620,11 @@ nm_status dopri5_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z,
         NM_TRY(eval_stage<T>(m, t + DP_C[s] * dt, fld, z, r, st));
         if (s < 6) fld = Yb[s & 1];
     }
-    NM_TRY(nm_launch_err_final(m, m->n_partials, 3.0 * (double)m->g.nodes, st));
+    NM_TRY(nm_launch_err_final(m, m->last_partials, 3.0 * (double)m->g.nodes, st));
     // y5 lives in Yb[5 & 1]
-    NM_TRY(nm_launch_commit<T>(m, y, Yb[1], m->partials + m->n_partials, renorm, st));
+    NM_TRY(nm_launch_commit<T>(m, y, Yb[1], m->partials + m->last_partials, renorm, st));
     if (err_host) {
-        NM_CUDA_TRY(cudaMemcpyAsync(err_host, m->partials + m->n_partials, sizeof(double),
+        NM_CUDA_TRY(cudaMemcpyAsync(err_host, m->partials + m->last_partials, sizeof(double),
                                     cudaMemcpyDeviceToHost, st));
         NM_CUDA_TRY(cudaStreamSynchronize(st));
     }

@@ -85,7 +85,10 @@ struct nm_mesh {
     void *Y[2];             // RK stage states
     void *Uc[2];            // cell scalars (adjoint RK)
     double *partials;       // reduction scratch [node blocks + 1]
-    int n_partials;
+    int n_partials;         // capacity
+    int last_partials;      // partial sums the last node-kernel launch wrote
+    // materials given as scalars at create (enables the separable node kernel)
+    bool uni_A, uni_Ku, uni_Ms;
     bool hc1_valid;
     // per-launch timing (nm_profile_begin / nm_profile_end)
     bool prof_on;

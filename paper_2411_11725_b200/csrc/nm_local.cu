@@ -39,15 +39,97 @@ __device__ __forceinline__ double block_sum(double v)
 {
     __shared__ double red[32];
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    const int t = threadIdx.y * blockDim.x + threadIdx.x;
+    const int w = t >> 5, l = t & 31;
     if (l == 0) red[w] = v;
     __syncthreads();
     double r = 0.0;
     if (w == 0) {
-        r = l < (blockDim.x + 31) / 32 ? red[l] : 0.0;
+        r = l < (blockDim.x * blockDim.y + 31) / 32 ? red[l] : 0.0;
         for (int o = 16; o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
     }
-    return r;   // valid in thread 0
+    return r;   // valid in thread (0, 0)
+}
+
+// a9-a11 on one node: what to do with H_n (modes of nm_local.cuh).  mc = fld_n, sms = (S Ms)_n.
+template <typename T>
+__device__ __forceinline__ void node_epilogue(const NmLocalArgs<T> &a, long long n, long long nn,
+                                              const T *mc, const T *H, T sms, double &err2)
+{
+    if (a.mode == NM_MODE_H) {
+        a.out[n] = H[0]; a.out[nn + n] = H[1]; a.out[2 * nn + n] = H[2];
+    } else if (a.mode == NM_MODE_ADJ2) {
+        // dadt = -(d + (S Ms) Hlin(q));  fld = q, H = Hlin(q)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) a.dadt[j * nn + n] = -(a.dadt[j * nn + n] + sms * H[j]);
+    } else {
+        T mxH[3], mxmxH[3], f[3];
+        cross3(mc, H, mxH);
+        cross3(mc, mxH, mxmxH);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) f[j] = -a.gp * mxH[j] - a.agp * mxmxH[j];
+        if (a.mode == NM_MODE_RHS) {
+            a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
+        } else if (a.mode == NM_MODE_RK) {
+            const NmRkArgs<T> &r = a.rk;
+            if (r.kstore) {
+                r.kstore[n] = f[0]; r.kstore[nn + n] = f[1]; r.kstore[2 * nn + n] = f[2];
+            }
+            T y0[3], y[3], er[3];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                y0[j] = r.y0[j * nn + n];
+                T acc = r.cself * f[j];
+                T ea = r.eself * f[j];
+                for (int q = 0; q < r.nprev; ++q) {
+                    const T kp = r.kprev[q][j * nn + n];
+                    acc += r.cprev[q] * kp;
+                    ea += r.eprev[q] * kp;
+                }
+                y[j] = y0[j] + r.dt * acc;
+                er[j] = r.dt * ea;
+            }
+            if (r.ynext) {
+                if (r.renorm) {
+                    const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+                    y[0] *= inv; y[1] *= inv; y[2] *= inv;
+                }
+                r.ynext[n] = y[0]; r.ynext[nn + n] = y[1]; r.ynext[2 * nn + n] = y[2];
+            }
+            if (r.want_err) {
+                // last Dormand-Prince stage: fld = y5 (un-normalised), y0 = start of step
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    const T sc = r.atol + r.rtol * max_t(abs_t(y0[j]), abs_t(mc[j]));
+                    const double q = (double)(er[j] / sc);
+                    err2 += q * q;
+                }
+            }
+        } else {   // NM_MODE_ADJ1
+            if (a.out) {
+                a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
+            }
+            const T av[3] = {a.adj[n], a.adj[nn + n], a.adj[2 * nn + n]};
+            T mxa[3], mxmxa[3], Hxa[3], b[3];
+            cross3(mc, av, mxa);
+            cross3(mc, mxa, mxmxa);
+            cross3(H, av, Hxa);
+            const T mH = mc[0] * H[0] + mc[1] * H[1] + mc[2] * H[2];
+            const T am = av[0] * mc[0] + av[1] * mc[1] + av[2] * mc[2];
+            const T aH = av[0] * H[0] + av[1] * H[1] + av[2] * H[2];
+            const T invS = sms > 0 ? (T)1 / sms : (T)0;
+            T bH = 0;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                b[j] = a.gp * mxa[j] - a.agp * mxmxa[j];
+                const T d = -a.gp * Hxa[j] - a.agp * (mH * av[j] + am * H[j] - (T)2 * aH * mc[j]);
+                a.dadt[j * nn + n] = d;
+                a.Q[j * nn + n] = b[j] * invS;
+                bH += b[j] * H[j];
+            }
+            a.W[n] = bH * invS;
+        }
+    }
 }
 
 // EXTRA = false: exchange + demag + uniform Zeeman only (no anisotropy, no nodal Zeeman arrays).
@@ -160,84 +242,196 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
             }
         }
 
-        if (a.mode == NM_MODE_H) {
-            a.out[n] = H[0]; a.out[nn + n] = H[1]; a.out[2 * nn + n] = H[2];
-        } else if (a.mode == NM_MODE_ADJ2) {
-            // dadt = -(d + (S Ms) Hlin(q));  fld = q, H = Hlin(q)
-#pragma unroll
-            for (int j = 0; j < 3; ++j) a.dadt[j * nn + n] = -(a.dadt[j * nn + n] + sms * H[j]);
-        } else {
-            T mxH[3], mxmxH[3], f[3];
-            cross3(mc, H, mxH);
-            cross3(mc, mxH, mxmxH);
-#pragma unroll
-            for (int j = 0; j < 3; ++j) f[j] = -a.gp * mxH[j] - a.agp * mxmxH[j];
-            if (a.mode == NM_MODE_RHS) {
-                a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
-            } else if (a.mode == NM_MODE_RK) {
-                const NmRkArgs<T> &r = a.rk;
-                if (r.kstore) {
-                    r.kstore[n] = f[0]; r.kstore[nn + n] = f[1]; r.kstore[2 * nn + n] = f[2];
-                }
-                T y0[3], y[3], er[3];
-#pragma unroll
-                for (int j = 0; j < 3; ++j) {
-                    y0[j] = r.y0[j * nn + n];
-                    T acc = r.cself * f[j];
-                    T ea = r.eself * f[j];
-                    for (int q = 0; q < r.nprev; ++q) {
-                        const T kp = r.kprev[q][j * nn + n];
-                        acc += r.cprev[q] * kp;
-                        ea += r.eprev[q] * kp;
-                    }
-                    y[j] = y0[j] + r.dt * acc;
-                    er[j] = r.dt * ea;
-                }
-                if (r.ynext) {
-                    if (r.renorm) {
-                        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
-                        y[0] *= inv; y[1] *= inv; y[2] *= inv;
-                    }
-                    r.ynext[n] = y[0]; r.ynext[nn + n] = y[1]; r.ynext[2 * nn + n] = y[2];
-                }
-                if (r.want_err) {
-                    // last Dormand-Prince stage: fld = y5 (un-normalised), y0 = start of step
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) {
-                        const T sc = r.atol + r.rtol * max_t(abs_t(y0[j]), abs_t(mc[j]));
-                        const double q = (double)(er[j] / sc);
-                        err2 += q * q;
-                    }
-                }
-            } else {   // NM_MODE_ADJ1
-                if (a.out) {
-                    a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
-                }
-                const T av[3] = {a.adj[n], a.adj[nn + n], a.adj[2 * nn + n]};
-                T mxa[3], mxmxa[3], Hxa[3], b[3];
-                cross3(mc, av, mxa);
-                cross3(mc, mxa, mxmxa);
-                cross3(H, av, Hxa);
-                const T mH = mc[0] * H[0] + mc[1] * H[1] + mc[2] * H[2];
-                const T am = av[0] * mc[0] + av[1] * mc[1] + av[2] * mc[2];
-                const T aH = av[0] * H[0] + av[1] * H[1] + av[2] * H[2];
-                const T invS = sms > 0 ? (T)1 / sms : (T)0;
-                T bH = 0;
-#pragma unroll
-                for (int j = 0; j < 3; ++j) {
-                    b[j] = a.gp * mxa[j] - a.agp * mxmxa[j];
-                    const T d = -a.gp * Hxa[j] - a.agp * (mH * av[j] + am * H[j] - (T)2 * aH * mc[j]);
-                    a.dadt[j * nn + n] = d;
-                    a.Q[j * nn + n] = b[j] * invS;
-                    bH += b[j] * H[j];
-                }
-                a.W[n] = bH * invS;
-            }
-        }
+        node_epilogue<T>(a, n, nn, mc, H, sms, err2);
     }
     if (a.mode == NM_MODE_RK && a.rk.want_err) {
         const double s = block_sum(err2);
         if (threadIdx.x == 0) a.rk.partials[blockIdx.y * gridDim.x + blockIdx.x] = s;
+    }
+}
+
+
+// -------------------------------------------------------------------------------------------------
+// Separable node kernel for uniform A and Ku (scalars at nm_mesh_create), any Ms.
+//
+// With a cell-constant coefficient the assembled tensor-product element operators of Eqs. (19)-(20)
+// factor into assembled 1-D operators along each axis (C2: K = V sum_d dx_d^-2 K1 (x) M1 (x) M1,
+// M = V M1 (x) M1 (x) M1):
+//     (A v)_i = [i>0] (v_i - v_{i-1}) + [i<N] (v_i - v_{i+1})                 stiffness, K1
+//     (B v)_i = [i>0] (v_i/3 + v_{i-1}/6) + [i<N] (v_i/3 + v_{i+1}/6)         mass, M1
+//     E_n   = dx^-2 (Bz By Ax m) + dy^-2 (Bz Ay Bx m) + dz^-2 (Az By Bx m)
+//     H^ex  = -(16 A / (mu0 (S Ms)_n)) E_n,   H^an = (16 Ku / (mu0 (S Ms)_n)) (Bz By Bx (m.k)) k
+// and the one-sided boundary stencils / reduced lumped mass of Eq. (22) come out of the [.] factors.
+// A CTA owns an SX x SY patch of node columns and marches along z: per plane it stages the m tile
+// (+1 halo) and the cell tile of H^cell in shared memory, forms the in-plane parts
+//     U = dx^-2 By Ax m + dy^-2 Ay Bx m,   W = By Bx m,   T = sum over the 2x2 cells of w_c Hc_c
+// and combines three consecutive planes in registers.  The next plane is prefetched into registers
+// while the current one is being used (one barrier per plane).
+constexpr int SX = 32, SY = 8;
+constexpr int MP = SX + 2;              // m tile pitch
+constexpr int MT = (SY + 2) * MP;       // m tile elements per component
+constexpr int CPT = SX + 1;             // cell tile pitch
+constexpr int CT = (SY + 1) * CPT;      // cell tile elements per component
+constexpr int MR = (MT + SX * SY - 1) / (SX * SY);
+constexpr int CR = (CT + SX * SY - 1) / (SX * SY);
+
+template <typename T, bool UNI_MS>
+__global__ void __launch_bounds__(SX * SY) k_node_sep(const NmLocalArgs<T> a, int zchunk)
+{
+    const NmGeom &g = a.g;
+    __shared__ T s_m[2][3][MT];
+    __shared__ T s_c[2][3][CT];
+    const int tid = threadIdx.y * SX + threadIdx.x;
+    const int x0 = blockIdx.x * SX, y0 = blockIdx.y * SY;
+    const int i1 = x0 + threadIdx.x, i2 = y0 + threadIdx.y;
+    const bool live = i1 < g.n1 && i2 < g.n2;
+    const int z0 = blockIdx.z * zchunk;
+    const int z1 = min(z0 + zchunk, g.n3);
+    const long long pl = (long long)g.n1 * g.n2, nn = g.nodes;
+    const long long cpl = (long long)g.N1 * g.N2;
+    const bool has_hc = a.Hc != nullptr;
+
+    // global offsets of this thread's tile elements (-1: outside the mesh -> 0)
+    int m_off[MR], c_off[CR];
+#pragma unroll
+    for (int r = 0; r < MR; ++r) {
+        const int idx = tid + r * SX * SY;
+        const int ly = idx / MP, lx = idx - ly * MP;
+        const int gx = x0 - 1 + lx, gy = y0 - 1 + ly;
+        m_off[r] = (idx < MT && gx >= 0 && gx < g.n1 && gy >= 0 && gy < g.n2) ? gy * g.n1 + gx : -1;
+    }
+#pragma unroll
+    for (int r = 0; r < CR; ++r) {
+        const int idx = tid + r * SX * SY;
+        const int ly = idx / CPT, lx = idx - ly * CPT;
+        const int gx = x0 - 1 + lx, gy = y0 - 1 + ly;
+        c_off[r] = (idx < CT && gx >= 0 && gx < g.N1 && gy >= 0 && gy < g.N2) ? gy * g.N1 + gx : -1;
+    }
+    // 1-D coefficients of this node column
+    const T eL = i1 > 0 ? (T)1 : (T)0, eR = i1 < g.N1 ? (T)1 : (T)0;
+    const T fL = i2 > 0 ? (T)1 : (T)0, fR = i2 < g.N2 ? (T)1 : (T)0;
+    const T third = (T)(1.0 / 3.0), sixth = (T)(1.0 / 6.0);
+    const T bx0 = (eL + eR) * third, bxL = eL * sixth, bxR = eR * sixth;
+    const T by0 = (fL + fR) * third, byL = fL * sixth, byR = fR * sixth;
+    const T cxy = (eL + eR) * (fL + fR);            // adjacent cells per plane of cells
+
+    T pm[MR][3], pc[CR][3];
+    auto fetch = [&](int k) {
+        // m plane k (node plane) and cell plane k - 1
+        const bool mv = k >= 0 && k < g.n3;
+        const bool cv = has_hc && k - 1 >= 0 && k - 1 < g.N3;
+#pragma unroll
+        for (int r = 0; r < MR; ++r)
+#pragma unroll
+            for (int j = 0; j < 3; ++j)
+                pm[r][j] = (mv && m_off[r] >= 0) ? a.fld[j * nn + (long long)k * pl + m_off[r]] : (T)0;
+#pragma unroll
+        for (int r = 0; r < CR; ++r) {
+            const bool ok = cv && c_off[r] >= 0;
+            const long long c = (long long)(k - 1) * cpl + c_off[r];
+            if (UNI_MS) {
+#pragma unroll
+                for (int j = 0; j < 3; ++j) pc[r][j] = ok ? a.Hc[j * g.cells + c] : (T)0;
+            } else {
+                const T ms = ok ? a.Ms[c] : (T)0;
+#pragma unroll
+                for (int j = 0; j < 3; ++j) pc[r][j] = ok ? ms * a.Hc[j * g.cells + c] : (T)0;
+            }
+        }
+    };
+    auto stash = [&](int b) {
+#pragma unroll
+        for (int r = 0; r < MR; ++r) {
+            const int idx = tid + r * SX * SY;
+            if (idx < MT) {
+#pragma unroll
+                for (int j = 0; j < 3; ++j) s_m[b][j][idx] = pm[r][j];
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < CR; ++r) {
+            const int idx = tid + r * SX * SY;
+            if (idx < CT) {
+#pragma unroll
+                for (int j = 0; j < 3; ++j) s_c[b][j][idx] = pc[r][j];
+            }
+        }
+    };
+
+    T Um[3] = {0, 0, 0}, U0[3] = {0, 0, 0}, Wm[3] = {0, 0, 0}, W0[3] = {0, 0, 0};
+    T T0[3] = {0, 0, 0}, mc0[3] = {0, 0, 0};
+    double err2 = 0.0;
+    const int kstart = max(z0 - 1, 0), kend = z1;         // kend may be n3 (no such plane: zeros)
+    int cur = 0;
+    fetch(kstart);
+    stash(0);
+    __syncthreads();
+    const int lm = (threadIdx.y + 1) * MP + threadIdx.x + 1;
+    const int lc = threadIdx.y * CPT + threadIdx.x;        // cell (i1-1, i2-1) of the tile
+    for (int k = kstart; k <= kend; ++k) {
+        if (k < kend) fetch(k + 1);
+        T Up[3], Wp[3], Tn[3], mcn[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const T *t = s_m[cur][j] + lm;
+            T P[3], Q[3];
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                const T *row = t + (r - 1) * MP;
+                const T l = row[-1], c = row[0], rr = row[1];
+                Q[r] = eL * (c - l) + eR * (c - rr);
+                P[r] = bx0 * c + bxL * l + bxR * rr;
+            }
+            mcn[j] = t[0];
+            const T AyP = fL * (P[1] - P[0]) + fR * (P[1] - P[2]);
+            const T ByQ = by0 * Q[1] + byL * Q[0] + byR * Q[2];
+            Wp[j] = by0 * P[1] + byL * P[0] + byR * P[2];
+            Up[j] = a.idx2[0] * ByQ + a.idx2[1] * AyP;
+            const T *cc = s_c[cur][j] + lc;
+            Tn[j] = (cc[0] + cc[1]) + (cc[CPT] + cc[CPT + 1]);
+        }
+        const int z = k - 1;
+        if (live && z >= z0 && z < z1) {
+            const T gL = z > 0 ? (T)1 : (T)0, gR = z < g.N3 ? (T)1 : (T)0;
+            const long long n = (long long)z * pl + (long long)i2 * g.n1 + i1;
+            const T sms = UNI_MS ? a.ms_uni * cxy * (gL + gR) : a.sMs[n];
+            T H[3] = {0, 0, 0};
+            if (sms > 0) {
+                const T inv = (T)1 / sms;
+                const T bz0 = (gL + gR) * third, bzL = gL * sixth, bzR = gR * sixth;
+                T BW[3], an = 0;
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    BW[j] = bz0 * W0[j] + bzL * Wm[j] + bzR * Wp[j];
+                    an += a.kax[j] * BW[j];
+                }
+                const T dsc = UNI_MS ? a.ms_uni * inv : inv;       // demag average weight
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    const T E = (bz0 * U0[j] + bzL * Um[j] + bzR * Up[j]) +
+                                a.idx2[2] * (gL * (W0[j] - Wm[j]) + gR * (W0[j] - Wp[j]));
+                    T hv = (a.cku * an * a.kax[j] - a.cex * E) * inv + (T0[j] + Tn[j]) * dsc;
+                    if (a.terms & NM_TERM_ZEEMAN) hv += a.hu[j];
+                    H[j] = hv;
+                }
+            }
+            node_epilogue<T>(a, n, nn, mc0, H, sms, err2);
+        }
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            Um[j] = U0[j]; U0[j] = Up[j];
+            Wm[j] = W0[j]; W0[j] = Wp[j];
+            T0[j] = Tn[j]; mc0[j] = mcn[j];
+        }
+        if (k < kend) {
+            stash(cur ^ 1);
+            __syncthreads();
+            cur ^= 1;
+        }
+    }
+    if (a.mode == NM_MODE_RK && a.rk.want_err) {
+        const double s = block_sum(err2);
+        if (tid == 0) a.rk.partials[(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
     }
 }
 
@@ -367,15 +561,37 @@ template <typename T> __global__ void k_lincomb(const LinArgs<T> a)
 
 inline unsigned nblk(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
+// Grid of k_node_sep: SX x SY patches of node columns, z split into chunks so that about eight
+// CTAs per SM exist (each chunk re-reads one halo plane on either side).
+inline dim3 sep_grid(const NmGeom &g, int *zchunk)
+{
+    const unsigned gx = nblk(g.n1, SX), gy = nblk(g.n2, SY);
+    int gz = (int)((148 * 8 + gx * gy - 1) / (gx * gy));
+    const int gz_max = g.n3 / 8 > 1 ? g.n3 / 8 : 1;
+    if (gz > gz_max) gz = gz_max;
+    if (gz < 1) gz = 1;
+    *zchunk = (g.n3 + gz - 1) / gz;
+    return dim3(gx, gy, nblk(g.n3, *zchunk));
+}
+
 } // namespace
 
 // ---- host launchers used by nm_api.cu -----------------------------------------------------------
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
 {
-    {
+    const bool nodal_zee = (a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse);
+    if (a.sep && !nodal_zee) {
+        int zchunk;
+        const dim3 grid = sep_grid(a.g, &zchunk);
+        mesh->last_partials = (int)(grid.x * grid.y * grid.z);
+        NmLaunchScope sc(mesh, NM_K_NODE, st);
+        if (a.ms_uni > 0) k_node_sep<T, true><<<grid, dim3(SX, SY), 0, st>>>(a, zchunk);
+        else k_node_sep<T, false><<<grid, dim3(SX, SY), 0, st>>>(a, zchunk);
+    } else {
         NmLaunchScope sc(mesh, NM_K_NODE, st);
         const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
-        const bool extra = (a.terms & NM_TERM_ANISO) || ((a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse));
+        mesh->last_partials = (int)(grid.x * grid.y);
+        const bool extra = (a.terms & NM_TERM_ANISO) || nodal_zee;
         if (extra) k_node<T, true><<<grid, kBlock, 0, st>>>(a);
         else k_node<T, false><<<grid, kBlock, 0, st>>>(a);
     }
@@ -384,7 +600,14 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
     return NM_OK;
 }
 
-int nm_node_blocks(const NmGeom &g) { return (int)(nblk((long long)g.n1 * g.n2, kBlock) * g.n3); }
+int nm_node_blocks(const NmGeom &g)
+{
+    int zchunk;
+    const dim3 sg = sep_grid(g, &zchunk);
+    const int gen = (int)(nblk((long long)g.n1 * g.n2, kBlock) * g.n3);
+    const int sep = (int)(sg.x * sg.y * sg.z);
+    return gen > sep ? gen : sep;
+}
 
 nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st)
 {

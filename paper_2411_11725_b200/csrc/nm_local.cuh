@@ -49,6 +49,11 @@ template <typename T> struct NmLocalArgs {
     const T *adj;       // a
     T *Q, *W, *dadt;
     NmRkArgs<T> rk;
+    // separable kernel k_node_sep (uniform A and Ku, no nodal Zeeman arrays)
+    int sep;            // 1: eligible
+    T cex, cku;         // 16 A / mu0 and 16 Ku / mu0 (0 when the term is off)
+    T idx2[3];          // 1 / dx_d^2
+    T ms_uni;           // > 0: Ms has this value in every cell; 0: read the Ms / sMs arrays
 };
 
 template <typename T> struct NmAdjCellArgs {
@@ -64,7 +69,7 @@ template <typename T> struct NmAdjCellArgs {
 
 // host launchers defined in nm_local.cu
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st);
-int nm_node_blocks(const NmGeom &g);
+int nm_node_blocks(const NmGeom &g);   // capacity needed for the error-norm partials
 nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st);
 template <typename T>
 nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st);

@@ -210,6 +210,8 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
         if (env && strcmp(env, "generic") == 0) m->fast.on = false;
         const char *ch = getenv("NM_KT_CHUNK");
         m->fast.kt_chunk = ch ? atoi(ch) : 0;
+        const char *pp = getenv("NM_PIPE");              // "0" forces the non-pipelined fast kernels
+        m->fast.pipe = !(pp && strcmp(pp, "0") == 0);
     }
     make_plan(m->g.Lx, &m->plan_x);
     make_plan(m->g.P2, &m->plan_y);

@@ -8,7 +8,7 @@
 //   * spectra live in k1-blocked layouts (8 complex = 64 B per row) so that every pass moves
 //     contiguous blocks:  A[kt][comp][c3][c2][8],  B[kt][ky][comp][c3][8],
 //     with the 8 columns of a row XOR-swizzled by the row index of the *consuming* pass
-//     (slot = k1 ^ (row & 7)) so that its strided shared-memory reads are conflict-free,
+//     (slot = k1 ^ swz(row), nm_fft16.cuh) so that its strided shared-memory reads are conflict-free,
 //   * the tensor is stored as T[kt][|ky|][6][k1][|kz|] and read coalesced along kz.
 // Passes: k_fx_fwd (avg * Ms, x R2C) -> k_fy_fwd -> k_fz_mid (z fwd, H^ = -N^ M^, z inv) ->
 // k_fy_inv -> k_fx_inv (C2R, crop) -> Hc[3][N3][N2][N1] for the node kernel.
@@ -21,7 +21,6 @@ namespace {
 
 constexpr int kWarps = 8;
 constexpr int kThreadsF = 32 * kWarps;
-constexpr int TW = 8;   // complex columns (k1) per blocked row
 
 template <typename V> __device__ __forceinline__ void copy_in(V *dst, const V *__restrict__ src, int n)
 {
@@ -64,14 +63,14 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
 #pragma unroll
     for (int t = 0; t < 16; ++t) {
         const int e = j + M * t;
-        V v = s_io[(sub * N + e) * TW + (k1 ^ (e & 7))];
+        V v = s_io[(sub * N + e) * TW + (k1 ^ swz(e))];
         if (h) v = cmul(v, wP[e]);
         a[t] = v;
     }
     __syncthreads();   // the input tile is dead; s_io becomes the output tile
     V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
     fft_fwd<T, M>(a, tw, scr, i);
-    const int sl = k1 ^ ((c3_0 + sub) & 7);
+    const int sl = k1 ^ swz(c3_0 + sub);
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int ky = 2 * slot_freq<M>(j, s) + h;
@@ -115,7 +114,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
     V a[16];
-    const int sl = k1 ^ ((c3_0 + sub) & 7);
+    const int sl = k1 ^ swz(c3_0 + sub);
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int ky = 2 * slot_freq<M>(j, s) + h;
@@ -132,7 +131,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
         // sum of the even and odd halves: partner lane = lane ^ 1
         v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
         v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
-        if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ (e & 7))] = v;
+        if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ swz(e))] = v;
     }
     __syncthreads();
     V *dst = A + ((((long long)kt * 3 + comp) * N3 + c3_0) * N) * TW;
@@ -180,7 +179,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
             const int e = j + M * t;
-            V v = my[(c * N + e) * TW + (k1 ^ (e & 7))];
+            V v = my[(c * N + e) * TW + (k1 ^ swz(e))];
             if (h) v = cmul(v, wP[e]);
             a[c][t] = v;
         }
@@ -215,7 +214,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
             if (h) v = cmulc(v, wP[e]);
             v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
             v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
-            if ((t >> 3) == h) my[(c * N + e) * TW + (k1 ^ (e & 7))] = v;
+            if ((t >> 3) == h) my[(c * N + e) * TW + (k1 ^ swz(e))] = v;
         }
     }
     __syncthreads();
@@ -277,7 +276,7 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
             const int kt = idx / (R * TW), rem = idx % (R * TW);
             const int r = rem / TW, slot = rem % TW;
             const int c2 = r0 + r;
-            const int k = kt * TW + (slot ^ (c2 & 7));
+            const int k = kt * TW + (slot ^ swz(c2));
             V out = mk<T>((T)0, (T)0);
             if (k <= N) {
                 const V zk = s_z[(r >> 1) * P + k];
@@ -319,7 +318,7 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             const int kt = idx / (R * TW), rem = idx % (R * TW);
             const int r = rem / TW, slot = rem % TW;
             const int c2 = r0 + r;
-            s_x[r * XP + kt * TW + (slot ^ (c2 & 7))] =
+            s_x[r * XP + kt * TW + (slot ^ swz(c2))] =
                 A[((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW + rem];
         }
         __syncthreads();
@@ -419,6 +418,7 @@ nm_status launch_z(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     typedef typename VT<T>::V V;
     const NmGeom &g = mesh->g;
     constexpr int N = 16 * M, LT = 16 / M;
+    if (nm_pipe_mid_ok(mesh)) return nm_pipe_mid(mesh, kt0, nkt, st);
     const size_t sm = (size_t)LT * 3 * N * TW * sizeof(V) + scratch_bytes<T>(kWarps);
     NM_TRY(set_smem_f(k_fz_mid<T, M>, sm));
     const dim3 grid(g.P2 / LT, nkt);

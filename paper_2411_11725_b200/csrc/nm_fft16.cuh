@@ -23,6 +23,14 @@ namespace nmf {
 
 template <typename T> struct VT { typedef typename NmVec2<T>::type V; };
 
+constexpr int TW = 8;   // complex columns (k1) per blocked spectrum row
+
+// Column swizzle of a blocked row: the 8 columns of row r (r = the index the consuming pass
+// transforms along) are stored at slot = k1 ^ swz(r).  16 consecutive rows of one column then
+// fall into 16 different 8-byte bank pairs of shared memory (row parity picks the half, swz the
+// slot), so the strided column reads of the consuming pass are conflict-free.
+__host__ __device__ __forceinline__ int swz(int r) { return (r >> 1) & 7; }
+
 template <typename T> __device__ __forceinline__ typename VT<T>::V mk(T a, T b)
 {
     typename VT<T>::V v;
@@ -109,6 +117,50 @@ template <typename T, bool INV, int Q> __device__ __forceinline__ typename VT<T>
     else { c = c1; s = -s1; }   // 15
     const V w = mk<T>(c, -s);
     return ctw<INV>(a, w);
+}
+
+// exp(-+ 2 pi i q/32) as compile-time constants, q = 0..15
+template <typename T, bool INV, int Q> __device__ __forceinline__ typename VT<T>::V mul_w32(typename VT<T>::V a)
+{
+    typedef typename VT<T>::V V;
+    if (Q % 2 == 0) return mul_w16<T, INV, Q / 2>(a);
+    const T c1 = (T)0.98078528040323044912618223613424;   // cos(pi/16)
+    const T s1 = (T)0.19509032201612826784828486847702;   // sin(pi/16)
+    const T c3 = (T)0.83146961230254523707878837761791;   // cos(3 pi/16)
+    const T s3 = (T)0.55557023301960222474283081394853;   // sin(3 pi/16)
+    T c, s;   // w = c - i s (forward)
+    if (Q == 1) { c = c1; s = s1; }
+    else if (Q == 3) { c = c3; s = s3; }
+    else if (Q == 5) { c = s3; s = c3; }
+    else if (Q == 7) { c = s1; s = c1; }
+    else if (Q == 9) { c = -s1; s = c1; }
+    else if (Q == 11) { c = -s3; s = c3; }
+    else if (Q == 13) { c = -c3; s = s3; }
+    else { c = -c1; s = s1; }   // 15
+    const V w = mk<T>(c, -s);
+    return ctw<INV>(a, w);
+}
+
+// a[t] *= exp(-+ 2 pi i t/32), t = 0..15: the part of the half-sample shift w_P^(j + M t) of the odd
+// half of a padded transform that depends on the register index (the w_P^j part rides in the
+// stage twiddles, see load_twiddles_h).
+template <typename T, bool INV> __device__ __forceinline__ void shift32(typename VT<T>::V *a)
+{
+    a[1] = mul_w32<T, INV, 1>(a[1]);
+    a[2] = mul_w32<T, INV, 2>(a[2]);
+    a[3] = mul_w32<T, INV, 3>(a[3]);
+    a[4] = mul_w32<T, INV, 4>(a[4]);
+    a[5] = mul_w32<T, INV, 5>(a[5]);
+    a[6] = mul_w32<T, INV, 6>(a[6]);
+    a[7] = mul_w32<T, INV, 7>(a[7]);
+    a[8] = mul_w32<T, INV, 8>(a[8]);
+    a[9] = mul_w32<T, INV, 9>(a[9]);
+    a[10] = mul_w32<T, INV, 10>(a[10]);
+    a[11] = mul_w32<T, INV, 11>(a[11]);
+    a[12] = mul_w32<T, INV, 12>(a[12]);
+    a[13] = mul_w32<T, INV, 13>(a[13]);
+    a[14] = mul_w32<T, INV, 14>(a[14]);
+    a[15] = mul_w32<T, INV, 15>(a[15]);
 }
 
 // Position <-> frequency of the in-register butterflies (DIF leaves digit-reversed order).
@@ -221,9 +273,20 @@ __device__ __forceinline__ void load_twiddles2(typename VT<T>::V *tw, const type
     for (int t = 1; t < 16; ++t) tw[t] = wP[(2 * j * t) & (32 * M - 1)];
 }
 
+// Twiddles of team half h with the half-sample shift of the odd half folded in:
+// tw[t'] = w_N^(j t') w_P^(j h) = w_P^(j (2 t' + h)), t' = 0..15 (tw[0] = 1 for h = 0).  Used with
+// fft_fwd/fft_inv<..., TW0 = true> and shift32 on the register index.
+template <typename T, int M>
+__device__ __forceinline__ void load_twiddles_h(typename VT<T>::V *tw, const typename VT<T>::V *__restrict__ wP, int j,
+                                                int h)
+{
+#pragma unroll
+    for (int t = 0; t < 16; ++t) tw[t] = wP[(j * (2 * t + h)) & (32 * M - 1)];
+}
+
 // Forward N-point transform of the team's lines.  a[t] = x[j + M t] on entry (natural), on exit
 // slot s holds frequency slot_freq<M>(q, s).  `scr` = this team's scratch, i = team thread index.
-template <typename T, int M>
+template <typename T, int M, bool TW0 = false>
 __device__ __forceinline__ void fft_fwd(typename VT<T>::V *a, const typename VT<T>::V *tw,
                                         typename VT<T>::V *scr, int i)
 {
@@ -244,7 +307,7 @@ __device__ __forceinline__ void fft_fwd(typename VT<T>::V *a, const typename VT<
     for (int p = 0; p < 16; ++p) {
         const int tp = rev16(p);
         V v = a[p];
-        if (tp != 0) v = cmul(v, tw[tp]);
+        if (tp != 0 || TW0) v = cmul(v, tw[tp]);
         scr[skew((l * 16 + tp) * M + j)] = v;
     }
     __syncwarp();
@@ -258,7 +321,7 @@ __device__ __forceinline__ void fft_fwd(typename VT<T>::V *a, const typename VT<
 }
 
 // Inverse: slot order in, a[t] = N * x[j + M t] out (unscaled).
-template <typename T, int M>
+template <typename T, int M, bool TW0 = false>
 __device__ __forceinline__ void fft_inv(typename VT<T>::V *a, const typename VT<T>::V *tw,
                                         typename VT<T>::V *scr, int i)
 {
@@ -286,7 +349,7 @@ __device__ __forceinline__ void fft_inv(typename VT<T>::V *a, const typename VT<
     for (int p = 0; p < 16; ++p) {
         const int tp = rev16(p);
         V v = scr[skew((l * 16 + tp) * M + j)];
-        if (tp != 0) v = cmulc(v, tw[tp]);
+        if (tp != 0 || TW0) v = cmulc(v, tw[tp]);
         a[p] = v;
     }
     dft16<T, true>(a);

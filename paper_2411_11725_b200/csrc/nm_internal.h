@@ -55,6 +55,7 @@ struct NmFast {
     int NKT;           // k1 tiles of 8 columns
     int Kzp;           // pitch of the |kz| axis of the tensor
     int kt_chunk;      // k1 tiles per y/z/y launch group (0 = all)
+    bool pipe;         // use the persistent TMA-pipelined kernels (nm_demag_pipe.cu) where they apply
     void *Tn;          // tensor [NKT][N2+1][6][8][Kzp] (real)
     void *wPx;         // exp(-2 pi i q / P1), q < P1
 };
@@ -154,6 +155,9 @@ size_t nm_fast_bufB_elems(const NmGeom &g, const NmFast &f);
 nm_status nm_fast_store_tensor(nm_mesh *mesh, const double *octant, double scale, cudaStream_t st);
 template <typename T>
 nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *field_nodes, T *Hc_out, cudaStream_t st);
+// nm_demag_pipe.cu
+bool nm_pipe_mid_ok(const nm_mesh *mesh);
+nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st);
 // nm_local.cu
 nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st);
 

@@ -9,7 +9,7 @@
 //     contiguous blocks:  A[kt][comp][c3][c2][8],  B[kt][ky][comp][c3][8],
 //     with the 8 columns of a row XOR-swizzled by the row index of the *consuming* pass
 //     (slot = k1 ^ swz(row), nm_fft16.cuh) so that its strided shared-memory reads are conflict-free,
-//   * the tensor is stored as T[kt][|ky|][6][k1][|kz|] and read coalesced along kz.
+//   * the tensor is stored as T[kt][|ky|][k1][6][|kz|] and read coalesced along kz.
 // Passes: k_fx_fwd (avg * Ms, x R2C) -> k_fy_fwd -> k_fz_mid (z fwd, H^ = -N^ M^, z inv) ->
 // k_fy_inv -> k_fx_inv (C2R, crop) -> Hc[3][N3][N2][N1] for the node kernel.
 #include "nm_fft16.cuh"
@@ -68,7 +68,7 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
         a[t] = v;
     }
     __syncthreads();   // the input tile is dead; s_io becomes the output tile
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     fft_fwd<T, M>(a, tw, scr, i);
     const int sl = k1 ^ swz(c3_0 + sub);
 #pragma unroll
@@ -121,7 +121,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
         a[s] = s_io[ky * PITCH + sub * TW + sl];
     }
     __syncthreads();
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     fft_inv<T, M>(a, tw, scr, i);
 #pragma unroll
     for (int t = 0; t < 16; ++t) {
@@ -140,7 +140,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
 
 // -------------------------------------------------------------------------------------------------
 // z forward, tensor multiply, z inverse, in place on B.  CTA = LT consecutive ky of one kt.
-//   Tn[kt][|ky|][6][k1][|kz|] (pitch Kzp), components xx,yy,zz,xy,xz,yz, scaled by 1/(P1 P2 P3);
+//   Tn[kt][|ky|][k1][6][|kz|] (pitch Kzp), components xx,yy,zz,xy,xz,yz, scaled by 1/(P1 P2 P3);
 //   off-diagonal components are odd in their two axes: sign -1 per folded axis (ky > N2, kz > N3).
 template <typename T, int M>
 __global__ void __launch_bounds__(kThreadsF)
@@ -169,7 +169,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
     const int line = w * LT + l, sub = line / TW, k1 = line % TW;
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
     V a[3][16];
@@ -189,8 +189,8 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     const int ky = ky0 + sub;
     const int kyf = ky <= N2 ? ky : P2 - ky;
     const T sy = ky <= N2 ? (T)1 : (T)-1;
-    const long long cstride = (long long)TW * Kzp;
-    const T *trow = Tn + ((((long long)kt * (N2 + 1) + kyf) * 6) * TW + k1) * Kzp;
+    const long long cstride = Kzp;
+    const T *trow = Tn + ((((long long)kt * (N2 + 1) + kyf) * TW + k1) * 6) * Kzp;
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int kz = 2 * slot_freq<M>(j, s) + h;
@@ -237,13 +237,13 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     V *s_z = reinterpret_cast<V *>(smem_raw);               // W*LT lines x P
     V *s_scr = s_z + W * LT * P;                            // 2 W teams
-    T *s_cell = reinterpret_cast<T *>(s_scr + 2 * W * Team<M>::SCRATCH);   // R x CP
+    T *s_cell = reinterpret_cast<T *>(s_scr + 2 * W * team_scratch<T, M>());   // R x CP
     const int r0 = blockIdx.x * R, c3 = blockIdx.y;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
     const int line = w * LT + l;
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
     const long long plane = (long long)g.n1 * g.n2;
@@ -310,7 +310,7 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
     const int line = w * LT + l;
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
     for (int comp = 0; comp < 3; ++comp) {
@@ -362,7 +362,7 @@ template <typename K> nm_status set_smem_f(K kernel, size_t bytes)
 
 template <typename T> size_t scratch_bytes(int warps)
 {
-    return (size_t)2 * warps * 272 * sizeof(typename VT<T>::V);
+    return (size_t)2 * warps * team_scratch<T, 16>() * sizeof(typename VT<T>::V);
 }
 
 // ---- per-axis launchers (M is a template parameter of the kernels) ----
@@ -447,8 +447,8 @@ __global__ void k_tensor_store_fast(const double *__restrict__ in, T *__restrict
     if (idx >= total) return;
     long long r = idx;
     const int kz = (int)(r % Kzp); r /= Kzp;
-    const int k1 = (int)(r % TW); r /= TW;
     const int a = (int)(r % 6); r /= 6;
+    const int k1 = (int)(r % TW); r /= TW;
     const int ky = (int)(r % K2);
     const int kt = (int)(r / K2);
     const int kx = kt * TW + k1;
@@ -480,7 +480,7 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
     f->M1 = M[0]; f->M2 = M[1]; f->M3 = M[2];
     f->Wx = W;
     f->NKT = (g.C1 + TW - 1) / TW;
-    f->Kzp = (g.N3 + 1 + 3) & ~3;
+    f->Kzp = (g.N3 + 1 + 1) & ~1;   // even: a warp's 6 rows are a multiple of 16 bytes
     f->on = true;
 }
 

@@ -29,14 +29,15 @@ struct PzSmem {
     static constexpr int TILE_ELEMS = 3 * N * TW;                   // complex
     static constexpr int TILE_BYTES = TILE_ELEMS * 8;               // 49152
     static constexpr int NBUF = 3;
-    static constexpr int KZP = 260;                                 // tensor |kz| pitch (reals)
-    static constexpr int TROW_BYTES = KZP * 4;                      // 1040
-    static constexpr int TSLICE = 6 * KZP;                          // reals per warp
+    static constexpr int KZP = 258;                                 // tensor |kz| pitch (reals), even
+    static constexpr int TSLICE = 6 * KZP;                          // reals per warp (6192 B, one bulk copy)
+    static constexpr int WSCR = 2 * Team<16>::SCRATCH - 8;          // scratch per warp: teams at 0 and SCRATCH
     static constexpr int OFF_T = NBUF * TILE_BYTES;
     static constexpr int OFF_SCR = OFF_T + 8 * TSLICE * 4;
-    static constexpr int OFF_BAR = OFF_SCR + 16 * Team<16>::SCRATCH * 8;
+    static constexpr int OFF_BAR = OFF_SCR + 8 * WSCR * 8;
     static constexpr int BYTES = OFF_BAR + (NBUF + 8) * 8;
 };
+static_assert(PzSmem::BYTES <= 227 * 1024, "k_pz_mid shared memory exceeds the sm_100a per-CTA limit");
 
 __global__ void __launch_bounds__(kPipeThreads, 1)
 k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItems, int kt0,
@@ -73,14 +74,12 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
         const int kyf = g % K2;
         return (kyf == 0 || kyf == N2) ? 1 : 2;
     };
-    // this warp's tensor rows of item g: Tn[kt][|ky|][6][k1 = w][KZP]
+    // this warp's tensor rows of item g: Tn[kt][|ky|][k1 = w][6][KZP], contiguous
     auto load_tensor = [&](int g) {
         const int kyf = g % K2, kt = kt0 + g / K2;
-        const T *src = Tn + ((((long long)kt * K2 + kyf) * 6) * TW + w) * S::KZP;
-        mbar_expect_tx(fullT + w, 6 * S::TROW_BYTES);
-#pragma unroll
-        for (int a = 0; a < 6; ++a)
-            bulk_load(s_T + w * S::TSLICE + a * S::KZP, src + (long long)a * TW * S::KZP, S::TROW_BYTES, fullT + w);
+        const T *src = Tn + (((long long)kt * K2 + kyf) * TW + w) * S::TSLICE;
+        mbar_expect_tx(fullT + w, S::TSLICE * 4);
+        bulk_load(s_T + w * S::TSLICE, src, S::TSLICE * 4, fullT + w);
     };
 
     // prefetch iterator of thread 0: two tiles ahead of the compute iterator
@@ -99,7 +98,7 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + w * S::WSCR + h * Team<M>::SCRATCH;
     const T *ts = s_T + w * S::TSLICE;
     const int cwj = w ^ swz(j);          // swz(j + 16 t) = swz(j)
     int n = 0;

@@ -252,8 +252,17 @@ template <int M> struct Team {
     static constexpr int N = 16 * M;
     static constexpr int U = 16 / M;        // radix-M butterflies per thread in stage 2
     static constexpr int LINES = 16 / M;    // lines per team
-    static constexpr int SCRATCH = 256 + 16;   // complex elements of exchange scratch per team
+    // Complex elements of exchange scratch per team: 256 + 15 of skew, rounded so that the two
+    // teams of a warp (lanes 2i and 2i+1 sit in the same half-warp) start 64 bytes apart modulo
+    // the 128-byte bank period -- their simultaneous 64-bit (fp32) or 128-bit (fp64) accesses then
+    // use disjoint halves of the banks.
+    static constexpr int SCRATCH = 280;        // fp32: 280 * 8 B = 17.5 * 128 B
+    static constexpr int SCRATCH64 = 276;      // fp64: 276 * 16 B = 34.5 * 128 B
 };
+template <typename T, int M> __host__ __device__ constexpr int team_scratch()
+{
+    return sizeof(T) == 8 ? Team<M>::SCRATCH64 : Team<M>::SCRATCH;
+}
 
 // frequency (0..N-1) of the N-point transform held in slot s = u*M + p of team thread with q = i % M
 template <int M> __device__ __forceinline__ int slot_freq(int q, int s)

@@ -56,7 +56,7 @@ struct NmFast {
     int Kzp;           // pitch of the |kz| axis of the tensor
     int kt_chunk;      // k1 tiles per y/z/y launch group (0 = all)
     bool pipe;         // use the persistent TMA-pipelined kernels (nm_demag_pipe.cu) where they apply
-    void *Tn;          // tensor [NKT][N2+1][6][8][Kzp] (real)
+    void *Tn;          // tensor [NKT][N2+1][8][6][Kzp] (real)
     void *wPx;         // exp(-2 pi i q / P1), q < P1
 };
 

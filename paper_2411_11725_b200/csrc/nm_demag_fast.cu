@@ -509,7 +509,9 @@ template <typename T>
 nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
 {
     const NmFast &f = mesh->fast;
-    NM_SWITCH_M(f.M1, (launch_x<T, MM>(mesh, false, fld, Hc_out, st)));
+    const bool px = nm_pipe_x_ok(mesh);
+    if (px) NM_TRY(nm_pipe_x<T>(mesh, false, fld, Hc_out, st));
+    else NM_SWITCH_M(f.M1, (launch_x<T, MM>(mesh, false, fld, Hc_out, st)));
     const int chunk = f.kt_chunk > 0 && f.kt_chunk < f.NKT ? f.kt_chunk : f.NKT;
     for (int kt0 = 0; kt0 < f.NKT; kt0 += chunk) {
         const int nkt = kt0 + chunk <= f.NKT ? chunk : f.NKT - kt0;
@@ -517,7 +519,8 @@ nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_
         NM_SWITCH_M(f.M3, (launch_z<T, MM>(mesh, kt0, nkt, st)));
         NM_SWITCH_M(f.M2, (launch_y<T, MM>(mesh, true, kt0, nkt, st)));
     }
-    NM_SWITCH_M(f.M1, (launch_x<T, MM>(mesh, true, fld, Hc_out, st)));
+    if (px) NM_TRY(nm_pipe_x<T>(mesh, true, fld, Hc_out, st));
+    else NM_SWITCH_M(f.M1, (launch_x<T, MM>(mesh, true, fld, Hc_out, st)));
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;
 }

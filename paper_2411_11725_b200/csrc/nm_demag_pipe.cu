@@ -181,6 +181,200 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
     if (tid == 0) bulk_wait<0>();
 }
 
+
+// ---- x passes ----------------------------------------------------------------------------------
+// Geometry shared by k_px_fwd / k_px_inv for N1 = 16 M: a CTA of 8 warps owns R = 2 LINES cell rows
+// (c2) of one cell plane c3; warp w transforms LINES/8 = 16/M complex lines, each packing the two
+// real rows 2 line, 2 line + 1.  The half spectrum has NKT = 2 M + 1 tiles of 8 columns.
+template <typename T, int M> struct PxGeom {
+    static constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    static constexpr int LINES = 8 * LT, R = 2 * LINES;
+    static constexpr int NKT = 2 * M + 1;
+    static constexpr int YP = N + 2;            // pitch of the y-summed node rows (row pairs)
+    static constexpr int PZ = P + 8;            // pitch of a packed spectrum line
+    static constexpr int SCR = team_scratch<T, M>();
+    static constexpr size_t FWD_BYTES = ((size_t)LINES * YP + (size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T);
+    static constexpr size_t INV_BYTES = ((size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T) + (size_t)R * N * sizeof(T);
+};
+
+template <typename V> __device__ __forceinline__ void store2(V *dst, V a, V b);
+template <> __device__ __forceinline__ void store2<float2>(float2 *dst, float2 a, float2 b)
+{
+    *reinterpret_cast<float4 *>(dst) = make_float4(a.x, a.y, b.x, b.y);
+}
+template <> __device__ __forceinline__ void store2<double2>(double2 *dst, double2 a, double2 b)
+{
+    dst[0] = a;
+    dst[1] = b;
+}
+template <typename V> __device__ __forceinline__ void load2(const V *src, V &a, V &b);
+template <> __device__ __forceinline__ void load2<float2>(const float2 *src, float2 &a, float2 &b)
+{
+    const float4 v = *reinterpret_cast<const float4 *>(src);
+    a = make_float2(v.x, v.y);
+    b = make_float2(v.z, v.w);
+}
+template <> __device__ __forceinline__ void load2<double2>(const double2 *src, double2 &a, double2 &b)
+{
+    a = src[0];
+    b = src[1];
+}
+
+// x forward (a1 + the x part of a2): M_c = Ms_c (1/8) sum of the 8 vertices, two real cell rows per
+// complex line, padded transform, untangle, blocked swizzled store A[kt][comp][c3][c2][8].
+//   phase 1  thread = node column, marches over 17 node rows adding the two planes (z) and
+//            consecutive rows (y): ys2[line][n1] = (row 2 line, row 2 line + 1)
+//   phase 2  cell value = Ms/8 (ys2[e] + ys2[e+1]) on the way into the registers; transform
+//   phase 3  Xa[k] = (Z[k] + conj Z[P-k])/2, Xb[k] = (Z[k] - conj Z[P-k])/(2i), both rows of a line
+//            by one thread, 16-byte stores
+template <typename T, int M, bool UNI>
+__global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
+k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename VT<T>::V *__restrict__ A,
+         NmGeom g, const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    typedef PxGeom<T, M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
+    extern __shared__ __align__(128) unsigned char smem[];
+    V *s_y = reinterpret_cast<V *>(smem);                   // LINES x YP
+    V *s_z = s_y + LINES * G::YP;                           // LINES x PZ
+    V *s_scr = s_z + LINES * G::PZ;
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l;
+    const int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    V *scr = s_scr + (2 * w + h) * G::SCR;
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    // Ms/8 of this thread's cells (rows 2 line, 2 line + 1; columns e = j + M t)
+    V msr[UNI ? 1 : 16];
+    if (UNI) msr[0] = mk<T>((T)0.125 * ms_uni, (T)0.125 * ms_uni);
+    else {
+        const T *mrow = Ms + ((long long)c3 * g.N2 + r0 + 2 * line) * N + j;
+#pragma unroll
+        for (int t = 0; t < 16; ++t) msr[UNI ? 0 : t] = mk<T>((T)0.125 * mrow[M * t], (T)0.125 * mrow[N + M * t]);
+    }
+    const long long plane = (long long)g.n1 * g.n2;
+    const int rg = tid / N, col = tid % N;                  // phase 1: row group (16 cell rows) and node column
+    for (int comp = 0; comp < 3; ++comp) {
+        const T *base = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + rg * 16) * g.n1;
+        {
+            T z[17];
+#pragma unroll
+            for (int r = 0; r < 17; ++r) z[r] = base[(long long)r * g.n1 + col] + base[plane + (long long)r * g.n1 + col];
+#pragma unroll
+            for (int r = 0; r < 16; r += 2)
+                s_y[(rg * 8 + (r >> 1)) * G::YP + col] = mk<T>(z[r] + z[r + 1], z[r + 1] + z[r + 2]);
+            if (tid < R) {   // last node column n1 = N
+                const T *q = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + tid) * g.n1 + N;
+                const T v = (q[0] + q[plane]) + (q[g.n1] + q[plane + g.n1]);
+                reinterpret_cast<T *>(s_y + (tid >> 1) * G::YP + N)[tid & 1] = v;
+            }
+        }
+        __syncthreads();
+        V a[16];
+        const V *yl = s_y + line * G::YP + j;
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            const V v0 = yl[M * t], v1 = yl[M * t + 1];
+            const V mm = msr[UNI ? 0 : t];
+            a[t] = mk<T>(mm.x * (v0.x + v1.x), mm.y * (v0.y + v1.y));
+        }
+        if (h) shift32<T, false>(a);
+        fft_fwd<T, M, true>(a, tw, scr, i);
+#pragma unroll
+        for (int s = 0; s < 16; ++s) s_z[line * G::PZ + 2 * slot_freq<M>(j, s) + h] = a[s];
+        __syncthreads();
+        for (int idx = tid; idx < NKT * LINES * 4; idx += kPipeThreads) {
+            const int q = idx & 3, ln = (idx >> 2) % LINES, kt = idx / (4 * LINES);
+            const int c2 = r0 + 2 * ln;
+            const int p0 = 2 * q;                           // physical slots p0, p0 + 1 of the blocked row
+            const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
+            const V *zl = s_z + ln * G::PZ;
+            V ze, zo;
+            load2(zl + (k0 & ~1), ze, zo);
+            const V za = (k0 & 1) ? zo : ze, zb = (k0 & 1) ? ze : zo;      // Z[k0], Z[k1]
+            const V ma = zl[(P - k0) & (P - 1)], mb = zl[(P - k1) & (P - 1)];
+            const T hf = (T)0.5;
+            V a0 = mk<T>(hf * (za.x + ma.x), hf * (za.y - ma.y)), b0 = mk<T>(hf * (za.y + ma.y), hf * (ma.x - za.x));
+            V a1 = mk<T>(hf * (zb.x + mb.x), hf * (zb.y - mb.y)), b1 = mk<T>(hf * (zb.y + mb.y), hf * (mb.x - zb.x));
+            if (k0 > N) { a0 = mk<T>((T)0, (T)0); b0 = a0; }
+            if (k1 > N) { a1 = mk<T>((T)0, (T)0); b1 = a1; }
+            V *dst = A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + c2) * TW + p0;
+            store2(dst, a0, a1);
+            store2(dst + TW, b0, b1);
+        }
+    }
+}
+
+// x inverse (the x part of a4): rebuild the packed spectrum Z = Xa + i Xb of two real rows from their
+// half spectra (Z[P-k] = conj Xa[k] + i conj Xb[k]), inverse transform cropped to N1, write the cell
+// field Hc[comp][c3][c2][c1] through a row-major staging tile with 16-byte stores.
+template <typename T, int M>
+__global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
+k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, const typename VT<T>::V *__restrict__ wP)
+{
+    typedef typename VT<T>::V V;
+    typedef PxGeom<T, M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
+    extern __shared__ __align__(128) unsigned char smem[];
+    V *s_z = reinterpret_cast<V *>(smem);                   // LINES x PZ
+    V *s_scr = s_z + LINES * G::PZ;
+    T *s_out = reinterpret_cast<T *>(s_scr + 16 * G::SCR);  // R x N
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i / M, j = i % M;
+    const int line = w * LT + l;
+    const int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    V *scr = s_scr + (2 * w + h) * G::SCR;
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    for (int comp = 0; comp < 3; ++comp) {
+        for (int idx = tid; idx < NKT * LINES * 4; idx += kPipeThreads) {
+            const int q = idx & 3, ln = (idx >> 2) % LINES, kt = idx / (4 * LINES);
+            const int c2 = r0 + 2 * ln;
+            const int p0 = 2 * q;
+            const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
+            const V *src = A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + c2) * TW + p0;
+            V u0, u1, v0, v1;                               // Xa[k0], Xa[k1], Xb[k0], Xb[k1]
+            load2(src, u0, u1);
+            load2(src + TW, v0, v1);
+            V *zl = s_z + ln * G::PZ;
+            if (k0 <= N) {
+                zl[k0] = mk<T>(u0.x - v0.y, u0.y + v0.x);
+                if (k0 != 0 && k0 != N) zl[P - k0] = mk<T>(u0.x + v0.y, v0.x - u0.y);
+            }
+            if (k1 <= N) {
+                zl[k1] = mk<T>(u1.x - v1.y, u1.y + v1.x);
+                if (k1 != 0 && k1 != N) zl[P - k1] = mk<T>(u1.x + v1.y, v1.x - u1.y);
+            }
+        }
+        __syncthreads();
+        V a[16];
+#pragma unroll
+        for (int s = 0; s < 16; ++s) a[s] = s_z[line * G::PZ + 2 * slot_freq<M>(j, s) + h];
+        fft_inv<T, M, true>(a, tw, scr, i);
+        if (h) shift32<T, true>(a);
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            V v = a[t];
+            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
+            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            if ((t >> 3) == h) {
+                s_out[(2 * line) * N + j + M * t] = v.x;
+                s_out[(2 * line + 1) * N + j + M * t] = v.y;
+            }
+        }
+        __syncthreads();
+        // R consecutive rows of Hc are contiguous
+        T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * N;
+        constexpr int VEC = 16 / sizeof(T);
+        for (int idx = tid; idx < R * N / VEC; idx += kPipeThreads)
+            reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[idx];
+    }
+}
+
 } // namespace
 
 // ---- host side ----------------------------------------------------------------------------------
@@ -200,3 +394,49 @@ nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
                                                         nItems, kt0, (const float2 *)mesh->tw_z);
     return NM_OK;
 }
+
+// x passes: any fast-path size with whole CTAs of R rows along y
+template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_t st)
+{
+    typedef typename VT<T>::V V;
+    typedef PxGeom<T, M> G;
+    const NmGeom &g = mesh->g;
+    const dim3 grid(g.N2 / G::R, g.N3);
+    if (!inverse) {
+        NmLaunchScope sc(mesh, NM_K_X_FWD, st);
+        if (mesh->uni_Ms) {
+            NM_CUDA_TRY(cudaFuncSetAttribute(k_px_fwd<T, M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::FWD_BYTES));
+            k_px_fwd<T, M, true><<<grid, kPipeThreads, G::FWD_BYTES, st>>>(fld, (const T *)mesh->Ms, (T)mesh->desc.Ms_scalar,
+                                                                          (V *)mesh->bufA, g, (const V *)mesh->fast.wPx);
+        } else {
+            NM_CUDA_TRY(cudaFuncSetAttribute(k_px_fwd<T, M, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::FWD_BYTES));
+            k_px_fwd<T, M, false><<<grid, kPipeThreads, G::FWD_BYTES, st>>>(fld, (const T *)mesh->Ms, (T)0, (V *)mesh->bufA, g,
+                                                                           (const V *)mesh->fast.wPx);
+        }
+    } else {
+        NmLaunchScope sc(mesh, NM_K_X_INV, st);
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_px_inv<T, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::INV_BYTES));
+        k_px_inv<T, M><<<grid, kPipeThreads, G::INV_BYTES, st>>>((const V *)mesh->bufA, Hc, g, (const V *)mesh->fast.wPx);
+    }
+    return NM_OK;
+}
+
+bool nm_pipe_x_ok(const nm_mesh *mesh)
+{
+    if (!mesh->fast.on || !mesh->fast.pipe) return false;
+    const int R = 2 * 8 * (16 / mesh->fast.M1);
+    return mesh->g.N2 % R == 0;
+}
+
+template <typename T> nm_status nm_pipe_x(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_t st)
+{
+    switch (mesh->fast.M1) {
+    case 1: return launch_px<T, 1>(mesh, inverse, fld, Hc, st);
+    case 2: return launch_px<T, 2>(mesh, inverse, fld, Hc, st);
+    case 4: return launch_px<T, 4>(mesh, inverse, fld, Hc, st);
+    case 8: return launch_px<T, 8>(mesh, inverse, fld, Hc, st);
+    default: return launch_px<T, 16>(mesh, inverse, fld, Hc, st);
+    }
+}
+template nm_status nm_pipe_x<float>(nm_mesh *, bool, const float *, float *, cudaStream_t);
+template nm_status nm_pipe_x<double>(nm_mesh *, bool, const double *, double *, cudaStream_t);

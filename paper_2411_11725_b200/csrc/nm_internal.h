@@ -158,6 +158,8 @@ nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *field_nodes, T *Hc_out, cud
 // nm_demag_pipe.cu
 bool nm_pipe_mid_ok(const nm_mesh *mesh);
 nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st);
+bool nm_pipe_x_ok(const nm_mesh *mesh);
+template <typename T> nm_status nm_pipe_x(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_t st);
 // nm_local.cu
 nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st);
 

@@ -360,6 +360,7 @@ extern "C" nm_status nm_mesh_create(nm_mesh **out, const nm_mesh_desc *desc, voi
             if ((s = set_material<float>(m, m->Ku, desc->Ku, desc->Ku_scalar, st)) != NM_OK) break;
         }
         if ((s = nm_compute_sMs(m, st)) != NM_OK) break;
+        if ((s = nm_pipe_setup(m)) != NM_OK) break;
         if (desc->terms & NM_TERM_DEMAG) {
             s = m->f64 ? setup_tables<double>(m, st) : setup_tables<float>(m, st);
             if (s != NM_OK) break;

@@ -34,7 +34,7 @@ template <typename V> __device__ __forceinline__ void copy_in(V *dst, const V *_
 // -------------------------------------------------------------------------------------------------
 // y forward.  CTA = LT consecutive c3 of one (kt, comp); 8 warps x LT lines.
 //   in : A[kt][comp][c3][c2][8]           (rows swizzled by c2)
-//   out: B[kt][ky][comp][c3][8]           (rows swizzled by c3), ky natural 0..P2-1
+//   out: B[kt][ky][comp][c3][8]           (rows swizzled by c3 and ky), ky natural 0..P2-1
 template <typename T, int M>
 __global__ void __launch_bounds__(kThreadsF)
 k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict__ B, int N3, int kt0,
@@ -74,7 +74,7 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int ky = 2 * slot_freq<M>(j, s) + h;
-        s_io[ky * OUT_PITCH + sub * TW + sl] = a[s];
+        s_io[ky * OUT_PITCH + sub * TW + (sl ^ swz(ky))] = a[s];
     }
     __syncthreads();
     // rows of LT*8 complex, one per ky
@@ -118,7 +118,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int ky = 2 * slot_freq<M>(j, s) + h;
-        a[s] = s_io[ky * PITCH + sub * TW + sl];
+        a[s] = s_io[ky * PITCH + sub * TW + (sl ^ swz(ky))];
     }
     __syncthreads();
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
@@ -174,12 +174,13 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     load_twiddles2<T, M>(tw, wP, j);
     V a[3][16];
     V *my = s_io + (sub * 3) * N * TW;
+    const int kq = k1 ^ swz(ky0 + sub);                     // rows of B are swizzled by c3 and by ky
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
             const int e = j + M * t;
-            V v = my[(c * N + e) * TW + (k1 ^ swz(e))];
+            V v = my[(c * N + e) * TW + (kq ^ swz(e))];
             if (h) v = cmul(v, wP[e]);
             a[c][t] = v;
         }
@@ -214,7 +215,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
             if (h) v = cmulc(v, wP[e]);
             v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
             v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
-            if ((t >> 3) == h) my[(c * N + e) * TW + (k1 ^ swz(e))] = v;
+            if ((t >> 3) == h) my[(c * N + e) * TW + (kq ^ swz(e))] = v;
         }
     }
     __syncthreads();
@@ -396,6 +397,7 @@ nm_status launch_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t s
     typedef typename VT<T>::V V;
     const NmGeom &g = mesh->g;
     constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    if (nm_pipe_y_ok(mesh)) return nm_pipe_y(mesh, inverse, kt0, nkt, st);
     const size_t sm = (size_t)P * (LT * TW + 1) * sizeof(V) + scratch_bytes<T>(kWarps);
     const dim3 grid(g.N3 / LT, 3, nkt);
     if (!inverse) {

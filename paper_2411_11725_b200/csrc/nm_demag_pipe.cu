@@ -100,7 +100,7 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
     load_twiddles_h<T, M>(tw, wP, j, h);
     V *scr = s_scr + w * S::WSCR + h * Team<M>::SCRATCH;
     const T *ts = s_T + w * S::TSLICE;
-    const int cwj = w ^ swz(j);          // swz(j + 16 t) = swz(j)
+    const int cw0 = w ^ swz(j);          // swz(j + 16 t) = swz(j)
     int n = 0;
     uint32_t tphase = 0;
 
@@ -110,6 +110,7 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
         for (int sub = 0; sub < nt; ++sub, ++n) {
             const int b = n % S::NBUF;
             mbar_wait(fullB + b, (uint32_t)((n / S::NBUF) & 1));
+            const int cwj = cw0 ^ swz(sub ? P2 - kyf : kyf);     // rows of B are swizzled by c3 and by ky
             V *col = s_B + b * S::TILE_ELEMS + j * TW + cwj;      // element (c, e = j + 16 t): + (c N + 16 t) TW
             V a[3][16];
 #pragma unroll
@@ -375,6 +376,158 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     }
 }
 
+
+// ---- y passes ----------------------------------------------------------------------------------
+// Tile = one (k1 tile, component, c3): the A side is a contiguous [c2 = 256][8] block (one bulk
+// copy), the B side is 512 rows of 64 bytes, one per ky, 3 N3 rows apart: a 4-D tensor map over
+// B[kt P2 + ky][comp][c3][16 floats] moves them as two boxes of 256 rows.  Persistent CTAs, two per
+// SM; thread 0 keeps the copies of the neighbouring tiles in flight around the transform.
+struct PySmem {
+    static constexpr int N = 256, P = 512;
+    static constexpr int A_ELEMS = N * TW, A_BYTES = A_ELEMS * 8;           // 16384
+    static constexpr int B_ELEMS = P * TW, B_BYTES = B_ELEMS * 8;           // 32768
+    static constexpr int SCR_BYTES = 16 * Team<16>::SCRATCH * 8;            // 35840
+    // forward: two A stages in, one B tile out; inverse: one B stage in (reloaded as soon as it is read), one A tile out
+    static constexpr int FWD_BYTES = 2 * A_BYTES + B_BYTES + SCR_BYTES + 64;
+    static constexpr int INV_BYTES = B_BYTES + A_BYTES + SCR_BYTES + 64;
+};
+
+__global__ void __launch_bounds__(kPipeThreads, 2)
+k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
+         const float2 *__restrict__ wP)
+{
+    typedef float T;
+    typedef float2 V;
+    typedef PySmem S;
+    constexpr int M = 16;
+    extern __shared__ __align__(128) unsigned char smem[];
+    V *s_out = reinterpret_cast<V *>(smem);                                 // [P][8]
+    V *s_in = reinterpret_cast<V *>(smem + S::B_BYTES);                     // 2 x [N][8]
+    V *s_scr = reinterpret_cast<V *>(smem + S::B_BYTES + 2 * S::A_BYTES);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + S::B_BYTES + 2 * S::A_BYTES + S::SCR_BYTES);
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, j = lane >> 1;
+    const int G = gridDim.x;
+    if (tid == 0) {
+        mbar_init(full, 1);
+        mbar_init(full + 1, 1);
+        mbar_fence_init();
+        tensormap_prefetch(&tmB);
+    }
+    __syncthreads();
+    // tile tl -> (ktl, comp, c3), c3 fastest: consecutive tiles are consecutive 16 KB blocks of A
+    auto a_tile = [&](int tl) -> const V * { return A + ((long long)kt0 * 3 * N3 + tl) * S::A_ELEMS; };
+    if (tid == 0) {
+        for (int q = 0; q < 2; ++q) {
+            const int tl = blockIdx.x + q * G;
+            if (tl < nTiles) {
+                mbar_expect_tx(full + q, S::A_BYTES);
+                bulk_load(s_in + q * S::A_ELEMS, a_tile(tl), S::A_BYTES, full + q);
+            }
+        }
+    }
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    const int cin = j * TW + (w ^ swz(j));                  // A rows are swizzled by c2 = e, swz(j + 16 t) = swz(j)
+    int n = 0;
+    for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
+        const int c3 = tl % N3, comp = (tl / N3) % 3, ktl = tl / (3 * N3);
+        const int b = n & 1;
+        mbar_wait(full + b, (uint32_t)((n >> 1) & 1));
+        const V *in = s_in + b * S::A_ELEMS + cin;
+        V a[16];
+#pragma unroll
+        for (int t = 0; t < 16; ++t) a[t] = in[M * t * TW];
+        __syncthreads();                                    // stage b is free again
+        if (tid == 0 && tl + 2 * G < nTiles) {
+            mbar_expect_tx(full + b, S::A_BYTES);
+            bulk_load(s_in + b * S::A_ELEMS, a_tile(tl + 2 * G), S::A_BYTES, full + b);
+        }
+        if (h) shift32<T, false>(a);
+        fft_fwd<T, M, true>(a, tw, scr, j);
+        if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
+        __syncthreads();
+        // row ky = 2 (j + 16 rev16(s)) + h, column k1 = w swizzled by c3 and ky: swz(ky) = j & 7
+        V *out = s_out + (2 * j + h) * TW + (w ^ swz(c3) ^ (j & 7));
+#pragma unroll
+        for (int s = 0; s < 16; ++s) out[32 * rev16(s) * TW] = a[s];
+        fence_async_smem();
+        __syncthreads();
+        if (tid == 0) {
+            tensor_store_4d(&tmB, s_out, 0, c3, comp, ktl * S::P);
+            tensor_store_4d(&tmB, s_out + 256 * TW, 0, c3, comp, ktl * S::P + 256);
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+__global__ void __launch_bounds__(kPipeThreads, 2)
+k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3, int nTiles, int kt0,
+         const float2 *__restrict__ wP)
+{
+    typedef float T;
+    typedef float2 V;
+    typedef PySmem S;
+    constexpr int M = 16;
+    extern __shared__ __align__(128) unsigned char smem[];
+    V *s_in = reinterpret_cast<V *>(smem);                                  // [P][8]
+    V *s_out = reinterpret_cast<V *>(smem + S::B_BYTES);                    // [N][8]
+    V *s_scr = reinterpret_cast<V *>(smem + S::B_BYTES + S::A_BYTES);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + S::B_BYTES + S::A_BYTES + S::SCR_BYTES);
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, j = lane >> 1;
+    const int G = gridDim.x;
+    if (tid == 0) {
+        mbar_init(full, 1);
+        mbar_fence_init();
+        tensormap_prefetch(&tmB);
+    }
+    __syncthreads();
+    auto load_b = [&](int tl) {
+        const int c3 = tl % N3, comp = (tl / N3) % 3, ktl = tl / (3 * N3);
+        mbar_expect_tx(full, S::B_BYTES);
+        tensor_load_4d(s_in, &tmB, 0, c3, comp, ktl * S::P, full);
+        tensor_load_4d(s_in + 256 * TW, &tmB, 0, c3, comp, ktl * S::P + 256, full);
+    };
+    if (tid == 0 && (int)blockIdx.x < nTiles) load_b(blockIdx.x);
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    const int cout = j * TW + (w ^ swz(j));
+    int n = 0;
+    for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
+        const int c3 = tl % N3;
+        mbar_wait(full, (uint32_t)(n & 1));
+        const V *in = s_in + (2 * j + h) * TW + (w ^ swz(c3) ^ (j & 7));
+        V a[16];
+#pragma unroll
+        for (int s = 0; s < 16; ++s) a[s] = in[32 * rev16(s) * TW];
+        __syncthreads();                                    // the stage is free again
+        if (tid == 0 && tl + G < nTiles) load_b(tl + G);
+        fft_inv<T, M, true>(a, tw, scr, j);
+        if (h) shift32<T, true>(a);
+        if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
+        __syncthreads();
+        V *out = s_out + cout;
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            V v = a[t];
+            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
+            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            if ((t >> 3) == h) out[M * t * TW] = v;
+        }
+        fence_async_smem();
+        __syncthreads();
+        if (tid == 0) {
+            bulk_store(A + ((long long)kt0 * 3 * N3 + tl) * S::A_ELEMS, s_out, S::A_BYTES);
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
 } // namespace
 
 // ---- host side ----------------------------------------------------------------------------------
@@ -440,3 +593,61 @@ template <typename T> nm_status nm_pipe_x(nm_mesh *mesh, bool inverse, const T *
 }
 template nm_status nm_pipe_x<float>(nm_mesh *, bool, const float *, float *, cudaStream_t);
 template nm_status nm_pipe_x<double>(nm_mesh *, bool, const double *, double *, cudaStream_t);
+
+// ---- y passes: tensor map over B and launchers ---------------------------------------------------
+#include <cuda.h>
+
+static_assert(sizeof(NmTensorMap) == sizeof(CUtensorMap), "NmTensorMap must mirror CUtensorMap");
+
+typedef CUresult (*NmEncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// B[kt][ky][comp][c3][8 complex] seen as floats [NKT P2][3][N3][16]; box = 256 ky rows of one (comp, c3)
+nm_status nm_pipe_setup(nm_mesh *mesh)
+{
+    mesh->fast.tmapB_ok = false;
+    if (!mesh->fast.on || mesh->f64 || !mesh->fast.pipe || mesh->fast.M2 != 16) return NM_OK;
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+        qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return NM_OK;                       // the non-pipelined y kernels serve instead
+    }
+    const NmGeom &g = mesh->g;
+    const cuuint64_t dims[4] = {16, (cuuint64_t)g.N3, 3, (cuuint64_t)mesh->fast.NKT * g.P2};
+    const cuuint64_t strides[3] = {64, (cuuint64_t)g.N3 * 64, (cuuint64_t)3 * g.N3 * 64};
+    const cuuint32_t box[4] = {16, 1, 1, 256};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = ((NmEncodeTiledFn)fn)((CUtensorMap *)&mesh->fast.tmapB, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, mesh->bufB,
+                                       dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        nm_set_error("cuTensorMapEncodeTiled failed with code %d", (int)r);
+        return NM_ECUDA;
+    }
+    mesh->fast.tmapB_ok = true;
+    return NM_OK;
+}
+
+bool nm_pipe_y_ok(const nm_mesh *mesh) { return mesh->fast.on && mesh->fast.pipe && mesh->fast.tmapB_ok; }
+
+nm_status nm_pipe_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st)
+{
+    const NmGeom &g = mesh->g;
+    const int nTiles = nkt * 3 * g.N3;
+    const int grid = nTiles < 2 * mesh->sm_count ? nTiles : 2 * mesh->sm_count;
+    if (!inverse) {
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_py_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::FWD_BYTES));
+        NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
+        k_py_fwd<<<grid, kPipeThreads, PySmem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3, nTiles, kt0,
+                                                              (const float2 *)mesh->tw_y);
+    } else {
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::INV_BYTES));
+        NmLaunchScope sc(mesh, NM_K_Y_INV, st);
+        k_py_inv<<<grid, kPipeThreads, PySmem::INV_BYTES, st>>>(mesh->fast.tmapB, (float2 *)mesh->bufA, g.N3, nTiles, kt0,
+                                                              (const float2 *)mesh->tw_y);
+    }
+    return NM_OK;
+}

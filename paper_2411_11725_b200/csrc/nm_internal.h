@@ -47,6 +47,11 @@ struct NmGeom {
     long long cells, nodes;
 };
 
+// Opaque copy of a CUtensorMap (128 bytes, 64-byte aligned) so that this header does not need cuda.h
+struct alignas(64) NmTensorMap {
+    unsigned char bytes[128];
+};
+
 // Fast demag path (nm_demag_fast.cu): sizes 16 M_d per axis, blocked spectrum layouts.
 struct NmFast {
     bool on;
@@ -56,6 +61,8 @@ struct NmFast {
     int Kzp;           // pitch of the |kz| axis of the tensor
     int kt_chunk;      // k1 tiles per y/z/y launch group (0 = all)
     bool pipe;         // use the persistent TMA-pipelined kernels (nm_demag_pipe.cu) where they apply
+    bool tmapB_ok;     // tmapB describes bufB (fp32, N2 = 256)
+    NmTensorMap tmapB; // 4-D tiled view of bufB for the pipelined y passes
     void *Tn;          // tensor [NKT][N2+1][8][6][Kzp] (real)
     void *wPx;         // exp(-2 pi i q / P1), q < P1
 };
@@ -158,6 +165,9 @@ nm_status nm_demag_conv_fast(nm_mesh *mesh, const T *field_nodes, T *Hc_out, cud
 // nm_demag_pipe.cu
 bool nm_pipe_mid_ok(const nm_mesh *mesh);
 nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st);
+nm_status nm_pipe_setup(nm_mesh *mesh);      // after the workspace is carved
+bool nm_pipe_y_ok(const nm_mesh *mesh);
+nm_status nm_pipe_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st);
 bool nm_pipe_x_ok(const nm_mesh *mesh);
 template <typename T> nm_status nm_pipe_x(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_t st);
 // nm_local.cu

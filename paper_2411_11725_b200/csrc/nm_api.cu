@@ -497,8 +497,9 @@ void base_args(const nm_mesh *m, double t, const nm_zeeman *z, unsigned terms, N
     const bool an_on = (terms & NM_TERM_ANISO) != 0;
     a->sep = (m->uni_A && (m->uni_Ku || !an_on)) ? 1 : 0;
     {
-        const char *env = getenv("NM_NODE_PATH");        // "generic" forces the 27-point kernel
+        const char *env = getenv("NM_NODE_PATH");        // "generic" forces the 27-point kernel, "sep" k_node_sep
         if (env && strcmp(env, "generic") == 0) a->sep = 0;
+        else if (env && strcmp(env, "sep") == 0 && a->sep) a->sep = 2;
     }
     a->cex = (terms & NM_TERM_EXCHANGE) ? (T)(16.0 * m->desc.A_scalar / NM_MU0) : (T)0;
     a->cku = an_on ? (T)(16.0 * m->desc.Ku_scalar / NM_MU0) : (T)0;

@@ -580,6 +580,7 @@ inline dim3 sep_grid(const NmGeom &g, int *zchunk)
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
 {
     const bool nodal_zee = (a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse);
+    if (a.sep == 1 && !nodal_zee && nm_node_col_ok<T>(mesh, a)) return nm_launch_node_col<T>(mesh, a, st);
     if (a.sep && !nodal_zee) {
         int zchunk;
         const dim3 grid = sep_grid(a.g, &zchunk);
@@ -606,7 +607,8 @@ int nm_node_blocks(const NmGeom &g)
     const dim3 sg = sep_grid(g, &zchunk);
     const int gen = (int)(nblk((long long)g.n1 * g.n2, kBlock) * g.n3);
     const int sep = (int)(sg.x * sg.y * sg.z);
-    return gen > sep ? gen : sep;
+    const int col = nm_node_col_blocks(g);
+    return gen > sep ? (gen > col ? gen : col) : (sep > col ? sep : col);
 }
 
 nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st)

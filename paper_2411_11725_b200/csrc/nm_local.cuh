@@ -50,7 +50,7 @@ template <typename T> struct NmLocalArgs {
     T *Q, *W, *dadt;
     NmRkArgs<T> rk;
     // separable kernel k_node_sep (uniform A and Ku, no nodal Zeeman arrays)
-    int sep;            // 1: eligible
+    int sep;            // 0: 27-point kernel; 1: separable kernels (column-marching where it applies); 2: k_node_sep only
     T cex, cku;         // 16 A / mu0 and 16 Ku / mu0 (0 when the term is off)
     T idx2[3];          // 1 / dx_d^2
     T ms_uni;           // > 0: Ms has this value in every cell; 0: read the Ms / sMs arrays
@@ -69,6 +69,10 @@ template <typename T> struct NmAdjCellArgs {
 
 // host launchers defined in nm_local.cu
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st);
+// nm_node_col.cu: column-marching form of the separable kernel (cp.async stage ring)
+template <typename T> bool nm_node_col_ok(const nm_mesh *mesh, const NmLocalArgs<T> &a);
+template <typename T> nm_status nm_launch_node_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st);
+int nm_node_col_blocks(const NmGeom &g);
 int nm_node_blocks(const NmGeom &g);   // capacity needed for the error-norm partials
 nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaStream_t st);
 template <typename T>

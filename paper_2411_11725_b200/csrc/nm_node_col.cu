@@ -1,23 +1,30 @@
 // Column-marching node kernel: a5-a11 of the hot path for uniform A and Ku.
 //
-// Same separable operators as k_node_sep (nm_local.cu):
-//     (A v)_i = [i>0] (v_i - v_{i-1}) + [i<N] (v_i - v_{i+1})                 stiffness, K1
-//     (B v)_i = [i>0] (v_i/3 + v_{i-1}/6) + [i<N] (v_i/3 + v_{i+1}/6)         mass, M1
-//     E_n   = dx^-2 (Bz By Ax m) + dy^-2 (Bz Ay Bx m) + dz^-2 (Az By Bx m)    (Eqs. 17-22, reading C2)
+// The assembled tensor-product element operators of Eqs. (17)-(22) (reading C2) factor into 1-D
+// stiffness and mass operators along each axis,
+//     (A v)_i = [i>0] (v_i - v_{i-1}) + [i<N] (v_i - v_{i+1}),
+//     (B v)_i = [i>0] (v_i/3 + v_{i-1}/6) + [i<N] (v_i/3 + v_{i+1}/6)   =   d_i v_i - (A v)_i / 6,
+// with d_i = 1 inside and 1/2 on the two end nodes (the 1-D lumped mass), and A is the plain
+// interior formula 2 v_i - v_{i-1} - v_{i+1} on data whose ghost nodes mirror the end nodes.  So
+//     E_n   = dx^-2 (Bz By Ax m) + dy^-2 (Bz Ay Bx m) + dz^-2 (Az By Bx m)
 //     H^ex  = -(16 A / (mu0 (S Ms)_n)) E_n,   H^an = (16 Ku / (mu0 (S Ms)_n)) (Bz By Bx (m.k)) k
 //     H^d_n = S(Ms o H^cell)_n / (S Ms)_n                                     (reading C5)
-// followed by the LLG products (Eq. 1), the Runge-Kutta stage combination (a10) or the adjoint
-// products (a11, reading C7).
+// needs, per plane, only ax = Ax m, ay = Ay m and axy = Ay Ax m of the 3 x 3 neighbourhood:
+//     U = dx^-2 By Ax m + dy^-2 Ay Bx m = dx^-2 dy ax + dy^-2 dx ay - (dx^-2 + dy^-2)/6 axy
+//     W = By Bx m                       = dx dy m - dy/6 ax - dx/6 ay + axy/36
+//     E_z = dz U_z + (Az R)_z,   R = dz^-2 W - U/6;      (Bz W)_z = dz W_z - (Az W)_z / 6
+// (dx, dy, dz here: the factors d of the node along each axis) and no per-neighbour boundary
+// coefficients.  The z operators are accumulated plane by plane in two partial sums per output
+// (the sum that still waits for plane k + 1, and the start of the next one), so the march carries
+// 8 registers per node and no register rotation.  Then the LLG products (Eq. 1), the
+// Runge-Kutta stage combination (a10) or the adjoint products (a11, reading C7).
 //
-// What differs is how the SM is fed.  A CTA owns RY whole node rows (all of x: one thread per
-// node column i1, so every global and shared access of a warp is a contiguous row segment) and
-// marches along z.  Whole rows are contiguous in memory, so a plane's tile -- RY + 2 node rows of
-// each component of m, RY + 1 cell rows of each component of H^cell (and of Ms) -- is a handful
-// of contiguous ranges that cp.async (zero-filling what lies outside the mesh) streams into a
-// ring of CS stages, CS - 1 planes ahead of the arithmetic: the loads of later planes are in
-// flight while the current one is combined, one CTA barrier per plane.  Each thread keeps the x
-// operators of a row in registers and reuses them for the RY rows it owns.  The epilogue is
-// compiled per mode (template), so a stage launch carries no mode branches.
+// How the SM is fed: a CTA owns RY whole node rows (one thread per node column i1, so every global
+// and shared access of a warp is a contiguous row segment) and marches along z.  A plane's tile --
+// RY + 2 node rows of each component of m with one ghost column either side, fetched at clamped
+// (mirrored) row / column indices; RY + 1 cell rows of each component of H^cell (and of Ms),
+// zero-filled outside the mesh -- is streamed by cp.async into a ring of CS stages, CS - 2 planes
+// ahead of the arithmetic, one CTA barrier per plane.  The epilogue is compiled per mode.
 #include "nm_local.cuh"
 
 namespace {
@@ -37,20 +44,6 @@ template <typename T> __device__ __forceinline__ void cross_c(const T *a, const 
 
 __device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-// one element global -> shared, or zeros when !ok (src-size 0: nothing is read)
-template <typename T> __device__ __forceinline__ void cp_elem(T *dst, const T *src, bool ok)
-{
-    const int sz = ok ? (int)sizeof(T) : 0;
-    if (sizeof(T) == 4)
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(smem_addr(dst)), "l"(src), "r"(sz) : "memory");
-    else
-        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_addr(dst)), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_16(void *dst, const void *src, bool ok)
-{
-    const int sz = ok ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_addr(dst)), "l"(src), "r"(sz) : "memory");
-}
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
@@ -69,22 +62,33 @@ __device__ __forceinline__ double block_sum_c(double v, int nthreads)
     return r;   // valid in thread 0
 }
 
+template <typename T> __device__ __forceinline__ T rcp_c(T v);
+template <> __device__ __forceinline__ float rcp_c<float>(float v) { return __fdividef(1.0f, v); }
+template <> __device__ __forceinline__ double rcp_c<double>(double v) { return 1.0 / v; }
+
 // modes of the compiled epilogues: the NmLocalMode values, with the Runge-Kutta stage split by the
 // number of earlier derivatives it combines (0: first stages of RK4; 3: last stage of RK4; else a loop)
 enum { CM_H = 0, CM_RHS, CM_RK0, CM_RK3, CM_RKN, CM_ADJ1, CM_ADJ2, CM_COUNT };
 
-// a9-a11 on one node.  mc = fld_n, sms = (S Ms)_n.
+// element n of component j of a nodal vector array (n < nodes < 2^31: one 32-bit index per node)
+template <typename P> __device__ __forceinline__ P *comp(P *base, int j, size_t nn) { return base + j * nn; }
+
+// a9-a11 on one node.  mc = fld_n, sms = (S Ms)_n, y0 = start-of-step state (Runge-Kutta modes).
 template <typename T, int CM>
-__device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n, long long nn, const T *mc,
-                                           const T *H, T sms, double &err2)
+__device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, size_t nn, const T *mc,
+                                           const T *H, T sms, const T *y0, double &err2)
 {
     if (CM == CM_H) {
-        a.out[n] = H[0]; a.out[nn + n] = H[1]; a.out[2 * nn + n] = H[2];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) comp(a.out, j, nn)[n] = H[j];
         return;
     }
     if (CM == CM_ADJ2) {
 #pragma unroll
-        for (int j = 0; j < 3; ++j) a.dadt[j * nn + n] = -(a.dadt[j * nn + n] + sms * H[j]);
+        for (int j = 0; j < 3; ++j) {
+            T *d = comp(a.dadt, j, nn) + n;
+            *d = -(*d + sms * H[j]);
+        }
         return;
     }
     T mxH[3], mxmxH[3], f[3];
@@ -93,13 +97,13 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n,
 #pragma unroll
     for (int j = 0; j < 3; ++j) f[j] = -a.gp * mxH[j] - a.agp * mxmxH[j];
     if (CM == CM_RHS) {
-        a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) comp(a.out, j, nn)[n] = f[j];
     } else if (CM == CM_RK0 || CM == CM_RK3 || CM == CM_RKN) {
         const NmRkArgs<T> &r = a.rk;
-        T y0[3], acc[3], ea[3];
+        T acc[3], ea[3];
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
-            y0[j] = r.y0[j * nn + n];
             acc[j] = r.cself * f[j];
             ea[j] = r.eself * f[j];
         }
@@ -107,7 +111,7 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n,
 #pragma unroll
             for (int q = 0; q < 3; ++q)
 #pragma unroll
-                for (int j = 0; j < 3; ++j) acc[j] += r.cprev[q] * r.kprev[q][j * nn + n];
+                for (int j = 0; j < 3; ++j) acc[j] += r.cprev[q] * comp(r.kprev[q], j, nn)[n];
         } else if (CM == CM_RKN) {
             for (int q = 0; q < r.nprev; ++q) {
                 const T *kp = r.kprev[q] + n;
@@ -121,7 +125,8 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n,
             }
         }
         if (r.kstore) {
-            r.kstore[n] = f[0]; r.kstore[nn + n] = f[1]; r.kstore[2 * nn + n] = f[2];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) comp(r.kstore, j, nn)[n] = f[j];
         }
         if (r.ynext) {
             T y[3];
@@ -131,7 +136,8 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n,
                 const T inv = rsqrt_c<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
                 y[0] *= inv; y[1] *= inv; y[2] *= inv;
             }
-            r.ynext[n] = y[0]; r.ynext[nn + n] = y[1]; r.ynext[2 * nn + n] = y[2];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) comp(r.ynext, j, nn)[n] = y[j];
         }
         if (CM == CM_RKN && r.want_err) {
 #pragma unroll
@@ -143,9 +149,10 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n,
         }
     } else {   // CM_ADJ1
         if (a.out) {
-            a.out[n] = f[0]; a.out[nn + n] = f[1]; a.out[2 * nn + n] = f[2];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) comp(a.out, j, nn)[n] = f[j];
         }
-        const T av[3] = {a.adj[n], a.adj[nn + n], a.adj[2 * nn + n]};
+        const T av[3] = {comp(a.adj, 0, nn)[n], comp(a.adj, 1, nn)[n], comp(a.adj, 2, nn)[n]};
         T mxa[3], mxmxa[3], Hxa[3], b[3];
         cross_c(mc, av, mxa);
         cross_c(mc, mxa, mxmxa);
@@ -159,37 +166,42 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, long long n,
         for (int j = 0; j < 3; ++j) {
             b[j] = a.gp * mxa[j] - a.agp * mxmxa[j];
             const T d = -a.gp * Hxa[j] - a.agp * (mH * av[j] + am * H[j] - (T)2 * aH * mc[j]);
-            a.dadt[j * nn + n] = d;
-            a.Q[j * nn + n] = b[j] * invS;
+            comp(a.dadt, j, nn)[n] = d;
+            comp(a.Q, j, nn)[n] = b[j] * invS;
             bH += b[j] * H[j];
         }
         a.W[n] = bH * invS;
     }
 }
 
-// Tile geometry (host and device agree through this struct).  Per stage and component:
-//   m tile     [PAD][(RY + 2) n1][tail]   node rows r0 - 1 .. r0 + RY, flattened (pitch n1)
-//   cell tile  [PAD][(RY + 1) N1][tail]   cell rows r0 - 1 .. r0 + RY - 1 (pitch N1); 3 of H^cell (+ 1 of Ms)
-// PAD elements in front absorb the index -1 of the first column, the tail the index +1 of the last.
+// Tile geometry (host and device agree through this struct).  Elements per stage:
+//   m tiles    3 x (RY + 2) rows x MP,  MP = n1 + 2: ghost column, n1 nodes, ghost column
+//   cell tiles [4 zeros] ncell x (RY + 1) rows x CP,  CP = N1 (rounded up to 4) + 4: N1 cells, zeros
+// The zeros are written once and never touched by the copies: they are cell -1 (the pad of the row
+// before) and cell N1 of every cell row.
 struct ColGeom {
-    int mpitch, cpitch;     // elements per component tile
-    int ncell;              // cell tiles per stage: 0 (no demag), 3 (uniform Ms) or 4
+    int MP, CP;
+    int moff_cells;         // offset of cell (row 0, column 0) of component 0 in a stage
+    int ncell;              // cell tiles per stage: 0 (no demag), 3 (uniform Ms) or 4 (+ Ms)
     int stage;              // elements per stage
     int cvec;               // 1: cell rows are copied in 16-byte pieces
+    int cchunks;            // copies per component of the cell tile
 };
-constexpr int CPAD = 4;
 
 template <typename T, int RY> __host__ __device__ inline ColGeom col_geom(const NmGeom &g, bool has_hc, bool uni_ms)
 {
     ColGeom c;
-    const int blk = ((g.n1 + 31) / 32) * 32;
-    c.mpitch = ((CPAD + (RY + 2) * g.n1 + (blk - g.n1) + 2 + 3) / 4) * 4;
-    c.cpitch = ((CPAD + (RY + 1) * g.N1 + (blk - g.N1) + 2 + 3) / 4) * 4;
+    c.MP = g.n1 + 2;
+    c.CP = ((g.N1 + 3) / 4) * 4 + 4;
+    c.moff_cells = ((3 * (RY + 2) * c.MP + 3) / 4) * 4 + 4;
     c.ncell = has_hc ? (uni_ms ? 3 : 4) : 0;
-    c.stage = 3 * c.mpitch + c.ncell * c.cpitch;
+    c.stage = c.moff_cells + c.ncell * (RY + 1) * c.CP;
     c.cvec = ((g.N1 * sizeof(T)) % 16 == 0) ? 1 : 0;
+    c.cchunks = c.cvec ? (RY + 1) * (g.N1 / (16 / (int)sizeof(T))) : (RY + 1) * g.N1;
     return c;
 }
+
+constexpr int CQ = 3;       // cell copies per thread and component (host checks cchunks <= CQ * threads)
 
 template <typename T, int RY, int CS, int CM, bool UNI_MS, int MAXT>
 __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const NmLocalArgs<T> a, int zchunk)
@@ -197,136 +209,164 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
     extern __shared__ __align__(16) unsigned char col_smem[];
     T *sm = reinterpret_cast<T *>(col_smem);
     const NmGeom &g = a.g;
-    const int n1 = g.n1, N1 = g.N1;
+    const int n1 = g.n1, n2 = g.n2, N1 = g.N1;
     const bool has_hc = a.Hc != nullptr;
     const ColGeom cg = col_geom<T, RY>(g, has_hc, UNI_MS);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int i1 = tid;
     const int r0 = blockIdx.x * RY;                       // first node row of the CTA
     const int z0 = blockIdx.y * zchunk, z1 = min(z0 + zchunk, g.n3);
-    const long long pl = (long long)n1 * g.n2, nn = g.nodes;
-    const long long cpl = (long long)N1 * g.N2;
-    const bool live = i1 < n1;
+    const unsigned pl = (unsigned)n1 * n2, cpl = (unsigned)N1 * g.N2;
+    const size_t nn = (size_t)g.nodes, nc = (size_t)g.cells;
+    const bool live = tid < n1;
+    constexpr bool RK = CM == CM_RK0 || CM == CM_RK3 || CM == CM_RKN;
 
-    // the pads are never written by the copies: make them finite once
     for (int q = tid; q < CS * cg.stage; q += nthr) sm[q] = (T)0;
     __syncthreads();
 
-    // rows of the tiles that exist in the mesh: node rows r0-1+r, r in [mlo, mhi); cell rows r0-1+r, r in [clo, chi)
-    const int mlo = r0 == 0 ? 1 : 0, mhi = min(RY + 2, g.n2 - (r0 - 1));
-    const int clo = mlo, chi = min(RY + 1, g.N2 - (r0 - 1));
-    const int mlen = (RY + 2) * n1, clen = (RY + 1) * N1;
-
-    auto issue = [&](int k, int slot) {
-        T *st = sm + slot * cg.stage;
-        const bool mv = k >= 0 && k < g.n3;
-        {
-            const T *src = a.fld + ((long long)k * g.n2 + (r0 - 1)) * n1;
-            for (int e = tid; e < mlen; e += nthr) {
-                const bool ok = mv && e >= mlo * n1 && e < mhi * n1;
-                const T *s = ok ? src + e : a.fld;
-                T *d = st + CPAD + e;
+    // ---- what this thread copies every plane (fixed offsets; only the plane base moves) ----------
+    // m: column t of every tile row <- node column clamp(t - 1) of node row clamp(r0 - 1 + r)
+    const bool mcopy = tid < n1 + 2;
+    const unsigned mx = (unsigned)min(max(tid - 1, 0), n1 - 1);
+    unsigned mrow[RY + 2];
 #pragma unroll
-                for (int j = 0; j < 3; ++j) cp_elem<T>(d + j * cg.mpitch, s + j * nn, ok);
+    for (int r = 0; r < RY + 2; ++r) mrow[r] = (unsigned)min(max(r0 - 1 + r, 0), n2 - 1) * n1 + mx;
+    // cells: piece e = tid + q nthr of the (RY + 1) x N1 rows, zero-filled where the row does not exist
+    unsigned csrc[CQ], cdst[CQ];
+    bool cok[CQ], cdo[CQ];
+    {
+        const int V = cg.cvec ? 16 / (int)sizeof(T) : 1;
+        const int per_row = N1 / V;
+#pragma unroll
+        for (int q = 0; q < CQ; ++q) {
+            const int e = tid + q * nthr;
+            const int row = e / per_row, ch = e - row * per_row;
+            const int c2 = r0 - 1 + row;
+            cdo[q] = has_hc && e < cg.cchunks;
+            cok[q] = cdo[q] && c2 >= 0 && c2 < g.N2;
+            csrc[q] = cok[q] ? (unsigned)c2 * N1 + ch * V : 0u;
+            cdst[q] = (unsigned)(cg.moff_cells + row * cg.CP + ch * V);
+        }
+    }
+    const unsigned sm_base = smem_addr(sm);
+    auto issue = [&](int k, int slot) {
+        const unsigned sbase = sm_base + (unsigned)(slot * cg.stage) * (unsigned)sizeof(T);
+        if (mcopy) {
+            const unsigned kc = (unsigned)min(max(k, 0), g.n3 - 1) * pl;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                const T *src = comp(a.fld, j, nn) + kc;
+#pragma unroll
+                for (int r = 0; r < RY + 2; ++r) {
+                    const unsigned d = sbase + (unsigned)((j * (RY + 2) + r) * cg.MP + tid) * (unsigned)sizeof(T);
+                    if (sizeof(T) == 4)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(src + mrow[r]) : "memory");
+                    else
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(src + mrow[r]) : "memory");
+                }
             }
         }
         if (has_hc) {
             const bool cv = k - 1 >= 0 && k - 1 < g.N3;
-            const long long cbase = ((long long)(k - 1) * g.N2 + (r0 - 1)) * N1;
-            T *dc = st + 3 * cg.mpitch + CPAD;
-            if (cg.cvec) {
-                constexpr int V = 16 / sizeof(T);
-                for (int e = tid * V; e < clen; e += nthr * V) {
-                    const bool ok = cv && e >= clo * N1 && e < chi * N1;
-                    const long long off = ok ? cbase + e : 0;
+            const unsigned kc = cv ? (unsigned)(k - 1) * cpl : 0u;
 #pragma unroll
-                    for (int j = 0; j < 3; ++j) cp_16(dc + j * cg.cpitch + e, a.Hc + j * g.cells + off, ok);
-                    if (!UNI_MS) cp_16(dc + 3 * cg.cpitch + e, a.Ms + off, ok);
-                }
-            } else {
-                for (int e = tid; e < clen; e += nthr) {
-                    const bool ok = cv && e >= clo * N1 && e < chi * N1;
-                    const long long off = ok ? cbase + e : 0;
+            for (int q = 0; q < CQ; ++q) {
+                if (!cdo[q]) continue;
+                const int sz = (cv && cok[q]) ? (cg.cvec ? 16 : (int)sizeof(T)) : 0;
 #pragma unroll
-                    for (int j = 0; j < 3; ++j) cp_elem<T>(dc + j * cg.cpitch + e, a.Hc + j * g.cells + off, ok);
-                    if (!UNI_MS) cp_elem<T>(dc + 3 * cg.cpitch + e, a.Ms + off, ok);
+                for (int j = 0; j < 4; ++j) {
+                    if (j == 3 && UNI_MS) continue;
+                    const T *src = (j < 3 ? comp(a.Hc, j, nc) : a.Ms) + kc + csrc[q];
+                    const unsigned d = sbase + (cdst[q] + (unsigned)(j * (RY + 1) * cg.CP)) * (unsigned)sizeof(T);
+                    if (cg.cvec)
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+                    else if (sizeof(T) == 4)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
+                    else
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(src), "r"(sz) : "memory");
                 }
             }
         }
     };
 
-    // 1-D coefficients of this node column and of the RY rows
-    const T third = (T)(1.0 / 3.0), sixth = (T)(1.0 / 6.0);
-    const T eL = i1 > 0 ? (T)1 : (T)0, eR = i1 < N1 ? (T)1 : (T)0;
-    const T bx0 = (eL + eR) * third, bxL = eL * sixth, bxR = eR * sixth;
-    T fL[RY], fR[RY];
+    // ---- per-thread constants -------------------------------------------------------------------------
+    // lumped 1-D mass factors of this node column and of the RY rows (1 inside, 1/2 at the two ends;
+    // an axis with a single node never occurs: N_d >= 1)
+    const T dxf = (tid > 0 && tid < N1) ? (T)1 : (T)0.5;
+    const T sixth = (T)(1.0 / 6.0);
+    const T c3 = (a.idx2[0] + a.idx2[1]) * sixth;
+    const T cUy = a.idx2[1] * dxf, cWy = dxf * sixth;
+    T dyf[RY], inv_xy[RY];
     bool rowlive[RY];
 #pragma unroll
     for (int ry = 0; ry < RY; ++ry) {
         const int i2 = r0 + ry;
-        fL[ry] = i2 > 0 ? (T)1 : (T)0;
-        fR[ry] = i2 < g.N2 ? (T)1 : (T)0;
-        rowlive[ry] = live && i2 < g.n2;
+        dyf[ry] = (i2 > 0 && i2 < g.N2) ? (T)1 : (T)0.5;
+        rowlive[ry] = live && i2 < n2;
+        inv_xy[ry] = UNI_MS ? (T)1 / (a.ms_uni * (T)4 * dxf * dyf[ry]) : (T)0;   // 1 / (S Ms) up to the z factor
     }
+    const T cT = UNI_MS ? a.ms_uni : (T)1;
 
-    T Um[RY][3], U0[RY][3], Wm[RY][3], W0[RY][3], T0[RY][3], mc0[RY][3];
+    // partial sums of the z operators: P waits for the next plane, M starts the output after it
+    T GP[RY][3], GM[RY][3], aP[RY], aM[RY];
 #pragma unroll
-    for (int ry = 0; ry < RY; ++ry)
+    for (int ry = 0; ry < RY; ++ry) {
+        aP[ry] = aM[ry] = (T)0;
 #pragma unroll
-        for (int j = 0; j < 3; ++j) Um[ry][j] = U0[ry][j] = Wm[ry][j] = W0[ry][j] = T0[ry][j] = mc0[ry][j] = (T)0;
+        for (int j = 0; j < 3; ++j) GP[ry][j] = GM[ry][j] = (T)0;
+    }
     double err2 = 0.0;
 
-    const int kstart = max(z0 - 1, 0), kend = z1;         // kend may be n3 (no such plane: zeros)
+    const int kstart = max(z0 - 1, 0), kend = z1;         // plane kend = n3 is fetched clamped and weighted 0
 #pragma unroll
-    for (int s = 0; s < CS - 1; ++s) {
+    for (int s = 0; s < CS - 2; ++s) {
         if (kstart + s <= kend) issue(kstart + s, s);
         cp_commit();
     }
     int slot = 0;
-    for (int k = kstart; k <= kend; ++k) {
-        cp_wait<CS - 2>();
+    unsigned nbase = (unsigned)(kstart - 1) * pl + (unsigned)r0 * n1 + tid;    // node (z = k - 1, row r0, column tid); unused while z < 0
+    for (int k = kstart; k <= kend; ++k, nbase += pl) {
+        cp_wait<CS - 3>();
         __syncthreads();
         {
-            const int kn = k + CS - 1;
-            int sn = slot + CS - 1;
+            const int kn = k + CS - 2;
+            int sn = slot + CS - 2;
             if (sn >= CS) sn -= CS;
             if (kn <= kend) issue(kn, sn);
             cp_commit();
         }
+        const int z = k - 1;
+        const bool zout = z >= z0 && z < z1;
+        // start-of-step state for the stage combination: loaded now, used after the plane arithmetic
+        T y0[RY][3];
+        if (RK && zout) {
+#pragma unroll
+            for (int ry = 0; ry < RY; ++ry)
+#pragma unroll
+                for (int j = 0; j < 3; ++j)
+                    y0[ry][j] = rowlive[ry] ? comp(a.rk.y0, j, nn)[nbase + ry * n1] : (T)0;
+        }
+        // plane-uniform z coefficients: plane k is the centre of output k, the upper neighbour of
+        // output k - 1 and the lower neighbour of output k + 1
+        const T gLk = k > 0 ? (T)1 : (T)0, gRk = k < g.N3 ? (T)1 : (T)0;      // of output k
+        const T gRm = (k - 1 < g.N3) ? (T)1 : (T)0;                           // gR of output k - 1
+        const T gLp = (T)1;                                                   // gL of output k + 1
+        const T dzk = (T)0.5 * (gLk + gRk);
+        const T eR_out = a.cex * gRm;                     // -cex * (-gR R_k)
+        const T eU_P = -a.cex * dzk, eR_P = -a.cex * (gLk + gRk);
+        const T eR_M = a.cex * gLp;
+        const T wR_out = gRm * sixth, w_P = dzk - (gLk + gRk) * sixth, w_M = gLp * sixth;
         const T *st = sm + slot * cg.stage;
-        T Up[RY][3], Wp[RY][3], Tn[RY][3], mcn[RY][3];
         if (live) {
-#pragma unroll
-            for (int j = 0; j < 3; ++j) {
-                const T *t = st + j * cg.mpitch + CPAD + i1;
-                T P[RY + 2], Q[RY + 2];
-#pragma unroll
-                for (int r = 0; r < RY + 2; ++r) {
-                    const T *row = t + r * n1;
-                    const T l = row[-1], c = row[0], rr = row[1];
-                    Q[r] = eL * (c - l) + eR * (c - rr);
-                    P[r] = bx0 * c + bxL * l + bxR * rr;
-                    if (r >= 1 && r <= RY) mcn[r - 1][j] = c;
-                }
-#pragma unroll
-                for (int ry = 0; ry < RY; ++ry) {
-                    const T by0 = (fL[ry] + fR[ry]) * third, byL = fL[ry] * sixth, byR = fR[ry] * sixth;
-                    const T AyP = fL[ry] * (P[ry + 1] - P[ry]) + fR[ry] * (P[ry + 1] - P[ry + 2]);
-                    const T ByQ = by0 * Q[ry + 1] + byL * Q[ry] + byR * Q[ry + 2];
-                    Wp[ry][j] = by0 * P[ry + 1] + byL * P[ry] + byR * P[ry + 2];
-                    Up[ry][j] = a.idx2[0] * ByQ + a.idx2[1] * AyP;
-                }
-            }
+            T Tn[RY][3];
             if (has_hc) {
-                const T *cb = st + 3 * cg.mpitch + CPAD + i1;
-                T wl_[RY + 1], wr_[RY + 1];                // x weights of the two cells of a row (eL, eR, times Ms)
+                const T *cb = st + cg.moff_cells + tid;
+                T ml[RY + 1], mr[RY + 1];
+                if (!UNI_MS) {
 #pragma unroll
-                for (int cr = 0; cr < RY + 1; ++cr) {
-                    if (UNI_MS) { wl_[cr] = eL; wr_[cr] = eR; }
-                    else {
-                        const T *mrow = cb + 3 * cg.cpitch + cr * N1;
-                        wl_[cr] = eL * mrow[-1];
-                        wr_[cr] = eR * mrow[0];
+                    for (int cr = 0; cr < RY + 1; ++cr) {
+                        const T *mrow_ = cb + (3 * (RY + 1) + cr) * cg.CP;
+                        ml[cr] = mrow_[-1];
+                        mr[cr] = mrow_[0];
                     }
                 }
 #pragma unroll
@@ -334,53 +374,85 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                     T X[RY + 1];
 #pragma unroll
                     for (int cr = 0; cr < RY + 1; ++cr) {
-                        const T *crow = cb + j * cg.cpitch + cr * N1;
-                        X[cr] = wl_[cr] * crow[-1] + wr_[cr] * crow[0];
+                        const T *crow = cb + (j * (RY + 1) + cr) * cg.CP;
+                        X[cr] = UNI_MS ? crow[-1] + crow[0] : ml[cr] * crow[-1] + mr[cr] * crow[0];
                     }
 #pragma unroll
-                    for (int ry = 0; ry < RY; ++ry) Tn[ry][j] = fL[ry] * X[ry] + fR[ry] * X[ry + 1];
+                    for (int ry = 0; ry < RY; ++ry) Tn[ry][j] = cT * (X[ry] + X[ry + 1]);
                 }
             } else {
 #pragma unroll
                 for (int ry = 0; ry < RY; ++ry) Tn[ry][0] = Tn[ry][1] = Tn[ry][2] = (T)0;
             }
-        }
-        const int z = k - 1;
-        if (z >= z0 && z < z1) {
-            const T gL = z > 0 ? (T)1 : (T)0, gR = z < g.N3 ? (T)1 : (T)0;
-            const T bz0 = (gL + gR) * third, bzL = gL * sixth, bzR = gR * sixth;
+            T wk[RY];
 #pragma unroll
-            for (int ry = 0; ry < RY; ++ry) {
-                if (!rowlive[ry]) continue;
-                const long long n = (long long)z * pl + (long long)(r0 + ry) * n1 + i1;
-                const T sms = UNI_MS ? a.ms_uni * (eL + eR) * (fL[ry] + fR[ry]) * (gL + gR) : a.sMs[n];
-                T H[3] = {0, 0, 0};
-                if (sms > 0) {
-                    const T inv = (T)1 / sms;
-                    T an = 0;
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) an += a.kax[j] * (bz0 * W0[ry][j] + bzL * Wm[ry][j] + bzR * Wp[ry][j]);
-                    const T dsc = UNI_MS ? a.ms_uni * inv : inv;       // demag average weight
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) {
-                        const T E = (bz0 * U0[ry][j] + bzL * Um[ry][j] + bzR * Up[ry][j]) +
-                                    a.idx2[2] * (gL * (W0[ry][j] - Wm[ry][j]) + gR * (W0[ry][j] - Wp[ry][j]));
-                        T hv = (a.cku * an * a.kax[j] - a.cex * E) * inv + (T0[ry][j] + Tn[ry][j]) * dsc;
-                        if (a.terms & NM_TERM_ZEEMAN) hv += a.hu[j];
-                        H[j] = hv;
-                    }
-                }
-                epilogue_c<T, CM>(a, n, nn, mc0[ry], H, sms, err2);
-            }
-        }
-#pragma unroll
-        for (int ry = 0; ry < RY; ++ry)
+            for (int ry = 0; ry < RY; ++ry) wk[ry] = (T)0;
+            T Gout[RY][3];
 #pragma unroll
             for (int j = 0; j < 3; ++j) {
-                Um[ry][j] = U0[ry][j]; U0[ry][j] = Up[ry][j];
-                Wm[ry][j] = W0[ry][j]; W0[ry][j] = Wp[ry][j];
-                T0[ry][j] = Tn[ry][j]; mc0[ry][j] = mcn[ry][j];
+                const T *t = st + j * (RY + 2) * cg.MP + tid;     // columns tid, tid + 1, tid + 2 = i1 - 1, i1, i1 + 1
+                T c[RY + 2], sx[RY + 2];
+#pragma unroll
+                for (int r = 0; r < RY + 2; ++r) {
+                    const T *row = t + r * cg.MP;
+                    c[r] = row[1];
+                    sx[r] = row[0] + row[2];
+                }
+#pragma unroll
+                for (int ry = 0; ry < RY; ++ry) {
+                    const T cc = c[ry + 1];
+                    const T ax = (T)2 * cc - sx[ry + 1];
+                    const T ay = (T)2 * cc - (c[ry] + c[ry + 2]);
+                    const T axy = (T)2 * (ax + ay) - (T)4 * cc + (sx[ry] + sx[ry + 2]);
+                    const T U = (a.idx2[0] * dyf[ry]) * ax + cUy * ay - c3 * axy;
+                    const T W = dxf * (dyf[ry] * cc) - (dyf[ry] * sixth) * ax - cWy * ay + (T)(1.0 / 36.0) * axy;
+                    const T R = a.idx2[2] * W - sixth * U;
+                    wk[ry] += a.kax[j] * W;
+                    Gout[ry][j] = GP[ry][j] + eR_out * R + Tn[ry][j];
+                    GP[ry][j] = GM[ry][j] + eU_P * U + eR_P * R + Tn[ry][j];
+                    GM[ry][j] = eR_M * R;
+                }
             }
+            T aout[RY];
+#pragma unroll
+            for (int ry = 0; ry < RY; ++ry) {
+                aout[ry] = aP[ry] + wR_out * wk[ry];
+                aP[ry] = aM[ry] + w_P * wk[ry];
+                aM[ry] = w_M * wk[ry];
+            }
+            if (zout) {
+                const T gLz = z > 0 ? (T)1 : (T)0;
+                const T izf = (z > 0 && z < g.N3) ? (T)0.5 : (T)1;             // 1 / (gL + gR) of output z
+                int sp = slot - 1;
+                if (sp < 0) sp += CS;
+                const T *sprev = sm + sp * cg.stage + tid + 1;                // centre column of plane z
+#pragma unroll
+                for (int ry = 0; ry < RY; ++ry) {
+                    if (!rowlive[ry]) continue;
+                    const unsigned n = nbase + ry * n1;
+                    T mc[3];
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) mc[j] = sprev[(j * (RY + 2) + ry + 1) * cg.MP];
+                    T sms, inv;
+                    if (UNI_MS) {
+                        inv = inv_xy[ry] * izf;
+                        sms = (CM == CM_ADJ1 || CM == CM_ADJ2) ? a.ms_uni * (T)4 * dxf * dyf[ry] * (gLz + gRm) : (T)1;
+                    } else {
+                        sms = a.sMs[n];
+                        inv = sms > 0 ? rcp_c<T>(sms) : (T)0;
+                    }
+                    T H[3];
+                    const T ak = a.cku * aout[ry];
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) {
+                        T hv = (ak * a.kax[j] + Gout[ry][j]) * inv;
+                        if (a.terms & NM_TERM_ZEEMAN) hv += a.hu[j];
+                        H[j] = (UNI_MS || sms > 0) ? hv : (T)0;
+                    }
+                    epilogue_c<T, CM>(a, n, nn, mc, H, sms, y0[ry], err2);
+                }
+            }
+        }
         if (++slot == CS) slot = 0;
     }
     cp_wait<0>();
@@ -397,6 +469,7 @@ constexpr int kMaxT = 320;
 template <typename T> struct ColStages { static constexpr int CS = sizeof(T) == 8 ? 3 : 4; };
 
 inline int col_zchunk(const NmGeom &g) { return g.n3 <= 40 ? g.n3 : 32; }
+inline int col_threads(const NmGeom &g) { return ((g.n1 + 2 + 31) / 32) * 32; }
 
 template <typename T, int CM, bool UNI_MS>
 nm_status launch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
@@ -407,13 +480,12 @@ nm_status launch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
     const size_t bytes = (size_t)CS * cg.stage * sizeof(T);
     const int zchunk = col_zchunk(g);
     const dim3 grid((g.n2 + kRY - 1) / kRY, (g.n3 + zchunk - 1) / zchunk);
-    const int threads = ((g.n1 + 31) / 32) * 32;
     auto kern = k_node_col<T, kRY, CS, CM, UNI_MS, kMaxT>;
     NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     mesh->last_partials = (int)(grid.x * grid.y);
     {
         NmLaunchScope sc(mesh, NM_K_NODE, st);
-        kern<<<grid, threads, bytes, st>>>(a, zchunk);
+        kern<<<grid, col_threads(g), bytes, st>>>(a, zchunk);
     }
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;
@@ -436,15 +508,17 @@ template <typename T, bool UNI_MS> nm_status dispatch_col(nm_mesh *mesh, const N
 } // namespace
 
 // Eligibility: the separable operators (uniform A, Ku; no nodal Zeeman arrays -- decided by the
-// caller), a thread per node column, and a ring of stages that fits the shared memory of an SM.
+// caller), a thread per node column plus the two ghost columns, 32-bit node indices, and a ring of
+// stages that fits the shared memory of an SM (two CTAs per SM in fp32).
 template <typename T> bool nm_node_col_ok(const nm_mesh *mesh, const NmLocalArgs<T> &a)
 {
-    const NmGeom &g = a.g;
-    if (g.n1 < 96 || g.n1 > kMaxT) return false;
-    const ColGeom cg = col_geom<T, kRY>(g, a.Hc != nullptr, a.ms_uni > 0);
-    const size_t bytes = (size_t)ColStages<T>::CS * cg.stage * sizeof(T);
     (void)mesh;
+    const NmGeom &g = a.g;
+    if (g.n1 < 96 || g.n1 + 2 > kMaxT || g.nodes >= (1ll << 31)) return false;
+    const ColGeom cg = col_geom<T, kRY>(g, a.Hc != nullptr, a.ms_uni > 0);
+    if (cg.cchunks > CQ * col_threads(g)) return false;
     if (cg.cvec && a.Hc && ((((uintptr_t)a.Hc) | ((uintptr_t)a.Ms)) & 15)) return false;   // 16-byte cell copies
+    const size_t bytes = (size_t)ColStages<T>::CS * cg.stage * sizeof(T);
     return bytes <= (sizeof(T) == 8 ? 200u : 110u) * 1024u;
 }
 

@@ -73,7 +73,8 @@ enum { CM_H = 0, CM_RHS, CM_RK0, CM_RK3, CM_RKN, CM_ADJ1, CM_ADJ2, CM_COUNT };
 // element n of component j of a nodal vector array (n < nodes < 2^31: one 32-bit index per node)
 template <typename P> __device__ __forceinline__ P *comp(P *base, int j, size_t nn) { return base + j * nn; }
 
-// a9-a11 on one node.  mc = fld_n, sms = (S Ms)_n, y0 = start-of-step state (Runge-Kutta modes).
+// a9-a11 on one node.  mc = fld_n, sms = (S Ms)_n; y0 = what the mode reads at this node, loaded
+// before the plane arithmetic: the start-of-step state (Runge-Kutta), a (ADJ1) or d (ADJ2).
 template <typename T, int CM>
 __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, size_t nn, const T *mc,
                                            const T *H, T sms, const T *y0, double &err2)
@@ -85,10 +86,7 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
     }
     if (CM == CM_ADJ2) {
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            T *d = comp(a.dadt, j, nn) + n;
-            *d = -(*d + sms * H[j]);
-        }
+        for (int j = 0; j < 3; ++j) comp(a.dadt, j, nn)[n] = -(y0[j] + sms * H[j]);
         return;
     }
     T mxH[3], mxmxH[3], f[3];
@@ -152,7 +150,7 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
 #pragma unroll
             for (int j = 0; j < 3; ++j) comp(a.out, j, nn)[n] = f[j];
         }
-        const T av[3] = {comp(a.adj, 0, nn)[n], comp(a.adj, 1, nn)[n], comp(a.adj, 2, nn)[n]};
+        const T av[3] = {y0[0], y0[1], y0[2]};
         T mxa[3], mxmxa[3], Hxa[3], b[3];
         cross_c(mc, av, mxa);
         cross_c(mc, mxa, mxmxa);
@@ -336,14 +334,16 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
         }
         const int z = k - 1;
         const bool zout = z >= z0 && z < z1;
-        // start-of-step state for the stage combination: loaded now, used after the plane arithmetic
+        // what the epilogue reads at its nodes (start-of-step state, a, or d): loaded now, used after
+        // the plane arithmetic
         T y0[RY][3];
-        if (RK && zout) {
+        if ((RK || CM == CM_ADJ1 || CM == CM_ADJ2) && zout) {
+            const T *pre = RK ? a.rk.y0 : (CM == CM_ADJ1 ? a.adj : a.dadt);
 #pragma unroll
             for (int ry = 0; ry < RY; ++ry)
 #pragma unroll
                 for (int j = 0; j < 3; ++j)
-                    y0[ry][j] = rowlive[ry] ? comp(a.rk.y0, j, nn)[nbase + ry * n1] : (T)0;
+                    y0[ry][j] = rowlive[ry] ? comp(pre, j, nn)[nbase + ry * n1] : (T)0;
         }
         // plane-uniform z coefficients: plane k is the centre of output k, the upper neighbour of
         // output k - 1 and the lower neighbour of output k + 1

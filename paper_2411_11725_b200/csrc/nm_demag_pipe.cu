@@ -195,7 +195,9 @@ template <typename T, int M> struct PxGeom {
     static constexpr int PZ = P + 8;            // pitch of a packed spectrum line
     static constexpr int SCR = team_scratch<T, M>();
     static constexpr size_t FWD_BYTES = ((size_t)LINES * YP + (size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T);
-    static constexpr size_t INV_BYTES = ((size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T) + (size_t)R * N * sizeof(T);
+    // packed lines (the output tile of R x N reals aliases them) + exchange scratch + staged spectrum rows
+    static constexpr size_t INV_BYTES = ((size_t)LINES * PZ + 16 * SCR + (size_t)NKT * R * 8) * 2 * sizeof(T);
+    static_assert((size_t)R * N <= (size_t)LINES * PZ * 2, "output tile must fit the packed-line buffer");
 };
 
 template <typename V> __device__ __forceinline__ void store2(V *dst, V a, V b);
@@ -312,6 +314,10 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
 // x inverse (the x part of a4): rebuild the packed spectrum Z = Xa + i Xb of two real rows from their
 // half spectra (Z[P-k] = conj Xa[k] + i conj Xb[k]), inverse transform cropped to N1, write the cell
 // field Hc[comp][c3][c2][c1] through a row-major staging tile with 16-byte stores.
+// The spectrum rows of a component are NKT contiguous blocks of R rows x 8 columns; cp.async brings
+// the blocks of component c + 1 into a raw staging buffer while component c is transformed and
+// stored, so the global-load latency of a CTA is hidden behind its own arithmetic (the output tile
+// aliases the packed-line buffer, which keeps two CTAs per SM in fp32).
 template <typename T, int M>
 __global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
 k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, const typename VT<T>::V *__restrict__ wP)
@@ -320,9 +326,10 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     typedef PxGeom<T, M> G;
     constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
     extern __shared__ __align__(128) unsigned char smem[];
-    V *s_z = reinterpret_cast<V *>(smem);                   // LINES x PZ
+    V *s_z = reinterpret_cast<V *>(smem);                   // LINES x PZ; the output tile R x N (reals) aliases it
+    T *s_out = reinterpret_cast<T *>(smem);
     V *s_scr = s_z + LINES * G::PZ;
-    T *s_out = reinterpret_cast<T *>(s_scr + 16 * G::SCR);  // R x N
+    V *s_raw = s_scr + 16 * G::SCR;                         // NKT x R x 8 staged spectrum rows of one component
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
@@ -331,13 +338,26 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     V *scr = s_scr + (2 * w + h) * G::SCR;
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
+    constexpr int PIECES = R * TW * (int)sizeof(V) / 16;    // 16-byte pieces per block
+    auto stage = [&](int comp) {
+        for (int e = tid; e < NKT * PIECES; e += kPipeThreads) {
+            const int kt = e / PIECES, off = e - kt * PIECES;
+            const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW) + off * 16;
+            const unsigned dst = smem_u32(reinterpret_cast<char *>(s_raw) + e * 16);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    stage(0);
     for (int comp = 0; comp < 3; ++comp) {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                                    // staged rows visible; the output tile has been read
         for (int idx = tid; idx < NKT * LINES * 4; idx += kPipeThreads) {
             const int q = idx & 3, ln = (idx >> 2) % LINES, kt = idx / (4 * LINES);
             const int c2 = r0 + 2 * ln;
             const int p0 = 2 * q;
             const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
-            const V *src = A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + c2) * TW + p0;
+            const V *src = s_raw + (kt * R + 2 * ln) * TW + p0;
             V u0, u1, v0, v1;                               // Xa[k0], Xa[k1], Xb[k0], Xb[k1]
             load2(src, u0, u1);
             load2(src + TW, v0, v1);
@@ -351,10 +371,12 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
                 if (k1 != 0 && k1 != N) zl[P - k1] = mk<T>(u1.x + v1.y, v1.x - u1.y);
             }
         }
-        __syncthreads();
+        __syncthreads();                                    // packed lines complete; the staging buffer is free
+        if (comp < 2) stage(comp + 1);
         V a[16];
 #pragma unroll
         for (int s = 0; s < 16; ++s) a[s] = s_z[line * G::PZ + 2 * slot_freq<M>(j, s) + h];
+        __syncthreads();                                    // the lines are in registers: the output tile may overwrite them
         fft_inv<T, M, true>(a, tw, scr, i);
         if (h) shift32<T, true>(a);
 #pragma unroll
@@ -578,6 +600,7 @@ bool nm_pipe_x_ok(const nm_mesh *mesh)
 {
     if (!mesh->fast.on || !mesh->fast.pipe) return false;
     const int R = 2 * 8 * (16 / mesh->fast.M1);
+    if (mesh->f64 && mesh->fast.M1 == 1) return false;      // the staged inverse would need more than 227 KB
     return mesh->g.N2 % R == 0;
 }
 

@@ -132,9 +132,13 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
             const T sy = sub ? (T)-1 : (T)1;
 #pragma unroll
             for (int s = 0; s < 16; ++s) {
+                // kz = 2 j + 32 rev16(s) + h: which side of the fold it lies on is fixed by the slot,
+                // except for the slot that straddles kz = N
+                const int rs = rev16(s);
                 const int kz = 2 * slot_freq<M>(j, s) + h;
-                const int kzf = kz <= N ? kz : P - kz;
-                const T sz = kz <= N ? (T)1 : (T)-1;
+                const bool up = rs > 8 || (rs == 8 && (j | h) != 0);
+                const int kzf = up ? P - kz : kz;
+                const T sz = up ? (T)-1 : (T)1;
                 const T *tp = ts + kzf;
                 const T nxx = tp[0], nyy = tp[S::KZP], nzz = tp[2 * S::KZP];
                 const T nxy = sy * tp[3 * S::KZP], nxz = sz * tp[4 * S::KZP], nyz = sy * sz * tp[5 * S::KZP];
@@ -343,7 +347,10 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
         for (int e = tid; e < NKT * PIECES; e += kPipeThreads) {
             const int kt = e / PIECES, off = e - kt * PIECES;
             const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW) + off * 16;
-            const unsigned dst = smem_u32(reinterpret_cast<char *>(s_raw) + e * 16);
+            // fp32: the two rows of every second line swap places, so that the 16-byte reads of a
+            // quarter warp below (rows 2 ln of two lines) fall into different halves of the banks
+            const int es = sizeof(V) == 8 ? e ^ (((e >> 3) & 1) << 2) : e;
+            const unsigned dst = smem_u32(reinterpret_cast<char *>(s_raw) + es * 16);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
@@ -357,10 +364,11 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             const int c2 = r0 + 2 * ln;
             const int p0 = 2 * q;
             const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
+            const int sw = sizeof(V) == 8 ? (ln & 1) : 0;
             const V *src = s_raw + (kt * R + 2 * ln) * TW + p0;
             V u0, u1, v0, v1;                               // Xa[k0], Xa[k1], Xb[k0], Xb[k1]
-            load2(src, u0, u1);
-            load2(src + TW, v0, v1);
+            load2(src + sw * TW, u0, u1);
+            load2(src + (1 - sw) * TW, v0, v1);
             V *zl = s_z + ln * G::PZ;
             if (k0 <= N) {
                 zl[k0] = mk<T>(u0.x - v0.y, u0.y + v0.x);

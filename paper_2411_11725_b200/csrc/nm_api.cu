@@ -554,30 +554,28 @@ nm_status eval_stage(nm_mesh *m, double t, const T *fld, const nm_zeeman *z, con
 template <typename T>
 nm_status rk4_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z, int renorm, cudaStream_t st)
 {
-    T *K0 = (T *)m->K[0], *K1 = (T *)m->K[1], *K2 = (T *)m->K[2];
-    T *Y0 = (T *)m->Y[0], *Y1 = (T *)m->Y[1];
+    // Classical RK4 without stored derivatives: the stage states carry them,
+    //   Y0 = y + dt/2 k1,  Y1 = y + dt/2 k2,  Y2 = y + dt k3
+    //   y + dt/6 (k1 + 2 k2 + 2 k3 + k4) = -1/3 y + 1/3 Y0 + 2/3 Y1 + 1/3 Y2 + dt/6 k4,
+    // so a stage writes one nodal vector and the last one reads y, Y0, Y1 (Y2 is its own input).
+    T *Y0 = (T *)m->Y[0], *Y1 = (T *)m->Y[1], *Y2 = (T *)m->K[0];
     NmRkArgs<T> r;
     memset(&r, 0, sizeof(r));
     r.y0 = y;
     r.dt = (T)dt;
-    // k1 = f(t, y);  Y0 = y + dt/2 k1
-    r.kstore = K0; r.nprev = 0; r.cself = (T)0.5; r.ynext = Y0;
+    r.cself = (T)0.5; r.ynext = Y0;
     NM_TRY(eval_stage<T>(m, t, y, z, r, st));
-    // k2 = f(t + dt/2, Y0);  Y1 = y + dt/2 k2
-    r.kstore = K1; r.ynext = Y1;
+    r.ynext = Y1;
     NM_TRY(eval_stage<T>(m, t + 0.5 * dt, Y0, z, r, st));
-    // k3 = f(t + dt/2, Y1);  Y0 = y + dt k3
-    r.kstore = K2; r.cself = (T)1; r.ynext = Y0;
+    r.cself = (T)1; r.ynext = Y2;
     NM_TRY(eval_stage<T>(m, t + 0.5 * dt, Y1, z, r, st));
-    // k4 = f(t + dt, Y0);  y <- y + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised
-    r.kstore = nullptr;
-    r.nprev = 3;
-    r.kprev[0] = K0; r.kprev[1] = K1; r.kprev[2] = K2;
-    r.cprev[0] = (T)(1.0 / 6.0); r.cprev[1] = (T)(2.0 / 6.0); r.cprev[2] = (T)(2.0 / 6.0);
+    r.nstate = 2;
+    r.sprev[0] = Y0; r.sprev[1] = Y1;
+    r.bs[0] = (T)(-1.0 / 3.0); r.bs[1] = (T)(1.0 / 3.0); r.bs[2] = (T)(2.0 / 3.0); r.bs[3] = (T)(1.0 / 3.0);
     r.cself = (T)(1.0 / 6.0);
     r.ynext = y;
     r.renorm = renorm;
-    return eval_stage<T>(m, t + dt, Y0, z, r, st);
+    return eval_stage<T>(m, t + dt, Y2, z, r, st);
 }
 
 // Dormand-Prince 5(4) (Dormand & Prince 1980; "Dormand-Prince method")

@@ -87,6 +87,9 @@ __device__ __forceinline__ void node_epilogue(const NmLocalArgs<T> &a, long long
                     ea += r.eprev[q] * kp;
                 }
                 y[j] = y0[j] + r.dt * acc;
+                if (r.nstate == 2)
+                    y[j] = r.bs[0] * y0[j] + r.bs[1] * r.sprev[0][j * nn + n] + r.bs[2] * r.sprev[1][j * nn + n] +
+                           r.bs[3] * mc[j] + r.dt * acc;
                 er[j] = r.dt * ea;
             }
             if (r.ynext) {

@@ -19,6 +19,12 @@ template <typename T> struct NmRkArgs {
     T eprev[6];         // their weights in the embedded error (last Dormand-Prince stage)
     int nprev;
     T cself, eself;
+    // nstate = 2: last stage of RK4 from the stage states (no stored derivatives): with
+    // Y0 = y + dt/2 k1, Y1 = y + dt/2 k2 and fld = y + dt k3,
+    //   ynext = bs[0] y0 + bs[1] sprev[0] + bs[2] sprev[1] + bs[3] fld + dt cself f
+    const T *sprev[2];
+    T bs[4];
+    int nstate;
     T *ynext;           // y0 + dt (sum cprev kprev + cself f), or null
     T dt;
     int renorm;         // normalise ynext (final RK4 update written to m in place)

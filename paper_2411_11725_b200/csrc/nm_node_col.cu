@@ -67,8 +67,9 @@ template <> __device__ __forceinline__ float rcp_c<float>(float v) { return __fd
 template <> __device__ __forceinline__ double rcp_c<double>(double v) { return 1.0 / v; }
 
 // modes of the compiled epilogues: the NmLocalMode values, with the Runge-Kutta stage split by the
-// number of earlier derivatives it combines (0: first stages of RK4; 3: last stage of RK4; else a loop)
-enum { CM_H = 0, CM_RHS, CM_RK0, CM_RK3, CM_RKN, CM_ADJ1, CM_ADJ2, CM_COUNT };
+// way it combines (RK0: no earlier derivative, the first stages of RK4; RKS: last stage of RK4 from the
+// stage states; RKN: a loop over stored derivatives, Dormand-Prince)
+enum { CM_H = 0, CM_RHS, CM_RK0, CM_RKS, CM_RKN, CM_ADJ1, CM_ADJ2, CM_COUNT };
 
 // element n of component j of a nodal vector array (n < nodes < 2^31: one 32-bit index per node)
 template <typename P> __device__ __forceinline__ P *comp(P *base, int j, size_t nn) { return base + j * nn; }
@@ -97,7 +98,7 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
     if (CM == CM_RHS) {
 #pragma unroll
         for (int j = 0; j < 3; ++j) comp(a.out, j, nn)[n] = f[j];
-    } else if (CM == CM_RK0 || CM == CM_RK3 || CM == CM_RKN) {
+    } else if (CM == CM_RK0 || CM == CM_RKS || CM == CM_RKN) {
         const NmRkArgs<T> &r = a.rk;
         T acc[3], ea[3];
 #pragma unroll
@@ -105,11 +106,12 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
             acc[j] = r.cself * f[j];
             ea[j] = r.eself * f[j];
         }
-        if (CM == CM_RK3) {
+        T base[3] = {y0[0], y0[1], y0[2]};
+        if (CM == CM_RKS) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q)
-#pragma unroll
-                for (int j = 0; j < 3; ++j) acc[j] += r.cprev[q] * comp(r.kprev[q], j, nn)[n];
+            for (int j = 0; j < 3; ++j)
+                base[j] = r.bs[0] * y0[j] + r.bs[1] * comp(r.sprev[0], j, nn)[n] + r.bs[2] * comp(r.sprev[1], j, nn)[n] +
+                          r.bs[3] * mc[j];
         } else if (CM == CM_RKN) {
             for (int q = 0; q < r.nprev; ++q) {
                 const T *kp = r.kprev[q] + n;
@@ -129,7 +131,7 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
         if (r.ynext) {
             T y[3];
 #pragma unroll
-            for (int j = 0; j < 3; ++j) y[j] = y0[j] + r.dt * acc[j];
+            for (int j = 0; j < 3; ++j) y[j] = base[j] + r.dt * acc[j];
             if (r.renorm) {
                 const T inv = rsqrt_c<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
                 y[0] *= inv; y[1] *= inv; y[2] *= inv;
@@ -216,7 +218,7 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
     const unsigned pl = (unsigned)n1 * n2, cpl = (unsigned)N1 * g.N2;
     const size_t nn = (size_t)g.nodes, nc = (size_t)g.cells;
     const bool live = tid < n1;
-    constexpr bool RK = CM == CM_RK0 || CM == CM_RK3 || CM == CM_RKN;
+    constexpr bool RK = CM == CM_RK0 || CM == CM_RKS || CM == CM_RKN;
 
     for (int q = tid; q < CS * cg.stage; q += nthr) sm[q] = (T)0;
     __syncthreads();
@@ -499,8 +501,8 @@ template <typename T, bool UNI_MS> nm_status dispatch_col(nm_mesh *mesh, const N
     case NM_MODE_ADJ1: return launch_col<T, CM_ADJ1, UNI_MS>(mesh, a, st);
     case NM_MODE_ADJ2: return launch_col<T, CM_ADJ2, UNI_MS>(mesh, a, st);
     default:
-        if (!a.rk.want_err && a.rk.nprev == 0) return launch_col<T, CM_RK0, UNI_MS>(mesh, a, st);
-        if (!a.rk.want_err && a.rk.nprev == 3) return launch_col<T, CM_RK3, UNI_MS>(mesh, a, st);
+        if (!a.rk.want_err && a.rk.nprev == 0 && a.rk.nstate == 0) return launch_col<T, CM_RK0, UNI_MS>(mesh, a, st);
+        if (!a.rk.want_err && a.rk.nprev == 0 && a.rk.nstate == 2) return launch_col<T, CM_RKS, UNI_MS>(mesh, a, st);
         return launch_col<T, CM_RKN, UNI_MS>(mesh, a, st);
     }
 }

@@ -129,8 +129,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
         V v = a[t];
         if (h) v = cmulc(v, wP[e]);
         // sum of the even and odd halves: partner lane = lane ^ 1
-        v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
-        v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+        v = cadd(v, shfl1(v));
         if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ swz(e))] = v;
     }
     __syncthreads();
@@ -201,9 +200,12 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
         const T nxx = tp[0], nyy = tp[cstride], nzz = tp[2 * cstride];
         const T nxy = sy * tp[3 * cstride], nxz = sz * tp[4 * cstride], nyz = sy * sz * tp[5 * cstride];
         const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
-        a[0][s] = mk<T>(-(nxx * mx.x + nxy * my_.x + nxz * mz.x), -(nxx * mx.y + nxy * my_.y + nxz * mz.y));
-        a[1][s] = mk<T>(-(nxy * mx.x + nyy * my_.x + nyz * mz.x), -(nxy * mx.y + nyy * my_.y + nyz * mz.y));
-        a[2][s] = mk<T>(-(nxz * mx.x + nyz * my_.x + nzz * mz.x), -(nxz * mx.y + nyz * my_.y + nzz * mz.y));
+        const V hx = caxpy(nxz, mz, caxpy(nxy, my_, cscale(nxx, mx)));
+        const V hy = caxpy(nyz, mz, caxpy(nyy, my_, cscale(nxy, mx)));
+        const V hz = caxpy(nzz, mz, caxpy(nyz, my_, cscale(nxz, mx)));
+        a[0][s] = mk<T>(-hx.x, -hx.y);
+        a[1][s] = mk<T>(-hy.x, -hy.y);
+        a[2][s] = mk<T>(-hz.x, -hz.y);
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -213,8 +215,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
             const int e = j + M * t;
             V v = a[c][t];
             if (h) v = cmulc(v, wP[e]);
-            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
-            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            v = cadd(v, shfl1(v));
             if ((t >> 3) == h) my[(c * N + e) * TW + (kq ^ swz(e))] = v;
         }
     }
@@ -343,8 +344,7 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             const int e = j + M * t;
             V v = a[t];
             if (h) v = cmulc(v, wP[e]);
-            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
-            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            v = cadd(v, shfl1(v));
             if ((t >> 3) == h) {
                 ha[e] = v.x;
                 ha[g.N1 + e] = v.y;

@@ -143,9 +143,12 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
                 const T nxx = tp[0], nyy = tp[S::KZP], nzz = tp[2 * S::KZP];
                 const T nxy = sy * tp[3 * S::KZP], nxz = sz * tp[4 * S::KZP], nyz = sy * sz * tp[5 * S::KZP];
                 const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
-                a[0][s] = mk<T>(-(nxx * mx.x + nxy * my_.x + nxz * mz.x), -(nxx * mx.y + nxy * my_.y + nxz * mz.y));
-                a[1][s] = mk<T>(-(nxy * mx.x + nyy * my_.x + nyz * mz.x), -(nxy * mx.y + nyy * my_.y + nyz * mz.y));
-                a[2][s] = mk<T>(-(nxz * mx.x + nyz * my_.x + nzz * mz.x), -(nxz * mx.y + nyz * my_.y + nzz * mz.y));
+                const V hx = caxpy(nxz, mz, caxpy(nxy, my_, cscale(nxx, mx)));
+                const V hy = caxpy(nyz, mz, caxpy(nyy, my_, cscale(nxy, mx)));
+                const V hz = caxpy(nzz, mz, caxpy(nyz, my_, cscale(nxz, mx)));
+                a[0][s] = mk<T>(-hx.x, -hx.y);
+                a[1][s] = mk<T>(-hy.x, -hy.y);
+                a[2][s] = mk<T>(-hz.x, -hz.y);
             }
             if (sub == nt - 1) {
                 __syncwarp();
@@ -162,8 +165,7 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 #pragma unroll
                 for (int t = 0; t < 16; ++t) {
                     V v = a[c][t];
-                    v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
-                    v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+                    v = cadd(v, shfl1(v));
                     if ((t >> 3) == h) col[(c * N + M * t) * TW] = v;
                 }
             }
@@ -390,8 +392,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
             V v = a[t];
-            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
-            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            v = cadd(v, shfl1(v));
             if ((t >> 3) == h) {
                 s_out[(2 * line) * N + j + M * t] = v.x;
                 s_out[(2 * line + 1) * N + j + M * t] = v.y;
@@ -544,8 +545,7 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
             V v = a[t];
-            v.x += __shfl_xor_sync(0xffffffffu, v.x, 1);
-            v.y += __shfl_xor_sync(0xffffffffu, v.y, 1);
+            v = cadd(v, shfl1(v));
             if ((t >> 3) == h) out[M * t * TW] = v;
         }
         fence_async_smem();

@@ -54,6 +54,89 @@ template <typename V> __device__ __forceinline__ V cmulc(V a, V b)   // a * conj
     r.y = a.y * b.x - a.x * b.y;
     return r;
 }
+// ---- fp32: packed pair arithmetic (FADD2 / FMUL2 / FFMA2 of sm_100a) -----------------------------
+// A complex fp32 value is one aligned register pair; add.f32x2 / mul.f32x2 / fma.f32x2 work on both
+// halves with one issue slot, and ptxas folds half swaps, per-half negation and scalar broadcast
+// into their operand modifiers (.LO_HI, .NP, .F32), so a rotation by +-i or a complex product costs
+// no extra instruction.  Same rounding per element as the scalar forms.  These non-template
+// overloads win over the templates above for float2 arguments.
+__device__ __forceinline__ unsigned long long pk2(float x, float y)
+{
+    unsigned long long v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(x), "f"(y));
+    return v;
+}
+__device__ __forceinline__ float2 up2(unsigned long long v)
+{
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ float2 padd(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
+    return up2(r);
+}
+__device__ __forceinline__ float2 psub(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
+    return up2(r);
+}
+__device__ __forceinline__ float2 pmul(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
+    return up2(r);
+}
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)), "l"(pk2(c.x, c.y)));
+    return up2(r);
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return padd(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return psub(a, b); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 w)     // (ax wx - ay wy, ax wy + ay wx)
+{
+    const float2 t = pmul(make_float2(a.y, a.y), make_float2(w.y, w.x));
+    return pfma(make_float2(a.x, a.x), w, make_float2(-t.x, t.y));
+}
+__device__ __forceinline__ float2 cmulc(float2 a, float2 w)    // (ax wx + ay wy, ay wx - ax wy)
+{
+    const float2 t = pmul(make_float2(a.x, a.x), w);
+    return pfma(make_float2(a.y, a.y), make_float2(w.y, w.x), make_float2(t.x, -t.y));
+}
+// a * (c - i s): forward twiddle with compile-time c, s (INV: a * (c + i s)); the constants ride as
+// broadcast immediates
+template <bool INV> __device__ __forceinline__ float2 cmul_cs(float2 a, float c, float s)
+{
+    const float2 t = pmul(make_float2(a.y, a.x), make_float2(s, s));        // (s ay, s ax)
+    return pfma(a, make_float2(c, c), INV ? make_float2(-t.x, t.y) : make_float2(t.x, -t.y));
+}
+template <bool INV> __device__ __forceinline__ double2 cmul_cs(double2 a, double c, double s)
+{
+    double2 r;
+    if (INV) { r.x = a.x * c - a.y * s; r.y = a.y * c + a.x * s; }
+    else { r.x = a.x * c + a.y * s; r.y = a.y * c - a.x * s; }
+    return r;
+}
+// s * a and a + s * b with a real scalar s
+__device__ __forceinline__ float2 cscale(float s, float2 a) { return pmul(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 caxpy(float s, float2 b, float2 a) { return pfma(b, make_float2(s, s), a); }
+__device__ __forceinline__ double2 cscale(double s, double2 a) { a.x *= s; a.y *= s; return a; }
+__device__ __forceinline__ double2 caxpy(double s, double2 b, double2 a) { a.x += s * b.x; a.y += s * b.y; return a; }
+
+// the value held by the partner lane (lane ^ 1: the other half h of the same team thread)
+template <typename V> __device__ __forceinline__ V shfl1(V v)
+{
+    V r;
+    r.x = __shfl_xor_sync(0xffffffffu, v.x, 1);
+    r.y = __shfl_xor_sync(0xffffffffu, v.y, 1);
+    return r;
+}
+
 // a * w (INV = false) or a * conj(w) (INV = true)
 template <bool INV, typename V> __device__ __forceinline__ V ctw(V a, V w)
 {
@@ -98,16 +181,12 @@ template <typename T, bool INV, int Q> __device__ __forceinline__ typename VT<T>
     if (q == 4) return rot90<INV>(a);
     if (q == 8) return mk<T>(-a.x, -a.y);
     if (q == 12) return rot90<!INV>(a);
-    if (q == 2) {   // h (1 -+ i)
-        return INV ? mk<T>(h * (a.x - a.y), h * (a.x + a.y)) : mk<T>(h * (a.x + a.y), h * (a.y - a.x));
-    }
-    if (q == 6) {   // h (-1 -+ i)
-        return INV ? mk<T>(-h * (a.x + a.y), h * (a.x - a.y)) : mk<T>(h * (a.y - a.x), -h * (a.x + a.y));
-    }
     T c, s;   // w = c - i s (forward)
     if (q == 1) { c = c1; s = s1; }
+    else if (q == 2) { c = h; s = h; }
     else if (q == 3) { c = s1; s = c1; }
     else if (q == 5) { c = -s1; s = c1; }
+    else if (q == 6) { c = -h; s = h; }
     else if (q == 7) { c = -c1; s = s1; }
     else if (q == 9) { c = -c1; s = -s1; }
     else if (q == 10) { c = -h; s = -h; }
@@ -115,8 +194,7 @@ template <typename T, bool INV, int Q> __device__ __forceinline__ typename VT<T>
     else if (q == 13) { c = s1; s = -c1; }
     else if (q == 14) { c = h; s = -h; }
     else { c = c1; s = -s1; }   // 15
-    const V w = mk<T>(c, -s);
-    return ctw<INV>(a, w);
+    return cmul_cs<INV>(a, c, s);
 }
 
 // exp(-+ 2 pi i q/32) as compile-time constants, q = 0..15
@@ -137,8 +215,7 @@ template <typename T, bool INV, int Q> __device__ __forceinline__ typename VT<T>
     else if (Q == 11) { c = -s3; s = c3; }
     else if (Q == 13) { c = -c3; s = s3; }
     else { c = -c1; s = s1; }   // 15
-    const V w = mk<T>(c, -s);
-    return ctw<INV>(a, w);
+    return cmul_cs<INV>(a, c, s);
 }
 
 // a[t] *= exp(-+ 2 pi i t/32), t = 0..15: the part of the half-sample shift w_P^(j + M t) of the odd

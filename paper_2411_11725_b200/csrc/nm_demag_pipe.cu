@@ -6,7 +6,9 @@
 // asynchronous copies (cp.async.bulk, mbarrier transaction counts) bring tile n+2 into shared
 // memory and drain tile n-1 back to HBM while the eight warps transform tile n, so that the load,
 // the arithmetic and the store of different tiles overlap on an SM that holds only eight warps
-// (the z pass keeps 3 x 16 complex spectrum values plus twiddles per thread: ~250 registers).
+// (the z pass keeps 3 x 16 complex spectrum values plus twiddles per thread).  In the z pass a
+// ninth warp issues the copies and the transform warps synchronise only through the tile
+// barriers (full / done), never with one another.
 //
 //   k_pz_mid : z forward, H^ = -N^ M^, z inverse, in place on B[ktl][ky][comp][c3][8].
 //              Work item = one folded tensor row |ky| of one k1 tile: the tiles +ky and -ky share
@@ -35,11 +37,12 @@ struct PzSmem {
     static constexpr int OFF_T = NBUF * TILE_BYTES;
     static constexpr int OFF_SCR = OFF_T + 8 * TSLICE * 4;
     static constexpr int OFF_BAR = OFF_SCR + 8 * WSCR * 8;
-    static constexpr int BYTES = OFF_BAR + (NBUF + 8) * 8;
+    static constexpr int BYTES = OFF_BAR + (2 * NBUF + 8) * 8;
 };
+constexpr int kMidThreads = 288;      // eight transform warps and one copy warp
 static_assert(PzSmem::BYTES <= 227 * 1024, "k_pz_mid shared memory exceeds the sm_100a per-CTA limit");
 
-__global__ void __launch_bounds__(kPipeThreads, 1)
+__global__ void __launch_bounds__(kMidThreads, 1)
 k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItems, int kt0,
          const float2 *__restrict__ wP)
 {
@@ -52,7 +55,8 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
     T *s_T = reinterpret_cast<T *>(smem + S::OFF_T);
     V *s_scr = reinterpret_cast<V *>(smem + S::OFF_SCR);
     uint64_t *fullB = reinterpret_cast<uint64_t *>(smem + S::OFF_BAR);
-    uint64_t *fullT = fullB + S::NBUF;
+    uint64_t *doneB = fullB + S::NBUF;
+    uint64_t *fullT = doneB + S::NBUF;
 
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int h = lane & 1, j = lane >> 1;
@@ -60,7 +64,11 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
     const int G = gridDim.x;
 
     if (tid == 0) {
-        for (int q = 0; q < S::NBUF + 8; ++q) mbar_init(fullB + q, 1);
+        for (int q = 0; q < S::NBUF; ++q) {
+            mbar_init(fullB + q, 1);
+            mbar_init(doneB + q, 8);
+        }
+        for (int q = 0; q < 8; ++q) mbar_init(fullT + q, 1);
         mbar_fence_init();
     }
     __syncthreads();
@@ -82,9 +90,13 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
         bulk_load(s_T + w * S::TSLICE, src, S::TSLICE * 4, fullT + w);
     };
 
-    // prefetch iterator of thread 0: two tiles ahead of the compute iterator
-    int pg = blockIdx.x, psub = 0;
-    if (tid == 0) {
+    // ---- copy warp: one thread walks the same tile list; it loads two tiles ahead of the one being
+    // stored and stores tile n as soon as the eight transform warps have left it, so the transform
+    // warps never wait for one another and drift into different phases (butterflies of one warp
+    // over the scratch exchange of another)
+    if (w == 8) {
+        if (lane != 0) return;
+        int pg = blockIdx.x, psub = 0;
         for (int q = 0; q < 2; ++q) {
             if (pg < nItems) {
                 mbar_expect_tx(fullB + q, S::TILE_BYTES);
@@ -93,6 +105,26 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
                 else { pg += G; psub = 0; }
             }
         }
+        int n = 0;
+        for (int g = blockIdx.x; g < nItems; g += G) {
+            const int nt = n_tiles(g);
+            for (int sub = 0; sub < nt; ++sub, ++n) {
+                const int b = n % S::NBUF;
+                mbar_wait(doneB + b, (uint32_t)((n / S::NBUF) & 1));
+                bulk_store(tile_ptr(g, sub), s_B + b * S::TILE_ELEMS, S::TILE_BYTES);
+                bulk_commit();
+                bulk_wait_read<1>();          // the store of tile n-1 has left its buffer
+                if (pg < nItems) {
+                    const int nb = (n + 2) % S::NBUF;
+                    mbar_expect_tx(fullB + nb, S::TILE_BYTES);
+                    bulk_load(s_B + nb * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + nb);
+                    if (psub + 1 < n_tiles(pg)) ++psub;
+                    else { pg += G; psub = 0; }
+                }
+            }
+        }
+        bulk_wait<0>();
+        return;
     }
     if (lane == 0 && (int)blockIdx.x < nItems) load_tensor(blockIdx.x);
 
@@ -122,8 +154,20 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 #pragma unroll
                 for (int c = 0; c < 3; ++c) shift32<T, false>(a[c]);
             }
-#pragma unroll
-            for (int c = 0; c < 3; ++c) fft_fwd<T, M, true>(a[c], tw, scr, j);
+            // three forward transforms, the butterflies of one component between the scratch
+            // stores and loads of another (one scratch per team: put(c + 1) follows get(c))
+            dft16<T, false>(a[0]);
+            fwd_put<T, M, true>(a[0], tw, scr, j);
+            dft16<T, false>(a[1]);
+            fwd_get<T, M>(a[0], scr, j);
+            dft16<T, false>(a[2]);
+            fwd_put<T, M, true>(a[1], tw, scr, j);
+            dft16<T, false>(a[0]);
+            fwd_get<T, M>(a[1], scr, j);
+            fwd_put<T, M, true>(a[2], tw, scr, j);
+            dft16<T, false>(a[1]);
+            fwd_get<T, M>(a[2], scr, j);
+            dft16<T, false>(a[2]);
             // H^ = -N^ M^ ; rows of the folded tensor: sign -1 per folded odd axis
             if (sub == 0) {
                 mbar_wait(fullT + w, tphase);
@@ -154,8 +198,18 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
                 __syncwarp();
                 if (lane == 0 && g + G < nItems) load_tensor(g + G);
             }
-#pragma unroll
-            for (int c = 0; c < 3; ++c) fft_inv<T, M, true>(a[c], tw, scr, j);
+            dft16<T, true>(a[0]);
+            inv_put<T, M>(a[0], scr, j);
+            dft16<T, true>(a[1]);
+            inv_get<T, M, true>(a[0], tw, scr, j);
+            dft16<T, true>(a[2]);
+            inv_put<T, M>(a[1], scr, j);
+            dft16<T, true>(a[0]);
+            inv_get<T, M, true>(a[1], tw, scr, j);
+            inv_put<T, M>(a[2], scr, j);
+            dft16<T, true>(a[1]);
+            inv_get<T, M, true>(a[2], tw, scr, j);
+            dft16<T, true>(a[2]);
             if (h) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) shift32<T, true>(a[c]);
@@ -170,22 +224,10 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
                 }
             }
             fence_async_smem();
-            __syncthreads();
-            if (tid == 0) {
-                bulk_store(tile_ptr(g, sub), s_B + b * S::TILE_ELEMS, S::TILE_BYTES);
-                bulk_commit();
-                bulk_wait_read<1>();          // the store of tile n-1 has left its buffer
-                if (pg < nItems) {
-                    const int nb = (n + 2) % S::NBUF;
-                    mbar_expect_tx(fullB + nb, S::TILE_BYTES);
-                    bulk_load(s_B + nb * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + nb);
-                    if (psub + 1 < n_tiles(pg)) ++psub;
-                    else { pg += G; psub = 0; }
-                }
-            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(doneB + b);
         }
     }
-    if (tid == 0) bulk_wait<0>();
 }
 
 
@@ -573,8 +615,8 @@ nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     const int nItems = nkt * (g.N2 + 1);
     const int grid = nItems < mesh->sm_count ? nItems : mesh->sm_count;
     NmLaunchScope sc(mesh, NM_K_MID, st);
-    k_pz_mid<<<grid, kPipeThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn, g.N2,
-                                                        nItems, kt0, (const float2 *)mesh->tw_z);
+    k_pz_mid<<<grid, kMidThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn, g.N2,
+                                                       nItems, kt0, (const float2 *)mesh->tw_z);
     return NM_OK;
 }
 

@@ -441,4 +441,63 @@ __device__ __forceinline__ void fft_inv(typename VT<T>::V *a, const typename VT<
     dft16<T, true>(a);
 }
 
+// The same transforms cut at the exchange, so that a caller holding several independent lines per
+// thread (the three components of the z pass) can place the butterflies of one line between the
+// scratch stores and loads of another:
+//   forward  dft16 -> fwd_put | fwd_get -> dftM          inverse  dftM -> inv_put | inv_get -> dft16
+template <typename T, int M, bool TW0>
+__device__ __forceinline__ void fwd_put(const typename VT<T>::V *a, const typename VT<T>::V *tw,
+                                        typename VT<T>::V *scr, int i)
+{
+    typedef typename VT<T>::V V;
+    const int l = i / M, j = i % M;
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+        const int tp = rev16(p);
+        V v = a[p];
+        if (tp != 0 || TW0) v = cmul(v, tw[tp]);
+        scr[skew((l * 16 + tp) * M + j)] = v;
+    }
+}
+template <typename T, int M>
+__device__ __forceinline__ void fwd_get(typename VT<T>::V *a, const typename VT<T>::V *scr, int i)
+{
+    const int l = i / M, j = i % M;
+    constexpr int U = 16 / M;
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int u = s / M, jj = s % M;
+        a[s] = scr[skew((l * 16 + j * U + u) * M + jj)];
+    }
+}
+template <typename T, int M>
+__device__ __forceinline__ void inv_put(const typename VT<T>::V *a, typename VT<T>::V *scr, int i)
+{
+    const int l = i / M, j = i % M;
+    constexpr int U = 16 / M;
+    __syncwarp();
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const int u = s / M, jj = s % M;
+        scr[skew((l * 16 + j * U + u) * M + jj)] = a[s];
+    }
+}
+template <typename T, int M, bool TW0>
+__device__ __forceinline__ void inv_get(typename VT<T>::V *a, const typename VT<T>::V *tw,
+                                        const typename VT<T>::V *scr, int i)
+{
+    typedef typename VT<T>::V V;
+    const int l = i / M, j = i % M;
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+        const int tp = rev16(p);
+        V v = scr[skew((l * 16 + tp) * M + j)];
+        if (tp != 0 || TW0) v = cmulc(v, tw[tp]);
+        a[p] = v;
+    }
+}
+
 } // namespace nmf

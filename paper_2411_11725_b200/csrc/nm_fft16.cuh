@@ -18,8 +18,11 @@
 #pragma once
 
 #include "nm_internal.h"
+#include "nm_pair.cuh"
 
 namespace nmf {
+
+using namespace nmp;
 
 template <typename T> struct VT { typedef typename NmVec2<T>::type V; };
 
@@ -54,48 +57,8 @@ template <typename V> __device__ __forceinline__ V cmulc(V a, V b)   // a * conj
     r.y = a.y * b.x - a.x * b.y;
     return r;
 }
-// ---- fp32: packed pair arithmetic (FADD2 / FMUL2 / FFMA2 of sm_100a) -----------------------------
-// A complex fp32 value is one aligned register pair; add.f32x2 / mul.f32x2 / fma.f32x2 work on both
-// halves with one issue slot, and ptxas folds half swaps, per-half negation and scalar broadcast
-// into their operand modifiers (.LO_HI, .NP, .F32), so a rotation by +-i or a complex product costs
-// no extra instruction.  Same rounding per element as the scalar forms.  These non-template
-// overloads win over the templates above for float2 arguments.
-__device__ __forceinline__ unsigned long long pk2(float x, float y)
-{
-    unsigned long long v;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(x), "f"(y));
-    return v;
-}
-__device__ __forceinline__ float2 up2(unsigned long long v)
-{
-    float2 r;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
-    return r;
-}
-__device__ __forceinline__ float2 padd(float2 a, float2 b)
-{
-    unsigned long long r;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
-    return up2(r);
-}
-__device__ __forceinline__ float2 psub(float2 a, float2 b)
-{
-    unsigned long long r;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
-    return up2(r);
-}
-__device__ __forceinline__ float2 pmul(float2 a, float2 b)
-{
-    unsigned long long r;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
-    return up2(r);
-}
-__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c)
-{
-    unsigned long long r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)), "l"(pk2(c.x, c.y)));
-    return up2(r);
-}
+// fp32 complex arithmetic on packed pairs (nm_pair.cuh); these non-template overloads win over the
+// templates above for float2 arguments
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return padd(a, b); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return psub(a, b); }
 __device__ __forceinline__ float2 cmul(float2 a, float2 w)     // (ax wx - ay wy, ax wy + ay wx)

@@ -26,8 +26,24 @@
 // zero-filled outside the mesh -- is streamed by cp.async into a ring of CS stages, CS - 2 planes
 // ahead of the arithmetic, one CTA barrier per plane.  The epilogue is compiled per mode.
 #include "nm_local.cuh"
+#include "nm_pair.cuh"
+
+using namespace nmp;
 
 namespace {
+
+// A pair = the same quantity on the two node rows (ry = 0, 1) a thread owns: fp32 pairs run on the
+// packed instructions of nm_pair.cuh, fp64 pairs on scalar ones.
+template <typename T> struct PairOf { typedef typename NmVec2<T>::type V; };
+template <typename T> __device__ __forceinline__ typename PairOf<T>::V pr(T a, T b)
+{
+    typename PairOf<T>::V v;
+    v.x = a;
+    v.y = b;
+    return v;
+}
+template <typename T> __device__ __forceinline__ typename PairOf<T>::V pr1(T a) { return pr<T>(a, a); }
+template <typename V> __device__ __forceinline__ V pneg(V a) { a.x = -a.x; a.y = -a.y; return a; }
 
 template <typename T> __device__ __forceinline__ T rsqrt_c(T v);
 template <> __device__ __forceinline__ float rsqrt_c<float>(float v) { return 1.0f / sqrtf(v); }
@@ -74,11 +90,12 @@ enum { CM_H = 0, CM_RHS, CM_RK0, CM_RKS, CM_RKN, CM_ADJ1, CM_ADJ2, CM_COUNT };
 // element n of component j of a nodal vector array (n < nodes < 2^31: one 32-bit index per node)
 template <typename P> __device__ __forceinline__ P *comp(P *base, int j, size_t nn) { return base + j * nn; }
 
-// a9-a11 on one node.  mc = fld_n, sms = (S Ms)_n; y0 = what the mode reads at this node, loaded
-// before the plane arithmetic: the start-of-step state (Runge-Kutta), a (ADJ1) or d (ADJ2).
+// a10-a11 on one node.  mc = fld_n, f = the LLG right-hand side (a9, computed by the caller for both
+// rows at once), sms = (S Ms)_n; y0 = what the mode reads at this node, loaded before the plane
+// arithmetic: the start-of-step state (Runge-Kutta), a (ADJ1) or d (ADJ2).
 template <typename T, int CM>
 __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, size_t nn, const T *mc,
-                                           const T *H, T sms, const T *y0, double &err2)
+                                           const T *H, const T *f, T sms, const T *y0, double &err2)
 {
     if (CM == CM_H) {
 #pragma unroll
@@ -90,11 +107,6 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
         for (int j = 0; j < 3; ++j) comp(a.dadt, j, nn)[n] = -(y0[j] + sms * H[j]);
         return;
     }
-    T mxH[3], mxmxH[3], f[3];
-    cross_c(mc, H, mxH);
-    cross_c(mc, mxH, mxmxH);
-#pragma unroll
-    for (int j = 0; j < 3; ++j) f[j] = -a.gp * mxH[j] - a.agp * mxmxH[j];
     if (CM == CM_RHS) {
 #pragma unroll
         for (int j = 0; j < 3; ++j) comp(a.out, j, nn)[n] = f[j];
@@ -175,10 +187,12 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
 }
 
 // Tile geometry (host and device agree through this struct).  Elements per stage:
-//   m tiles    3 x (RY + 2) rows x MP,  MP = n1 + 2: ghost column, n1 nodes, ghost column
-//   cell tiles [4 zeros] ncell x (RY + 1) rows x CP,  CP = N1 (rounded up to 4) + 4: N1 cells, zeros
+//   m tiles    3 x (RY + 2) rows x MP: ghost column, n1 nodes, ghost column
+//   cell tiles [4 zeros] ncell x (RY + 1) rows x CP: N1 cells, zeros
 // The zeros are written once and never touched by the copies: they are cell -1 (the pad of the row
-// before) and cell N1 of every cell row.
+// before) and cell N1 of every cell row.  The row pitches MP = PITCH >= n1 + 2 and CP = PITCH + 4 are
+// compile-time (two classes, 264 and 320), so every shared-memory access of the plane arithmetic is
+// a base register plus an immediate.
 struct ColGeom {
     int MP, CP;
     int moff_cells;         // offset of cell (row 0, column 0) of component 0 in a stage
@@ -188,11 +202,12 @@ struct ColGeom {
     int cchunks;            // copies per component of the cell tile
 };
 
-template <typename T, int RY> __host__ __device__ inline ColGeom col_geom(const NmGeom &g, bool has_hc, bool uni_ms)
+template <typename T, int RY, int PITCH>
+__host__ __device__ inline ColGeom col_geom(const NmGeom &g, bool has_hc, bool uni_ms)
 {
     ColGeom c;
-    c.MP = g.n1 + 2;
-    c.CP = ((g.N1 + 3) / 4) * 4 + 4;
+    c.MP = PITCH;
+    c.CP = PITCH + 4;
     c.moff_cells = ((3 * (RY + 2) * c.MP + 3) / 4) * 4 + 4;
     c.ncell = has_hc ? (uni_ms ? 3 : 4) : 0;
     c.stage = c.moff_cells + c.ncell * (RY + 1) * c.CP;
@@ -203,15 +218,17 @@ template <typename T, int RY> __host__ __device__ inline ColGeom col_geom(const 
 
 constexpr int CQ = 3;       // cell copies per thread and component (host checks cchunks <= CQ * threads)
 
-template <typename T, int RY, int CS, int CM, bool UNI_MS, int MAXT>
+template <typename T, int RY, int CS, int CM, bool UNI_MS, int MAXT, int PITCH>
 __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const NmLocalArgs<T> a, int zchunk)
 {
+    static_assert(RY == 2, "the plane arithmetic pairs the two node rows of a thread");
+    typedef typename PairOf<T>::V V;
     extern __shared__ __align__(16) unsigned char col_smem[];
     T *sm = reinterpret_cast<T *>(col_smem);
     const NmGeom &g = a.g;
     const int n1 = g.n1, n2 = g.n2, N1 = g.N1;
     const bool has_hc = a.Hc != nullptr;
-    const ColGeom cg = col_geom<T, RY>(g, has_hc, UNI_MS);
+    const ColGeom cg = col_geom<T, RY, PITCH>(g, has_hc, UNI_MS);
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int r0 = blockIdx.x * RY;                       // first node row of the CTA
     const int z0 = blockIdx.y * zchunk, z1 = min(z0 + zchunk, g.n3);
@@ -306,14 +323,17 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
     }
     const T cT = UNI_MS ? a.ms_uni : (T)1;
 
+    // pair constants of the plane arithmetic (lo = row r0, hi = row r0 + 1)
+    const V DYF = pr<T>(dyf[0], dyf[1]);
+    const V kUx = pmul(pr1<T>(a.idx2[0]), DYF);            // dx^-2 dy
+    const V kW0 = pmul(pr1<T>(dxf), DYF);                  // dx dy
+    const V kW1n = pmul(pr1<T>(-sixth), DYF);              // -dy/6
+
     // partial sums of the z operators: P waits for the next plane, M starts the output after it
-    T GP[RY][3], GM[RY][3], aP[RY], aM[RY];
+    V GP[3], GM[3], aP, aM;
+    aP = aM = pr1<T>((T)0);
 #pragma unroll
-    for (int ry = 0; ry < RY; ++ry) {
-        aP[ry] = aM[ry] = (T)0;
-#pragma unroll
-        for (int j = 0; j < 3; ++j) GP[ry][j] = GM[ry][j] = (T)0;
-    }
+    for (int j = 0; j < 3; ++j) GP[j] = GM[j] = pr1<T>((T)0);
     double err2 = 0.0;
 
     const int kstart = max(z0 - 1, 0), kend = z1;         // plane kend = n3 is fetched clamped and weighted 0
@@ -359,7 +379,7 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
         const T wR_out = gRm * sixth, w_P = dzk - (gLk + gRk) * sixth, w_M = gLp * sixth;
         const T *st = sm + slot * cg.stage;
         if (live) {
-            T Tn[RY][3];
+            V Tn[3];
             if (has_hc) {
                 const T *cb = st + cg.moff_cells + tid;
                 T ml[RY + 1], mr[RY + 1];
@@ -379,17 +399,13 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                         const T *crow = cb + (j * (RY + 1) + cr) * cg.CP;
                         X[cr] = UNI_MS ? crow[-1] + crow[0] : ml[cr] * crow[-1] + mr[cr] * crow[0];
                     }
-#pragma unroll
-                    for (int ry = 0; ry < RY; ++ry) Tn[ry][j] = cT * (X[ry] + X[ry + 1]);
+                    Tn[j] = pmul(pr1<T>(cT), padd(pr<T>(X[0], X[1]), pr<T>(X[1], X[2])));
                 }
             } else {
-#pragma unroll
-                for (int ry = 0; ry < RY; ++ry) Tn[ry][0] = Tn[ry][1] = Tn[ry][2] = (T)0;
+                Tn[0] = Tn[1] = Tn[2] = pr1<T>((T)0);
             }
-            T wk[RY];
-#pragma unroll
-            for (int ry = 0; ry < RY; ++ry) wk[ry] = (T)0;
-            T Gout[RY][3];
+            V wk = pr1<T>((T)0);
+            V Gout[3];
 #pragma unroll
             for (int j = 0; j < 3; ++j) {
                 const T *t = st + j * (RY + 2) * cg.MP + tid;     // columns tid, tid + 1, tid + 2 = i1 - 1, i1, i1 + 1
@@ -400,58 +416,74 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                     c[r] = row[1];
                     sx[r] = row[0] + row[2];
                 }
-#pragma unroll
-                for (int ry = 0; ry < RY; ++ry) {
-                    const T cc = c[ry + 1];
-                    const T ax = (T)2 * cc - sx[ry + 1];
-                    const T ay = (T)2 * cc - (c[ry] + c[ry + 2]);
-                    const T axy = (T)2 * (ax + ay) - (T)4 * cc + (sx[ry] + sx[ry + 2]);
-                    const T U = (a.idx2[0] * dyf[ry]) * ax + cUy * ay - c3 * axy;
-                    const T W = dxf * (dyf[ry] * cc) - (dyf[ry] * sixth) * ax - cWy * ay + (T)(1.0 / 36.0) * axy;
-                    const T R = a.idx2[2] * W - sixth * U;
-                    wk[ry] += a.kax[j] * W;
-                    Gout[ry][j] = GP[ry][j] + eR_out * R + Tn[ry][j];
-                    GP[ry][j] = GM[ry][j] + eU_P * U + eR_P * R + Tn[ry][j];
-                    GM[ry][j] = eR_M * R;
-                }
+                const V CC = pr<T>(c[1], c[2]), SXc = pr<T>(sx[1], sx[2]);
+                const V ax = pfma(CC, pr1<T>((T)2), pneg(SXc));
+                const V ay = pfma(CC, pr1<T>((T)2), pneg(padd(pr<T>(c[0], c[1]), pr<T>(c[2], c[3]))));
+                const V axy = pfma(padd(ax, ay), pr1<T>((T)2),
+                                   pfma(CC, pr1<T>((T)-4), padd(pr<T>(sx[0], sx[1]), pr<T>(sx[2], sx[3]))));
+                const V U = pfma(kUx, ax, pfma(ay, pr1<T>(cUy), pmul(axy, pr1<T>(-c3))));
+                const V W = pfma(kW0, CC, pfma(kW1n, ax, pfma(ay, pr1<T>(-cWy), pmul(axy, pr1<T>((T)(1.0 / 36.0))))));
+                const V R = pfma(W, pr1<T>(a.idx2[2]), pmul(U, pr1<T>(-sixth)));
+                wk = pfma(W, pr1<T>(a.kax[j]), wk);
+                Gout[j] = padd(pfma(R, pr1<T>(eR_out), GP[j]), Tn[j]);
+                GP[j] = padd(pfma(R, pr1<T>(eR_P), pfma(U, pr1<T>(eU_P), GM[j])), Tn[j]);
+                GM[j] = pmul(R, pr1<T>(eR_M));
             }
-            T aout[RY];
-#pragma unroll
-            for (int ry = 0; ry < RY; ++ry) {
-                aout[ry] = aP[ry] + wR_out * wk[ry];
-                aP[ry] = aM[ry] + w_P * wk[ry];
-                aM[ry] = w_M * wk[ry];
-            }
+            const V aout = pfma(wk, pr1<T>(wR_out), aP);
+            aP = pfma(wk, pr1<T>(w_P), aM);
+            aM = pmul(wk, pr1<T>(w_M));
             if (zout) {
                 const T gLz = z > 0 ? (T)1 : (T)0;
                 const T izf = (z > 0 && z < g.N3) ? (T)0.5 : (T)1;             // 1 / (gL + gR) of output z
                 int sp = slot - 1;
                 if (sp < 0) sp += CS;
                 const T *sprev = sm + sp * cg.stage + tid + 1;                // centre column of plane z
+                const unsigned nrow[RY] = {nbase, nbase + (unsigned)n1};
+                V mcp[3];
+#pragma unroll
+                for (int j = 0; j < 3; ++j)
+                    mcp[j] = pr<T>(sprev[(j * (RY + 2) + 1) * cg.MP], sprev[(j * (RY + 2) + 2) * cg.MP]);
+                V smsp, invp;
+                if (UNI_MS) {
+                    invp = pmul(pr<T>(inv_xy[0], inv_xy[1]), pr1<T>(izf));
+                    smsp = (CM == CM_ADJ1 || CM == CM_ADJ2) ? pmul(DYF, pr1<T>(a.ms_uni * (T)4 * dxf * (gLz + gRm))) : pr1<T>((T)1);
+                } else {
+                    smsp = pr<T>(rowlive[0] ? a.sMs[nrow[0]] : (T)0, rowlive[1] ? a.sMs[nrow[1]] : (T)0);
+                    invp = pr<T>(smsp.x > 0 ? rcp_c<T>(smsp.x) : (T)0, smsp.y > 0 ? rcp_c<T>(smsp.y) : (T)0);
+                }
+                // H = (anisotropy + exchange + demag sums) / (S Ms) + uniform Zeeman; 0 where S Ms = 0
+                const V ak = pmul(aout, pr1<T>(a.cku));
+                V Hp[3];
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    Hp[j] = pmul(pfma(ak, pr1<T>(a.kax[j]), Gout[j]), invp);
+                    if (a.terms & NM_TERM_ZEEMAN) {
+                        const T hz = a.hu[j];
+                        Hp[j] = padd(Hp[j], UNI_MS ? pr1<T>(hz) : pr<T>(smsp.x > 0 ? hz : (T)0, smsp.y > 0 ? hz : (T)0));
+                    }
+                }
+                // a9 (Eq. 1) on both rows: f = -gamma' m x H - alpha gamma' m x (m x H)
+                V fp[3];
+                if (CM != CM_H && CM != CM_ADJ2) {
+                    V mxH[3], mm[3];
+                    mxH[0] = pfma(mcp[1], Hp[2], pneg(pmul(mcp[2], Hp[1])));
+                    mxH[1] = pfma(mcp[2], Hp[0], pneg(pmul(mcp[0], Hp[2])));
+                    mxH[2] = pfma(mcp[0], Hp[1], pneg(pmul(mcp[1], Hp[0])));
+                    mm[0] = pfma(mcp[1], mxH[2], pneg(pmul(mcp[2], mxH[1])));
+                    mm[1] = pfma(mcp[2], mxH[0], pneg(pmul(mcp[0], mxH[2])));
+                    mm[2] = pfma(mcp[0], mxH[1], pneg(pmul(mcp[1], mxH[0])));
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) fp[j] = pfma(mxH[j], pr1<T>(-a.gp), pmul(mm[j], pr1<T>(-a.agp)));
+                } else {
+                    fp[0] = fp[1] = fp[2] = pr1<T>((T)0);
+                }
 #pragma unroll
                 for (int ry = 0; ry < RY; ++ry) {
                     if (!rowlive[ry]) continue;
-                    const unsigned n = nbase + ry * n1;
-                    T mc[3];
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) mc[j] = sprev[(j * (RY + 2) + ry + 1) * cg.MP];
-                    T sms, inv;
-                    if (UNI_MS) {
-                        inv = inv_xy[ry] * izf;
-                        sms = (CM == CM_ADJ1 || CM == CM_ADJ2) ? a.ms_uni * (T)4 * dxf * dyf[ry] * (gLz + gRm) : (T)1;
-                    } else {
-                        sms = a.sMs[n];
-                        inv = sms > 0 ? rcp_c<T>(sms) : (T)0;
-                    }
-                    T H[3];
-                    const T ak = a.cku * aout[ry];
-#pragma unroll
-                    for (int j = 0; j < 3; ++j) {
-                        T hv = (ak * a.kax[j] + Gout[ry][j]) * inv;
-                        if (a.terms & NM_TERM_ZEEMAN) hv += a.hu[j];
-                        H[j] = (UNI_MS || sms > 0) ? hv : (T)0;
-                    }
-                    epilogue_c<T, CM>(a, n, nn, mc, H, sms, y0[ry], err2);
+                    const T mc[3] = {ry ? mcp[0].y : mcp[0].x, ry ? mcp[1].y : mcp[1].x, ry ? mcp[2].y : mcp[2].x};
+                    const T H[3] = {ry ? Hp[0].y : Hp[0].x, ry ? Hp[1].y : Hp[1].x, ry ? Hp[2].y : Hp[2].x};
+                    const T f[3] = {ry ? fp[0].y : fp[0].x, ry ? fp[1].y : fp[1].x, ry ? fp[2].y : fp[2].x};
+                    epilogue_c<T, CM>(a, nrow[ry], nn, mc, H, f, ry ? smsp.y : smsp.x, y0[ry], err2);
                 }
             }
         }
@@ -473,16 +505,24 @@ template <typename T> struct ColStages { static constexpr int CS = sizeof(T) == 
 inline int col_zchunk(const NmGeom &g) { return g.n3 <= 40 ? g.n3 : 32; }
 inline int col_threads(const NmGeom &g) { return ((g.n1 + 2 + 31) / 32) * 32; }
 
-template <typename T, int CM, bool UNI_MS>
-nm_status launch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
+// pitch class of a mesh: the smaller compile-time row pitch that holds n1 + 2 columns
+constexpr int kPitchS = 264, kPitchL = 320;
+inline int col_pitch(const NmGeom &g) { return g.n1 + 2 <= kPitchS ? kPitchS : kPitchL; }
+template <typename T> inline ColGeom col_geom_rt(const NmGeom &g, bool has_hc, bool uni_ms)
+{
+    return col_pitch(g) == kPitchS ? col_geom<T, kRY, kPitchS>(g, has_hc, uni_ms) : col_geom<T, kRY, kPitchL>(g, has_hc, uni_ms);
+}
+
+template <typename T, int CM, bool UNI_MS, int PITCH>
+nm_status launch_col_p(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
 {
     constexpr int CS = ColStages<T>::CS;
     const NmGeom &g = a.g;
-    const ColGeom cg = col_geom<T, kRY>(g, a.Hc != nullptr, UNI_MS);
+    const ColGeom cg = col_geom<T, kRY, PITCH>(g, a.Hc != nullptr, UNI_MS);
     const size_t bytes = (size_t)CS * cg.stage * sizeof(T);
     const int zchunk = col_zchunk(g);
     const dim3 grid((g.n2 + kRY - 1) / kRY, (g.n3 + zchunk - 1) / zchunk);
-    auto kern = k_node_col<T, kRY, CS, CM, UNI_MS, kMaxT>;
+    auto kern = k_node_col<T, kRY, CS, CM, UNI_MS, kMaxT, PITCH>;
     NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     mesh->last_partials = (int)(grid.x * grid.y);
     {
@@ -491,6 +531,13 @@ nm_status launch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
     }
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;
+}
+
+template <typename T, int CM, bool UNI_MS>
+nm_status launch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
+{
+    return col_pitch(a.g) == kPitchS ? launch_col_p<T, CM, UNI_MS, kPitchS>(mesh, a, st)
+                                     : launch_col_p<T, CM, UNI_MS, kPitchL>(mesh, a, st);
 }
 
 template <typename T, bool UNI_MS> nm_status dispatch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
@@ -517,7 +564,7 @@ template <typename T> bool nm_node_col_ok(const nm_mesh *mesh, const NmLocalArgs
     (void)mesh;
     const NmGeom &g = a.g;
     if (g.n1 < 96 || g.n1 + 2 > kMaxT || g.nodes >= (1ll << 31)) return false;
-    const ColGeom cg = col_geom<T, kRY>(g, a.Hc != nullptr, a.ms_uni > 0);
+    const ColGeom cg = col_geom_rt<T>(g, a.Hc != nullptr, a.ms_uni > 0);
     if (cg.cchunks > CQ * col_threads(g)) return false;
     if (cg.cvec && a.Hc && ((((uintptr_t)a.Hc) | ((uintptr_t)a.Ms)) & 15)) return false;   // 16-byte cell copies
     const size_t bytes = (size_t)ColStages<T>::CS * cg.stage * sizeof(T);

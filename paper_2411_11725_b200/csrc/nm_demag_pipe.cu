@@ -50,7 +50,7 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
     typedef float2 V;
     typedef PzSmem S;
     constexpr int M = 16, N = 256, P = 512;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     V *s_B = reinterpret_cast<V *>(smem);
     T *s_T = reinterpret_cast<T *>(smem + S::OFF_T);
     V *s_scr = reinterpret_cast<V *>(smem + S::OFF_SCR);
@@ -90,14 +90,14 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
         bulk_load(s_T + w * S::TSLICE, src, S::TSLICE * 4, fullT + w);
     };
 
-    // ---- copy warp: one thread walks the same tile list; it loads two tiles ahead of the one being
-    // stored and stores tile n as soon as the eight transform warps have left it, so the transform
+    // ---- copy warp: one thread walks the same tile list; it stores tile n as soon as the eight
+    // transform warps have left it and refills the buffer with tile n + NBUF at once, so the transform
     // warps never wait for one another and drift into different phases (butterflies of one warp
     // over the scratch exchange of another)
     if (w == 8) {
         if (lane != 0) return;
         int pg = blockIdx.x, psub = 0;
-        for (int q = 0; q < 2; ++q) {
+        for (int q = 0; q < S::NBUF; ++q) {
             if (pg < nItems) {
                 mbar_expect_tx(fullB + q, S::TILE_BYTES);
                 bulk_load(s_B + q * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + q);
@@ -113,11 +113,10 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
                 mbar_wait(doneB + b, (uint32_t)((n / S::NBUF) & 1));
                 bulk_store(tile_ptr(g, sub), s_B + b * S::TILE_ELEMS, S::TILE_BYTES);
                 bulk_commit();
-                bulk_wait_read<1>();          // the store of tile n-1 has left its buffer
+                bulk_wait_read<0>();          // the store has left the buffer: refill it with tile n + NBUF
                 if (pg < nItems) {
-                    const int nb = (n + 2) % S::NBUF;
-                    mbar_expect_tx(fullB + nb, S::TILE_BYTES);
-                    bulk_load(s_B + nb * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + nb);
+                    mbar_expect_tx(fullB + b, S::TILE_BYTES);
+                    bulk_load(s_B + b * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + b);
                     if (psub + 1 < n_tiles(pg)) ++psub;
                     else { pg += G; psub = 0; }
                 }
@@ -286,7 +285,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
     constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     V *s_y = reinterpret_cast<V *>(smem);                   // LINES x YP
     V *s_z = s_y + LINES * G::YP;                           // LINES x PZ
     V *s_scr = s_z + LINES * G::PZ;
@@ -373,7 +372,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
     constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     V *s_z = reinterpret_cast<V *>(smem);                   // LINES x PZ; the output tile R x N (reals) aliases it
     T *s_out = reinterpret_cast<T *>(smem);
     V *s_scr = s_z + LINES * G::PZ;
@@ -473,7 +472,7 @@ k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, 
     typedef float2 V;
     typedef PySmem S;
     constexpr int M = 16;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     V *s_out = reinterpret_cast<V *>(smem);                                 // [P][8]
     V *s_in = reinterpret_cast<V *>(smem + S::B_BYTES);                     // 2 x [N][8]
     V *s_scr = reinterpret_cast<V *>(smem + S::B_BYTES + 2 * S::A_BYTES);
@@ -544,7 +543,7 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3
     typedef float2 V;
     typedef PySmem S;
     constexpr int M = 16;
-    extern __shared__ __align__(128) unsigned char smem[];
+    extern __shared__ __align__(1024) unsigned char smem[];
     V *s_in = reinterpret_cast<V *>(smem);                                  // [P][8]
     V *s_out = reinterpret_cast<V *>(smem + S::B_BYTES);                    // [N][8]
     V *s_scr = reinterpret_cast<V *>(smem + S::B_BYTES + S::A_BYTES);
@@ -611,10 +610,10 @@ bool nm_pipe_mid_ok(const nm_mesh *mesh)
 nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
 {
     const NmGeom &g = mesh->g;
-    NM_CUDA_TRY(cudaFuncSetAttribute(k_pz_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, PzSmem::BYTES));
     const int nItems = nkt * (g.N2 + 1);
     const int grid = nItems < mesh->sm_count ? nItems : mesh->sm_count;
     NmLaunchScope sc(mesh, NM_K_MID, st);
+    NM_CUDA_TRY(cudaFuncSetAttribute(k_pz_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, PzSmem::BYTES));
     k_pz_mid<<<grid, kMidThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn, g.N2,
                                                        nItems, kt0, (const float2 *)mesh->tw_z);
     return NM_OK;

@@ -530,6 +530,62 @@ __global__ void k_adj_cell(const NmAdjCellArgs<T> a)
     a.dudt[c] = -grad;
 }
 
+// The same without nodal Zeeman arrays, marching along z: a thread owns one cell column (c1, c2) of
+// a z chunk and keeps the sums over the four nodes (c1 + {0,1}, c2 + {0,1}) of the previous node
+// plane, so every plane costs four loads per array instead of eight (rows of a warp are contiguous;
+// the x + 1 / y + 1 overlaps are served by L1).
+template <typename T>
+__global__ void __launch_bounds__(256) k_adj_cell_march(const NmAdjCellArgs<T> a, int zchunk)
+{
+    const NmGeom &g = a.g;
+    const int c1 = blockIdx.x * 32 + threadIdx.x, c2 = blockIdx.y * 8 + threadIdx.y;
+    if (c1 >= g.N1 || c2 >= g.N2) return;
+    const int z0 = blockIdx.z * zchunk, z1 = min(z0 + zchunk, g.N3);
+    const long long nn = g.nodes;
+    const long long pl = (long long)g.n1 * g.n2;
+    const bool zee_on = (a.terms & NM_TERM_ZEEMAN) != 0;
+    T pw = 0, pq[3] = {0, 0, 0}, pm[3] = {0, 0, 0};
+    const T *w0 = a.W + (long long)z0 * pl + (long long)c2 * g.n1 + c1;
+    const T *q0 = a.Q + (long long)z0 * pl + (long long)c2 * g.n1 + c1;
+    const T *m0 = a.m + (long long)z0 * pl + (long long)c2 * g.n1 + c1;
+    long long c = ((long long)z0 * g.N2 + c2) * g.N1 + c1;
+    const long long cpl = (long long)g.N1 * g.N2;
+    for (int k = z0; k <= z1; ++k, w0 += pl, q0 += pl, m0 += pl) {
+        const int r1 = g.n1;
+        const T cw = (w0[0] + w0[1]) + (w0[r1] + w0[r1 + 1]);
+        T cq[3], cm[3];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const T *q = q0 + j * nn, *m = m0 + j * nn;
+            cq[j] = (q[0] + q[1]) + (q[r1] + q[r1 + 1]);
+            cm[j] = (m[0] + m[1]) + (m[r1] + m[r1 + 1]);
+        }
+        if (k > z0) {          // cell plane k - 1
+            const T sw = pw + cw;
+            T grad = -sw;
+            T sq[3], sm[3];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                sq[j] = pq[j] + cq[j];
+                sm[j] = pm[j] + cm[j];
+            }
+            if (zee_on) grad += sq[0] * a.hu[0] + sq[1] * a.hu[1] + sq[2] * a.hu[2];
+            if (a.Hc1) {
+#pragma unroll
+                for (int j = 0; j < 3; ++j) grad += sq[j] * a.Hc1[j * g.cells + c] + sm[j] * a.Hc2[j * g.cells + c];
+            }
+            a.dudt[c] = -grad;
+            c += cpl;
+        }
+        pw = cw;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            pq[j] = cq[j];
+            pm[j] = cm[j];
+        }
+    }
+}
+
 // out = base + sum_j coef_j src_j  (optionally normalised as 3-vectors over `vec_n` nodes)
 template <typename T> struct LinArgs {
     T *out;
@@ -641,7 +697,13 @@ template <typename T> nm_status nm_launch_adj_cell(nm_mesh *mesh, const NmAdjCel
 {
     {
         NmLaunchScope sc(mesh, NM_K_ADJ_CELL, st);
-        k_adj_cell<T><<<nblk(a.g.cells, 128), 128, 0, st>>>(a);
+        const bool zee_nodal = (a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse);
+        if (zee_nodal || a.g.N3 < 8) k_adj_cell<T><<<nblk(a.g.cells, 128), 128, 0, st>>>(a);
+        else {
+            const int zchunk = a.g.N3 >= 64 ? 32 : a.g.N3;
+            const dim3 grid((a.g.N1 + 31) / 32, (a.g.N2 + 7) / 8, (a.g.N3 + zchunk - 1) / zchunk);
+            k_adj_cell_march<T><<<grid, dim3(32, 8), 0, st>>>(a, zchunk);
+        }
     }
 
     NM_CUDA_TRY(cudaGetLastError());

@@ -151,6 +151,11 @@ nm_status nm_debug_get_cell_field(nm_mesh *mesh, void *Hc_out, void *stream);
 /* Number of kernel launches this library has issued on this mesh since create (for bench). */
 long long nm_launch_count(const nm_mesh *mesh);
 
+/* Which demag kernels serve this mesh (tests check that a grid takes the path they mean to cover):
+ * 0 no demag term or general-size kernels, 1 register-FFT fast path (every N_d = 16 * 2^k),
+ * 2 fast path on the zero-extended mesh (fp32; N2, N3 in (128, 256] rounded up to 256). */
+int nm_debug_demag_path(const nm_mesh *mesh);
+
 /* Per-kernel timing for the roofline line of bench.py.  Between
  * nm_profile_begin and nm_profile_end every kernel launch on this mesh is bracketed by a pair of
  * CUDA events on the launching stream (at most 4096 launches are recorded; later ones are only

@@ -23,7 +23,7 @@ NM_RK4, NM_DOPRI5 = 0, 1
 EXPORTS = ("nm_mesh_query_workspace", "nm_mesh_create", "nm_mesh_set_Ms", "nm_mesh_destroy",
            "nm_last_error", "nm_heff", "nm_llg_rhs", "nm_rk_step", "nm_llg_adjoint_rhs",
            "nm_adjoint_rk4_step", "nm_debug_get_tensor", "nm_debug_get_cell_field",
-           "nm_launch_count", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
+           "nm_launch_count", "nm_debug_demag_path", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
            "nm_profile_end")
 
 
@@ -85,13 +85,15 @@ def lib():
         L.nm_debug_get_cell_field.argtypes = [vp, vp, vp]
         L.nm_launch_count.argtypes = [vp]
         L.nm_launch_count.restype = ctypes.c_longlong
+        L.nm_debug_demag_path.argtypes = [vp]
+        L.nm_debug_demag_path.restype = ctypes.c_int
         L.nm_profile_class_count.argtypes = []
         L.nm_profile_class_name.argtypes = [i32]
         L.nm_profile_class_name.restype = ctypes.c_char_p
         L.nm_profile_begin.argtypes = [vp]
         L.nm_profile_end.argtypes = [vp, vp, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_longlong)]
         for name in EXPORTS:
-            if name not in ("nm_last_error", "nm_launch_count", "nm_profile_class_name"):
+            if name not in ("nm_last_error", "nm_launch_count", "nm_debug_demag_path", "nm_profile_class_name"):
                 getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -238,6 +240,9 @@ class Mesh:
 
     def nm_launch_count(self):
         return int(lib().nm_launch_count(self.handle))
+
+    def nm_debug_demag_path(self):
+        return int(lib().nm_debug_demag_path(self.handle))
 
     def nm_profile_begin(self):
         _check(lib().nm_profile_begin(self.handle))

@@ -67,6 +67,8 @@ void make_maps(const NmFftPlan &p, std::vector<int> &kmap, std::vector<int> &pos
     }
 }
 
+void make_geom(const nm_mesh_desc *d, NmGeom *g);
+
 nm_status validate(const nm_mesh_desc *d)
 {
     if (!d) { nm_set_error("desc is NULL"); return NM_EINVAL; }
@@ -84,8 +86,14 @@ nm_status validate(const nm_mesh_desc *d)
         if (std::fabs(n2 - 1.0) > 1e-9) { nm_set_error("ku_axis must be a unit vector"); return NM_EINVAL; }
     }
     if (d->terms & NM_TERM_DEMAG) {
+        // a mesh the zero-extended fast path serves needs no radix-2/3 factorisation of its own
+        NmGeom ge;
+        NmFast fe;
+        make_geom(d, &ge);
+        nm_fast_plan(d, ge, &fe);
+        const bool embedded = fe.on && fe.embed && !getenv("NM_DEMAG_PATH") && !getenv("NM_PIPE");
         for (int i = 0; i < 3; ++i)
-            if (d->n_cells[i] > 1 && !smooth23(d->n_cells[i])) {
+            if (!embedded && d->n_cells[i] > 1 && !smooth23(d->n_cells[i])) {
                 nm_set_error("n_cells[%d] = %d is not of the form 2^a 3^b (demag FFT radices)", i, d->n_cells[i]);
                 return NM_EUNSUPPORTED;
             }
@@ -212,6 +220,18 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
         m->fast.kt_chunk = ch ? atoi(ch) : 0;
         const char *pp = getenv("NM_PIPE");              // "0" forces the non-pipelined fast kernels
         m->fast.pipe = !(pp && strcmp(pp, "0") == 0);
+        if (m->fast.embed && !m->fast.pipe) m->fast.on = false;   // embedded meshes exist in the pipelined kernels only
+        if (!m->fast.on) m->fast.embed = false;
+    }
+    if (m->fast.on && m->fast.embed) {      // spectral extents follow the transform sizes
+        NmGeom &g = m->g;
+        const NmFast &f = m->fast;
+        g.P1 = 2 * f.F1; g.P2 = 2 * f.F2; g.P3 = 2 * f.F3;
+        g.C1 = f.F1 + 1;
+        g.C1p = (g.C1 + 3) & ~3;
+        g.K2 = f.F2 + 1;
+        g.K3 = f.F3 + 1;
+        g.Lx = f.F1;
     }
     make_plan(m->g.Lx, &m->plan_x);
     make_plan(m->g.P2, &m->plan_y);
@@ -435,6 +455,12 @@ extern "C" nm_status nm_profile_end(nm_mesh *mesh, void *stream, double *ms_host
 }
 
 extern "C" long long nm_launch_count(const nm_mesh *mesh) { return mesh ? mesh->launches : 0; }
+
+extern "C" int nm_debug_demag_path(const nm_mesh *mesh)
+{
+    if (!mesh || !mesh->fast.on) return 0;
+    return mesh->fast.embed ? 2 : 1;
+}
 
 extern "C" nm_status nm_debug_get_tensor(nm_mesh *mesh, double *N_host)
 {

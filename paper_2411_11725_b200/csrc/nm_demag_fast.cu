@@ -465,33 +465,51 @@ __global__ void k_tensor_store_fast(const double *__restrict__ in, T *__restrict
 } // namespace
 
 // Which grids the fast path serves, and its sizes.  Host only.
+// Exact sizes: every N_d in {16,...,256}.  Embedded sizes (fp32): any N_d <= 256 whose y and z
+// extents round up to 256 -- the convolution is then computed on the zero-extended 2 F_d grid
+// (longer than the 2 N_d - 1 a linear convolution needs, so the result is the same), the x passes
+// touching only the N1 x N2 x N3 cells that exist and the y / z passes masking the rows that do not.
 void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
 {
     f->on = false;
+    f->embed = false;
     if (!(d->terms & NM_TERM_DEMAG)) return;
-    int M[3];
+    int M[3], F[3];
     const int N[3] = {g.N1, g.N2, g.N3};
+    bool exact = true;
     for (int a = 0; a < 3; ++a) {
-        if (N[a] != 16 && N[a] != 32 && N[a] != 64 && N[a] != 128 && N[a] != 256) return;
-        M[a] = N[a] / 16;
+        if (N[a] > 256) return;
+        F[a] = 16;
+        while (F[a] < N[a]) F[a] *= 2;
+        if (F[a] != N[a]) exact = false;
+        M[a] = F[a] / 16;
     }
     const int LTx = 16 / M[0];
+    if (!exact) {
+        if (d->dtype != NM_F32 || F[1] != 256 || F[2] != 256) return;           // pipelined y / z kernels only
+        if (N[1] < 2 || N[2] < 2 || (long long)N[1] * N[2] * 2 < (long long)F[1] * F[2]) return;   // not worth the full z pass
+        if (N[1] % (2 * 8 * LTx) != 0 || N[0] % 4 != 0) return;               // whole CTAs of rows, 16-byte cell rows
+        f->embed = true;
+    }
     int W = kWarps;
-    while (W >= 1 && (g.N2 % (2 * LTx * W)) != 0) W >>= 1;
+    while (W >= 1 && (N[1] % (2 * LTx * W)) != 0) W >>= 1;
     if (W < 1) return;
     f->M1 = M[0]; f->M2 = M[1]; f->M3 = M[2];
+    f->F1 = F[0]; f->F2 = F[1]; f->F3 = F[2];
     f->Wx = W;
-    f->NKT = (g.C1 + TW - 1) / TW;
-    f->Kzp = (g.N3 + 1 + 1) & ~1;   // even: a warp's 6 rows are a multiple of 16 bytes
+    f->NKT = (F[0] + 1 + TW - 1) / TW;
+    f->Kzp = (F[2] + 1 + 1) & ~1;   // even: a warp's 6 rows are a multiple of 16 bytes
     f->on = true;
 }
 
+// (g here already carries the transform extents in P_d, C1, K_d)
 size_t nm_fast_tensor_elems(const NmGeom &g, const NmFast &f)
 {
-    return (size_t)f.NKT * (g.N2 + 1) * 6 * TW * f.Kzp;
+    return (size_t)f.NKT * g.K2 * 6 * TW * f.Kzp;
 }
-size_t nm_fast_bufA_elems(const NmGeom &g, const NmFast &f) { return (size_t)f.NKT * 3 * g.N3 * g.N2 * TW; }
-size_t nm_fast_bufB_elems(const NmGeom &g, const NmFast &f) { return (size_t)f.NKT * g.P2 * 3 * g.N3 * TW; }
+// A[kt][comp][c3 < N3][c2 < F2][8], B[kt][ky < 2 F2][comp][c3 < F3][8]
+size_t nm_fast_bufA_elems(const NmGeom &g, const NmFast &f) { return (size_t)f.NKT * 3 * g.N3 * f.F2 * TW; }
+size_t nm_fast_bufB_elems(const NmGeom &g, const NmFast &f) { return (size_t)f.NKT * g.P2 * 3 * f.F3 * TW; }
 
 nm_status nm_fast_store_tensor(nm_mesh *mesh, const double *octant, double scale, cudaStream_t st)
 {

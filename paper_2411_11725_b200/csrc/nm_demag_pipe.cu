@@ -42,9 +42,12 @@ struct PzSmem {
 constexpr int kMidThreads = 288;      // eight transform warps and one copy warp
 static_assert(PzSmem::BYTES <= 227 * 1024, "k_pz_mid shared memory exceeds the sm_100a per-CTA limit");
 
+// EMB: the mesh has n3v < 256 cell layers (embedded, nm_fast_plan): rows c3 >= n3v of a tile were
+// never written and enter the transform as zeros.
+template <bool EMB>
 __global__ void __launch_bounds__(kMidThreads, 1)
 k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItems, int kt0,
-         const float2 *__restrict__ wP)
+         const float2 *__restrict__ wP, int n3v)
 {
     typedef float T;
     typedef float2 V;
@@ -147,7 +150,10 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
 #pragma unroll
-                for (int t = 0; t < 16; ++t) a[c][t] = col[(c * N + M * t) * TW];
+                for (int t = 0; t < 16; ++t) {
+                    a[c][t] = col[(c * N + M * t) * TW];
+                    if (EMB && j + M * t >= n3v) a[c][t] = mk<T>((T)0, (T)0);
+                }
             }
             if (h) {
 #pragma unroll
@@ -277,10 +283,12 @@ template <> __device__ __forceinline__ void load2<double2>(const double2 *src, d
 //   phase 2  cell value = Ms/8 (ys2[e] + ys2[e+1]) on the way into the registers; transform
 //   phase 3  Xa[k] = (Z[k] + conj Z[P-k])/2, Xb[k] = (Z[k] - conj Z[P-k])/(2i), both rows of a line
 //            by one thread, 16-byte stores
-template <typename T, int M, bool UNI>
+// EMB (embedded mesh, nm_fast_plan): the mesh has N1 <= N cells per row; cells beyond it are zero, node
+// columns beyond n1 are not read, and the rows of A have pitch f2 (the y transform extent) >= N2.
+template <typename T, int M, bool UNI, bool EMB>
 __global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
 k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename VT<T>::V *__restrict__ A,
-         NmGeom g, const typename VT<T>::V *__restrict__ wP)
+         NmGeom g, const typename VT<T>::V *__restrict__ wP, int f2)
 {
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
@@ -298,12 +306,20 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     // Ms/8 of this thread's cells (rows 2 line, 2 line + 1; columns e = j + M t)
-    V msr[UNI ? 1 : 16];
-    if (UNI) msr[0] = mk<T>((T)0.125 * ms_uni, (T)0.125 * ms_uni);
+    constexpr bool MS1 = UNI && !EMB;                       // one Ms/8 for every cell of the thread
+    V msr[MS1 ? 1 : 16];
+    if (MS1) msr[0] = mk<T>((T)0.125 * ms_uni, (T)0.125 * ms_uni);
     else {
-        const T *mrow = Ms + ((long long)c3 * g.N2 + r0 + 2 * line) * N + j;
+        const int N1 = EMB ? g.N1 : N;
+        const T *mrow = Ms + ((long long)c3 * g.N2 + r0 + 2 * line) * N1 + j;
 #pragma unroll
-        for (int t = 0; t < 16; ++t) msr[UNI ? 0 : t] = mk<T>((T)0.125 * mrow[M * t], (T)0.125 * mrow[N + M * t]);
+        for (int t = 0; t < 16; ++t) {
+            V v;
+            if (EMB && j + M * t >= N1) v = mk<T>((T)0, (T)0);
+            else if (UNI) v = mk<T>((T)0.125 * ms_uni, (T)0.125 * ms_uni);
+            else v = mk<T>((T)0.125 * mrow[M * t], (T)0.125 * mrow[N1 + M * t]);
+            msr[MS1 ? 0 : t] = v;
+        }
     }
     const long long plane = (long long)g.n1 * g.n2;
     const int rg = tid / N, col = tid % N;                  // phase 1: row group (16 cell rows) and node column
@@ -312,13 +328,14 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
         {
             T z[17];
 #pragma unroll
-            for (int r = 0; r < 17; ++r) z[r] = base[(long long)r * g.n1 + col] + base[plane + (long long)r * g.n1 + col];
+            for (int r = 0; r < 17; ++r)
+                z[r] = (!EMB || col < g.n1) ? base[(long long)r * g.n1 + col] + base[plane + (long long)r * g.n1 + col] : (T)0;
 #pragma unroll
             for (int r = 0; r < 16; r += 2)
                 s_y[(rg * 8 + (r >> 1)) * G::YP + col] = mk<T>(z[r] + z[r + 1], z[r + 1] + z[r + 2]);
             if (tid < R) {   // last node column n1 = N
                 const T *q = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + tid) * g.n1 + N;
-                const T v = (q[0] + q[plane]) + (q[g.n1] + q[plane + g.n1]);
+                const T v = (!EMB || N < g.n1) ? (q[0] + q[plane]) + (q[g.n1] + q[plane + g.n1]) : (T)0;
                 reinterpret_cast<T *>(s_y + (tid >> 1) * G::YP + N)[tid & 1] = v;
             }
         }
@@ -328,7 +345,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
             const V v0 = yl[M * t], v1 = yl[M * t + 1];
-            const V mm = msr[UNI ? 0 : t];
+            const V mm = msr[MS1 ? 0 : t];
             a[t] = mk<T>(mm.x * (v0.x + v1.x), mm.y * (v0.y + v1.y));
         }
         if (h) shift32<T, false>(a);
@@ -351,7 +368,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
             V a1 = mk<T>(hf * (zb.x + mb.x), hf * (zb.y - mb.y)), b1 = mk<T>(hf * (zb.y + mb.y), hf * (mb.x - zb.x));
             if (k0 > N) { a0 = mk<T>((T)0, (T)0); b0 = a0; }
             if (k1 > N) { a1 = mk<T>((T)0, (T)0); b1 = a1; }
-            V *dst = A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + c2) * TW + p0;
+            V *dst = A + ((((long long)kt * 3 + comp) * g.N3 + c3) * f2 + c2) * TW + p0;
             store2(dst, a0, a1);
             store2(dst + TW, b0, b1);
         }
@@ -365,9 +382,10 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
 // the blocks of component c + 1 into a raw staging buffer while component c is transformed and
 // stored, so the global-load latency of a CTA is hidden behind its own arithmetic (the output tile
 // aliases the packed-line buffer, which keeps two CTAs per SM in fp32).
-template <typename T, int M>
+template <typename T, int M, bool EMB>
 __global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
-k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, const typename VT<T>::V *__restrict__ wP)
+k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, const typename VT<T>::V *__restrict__ wP,
+         int f2)
 {
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
@@ -389,7 +407,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     auto stage = [&](int comp) {
         for (int e = tid; e < NKT * PIECES; e += kPipeThreads) {
             const int kt = e / PIECES, off = e - kt * PIECES;
-            const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW) + off * 16;
+            const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + c3) * f2 + r0) * TW) + off * 16;
             // fp32: the two rows of every second line swap places, so that the 16-byte reads of a
             // quarter warp below (rows 2 ln of two lines) fall into different halves of the banks
             const int es = sizeof(V) == 8 ? e ^ (((e >> 3) & 1) << 2) : e;
@@ -440,11 +458,19 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             }
         }
         __syncthreads();
-        // R consecutive rows of Hc are contiguous
-        T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * N;
         constexpr int VEC = 16 / sizeof(T);
-        for (int idx = tid; idx < R * N / VEC; idx += kPipeThreads)
-            reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[idx];
+        if (!EMB) {     // R consecutive rows of Hc are contiguous
+            T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * N;
+            for (int idx = tid; idx < R * N / VEC; idx += kPipeThreads)
+                reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[idx];
+        } else {        // rows of N1 <= N cells (N1 a multiple of 4): the first N1 columns of every tile row
+            const int pr = g.N1 / VEC;
+            T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * g.N1;
+            for (int idx = tid; idx < R * pr; idx += kPipeThreads) {
+                const int row = idx / pr, cv = idx - row * pr;
+                reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[row * (N / VEC) + cv];
+            }
+        }
     }
 }
 
@@ -464,9 +490,11 @@ struct PySmem {
     static constexpr int INV_BYTES = B_BYTES + A_BYTES + SCR_BYTES + 64;
 };
 
+// EMB: rows c2 >= n2v of an A tile were never written (embedded mesh) and enter as zeros.
+template <bool EMB>
 __global__ void __launch_bounds__(kPipeThreads, 2)
 k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
-         const float2 *__restrict__ wP)
+         const float2 *__restrict__ wP, int n2v)
 {
     typedef float T;
     typedef float2 V;
@@ -510,7 +538,10 @@ k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, 
         const V *in = s_in + b * S::A_ELEMS + cin;
         V a[16];
 #pragma unroll
-        for (int t = 0; t < 16; ++t) a[t] = in[M * t * TW];
+        for (int t = 0; t < 16; ++t) {
+            a[t] = in[M * t * TW];
+            if (EMB && j + M * t >= n2v) a[t] = mk<T>((T)0, (T)0);
+        }
         __syncthreads();                                    // stage b is free again
         if (tid == 0 && tl + 2 * G < nTiles) {
             mbar_expect_tx(full + b, S::A_BYTES);
@@ -610,12 +641,18 @@ bool nm_pipe_mid_ok(const nm_mesh *mesh)
 nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
 {
     const NmGeom &g = mesh->g;
-    const int nItems = nkt * (g.N2 + 1);
+    const int nItems = nkt * g.K2;
     const int grid = nItems < mesh->sm_count ? nItems : mesh->sm_count;
     NmLaunchScope sc(mesh, NM_K_MID, st);
-    NM_CUDA_TRY(cudaFuncSetAttribute(k_pz_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, PzSmem::BYTES));
-    k_pz_mid<<<grid, kMidThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn, g.N2,
-                                                       nItems, kt0, (const float2 *)mesh->tw_z);
+    if (mesh->fast.embed) {
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_pz_mid<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PzSmem::BYTES));
+        k_pz_mid<true><<<grid, kMidThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn,
+                                                                 mesh->fast.F2, nItems, kt0, (const float2 *)mesh->tw_z, g.N3);
+    } else {
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_pz_mid<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PzSmem::BYTES));
+        k_pz_mid<false><<<grid, kMidThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn,
+                                                                  mesh->fast.F2, nItems, kt0, (const float2 *)mesh->tw_z, g.N3);
+    }
     return NM_OK;
 }
 
@@ -626,21 +663,26 @@ template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, co
     typedef PxGeom<T, M> G;
     const NmGeom &g = mesh->g;
     const dim3 grid(g.N2 / G::R, g.N3);
+    const int f2 = mesh->fast.F2;
     if (!inverse) {
         NmLaunchScope sc(mesh, NM_K_X_FWD, st);
-        if (mesh->uni_Ms) {
-            NM_CUDA_TRY(cudaFuncSetAttribute(k_px_fwd<T, M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::FWD_BYTES));
-            k_px_fwd<T, M, true><<<grid, kPipeThreads, G::FWD_BYTES, st>>>(fld, (const T *)mesh->Ms, (T)mesh->desc.Ms_scalar,
-                                                                          (V *)mesh->bufA, g, (const V *)mesh->fast.wPx);
-        } else {
-            NM_CUDA_TRY(cudaFuncSetAttribute(k_px_fwd<T, M, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::FWD_BYTES));
-            k_px_fwd<T, M, false><<<grid, kPipeThreads, G::FWD_BYTES, st>>>(fld, (const T *)mesh->Ms, (T)0, (V *)mesh->bufA, g,
-                                                                           (const V *)mesh->fast.wPx);
-        }
+        auto go = [&](auto kern, T ms) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::FWD_BYTES));
+            kern<<<grid, kPipeThreads, G::FWD_BYTES, st>>>(fld, (const T *)mesh->Ms, ms, (V *)mesh->bufA, g,
+                                                           (const V *)mesh->fast.wPx, f2);
+            return NM_OK;
+        };
+        const T ms = (T)mesh->desc.Ms_scalar;
+        if (mesh->fast.embed) NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, true>, ms) : go(k_px_fwd<T, M, false, true>, (T)0));
+        else NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, false>, ms) : go(k_px_fwd<T, M, false, false>, (T)0));
     } else {
         NmLaunchScope sc(mesh, NM_K_X_INV, st);
-        NM_CUDA_TRY(cudaFuncSetAttribute(k_px_inv<T, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::INV_BYTES));
-        k_px_inv<T, M><<<grid, kPipeThreads, G::INV_BYTES, st>>>((const V *)mesh->bufA, Hc, g, (const V *)mesh->fast.wPx);
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::INV_BYTES));
+            kern<<<grid, kPipeThreads, G::INV_BYTES, st>>>((const V *)mesh->bufA, Hc, g, (const V *)mesh->fast.wPx, f2);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_px_inv<T, M, true>) : go(k_px_inv<T, M, false>));
     }
     return NM_OK;
 }
@@ -685,11 +727,15 @@ nm_status nm_pipe_setup(nm_mesh *mesh)
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
         qres != cudaDriverEntryPointSuccess) {
         cudaGetLastError();
+        if (mesh->fast.embed) {
+            nm_set_error("embedded meshes need cuTensorMapEncodeTiled");
+            return NM_EUNSUPPORTED;
+        }
         return NM_OK;                       // the non-pipelined y kernels serve instead
     }
     const NmGeom &g = mesh->g;
-    const cuuint64_t dims[4] = {16, (cuuint64_t)g.N3, 3, (cuuint64_t)mesh->fast.NKT * g.P2};
-    const cuuint64_t strides[3] = {64, (cuuint64_t)g.N3 * 64, (cuuint64_t)3 * g.N3 * 64};
+    const cuuint64_t dims[4] = {16, (cuuint64_t)mesh->fast.F3, 3, (cuuint64_t)mesh->fast.NKT * g.P2};
+    const cuuint64_t strides[3] = {64, (cuuint64_t)mesh->fast.F3 * 64, (cuuint64_t)3 * mesh->fast.F3 * 64};
     const cuuint32_t box[4] = {16, 1, 1, 256};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = ((NmEncodeTiledFn)fn)((CUtensorMap *)&mesh->fast.tmapB, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, mesh->bufB,
@@ -711,10 +757,16 @@ nm_status nm_pipe_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t 
     const int nTiles = nkt * 3 * g.N3;
     const int grid = nTiles < 2 * mesh->sm_count ? nTiles : 2 * mesh->sm_count;
     if (!inverse) {
-        NM_CUDA_TRY(cudaFuncSetAttribute(k_py_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::FWD_BYTES));
         NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
-        k_py_fwd<<<grid, kPipeThreads, PySmem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3, nTiles, kt0,
-                                                              (const float2 *)mesh->tw_y);
+        if (mesh->fast.embed) {
+            NM_CUDA_TRY(cudaFuncSetAttribute(k_py_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::FWD_BYTES));
+            k_py_fwd<true><<<grid, kPipeThreads, PySmem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3,
+                                                                         nTiles, kt0, (const float2 *)mesh->tw_y, g.N2);
+        } else {
+            NM_CUDA_TRY(cudaFuncSetAttribute(k_py_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::FWD_BYTES));
+            k_py_fwd<false><<<grid, kPipeThreads, PySmem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3,
+                                                                          nTiles, kt0, (const float2 *)mesh->tw_y, g.N2);
+        }
     } else {
         NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::INV_BYTES));
         NmLaunchScope sc(mesh, NM_K_Y_INV, st);

@@ -55,7 +55,9 @@ struct alignas(64) NmTensorMap {
 // Fast demag path (nm_demag_fast.cu): sizes 16 M_d per axis, blocked spectrum layouts.
 struct NmFast {
     bool on;
-    int M1, M2, M3;    // N_d / 16
+    int M1, M2, M3;    // F_d / 16
+    int F1, F2, F3;    // transform extents: F_d = N_d, or the next fast size above N_d (embedded mesh)
+    bool embed;        // some F_d > N_d: the mesh is zero-extended to the fast size (fp32 pipelined kernels only)
     int Wx;            // warps per CTA of the x passes
     int NKT;           // k1 tiles of 8 columns
     int Kzp;           // pitch of the |kz| axis of the tensor

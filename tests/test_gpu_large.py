@@ -82,15 +82,17 @@ def _oracle_exchange_at(node, m, w, dtype):
     return H[(slice(None),) + q]
 
 
-def test_heff_256_sparse_sources_sampled_fp32():
-    """Bench configuration (256^3, fp32, exchange + demag): sampled H^cell and nodal H_eff."""
+@pytest.mark.parametrize("N", [256, 192])
+def test_heff_sparse_sources_sampled_fp32(N):
+    """Bench configuration (256^3, fp32, exchange + demag) and the 192^3 point of the sweep (fast
+    path on the mesh zero-extended to 256^3): sampled H^cell and nodal H_eff."""
     from oracle import demag, mesh as omesh
-    N = 256
     w = wl.config4_sweep(N)
     nd = np.float32
     m, pts = _sparse_field(w.node_shape, 120, seed=2561)
     m = wl.round_to(m, nd)
     msh = gpu_mesh(w, torch.float32)
+    assert msh.nm_debug_demag_path() == (1 if N == 256 else 2)
     H = host(msh.nm_heff(0.0, dev(m, torch.float32)))
     Hc = host(msh.nm_debug_get_cell_field())
 
@@ -111,7 +113,7 @@ def test_heff_256_sparse_sources_sampled_fp32():
     rng = np.random.default_rng(2562)
     cells = [tuple(int(v) for v in rng.integers(0, N, 3)) for _ in range(40)]
     cells += [tuple(int(v) for v in src_idx[i]) for i in rng.integers(0, len(src_idx), 20)]
-    cells += [(0, 0, 0), (N - 1, N - 1, N - 1), (N - 1, 0, 17), (128, 128, 128), (127, 128, 255)]
+    cells += [(0, 0, 0), (N - 1, N - 1, N - 1), (N - 1, 0, 17), (128, 128, 128), (127, 128, N - 1)]
     ref_c = _oracle_cell_field_at(cells, src_idx, src_M, w.dx)
     got_c = np.array([Hc[(slice(None),) + c] for c in cells])
     peak = np.abs(Hc).max()
@@ -132,11 +134,11 @@ def test_heff_256_sparse_sources_sampled_fp32():
     assert rel_l2(np.array(got_n), np.array(ref_n)) <= 1e-5
 
 
-def test_uniform_cube_256_demag_factor_fp32():
-    """Uniformly magnetised 256^3 cube: the L-weighted mean nodal demag field is -Ms/3 along m
+@pytest.mark.parametrize("N", [256, 192])
+def test_uniform_cube_demag_factor_fp32(N):
+    """Uniformly magnetised N^3 cube: the L-weighted mean nodal demag field is -Ms/3 along m
     (magnetometric factor of a cube, exact for the discrete operator: oracle pin
     test_uniform_cube_magnetometric_factor), zero across, and the exchange field vanishes."""
-    N = 256
     w = wl.config4_sweep(N)
     msh = gpu_mesh(w, torch.float32)
     m = torch.zeros(msh.node_shape_abi, dtype=torch.float32, device="cuda:0")
@@ -154,3 +156,22 @@ def test_uniform_cube_256_demag_factor_fp32():
     Hz = H[2]
     assert float((Hz - Hz.flip(0)).abs().max()) <= 2e-5 * Ms
     assert float((Hz - Hz.flip(2)).abs().max()) <= 2e-5 * Ms
+
+
+@pytest.mark.parametrize("n", [(36, 192, 176), (20, 256, 144)])
+def test_heff_embedded_sizes_dense_fp32(n):
+    """Grids served by the fast path on the zero-extended mesh (N2, N3 rounded up to 256, N1 to the
+    next 16 * 2^k): all terms, cell-wise random Ms with a vacuum block, A, Ku, nodal static field;
+    every node against the oracle."""
+    from oracle import llg
+    from _sides import gpu_zeeman, oracle_zeeman
+    w, hs = wl.varied_case(n, vacuum=True)
+    nd = np.float32
+    p = oracle_problem(w, nd)
+    m = wl.round_to(w.m0, nd)
+    z = oracle_zeeman(w, nd, hs)
+    ref = llg.effective_field(p, m, z(0.0) if z else None)
+    mesh = gpu_mesh(w, torch.float32)
+    assert mesh.nm_debug_demag_path() == 2
+    H = host(mesh.nm_heff(0.0, dev(m, torch.float32), gpu_zeeman(w, torch.float32, h_static=hs)))
+    assert rel_l2(H, ref) <= 1e-5

@@ -61,7 +61,9 @@ typedef enum { NM_RK4 = 0, NM_DOPRI5 = 1 } nm_scheme;
 /* Statement of the problem: regular grid, nodal m, cell-wise materials. */
 typedef struct {
     int n_cells[3];       /* N1, N2, N3 >= 1.  With NM_TERM_DEMAG every N_d > 1 must be
-                             2^a 3^b (FFT radices 2,3,4,8), else NM_EUNSUPPORTED. */
+                             2^a 3^b (FFT radices 2,3,4,8), else NM_EUNSUPPORTED -- except
+                             fp32 meshes the zero-extended fast path serves (N_d <= 256,
+                             N2 and N3 in (128, 256]; see nm_debug_demag_path), any N_d. */
     double cell_size[3];  /* metres, > 0 */
     nm_dtype dtype;
     int device;           /* CUDA device ordinal */

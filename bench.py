@@ -293,6 +293,11 @@ def run_b200(args):
     # ---- breakdown: the three calls of BASELINE.json's metric, timed alone ----
     H = torch.empty_like(m)
     reps = max(5, args.steps)
+    _timed = timed
+
+    def timed(fn, n):       # one untimed call first: a kernel variant's first launch loads its module
+        fn()
+        return _timed(fn, n)
     t_heff = over_ranks(timed(lambda: mesh.nm_heff(0.0, m, None, H), reps)) / reps
     t_rhs = over_ranks(timed(lambda: mesh.nm_llg_rhs(0.0, m, None, H), reps)) / reps
     t_rk4 = over_ranks(timed(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, m), reps)) / reps

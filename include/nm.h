@@ -62,8 +62,9 @@ typedef enum { NM_RK4 = 0, NM_DOPRI5 = 1 } nm_scheme;
 typedef struct {
     int n_cells[3];       /* N1, N2, N3 >= 1.  With NM_TERM_DEMAG every N_d > 1 must be
                              2^a 3^b (FFT radices 2,3,4,8), else NM_EUNSUPPORTED -- except
-                             fp32 meshes the zero-extended fast path serves (N_d <= 256,
-                             N2 and N3 in (128, 256]; see nm_debug_demag_path), any N_d. */
+                             meshes the zero-extended fast path serves (2 <= N_d <= 256 that
+                             fill half of the (y, z) plane of the next sizes 16 * 2^k and
+                             meet its row granularities; see nm_debug_demag_path), any N_d. */
     double cell_size[3];  /* metres, > 0 */
     nm_dtype dtype;
     int device;           /* CUDA device ordinal */
@@ -155,7 +156,7 @@ long long nm_launch_count(const nm_mesh *mesh);
 
 /* Which demag kernels serve this mesh (tests check that a grid takes the path they mean to cover):
  * 0 no demag term or general-size kernels, 1 register-FFT fast path (every N_d = 16 * 2^k),
- * 2 fast path on the zero-extended mesh (fp32; N2, N3 in (128, 256] rounded up to 256). */
+ * 2 fast path on the mesh zero-extended to the next sizes 16 * 2^k. */
 int nm_debug_demag_path(const nm_mesh *mesh);
 
 /* Per-kernel timing for the roofline line of bench.py.  Between

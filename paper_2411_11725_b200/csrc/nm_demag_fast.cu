@@ -38,7 +38,7 @@ template <typename V> __device__ __forceinline__ void copy_in(V *dst, const V *_
 template <typename T, int M>
 __global__ void __launch_bounds__(kThreadsF)
 k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict__ B, int N3, int kt0,
-         const typename VT<T>::V *__restrict__ wP)
+         const typename VT<T>::V *__restrict__ wP, int F3, int n2v)
 {
     typedef typename VT<T>::V V;
     constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
@@ -64,6 +64,7 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
     for (int t = 0; t < 16; ++t) {
         const int e = j + M * t;
         V v = s_io[(sub * N + e) * TW + (k1 ^ swz(e))];
+        if (e >= n2v) v = mk<T>((T)0, (T)0);                // embedded mesh: rows the x pass never wrote
         if (h) v = cmul(v, wP[e]);
         a[t] = v;
     }
@@ -78,10 +79,10 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
     }
     __syncthreads();
     // rows of LT*8 complex, one per ky
-    V *dst = B + ((long long)ktl * P * 3 + comp) * N3 * TW + (long long)c3_0 * TW;
+    V *dst = B + ((long long)ktl * P * 3 + comp) * F3 * TW + (long long)c3_0 * TW;     // B keeps F3 >= N3 planes
     for (int idx = threadIdx.x; idx < P * LT * TW; idx += blockDim.x) {
         const int ky = idx / (LT * TW), r = idx % (LT * TW);
-        dst[(long long)ky * 3 * N3 * TW + r] = s_io[ky * OUT_PITCH + r];
+        dst[(long long)ky * 3 * F3 * TW + r] = s_io[ky * OUT_PITCH + r];
     }
 }
 
@@ -89,7 +90,7 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
 template <typename T, int M>
 __global__ void __launch_bounds__(kThreadsF)
 k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict__ A, int N3, int kt0,
-         const typename VT<T>::V *__restrict__ wP)
+         const typename VT<T>::V *__restrict__ wP, int F3)
 {
     typedef typename VT<T>::V V;
     constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
@@ -101,10 +102,10 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
     const int comp = blockIdx.y;
     const int kt = kt0 + blockIdx.z;
     const int ktl = blockIdx.z;
-    const V *src = B + ((long long)ktl * P * 3 + comp) * N3 * TW + (long long)c3_0 * TW;
+    const V *src = B + ((long long)ktl * P * 3 + comp) * F3 * TW + (long long)c3_0 * TW;
     for (int idx = threadIdx.x; idx < P * LT * TW; idx += blockDim.x) {
         const int ky = idx / (LT * TW), r = idx % (LT * TW);
-        s_io[ky * PITCH + r] = src[(long long)ky * 3 * N3 * TW + r];
+        s_io[ky * PITCH + r] = src[(long long)ky * 3 * F3 * TW + r];
     }
     __syncthreads();
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -141,10 +142,10 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
 // z forward, tensor multiply, z inverse, in place on B.  CTA = LT consecutive ky of one kt.
 //   Tn[kt][|ky|][k1][6][|kz|] (pitch Kzp), components xx,yy,zz,xy,xz,yz, scaled by 1/(P1 P2 P3);
 //   off-diagonal components are odd in their two axes: sign -1 per folded axis (ky > N2, kz > N3).
-template <typename T, int M>
+template <typename T, int M, bool EMB>
 __global__ void __launch_bounds__(kThreadsF)
 k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, int kt0, int Kzp,
-         const typename VT<T>::V *__restrict__ wP)
+         const typename VT<T>::V *__restrict__ wP, int n3v)
 {
     typedef typename VT<T>::V V;
     constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
@@ -180,6 +181,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
         for (int t = 0; t < 16; ++t) {
             const int e = j + M * t;
             V v = my[(c * N + e) * TW + (kq ^ swz(e))];
+            if (EMB && e >= n3v) v = mk<T>((T)0, (T)0);     // embedded mesh: planes the y pass never wrote
             if (h) v = cmul(v, wP[e]);
             a[c][t] = v;
         }
@@ -404,12 +406,12 @@ nm_status launch_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t s
         NM_TRY(set_smem_f(k_fy_fwd<T, M>, sm));
         NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
         k_fy_fwd<T, M><<<grid, kThreadsF, sm, st>>>((const V *)mesh->bufA, (V *)mesh->bufB, g.N3, kt0,
-                                                    (const V *)mesh->tw_y);
+                                                    (const V *)mesh->tw_y, mesh->fast.F3, g.N2);
     } else {
         NM_TRY(set_smem_f(k_fy_inv<T, M>, sm));
         NmLaunchScope sc(mesh, NM_K_Y_INV, st);
         k_fy_inv<T, M><<<grid, kThreadsF, sm, st>>>((const V *)mesh->bufB, (V *)mesh->bufA, g.N3, kt0,
-                                                    (const V *)mesh->tw_y);
+                                                    (const V *)mesh->tw_y, mesh->fast.F3);
     }
     return NM_OK;
 }
@@ -422,11 +424,17 @@ nm_status launch_z(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     constexpr int N = 16 * M, LT = 16 / M;
     if (nm_pipe_mid_ok(mesh)) return nm_pipe_mid(mesh, kt0, nkt, st);
     const size_t sm = (size_t)LT * 3 * N * TW * sizeof(V) + scratch_bytes<T>(kWarps);
-    NM_TRY(set_smem_f(k_fz_mid<T, M>, sm));
     const dim3 grid(g.P2 / LT, nkt);
     NmLaunchScope sc(mesh, NM_K_MID, st);
-    k_fz_mid<T, M><<<grid, kThreadsF, sm, st>>>((V *)mesh->bufB, (const T *)mesh->fast.Tn, g.N2, kt0,
-                                                mesh->fast.Kzp, (const V *)mesh->tw_z);
+    if (mesh->fast.embed) {
+        NM_TRY(set_smem_f(k_fz_mid<T, M, true>, sm));
+        k_fz_mid<T, M, true><<<grid, kThreadsF, sm, st>>>((V *)mesh->bufB, (const T *)mesh->fast.Tn, mesh->fast.F2, kt0,
+                                                          mesh->fast.Kzp, (const V *)mesh->tw_z, g.N3);
+    } else {
+        NM_TRY(set_smem_f(k_fz_mid<T, M, false>, sm));
+        k_fz_mid<T, M, false><<<grid, kThreadsF, sm, st>>>((V *)mesh->bufB, (const T *)mesh->fast.Tn, mesh->fast.F2, kt0,
+                                                           mesh->fast.Kzp, (const V *)mesh->tw_z, g.N3);
+    }
     return NM_OK;
 }
 
@@ -465,8 +473,9 @@ __global__ void k_tensor_store_fast(const double *__restrict__ in, T *__restrict
 } // namespace
 
 // Which grids the fast path serves, and its sizes.  Host only.
-// Exact sizes: every N_d in {16,...,256}.  Embedded sizes (fp32): any N_d <= 256 whose y and z
-// extents round up to 256 -- the convolution is then computed on the zero-extended 2 F_d grid
+// Exact sizes: every N_d in {16,...,256}.  Embedded sizes: any 2 <= N_d <= 256 that fills at least
+// half of the (y, z) plane of the next fast sizes F_d and meets the CTA granularities below -- the
+// convolution is then computed on the zero-extended 2 F_d grid
 // (longer than the 2 N_d - 1 a linear convolution needs, so the result is the same), the x passes
 // touching only the N1 x N2 x N3 cells that exist and the y / z passes masking the rows that do not.
 void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
@@ -486,9 +495,22 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
     }
     const int LTx = 16 / M[0];
     if (!exact) {
-        if (d->dtype != NM_F32 || F[1] != 256 || F[2] != 256) return;           // pipelined y / z kernels only
-        if (N[1] < 2 || N[2] < 2 || (long long)N[1] * N[2] * 2 < (long long)F[1] * F[2]) return;   // not worth the full z pass
-        if (N[1] % (2 * 8 * LTx) != 0 || N[0] % 4 != 0) return;               // whole CTAs of rows, 16-byte cell rows
+        const int vec = d->dtype == NM_F64 ? 2 : 4;
+        if (N[0] < 2 || N[1] < 2 || N[2] < 2) return;                           // films and rods: the 2-D / 1-D general path
+        // a mesh the general path can serve (every N_d = 2^a 3^b) is embedded only where that is faster:
+        // it must fill 1/2 (fp32) or 3/4 (fp64) of the (y, z) plane the z pass transforms in full
+        bool smooth = true;
+        for (int a = 0; a < 3; ++a) {
+            int v = N[a];
+            while (v % 2 == 0) v /= 2;
+            while (v % 3 == 0) v /= 3;
+            if (v != 1) smooth = false;
+        }
+        const long long fill = (long long)N[1] * N[2] * 4, plane = (long long)F[1] * F[2];
+        if (smooth && fill < (d->dtype == NM_F64 ? 3 : 2) * plane) return;
+        if (N[1] % (2 * 8 * LTx) != 0 || N[0] % vec != 0) return;              // whole x-pass CTAs of rows, 16-byte cell rows
+        if (N[2] % (16 / M[1]) != 0) return;                                   // whole y-pass CTAs of planes
+        if (d->dtype == NM_F64 && M[0] == 1) return;                           // no staged fp64 x pass at N1 = 16
         f->embed = true;
     }
     int W = kWarps;

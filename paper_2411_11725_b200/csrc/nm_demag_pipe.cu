@@ -727,10 +727,6 @@ nm_status nm_pipe_setup(nm_mesh *mesh)
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
         qres != cudaDriverEntryPointSuccess) {
         cudaGetLastError();
-        if (mesh->fast.embed) {
-            nm_set_error("embedded meshes need cuTensorMapEncodeTiled");
-            return NM_EUNSUPPORTED;
-        }
         return NM_OK;                       // the non-pipelined y kernels serve instead
     }
     const NmGeom &g = mesh->g;

@@ -87,6 +87,18 @@ def test_heff_fast_path_sizes(n, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(36, 128, 112), (68, 96, 100), (52, 64, 40), (100, 32, 24)])
+def test_heff_embedded_fast_path_sizes(n, prec):
+    """Grids the fast path serves on the zero-extended mesh (some N_d below the next 16 * 2^k, not
+    necessarily 2^a 3^b), non-pipelined y / z kernels, both precisions; all terms, cell-wise
+    materials, vacuum block."""
+    w, hs = wl.varied_case(n, vacuum=True)
+    got, ref, mesh, *_ = _heff_case(w, prec, hs)
+    assert mesh.nm_debug_demag_path() == 2
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
 def test_heff_term_by_term(prec):
     """Each term alone against the oracle's part (a dropped or mis-signed term cannot hide)."""
     from oracle import llg

@@ -236,6 +236,204 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 }
 
 
+// ---- z pass, 128 cells along z ---------------------------------------------------------------------
+// The same pipeline for N3 = 128 (M = 8): a team transforms two lines at once, so a warp owns two
+// columns of a tile and four warps a whole tile; warps 0-3 take the +ky tile of an item and warps
+// 4-7 the -ky tile at the same time (both read the same folded tensor rows, staged once per column
+// pair).  A buffer holds the tile pair of one item (2 x 24 KB).  The copy warp also brings the
+// tensor rows of item n + 1 as soon as the eight warps have finished the products of item n
+// (`freeT`), half an item before it stores item n.
+struct Pz8Smem {
+    static constexpr int N = 128;
+    static constexpr int TILE_ELEMS = 3 * N * TW;                   // complex
+    static constexpr int TILE_BYTES = TILE_ELEMS * 8;               // 24576
+    static constexpr int SLOT_ELEMS = 2 * TILE_ELEMS;
+    static constexpr int NBUF = 3;
+    static constexpr int KZP = 130;                                 // tensor |kz| pitch (reals), even
+    static constexpr int TSLICE = 2 * 6 * KZP;                      // reals per column pair (6240 B, one bulk copy)
+    static constexpr int WSCR = 2 * Team<8>::SCRATCH - 8;
+    static constexpr int OFF_T = NBUF * 2 * TILE_BYTES;
+    static constexpr int OFF_SCR = OFF_T + 4 * TSLICE * 4;
+    static constexpr int OFF_BAR = OFF_SCR + 8 * WSCR * 8;
+    static constexpr int BYTES = OFF_BAR + (2 * NBUF + 2) * 8;
+};
+static_assert(Pz8Smem::BYTES <= 227 * 1024, "k_pz_mid8 shared memory exceeds the sm_100a per-CTA limit");
+static_assert((Pz8Smem::TSLICE * 4) % 16 == 0 && Pz8Smem::OFF_SCR % 16 == 0 && Pz8Smem::OFF_BAR % 8 == 0, "alignment");
+
+template <bool EMB>
+__global__ void __launch_bounds__(kMidThreads, 1)
+k_pz_mid8(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItems, int kt0,
+          const float2 *__restrict__ wP, int n3v)
+{
+    typedef float T;
+    typedef float2 V;
+    typedef Pz8Smem S;
+    constexpr int M = 8, N = 128, P = 256;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    V *s_B = reinterpret_cast<V *>(smem);
+    T *s_T = reinterpret_cast<T *>(smem + S::OFF_T);
+    V *s_scr = reinterpret_cast<V *>(smem + S::OFF_SCR);
+    uint64_t *fullB = reinterpret_cast<uint64_t *>(smem + S::OFF_BAR);
+    uint64_t *doneB = fullB + S::NBUF;
+    uint64_t *fullT = doneB + S::NBUF;      // one barrier for the four slices of an item
+    uint64_t *freeT = fullT + 1;
+
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int P2 = 2 * N2, K2 = N2 + 1;
+    const int G = gridDim.x;
+
+    if (tid == 0) {
+        for (int q = 0; q < S::NBUF; ++q) {
+            mbar_init(fullB + q, 1);
+            mbar_init(doneB + q, 8);
+        }
+        mbar_init(fullT, 1);
+        mbar_init(freeT, 8);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto tile_ptr = [&](int g, int sub) -> V * {
+        const int kyf = g % K2, ktl = g / K2;
+        const int ky = sub ? P2 - kyf : kyf;
+        return B + ((long long)ktl * P2 + ky) * S::TILE_ELEMS;
+    };
+    auto n_tiles = [&](int g) -> int {
+        const int kyf = g % K2;
+        return (kyf == 0 || kyf == N2) ? 1 : 2;
+    };
+
+    if (w == 8) {           // copy warp
+        if (lane != 0) return;
+        auto load_item = [&](int g, int b) {
+            const int nt = n_tiles(g);
+            mbar_expect_tx(fullB + b, nt * S::TILE_BYTES);
+            for (int sub = 0; sub < nt; ++sub)
+                bulk_load(s_B + b * S::SLOT_ELEMS + sub * S::TILE_ELEMS, tile_ptr(g, sub), S::TILE_BYTES, fullB + b);
+        };
+        // tensor rows of item g: Tn[kt][|ky|][k1 = 0..7][6][KZP], the eight columns contiguous
+        auto load_tensor = [&](int g) {
+            const int kyf = g % K2, kt = kt0 + g / K2;
+            const T *src = Tn + ((long long)kt * K2 + kyf) * TW * 6 * S::KZP;
+            mbar_expect_tx(fullT, 4 * S::TSLICE * 4);
+            bulk_load(s_T, src, 4 * S::TSLICE * 4, fullT);
+        };
+        int pg = blockIdx.x;
+        for (int q = 0; q < S::NBUF; ++q, pg += G)
+            if (pg < nItems) load_item(pg, q);
+        if ((int)blockIdx.x < nItems) load_tensor(blockIdx.x);
+        int n = 0;
+        for (int g = blockIdx.x; g < nItems; g += G, ++n) {
+            const int b = n % S::NBUF;
+            mbar_wait(freeT, (uint32_t)(n & 1));            // the products of item n are done
+            if (g + G < nItems) load_tensor(g + G);
+            mbar_wait(doneB + b, (uint32_t)((n / S::NBUF) & 1));
+            const int nt = n_tiles(g);
+            for (int sub = 0; sub < nt; ++sub)
+                bulk_store(tile_ptr(g, sub), s_B + b * S::SLOT_ELEMS + sub * S::TILE_ELEMS, S::TILE_BYTES);
+            bulk_commit();
+            bulk_wait_read<0>();
+            if (pg < nItems) {
+                load_item(pg, b);
+                pg += G;
+            }
+        }
+        bulk_wait<0>();
+        return;
+    }
+
+    // ---- transform warps: warp = (which tile of the pair, column pair), lane = (line, j, half)
+    const int sub = w >> 2, cp = w & 3;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i >> 3, j = i & 7;
+    const int k1 = 2 * cp + l;
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    V *scr = s_scr + w * S::WSCR + h * Team<M>::SCRATCH;
+    const T *ts = s_T + k1 * 6 * S::KZP;
+    int n = 0;
+    for (int g = blockIdx.x; g < nItems; g += G, ++n) {
+        const int kyf = g % K2;
+        const int nt = (kyf == 0 || kyf == N2) ? 1 : 2;
+        const int b = n % S::NBUF;
+        if (sub < nt) {
+            mbar_wait(fullB + b, (uint32_t)((n / S::NBUF) & 1));
+            // element (c, e = j + 8 t) of column k1: row (c N + e), slot k1 ^ swz(e) ^ swz(ky);
+            // swz(j + 8 t) = (j >> 1) ^ 4 (t & 1)
+            const int cw = k1 ^ swz(sub ? P2 - kyf : kyf) ^ (j >> 1);
+            V *colE = s_B + b * S::SLOT_ELEMS + sub * S::TILE_ELEMS + j * TW + cw;
+            V *colO = s_B + b * S::SLOT_ELEMS + sub * S::TILE_ELEMS + j * TW + (cw ^ 4);
+            V a[3][16];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    a[c][t] = ((t & 1) ? colO : colE)[(c * N + M * t) * TW];
+                    if (EMB && j + M * t >= n3v) a[c][t] = mk<T>((T)0, (T)0);
+                }
+            }
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, false>(a[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) fft_fwd<T, M, true>(a[c], tw, scr, i);
+            // H^ = -N^ M^ ; rows of the folded tensor: sign -1 per folded odd axis
+            mbar_wait(fullT, (uint32_t)(n & 1));
+            const T sy = sub ? (T)-1 : (T)1;
+#pragma unroll
+            for (int s = 0; s < 16; ++s) {
+                // kz = 2 (2 j + u + 16 rev8(p)) + h, s = 8 u + p: the side of the fold is fixed by the
+                // slot, except for the slot that straddles kz = N
+                const int u = s / M, r8 = rev8(s % M);
+                const int kz = 2 * slot_freq<M>(j, s) + h;
+                const bool up = r8 > 4 || (r8 == 4 && (j | u | h) != 0);
+                const int kzf = up ? P - kz : kz;
+                const T sz = up ? (T)-1 : (T)1;
+                const T *tp = ts + kzf;
+                const T nxx = tp[0], nyy = tp[S::KZP], nzz = tp[2 * S::KZP];
+                const T nxy = sy * tp[3 * S::KZP], nxz = sz * tp[4 * S::KZP], nyz = sy * sz * tp[5 * S::KZP];
+                const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
+                const V hx = caxpy(nxz, mz, caxpy(nxy, my_, cscale(nxx, mx)));
+                const V hy = caxpy(nyz, mz, caxpy(nyy, my_, cscale(nxy, mx)));
+                const V hz = caxpy(nzz, mz, caxpy(nyz, my_, cscale(nxz, mx)));
+                a[0][s] = mk<T>(-hx.x, -hx.y);
+                a[1][s] = mk<T>(-hy.x, -hy.y);
+                a[2][s] = mk<T>(-hz.x, -hz.y);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(freeT);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) fft_inv<T, M, true>(a[c], tw, scr, i);
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, true>(a[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    V v = a[c][t];
+                    v = cadd(v, shfl1(v));
+                    if ((t >> 3) == h) ((t & 1) ? colO : colE)[(c * N + M * t) * TW] = v;
+                }
+            }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(doneB + b);
+        } else {                    // the item has one tile only: this warp just keeps the barrier counts,
+            // after the same waits as a working warp (an arrival must not run into the previous phase)
+            mbar_wait(fullB + b, (uint32_t)((n / S::NBUF) & 1));
+            mbar_wait(fullT, (uint32_t)(n & 1));
+            if (lane == 0) {
+                mbar_arrive(freeT);
+                mbar_arrive(doneB + b);
+            }
+        }
+    }
+}
+
+
 // ---- x passes ----------------------------------------------------------------------------------
 // Geometry shared by k_px_fwd / k_px_inv for N1 = 16 M: a CTA of 8 warps owns R = 2 LINES cell rows
 // (c2) of one cell plane c3; warp w transforms LINES/8 = 16/M complex lines, each packing the two
@@ -635,7 +833,8 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3
 // ---- host side ----------------------------------------------------------------------------------
 bool nm_pipe_mid_ok(const nm_mesh *mesh)
 {
-    return mesh->fast.on && !mesh->f64 && mesh->fast.M3 == 16 && mesh->fast.Kzp == PzSmem::KZP && mesh->fast.pipe;
+    if (!mesh->fast.on || mesh->f64 || !mesh->fast.pipe) return false;
+    return (mesh->fast.M3 == 16 && mesh->fast.Kzp == PzSmem::KZP) || (mesh->fast.M3 == 8 && mesh->fast.Kzp == Pz8Smem::KZP);
 }
 
 nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
@@ -644,6 +843,16 @@ nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     const int nItems = nkt * g.K2;
     const int grid = nItems < mesh->sm_count ? nItems : mesh->sm_count;
     NmLaunchScope sc(mesh, NM_K_MID, st);
+    if (mesh->fast.M3 == 8) {
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pz8Smem::BYTES));
+            kern<<<grid, kMidThreads, Pz8Smem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn, mesh->fast.F2,
+                                                           nItems, kt0, (const float2 *)mesh->tw_z, g.N3);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_pz_mid8<true>) : go(k_pz_mid8<false>));
+        return NM_OK;
+    }
     if (mesh->fast.embed) {
         NM_CUDA_TRY(cudaFuncSetAttribute(k_pz_mid<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PzSmem::BYTES));
         k_pz_mid<true><<<grid, kMidThreads, PzSmem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn,

@@ -175,3 +175,60 @@ def test_heff_embedded_sizes_dense_fp32(n):
     assert mesh.nm_debug_demag_path() == 2
     H = host(mesh.nm_heff(0.0, dev(m, torch.float32), gpu_zeeman(w, torch.float32, h_static=hs)))
     assert rel_l2(H, ref) <= 1e-5
+
+
+def _bench_mesh_and_state(seed=7):
+    """The bench workload (config 4, 256^3, fp32) with its seeded m and a random adjoint vector."""
+    w = wl.config4_sweep(256)
+    msh = gpu_mesh(w, torch.float32)
+    m = dev(wl.round_to(w.m0, np.float32), torch.float32)
+    g = torch.Generator(device="cuda:0").manual_seed(seed)
+    a = torch.randn(m.shape, dtype=torch.float32, device="cuda:0", generator=g)
+    return w, msh, m, a
+
+
+def test_rk4_step_256_matches_stage_composition_fp32():
+    """nm_rk_step(NM_RK4) at the bench size (fused stage epilogues, no stored derivatives) against the
+    textbook composition of four nm_llg_rhs evaluations (whose field is checked at this size by the
+    sampled test above), combined in fp64 by torch; |m| = 1 after the step (reading C6)."""
+    w, msh, m, _ = _bench_mesh_and_state()
+    dt = w.dt
+    f = lambda y: msh.nm_llg_rhs(0.0, y.float().contiguous()).double()
+    y0 = m.double()
+    k1 = f(y0)
+    k2 = f(y0 + 0.5 * dt * k1)
+    k3 = f(y0 + 0.5 * dt * k2)
+    k4 = f(y0 + dt * k3)
+    ref = y0 + dt / 6.0 * (k1 + 2 * k2 + 2 * k3 + k4)
+    ref = ref / ref.norm(dim=0, keepdim=True)
+    y = m.clone()
+    msh.nm_rk_step(0, 0.0, dt, y)
+    err = float((y.double() - ref).norm() / ref.norm())
+    assert err <= 1e-6                      # the step changes m by ~1e-3: 1e-6 here is 1e-3 of the update
+    upd = float((y.double() - y0).norm() / y0.norm())
+    assert upd > 1e-5                       # the step did move m
+    assert float((y.double().norm(dim=0) - 1).abs().max()) <= 5e-7
+
+
+def test_adjoint_rhs_256_transpose_property_fp32():
+    """nm_llg_adjoint_rhs at the bench size: da/dt = -(df/dm)^T a, so for any direction v
+    <da/dt, v> = -<a, (df/dm) v>, the right side from a central difference of the forward RHS on the
+    GPU (fp32, hence the tolerance); linear in a; f returned alongside equals nm_llg_rhs."""
+    w, msh, m, a = _bench_mesh_and_state()
+    g = torch.Generator(device="cuda:0").manual_seed(11)
+    v = torch.randn(m.shape, dtype=torch.float32, device="cuda:0", generator=g)
+    # smooth the direction a little so that the difference quotient is well inside fp32's range
+    eps = 1e-2
+    fp = msh.nm_llg_rhs(0.0, (m + eps * v).contiguous()).double()
+    fm = msh.nm_llg_rhs(0.0, (m - eps * v).contiguous()).double()
+    jv = (fp - fm) / (2 * eps)
+    f, da, du = msh.nm_llg_adjoint_rhs(0.0, m, a)
+    lhs = float((da.double() * v.double()).sum())
+    rhs = -float((a.double() * jv).sum())
+    assert abs(lhs - rhs) <= 2e-3 * max(abs(lhs), abs(rhs))
+    f2 = msh.nm_llg_rhs(0.0, m)
+    assert float((f.double() - f2.double()).norm() / f2.double().norm()) <= 1e-6
+    # linearity in a
+    _, da2, du2 = msh.nm_llg_adjoint_rhs(0.0, m, (2.5 * a).contiguous())
+    assert float((da2.double() - 2.5 * da.double()).norm() / da2.double().norm()) <= 1e-5
+    assert float((du2.double() - 2.5 * du.double()).norm() / du2.double().norm()) <= 1e-4

@@ -49,10 +49,10 @@ def parse():
 
 
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class from the
-# committed `ncu --set full` capture of this command (profiles/r1d_packed.md); only for the workload
+# committed `ncu --set full` capture of this command (profiles/r1e_final.md); only for the workload
 # that capture was taken on (256^3, fp32)
-NCU_TRAFFIC = {(256, "f32"): {"mid": 2026074952, "y_fwd": 1194564056, "y_inv": 1217670008,
-                              "x_fwd": 566699912, "x_inv": 587649816, "node": 810019080}}
+NCU_TRAFFIC = {(256, "f32"): {"mid": 2025138896, "y_fwd": 1195136896, "y_inv": 1215810952,
+                              "x_fwd": 569166424, "x_inv": 586457048, "node": 808990384}}
 
 
 def peaks():
@@ -379,7 +379,7 @@ def run_b200(args):
     eval_bytes = sum(alg.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((N, args.dtype), {}).get(dom),
-                "traffic_source": "profiles/r1d_packed.md (ncu --set full, per launch)", "peak_source": peak_src,
+                "traffic_source": "profiles/r1e_final.md (ncu --set full, per launch)", "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg[dom], "launches": dom_n,
                 "avg_launch_ms": dom_ms / dom_n, "share_of_step": dom_ms / tot_ms}
     per_kernel = {k: {"ms_per_launch": prof[k][0] / prof[k][1], "launches": prof[k][1],

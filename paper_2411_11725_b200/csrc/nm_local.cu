@@ -698,9 +698,13 @@ template <typename T> nm_status nm_launch_adj_cell(nm_mesh *mesh, const NmAdjCel
     {
         NmLaunchScope sc(mesh, NM_K_ADJ_CELL, st);
         const bool zee_nodal = (a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse);
-        if (zee_nodal || a.g.N3 < 8) k_adj_cell<T><<<nblk(a.g.cells, 128), 128, 0, st>>>(a);
+        if (zee_nodal || a.g.N3 < 32) k_adj_cell<T><<<nblk(a.g.cells, 128), 128, 0, st>>>(a);
         else {
-            const int zchunk = a.g.N3 >= 64 ? 32 : a.g.N3;
+            // z chunks of 4..32 planes, short enough for about eight CTAs per SM
+            const int base = ((a.g.N1 + 31) / 32) * ((a.g.N2 + 7) / 8);
+            const int nz = (8 * mesh->sm_count + base - 1) / base;
+            int zchunk = (a.g.N3 + nz - 1) / nz;
+            zchunk = zchunk < 4 ? 4 : (zchunk > 32 ? 32 : zchunk);
             const dim3 grid((a.g.N1 + 31) / 32, (a.g.N2 + 7) / 8, (a.g.N3 + zchunk - 1) / zchunk);
             k_adj_cell_march<T><<<grid, dim3(32, 8), 0, st>>>(a, zchunk);
         }

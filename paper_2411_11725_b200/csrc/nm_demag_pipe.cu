@@ -828,6 +828,172 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3
     if (tid == 0) bulk_wait<0>();
 }
 
+// ---- y passes, 128 cells along y ---------------------------------------------------------------------
+// M = 8: a team transforms two lines, here the planes c3_0, c3_0 + 1 of one (k1 tile, component); the
+// warps are the eight columns as before.  A side: two contiguous [128][8] blocks (8 KB each), the
+// second one staged 16 bytes further so that the two lines of a half-warp use different banks.
+// B side: 256 rows of 128 bytes (ky; both planes), one 4-D box.  Lane = (j, line, half) with the line
+// in bit 1, so that a half-warp scatters into both 64-byte halves of the B rows (the slot parity of
+// an output is the same for every lane, which leaves a two-way conflict on that side).
+struct Py8Smem {
+    static constexpr int N = 128, P = 256;
+    static constexpr int LINE_ELEMS = N * TW;                               // 1024 complex, 8 KB
+    static constexpr int A_ELEMS = 2 * LINE_ELEMS + 16;                     // two lines, 16 B skew, padded to 128 B
+    static constexpr int A_BYTES = A_ELEMS * 8;
+    static constexpr int B_ELEMS = P * 2 * TW, B_BYTES = B_ELEMS * 8;       // 32768
+    static constexpr int SCR_BYTES = 16 * Team<8>::SCRATCH * 8;
+    static constexpr int FWD_BYTES = 2 * A_BYTES + B_BYTES + SCR_BYTES + 64;
+    static constexpr int INV_BYTES = B_BYTES + A_BYTES + SCR_BYTES + 64;
+};
+
+template <bool EMB>
+__global__ void __launch_bounds__(kPipeThreads, 2)
+k_py_fwd8(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
+          const float2 *__restrict__ wP, int n2v)
+{
+    typedef float T;
+    typedef float2 V;
+    typedef Py8Smem S;
+    constexpr int M = 8;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    V *s_out = reinterpret_cast<V *>(smem);                                 // [P][2][8]
+    V *s_in = reinterpret_cast<V *>(smem + S::B_BYTES);                     // 2 stages
+    V *s_scr = reinterpret_cast<V *>(smem + S::B_BYTES + 2 * S::A_BYTES);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + S::B_BYTES + 2 * S::A_BYTES + S::SCR_BYTES);
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, l = (lane >> 1) & 1, j = lane >> 2, i = l * M + j;
+    const int G = gridDim.x, H3 = N3 / 2;
+    if (tid == 0) {
+        mbar_init(full, 1);
+        mbar_init(full + 1, 1);
+        mbar_fence_init();
+        tensormap_prefetch(&tmB);
+    }
+    __syncthreads();
+    // tile tl -> (ktl, comp, plane pair q), q fastest: consecutive tiles are consecutive 16 KB of A
+    auto load_a = [&](int tl, int b) {
+        const V *src = A + ((long long)kt0 * 3 * H3 + tl) * 2 * S::LINE_ELEMS;
+        mbar_expect_tx(full + b, 2 * S::LINE_ELEMS * 8);
+        bulk_load(s_in + b * S::A_ELEMS, src, S::LINE_ELEMS * 8, full + b);
+        bulk_load(s_in + b * S::A_ELEMS + S::LINE_ELEMS + 2, src + S::LINE_ELEMS, S::LINE_ELEMS * 8, full + b);
+    };
+    if (tid == 0) {
+        for (int q = 0; q < 2; ++q)
+            if ((int)blockIdx.x + q * G < nTiles) load_a(blockIdx.x + q * G, q);
+    }
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    // element e = j + 8 t of line l: row e, slot w ^ swz(e), swz(j + 8 t) = (j >> 1) ^ 4 (t & 1)
+    const int cinE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1));
+    const int cinO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1) ^ 4);
+    int n = 0;
+    for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
+        const int q = tl % H3, comp = (tl / H3) % 3, ktl = tl / (3 * H3);
+        const int c3_0 = 2 * q;
+        const int b = n & 1;
+        mbar_wait(full + b, (uint32_t)((n >> 1) & 1));
+        const V *in = s_in + b * S::A_ELEMS;
+        V a[16];
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            a[t] = in[((t & 1) ? cinO : cinE) + M * t * TW];
+            if (EMB && j + M * t >= n2v) a[t] = mk<T>((T)0, (T)0);
+        }
+        __syncthreads();                                    // stage b is free again
+        if (tid == 0 && tl + 2 * G < nTiles) load_a(tl + 2 * G, b);
+        if (h) shift32<T, false>(a);
+        fft_fwd<T, M, true>(a, tw, scr, i);
+        if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
+        __syncthreads();
+        // slot s = 8 u + p holds ky = 2 (2 j + u + 16 rev8(p)) + h; element (ky, l): row 2 ky + l,
+        // column w swizzled by the plane pair and by ky: swz(ky) = (2 j + u) & 7
+        const int cs = w ^ swz(c3_0);
+#pragma unroll
+        for (int s = 0; s < 16; ++s) {
+            const int u = s / M, r8 = rev8(s % M);
+            const int ky = 4 * j + 2 * u + 32 * r8 + h;
+            s_out[(2 * ky + l) * TW + (cs ^ ((2 * j + u) & 7))] = a[s];
+        }
+        fence_async_smem();
+        __syncthreads();
+        if (tid == 0) {
+            tensor_store_4d(&tmB, s_out, 0, c3_0, comp, ktl * S::P);
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+__global__ void __launch_bounds__(kPipeThreads, 2)
+k_py_inv8(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3, int nTiles, int kt0,
+          const float2 *__restrict__ wP)
+{
+    typedef float T;
+    typedef float2 V;
+    typedef Py8Smem S;
+    constexpr int M = 8;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    V *s_in = reinterpret_cast<V *>(smem);                                  // [P][2][8]
+    V *s_out = reinterpret_cast<V *>(smem + S::B_BYTES);                    // two lines, skewed
+    V *s_scr = reinterpret_cast<V *>(smem + S::B_BYTES + S::A_BYTES);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + S::B_BYTES + S::A_BYTES + S::SCR_BYTES);
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, l = (lane >> 1) & 1, j = lane >> 2, i = l * M + j;
+    const int G = gridDim.x, H3 = N3 / 2;
+    if (tid == 0) {
+        mbar_init(full, 1);
+        mbar_fence_init();
+        tensormap_prefetch(&tmB);
+    }
+    __syncthreads();
+    auto load_b = [&](int tl) {
+        const int q = tl % H3, comp = (tl / H3) % 3, ktl = tl / (3 * H3);
+        mbar_expect_tx(full, S::B_BYTES);
+        tensor_load_4d(s_in, &tmB, 0, 2 * q, comp, ktl * S::P, full);
+    };
+    if (tid == 0 && (int)blockIdx.x < nTiles) load_b(blockIdx.x);
+    V tw[16];
+    load_twiddles_h<T, M>(tw, wP, j, h);
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    const int coutE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1));
+    const int coutO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1) ^ 4);
+    int n = 0;
+    for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
+        const int c3_0 = 2 * (tl % H3);
+        mbar_wait(full, (uint32_t)(n & 1));
+        const int cs = w ^ swz(c3_0);
+        V a[16];
+#pragma unroll
+        for (int s = 0; s < 16; ++s) {
+            const int u = s / M, r8 = rev8(s % M);
+            const int ky = 4 * j + 2 * u + 32 * r8 + h;
+            a[s] = s_in[(2 * ky + l) * TW + (cs ^ ((2 * j + u) & 7))];
+        }
+        __syncthreads();                                    // the stage is free again
+        if (tid == 0 && tl + G < nTiles) load_b(tl + G);
+        fft_inv<T, M, true>(a, tw, scr, i);
+        if (h) shift32<T, true>(a);
+        if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
+        __syncthreads();
+#pragma unroll
+        for (int t = 0; t < 16; ++t) {
+            V v = a[t];
+            v = cadd(v, shfl1(v));
+            if ((t >> 3) == h) s_out[((t & 1) ? coutO : coutE) + M * t * TW] = v;
+        }
+        fence_async_smem();
+        __syncthreads();
+        if (tid == 0) {
+            V *dst = A + ((long long)kt0 * 3 * H3 + tl) * 2 * S::LINE_ELEMS;
+            bulk_store(dst, s_out, S::LINE_ELEMS * 8);
+            bulk_store(dst + S::LINE_ELEMS, s_out + S::LINE_ELEMS + 2, S::LINE_ELEMS * 8);
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
 } // namespace
 
 // ---- host side ----------------------------------------------------------------------------------
@@ -930,7 +1096,9 @@ typedef CUresult (*NmEncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32
 nm_status nm_pipe_setup(nm_mesh *mesh)
 {
     mesh->fast.tmapB_ok = false;
-    if (!mesh->fast.on || mesh->f64 || !mesh->fast.pipe || mesh->fast.M2 != 16) return NM_OK;
+    if (!mesh->fast.on || mesh->f64 || !mesh->fast.pipe) return NM_OK;
+    const bool y8 = mesh->fast.M2 == 8 && mesh->g.N3 % 2 == 0;     // two planes per tile
+    if (mesh->fast.M2 != 16 && !y8) return NM_OK;
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
@@ -941,7 +1109,7 @@ nm_status nm_pipe_setup(nm_mesh *mesh)
     const NmGeom &g = mesh->g;
     const cuuint64_t dims[4] = {16, (cuuint64_t)mesh->fast.F3, 3, (cuuint64_t)mesh->fast.NKT * g.P2};
     const cuuint64_t strides[3] = {64, (cuuint64_t)mesh->fast.F3 * 64, (cuuint64_t)3 * mesh->fast.F3 * 64};
-    const cuuint32_t box[4] = {16, 1, 1, 256};
+    const cuuint32_t box[4] = {16, y8 ? 2u : 1u, 1, 256};       // M2 = 8: both planes of a tile, all 256 ky rows
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = ((NmEncodeTiledFn)fn)((CUtensorMap *)&mesh->fast.tmapB, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, mesh->bufB,
                                        dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -959,6 +1127,26 @@ bool nm_pipe_y_ok(const nm_mesh *mesh) { return mesh->fast.on && mesh->fast.pipe
 nm_status nm_pipe_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st)
 {
     const NmGeom &g = mesh->g;
+    if (mesh->fast.M2 == 8) {
+        const int nTiles = nkt * 3 * (g.N3 / 2);
+        const int grid = nTiles < 2 * mesh->sm_count ? nTiles : 2 * mesh->sm_count;
+        if (!inverse) {
+            NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
+            auto go = [&](auto kern) -> nm_status {
+                NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Py8Smem::FWD_BYTES));
+                kern<<<grid, kPipeThreads, Py8Smem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3, nTiles,
+                                                                      kt0, (const float2 *)mesh->tw_y, g.N2);
+                return NM_OK;
+            };
+            NM_TRY(mesh->fast.embed ? go(k_py_fwd8<true>) : go(k_py_fwd8<false>));
+        } else {
+            NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv8, cudaFuncAttributeMaxDynamicSharedMemorySize, Py8Smem::INV_BYTES));
+            NmLaunchScope sc(mesh, NM_K_Y_INV, st);
+            k_py_inv8<<<grid, kPipeThreads, Py8Smem::INV_BYTES, st>>>(mesh->fast.tmapB, (float2 *)mesh->bufA, g.N3, nTiles, kt0,
+                                                                      (const float2 *)mesh->tw_y);
+        }
+        return NM_OK;
+    }
     const int nTiles = nkt * 3 * g.N3;
     const int grid = nTiles < 2 * mesh->sm_count ? nTiles : 2 * mesh->sm_count;
     if (!inverse) {

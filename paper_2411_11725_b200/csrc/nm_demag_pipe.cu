@@ -446,9 +446,11 @@ template <typename T, int M> struct PxGeom {
     static constexpr int PZ = P + 8;            // pitch of a packed spectrum line
     static constexpr int SCR = team_scratch<T, M>();
     static constexpr size_t FWD_BYTES = ((size_t)LINES * YP + (size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T);
-    // packed lines (the output tile of R x N reals aliases them) + exchange scratch + staged spectrum rows
-    static constexpr size_t INV_BYTES = ((size_t)LINES * PZ + 16 * SCR + (size_t)NKT * R * 8) * 2 * sizeof(T);
-    static_assert((size_t)R * N <= (size_t)LINES * PZ * 2, "output tile must fit the packed-line buffer");
+    // inverse: output tile (R x N reals) + exchange scratch + staged spectrum rows of one component, the
+    // blocks of consecutive k1 tiles 64 bytes apart modulo 128 (the gather of a half-warp spans two)
+    static constexpr int SK = 64 / (2 * (int)sizeof(T));    // 64 bytes of complex elements
+    static constexpr int KP = R * 8 + SK;                   // pitch of a staged k1 tile
+    static constexpr size_t INV_BYTES = (size_t)R * N * sizeof(T) + ((size_t)16 * SCR + (size_t)NKT * KP) * 2 * sizeof(T);
 };
 
 template <typename V> __device__ __forceinline__ void store2(V *dst, V a, V b);
@@ -587,12 +589,11 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
 {
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
-    constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
+    constexpr int N = G::N, P = G::P, LT = G::LT, R = G::R, NKT = G::NKT;
     extern __shared__ __align__(1024) unsigned char smem[];
-    V *s_z = reinterpret_cast<V *>(smem);                   // LINES x PZ; the output tile R x N (reals) aliases it
-    T *s_out = reinterpret_cast<T *>(smem);
-    V *s_scr = s_z + LINES * G::PZ;
-    V *s_raw = s_scr + 16 * G::SCR;                         // NKT x R x 8 staged spectrum rows of one component
+    T *s_out = reinterpret_cast<T *>(smem);                 // output tile R x N (reals)
+    V *s_scr = reinterpret_cast<V *>(smem + (size_t)R * N * sizeof(T));
+    V *s_raw = s_scr + 16 * G::SCR;                         // NKT blocks of R x 8 staged spectrum rows (pitch KP)
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
@@ -606,44 +607,33 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
         for (int e = tid; e < NKT * PIECES; e += kPipeThreads) {
             const int kt = e / PIECES, off = e - kt * PIECES;
             const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + c3) * f2 + r0) * TW) + off * 16;
-            // fp32: the two rows of every second line swap places, so that the 16-byte reads of a
-            // quarter warp below (rows 2 ln of two lines) fall into different halves of the banks
-            const int es = sizeof(V) == 8 ? e ^ (((e >> 3) & 1) << 2) : e;
-            const unsigned dst = smem_u32(reinterpret_cast<char *>(s_raw) + es * 16);
+            const unsigned dst = smem_u32(reinterpret_cast<char *>(s_raw + kt * G::KP) + off * 16);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     stage(0);
+    // Xa, Xb of this thread's line: rows 2 line, 2 line + 1 of every block, column k1 at slot k1 ^ swz(c2)
+    const V *ra = s_raw + (2 * line) * TW;
+    const int sw = swz(r0 + 2 * line);
     for (int comp = 0; comp < 3; ++comp) {
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                                    // staged rows visible; the output tile has been read
-        for (int idx = tid; idx < NKT * LINES * 4; idx += kPipeThreads) {
-            const int q = idx & 3, ln = (idx >> 2) % LINES, kt = idx / (4 * LINES);
-            const int c2 = r0 + 2 * ln;
-            const int p0 = 2 * q;
-            const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
-            const int sw = sizeof(V) == 8 ? (ln & 1) : 0;
-            const V *src = s_raw + (kt * R + 2 * ln) * TW + p0;
-            V u0, u1, v0, v1;                               // Xa[k0], Xa[k1], Xb[k0], Xb[k1]
-            load2(src + sw * TW, u0, u1);
-            load2(src + (1 - sw) * TW, v0, v1);
-            V *zl = s_z + ln * G::PZ;
-            if (k0 <= N) {
-                zl[k0] = mk<T>(u0.x - v0.y, u0.y + v0.x);
-                if (k0 != 0 && k0 != N) zl[P - k0] = mk<T>(u0.x + v0.y, v0.x - u0.y);
-            }
-            if (k1 <= N) {
-                zl[k1] = mk<T>(u1.x - v1.y, u1.y + v1.x);
-                if (k1 != 0 && k1 != N) zl[P - k1] = mk<T>(u1.x + v1.y, v1.x - u1.y);
-            }
-        }
-        __syncthreads();                                    // packed lines complete; the staging buffer is free
-        if (comp < 2) stage(comp + 1);
+        // packed spectrum of the two rows, gathered straight into transform order:
+        //   Z[k] = Xa[k] + i Xb[k] (k <= N),   Z[k] = conj Xa[P-k] + i conj Xb[P-k] (k > N)
         V a[16];
 #pragma unroll
-        for (int s = 0; s < 16; ++s) a[s] = s_z[line * G::PZ + 2 * slot_freq<M>(j, s) + h];
-        __syncthreads();                                    // the lines are in registers: the output tile may overwrite them
+        for (int s = 0; s < 16; ++s) {
+            const int k = 2 * slot_freq<M>(j, s) + h;
+            const bool up = k > N;
+            const int kk = up ? P - k : k;
+            const V *q = ra + (kk >> 3) * G::KP + ((kk & 7) ^ sw);
+            const V u = q[0], v = q[TW];
+            const T sg = up ? (T)-1 : (T)1;
+            a[s] = mk<T>(u.x - sg * v.y, v.x + sg * u.y);
+        }
+        __syncthreads();                                    // the staging buffer is free
+        if (comp < 2) stage(comp + 1);
         fft_inv<T, M, true>(a, tw, scr, i);
         if (h) shift32<T, true>(a);
 #pragma unroll

@@ -636,27 +636,45 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
         if (comp < 2) stage(comp + 1);
         fft_inv<T, M, true>(a, tw, scr, i);
         if (h) shift32<T, true>(a);
+        if (M >= 8) {
+            // straight to Hc: in one store the 16 (M = 16) or 8 lanes of a line cover 64 / 32 contiguous
+            // bytes of a cell row; half h of a thread stores elements j + M (tt + 8 h)
+            const int n1row = EMB ? g.N1 : N;
+            T *rowA = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0 + 2 * line) * n1row;
 #pragma unroll
-        for (int t = 0; t < 16; ++t) {
-            V v = a[t];
-            v = cadd(v, shfl1(v));
-            if ((t >> 3) == h) {
-                s_out[(2 * line) * N + j + M * t] = v.x;
-                s_out[(2 * line + 1) * N + j + M * t] = v.y;
+            for (int tt = 0; tt < 8; ++tt) {
+                const V lo = cadd(a[tt], shfl1(a[tt])), hi = cadd(a[tt + 8], shfl1(a[tt + 8]));
+                const V v = h ? hi : lo;
+                const int e = j + M * (tt + 8 * h);
+                if (!EMB || e < n1row) {
+                    rowA[e] = v.x;
+                    rowA[n1row + e] = v.y;
+                }
             }
-        }
-        __syncthreads();
-        constexpr int VEC = 16 / sizeof(T);
-        if (!EMB) {     // R consecutive rows of Hc are contiguous
-            T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * N;
-            for (int idx = tid; idx < R * N / VEC; idx += kPipeThreads)
-                reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[idx];
-        } else {        // rows of N1 <= N cells (N1 a multiple of 4): the first N1 columns of every tile row
-            const int pr = g.N1 / VEC;
-            T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * g.N1;
-            for (int idx = tid; idx < R * pr; idx += kPipeThreads) {
-                const int row = idx / pr, cv = idx - row * pr;
-                reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[row * (N / VEC) + cv];
+        } else {
+            // short lines: through a row-major staging tile, 16-byte stores
+#pragma unroll
+            for (int t = 0; t < 16; ++t) {
+                V v = a[t];
+                v = cadd(v, shfl1(v));
+                if ((t >> 3) == h) {
+                    s_out[(2 * line) * N + j + M * t] = v.x;
+                    s_out[(2 * line + 1) * N + j + M * t] = v.y;
+                }
+            }
+            __syncthreads();
+            constexpr int VEC = 16 / sizeof(T);
+            if (!EMB) {     // R consecutive rows of Hc are contiguous
+                T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * N;
+                for (int idx = tid; idx < R * N / VEC; idx += kPipeThreads)
+                    reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[idx];
+            } else {        // rows of N1 <= N cells (N1 a multiple of 4): the first N1 columns of every tile row
+                const int pr = g.N1 / VEC;
+                T *dst = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0) * g.N1;
+                for (int idx = tid; idx < R * pr; idx += kPipeThreads) {
+                    const int row = idx / pr, cv = idx - row * pr;
+                    reinterpret_cast<int4 *>(dst)[idx] = reinterpret_cast<const int4 *>(s_out)[row * (N / VEC) + cv];
+                }
             }
         }
     }

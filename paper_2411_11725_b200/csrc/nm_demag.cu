@@ -325,6 +325,10 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
     {
         int bt = Tile<T>::lines_mid;
         while ((size_t)3 * ma.P * bt * sizeof(V) > kSmemCap && bt > 1) bt >>= 1;
+        // single-layer films have C1p / bt CTAs only: narrower tiles (down to two columns) until
+        // there are two CTAs per SM (512 x 512 x 1: 0.105 -> 0.048 ms)
+        if (ma.n_fixed == 1)
+            while (bt > 2 && (g.C1p + bt - 1) / bt < 2 * mesh->sm_count) bt >>= 1;
         const size_t smm = (size_t)3 * ma.P * bt * sizeof(V);
         if (smm > kSmemCap) {
             nm_set_error("padded length %d too long for the middle pass", ma.P);

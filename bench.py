@@ -382,6 +382,19 @@ def run_b200(args):
                 "traffic_source": "profiles/r1e_final.md (ncu --set full, per launch)", "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg[dom], "launches": dom_n,
                 "avg_launch_ms": dom_ms / dom_n, "share_of_step": dom_ms / tot_ms}
+    # The z pass is as close to the FP32 pipe as to HBM: the same launch against the
+    # arithmetic peak.  Lane operations per launch from the committed ncu capture (packed
+    # FADD2/FMUL2/FFMA2 = 64 per warp instruction, scalar = 32; profiles/r1d_packed.md); peak =
+    # 128 FP32 lanes per clock and SM at the maximum SM clock.
+    roofline_alu = None
+    if dom == "mid" and (N, args.dtype) == (256, "f32"):
+        lane_ops = 1.32e10
+        sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+        alu_peak = 128.0 * sm_count * float((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6
+        alu_ach = lane_ops / (dom_ms * 1e-3 / dom_n)
+        roofline_alu = {"bound": "alu", "kernel": dom, "achieved": alu_ach / 1e12, "peak": alu_peak / 1e12,
+                        "unit": "T FP32 lane-op/s", "frac": alu_ach / alu_peak,
+                        "lane_ops_per_launch": lane_ops, "source": "profiles/r1d_packed.md"}
     per_kernel = {k: {"ms_per_launch": prof[k][0] / prof[k][1], "launches": prof[k][1],
                       "share": prof[k][0] / tot_ms,
                       "GBps": (alg[k] / (prof[k][0] * 1e-3 / prof[k][1]) / 1e9) if k in alg else None}
@@ -402,6 +415,7 @@ def run_b200(args):
         "gpu_launches": launches,
         "clocks": clocks,
         "roofline": roofline,
+        "roofline_alu": roofline_alu,
         "roofline_eval": {"what": "one fused nm_llg_rhs: algorithmic bytes of all passes / its time",
                           "bytes": eval_bytes, "ms": 1e3 * t_rhs, "achieved": eval_bytes / t_rhs / 1e9,
                           "frac": eval_bytes / t_rhs / 1e9 / peak, "frac_of_8TBps_nominal":

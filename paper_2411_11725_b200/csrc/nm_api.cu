@@ -161,6 +161,7 @@ size_t carve(nm_mesh *m, char *base)
     m->W = c.take(g.nodes * e);
     m->Uc[0] = c.take(g.cells * e);
     m->Uc[1] = c.take(g.cells * e);
+    m->Zs = (m->desc.terms & NM_TERM_ZEEMAN) ? c.take(vec) : nullptr;
     m->Hc1 = m->Hc2 = nullptr;
     m->Nreal = nullptr;
     m->fast.Tn = m->fast.wPx = nullptr;

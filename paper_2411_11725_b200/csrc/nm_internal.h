@@ -91,6 +91,7 @@ struct nm_mesh {
     void *bufA, *bufB;      // spectrum buffers (complex)
     void *Hc1, *Hc2;        // cell demag fields [3][cells]
     void *Q, *W;            // adjoint scratch: nodal vector, nodal scalar
+    void *Zs;               // weak-form nodal Zeeman field of the current stage (nodal vector), or null
     void *K[7];             // RK stage derivatives (nodal vectors)
     void *Y[2];             // RK stage states
     void *Uc[2];            // cell scalars (adjoint RK)

@@ -254,6 +254,67 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
 }
 
 
+// a8 with nodal external fields, separately from the other terms (they are linear in H_ext and do not
+// involve m): Zs_n = (mu0 / L_n) sum_{c in n} Ms_c sum_{i'} M_{i,i'} H^ext_{c+i'}  (Eq. 21, reading
+// C3(ii)), H^ext = h_static + amp h_pulse; 0 where (S Ms)_n = 0.  Lets meshes with uniform A and Ku keep
+// the separable node kernels when the Zeeman field is a nodal array (config 3's stripe pulse).
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a, T *__restrict__ Zs)
+{
+    const NmGeom &g = a.g;
+    const int pl = g.n1 * g.n2;
+    const int p = blockIdx.x * kBlock + threadIdx.x;
+    const int i3 = blockIdx.y;
+    if (p >= pl) return;
+    const int i2 = p / g.n1, i1 = p - i2 * g.n1;
+    const long long nn = g.nodes;
+    const long long n = (long long)i3 * pl + p;
+    const int ox[3] = {i1 > 0 ? -1 : 0, 0, i1 < g.N1 ? 1 : 0};
+    const int oy[3] = {i2 > 0 ? -g.n1 : 0, 0, i2 < g.N2 ? g.n1 : 0};
+    const int oz[3] = {i3 > 0 ? -pl : 0, 0, i3 < g.N3 ? pl : 0};
+    const bool vx[2] = {i1 > 0, i1 < g.N1}, vy[2] = {i2 > 0, i2 < g.N2}, vz[2] = {i3 > 0, i3 < g.N3};
+    const int cx[2] = {i1 > 0 ? i1 - 1 : 0, i1 < g.N1 ? i1 : g.N1 - 1};
+    const int cy[2] = {i2 > 0 ? i2 - 1 : 0, i2 < g.N2 ? i2 : g.N2 - 1};
+    const int cz[2] = {i3 > 0 ? i3 - 1 : 0, i3 < g.N3 ? i3 : g.N3 - 1};
+    T cM[8], sms = 0;
+#pragma unroll
+    for (int ci = 0; ci < 8; ++ci) {
+        const int bx = ci & 1, by = (ci >> 1) & 1, bz = ci >> 2;
+        const long long c = ((long long)cz[bz] * g.N2 + cy[by]) * g.N1 + cx[bx];
+        cM[ci] = (vx[bx] && vy[by] && vz[bz]) ? a.Ms[c] : (T)0;
+        sms += cM[ci];
+    }
+    T ze[3] = {0, 0, 0};
+#pragma unroll
+    for (int dz = -1; dz <= 1; ++dz)
+#pragma unroll
+        for (int dy = -1; dy <= 1; ++dy)
+#pragma unroll
+            for (int dx = -1; dx <= 1; ++dx) {
+                const int e = (dx != 0) | ((dy != 0) << 1) | ((dz != 0) << 2);
+                T sM = 0;
+#pragma unroll
+                for (int ci = 0; ci < 8; ++ci) {
+                    const int bx = ci & 1, by = (ci >> 1) & 1, bz = ci >> 2;
+                    const bool in = (dx == 0 || bx == (dx + 1) / 2) && (dy == 0 || by == (dy + 1) / 2) &&
+                                    (dz == 0 || bz == (dz + 1) / 2);
+                    if (in) sM += cM[ci];
+                }
+                const long long q = n + ox[dx + 1] + oy[dy + 1] + oz[dz + 1];
+                const T w = a.wM[e] * sM;
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    T hv = 0;
+                    if (a.h_static) hv += a.h_static[j * nn + q];
+                    if (a.h_pulse) hv += a.amp * a.h_pulse[j * nn + q];
+                    ze[j] += w * hv;
+                }
+            }
+    const T sc = sms > 0 ? a.mu0 / (a.mu0V8 * sms) : (T)0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) Zs[j * nn + n] = sc * ze[j];
+}
+
 // -------------------------------------------------------------------------------------------------
 // Separable node kernel for uniform A and Ku (scalars at nm_mesh_create), any Ms.
 //
@@ -415,6 +476,7 @@ __global__ void __launch_bounds__(SX * SY) k_node_sep(const NmLocalArgs<T> a, in
                                 a.idx2[2] * (gL * (W0[j] - Wm[j]) + gR * (W0[j] - Wp[j]));
                     T hv = (a.cku * an * a.kax[j] - a.cex * E) * inv + (T0[j] + Tn[j]) * dsc;
                     if (a.terms & NM_TERM_ZEEMAN) hv += a.hu[j];
+                    if (a.hadd) hv += a.hadd[j * nn + n];
                     H[j] = hv;
                 }
             }
@@ -639,6 +701,20 @@ inline dim3 sep_grid(const NmGeom &g, int *zchunk)
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
 {
     const bool nodal_zee = (a.terms & NM_TERM_ZEEMAN) && (a.h_static || a.h_pulse);
+    const bool fwd_mode = a.mode == NM_MODE_H || a.mode == NM_MODE_RHS || a.mode == NM_MODE_RK;
+    if (a.sep && nodal_zee && fwd_mode && mesh->Zs) {
+        // nodal Zeeman arrays with uniform A and Ku: smooth the field once, then the separable kernels
+        {
+            NmLaunchScope sc(mesh, NM_K_NODE, st);
+            const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
+            k_zeeman_smooth<T><<<grid, kBlock, 0, st>>>(a, (T *)mesh->Zs);
+        }
+        NM_CUDA_TRY(cudaGetLastError());
+        NmLocalArgs<T> b = a;
+        b.h_static = b.h_pulse = nullptr;
+        b.hadd = (const T *)mesh->Zs;
+        return nm_launch_node<T>(mesh, b, st);
+    }
     if (a.sep == 1 && !nodal_zee && nm_node_col_ok<T>(mesh, a)) return nm_launch_node_col<T>(mesh, a, st);
     if (a.sep && !nodal_zee) {
         int zchunk;

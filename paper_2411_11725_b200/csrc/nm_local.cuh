@@ -47,6 +47,7 @@ template <typename T> struct NmLocalArgs {
     const T *h_static, *h_pulse;
     T amp;
     T hu[3];
+    const T *hadd;      // nodal field added to H as it stands (the smoothed nodal Zeeman field, k_zeeman_smooth), or null
     // LLG
     T gp, agp;          // gamma' = gamma/(1+alpha^2), alpha gamma'
     int mode;

@@ -23,10 +23,10 @@ template <typename T> struct Tile {
 };
 
 constexpr int kThreads = 256;
-constexpr int kRowsX = 4;   // cell rows (c2) per CTA in the x passes
+constexpr int kRowsX = 4;   // cell rows (c2) per CTA in the x passes (2 where that leaves SMs without a CTA)
 
 // ---------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, int RX>
 __global__ void __launch_bounds__(kThreads)
 k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *__restrict__ A,
         NmGeom g, NmFftPlan plan, const typename Cx<T>::V *__restrict__ tw,
@@ -38,14 +38,14 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
     V *s = reinterpret_cast<V *>(smem_raw);
     const int Lx = g.Lx;
     const int c3 = blockIdx.y;
-    const int row0 = blockIdx.x * kRowsX;
-    const int n_lines = 3 * kRowsX;
+    const int row0 = blockIdx.x * RX;
+    const int n_lines = 3 * RX;
     const long long plane = (long long)g.n1 * g.n2;
     // 1. cell averages, packed two reals per complex slot
     for (int idx = threadIdx.x; idx < n_lines * Lx; idx += blockDim.x) {
         const int n = idx % Lx;
         const int line = idx / Lx;
-        const int r = line % kRowsX, comp = line / kRowsX;
+        const int r = line % RX, comp = line / RX;
         const int c2 = row0 + r;
         T v0 = 0, v1 = 0;
         if (c2 < g.N2) {
@@ -75,7 +75,7 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
     for (int idx = threadIdx.x; idx < n_lines * g.C1; idx += blockDim.x) {
         const int k = idx % g.C1;
         const int line = idx / g.C1;
-        const int r = line % kRowsX, comp = line / kRowsX;
+        const int r = line % RX, comp = line / RX;
         const int c2 = row0 + r;
         if (c2 >= g.N2) continue;
         const V *ln = s + line * Lx;
@@ -90,7 +90,7 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
     }
 }
 
-template <typename T>
+template <typename T, int RX>
 __global__ void __launch_bounds__(kThreads)
 k_x_inv(const typename Cx<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, NmFftPlan plan,
         const typename Cx<T>::V *__restrict__ tw, const typename Cx<T>::V *__restrict__ tw2,
@@ -102,13 +102,13 @@ k_x_inv(const typename Cx<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, N
     V *s = reinterpret_cast<V *>(smem_raw);
     const int Lx = g.Lx;
     const int c3 = blockIdx.y;
-    const int row0 = blockIdx.x * kRowsX;
-    const int n_lines = 3 * kRowsX;
+    const int row0 = blockIdx.x * RX;
+    const int n_lines = 3 * RX;
     // 1. Z'[k] = (X[k] + conj X[Lx-k]) + i conj(W^k) (X[k] - conj X[Lx-k]), stored at its position
     for (int idx = threadIdx.x; idx < n_lines * Lx; idx += blockDim.x) {
         const int k = idx % Lx;
         const int line = idx / Lx;
-        const int r = line % kRowsX, comp = line / kRowsX;
+        const int r = line % RX, comp = line / RX;
         const int c2 = row0 + r;
         V z = C::make((T)0, (T)0);
         if (c2 < g.N2) {
@@ -132,7 +132,7 @@ k_x_inv(const typename Cx<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, N
     for (int idx = threadIdx.x; idx < n_lines * g.N1; idx += blockDim.x) {
         const int c1 = idx % g.N1;
         const int line = idx / g.N1;
-        const int r = line % kRowsX, comp = line / kRowsX;
+        const int r = line % RX, comp = line / RX;
         const int c2 = row0 + r;
         if (c2 >= g.N2) continue;
         const V z = s[line * Lx + (c1 >> 1)];
@@ -275,17 +275,26 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
     typedef typename Cx<T>::V V;
     const NmGeom &g = mesh->g;
     V *A = (V *)mesh->bufA, *B = (V *)mesh->bufB;
-    const dim3 gx((g.N2 + kRowsX - 1) / kRowsX, g.N3);
-    const size_t smx = (size_t)3 * kRowsX * g.Lx * sizeof(V);
+    // x passes: 4 cell rows per CTA, or 2 where 4 would leave fewer than two CTAs per SM (films)
+    const bool rx2 = (long long)((g.N2 + kRowsX - 1) / kRowsX) * g.N3 < 2LL * mesh->sm_count;
+    const int RXv = rx2 ? 2 : kRowsX;
+    const dim3 gx((g.N2 + RXv - 1) / RXv, g.N3);
+    const size_t smx = (size_t)3 * RXv * g.Lx * sizeof(V);
     if (smx > kSmemCap) {
         nm_set_error("N1 = %d too long for the x pass", g.N1);
         return NM_EUNSUPPORTED;
     }
-    NM_TRY(set_smem(k_x_fwd<T>, smx));
     {
         NmLaunchScope sc(mesh, NM_K_X_FWD, st);
-        k_x_fwd<T><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
-                                             (const V *)mesh->tw_x, (const V *)mesh->tw_x2, mesh->pos_x);
+        if (rx2) {
+            NM_TRY(set_smem(k_x_fwd<T, 2>, smx));
+            k_x_fwd<T, 2><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
+                                                    (const V *)mesh->tw_x, (const V *)mesh->tw_x2, mesh->pos_x);
+        } else {
+            NM_TRY(set_smem(k_x_fwd<T, kRowsX>, smx));
+            k_x_fwd<T, kRowsX><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
+                                                         (const V *)mesh->tw_x, (const V *)mesh->tw_x2, mesh->pos_x);
+        }
     }
 
 
@@ -354,11 +363,17 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
         }
 
     }
-    NM_TRY(set_smem(k_x_inv<T>, smx));
     {
         NmLaunchScope sc(mesh, NM_K_X_INV, st);
-        k_x_inv<T><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
-                                             (const V *)mesh->tw_x2, mesh->pos_x);
+        if (rx2) {
+            NM_TRY(set_smem(k_x_inv<T, 2>, smx));
+            k_x_inv<T, 2><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
+                                                    (const V *)mesh->tw_x2, mesh->pos_x);
+        } else {
+            NM_TRY(set_smem(k_x_inv<T, kRowsX>, smx));
+            k_x_inv<T, kRowsX><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
+                                                         (const V *)mesh->tw_x2, mesh->pos_x);
+        }
     }
 
     NM_CUDA_TRY(cudaGetLastError());

@@ -251,7 +251,8 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
     const long long plane = (long long)g.n1 * g.n2;
-    for (int comp = 0; comp < 3; ++comp) {
+    // small grids: one component per CTA (gridDim.z = 3)
+    for (int comp = gridDim.z == 3 ? (int)blockIdx.z : 0; comp < (gridDim.z == 3 ? (int)blockIdx.z + 1 : 3); ++comp) {
         // a1: M_c = Ms_c (1/8) sum of the 8 vertices
         const T *base = fld + (long long)comp * g.nodes + (long long)c3 * plane;
         for (int idx = threadIdx.x; idx < R * N; idx += blockDim.x) {
@@ -317,7 +318,8 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
-    for (int comp = 0; comp < 3; ++comp) {
+    // small grids: one component per CTA (gridDim.z = 3)
+    for (int comp = gridDim.z == 3 ? (int)blockIdx.z : 0; comp < (gridDim.z == 3 ? (int)blockIdx.z + 1 : 3); ++comp) {
         for (int idx = threadIdx.x; idx < NKT * R * TW; idx += blockDim.x) {
             const int kt = idx / (R * TW), rem = idx % (R * TW);
             const int r = rem / TW, slot = rem % TW;
@@ -377,7 +379,8 @@ nm_status launch_x(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_
     const NmFast &f = mesh->fast;
     constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
     const int W = f.Wx, R = 2 * LT * W;
-    const dim3 grid(g.N2 / R, g.N3);
+    const bool split = (long long)(g.N2 / R) * g.N3 < 2LL * mesh->sm_count;
+    const dim3 grid(g.N2 / R, g.N3, split ? 3 : 1);
     if (!inverse) {
         const size_t sm = (size_t)W * LT * P * sizeof(V) + scratch_bytes<T>(W) + (size_t)R * (N + 1) * sizeof(T);
         NM_TRY(set_smem_f(k_fx_fwd<T, M>, sm));

@@ -523,7 +523,9 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
     }
     const long long plane = (long long)g.n1 * g.n2;
     const int rg = tid / N, col = tid % N;                  // phase 1: row group (16 cell rows) and node column
-    for (int comp = 0; comp < 3; ++comp) {
+    // small grids: the three components in three CTAs (gridDim.z = 3)
+    const int comp_lo = gridDim.z == 3 ? blockIdx.z : 0, comp_hi = gridDim.z == 3 ? comp_lo + 1 : 3;
+    for (int comp = comp_lo; comp < comp_hi; ++comp) {
         const T *base = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + rg * 16) * g.n1;
         {
             T z[17];
@@ -612,11 +614,12 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    stage(0);
+    const int comp_lo = gridDim.z == 3 ? blockIdx.z : 0, comp_hi = gridDim.z == 3 ? comp_lo + 1 : 3;
+    stage(comp_lo);
     // Xa, Xb of this thread's line: rows 2 line, 2 line + 1 of every block, column k1 at slot k1 ^ swz(c2)
     const V *ra = s_raw + (2 * line) * TW;
     const int sw = swz(r0 + 2 * line);
-    for (int comp = 0; comp < 3; ++comp) {
+    for (int comp = comp_lo; comp < comp_hi; ++comp) {
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                                    // staged rows visible; the output tile has been read
         // packed spectrum of the two rows, gathered straight into transform order:
@@ -633,7 +636,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             a[s] = mk<T>(u.x - sg * v.y, v.x + sg * u.y);
         }
         __syncthreads();                                    // the staging buffer is free
-        if (comp < 2) stage(comp + 1);
+        if (comp + 1 < comp_hi) stage(comp + 1);
         fft_inv<T, M, true>(a, tw, scr, i);
         if (h) shift32<T, true>(a);
         if (M >= 8) {
@@ -1045,7 +1048,9 @@ template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, co
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
     const NmGeom &g = mesh->g;
-    const dim3 grid(g.N2 / G::R, g.N3);
+    // fewer than two CTAs per SM: one component per CTA
+    const bool split = (long long)(g.N2 / G::R) * g.N3 < 2LL * mesh->sm_count;
+    const dim3 grid(g.N2 / G::R, g.N3, split ? 3 : 1);
     const int f2 = mesh->fast.F2;
     if (!inverse) {
         NmLaunchScope sc(mesh, NM_K_X_FWD, st);

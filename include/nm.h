@@ -124,7 +124,14 @@ nm_status nm_llg_rhs(nm_mesh *mesh, double t, const void *m, const nm_zeeman *ze
  *              otherwise m_inout is left unchanged.  If err_norm_host != NULL the stream is
  *              synchronised once and *err_norm_host = err (the caller adapts dt).
  *   renormalise != 0: m_n <- m_n/|m_n| once per committed step (reading C6); stages see the
- *              un-normalised intermediate states. */
+ *              un-normalised intermediate states.
+ * Launch replay: on meshes of at most 2^21 cells (launch-latency-bound; NM_GRAPH=0/1 in the
+ * environment at nm_mesh_create forces off/on), when a step arrives with the arguments of the
+ * step before it (scheme, dt, m_inout, renormalise, rtol, atol, the arrays and h_uniform of
+ * `zeeman`) and zeeman->amp is NULL, its kernel launches are captured once into a CUDA graph
+ * and replayed with one launch on `stream`; same kernels, same arguments, identical results.
+ * The arrays `zeeman` points to are then read at replay time, as the launches would.  The same
+ * holds for nm_adjoint_rk4_step (key: dt, m_inout, a_inout, u_inout, renormalise, zeeman). */
 nm_status nm_rk_step(nm_mesh *mesh, nm_scheme scheme, double t, double dt, void *m_inout,
                      const nm_zeeman *zeeman, int renormalise, double rtol, double atol,
                      double *err_norm_host, void *stream);

@@ -213,6 +213,15 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
     m->prof_on = false;
     m->prof_n = 0;
     m->prof_ev_made = 0;
+    {
+        // whole steps of small meshes are launch-latency-bound: replay them as graphs (NM_GRAPH=0 / 1
+        // forces the choice)
+        const char *ge = getenv("NM_GRAPH");
+        m->graph_on = ge ? atoi(ge) != 0 : m->g.cells <= (1LL << 21);
+        m->cap_stream = nullptr;
+        m->graph_epoch = 0;
+        memset(m->step_graph, 0, sizeof(m->step_graph));
+    }
     nm_fast_plan(d, m->g, &m->fast);
     {
         const char *env = getenv("NM_DEMAG_PATH");      // "generic" forces the general-size kernels
@@ -337,6 +346,7 @@ extern "C" nm_status nm_mesh_set_Ms(nm_mesh *mesh, const void *Ms, void *stream)
     NM_CUDA_TRY(cudaMemcpyAsync(mesh->Ms, Ms, mesh->g.cells * mesh->esz, cudaMemcpyDeviceToDevice, st));
     mesh->hc1_valid = false;
     mesh->uni_Ms = false;
+    mesh->graph_epoch++;
     return nm_compute_sMs(mesh, st);
 }
 
@@ -415,6 +425,9 @@ extern "C" nm_status nm_mesh_destroy(nm_mesh *mesh)
             cudaEventDestroy(mesh->prof_ev[i][0]);
             cudaEventDestroy(mesh->prof_ev[i][1]);
         }
+        for (int i = 0; i < NM_GRAPH_SLOTS; ++i)
+            if (mesh->step_graph[i].exec) cudaGraphExecDestroy(mesh->step_graph[i].exec);
+        if (mesh->cap_stream) cudaStreamDestroy(mesh->cap_stream);
     }
     delete mesh;
     return NM_OK;
@@ -621,7 +634,7 @@ const double DP_B4[7] = {5179.0 / 57600, 0.0, 7571.0 / 16695, 393.0 / 640, -9209
 
 template <typename T>
 nm_status dopri5_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z, int renorm,
-                      double rtol, double atol, double *err_host, cudaStream_t st)
+                      double rtol, double atol, cudaStream_t st)
 {
     T *Yb[2] = {(T *)m->Y[0], (T *)m->Y[1]};
     const T *fld = y;
@@ -651,13 +664,7 @@ nm_status dopri5_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z,
     }
     NM_TRY(nm_launch_err_final(m, m->last_partials, 3.0 * (double)m->g.nodes, st));
     // y5 lives in Yb[5 & 1]
-    NM_TRY(nm_launch_commit<T>(m, y, Yb[1], m->partials + m->last_partials, renorm, st));
-    if (err_host) {
-        NM_CUDA_TRY(cudaMemcpyAsync(err_host, m->partials + m->last_partials, sizeof(double),
-                                    cudaMemcpyDeviceToHost, st));
-        NM_CUDA_TRY(cudaStreamSynchronize(st));
-    }
-    return NM_OK;
+    return nm_launch_commit<T>(m, y, Yb[1], m->partials + m->last_partials, renorm, st);
 }
 
 // (f, -(df/dm)^T a, -(df/dMs)^T a): reading C7, two demag convolutions and two node passes.
@@ -746,6 +753,62 @@ nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, const
     return NM_OK;
 }
 
+// Whole-step graph replay.  A step whose launch sequence is fixed by `key` (no host callback, no
+// per-launch timing) runs eagerly the first time; when the same key arrives again the sequence is
+// captured once on the mesh's capture stream (capture executes nothing) and from then on replayed
+// with one cudaGraphLaunch on the caller's stream.  `issue(stream)` enqueues the step.
+template <typename F>
+nm_status run_step(nm_mesh *m, int slot, const nm_zeeman *z, NmStepKey key, cudaStream_t st, F issue)
+{
+    if (!m->graph_on || m->prof_on || (z && z->amp)) return issue(st);
+    key.kind = slot;
+    key.epoch = m->graph_epoch;
+    key.has_z = z != nullptr;
+    if (z) {
+        key.hs = z->h_static;
+        key.hp = z->h_pulse;
+        for (int j = 0; j < 3; ++j) key.hu[j] = z->h_uniform[j];
+    }
+    NmStepGraph &sg = m->step_graph[slot];
+    if (sg.seen && memcmp(&sg.key, &key, sizeof(key)) == 0) {
+        if (!sg.exec) {
+            if (!m->cap_stream) NM_CUDA_TRY(cudaStreamCreateWithFlags(&m->cap_stream, cudaStreamNonBlocking));
+            NM_CUDA_TRY(cudaStreamBeginCapture(m->cap_stream, cudaStreamCaptureModeRelaxed));
+            const long long before = m->launches;
+            const nm_status s = issue(m->cap_stream);
+            cudaGraph_t graph = nullptr;
+            const cudaError_t e = cudaStreamEndCapture(m->cap_stream, &graph);
+            sg.launches = m->launches - before;
+            m->launches = before;
+            if (s != NM_OK || e != cudaSuccess || !graph) {
+                if (graph) cudaGraphDestroy(graph);
+                cudaGetLastError();
+                if (s != NM_OK) return s;
+                m->graph_on = false;            // capture not possible here: stay on plain launches
+                return issue(st);
+            }
+            const cudaError_t ei = cudaGraphInstantiate(&sg.exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ei != cudaSuccess) {
+                sg.exec = nullptr;
+                cudaGetLastError();
+                m->graph_on = false;
+                return issue(st);
+            }
+        }
+        NM_CUDA_TRY(cudaGraphLaunch(sg.exec, st));
+        m->launches += sg.launches;
+        return NM_OK;
+    }
+    if (sg.exec) {
+        cudaGraphExecDestroy(sg.exec);
+        sg.exec = nullptr;
+    }
+    sg.key = key;
+    sg.seen = true;
+    return issue(st);
+}
+
 nm_status check_call(nm_mesh *mesh, const void *p0, const void *p1)
 {
     if (!mesh || !p0 || !p1) { nm_set_error("NULL argument"); return NM_EINVAL; }
@@ -779,20 +842,38 @@ extern "C" nm_status nm_rk_step(nm_mesh *mesh, nm_scheme scheme, double t, doubl
 {
     NM_TRY(check_call(mesh, m_inout, m_inout));
     cudaStream_t st = (cudaStream_t)stream;
+    NmStepKey key;
+    memset(&key, 0, sizeof(key));
+    key.dt = dt;
+    key.renorm = renormalise;
+    key.p[0] = m_inout;
     if (scheme == NM_RK4) {
         if (err_norm_host) *err_norm_host = 0.0;
-        return mesh->f64 ? rk4_step<double>(mesh, t, dt, (double *)m_inout, zeeman, renormalise, st)
-                         : rk4_step<float>(mesh, t, dt, (float *)m_inout, zeeman, renormalise, st);
+        return run_step(mesh, NM_GRAPH_RK4, zeeman, key, st, [&](cudaStream_t s) {
+            return mesh->f64 ? rk4_step<double>(mesh, t, dt, (double *)m_inout, zeeman, renormalise, s)
+                             : rk4_step<float>(mesh, t, dt, (float *)m_inout, zeeman, renormalise, s);
+        });
     }
     if (scheme == NM_DOPRI5) {
         if (!(rtol >= 0) || !(atol >= 0) || (rtol == 0 && atol == 0)) {
             nm_set_error("rtol / atol must be non-negative and not both zero");
             return NM_EINVAL;
         }
-        return mesh->f64 ? dopri5_step<double>(mesh, t, dt, (double *)m_inout, zeeman, renormalise, rtol,
-                                               atol, err_norm_host, st)
-                         : dopri5_step<float>(mesh, t, dt, (float *)m_inout, zeeman, renormalise, rtol,
-                                              atol, err_norm_host, st);
+        key.rtol = rtol;
+        key.atol = atol;
+        // the launches replay; the read-back of the error norm stays outside the graph
+        NM_TRY(run_step(mesh, NM_GRAPH_DOPRI5, zeeman, key, st, [&](cudaStream_t s) {
+            return mesh->f64 ? dopri5_step<double>(mesh, t, dt, (double *)m_inout, zeeman, renormalise, rtol,
+                                                   atol, s)
+                             : dopri5_step<float>(mesh, t, dt, (float *)m_inout, zeeman, renormalise, rtol,
+                                                  atol, s);
+        }));
+        if (err_norm_host) {
+            NM_CUDA_TRY(cudaMemcpyAsync(err_norm_host, mesh->partials + mesh->last_partials, sizeof(double),
+                                        cudaMemcpyDeviceToHost, st));
+            NM_CUDA_TRY(cudaStreamSynchronize(st));
+        }
+        return NM_OK;
     }
     nm_set_error("unknown scheme %d", (int)scheme);
     return NM_EINVAL;
@@ -817,8 +898,17 @@ extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, voi
     NM_TRY(check_call(mesh, m_inout, a_inout));
     if (!u_inout) { nm_set_error("u_inout is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
-    return mesh->f64 ? adjoint_rk4<double>(mesh, t, dt, (double *)m_inout, (double *)a_inout,
-                                           (double *)u_inout, zeeman, renormalise, st)
-                     : adjoint_rk4<float>(mesh, t, dt, (float *)m_inout, (float *)a_inout,
-                                          (float *)u_inout, zeeman, renormalise, st);
+    NmStepKey key;
+    memset(&key, 0, sizeof(key));
+    key.dt = dt;
+    key.renorm = renormalise;
+    key.p[0] = m_inout;
+    key.p[1] = a_inout;
+    key.p[2] = u_inout;
+    return run_step(mesh, NM_GRAPH_ADJ_RK4, zeeman, key, st, [&](cudaStream_t s) {
+        return mesh->f64 ? adjoint_rk4<double>(mesh, t, dt, (double *)m_inout, (double *)a_inout,
+                                               (double *)u_inout, zeeman, renormalise, s)
+                         : adjoint_rk4<float>(mesh, t, dt, (float *)m_inout, (float *)a_inout,
+                                              (float *)u_inout, zeeman, renormalise, s);
+    });
 }

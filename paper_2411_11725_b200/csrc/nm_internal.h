@@ -69,6 +69,22 @@ struct NmFast {
     void *wPx;         // exp(-2 pi i q / P1), q < P1
 };
 
+// One cached time step: the arguments that fix its launch sequence, and the instantiated graph
+// (null until the same arguments arrive a second time in a row).
+struct NmStepKey {
+    int kind, renorm, has_z, pad;   // no implicit padding: keys are compared with memcmp
+    double dt, rtol, atol, hu[3];
+    const void *p[3], *hs, *hp;
+    unsigned long long epoch;
+};
+struct NmStepGraph {
+    bool seen;
+    NmStepKey key;
+    cudaGraphExec_t exec;
+    long long launches;                // kernels in the graph
+};
+enum { NM_GRAPH_RK4 = 0, NM_GRAPH_DOPRI5, NM_GRAPH_ADJ_RK4, NM_GRAPH_SLOTS };
+
 struct nm_mesh {
     nm_mesh_desc desc;
     NmGeom g;
@@ -107,6 +123,11 @@ struct nm_mesh {
     int prof_cls[NM_PROF_MAX];
     cudaEvent_t prof_ev[NM_PROF_MAX][2];
     int prof_ev_made;       // events created so far (created lazily, destroyed with the mesh)
+    // Replay of whole time steps as CUDA graphs (launch-latency-bound meshes; nm_api.cu)
+    bool graph_on;
+    cudaStream_t cap_stream;           // capture vehicle, created lazily (nothing ever runs on it)
+    unsigned long long graph_epoch;    // bumped by whatever changes the launch sequence (nm_mesh_set_Ms)
+    NmStepGraph step_graph[NM_GRAPH_SLOTS];
 };
 
 // Brackets one kernel launch with an event pair when profiling is on, and counts it.

@@ -733,21 +733,22 @@ nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, const
     for (int s = 0; s < 4; ++s) {
         NM_TRY(adjoint_eval<T>(m, ts[s], sm, sa, z, F, DA, DU, st));
         const T ws = (T)w[s];
-        const T *srcF[1] = {F}, *srcA[1] = {DA}, *srcU[1] = {DU};
         if (s < 3) {
-            // accumulators (first stage starts them from the state)
-            NM_TRY(nm_lincomb<T>(m, AM, s == 0 ? mm : AM, 1, srcF, &ws, nv, 0, st));
-            NM_TRY(nm_lincomb<T>(m, AA, s == 0 ? av : AA, 1, srcA, &ws, nv, 0, st));
-            NM_TRY(nm_lincomb<T>(m, AU, s == 0 ? u : AU, 1, srcU, &ws, nc, 0, st));
+            // accumulators (the first stage starts them from the state) and the next stage state
             const T c = (T)cn[s];
-            NM_TRY(nm_lincomb<T>(m, Ym, mm, 1, srcF, &c, nv, 0, st));
-            NM_TRY(nm_lincomb<T>(m, Ya, av, 1, srcA, &c, nv, 0, st));
+            const NmLinOp<T> ops[5] = {{AM, s == 0 ? mm : AM, F, ws, nv, 0},
+                                       {AA, s == 0 ? av : AA, DA, ws, nv, 0},
+                                       {AU, s == 0 ? u : AU, DU, ws, nc, 0},
+                                       {Ym, mm, F, c, nv, 0},
+                                       {Ya, av, DA, c, nv, 0}};
+            NM_TRY(nm_lincomb_batch<T>(m, ops, 5, st));
             sm = Ym;
             sa = Ya;
         } else {
-            NM_TRY(nm_lincomb<T>(m, mm, AM, 1, srcF, &ws, nv, renorm ? nn : 0, st));
-            NM_TRY(nm_lincomb<T>(m, av, AA, 1, srcA, &ws, nv, 0, st));
-            NM_TRY(nm_lincomb<T>(m, u, AU, 1, srcU, &ws, nc, 0, st));
+            const NmLinOp<T> ops[3] = {{mm, AM, F, ws, nv, renorm ? nn : 0},
+                                       {av, AA, DA, ws, nv, 0},
+                                       {u, AU, DU, ws, nc, 0}};
+            NM_TRY(nm_lincomb_batch<T>(m, ops, 3, st));
         }
     }
     return NM_OK;

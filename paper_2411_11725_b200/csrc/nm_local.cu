@@ -680,6 +680,34 @@ template <typename T> __global__ void k_lincomb(const LinArgs<T> a)
     }
 }
 
+// Up to NM_LIN_OPS independent out = base + coef src updates in one launch (blockIdx.y = update):
+// the stage updates of the adjoint Runge-Kutta step.  Same arithmetic as k_lincomb with one source.
+template <typename T> struct LinBatch {
+    LinArgs<T> op[NM_LIN_OPS];
+};
+
+template <typename T> __global__ void k_lincomb_batch(const LinBatch<T> b)
+{
+    const LinArgs<T> &a = b.op[blockIdx.y];
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a.vec_n > 0) {
+        if (i >= a.vec_n) return;
+        T y[3];
+        for (int j = 0; j < 3; ++j) {
+            T v = a.base[j * a.vec_n + i];
+            v += a.coef[0] * a.src[0][j * a.vec_n + i];
+            y[j] = v;
+        }
+        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+        for (int j = 0; j < 3; ++j) a.out[j * a.vec_n + i] = y[j] * inv;
+    } else {
+        if (i >= a.n) return;
+        T v = a.base[i];
+        v += a.coef[0] * a.src[0][i];
+        a.out[i] = v;
+    }
+}
+
 inline unsigned nblk(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 // Grid of k_node_sep: SX x SY patches of node columns, z split into chunks so that about eight
@@ -809,6 +837,29 @@ nm_status nm_lincomb(nm_mesh *mesh, T *out, const T *base, int nsrc, const T *co
     return NM_OK;
 }
 
+template <typename T>
+nm_status nm_lincomb_batch(nm_mesh *mesh, const NmLinOp<T> *ops, int nops, cudaStream_t st)
+{
+    if (nops < 1 || nops > NM_LIN_OPS) { nm_set_error("nm_lincomb_batch: %d updates", nops); return NM_EINVAL; }
+    LinBatch<T> b;
+    memset(&b, 0, sizeof(b));
+    long long longest = 0;
+    for (int o = 0; o < nops; ++o) {
+        LinArgs<T> &a = b.op[o];
+        a.out = ops[o].out; a.base = ops[o].base; a.nsrc = 1; a.n = ops[o].n; a.vec_n = ops[o].vec_n;
+        a.src[0] = ops[o].src;
+        a.coef[0] = ops[o].coef;
+        const long long threads = a.vec_n > 0 ? a.vec_n : a.n;
+        if (threads > longest) longest = threads;
+    }
+    {
+        NmLaunchScope sc(mesh, NM_K_LINCOMB, st);
+        k_lincomb_batch<T><<<dim3(nblk(longest, 256), nops), 256, 0, st>>>(b);
+    }
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
 nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st)
 {
     NmLaunchScope sc(mesh, NM_K_OTHER, st);
@@ -825,6 +876,7 @@ nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st)
     template nm_status nm_launch_commit<T>(nm_mesh *, T *, const T *, const double *, int, cudaStream_t); \
     template nm_status nm_launch_adj_cell<T>(nm_mesh *, const NmAdjCellArgs<T> &, cudaStream_t);        \
     template nm_status nm_lincomb<T>(nm_mesh *, T *, const T *, int, const T *const *, const T *,       \
-                                     long long, long long, cudaStream_t);
+                                     long long, long long, cudaStream_t);                               \
+    template nm_status nm_lincomb_batch<T>(nm_mesh *, const NmLinOp<T> *, int, cudaStream_t);
 NM_INST(float)
 NM_INST(double)

@@ -85,6 +85,18 @@ nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaS
 template <typename T>
 nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st);
 template <typename T> nm_status nm_launch_adj_cell(nm_mesh *mesh, const NmAdjCellArgs<T> &a, cudaStream_t st);
+// several independent updates out = base + coef * src in one launch (vec_n > 0: [3][vec_n] arrays,
+// result normalised per node); no update may read what another one writes
+enum { NM_LIN_OPS = 5 };
+template <typename T> struct NmLinOp {
+    T *out;
+    const T *base, *src;
+    T coef;
+    long long n, vec_n;
+};
+template <typename T>
+nm_status nm_lincomb_batch(nm_mesh *mesh, const NmLinOp<T> *ops, int nops, cudaStream_t st);
+
 template <typename T>
 nm_status nm_lincomb(nm_mesh *mesh, T *out, const T *base, int nsrc, const T *const *src, const T *coef,
                      long long n, long long vec_n, cudaStream_t st);

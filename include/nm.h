@@ -61,7 +61,7 @@ typedef enum { NM_RK4 = 0, NM_DOPRI5 = 1 } nm_scheme;
 /* Statement of the problem: regular grid, nodal m, cell-wise materials. */
 typedef struct {
     int n_cells[3];       /* N1, N2, N3 >= 1.  With NM_TERM_DEMAG every N_d > 1 must be
-                             2^a 3^b (FFT radices 2,3,4,8), else NM_EUNSUPPORTED -- except
+                             2^a 3^b 5^c 7^d (FFT radices 2,3,4,5,7,8), else NM_EUNSUPPORTED -- except
                              meshes the zero-extended fast path serves (2 <= N_d <= 256 that
                              fill half of the (y, z) plane of the next sizes 16 * 2^k and
                              meet its row granularities; see nm_debug_demag_path), any N_d. */

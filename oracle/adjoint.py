@@ -92,12 +92,18 @@ def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
     return m, ckpt
 
 
-def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0):
+def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, a_jumps=None):
     """Integrate Eq. (29) from T = t0 + n_steps dt back to t0 with RK4 steps of -dt.
 
     State (m, a, u); m is renormalised after every step and replaced by the stored forward
     value whenever a checkpoint index is reached (reading C8).  Returns (m0, a0, u0);
     u0 = dJ/dMs per cell (Eq. 30).
+
+    Objectives at several times ("adding appropriate terms depending on m(T_i)"):
+    for L = L_T(m(T)) + sum_i L_i(m(T_i)), T_i = t0 + s_i dt, pass aT = grad L_T and
+    a_jumps = {s_i: grad_m L_i(m(T_i))}; the adjoint variable takes the jump a += a_jumps[s_i]
+    when the backward integration arrives at T_i (the term of L_i enters the adjoint equation as
+    a delta function in time).
     """
     m, a = mT.copy(), aT.copy()
     u = np.zeros(p.n_cells)
@@ -117,4 +123,6 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0):
         u = u + h / 6.0 * (k1[2] + 2 * k2[2] + 2 * k3[2] + k4[2])
         if checkpoints is not None and (s - 1) in checkpoints:
             m = checkpoints[s - 1].copy()
+        if a_jumps is not None and (s - 1) in a_jumps:
+            a = a + a_jumps[s - 1]
     return m, a, u

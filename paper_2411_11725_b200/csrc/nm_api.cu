@@ -28,10 +28,10 @@ extern "C" const char *nm_last_error(void) { return g_err; }
 namespace {
 
 // ---- geometry, FFT plans -----------------------------------------------------------------------
-bool smooth23(int n)
+bool smooth7(int n)          // 2^a 3^b 5^c 7^d: the radices of nm_fft.cuh
 {
-    while (n % 2 == 0) n /= 2;
-    while (n % 3 == 0) n /= 3;
+    for (int r = 2; r <= 7; r += (r == 2 ? 1 : 2))
+        while (n % r == 0) n /= r;
     return n == 1;
 }
 
@@ -40,7 +40,9 @@ void make_plan(int L, NmFftPlan *p)
     p->L = L;
     p->n_stages = 0;
     int n = L;
-    // factors of three first (largest blocks), then 8s, then what is left of the power of two
+    // odd factors first (largest blocks), then 8s, then what is left of the power of two
+    while (n % 7 == 0) { p->radix[p->n_stages++] = 7; n /= 7; }
+    while (n % 5 == 0) { p->radix[p->n_stages++] = 5; n /= 5; }
     while (n % 3 == 0) { p->radix[p->n_stages++] = 3; n /= 3; }
     while (n % 8 == 0) { p->radix[p->n_stages++] = 8; n /= 8; }
     if (n % 4 == 0) { p->radix[p->n_stages++] = 4; n /= 4; }
@@ -86,15 +88,15 @@ nm_status validate(const nm_mesh_desc *d)
         if (std::fabs(n2 - 1.0) > 1e-9) { nm_set_error("ku_axis must be a unit vector"); return NM_EINVAL; }
     }
     if (d->terms & NM_TERM_DEMAG) {
-        // a mesh the zero-extended fast path serves needs no radix-2/3 factorisation of its own
+        // a mesh the zero-extended fast path serves needs no factorisation of its own
         NmGeom ge;
         NmFast fe;
         make_geom(d, &ge);
         nm_fast_plan(d, ge, &fe);
         const bool embedded = fe.on && fe.embed && !getenv("NM_DEMAG_PATH") && !getenv("NM_PIPE");
         for (int i = 0; i < 3; ++i)
-            if (!embedded && d->n_cells[i] > 1 && !smooth23(d->n_cells[i])) {
-                nm_set_error("n_cells[%d] = %d is not of the form 2^a 3^b (demag FFT radices)", i, d->n_cells[i]);
+            if (!embedded && d->n_cells[i] > 1 && !smooth7(d->n_cells[i])) {
+                nm_set_error("n_cells[%d] = %d is not of the form 2^a 3^b 5^c 7^d (demag FFT radices)", i, d->n_cells[i]);
                 return NM_EUNSUPPORTED;
             }
         const size_t cx = d->dtype == NM_F64 ? 16 : 8;

@@ -103,6 +103,34 @@ __device__ __forceinline__ void dft8(typename Cx<T>::V *x)
     x[7] = C::sub(e[3], t3);
 }
 
+// Odd prime radix (5, 7): the R-point DFT by its definition, y_k = sum_t x_t w^(k t mod R) with
+// w^q = exp(-/+ 2 pi i q / R) = tw[q L / R] (conjugated for the inverse) read from the table of
+// the whole transform.
+template <typename T, bool INV, int R>
+__device__ __forceinline__ void dft_prime(typename Cx<T>::V *x, const typename Cx<T>::V *__restrict__ tw, int L)
+{
+    typedef Cx<T> C;
+    typedef typename C::V V;
+    V w[R];
+    const int step = L / R;
+#pragma unroll
+    for (int q = 1; q < R; ++q) w[q] = tw[q * step];
+    V y[R];
+    y[0] = x[0];
+#pragma unroll
+    for (int t = 1; t < R; ++t) y[0] = C::add(y[0], x[t]);
+#pragma unroll
+    for (int k = 1; k < R; ++k) {
+        V acc = x[0];
+#pragma unroll
+        for (int t = 1; t < R; ++t)
+            acc = C::add(acc, INV ? C::mulc(x[t], w[(k * t) % R]) : C::mul(x[t], w[(k * t) % R]));
+        y[k] = acc;
+    }
+#pragma unroll
+    for (int k = 0; k < R; ++k) x[k] = y[k];
+}
+
 template <typename T, bool INV, int R>
 __device__ __forceinline__ void dftR(typename Cx<T>::V *x)
 {
@@ -148,7 +176,8 @@ __device__ __forceinline__ void fft_stage(typename Cx<T>::V *s, int n_lines, int
 #pragma unroll
             for (int t = 1; t < R; ++t) x[t] = C::mulc(x[t], tw[j * t * tw_step]);
         }
-        dftR<T, INV, R>(x);
+        if (R == 5 || R == 7) dft_prime<T, INV, R>(x, tw, L);
+        else dftR<T, INV, R>(x);
         if (!INV) {
 #pragma unroll
             for (int t = 1; t < R; ++t) x[t] = C::mul(x[t], tw[j * t * tw_step]);
@@ -167,6 +196,8 @@ __device__ __forceinline__ void fft_stage_any(int R, typename Cx<T>::V *s, int n
     case 2: fft_stage<T, INV, 2, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     case 3: fft_stage<T, INV, 3, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     case 4: fft_stage<T, INV, 4, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
+    case 5: fft_stage<T, INV, 5, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
+    case 7: fft_stage<T, INV, 7, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     default: fft_stage<T, INV, 8, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     }
 }

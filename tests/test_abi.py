@@ -55,13 +55,14 @@ def test_query_workspace_validates(nm):
     assert nm.nm_mesh_query_workspace(_desc(nm, terms=3)) > nm.nm_mesh_query_workspace(_desc(nm, terms=1))
     for bad, status in ((dict(n=(0, 8, 8)), nm.NM_EINVAL), (dict(terms=0), nm.NM_EINVAL),
                         (dict(terms=32), nm.NM_EINVAL), (dict(dx=(1e-9, 0.0, 1e-9)), nm.NM_EINVAL),
-                        (dict(n=(10, 8, 8)), nm.NM_EUNSUPPORTED), (dict(n=(7, 8, 8), terms=2), nm.NM_EUNSUPPORTED)):
+                        (dict(n=(11, 8, 8)), nm.NM_EUNSUPPORTED), (dict(n=(8, 13, 8), terms=2), nm.NM_EUNSUPPORTED)):
         with pytest.raises(nm.NmError) as e:
             nm.nm_mesh_query_workspace(_desc(nm, **bad))
         assert e.value.status == status, bad
         assert str(e.value)
-    # sizes that are not 2^a 3^b are fine without the demag term
+    # sizes that are not 2^a 3^b 5^c 7^d are fine without the demag term
     assert nm.nm_mesh_query_workspace(_desc(nm, n=(7, 5, 11), terms=1)) > 0
+    assert nm.nm_mesh_query_workspace(_desc(nm, n=(10, 7, 35), terms=3)) > 0
 
 
 def test_workspace_grows_with_the_grid(nm):

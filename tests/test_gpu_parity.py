@@ -87,6 +87,19 @@ def test_heff_fast_path_sizes(n, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n", [(20, 10, 5), (14, 7, 1), (5, 35, 6), (40, 24, 1), (50, 1, 1), (7, 7, 7),
+                               (10, 28, 45)])
+def test_heff_radix_5_7_sizes(n, prec, monkeypatch):
+    """N_d with factors 5 and 7 (general path: radix-5 / 7 stages by the DFT sum in the x, y and z
+    passes, mixed with the radix-8/4/3/2 stages); all terms, cell-wise materials, vacuum block."""
+    monkeypatch.setenv("NM_DEMAG_PATH", "generic")      # not the zero-extended fast path
+    w, hs = wl.varied_case(n, vacuum=(n[0] >= 6))
+    got, ref, mesh, *_ = _heff_case(w, prec, hs)
+    assert mesh.nm_debug_demag_path() == 0
+    assert rel_l2(got, ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("n", [(36, 128, 112), (68, 96, 100), (52, 64, 40), (100, 32, 24)])
 def test_heff_embedded_fast_path_sizes(n, prec):
     """Grids the fast path serves on the zero-extended mesh (some N_d below the next 16 * 2^k, not
@@ -329,7 +342,7 @@ def test_adjoint_gradient_driver_vs_finite_differences_config5_small_fp64():
 def test_errors_are_statuses_not_crashes():
     from paper_2411_11725_b200 import binding as nm
     with pytest.raises(nm.NmError) as e:
-        nm.Mesh((5, 4, 4), (1e-9,) * 3, terms=wl.TERM_DEMAG, Ms=1.0, A=0.0, Ku=0.0)
+        nm.Mesh((11, 4, 4), (1e-9,) * 3, terms=wl.TERM_DEMAG, Ms=1.0, A=0.0, Ku=0.0)
     assert e.value.status == nm.NM_EUNSUPPORTED
     with pytest.raises(nm.NmError) as e:
         nm.Mesh((0, 4, 4), (1e-9,) * 3, terms=1, Ms=1.0, A=1.0, Ku=0.0)

@@ -134,6 +134,57 @@ def test_adjoint_state_gradient_against_finite_differences():
     assert np.abs(u0_b - u0).max() < 1e-3 * np.abs(u0).max()
 
 
+def test_objectives_at_several_times_against_finite_differences():
+    """PAPER.md:228 on a 6x2x1 film: L = w1 . m(T1) + w2 . m(T2) + wT . m(T), T1 < T2 < T; the
+    adjoint variable jumps by grad L_i at T_i.  dL/dMs against central differences, and additivity:
+    the gradient equals the sum of the single-time gradients over [0, T1], [0, T2], [0, T]."""
+    rng = np.random.default_rng(17)
+    n, dx = (6, 2, 1), (4e-9, 4e-9, 5e-9)
+    p = Problem(n, dx, rng.uniform(1e5, 1.5e5, n), np.full(n, 3.65e-12), np.zeros(n), alpha=1e-2,
+                terms=TERM_EXCHANGE | TERM_DEMAG | TERM_ZEEMAN)
+    p.Nt
+    zee = lambda t: np.array([0.0, 2e3, 0.0])
+    m0 = 0.1 * rng.standard_normal((3,) + p.node_shape)
+    m0[0] += 1
+    m0 /= np.sqrt(np.sum(m0 * m0, axis=0))
+    dt, nst, s1, s2 = 5e-14, 120, 40, 90
+    w1, w2, wT = (rng.standard_normal(m0.shape) for _ in range(3))
+
+    def traj(prob):
+        out, m = {}, m0.copy()
+        for s in range(nst):
+            if s in (s1, s2):
+                out[s] = m.copy()
+            m = llg.rk4_step(prob, s * dt, dt, m, zee)
+        return out[s1], out[s2], m
+
+    def L(prob):
+        a, b, c = traj(prob)
+        return float(np.sum(w1 * a) + np.sum(w2 * b) + np.sum(wT * c))
+
+    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=30)
+    _, _, u0 = adjoint.backward_rk4(p, mT, wT, dt, nst, zee, checkpoints=ck, a_jumps={s1: w1, s2: w2})
+    for c in [(0, 0, 0), (3, 1, 0), (5, 0, 0)]:
+        h = 1e-4 * p.Ms[c]
+        Mp, Mm = p.Ms.copy(), p.Ms.copy()
+        Mp[c] += h
+        Mm[c] -= h
+        fd = (L(with_Ms(p, Mp)) - L(with_Ms(p, Mm))) / (2 * h)
+        assert abs(u0[c] - fd) < 1e-3 * abs(fd), (c, u0[c], fd)
+    # additivity over the objectives (the adjoint system is linear in a): three single-time runs;
+    # equal up to the backward reconstruction of m between checkpoints (a run that ends at T_i
+    # starts from the exact m(T_i), the joint run arrives there by inverse integration)
+    total = np.zeros_like(u0)
+    for steps, w in ((s1, w1), (s2, w2), (nst, wT)):
+        mS, ckS = adjoint.forward_rk4(p, m0, dt, steps, zee, checkpoint_every=30)
+        total += adjoint.backward_rk4(p, mS, w, dt, steps, zee, checkpoints=ckS)[2]
+    assert np.abs(total - u0).max() < 1e-6 * np.abs(u0).max()
+    # a jump of zero is no jump
+    _, _, u_plain = adjoint.backward_rk4(p, mT, wT, dt, nst, zee, checkpoints=ck)
+    _, _, u_zero = adjoint.backward_rk4(p, mT, wT, dt, nst, zee, checkpoints=ck, a_jumps={s1: 0.0 * w1})
+    assert np.array_equal(u_plain, u_zero)
+
+
 def test_adjoint_driver_zero_and_linearity():
     rng = np.random.default_rng(8)
     n, dx = (4, 2, 1), (4e-9, 4e-9, 5e-9)

@@ -151,6 +151,13 @@ nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, const void 
 nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
                               void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream);
 
+/* Objectives at several times T_i ("adding appropriate terms depending on m(T_i)"):
+ * when the backward integration of Eq. (29) arrives at T_i the adjoint variable takes the jump
+ *   a_inout <- a_inout + scale * dLdm     (device nodal 3-vectors of the mesh dtype),
+ * dLdm = grad_m L_i(m(T_i)) from the caller.  a_inout and dLdm must not overlap. */
+nm_status nm_adjoint_add_objective(nm_mesh *mesh, void *a_inout, const void *dLdm, double scale,
+                                   void *stream);
+
 /* Debug / test getters (not hot path).  Copy the real-space demag tensor N[6][N3][N2][N1]
  * (components xx,yy,zz,xy,xz,yz; non-negative cell offsets; fp64) to a HOST buffer, and the
  * cell-wise demag field [3][N3][N2][N1] of the last nm_heff/nm_llg_rhs call (mesh dtype) to a

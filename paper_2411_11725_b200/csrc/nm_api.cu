@@ -915,3 +915,20 @@ extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, voi
                                               (float *)u_inout, zeeman, renormalise, s);
     });
 }
+
+extern "C" nm_status nm_adjoint_add_objective(nm_mesh *mesh, void *a_inout, const void *dLdm, double scale,
+                                              void *stream)
+{
+    NM_TRY(check_call(mesh, a_inout, dLdm));
+    if (a_inout == dLdm) { nm_set_error("a_inout and dLdm overlap"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long nv = 3 * mesh->g.nodes;
+    if (mesh->f64) {
+        const double c = scale;
+        const double *src[1] = {(const double *)dLdm};
+        return nm_lincomb<double>(mesh, (double *)a_inout, (const double *)a_inout, 1, src, &c, nv, 0, st);
+    }
+    const float c = (float)scale;
+    const float *src[1] = {(const float *)dLdm};
+    return nm_lincomb<float>(mesh, (float *)a_inout, (const float *)a_inout, 1, src, &c, nv, 0, st);
+}

@@ -45,14 +45,29 @@ def forward_rk4(mesh, m, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
     return ck
 
 
-def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_every=100, t0=0.0):
+def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_every=100, t0=0.0,
+                     objectives_at=None):
     """Adjoint-state gradient dJ/dMs (Eqs. 27-30; reading C8).
 
     Forward RK4 from m0 with checkpoints, a(T) = aT_of_mT(m(T)) (the caller's dJ/dm(T)), then the
     backward RK4 of (m, a, u) with step -dt, m replaced by the stored checkpoint whenever one is
-    reached.  Returns (m(T), a(0), u(0) = dJ/dMs per cell)."""
+    reached.  Returns (m(T), a(0), u(0) = dJ/dMs per cell).
+
+    objectives_at = {step index s < n_steps: callable m(t0 + s dt) -> dL_s/dm}: objective terms at
+    further times; each is evaluated on the forward pass and added to the adjoint
+    variable when the backward pass arrives at its time (nm_adjoint_add_objective)."""
     m = m0.clone()
-    ck = forward_rk4(mesh, m, dt, n_steps, zeeman, checkpoint_every, t0)
+    jumps = {}
+    if objectives_at:
+        ck = {}
+        for s in range(n_steps):
+            if checkpoint_every and s % checkpoint_every == 0:
+                ck[s] = m.clone()
+            if s in objectives_at:
+                jumps[s] = objectives_at[s](m).clone()
+            mesh.nm_rk_step(0, t0 + s * dt, dt, m, zeeman)
+    else:
+        ck = forward_rk4(mesh, m, dt, n_steps, zeeman, checkpoint_every, t0)
     mT = m.clone()
     a = aT_of_mT(mT).clone()
     u = torch.zeros(mesh.cell_shape_abi, dtype=m.dtype, device=m.device)
@@ -60,4 +75,6 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
         mesh.nm_adjoint_rk4_step(t0 + s * dt, dt, m, a, u, zeeman)
         if (s - 1) in ck:
             m.copy_(ck[s - 1])
+        if (s - 1) in jumps:
+            mesh.nm_adjoint_add_objective(a, jumps[s - 1])
     return mT, a, u

@@ -33,3 +33,56 @@ def test_integrate_dopri5_loop_control():
         assert t1 == t0 and h1 < h0
     # the last step is clipped to land on t1 exactly
     assert abs(mesh.calls[-1][0] + mesh.calls[-1][1] - 1.0) < 1e-15
+
+
+class _FakeAdjMesh:
+    """Scalar stand-in for the adjoint loops: m += 1 per forward step, m -= 1 per backward step;
+    records the order of the calls."""
+    cell_shape_abi = (1,)
+
+    def __init__(self):
+        self.log = []
+
+    def nm_rk_step(self, scheme, t, dt, m, zeeman):
+        m += 1.0
+        self.log.append(("fwd", round(t / dt)))
+
+    def nm_adjoint_rk4_step(self, t, dt, m, a, u, zeeman):
+        m -= 1.0
+        u += a.sum()
+        self.log.append(("bwd", round(t / dt)))
+
+    def nm_adjoint_add_objective(self, a, g, scale=1.0):
+        a += scale * g
+        self.log.append(("jump", float(g.sum())))
+
+
+def test_adjoint_gradient_loop_adds_objectives_at_their_times():
+    """a term L_s(m(t_s)) is evaluated on the forward pass at step s and added to the
+    adjoint variable right after the backward step that arrives at t_s (after the checkpoint
+    restore of that index)."""
+    import torch
+    mesh = _FakeAdjMesh()
+    m0 = torch.zeros(1, dtype=torch.float64)
+    seen = {}
+
+    def at(s):
+        def f(m):
+            seen[s] = float(m[0])
+            return torch.full((1,), 10.0 * s, dtype=torch.float64)
+        return f
+
+    mT, a0, u0 = drivers.adjoint_gradient(mesh, m0, lambda m: torch.ones(1, dtype=torch.float64), 1.0, 6,
+                                          checkpoint_every=3, objectives_at={2: at(2), 4: at(4)})
+    assert seen == {2: 2.0, 4: 4.0}                  # evaluated on m(t_s) of the forward pass
+    assert float(mT[0]) == 6.0
+    order = [e for e in mesh.log if e[0] != "fwd"]
+    assert order == [("bwd", 6), ("bwd", 5), ("jump", 40.0), ("bwd", 4), ("bwd", 3), ("jump", 20.0),
+                     ("bwd", 2), ("bwd", 1)]
+    assert float(a0[0]) == 1.0 + 40.0 + 20.0
+    # u sums a before each backward step: 1, 1, 41, 41, 61, 61
+    assert float(u0[0]) == 1 + 1 + 41 + 41 + 61 + 61
+    # without further objectives the loop is the plain one
+    mesh2 = _FakeAdjMesh()
+    drivers.adjoint_gradient(mesh2, m0, lambda m: torch.ones(1, dtype=torch.float64), 1.0, 4, checkpoint_every=2)
+    assert [e[0] for e in mesh2.log] == ["fwd"] * 4 + ["bwd"] * 4

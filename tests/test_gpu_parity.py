@@ -338,6 +338,45 @@ def test_adjoint_gradient_driver_vs_finite_differences_config5_small_fp64():
         assert abs(grad[c] - fd) <= 1e-3 * abs(fd), (c, grad[c], fd)
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_adjoint_gradient_objectives_at_several_times(prec):
+    """L = w1 . m(T1) + w2 . m(T2) + wT . m(T) on a 32x8x1 film (config 5's recipe, 36
+    steps, checkpoints every 12): drivers.adjoint_gradient with objectives_at (the jumps go through
+    nm_adjoint_add_objective) against the oracle's backward pass with the same jumps."""
+    from oracle import adjoint
+    from paper_2411_11725_b200 import drivers
+    td = DT[prec]
+    nd = np_dtype(td)
+    w = wl.config5_inverse((32, 8, 1), n_steps=36)
+    p = oracle_problem(w, nd)
+    z = oracle_zeeman(w, nd)
+    m0 = _m0(w, td)
+    rng = np.random.default_rng(23)
+    w1, w2 = (wl.round_to(rng.standard_normal(m0.shape), nd) for _ in range(2))
+    wT = wl.round_to(wl.objective_weights(w), nd)
+    s1, s2 = 10, 24
+    mT_ref, ck = adjoint.forward_rk4(p, m0, w.dt, w.n_steps, z, checkpoint_every=12)
+    _, a0_ref, u0_ref = adjoint.backward_rk4(p, mT_ref, wT, w.dt, w.n_steps, z, checkpoints=ck,
+                                             a_jumps={s1: w1, s2: w2})
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    g1, g2, gT = dev(w1, td), dev(w2, td), dev(wT, td)
+    mT, a0, u0 = drivers.adjoint_gradient(mesh, dev(m0, td), lambda m: gT, w.dt, w.n_steps, gz,
+                                          checkpoint_every=12,
+                                          objectives_at={s1: lambda m: g1, s2: lambda m: g2})
+    assert rel_l2(host(mT), mT_ref) <= TOL[prec]
+    assert rel_l2(host(a0), a0_ref) <= (1e-11 if prec == "f64" else 1e-5)
+    assert rel_l2(wl.from_abi(u0.cpu().double().numpy()), u0_ref) <= (1e-11 if prec == "f64" else 2e-4)
+    # the jump itself: a <- a + scale g, and overlapping arguments are refused
+    from paper_2411_11725_b200 import binding as nm
+    a = g1.clone()
+    mesh.nm_adjoint_add_objective(a, g2, scale=-0.5)
+    assert torch.equal(a, g1 + (-0.5) * g2)
+    with pytest.raises(nm.NmError) as e:
+        mesh.nm_adjoint_add_objective(a, a)
+    assert e.value.status == nm.NM_EINVAL
+
+
 # ---- boundary behaviour --------------------------------------------------------------------------
 def test_errors_are_statuses_not_crashes():
     from paper_2411_11725_b200 import binding as nm

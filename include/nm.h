@@ -131,7 +131,8 @@ nm_status nm_llg_rhs(nm_mesh *mesh, double t, const void *m, const nm_zeeman *ze
  * `zeeman`) and zeeman->amp is NULL, its kernel launches are captured once into a CUDA graph
  * and replayed with one launch on `stream`; same kernels, same arguments, identical results.
  * The arrays `zeeman` points to are then read at replay time, as the launches would.  The same
- * holds for nm_adjoint_rk4_step (key: dt, m_inout, a_inout, u_inout, renormalise, zeeman). */
+ * holds for nm_adjoint_rk4_step[_hext] (key: dt, m_inout, a_inout, u_inout, u_h_inout, renormalise,
+ * zeeman). */
 nm_status nm_rk_step(nm_mesh *mesh, nm_scheme scheme, double t, double dt, void *m_inout,
                      const nm_zeeman *zeeman, int renormalise, double rtol, double atol,
                      double *err_norm_host, void *stream);
@@ -150,6 +151,20 @@ nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, const void 
  * u_inout is the cell-wise accumulator whose value at t = 0 is grad_Ms of the objective (Eq. 30). */
 nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
                               void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream);
+
+/* Gradient with respect to a spatially uniform external field h (added to zeeman->h_uniform): the
+ * design variable of the field-angle problem, Eqs. (31)-(33).  A uniform field
+ * passes through the weak form of Eq. (21) unchanged at every node with (S Ms)_n > 0, so
+ *   -(df/dh)^T a = - sum_{n: (S Ms)_n > 0} b_n,   b = g' m x a - alpha g' m x (m x a)
+ * (fp64 accumulation in a fixed order; zero when the mesh has no Zeeman term).
+ *   nm_llg_adjoint_rhs_hext: dudt_h_out[3] (DEVICE, fp64) = that 3-vector for the given m, a.
+ *   nm_adjoint_rk4_step_hext: nm_adjoint_rk4_step that also integrates u_h_inout[3] (DEVICE, fp64)
+ *   backwards; with u_h(T) = 0, u_h(0) = dL/dh. */
+nm_status nm_llg_adjoint_rhs_hext(nm_mesh *mesh, const void *m, const void *a, double *dudt_h_out,
+                                  void *stream);
+nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                                   void *u_inout, double *u_h_inout, const nm_zeeman *zeeman,
+                                   int renormalise, void *stream);
 
 /* Objectives at several times T_i ("adding appropriate terms depending on m(T_i)"):
  * when the backward integration of Eq. (29) arrives at T_i the adjoint variable takes the jump

@@ -81,6 +81,23 @@ def adjoint_rhs(p, t, m, a, zeeman=None):
     return f, dadt, -grad
 
 
+def adjoint_rhs_hext(p, t, m, a):
+    """-(df/dh)^T a for a spatially uniform external field h added to H_ext (the design variable of
+    the field-angle problem, Eqs. 31-33).
+
+    A uniform h passes through the weak form of Eq. (21) unchanged at every node with L_n > 0 and
+    gives no field at vacuum nodes (reading C3(ii), (iii)), so dH_n/dh = [L_n > 0] I and
+        (df/dh)^T a = sum_{n: L_n > 0} b_n,   b = (df/dH)^T a = g' m x a - alpha g' m x (m x a)
+    (b depends on m and a only).  Returns the 3-vector -(df/dh)^T a; zero without the Zeeman term."""
+    if not (p.terms & _llg.TERM_ZEEMAN):
+        return np.zeros(3)
+    gp = p.gamma / (1.0 + p.alpha ** 2)
+    mxa = _llg.cross(m, a)
+    b = gp * mxa - p.alpha * gp * _llg.cross(m, mxa)
+    inside = p.L > 0
+    return -np.array([np.sum(b[j][inside]) for j in range(3)])
+
+
 def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
     """Fixed-step RK4 with renormalisation; returns (m_T, {step index: m}) (C8)."""
     m = m0.copy()
@@ -92,7 +109,8 @@ def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
     return m, ckpt
 
 
-def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, a_jumps=None):
+def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, a_jumps=None,
+                 with_hext=False):
     """Integrate Eq. (29) from T = t0 + n_steps dt back to t0 with RK4 steps of -dt.
 
     State (m, a, u); m is renormalised after every step and replaced by the stored forward
@@ -104,13 +122,19 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
     a_jumps = {s_i: grad_m L_i(m(T_i))}; the adjoint variable takes the jump a += a_jumps[s_i]
     when the backward integration arrives at T_i (the term of L_i enters the adjoint equation as
     a delta function in time).
+
+    with_hext: also integrate du_h/dt = -(df/dh)^T a (adjoint_rhs_hext) with u_h(T) = 0 and return
+    (m0, a0, u0, u_h(0)); u_h(0) = dL/dh for a uniform external field h.
     """
     m, a = mT.copy(), aT.copy()
     u = np.zeros(p.n_cells)
     h = -dt
 
+    uh = np.zeros(3)
+
     def F(t, m_, a_):
-        return adjoint_rhs(p, t, m_, a_, zeeman)
+        r = adjoint_rhs(p, t, m_, a_, zeeman)
+        return r + (adjoint_rhs_hext(p, t, m_, a_),) if with_hext else r
 
     for s in range(n_steps, 0, -1):
         t = t0 + s * dt
@@ -121,8 +145,12 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
         m = _llg.normalise(m + h / 6.0 * (k1[0] + 2 * k2[0] + 2 * k3[0] + k4[0]))
         a = a + h / 6.0 * (k1[1] + 2 * k2[1] + 2 * k3[1] + k4[1])
         u = u + h / 6.0 * (k1[2] + 2 * k2[2] + 2 * k3[2] + k4[2])
+        if with_hext:
+            uh = uh + h / 6.0 * (k1[3] + 2 * k2[3] + 2 * k3[3] + k4[3])
         if checkpoints is not None and (s - 1) in checkpoints:
             m = checkpoints[s - 1].copy()
         if a_jumps is not None and (s - 1) in a_jumps:
             a = a + a_jumps[s - 1]
+    if with_hext:
+        return m, a, u, uh
     return m, a, u

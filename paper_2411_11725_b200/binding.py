@@ -22,7 +22,7 @@ NM_RK4, NM_DOPRI5 = 0, 1
 
 EXPORTS = ("nm_mesh_query_workspace", "nm_mesh_create", "nm_mesh_set_Ms", "nm_mesh_destroy",
            "nm_last_error", "nm_heff", "nm_llg_rhs", "nm_rk_step", "nm_llg_adjoint_rhs",
-           "nm_adjoint_rk4_step", "nm_adjoint_add_objective", "nm_debug_get_tensor", "nm_debug_get_cell_field",
+           "nm_adjoint_rk4_step", "nm_adjoint_add_objective", "nm_llg_adjoint_rhs_hext", "nm_adjoint_rk4_step_hext", "nm_debug_get_tensor", "nm_debug_get_cell_field",
            "nm_launch_count", "nm_debug_demag_path", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
            "nm_profile_end")
 
@@ -82,6 +82,8 @@ def lib():
         L.nm_llg_adjoint_rhs.argtypes = [vp, dbl, vp, vp, ctypes.POINTER(nm_zeeman), vp, vp, vp, vp]
         L.nm_adjoint_rk4_step.argtypes = [vp, dbl, dbl, vp, vp, vp, ctypes.POINTER(nm_zeeman), i32, vp]
         L.nm_adjoint_add_objective.argtypes = [vp, vp, vp, dbl, vp]
+        L.nm_llg_adjoint_rhs_hext.argtypes = [vp, vp, vp, vp, vp]
+        L.nm_adjoint_rk4_step_hext.argtypes = [vp, dbl, dbl, vp, vp, vp, vp, ctypes.POINTER(nm_zeeman), i32, vp]
         L.nm_debug_get_tensor.argtypes = [vp, vp]
         L.nm_debug_get_cell_field.argtypes = [vp, vp, vp]
         L.nm_launch_count.argtypes = [vp]
@@ -227,6 +229,17 @@ class Mesh:
     def nm_adjoint_rk4_step(self, t, dt, m, a, u, zeeman=None, renormalise=True):
         _check(lib().nm_adjoint_rk4_step(self.handle, float(t), float(dt), _ptr(m), _ptr(a), _ptr(u),
                                          _zref(zeeman), 1 if renormalise else 0, _stream(self.device)))
+
+    def nm_llg_adjoint_rhs_hext(self, m, a):
+        out = torch.empty(3, dtype=torch.float64, device=m.device)
+        _check(lib().nm_llg_adjoint_rhs_hext(self.handle, _ptr(m), _ptr(a), _ptr(out), _stream(self.device)))
+        return out
+
+    def nm_adjoint_rk4_step_hext(self, t, dt, m, a, u, u_h, zeeman=None, renormalise=True):
+        assert u_h.dtype == torch.float64 and u_h.numel() == 3 and u_h.is_cuda
+        _check(lib().nm_adjoint_rk4_step_hext(self.handle, float(t), float(dt), _ptr(m), _ptr(a), _ptr(u),
+                                              _ptr(u_h), _zref(zeeman), 1 if renormalise else 0,
+                                              _stream(self.device)))
 
     def nm_adjoint_add_objective(self, a, dLdm, scale=1.0):
         _check(lib().nm_adjoint_add_objective(self.handle, _ptr(a), _ptr(dLdm), float(scale),

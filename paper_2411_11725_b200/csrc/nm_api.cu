@@ -149,6 +149,7 @@ size_t carve(nm_mesh *m, char *base)
     m->sMs = c.take(g.nodes * e);
     m->n_partials = nm_node_blocks(g);
     m->partials = (double *)c.take(((size_t)m->n_partials + 1) * sizeof(double));
+    m->hpart = (double *)c.take((size_t)3 * NM_HEXT_BLOCKS * sizeof(double));
     // Runge-Kutta / adjoint scratch; doubles as fp64 scratch of the tensor setup
     const size_t vec = (size_t)3 * g.nodes * e;
     size_t rk = 9 * vec;
@@ -720,9 +721,11 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
 }
 
 template <typename T>
-nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, const nm_zeeman *z,
+nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, double *uh, const nm_zeeman *z,
                       int renorm, cudaStream_t st)
 {
+    const double gp_h = m->desc.gamma / (1.0 + m->desc.alpha * m->desc.alpha);
+    const bool want_h = uh && (m->desc.terms & NM_TERM_ZEEMAN);
     const long long nv = 3 * m->g.nodes, nc = m->g.cells, nn = m->g.nodes;
     T *F = (T *)m->K[0], *DA = (T *)m->K[1], *AM = (T *)m->K[2], *AA = (T *)m->K[3];
     T *Ym = (T *)m->Y[0], *Ya = (T *)m->Y[1];
@@ -734,6 +737,8 @@ nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, const
     const T *sm = mm, *sa = av;
     for (int s = 0; s < 4; ++s) {
         NM_TRY(adjoint_eval<T>(m, ts[s], sm, sa, z, F, DA, DU, st));
+        // u_h += w_s (-(df/dh)^T a) of this stage (reads the stage state before it is overwritten)
+        if (want_h) NM_TRY(nm_launch_hext_grad<T>(m, sm, sa, gp_h, m->desc.alpha * gp_h, w[s], uh, st));
         const T ws = (T)w[s];
         if (s < 3) {
             // accumulators (the first stage starts them from the state) and the next stage state
@@ -895,8 +900,9 @@ extern "C" nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, 
                                            (float *)dmdt_out, (float *)dadt_out, (float *)dudt_Ms_out, st);
 }
 
-extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
-                                         void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
+namespace {
+nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout, void *u_inout,
+                            double *u_h_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
 {
     NM_TRY(check_call(mesh, m_inout, a_inout));
     if (!u_inout) { nm_set_error("u_inout is NULL"); return NM_EINVAL; }
@@ -908,12 +914,43 @@ extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, voi
     key.p[0] = m_inout;
     key.p[1] = a_inout;
     key.p[2] = u_inout;
+    key.p[3] = u_h_inout;
     return run_step(mesh, NM_GRAPH_ADJ_RK4, zeeman, key, st, [&](cudaStream_t s) {
         return mesh->f64 ? adjoint_rk4<double>(mesh, t, dt, (double *)m_inout, (double *)a_inout,
-                                               (double *)u_inout, zeeman, renormalise, s)
+                                               (double *)u_inout, u_h_inout, zeeman, renormalise, s)
                          : adjoint_rk4<float>(mesh, t, dt, (float *)m_inout, (float *)a_inout,
-                                              (float *)u_inout, zeeman, renormalise, s);
+                                              (float *)u_inout, u_h_inout, zeeman, renormalise, s);
     });
+}
+} // namespace
+
+extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                                         void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
+{
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, nullptr, zeeman, renormalise, stream);
+}
+
+extern "C" nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                                              void *u_inout, double *u_h_inout, const nm_zeeman *zeeman,
+                                              int renormalise, void *stream)
+{
+    if (!u_h_inout) { nm_set_error("u_h_inout is NULL"); return NM_EINVAL; }
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, u_h_inout, zeeman, renormalise, stream);
+}
+
+extern "C" nm_status nm_llg_adjoint_rhs_hext(nm_mesh *mesh, const void *m, const void *a, double *dudt_h_out,
+                                             void *stream)
+{
+    NM_TRY(check_call(mesh, m, a));
+    if (!dudt_h_out) { nm_set_error("dudt_h_out is NULL"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    NM_CUDA_TRY(cudaMemsetAsync(dudt_h_out, 0, 3 * sizeof(double), st));
+    if (!(mesh->desc.terms & NM_TERM_ZEEMAN)) return NM_OK;
+    const double gp = mesh->desc.gamma / (1.0 + mesh->desc.alpha * mesh->desc.alpha);
+    return mesh->f64 ? nm_launch_hext_grad<double>(mesh, (const double *)m, (const double *)a, gp,
+                                                   mesh->desc.alpha * gp, 1.0, dudt_h_out, st)
+                     : nm_launch_hext_grad<float>(mesh, (const float *)m, (const float *)a, gp,
+                                                  mesh->desc.alpha * gp, 1.0, dudt_h_out, st);
 }
 
 extern "C" nm_status nm_adjoint_add_objective(nm_mesh *mesh, void *a_inout, const void *dLdm, double scale,

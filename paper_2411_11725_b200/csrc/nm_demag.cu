@@ -26,7 +26,7 @@ constexpr int kThreads = 256;
 constexpr int kRowsX = 4;   // cell rows (c2) per CTA in the x passes (2 where that leaves SMs without a CTA)
 
 // ---------------------------------------------------------------------------------------------
-template <typename T, int RX>
+template <typename T, int RX, bool PR>
 __global__ void __launch_bounds__(kThreads)
 k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *__restrict__ A,
         NmGeom g, NmFftPlan plan, const typename Cx<T>::V *__restrict__ tw,
@@ -70,7 +70,7 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
     }
     __syncthreads();
     // 2. complex transform of length Lx
-    fft_forward<T, false>(s, n_lines, Lx, 1, plan, tw);
+    fft_forward<T, false, PR>(s, n_lines, Lx, 1, plan, tw);
     // 3. untangle: X[k] = 1/2 [(Z[k] + conj Z[Lx-k]) - i W^k (Z[k] - conj Z[Lx-k])], k = 0..N1
     for (int idx = threadIdx.x; idx < n_lines * g.C1; idx += blockDim.x) {
         const int k = idx % g.C1;
@@ -90,7 +90,7 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
     }
 }
 
-template <typename T, int RX>
+template <typename T, int RX, bool PR>
 __global__ void __launch_bounds__(kThreads)
 k_x_inv(const typename Cx<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, NmFftPlan plan,
         const typename Cx<T>::V *__restrict__ tw, const typename Cx<T>::V *__restrict__ tw2,
@@ -127,7 +127,7 @@ k_x_inv(const typename Cx<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, N
         s[line * Lx + pos[k]] = z;
     }
     __syncthreads();
-    fft_inverse<T, false>(s, n_lines, Lx, 1, plan, tw);
+    fft_inverse<T, false, PR>(s, n_lines, Lx, 1, plan, tw);
     // 2. x[2n] = Re z[n], x[2n+1] = Im z[n], cropped to N1
     for (int idx = threadIdx.x; idx < n_lines * g.N1; idx += blockDim.x) {
         const int c1 = idx % g.N1;
@@ -142,7 +142,7 @@ k_x_inv(const typename Cx<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, N
 
 // ---------------------------------------------------------------------------------------------
 // y transform of one (component, c3) slab for a tile of k1 columns.
-template <typename T, bool INV>
+template <typename T, bool INV, bool PR>
 __global__ void __launch_bounds__(kThreads)
 k_lines(const typename Cx<T>::V *__restrict__ src, typename Cx<T>::V *__restrict__ dst, NmGeom g,
         int bt, NmFftPlan plan, const typename Cx<T>::V *__restrict__ tw)
@@ -164,8 +164,8 @@ k_lines(const typename Cx<T>::V *__restrict__ src, typename Cx<T>::V *__restrict
         s[idx] = v;
     }
     __syncthreads();
-    if (INV) fft_inverse<T, true>(s, bt, 1, bt, plan, tw);
-    else fft_forward<T, true>(s, bt, 1, bt, plan, tw);
+    if (INV) fft_inverse<T, true, PR>(s, bt, 1, bt, plan, tw);
+    else fft_forward<T, true, PR>(s, bt, 1, bt, plan, tw);
     const int n_out = INV ? N : P;
     for (int idx = threadIdx.x; idx < n_out * bt; idx += blockDim.x) {
         const int b = idx % bt, e = idx / bt;
@@ -185,7 +185,7 @@ struct MidArgs {
     int n_fixed;              // extent of the fixed index (P2 in 3-D, 1 otherwise)
 };
 
-template <typename T>
+template <typename T, bool PR>
 __global__ void __launch_bounds__(kThreads)
 k_mid(typename Cx<T>::V *__restrict__ buf, const T *__restrict__ Nhat, NmGeom g, MidArgs a, int bt,
       NmFftPlan plan, const typename Cx<T>::V *__restrict__ tw, const int *__restrict__ kmap_line,
@@ -214,7 +214,7 @@ k_mid(typename Cx<T>::V *__restrict__ buf, const T *__restrict__ Nhat, NmGeom g,
         s[idx] = v;
     }
     __syncthreads();
-    fft_forward<T, true>(s, n_lines, 1, n_lines, plan, tw);
+    fft_forward<T, true, PR>(s, n_lines, 1, n_lines, plan, tw);
     // tensor multiply
     const long long tcomp = (long long)g.K3 * g.K2 * g.C1p;
     int kk_fixed = 0;
@@ -248,7 +248,7 @@ k_mid(typename Cx<T>::V *__restrict__ buf, const T *__restrict__ Nhat, NmGeom g,
         p[2 * bt] = C::make(-(nxz * mx.x + nyz * my.x + nzz * mz.x), -(nxz * mx.y + nyz * my.y + nzz * mz.y));
     }
     __syncthreads();
-    fft_inverse<T, true>(s, n_lines, 1, n_lines, plan, tw);
+    fft_inverse<T, true, PR>(s, n_lines, 1, n_lines, plan, tw);
     for (int idx = threadIdx.x; idx < a.N * n_lines; idx += blockDim.x) {
         const int l = idx % n_lines, e = idx / n_lines;
         const int b = l % bt, comp = l / bt;
@@ -268,10 +268,27 @@ template <typename K> nm_status set_smem(K kernel, size_t bytes)
 // Largest shared-memory footprint allowed per CTA for these passes
 static const size_t kSmemCap = 200 * 1024;
 
+static bool has_prime_radix(const NmFftPlan &p)
+{
+    for (int s = 0; s < p.n_stages; ++s)
+        if (p.radix[s] == 5 || p.radix[s] == 7) return true;
+    return false;
+}
+
+template <typename T, bool PR> nm_status conv_general(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st);
+
 template <typename T>
 nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
 {
     if (mesh->fast.on) return nm_demag_conv_fast<T>(mesh, fld, Hc_out, st);
+    // lengths 2^a 3^b keep the kernels without the radix-5 / 7 butterflies
+    const bool pr = has_prime_radix(mesh->plan_x) || has_prime_radix(mesh->plan_y) || has_prime_radix(mesh->plan_z);
+    return pr ? conv_general<T, true>(mesh, fld, Hc_out, st) : conv_general<T, false>(mesh, fld, Hc_out, st);
+}
+
+template <typename T, bool PR>
+nm_status conv_general(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
+{
     typedef typename Cx<T>::V V;
     const NmGeom &g = mesh->g;
     V *A = (V *)mesh->bufA, *B = (V *)mesh->bufB;
@@ -287,12 +304,12 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
     {
         NmLaunchScope sc(mesh, NM_K_X_FWD, st);
         if (rx2) {
-            NM_TRY(set_smem(k_x_fwd<T, 2>, smx));
-            k_x_fwd<T, 2><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
+            NM_TRY(set_smem(k_x_fwd<T, 2, PR>, smx));
+            k_x_fwd<T, 2, PR><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
                                                     (const V *)mesh->tw_x, (const V *)mesh->tw_x2, mesh->pos_x);
         } else {
-            NM_TRY(set_smem(k_x_fwd<T, kRowsX>, smx));
-            k_x_fwd<T, kRowsX><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
+            NM_TRY(set_smem(k_x_fwd<T, kRowsX, PR>, smx));
+            k_x_fwd<T, kRowsX, PR><<<gx, kThreads, smx, st>>>(fld, (const T *)mesh->Ms, A, g, mesh->plan_x,
                                                          (const V *)mesh->tw_x, (const V *)mesh->tw_x2, mesh->pos_x);
         }
     }
@@ -311,12 +328,12 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
             nm_set_error("N2 = %d too long for the y pass", g.N2);
             return NM_EUNSUPPORTED;
         }
-        NM_TRY(set_smem(k_lines<T, false>, smy));
-        NM_TRY(set_smem(k_lines<T, true>, smy));
+        NM_TRY(set_smem(k_lines<T, false, PR>, smy));
+        NM_TRY(set_smem(k_lines<T, true, PR>, smy));
         const dim3 gy((g.C1p + bt - 1) / bt, g.N3, 3);
         {
             NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
-            k_lines<T, false><<<gy, kThreads, smy, st>>>(A, B, g, bt, mesh->plan_y, (const V *)mesh->tw_y);
+            k_lines<T, false, PR><<<gy, kThreads, smy, st>>>(A, B, g, bt, mesh->plan_y, (const V *)mesh->tw_y);
         }
 
         ma.comp_stride = (long long)g.N3 * g.P2 * g.C1p;
@@ -343,11 +360,11 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
             nm_set_error("padded length %d too long for the middle pass", ma.P);
             return NM_EUNSUPPORTED;
         }
-        NM_TRY(set_smem(k_mid<T>, smm));
+        NM_TRY(set_smem(k_mid<T, PR>, smm));
         const dim3 gm((g.C1p + bt - 1) / bt, ma.n_fixed);
         {
             NmLaunchScope sc(mesh, NM_K_MID, st);
-            k_mid<T><<<gm, kThreads, smm, st>>>(midbuf, (const T *)mesh->Nhat, g, ma, bt, *mplan, mtw,
+            k_mid<T, PR><<<gm, kThreads, smm, st>>>(midbuf, (const T *)mesh->Nhat, g, ma, bt, *mplan, mtw,
                                                 kline, mesh->kmap_y, mesh->pos_y);
         }
 
@@ -359,19 +376,19 @@ nm_status nm_demag_conv(nm_mesh *mesh, const T *fld, T *Hc_out, cudaStream_t st)
         const dim3 gy((g.C1p + bt - 1) / bt, g.N3, 3);
         {
             NmLaunchScope sc(mesh, NM_K_Y_INV, st);
-            k_lines<T, true><<<gy, kThreads, smy, st>>>(B, A, g, bt, mesh->plan_y, (const V *)mesh->tw_y);
+            k_lines<T, true, PR><<<gy, kThreads, smy, st>>>(B, A, g, bt, mesh->plan_y, (const V *)mesh->tw_y);
         }
 
     }
     {
         NmLaunchScope sc(mesh, NM_K_X_INV, st);
         if (rx2) {
-            NM_TRY(set_smem(k_x_inv<T, 2>, smx));
-            k_x_inv<T, 2><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
+            NM_TRY(set_smem(k_x_inv<T, 2, PR>, smx));
+            k_x_inv<T, 2, PR><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
                                                     (const V *)mesh->tw_x2, mesh->pos_x);
         } else {
-            NM_TRY(set_smem(k_x_inv<T, kRowsX>, smx));
-            k_x_inv<T, kRowsX><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
+            NM_TRY(set_smem(k_x_inv<T, kRowsX, PR>, smx));
+            k_x_inv<T, kRowsX, PR><<<gx, kThreads, smx, st>>>(A, Hc_out, g, mesh->plan_x, (const V *)mesh->tw_x,
                                                          (const V *)mesh->tw_x2, mesh->pos_x);
         }
     }

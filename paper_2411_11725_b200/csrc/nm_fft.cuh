@@ -187,7 +187,9 @@ __device__ __forceinline__ void fft_stage(typename Cx<T>::V *s, int n_lines, int
     }
 }
 
-template <typename T, bool INV, bool LINE_FAST>
+// PR: the transform may contain radix-5 / 7 stages (kernels for 2^a 3^b lengths are compiled without
+// them, so their register allocation does not pay for the prime butterflies).
+template <typename T, bool INV, bool LINE_FAST, bool PR>
 __device__ __forceinline__ void fft_stage_any(int R, typename Cx<T>::V *s, int n_lines,
                                               int line_stride, int elem_stride, int L, int n,
                                               const typename Cx<T>::V *__restrict__ tw)
@@ -196,15 +198,15 @@ __device__ __forceinline__ void fft_stage_any(int R, typename Cx<T>::V *s, int n
     case 2: fft_stage<T, INV, 2, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     case 3: fft_stage<T, INV, 3, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     case 4: fft_stage<T, INV, 4, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
-    case 5: fft_stage<T, INV, 5, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
-    case 7: fft_stage<T, INV, 7, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
+    case 5: if (PR) fft_stage<T, INV, 5, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
+    case 7: if (PR) fft_stage<T, INV, 7, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     default: fft_stage<T, INV, 8, LINE_FAST>(s, n_lines, line_stride, elem_stride, L, n, tw); break;
     }
 }
 
 // Whole transform of n_lines lines in shared memory.  Caller must __syncthreads() before (data
 // visible) — a barrier follows every stage, so results are visible on return.
-template <typename T, bool LINE_FAST>
+template <typename T, bool LINE_FAST, bool PR>
 __device__ __forceinline__ void fft_forward(typename Cx<T>::V *s, int n_lines, int line_stride,
                                             int elem_stride, const NmFftPlan &plan,
                                             const typename Cx<T>::V *__restrict__ tw)
@@ -212,13 +214,13 @@ __device__ __forceinline__ void fft_forward(typename Cx<T>::V *s, int n_lines, i
     int n = plan.L;
     for (int st = 0; st < plan.n_stages; ++st) {
         const int R = plan.radix[st];
-        fft_stage_any<T, false, LINE_FAST>(R, s, n_lines, line_stride, elem_stride, plan.L, n, tw);
+        fft_stage_any<T, false, LINE_FAST, PR>(R, s, n_lines, line_stride, elem_stride, plan.L, n, tw);
         n /= R;
         __syncthreads();
     }
 }
 
-template <typename T, bool LINE_FAST>
+template <typename T, bool LINE_FAST, bool PR>
 __device__ __forceinline__ void fft_inverse(typename Cx<T>::V *s, int n_lines, int line_stride,
                                             int elem_stride, const NmFftPlan &plan,
                                             const typename Cx<T>::V *__restrict__ tw)
@@ -227,7 +229,7 @@ __device__ __forceinline__ void fft_inverse(typename Cx<T>::V *s, int n_lines, i
     for (int st = plan.n_stages - 1; st >= 0; --st) {
         const int R = plan.radix[st];
         n *= R;
-        fft_stage_any<T, true, LINE_FAST>(R, s, n_lines, line_stride, elem_stride, plan.L, n, tw);
+        fft_stage_any<T, true, LINE_FAST, PR>(R, s, n_lines, line_stride, elem_stride, plan.L, n, tw);
         __syncthreads();
     }
 }

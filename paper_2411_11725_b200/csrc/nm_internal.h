@@ -10,6 +10,7 @@
 #include "../../include/nm.h"
 
 #define NM_MAX_STAGES 20
+#define NM_HEXT_BLOCKS 1024
 #define NM_PROF_MAX 4096
 
 // kernel classes reported by nm_profile_end (order = NM_PROF_* of include/nm.h)
@@ -74,7 +75,7 @@ struct NmFast {
 struct NmStepKey {
     int kind, renorm, has_z, pad;   // no implicit padding: keys are compared with memcmp
     double dt, rtol, atol, hu[3];
-    const void *p[3], *hs, *hp;
+    const void *p[4], *hs, *hp;
     unsigned long long epoch;
 };
 struct NmStepGraph {
@@ -111,6 +112,7 @@ struct nm_mesh {
     void *K[7];             // RK stage derivatives (nodal vectors)
     void *Y[2];             // RK stage states
     void *Uc[2];            // cell scalars (adjoint RK)
+    double *hpart;          // partial sums of the uniform-field gradient [3][NM_HEXT_BLOCKS]
     double *partials;       // reduction scratch [node blocks + 1]
     int n_partials;         // capacity
     int last_partials;      // partial sums the last node-kernel launch wrote

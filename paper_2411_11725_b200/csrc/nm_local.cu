@@ -509,6 +509,43 @@ __global__ void k_err_final(double *partials, int n, double count)
     if (threadIdx.x == 0) partials[n] = sqrt(s / count);
 }
 
+// Uniform-field gradient, first pass: per-block fp64 sums of b_n over the nodes with (S Ms)_n > 0.
+template <typename T>
+__global__ void __launch_bounds__(256) k_hext_partial(const T *__restrict__ m, const T *__restrict__ av,
+                                                      const T *__restrict__ sMs, long long nn, T gp, T agp,
+                                                      double *__restrict__ part)
+{
+    double s[3] = {0.0, 0.0, 0.0};
+    for (long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x; n < nn; n += (long long)gridDim.x * blockDim.x) {
+        if (!(sMs[n] > 0)) continue;
+        const T mc[3] = {m[n], m[nn + n], m[2 * nn + n]};
+        const T ac[3] = {av[n], av[nn + n], av[2 * nn + n]};
+        T mxa[3], mxmxa[3];
+        cross3(mc, ac, mxa);
+        cross3(mc, mxa, mxmxa);
+#pragma unroll
+        for (int j = 0; j < 3; ++j) s[j] += (double)(gp * mxa[j] - agp * mxmxa[j]);
+    }
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const double r = block_sum(s[j]);
+        if (threadIdx.x == 0) part[j * gridDim.x + blockIdx.x] = r;
+        __syncthreads();                                    // block_sum's scratch is reused
+    }
+}
+
+// second pass: u_h[j] += coef * (-sum of the block sums), fixed order
+__global__ void k_hext_final(const double *__restrict__ part, int nblocks, double coef, double *__restrict__ u_h)
+{
+    for (int j = 0; j < 3; ++j) {
+        double v = 0.0;
+        for (int i = threadIdx.x; i < nblocks; i += blockDim.x) v += part[j * nblocks + i];
+        const double r = block_sum(v);
+        if (threadIdx.x == 0) u_h[j] += coef * (-r);
+        __syncthreads();
+    }
+}
+
 // Dormand-Prince commit: m <- (normalised) y5 iff err <= 1
 template <typename T>
 __global__ void k_commit(T *__restrict__ m, const T *__restrict__ y5, long long nodes,
@@ -786,6 +823,25 @@ nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaS
 }
 
 template <typename T>
+nm_status nm_launch_hext_grad(nm_mesh *mesh, const T *m, const T *a, double gp, double agp, double coef,
+                              double *u_h, cudaStream_t st)
+{
+    const long long nn = mesh->g.nodes;
+    long long nb = (nn + 255) / 256;
+    if (nb > NM_HEXT_BLOCKS) nb = NM_HEXT_BLOCKS;
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        k_hext_partial<T><<<(unsigned)nb, 256, 0, st>>>(m, a, (const T *)mesh->sMs, nn, (T)gp, (T)agp, mesh->hpart);
+    }
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        k_hext_final<<<1, 256, 0, st>>>(mesh->hpart, (int)nb, coef, u_h);
+    }
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+template <typename T>
 nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st)
 {
     {
@@ -874,6 +930,8 @@ nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st)
 #define NM_INST(T)                                                                                       \
     template nm_status nm_launch_node<T>(nm_mesh *, const NmLocalArgs<T> &, cudaStream_t);              \
     template nm_status nm_launch_commit<T>(nm_mesh *, T *, const T *, const double *, int, cudaStream_t); \
+    template nm_status nm_launch_hext_grad<T>(nm_mesh *, const T *, const T *, double, double, double,  \
+                                              double *, cudaStream_t);                                  \
     template nm_status nm_launch_adj_cell<T>(nm_mesh *, const NmAdjCellArgs<T> &, cudaStream_t);        \
     template nm_status nm_lincomb<T>(nm_mesh *, T *, const T *, int, const T *const *, const T *,       \
                                      long long, long long, cudaStream_t);                               \

@@ -85,6 +85,13 @@ nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaS
 template <typename T>
 nm_status nm_launch_commit(nm_mesh *mesh, T *m, const T *y5, const double *err, int renorm, cudaStream_t st);
 template <typename T> nm_status nm_launch_adj_cell(nm_mesh *mesh, const NmAdjCellArgs<T> &a, cudaStream_t st);
+// u_h[j] += coef * ( - sum over nodes with (S Ms)_n > 0 of b_n[j] ),  b = g' m x a - alpha g' m x (m x a):
+// -(df/dh)^T a for a uniform external field h, accumulated in
+// fp64 in a fixed summation order.
+template <typename T>
+nm_status nm_launch_hext_grad(nm_mesh *mesh, const T *m, const T *a, double gp, double agp, double coef,
+                              double *u_h, cudaStream_t st);
+
 // several independent updates out = base + coef * src in one launch (vec_n > 0: [3][vec_n] arrays,
 // result normalised per node); no update may read what another one writes
 enum { NM_LIN_OPS = 5 };

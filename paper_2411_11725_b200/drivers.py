@@ -46,7 +46,7 @@ def forward_rk4(mesh, m, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
 
 
 def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_every=100, t0=0.0,
-                     objectives_at=None):
+                     objectives_at=None, with_hext=False):
     """Adjoint-state gradient dJ/dMs (Eqs. 27-30; reading C8).
 
     Forward RK4 from m0 with checkpoints, a(T) = aT_of_mT(m(T)) (the caller's dJ/dm(T)), then the
@@ -55,7 +55,11 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
 
     objectives_at = {step index s < n_steps: callable m(t0 + s dt) -> dL_s/dm}: objective terms at
     further times; each is evaluated on the forward pass and added to the adjoint
-    variable when the backward pass arrives at its time (nm_adjoint_add_objective)."""
+    variable when the backward pass arrives at its time (nm_adjoint_add_objective).
+
+    with_hext: also integrate the gradient with respect to a uniform external field h
+    (nm_adjoint_rk4_step_hext; PAPER.md:339-347) and return (m(T), a(0), u(0), u_h(0) = dL/dh as a
+    device fp64 3-vector)."""
     m = m0.clone()
     jumps = {}
     if objectives_at:
@@ -71,10 +75,16 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
     mT = m.clone()
     a = aT_of_mT(mT).clone()
     u = torch.zeros(mesh.cell_shape_abi, dtype=m.dtype, device=m.device)
+    uh = torch.zeros(3, dtype=torch.float64, device=m.device) if with_hext else None
     for s in range(n_steps, 0, -1):
-        mesh.nm_adjoint_rk4_step(t0 + s * dt, dt, m, a, u, zeeman)
+        if with_hext:
+            mesh.nm_adjoint_rk4_step_hext(t0 + s * dt, dt, m, a, u, uh, zeeman)
+        else:
+            mesh.nm_adjoint_rk4_step(t0 + s * dt, dt, m, a, u, zeeman)
         if (s - 1) in ck:
             m.copy_(ck[s - 1])
         if (s - 1) in jumps:
             mesh.nm_adjoint_add_objective(a, jumps[s - 1])
+    if with_hext:
+        return mT, a, u, uh
     return mT, a, u

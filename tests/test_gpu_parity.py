@@ -377,6 +377,70 @@ def test_adjoint_gradient_objectives_at_several_times(prec):
     assert e.value.status == nm.NM_EINVAL
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_hext_gradient_rhs_and_backward_pass(prec):
+    """Gradient with respect to a uniform external field: nm_llg_adjoint_rhs_hext
+    against oracle adjoint_rhs_hext on a ragged all-terms mesh with a vacuum block (several reduction
+    blocks), and u_h(0) of drivers.adjoint_gradient(with_hext=True) against the oracle's backward pass
+    on a film with anisotropy and a uniform field."""
+    from oracle import adjoint
+    from paper_2411_11725_b200 import drivers
+    td = DT[prec]
+    nd = np_dtype(td)
+    # (1) single right-hand side
+    w, hs = wl.varied_case((24, 12, 6), vacuum=True)
+    p = oracle_problem(w, nd)
+    m = _m0(w, td)
+    a = wl.round_to(np.random.default_rng(31).standard_normal(m.shape), nd)
+    ref = adjoint.adjoint_rhs_hext(p, 0.0, m, a)
+    mesh = gpu_mesh(w, td)
+    got = mesh.nm_llg_adjoint_rhs_hext(dev(m, td), dev(a, td)).cpu().numpy()
+    # a sum of nodes of mixed sign: error relative to the sum of magnitudes, not to the result
+    scale = p.gamma * np.sum(np.abs(a))
+    assert np.max(np.abs(got - ref)) <= (1e-13 if prec == "f64" else 1e-6) * scale
+    assert np.max(np.abs(got - ref)) <= (1e-11 if prec == "f64" else 1e-4) * np.max(np.abs(ref))
+    # a mesh without the Zeeman term does not depend on h
+    w0 = wl.config4_sweep(16)
+    assert torch.all(gpu_mesh(w0, td).nm_llg_adjoint_rhs_hext(dev(_m0(w0, td), td), dev(_m0(w0, td), td)) == 0)
+    # (2) backward integration
+    w = wl.config5_inverse((32, 8, 1), n_steps=30)
+    w.terms = wl.TERM_EXCHANGE | wl.TERM_DEMAG | wl.TERM_ANISO | wl.TERM_ZEEMAN
+    w.Ku = 2e4
+    w.ku_axis = (0.0, 0.6, 0.8)
+    w.h_uniform = (1e3, 2e3, -1.5e3)
+    p = oracle_problem(w, nd)
+    z = oracle_zeeman(w, nd)
+    m0 = _m0(w, td)
+    wT = wl.round_to(wl.objective_weights(w), nd)
+    mT_ref, ck = adjoint.forward_rk4(p, m0, w.dt, w.n_steps, z, checkpoint_every=10)
+    _, a0_ref, u0_ref, uh_ref = adjoint.backward_rk4(p, mT_ref, wT, w.dt, w.n_steps, z, checkpoints=ck,
+                                                     with_hext=True)
+    assert np.max(np.abs(uh_ref)) > 0
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    gT = dev(wT, td)
+    out = {}
+    for graph in ("0", "1"):
+        import os
+        old = os.environ.get("NM_GRAPH")
+        os.environ["NM_GRAPH"] = graph
+        try:
+            mesh = gpu_mesh(w, td)
+        finally:
+            if old is None:
+                os.environ.pop("NM_GRAPH", None)
+            else:
+                os.environ["NM_GRAPH"] = old
+        mT, a0, u0, uh = drivers.adjoint_gradient(mesh, dev(m0, td), lambda m_: gT, w.dt, w.n_steps, gz,
+                                                  checkpoint_every=10, with_hext=True)
+        out[graph] = (a0.clone(), u0.clone(), uh.clone())
+        assert rel_l2(host(a0), a0_ref) <= (1e-11 if prec == "f64" else 1e-5)
+        assert rel_l2(wl.from_abi(u0.cpu().double().numpy()), u0_ref) <= (1e-11 if prec == "f64" else 2e-4)
+        assert rel_l2(uh.cpu().numpy(), uh_ref) <= (1e-11 if prec == "f64" else 2e-4)
+    for x, y in zip(out["0"], out["1"]):                # replayed steps accumulate u_h identically
+        assert torch.equal(x, y)
+
+
 # ---- boundary behaviour --------------------------------------------------------------------------
 def test_errors_are_statuses_not_crashes():
     from paper_2411_11725_b200 import binding as nm

@@ -147,7 +147,7 @@ def test_objectives_at_several_times_against_finite_differences():
     m0 = 0.1 * rng.standard_normal((3,) + p.node_shape)
     m0[0] += 1
     m0 /= np.sqrt(np.sum(m0 * m0, axis=0))
-    dt, nst, s1, s2 = 5e-14, 120, 40, 90
+    dt, nst, s1, s2 = 5e-14, 72, 24, 54
     w1, w2, wT = (rng.standard_normal(m0.shape) for _ in range(3))
 
     def traj(prob):
@@ -162,7 +162,7 @@ def test_objectives_at_several_times_against_finite_differences():
         a, b, c = traj(prob)
         return float(np.sum(w1 * a) + np.sum(w2 * b) + np.sum(wT * c))
 
-    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=30)
+    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=18)
     _, _, u0 = adjoint.backward_rk4(p, mT, wT, dt, nst, zee, checkpoints=ck, a_jumps={s1: w1, s2: w2})
     for c in [(0, 0, 0), (3, 1, 0), (5, 0, 0)]:
         h = 1e-4 * p.Ms[c]
@@ -176,13 +176,67 @@ def test_objectives_at_several_times_against_finite_differences():
     # starts from the exact m(T_i), the joint run arrives there by inverse integration)
     total = np.zeros_like(u0)
     for steps, w in ((s1, w1), (s2, w2), (nst, wT)):
-        mS, ckS = adjoint.forward_rk4(p, m0, dt, steps, zee, checkpoint_every=30)
+        mS, ckS = adjoint.forward_rk4(p, m0, dt, steps, zee, checkpoint_every=18)
         total += adjoint.backward_rk4(p, mS, w, dt, steps, zee, checkpoints=ckS)[2]
     assert np.abs(total - u0).max() < 1e-6 * np.abs(u0).max()
     # a jump of zero is no jump
     _, _, u_plain = adjoint.backward_rk4(p, mT, wT, dt, nst, zee, checkpoints=ck)
     _, _, u_zero = adjoint.backward_rk4(p, mT, wT, dt, nst, zee, checkpoints=ck, a_jumps={s1: 0.0 * w1})
     assert np.array_equal(u_plain, u_zero)
+
+
+def test_hext_vjp_against_finite_differences():
+    """adjoint_rhs_hext: a . (df/dh) e_j by central differences of the forward RHS in a uniform field
+    h added to a nodal H_ext, on a mesh with a vacuum corner (nodes with L = 0 see no field)."""
+    p, zee = make((3, 2, 2), seed=3)
+    Ms = p.Ms.copy()
+    Ms[0, 0, :] = 0.0
+    Ms[0, 1, 0] = 0.0
+    p = with_Ms(p, Ms)
+    assert np.any(p.L == 0) and np.any(p.L > 0)
+    m = rand_unit(p.node_shape, 4)
+    a = np.random.default_rng(5).standard_normal(m.shape)
+    base = zee(0.0)
+    got = adjoint.adjoint_rhs_hext(p, 0.0, m, a)
+    for j in range(3):
+        e = np.zeros((3, 1, 1, 1))
+        e[j] = 1.0
+        eps = 10.0
+        fp = llg.llg_rhs(p, 0.0, m, lambda t: base + eps * e)
+        fm = llg.llg_rhs(p, 0.0, m, lambda t: base - eps * e)
+        fd = -np.sum(a * (fp - fm)) / (2 * eps)
+        assert abs(got[j] - fd) <= 1e-9 * np.abs(got).max(), (j, got[j], fd)
+    # no Zeeman term: no dependence on h
+    p0 = Problem(p.n_cells, p.dx, p.Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha, TERM_EXCHANGE | TERM_DEMAG, p._Nt)
+    assert np.all(adjoint.adjoint_rhs_hext(p0, 0.0, m, a) == 0.0)
+
+
+def test_hext_gradient_of_a_trajectory_against_finite_differences():
+    """dL/dh of L = w . m(T) for a uniform external field h (the design variable behind the field
+    angles of Eqs. 31-33): u_h(0) of the backward pass vs central differences of the forward solve."""
+    rng = np.random.default_rng(27)
+    n, dx = (6, 2, 1), (4e-9, 4e-9, 5e-9)
+    p = Problem(n, dx, rng.uniform(1e5, 1.5e5, n), np.full(n, 3.65e-12), np.full(n, 2e4), ku_axis=(0.0, 0.6, 0.8),
+                alpha=0.05, terms=ALL)
+    p.Nt
+    h0 = np.array([1e3, 2e3, -1.5e3])
+    m0 = 0.1 * rng.standard_normal((3,) + p.node_shape)
+    m0[0] += 1
+    m0 /= np.sqrt(np.sum(m0 * m0, axis=0))
+    w = rng.standard_normal(m0.shape)
+    dt, nst = 5e-14, 80
+    zee = lambda t: h0
+    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=40)
+    _, _, u0, uh = adjoint.backward_rk4(p, mT, w, dt, nst, zee, checkpoints=ck, with_hext=True)
+    _, _, u0_plain = adjoint.backward_rk4(p, mT, w, dt, nst, zee, checkpoints=ck)
+    assert np.array_equal(u0, u0_plain)
+    for j in range(3):
+        e = np.zeros(3)
+        e[j] = 20.0
+        Jp = float(np.sum(w * adjoint.forward_rk4(p, m0, dt, nst, lambda t: h0 + e)[0]))
+        Jm = float(np.sum(w * adjoint.forward_rk4(p, m0, dt, nst, lambda t: h0 - e)[0]))
+        fd = (Jp - Jm) / 40.0
+        assert abs(uh[j] - fd) < 1e-3 * np.abs(uh).max(), (j, uh[j], fd)
 
 
 def test_adjoint_driver_zero_and_linearity():

@@ -769,6 +769,12 @@ template <typename F>
 nm_status run_step(nm_mesh *m, int slot, const nm_zeeman *z, NmStepKey key, cudaStream_t st, F issue)
 {
     if (!m->graph_on || m->prof_on || (z && z->amp)) return issue(st);
+    {
+        // the caller is capturing this stream into a graph of their own: plain launches go into it
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); return issue(st); }
+        if (cs != cudaStreamCaptureStatusNone) return issue(st);
+    }
     key.kind = slot;
     key.epoch = m->graph_epoch;
     key.has_z = z != nullptr;

@@ -152,3 +152,34 @@ def test_adjoint_rk4_replay_bit_identical_and_set_Ms_fp64():
     _, a0_ref, u0_ref = adjoint.backward_rk4(p, mT_ref, aT, w.dt, w.n_steps, z, checkpoints=None)
     assert rel_l2(host(out[True][2]), a0_ref) <= 1e-11
     assert rel_l2(wl.from_abi(out[True][3].cpu().numpy()), u0_ref) <= 1e-11
+
+
+def test_steps_inside_a_graph_the_caller_captures():
+    """A caller that captures its own CUDA graph (here: torch.cuda.graph) around nm_rk_step gets plain
+    launches recorded into that graph: the library neither starts a capture of its own nor launches
+    its cached step while the caller's stream is capturing, and replaying the caller's graph
+    advances the state like the steps themselves."""
+    td = torch.float64
+    w, hs = _case((12, 6, 4))
+    mesh = _mesh(w, td, True)
+    gz = gpu_zeeman(w, td, h_static=hs)
+    y = dev(_m0(w, td), td)
+    mesh.nm_rk_step(0, 0.0, w.dt, y, gz)                # these arguments have been seen once
+    want = y.clone()
+    for _ in range(4):
+        mesh.nm_rk_step(0, 0.0, w.dt, want, gz)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        mesh.nm_rk_step(0, 0.0, w.dt, y, gz)            # would be the library's own capture
+        mesh.nm_rk_step(0, 0.0, w.dt, y, gz)
+    g.replay()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(y, want)
+    mesh.nm_rk_step(0, 0.0, w.dt, y, gz)                # and the library's replay still works afterwards
+    mesh.nm_rk_step(0, 0.0, w.dt, y, gz)
+    for _ in range(2):
+        mesh.nm_rk_step(0, 0.0, w.dt, want, gz)
+    assert torch.equal(y, want)
+    mesh.close()

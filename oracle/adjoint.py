@@ -98,6 +98,35 @@ def adjoint_rhs_hext(p, t, m, a):
     return -np.array([np.sum(b[j][inside]) for j in range(3)])
 
 
+def adjoint_rhs_materials(p, t, m, a):
+    """(-(df/dA)^T a, -(df/dKu)^T a), cell-wise (design variables A_c, Ku_c).
+
+    A and Ku enter f only through H = -dE/L with L independent of both (Eq. 22), and dE is linear
+    in them (Eqs. 19-20; oracle/local_fields.py):
+        dE_{c+i} += 2 A_c sum_i' K[i,i'] m_{c+i'}            - 2 Ku_c sum_i' M[i,i'] (m_{c+i'}.k) k
+    so with b = (df/dH)^T a = g' m x a - alpha g' m x (m x a) and bL = b / L (0 where L = 0)
+        (df/dA_c)^T a  = -2 sum_{i,i'} K[i,i'] bL_{c+i} . m_{c+i'}
+        (df/dKu_c)^T a = +2 sum_{i,i'} M[i,i'] (bL_{c+i}.k) (m_{c+i'}.k)
+    Terms that are off contribute zero."""
+    gp = p.gamma / (1.0 + p.alpha ** 2)
+    mxa = _llg.cross(m, a)
+    b = gp * mxa - p.alpha * gp * _llg.cross(m, mxa)
+    bL = _safe_div(b, p.L)
+    K, M = element_matrices(p.dx)
+    k = np.asarray(p.ku_axis, dtype=np.float64)
+    bk = k[0] * bL[0] + k[1] * bL[1] + k[2] * bL[2]
+    mk = k[0] * m[0] + k[1] * m[1] + k[2] * m[2]
+    gA = np.zeros(p.n_cells)
+    gKu = np.zeros(p.n_cells)
+    for i in LOCAL:
+        for ip in LOCAL:
+            if p.terms & _llg.TERM_EXCHANGE:
+                gA += -2.0 * K[i + ip] * np.sum(node_view(bL, i) * node_view(m, ip), axis=0)
+            if p.terms & _llg.TERM_ANISO:
+                gKu += 2.0 * M[i + ip] * node_view(bk, i) * node_view(mk, ip)
+    return -gA, -gKu
+
+
 def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
     """Fixed-step RK4 with renormalisation; returns (m_T, {step index: m}) (C8)."""
     m = m0.copy()
@@ -110,7 +139,7 @@ def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
 
 
 def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, a_jumps=None,
-                 with_hext=False):
+                 with_hext=False, with_materials=False):
     """Integrate Eq. (29) from T = t0 + n_steps dt back to t0 with RK4 steps of -dt.
 
     State (m, a, u); m is renormalised after every step and replaced by the stored forward
@@ -125,6 +154,8 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
 
     with_hext: also integrate du_h/dt = -(df/dh)^T a (adjoint_rhs_hext) with u_h(T) = 0 and return
     (m0, a0, u0, u_h(0)); u_h(0) = dL/dh for a uniform external field h.
+    with_materials: also integrate (u_A, u_Ku) with adjoint_rhs_materials and append
+    (u_A(0), u_Ku(0)) = (dL/dA, dL/dKu) per cell to the returned tuple.
     """
     m, a = mT.copy(), aT.copy()
     u = np.zeros(p.n_cells)
@@ -134,7 +165,10 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
 
     def F(t, m_, a_):
         r = adjoint_rhs(p, t, m_, a_, zeeman)
-        return r + (adjoint_rhs_hext(p, t, m_, a_),) if with_hext else r
+        return r + (adjoint_rhs_hext(p, t, m_, a_) if with_hext else None,) + \
+            (adjoint_rhs_materials(p, t, m_, a_) if with_materials else (None, None))
+    uA = np.zeros(p.n_cells)
+    uKu = np.zeros(p.n_cells)
 
     for s in range(n_steps, 0, -1):
         t = t0 + s * dt
@@ -147,10 +181,12 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
         u = u + h / 6.0 * (k1[2] + 2 * k2[2] + 2 * k3[2] + k4[2])
         if with_hext:
             uh = uh + h / 6.0 * (k1[3] + 2 * k2[3] + 2 * k3[3] + k4[3])
+        if with_materials:
+            uA = uA + h / 6.0 * (k1[4] + 2 * k2[4] + 2 * k3[4] + k4[4])
+            uKu = uKu + h / 6.0 * (k1[5] + 2 * k2[5] + 2 * k3[5] + k4[5])
         if checkpoints is not None and (s - 1) in checkpoints:
             m = checkpoints[s - 1].copy()
         if a_jumps is not None and (s - 1) in a_jumps:
             a = a + a_jumps[s - 1]
-    if with_hext:
-        return m, a, u, uh
-    return m, a, u
+    out = (m, a, u) + ((uh,) if with_hext else ())
+    return out + ((uA, uKu) if with_materials else ())

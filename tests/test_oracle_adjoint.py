@@ -239,6 +239,71 @@ def test_hext_gradient_of_a_trajectory_against_finite_differences():
         assert abs(uh[j] - fd) < 1e-3 * np.abs(uh).max(), (j, uh[j], fd)
 
 
+def with_A_Ku(p, A, Ku):
+    return Problem(p.n_cells, p.dx, p.Ms, A, Ku, p.ku_axis, p.gamma, p.alpha, p.terms, p._Nt)
+
+
+def test_materials_vjp_against_finite_differences():
+    """adjoint_rhs_materials: a . (df/dA_c), a . (df/dKu_c) for every cell of a 3x2x2 mesh with a
+    vacuum corner by central differences of the forward RHS (f is linear in A and Ku)."""
+    p, zee = make((3, 2, 2), seed=13)
+    Ms = p.Ms.copy()
+    Ms[0, 0, :] = 0.0
+    p = with_Ms(p, Ms)
+    m = rand_unit(p.node_shape, 14)
+    a = np.random.default_rng(15).standard_normal(m.shape)
+    gA, gKu = adjoint.adjoint_rhs_materials(p, 0.0, m, a)
+    for c in np.ndindex(*p.n_cells):
+        for which, got in (("A", gA), ("Ku", gKu)):
+            base = p.A if which == "A" else p.Ku
+            h = 0.1 * base[c]
+            up, dn = base.copy(), base.copy()
+            up[c] += h
+            dn[c] -= h
+            pp = with_A_Ku(p, up, p.Ku) if which == "A" else with_A_Ku(p, p.A, up)
+            pm = with_A_Ku(p, dn, p.Ku) if which == "A" else with_A_Ku(p, p.A, dn)
+            fd = -np.sum(a * (llg.llg_rhs(pp, 0.0, m, zee) - llg.llg_rhs(pm, 0.0, m, zee))) / (2 * h)
+            assert abs(got[c] - fd) <= 1e-9 * np.abs(got).max(), (which, c, got[c], fd)
+    assert np.abs(gA).max() > 0 and np.abs(gKu).max() > 0
+    # terms that are off do not depend on their coefficient
+    p0 = Problem(p.n_cells, p.dx, p.Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha, TERM_DEMAG | TERM_ZEEMAN, p._Nt)
+    g0 = adjoint.adjoint_rhs_materials(p0, 0.0, m, a)
+    assert np.all(g0[0] == 0.0) and np.all(g0[1] == 0.0)
+
+
+def test_materials_gradient_of_a_trajectory_against_finite_differences():
+    """dL/dA_c and dL/dKu_c of L = w . m(T): (u_A, u_Ku)(0) of the backward pass vs central
+    differences of the forward solve on three cells."""
+    rng = np.random.default_rng(37)
+    n, dx = (6, 2, 1), (4e-9, 4e-9, 5e-9)
+    p = Problem(n, dx, rng.uniform(1e5, 1.5e5, n), rng.uniform(3e-12, 4e-12, n), rng.uniform(1e4, 3e4, n),
+                ku_axis=(0.0, 0.6, 0.8), alpha=0.05, terms=ALL)
+    p.Nt
+    zee = lambda t: np.array([1e3, 2e3, -1.5e3])
+    m0 = 0.3 * rng.standard_normal((3,) + p.node_shape)
+    m0[0] += 1
+    m0 /= np.sqrt(np.sum(m0 * m0, axis=0))
+    w = rng.standard_normal(m0.shape)
+    dt, nst = 5e-14, 50
+    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=25)
+    out = adjoint.backward_rk4(p, mT, w, dt, nst, zee, checkpoints=ck, with_hext=True, with_materials=True)
+    assert len(out) == 6
+    uA, uKu = out[4], out[5]
+    plain = adjoint.backward_rk4(p, mT, w, dt, nst, zee, checkpoints=ck)
+    assert np.array_equal(out[2], plain[2]) and np.array_equal(out[1], plain[1])
+    J = lambda prob: float(np.sum(w * adjoint.forward_rk4(prob, m0, dt, nst, zee)[0]))
+    for c in [(0, 0, 0), (3, 1, 0), (5, 0, 0)]:
+        for which, got, base in (("A", uA, p.A), ("Ku", uKu, p.Ku)):
+            h = 1e-3 * base[c]
+            up, dn = base.copy(), base.copy()
+            up[c] += h
+            dn[c] -= h
+            pp = with_A_Ku(p, up, p.Ku) if which == "A" else with_A_Ku(p, p.A, up)
+            pm = with_A_Ku(p, dn, p.Ku) if which == "A" else with_A_Ku(p, p.A, dn)
+            fd = (J(pp) - J(pm)) / (2 * h)
+            assert abs(got[c] - fd) < 2e-3 * np.abs(got).max(), (which, c, got[c], fd)
+
+
 def test_adjoint_driver_zero_and_linearity():
     rng = np.random.default_rng(8)
     n, dx = (4, 2, 1), (4e-9, 4e-9, 5e-9)

@@ -166,6 +166,27 @@ nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt, void *m_i
                                    void *u_inout, double *u_h_inout, const nm_zeeman *zeeman,
                                    int renormalise, void *stream);
 
+/* Gradients with respect to the cell-wise exchange constant A_c and anisotropy constant Ku_c (design
+ * variables beside Ms).  f depends on them through H = -dE/L only, dE linear in
+ * both (Eqs. 19-20, 22), so with b as above and bL = b / L (0 at nodes with L_n = 0), K and M the
+ * element matrices of Eq. (12):
+ *   -(df/dA_c)^T a  = +2 sum_{i,i'} K[i,i'] bL_{c+i} . m_{c+i'}
+ *   -(df/dKu_c)^T a = -2 sum_{i,i'} M[i,i'] (bL_{c+i}.k) (m_{c+i'}.k)
+ * (zero for a term the mesh does not have).  Outputs are DEVICE cell arrays [N3][N2][N1] of the mesh
+ * dtype; either may be NULL.
+ *   nm_llg_adjoint_rhs_materials: the two right-hand sides for the given m, a.
+ *   nm_adjoint_rk4_step_ex: nm_adjoint_rk4_step that also integrates the accumulators named in
+ *   `extra` backwards (any of them NULL = not wanted); with u_X(T) = 0, u_X(0) = dL/dX. */
+typedef struct {
+    void *u_A, *u_Ku;     /* device cell arrays, mesh dtype, in/out */
+    double *u_h;          /* device fp64 [3], in/out (uniform external field, see above) */
+} nm_adjoint_extra;
+nm_status nm_llg_adjoint_rhs_materials(nm_mesh *mesh, const void *m, const void *a, void *dudt_A_out,
+                                       void *dudt_Ku_out, void *stream);
+nm_status nm_adjoint_rk4_step_ex(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                                 void *u_inout, const nm_adjoint_extra *extra, const nm_zeeman *zeeman,
+                                 int renormalise, void *stream);
+
 /* Objectives at several times T_i ("adding appropriate terms depending on m(T_i)"):
  * when the backward integration of Eq. (29) arrives at T_i the adjoint variable takes the jump
  *   a_inout <- a_inout + scale * dLdm     (device nodal 3-vectors of the mesh dtype),

@@ -720,9 +720,39 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
     return NM_OK;
 }
 
+// VJPs with respect to the cell-wise A and Ku for the state (mm, av): write (accumulate == 0) or
+// u_X += coef g_X.
 template <typename T>
-nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, double *uh, const nm_zeeman *z,
-                      int renorm, cudaStream_t st)
+nm_status mat_grad(nm_mesh *m, const T *mm, const T *av, T *uA, T *uKu, double coef, int accumulate,
+                   cudaStream_t st)
+{
+    if (!uA && !uKu) return NM_OK;
+    NmLocalArgs<T> la;
+    base_args<T>(m, 0.0, nullptr, m->desc.terms, &la);
+    NmMatGradArgs<T> g;
+    memset(&g, 0, sizeof(g));
+    g.g = m->g;
+    g.m = mm;
+    g.a = av;
+    g.sMs = (const T *)m->sMs;
+    g.u_A = uA;
+    g.u_Ku = uKu;
+    for (int e = 0; e < 8; ++e) { g.wK[e] = la.wK[e]; g.wM[e] = la.wM[e]; }
+    for (int j = 0; j < 3; ++j) g.kax[j] = la.kax[j];
+    g.gp = la.gp;
+    g.agp = la.agp;
+    const double V = m->desc.cell_size[0] * m->desc.cell_size[1] * m->desc.cell_size[2];
+    g.invL = (T)(8.0 / (NM_MU0 * V));
+    g.coef = (T)coef;
+    g.accumulate = accumulate;
+    g.ex_on = (m->desc.terms & NM_TERM_EXCHANGE) != 0;
+    g.an_on = (m->desc.terms & NM_TERM_ANISO) != 0;
+    return nm_launch_mat_grad<T>(m, g, st);
+}
+
+template <typename T>
+nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, double *uh, T *uA, T *uKu,
+                      const nm_zeeman *z, int renorm, cudaStream_t st)
 {
     const double gp_h = m->desc.gamma / (1.0 + m->desc.alpha * m->desc.alpha);
     const bool want_h = uh && (m->desc.terms & NM_TERM_ZEEMAN);
@@ -739,6 +769,7 @@ nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, doubl
         NM_TRY(adjoint_eval<T>(m, ts[s], sm, sa, z, F, DA, DU, st));
         // u_h += w_s (-(df/dh)^T a) of this stage (reads the stage state before it is overwritten)
         if (want_h) NM_TRY(nm_launch_hext_grad<T>(m, sm, sa, gp_h, m->desc.alpha * gp_h, w[s], uh, st));
+        NM_TRY(mat_grad<T>(m, sm, sa, uA, uKu, w[s], 1, st));
         const T ws = (T)w[s];
         if (s < 3) {
             // accumulators (the first stage starts them from the state) and the next stage state
@@ -908,7 +939,8 @@ extern "C" nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, 
 
 namespace {
 nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout, void *u_inout,
-                            double *u_h_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
+                            double *u_h_inout, void *u_A, void *u_Ku, const nm_zeeman *zeeman, int renormalise,
+                            void *stream)
 {
     NM_TRY(check_call(mesh, m_inout, a_inout));
     if (!u_inout) { nm_set_error("u_inout is NULL"); return NM_EINVAL; }
@@ -921,11 +953,15 @@ nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, v
     key.p[1] = a_inout;
     key.p[2] = u_inout;
     key.p[3] = u_h_inout;
+    key.p[4] = u_A;
+    key.p[5] = u_Ku;
     return run_step(mesh, NM_GRAPH_ADJ_RK4, zeeman, key, st, [&](cudaStream_t s) {
         return mesh->f64 ? adjoint_rk4<double>(mesh, t, dt, (double *)m_inout, (double *)a_inout,
-                                               (double *)u_inout, u_h_inout, zeeman, renormalise, s)
+                                               (double *)u_inout, u_h_inout, (double *)u_A, (double *)u_Ku,
+                                               zeeman, renormalise, s)
                          : adjoint_rk4<float>(mesh, t, dt, (float *)m_inout, (float *)a_inout,
-                                              (float *)u_inout, u_h_inout, zeeman, renormalise, s);
+                                              (float *)u_inout, u_h_inout, (float *)u_A, (float *)u_Ku,
+                                              zeeman, renormalise, s);
     });
 }
 } // namespace
@@ -933,7 +969,8 @@ nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, v
 extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
                                          void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
 {
-    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, nullptr, zeeman, renormalise, stream);
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, nullptr, nullptr, nullptr, zeeman,
+                             renormalise, stream);
 }
 
 extern "C" nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
@@ -941,7 +978,29 @@ extern "C" nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt
                                               int renormalise, void *stream)
 {
     if (!u_h_inout) { nm_set_error("u_h_inout is NULL"); return NM_EINVAL; }
-    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, u_h_inout, zeeman, renormalise, stream);
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, u_h_inout, nullptr, nullptr, zeeman,
+                             renormalise, stream);
+}
+
+extern "C" nm_status nm_adjoint_rk4_step_ex(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
+                                            void *u_inout, const nm_adjoint_extra *extra,
+                                            const nm_zeeman *zeeman, int renormalise, void *stream)
+{
+    if (!extra) { nm_set_error("extra is NULL"); return NM_EINVAL; }
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, extra->u_h, extra->u_A, extra->u_Ku,
+                             zeeman, renormalise, stream);
+}
+
+extern "C" nm_status nm_llg_adjoint_rhs_materials(nm_mesh *mesh, const void *m, const void *a, void *dudt_A_out,
+                                                  void *dudt_Ku_out, void *stream)
+{
+    NM_TRY(check_call(mesh, m, a));
+    if (!dudt_A_out && !dudt_Ku_out) { nm_set_error("both outputs are NULL"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    return mesh->f64 ? mat_grad<double>(mesh, (const double *)m, (const double *)a, (double *)dudt_A_out,
+                                        (double *)dudt_Ku_out, 1.0, 0, st)
+                     : mat_grad<float>(mesh, (const float *)m, (const float *)a, (float *)dudt_A_out,
+                                       (float *)dudt_Ku_out, 1.0, 0, st);
 }
 
 extern "C" nm_status nm_llg_adjoint_rhs_hext(nm_mesh *mesh, const void *m, const void *a, double *dudt_h_out,

@@ -546,6 +546,50 @@ __global__ void k_hext_final(const double *__restrict__ part, int nblocks, doubl
     }
 }
 
+// VJPs with respect to the cell-wise A and Ku: one thread per cell gathers m, a and S Ms of its 8 vertices.
+template <typename T> __global__ void __launch_bounds__(128) k_mat_grad(const NmMatGradArgs<T> a)
+{
+    const NmGeom &g = a.g;
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= g.cells) return;
+    const int c1 = (int)(c % g.N1), c2 = (int)((c / g.N1) % g.N2), c3 = (int)(c / ((long long)g.N1 * g.N2));
+    const long long nn = g.nodes;
+    T mv[8][3], bl[8][3], mk[8], bk[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const long long n = ((long long)(c3 + ((i >> 2) & 1)) * g.n2 + (c2 + ((i >> 1) & 1))) * g.n1 + (c1 + (i & 1));
+        const T mc[3] = {a.m[n], a.m[nn + n], a.m[2 * nn + n]};
+        const T ac[3] = {a.a[n], a.a[nn + n], a.a[2 * nn + n]};
+        const T sms = a.sMs[n];
+        const T il = sms > 0 ? a.invL / sms : (T)0;
+        T mxa[3], mxmxa[3];
+        cross3(mc, ac, mxa);
+        cross3(mc, mxa, mxmxa);
+        mk[i] = 0;
+        bk[i] = 0;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            mv[i][j] = mc[j];
+            bl[i][j] = (a.gp * mxa[j] - a.agp * mxmxa[j]) * il;
+            mk[i] += mc[j] * a.kax[j];
+            bk[i] += bl[i][j] * a.kax[j];
+        }
+    }
+    T gA = 0, gKu = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int ip = 0; ip < 8; ++ip) {
+            const int e = i ^ ip;
+            gA += a.wK[e] * (bl[i][0] * mv[ip][0] + bl[i][1] * mv[ip][1] + bl[i][2] * mv[ip][2]);
+            gKu += a.wM[e] * bk[i] * mk[ip];
+        }
+    gA = a.ex_on ? (T)2 * gA : (T)0;
+    gKu = a.an_on ? (T)-2 * gKu : (T)0;
+    if (a.u_A) a.u_A[c] = a.accumulate ? a.u_A[c] + a.coef * gA : gA;
+    if (a.u_Ku) a.u_Ku[c] = a.accumulate ? a.u_Ku[c] + a.coef * gKu : gKu;
+}
+
 // Dormand-Prince commit: m <- (normalised) y5 iff err <= 1
 template <typename T>
 __global__ void k_commit(T *__restrict__ m, const T *__restrict__ y5, long long nodes,
@@ -822,6 +866,16 @@ nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaS
     return NM_OK;
 }
 
+template <typename T> nm_status nm_launch_mat_grad(nm_mesh *mesh, const NmMatGradArgs<T> &a, cudaStream_t st)
+{
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        k_mat_grad<T><<<nblk(a.g.cells, 128), 128, 0, st>>>(a);
+    }
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
 template <typename T>
 nm_status nm_launch_hext_grad(nm_mesh *mesh, const T *m, const T *a, double gp, double agp, double coef,
                               double *u_h, cudaStream_t st)
@@ -930,6 +984,7 @@ nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st)
 #define NM_INST(T)                                                                                       \
     template nm_status nm_launch_node<T>(nm_mesh *, const NmLocalArgs<T> &, cudaStream_t);              \
     template nm_status nm_launch_commit<T>(nm_mesh *, T *, const T *, const double *, int, cudaStream_t); \
+    template nm_status nm_launch_mat_grad<T>(nm_mesh *, const NmMatGradArgs<T> &, cudaStream_t);        \
     template nm_status nm_launch_hext_grad<T>(nm_mesh *, const T *, const T *, double, double, double,  \
                                               double *, cudaStream_t);                                  \
     template nm_status nm_launch_adj_cell<T>(nm_mesh *, const NmAdjCellArgs<T> &, cudaStream_t);        \

@@ -92,6 +92,22 @@ template <typename T>
 nm_status nm_launch_hext_grad(nm_mesh *mesh, const T *m, const T *a, double gp, double agp, double coef,
                               double *u_h, cudaStream_t st);
 
+// Cell-wise VJPs with respect to A_c and Ku_c, b = g' m x a - alpha g' m x (m x a),
+// bL = b / L (0 where (S Ms)_n = 0), the element matrices K, M of Eq. (12) by vertex difference pattern:
+//   gA_c  = +2 sum_{i,i'} K[i,i'] bL_{c+i} . m_{c+i'}           = -(df/dA_c)^T a
+//   gKu_c = -2 sum_{i,i'} M[i,i'] (bL_{c+i}.k) (m_{c+i'}.k)     = -(df/dKu_c)^T a
+// accumulate == 0: u_X = gX; else u_X += coef gX.  u_A / u_Ku may be null; a term that is off gives 0.
+template <typename T> struct NmMatGradArgs {
+    NmGeom g;
+    const T *m, *a, *sMs;
+    T *u_A, *u_Ku;
+    T wK[8], wM[8], kax[3];
+    T gp, agp, invL;        // invL = 8 / (mu0 V): bL = b invL / (S Ms)
+    T coef;
+    int accumulate, ex_on, an_on;
+};
+template <typename T> nm_status nm_launch_mat_grad(nm_mesh *mesh, const NmMatGradArgs<T> &a, cudaStream_t st);
+
 // several independent updates out = base + coef * src in one launch (vec_n > 0: [3][vec_n] arrays,
 // result normalised per node); no update may read what another one writes
 enum { NM_LIN_OPS = 5 };

@@ -46,7 +46,7 @@ def forward_rk4(mesh, m, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
 
 
 def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_every=100, t0=0.0,
-                     objectives_at=None, with_hext=False):
+                     objectives_at=None, with_hext=False, with_materials=False):
     """Adjoint-state gradient dJ/dMs (Eqs. 27-30; reading C8).
 
     Forward RK4 from m0 with checkpoints, a(T) = aT_of_mT(m(T)) (the caller's dJ/dm(T)), then the
@@ -59,7 +59,9 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
 
     with_hext: also integrate the gradient with respect to a uniform external field h
     (nm_adjoint_rk4_step_hext; PAPER.md:339-347) and return (m(T), a(0), u(0), u_h(0) = dL/dh as a
-    device fp64 3-vector)."""
+    device fp64 3-vector).
+    with_materials: also integrate the gradients with respect to the cell-wise A and Ku
+    (nm_adjoint_rk4_step_ex) and append (u_A(0), u_Ku(0)) to the returned tuple."""
     m = m0.clone()
     jumps = {}
     if objectives_at:
@@ -76,8 +78,12 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
     a = aT_of_mT(mT).clone()
     u = torch.zeros(mesh.cell_shape_abi, dtype=m.dtype, device=m.device)
     uh = torch.zeros(3, dtype=torch.float64, device=m.device) if with_hext else None
+    uA = torch.zeros_like(u) if with_materials else None
+    uKu = torch.zeros_like(u) if with_materials else None
     for s in range(n_steps, 0, -1):
-        if with_hext:
+        if with_materials:
+            mesh.nm_adjoint_rk4_step_ex(t0 + s * dt, dt, m, a, u, u_A=uA, u_Ku=uKu, u_h=uh, zeeman=zeeman)
+        elif with_hext:
             mesh.nm_adjoint_rk4_step_hext(t0 + s * dt, dt, m, a, u, uh, zeeman)
         else:
             mesh.nm_adjoint_rk4_step(t0 + s * dt, dt, m, a, u, zeeman)
@@ -85,6 +91,5 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
             m.copy_(ck[s - 1])
         if (s - 1) in jumps:
             mesh.nm_adjoint_add_objective(a, jumps[s - 1])
-    if with_hext:
-        return mT, a, u, uh
-    return mT, a, u
+    out = (mT, a, u) + ((uh,) if with_hext else ())
+    return out + ((uA, uKu) if with_materials else ())

@@ -441,6 +441,60 @@ def test_hext_gradient_rhs_and_backward_pass(prec):
         assert torch.equal(x, y)
 
 
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_materials_gradient_rhs_and_backward_pass(prec):
+    """VJPs with respect to the cell-wise A and Ku: nm_llg_adjoint_rhs_materials against the oracle on a
+    ragged all-terms mesh with a vacuum block, zero for terms a mesh does not have, and (u_A, u_Ku, u_h)
+    of drivers.adjoint_gradient(with_materials=True) against the oracle's backward pass."""
+    from oracle import adjoint
+    from paper_2411_11725_b200 import drivers
+    td = DT[prec]
+    nd = np_dtype(td)
+    w, hs = wl.varied_case((24, 12, 6), vacuum=True)
+    p = oracle_problem(w, nd)
+    m = _m0(w, td)
+    a = wl.round_to(np.random.default_rng(41).standard_normal(m.shape), nd)
+    gA_ref, gKu_ref = adjoint.adjoint_rhs_materials(p, 0.0, m, a)
+    mesh = gpu_mesh(w, td)
+    gA, gKu = mesh.nm_llg_adjoint_rhs_materials(dev(m, td), dev(a, td))
+    tol = 1e-11 if prec == "f64" else 2e-5
+    assert rel_l2(wl.from_abi(gA.cpu().double().numpy()), gA_ref) <= tol
+    assert rel_l2(wl.from_abi(gKu.cpu().double().numpy()), gKu_ref) <= tol
+    only_A, none_Ku = mesh.nm_llg_adjoint_rhs_materials(dev(m, td), dev(a, td), want_Ku=False)
+    assert none_Ku is None and torch.equal(only_A, gA)
+    w0 = wl.config4_sweep(16)                             # exchange + demag: nothing depends on Ku
+    m0_ = dev(_m0(w0, td), td)
+    gA0, gKu0 = gpu_mesh(w0, td).nm_llg_adjoint_rhs_materials(m0_, m0_.flip(0).contiguous())
+    assert torch.all(gKu0 == 0) and float(gA0.abs().max()) > 0
+    # backward integration: film with cell-wise A and Ku
+    w = wl.config5_inverse((32, 8, 1), n_steps=30)
+    rng = np.random.default_rng(43)
+    w.terms = wl.TERM_EXCHANGE | wl.TERM_DEMAG | wl.TERM_ANISO | wl.TERM_ZEEMAN
+    w.A = rng.uniform(3e-12, 4e-12, size=w.n_cells)
+    w.Ku = rng.uniform(1e4, 3e4, size=w.n_cells)
+    w.ku_axis = (0.0, 0.6, 0.8)
+    w.h_uniform = (1e3, 2e3, -1.5e3)
+    p = oracle_problem(w, nd)
+    z = oracle_zeeman(w, nd)
+    m0 = _m0(w, td)
+    wT = wl.round_to(wl.objective_weights(w), nd)
+    mT_ref, ck = adjoint.forward_rk4(p, m0, w.dt, w.n_steps, z, checkpoint_every=10)
+    ref = adjoint.backward_rk4(p, mT_ref, wT, w.dt, w.n_steps, z, checkpoints=ck, with_hext=True,
+                               with_materials=True)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    gT = dev(wT, td)
+    got = drivers.adjoint_gradient(mesh, dev(m0, td), lambda m_: gT, w.dt, w.n_steps, gz, checkpoint_every=10,
+                                   with_hext=True, with_materials=True)
+    cell = lambda x: wl.from_abi(x.cpu().double().numpy())
+    lo = 1e-11 if prec == "f64" else 2e-4
+    assert rel_l2(host(got[1]), ref[1]) <= (1e-11 if prec == "f64" else 1e-5)
+    assert rel_l2(cell(got[2]), ref[2]) <= lo
+    assert rel_l2(got[3].cpu().numpy(), ref[3]) <= lo
+    assert rel_l2(cell(got[4]), ref[4]) <= lo
+    assert rel_l2(cell(got[5]), ref[5]) <= lo
+
+
 # ---- boundary behaviour --------------------------------------------------------------------------
 def test_errors_are_statuses_not_crashes():
     from paper_2411_11725_b200 import binding as nm

@@ -93,3 +93,47 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
             mesh.nm_adjoint_add_objective(a, jumps[s - 1])
     out = (mT, a, u) + ((uh,) if with_hext else ())
     return out + ((uA, uKu) if with_materials else ())
+
+
+# ---- field-angle problem of Sec. VII (Eqs. 31-33) ------------------------------
+def field_from_angles(Hc, theta, phi):
+    """Eq. (31): H_ext = Hc (sin theta cos phi, sin theta sin phi, cos theta)."""
+    import math
+    return (Hc * math.sin(theta) * math.cos(phi), Hc * math.sin(theta) * math.sin(phi), Hc * math.cos(theta))
+
+
+def angle_gradient(dLdh, Hc, theta, phi):
+    """Chain rule of Eq. (31): (dL/dtheta, dL/dphi) from dL/dh (three host numbers)."""
+    import math
+    st, ct, sp, cp = math.sin(theta), math.cos(theta), math.sin(phi), math.cos(phi)
+    dth = Hc * (ct * cp * dLdh[0] + ct * sp * dLdh[1] - st * dLdh[2])
+    dph = Hc * (-st * sp * dLdh[0] + st * cp * dLdh[1])
+    return dth, dph
+
+
+def field_angle_gradient(mesh, m0, loss_grad, Hc, theta, phi, dt, n_steps, checkpoint_every=100,
+                         make_zeeman=None):
+    """One forward and one backward solve for the field angles: returns
+    (m(T), dL/dtheta, dL/dphi).  loss_grad(m(T)) is the caller's dL/dm(T) (the objective is the
+    caller's, Eq. 33); the uniform field of Eq. (31) is the only external field unless make_zeeman
+    (h_uniform -> Zeeman) adds nodal parts."""
+    from . import binding as nm
+    h = field_from_angles(Hc, theta, phi)
+    z = make_zeeman(h) if make_zeeman else nm.Zeeman(h_uniform=h)
+    mT, _, _, uh = adjoint_gradient(mesh, m0, loss_grad, dt, n_steps, z, checkpoint_every, with_hext=True)
+    dLdh = uh.cpu().tolist()                       # 24 bytes: the gradient the optimiser steps on
+    return (mT,) + angle_gradient(dLdh, Hc, theta, phi)
+
+
+def optimise_field_angles(mesh, m0, loss, loss_grad, Hc, theta, phi, dt, n_steps, rate, iterations,
+                          checkpoint_every=100):
+    """Plain gradient descent on (theta, phi) as in Sec. VII ("convergence is achieved after 30-50
+    gradient-descent steps").  loss(m(T)) -> float and loss_grad(m(T)) -> dL/dm(T) are
+    the caller's objective (Eq. 33).  Returns (theta, phi, [loss per iteration])."""
+    history = []
+    for _ in range(iterations):
+        mT, dth, dph = field_angle_gradient(mesh, m0, loss_grad, Hc, theta, phi, dt, n_steps, checkpoint_every)
+        history.append(float(loss(mT)))
+        theta -= rate * dth
+        phi -= rate * dph
+    return theta, phi, history

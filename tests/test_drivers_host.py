@@ -86,3 +86,17 @@ def test_adjoint_gradient_loop_adds_objectives_at_their_times():
     mesh2 = _FakeAdjMesh()
     drivers.adjoint_gradient(mesh2, m0, lambda m: torch.ones(1, dtype=torch.float64), 1.0, 4, checkpoint_every=2)
     assert [e[0] for e in mesh2.log] == ["fwd"] * 4 + ["bwd"] * 4
+
+
+def test_field_angle_chain_rule():
+    """Eq. (31) and its chain rule against central differences (host arithmetic on three numbers)."""
+    Hc, th, ph = 3.0e4, 0.7, -1.1
+    g = np.array([0.3, -1.2, 0.8])                                  # some dL/dh
+    f = lambda a, b: float(np.dot(g, drivers.field_from_angles(Hc, a, b)))
+    e = 1e-6
+    dth, dph = drivers.angle_gradient(g, Hc, th, ph)
+    assert abs(dth - (f(th + e, ph) - f(th - e, ph)) / (2 * e)) < 1e-5 * Hc
+    assert abs(dph - (f(th, ph + e) - f(th, ph - e)) / (2 * e)) < 1e-5 * Hc
+    h = drivers.field_from_angles(Hc, th, ph)
+    assert abs(np.sqrt(sum(v * v for v in h)) - Hc) < 1e-9 * Hc
+    assert drivers.field_from_angles(Hc, 0.0, 0.3)[2] == Hc

@@ -232,3 +232,56 @@ def test_adjoint_rhs_256_transpose_property_fp32():
     _, da2, du2 = msh.nm_llg_adjoint_rhs(0.0, m, (2.5 * a).contiguous())
     assert float((da2.double() - 2.5 * da.double()).norm() / da2.double().norm()) <= 1e-5
     assert float((du2.double() - 2.5 * du.double()).norm() / du2.double().norm()) <= 1e-4
+
+
+# ---- the film configs at their BASELINE.json sizes (dense, element by element) ---------------------
+def test_config3_full_size_rhs_and_dormand_prince_step_fp32():
+    """Config 3 at 512x512x1 cells, fp32, stripe pulse on: nm_llg_rhs at the pulse maximum and one
+    Dormand-Prince step (7 right-hand sides, error norm, commit) against the oracle, every node."""
+    from oracle import llg
+    from _sides import gpu_zeeman, oracle_zeeman
+    w = wl.config3_thin_film(512)
+    td = torch.float32
+    p = oracle_problem(w, np.float32)
+    z = oracle_zeeman(w, np.float32)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    m = wl.round_to(w.m0, np.float32)
+    t = w.pulse["t0"]                                   # sinc(0) = 1: full pulse amplitude
+    ref = llg.llg_rhs(p, t, m, z)
+    got = host(mesh.nm_llg_rhs(t, dev(m, td), gz))
+    assert rel_l2(got, ref) <= 1e-5
+    # the stripe is felt: the right-hand side differs from the one without the pulse
+    assert rel_l2(host(mesh.nm_llg_rhs(t + 1.0, dev(m, td), gz)), ref) > 1e-3
+    dt = 2e-13
+    out, err_ref, acc = llg.dopri5_step(p, t, dt, m, z, rtol=1e-5, atol=1e-5)
+    y = dev(m, td)
+    err = mesh.nm_rk_step(1, t, dt, y, gz, rtol=1e-5, atol=1e-5, want_err=True)
+    assert acc and err <= 1.0
+    assert abs(err - err_ref) <= 2e-2 * err_ref + 1e-4
+    assert rel_l2(host(y), out) <= 1e-5
+
+
+def test_config5_full_size_forward_and_backward_steps_fp64():
+    """Config 5 at 256x64x1 cells, fp64, cell-wise Ms: 12 RK4 steps forward, then the backward
+    integration of (m, a, u) with a checkpoint at step 6, against the oracle at 1e-11 (these steps
+    replay as CUDA graphs)."""
+    from oracle import adjoint
+    from _sides import gpu_zeeman, oracle_zeeman
+    from paper_2411_11725_b200 import drivers
+    w = wl.config5_inverse(n_steps=12)
+    assert tuple(w.n_cells) == (256, 64, 1)
+    td = torch.float64
+    p = oracle_problem(w)
+    z = oracle_zeeman(w)
+    mT_ref, ck = adjoint.forward_rk4(p, w.m0, w.dt, w.n_steps, z, checkpoint_every=6)
+    aT = wl.objective_weights(w)
+    _, a0_ref, u0_ref = adjoint.backward_rk4(p, mT_ref, aT, w.dt, w.n_steps, z, checkpoints=ck)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td)
+    g = dev(aT, td)
+    mT, a0, u0 = drivers.adjoint_gradient(mesh, dev(w.m0, td), lambda m_: g, w.dt, w.n_steps, gz,
+                                          checkpoint_every=6)
+    assert rel_l2(host(mT), mT_ref) <= 1e-11
+    assert rel_l2(host(a0), a0_ref) <= 1e-11
+    assert rel_l2(wl.from_abi(u0.cpu().numpy()), u0_ref) <= 1e-11

@@ -90,22 +90,25 @@ def tensor_at(Nt, a, p):
     return sign * Nt[a, abs(p[0]), abs(p[1]), abs(p[2])]
 
 
-def signed_tensor(Nt):
-    """Full array N[a, p1, p2, p3] over signed offsets p_d = -(N_d-1)..N_d-1 stored at index
-    p_d + N_d - 1 (shape 2 N_d - 1 per axis)."""
+def signed_component(Nt, a):
+    """Component a of the tensor over signed offsets p_d = -(N_d-1)..N_d-1, stored at index
+    p_d + N_d - 1 (shape 2 N_d - 1 per axis): the parity rule of tensor_at applied to the table."""
     n = Nt.shape[1:]
     idx = [np.abs(np.arange(-(k - 1), k)) for k in n]
     sgn = [np.sign(np.arange(-(k - 1), k) + 0.5) for k in n]
-    out = np.empty((6,) + tuple(2 * k - 1 for k in n))
-    for a, (r, s) in enumerate(COMPONENTS):
-        blk = Nt[a][np.ix_(idx[0], idx[1], idx[2])]
-        if r != s:
-            sg = [np.ones(2 * k - 1) for k in n]
-            sg[r] = sgn[r]
-            sg[s] = sgn[s]
-            blk = blk * sg[0][:, None, None] * sg[1][None, :, None] * sg[2][None, None, :]
-        out[a] = blk
-    return out
+    r, s = COMPONENTS[a]
+    blk = Nt[a][np.ix_(idx[0], idx[1], idx[2])]
+    if r != s:
+        sg = [np.ones(2 * k - 1) for k in n]
+        sg[r] = sgn[r]
+        sg[s] = sgn[s]
+        blk = blk * sg[0][:, None, None] * sg[1][None, :, None] * sg[2][None, None, :]
+    return blk
+
+
+def signed_tensor(Nt):
+    """Full array N[a, p1, p2, p3] over signed offsets (all six components of signed_component)."""
+    return np.stack([signed_component(Nt, a) for a in range(6)])
 
 
 def cell_magnetization(m, Ms):
@@ -135,22 +138,26 @@ def demag_field_cells_fft(M, Nt):
     """The same sum as a zero-padded circular convolution.
 
     The kernel is laid out on the padded grid at index (p mod P_d) for the signed offsets
-    p_d = -(N_d-1)..N_d-1; axes with N_d = 1 are not padded (P_d = 1)."""
+    p_d = -(N_d-1)..N_d-1; axes with N_d = 1 are not padded (P_d = 1).  The six tensor components
+    are laid out and transformed one after the other (memory only: a 256^3 mesh then needs one
+    padded kernel array at a time instead of six)."""
     n = M.shape[1:]
     P = tuple(2 * k if k > 1 else 1 for k in n)
-    Ns = signed_tensor(Nt)
-    ker = np.zeros((6,) + P)
     idx = [np.arange(-(k - 1), k) % p for k, p in zip(n, P)]
-    ker[np.ix_(np.arange(6), idx[0], idx[1], idx[2])] = Ns
     Mp = np.zeros((3,) + P)
     Mp[:, :n[0], :n[1], :n[2]] = M
     Mk = np.fft.rfftn(Mp, axes=(1, 2, 3))
-    Nk = np.fft.rfftn(ker, axes=(1, 2, 3))
+    del Mp
     Hk = np.zeros_like(Mk)
     for a, (r, s) in enumerate(COMPONENTS):
-        Hk[r] -= Nk[a] * Mk[s]
+        ker = np.zeros(P)
+        ker[np.ix_(idx[0], idx[1], idx[2])] = signed_component(Nt, a)
+        Nk = np.fft.rfftn(ker)
+        del ker
+        Hk[r] -= Nk * Mk[s]
         if r != s:
-            Hk[s] -= Nk[a] * Mk[r]
+            Hk[s] -= Nk * Mk[r]
+    del Mk
     Hp = np.fft.irfftn(Hk, s=P, axes=(1, 2, 3))
     return np.ascontiguousarray(Hp[:, :n[0], :n[1], :n[2]])
 

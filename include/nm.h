@@ -20,7 +20,7 @@
  *                workspace block handed to nm_mesh_create; the library allocates no device
  *                memory after nm_mesh_create returns and frees none that it did not allocate.
  *   Layout       nodal vector fields are structure-of-arrays [3][N3+1][N2+1][N1+1], x (index 1 of
- *                the paper's multi-index) fastest, contiguous.  Nodal scalars [N3+1][N2+1][N1+1].
+ *                the paper's multi-index) fastest, contiguous (no row padding).  Nodal scalars [N3+1][N2+1][N1+1].
  *                Cell scalars [N3][N2][N1], cell vectors [3][N3][N2][N1].
  *   Units        SI: H and Ms in A/m, A in J/m, Ku in J/m^3, gamma in m/(A s), t in s
  *                (PAPER.md:37).  mu0 = 4 pi 1e-7 exactly.
@@ -74,7 +74,6 @@ typedef struct {
     double ku_axis[3];    /* anisotropy axis k, unit vector, global (reading C3(i)) */
     const void *Ms, *A, *Ku; /* device, cell-wise [N3][N2][N1], copied at create; NULL => scalar below */
     double Ms_scalar, A_scalar, Ku_scalar;
-    long long node_pitch[3]; /* reserved for padded layouts; must be all 0 (contiguous) */
 } nm_mesh_desc;
 
 /* Bytes of device workspace nm_mesh_create needs for this description (spectrum buffers, demag
@@ -211,12 +210,13 @@ int nm_debug_demag_path(const nm_mesh *mesh);
 
 /* Per-kernel timing for the roofline line of bench.py.  Between
  * nm_profile_begin and nm_profile_end every kernel launch on this mesh is bracketed by a pair of
- * CUDA events on the launching stream (at most 4096 launches are recorded; later ones are only
- * counted by nm_launch_count).  nm_profile_end synchronises `stream` and writes, for each of the
- * nm_profile_class_count() kernel classes, the summed device time in milliseconds and the number
+ * CUDA events on the launching stream (at most 4096 launches are recorded; later ones are counted
+ * by nm_launch_count and nm_profile_dropped, so a caller can tell that its shares are incomplete).
+ * nm_profile_end synchronises `stream` and writes, for each of the nm_profile_class_count() kernel classes, the summed device time in milliseconds and the number
  * of recorded launches to the two HOST arrays (each of nm_profile_class_count() entries).
  * nm_profile_class_name(i) names class i ("x_fwd", "y_fwd", "mid", "y_inv", "x_inv", "node",
  * "adj_cell", "lincomb", "other"). */
+long long nm_profile_dropped(const nm_mesh *mesh); /* launches since nm_profile_begin that were not timed */
 int nm_profile_class_count(void);
 const char *nm_profile_class_name(int cls);
 nm_status nm_profile_begin(nm_mesh *mesh);

@@ -37,8 +37,11 @@ def _safe_div(num, den):
     return out
 
 
-def adjoint_rhs(p, t, m, a, zeeman=None):
-    """Returns (f, dadt, dudt_Ms) = (f(t,m), -(df/dm)^T a, -(df/dMs)^T a)."""
+def adjoint_rhs(p, t, m, a, zeeman=None, pieces=None):
+    """Returns (f, dadt, dudt_Ms) = (f(t,m), -(df/dm)^T a, -(df/dMs)^T a).
+
+    pieces: optional dict that receives the summands of (df/dMs)^T a as they are added ("field",
+    "zeeman", "demag_H", "demag_Y"), so that a test can state how strongly they cancel."""
     gp = p.gamma / (1.0 + p.alpha ** 2)
     al = p.alpha
     L = p.L
@@ -65,12 +68,22 @@ def adjoint_rhs(p, t, m, a, zeeman=None):
 
     # -(df/dMs)^T a
     grad = -gather_nodes_to_cells(_safe_div(dot(b, H), SMs))
+    if pieces is not None:
+        pieces["field"] = grad.copy()
+        # the same sum with every product b_j H_j taken in magnitude: b is perpendicular to m, so the
+        # m-parallel part of H (most of the exchange field of a smooth m) cancels inside b . H
+        pieces["field_abs"] = gather_nodes_to_cells(
+            _safe_div(np.abs(b[0] * H[0]) + np.abs(b[1] * H[1]) + np.abs(b[2] * H[2]), SMs))
     if (p.terms & _llg.TERM_ZEEMAN) and h_ext is not None:
         _, M = element_matrices(p.dx)
         bL = _safe_div(b, L)
+        zee = np.zeros_like(grad)
         for i in LOCAL:
             for ip in LOCAL:
-                grad = grad + MU0 * M[i + ip] * np.sum(node_view(bL, i) * node_view(h_ext, ip), axis=0)
+                zee = zee + MU0 * M[i + ip] * np.sum(node_view(bL, i) * node_view(h_ext, ip), axis=0)
+        grad = grad + zee
+        if pieces is not None:
+            pieces["zeeman"] = zee
     if p.terms & _llg.TERM_DEMAG:
         q = _safe_div(b, SMs)
         STq = gather_nodes_to_cells(q)
@@ -78,6 +91,9 @@ def adjoint_rhs(p, t, m, a, zeeman=None):
         Hcell = _demag.demag_field_cells_fft(p.Ms * mbar, p.Nt)
         Y = _demag.demag_field_cells_fft(p.Ms * STq, p.Nt)
         grad = grad + np.sum(STq * Hcell, axis=0) + np.sum(mbar * Y, axis=0)
+        if pieces is not None:
+            pieces["demag_H"] = np.sum(STq * Hcell, axis=0)
+            pieces["demag_Y"] = np.sum(mbar * Y, axis=0)
     return f, dadt, -grad
 
 

@@ -98,8 +98,10 @@ def llg_rhs(p, t, m, zeeman=None):
 
 
 def normalise(m):
+    """m_n / |m_n|; a zero vector stays zero (vacuum nodes are usually given m = 0; with reading
+    C3(iii) they feel H = 0, so they stay at 0 for ever and never enter a cell average as NaN)."""
     nrm = np.sqrt(m[0] ** 2 + m[1] ** 2 + m[2] ** 2)
-    return m / nrm
+    return m / np.where(nrm > 0, nrm, 1.0)
 
 
 def rk4_step(p, t, dt, m, zeeman=None, renormalise=True):
@@ -154,6 +156,8 @@ def dopri5_step(p, t, dt, m, zeeman=None, renormalise=True, rtol=1e-5, atol=1e-5
 
 def dopri5_next_dt(dt, err_norm):
     """dt_new = dt * clip(0.9 * err_norm^(-1/5), 0.2, 5) (reading C6)."""
+    if not np.isfinite(err_norm):
+        return 0.2 * dt          # a non-finite trial state is a rejected step: shrink
     if err_norm == 0.0:
         return 5.0 * dt
     return dt * min(5.0, max(0.2, 0.9 * err_norm ** (-0.2)))

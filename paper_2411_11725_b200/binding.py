@@ -24,7 +24,7 @@ EXPORTS = ("nm_mesh_query_workspace", "nm_mesh_create", "nm_mesh_set_Ms", "nm_me
            "nm_last_error", "nm_heff", "nm_llg_rhs", "nm_rk_step", "nm_llg_adjoint_rhs",
            "nm_adjoint_rk4_step", "nm_adjoint_add_objective", "nm_llg_adjoint_rhs_hext", "nm_adjoint_rk4_step_hext",
            "nm_llg_adjoint_rhs_materials", "nm_adjoint_rk4_step_ex", "nm_debug_get_tensor", "nm_debug_get_cell_field",
-           "nm_launch_count", "nm_debug_demag_path", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
+           "nm_launch_count", "nm_profile_dropped", "nm_debug_demag_path", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
            "nm_profile_end")
 
 
@@ -39,8 +39,7 @@ class nm_mesh_desc(ctypes.Structure):
                 ("ku_axis", ctypes.c_double * 3),
                 ("Ms", ctypes.c_void_p), ("A", ctypes.c_void_p), ("Ku", ctypes.c_void_p),
                 ("Ms_scalar", ctypes.c_double), ("A_scalar", ctypes.c_double),
-                ("Ku_scalar", ctypes.c_double),
-                ("node_pitch", ctypes.c_longlong * 3)]
+                ("Ku_scalar", ctypes.c_double)]
 
 
 AMP_FUNC = ctypes.CFUNCTYPE(ctypes.c_double, ctypes.c_double, ctypes.c_void_p)
@@ -96,6 +95,8 @@ def lib():
         L.nm_debug_get_cell_field.argtypes = [vp, vp, vp]
         L.nm_launch_count.argtypes = [vp]
         L.nm_launch_count.restype = ctypes.c_longlong
+        L.nm_profile_dropped.argtypes = [vp]
+        L.nm_profile_dropped.restype = ctypes.c_longlong
         L.nm_debug_demag_path.argtypes = [vp]
         L.nm_debug_demag_path.restype = ctypes.c_int
         L.nm_profile_class_count.argtypes = []
@@ -104,7 +105,7 @@ def lib():
         L.nm_profile_begin.argtypes = [vp]
         L.nm_profile_end.argtypes = [vp, vp, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_longlong)]
         for name in EXPORTS:
-            if name not in ("nm_last_error", "nm_launch_count", "nm_debug_demag_path", "nm_profile_class_name"):
+            if name not in ("nm_last_error", "nm_launch_count", "nm_profile_dropped", "nm_profile_dropped", "nm_debug_demag_path", "nm_profile_class_name"):
                 getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -143,7 +144,6 @@ def make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis=(0
         else:
             setattr(d, name, None)
             setattr(d, name + "_scalar", float(v) if v is not None else 0.0)
-    d.node_pitch[:] = [0, 0, 0]
     d._keep = keep
     return d
 
@@ -283,6 +283,9 @@ class Mesh:
 
     def nm_launch_count(self):
         return int(lib().nm_launch_count(self.handle))
+
+    def nm_profile_dropped(self):
+        return int(lib().nm_profile_dropped(self.handle))
 
     def nm_debug_demag_path(self):
         return int(lib().nm_debug_demag_path(self.handle))

@@ -77,7 +77,6 @@ nm_status validate(const nm_mesh_desc *d)
     for (int i = 0; i < 3; ++i) {
         if (d->n_cells[i] < 1) { nm_set_error("n_cells[%d] = %d < 1", i, d->n_cells[i]); return NM_EINVAL; }
         if (!(d->cell_size[i] > 0)) { nm_set_error("cell_size[%d] must be > 0", i); return NM_EINVAL; }
-        if (d->node_pitch[i] != 0) { nm_set_error("node_pitch must be 0 (contiguous layout)"); return NM_EINVAL; }
     }
     if (d->dtype != NM_F32 && d->dtype != NM_F64) { nm_set_error("bad dtype"); return NM_EINVAL; }
     if (d->terms == 0 || (d->terms & ~15u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
@@ -215,6 +214,7 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
     m->hc1_valid = false;
     m->prof_on = false;
     m->prof_n = 0;
+    m->prof_dropped = 0;
     m->prof_ev_made = 0;
     {
         // whole steps of small meshes are launch-latency-bound: replay them as graphs (NM_GRAPH=0 / 1
@@ -224,6 +224,12 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
         m->cap_stream = nullptr;
         m->graph_epoch = 0;
         memset(m->step_graph, 0, sizeof(m->step_graph));
+    }
+    {
+        // test switch, read here once (never on the evaluation path): NM_NODE_PATH = "generic" forces the
+        // 27-point node kernel, "sep" k_node_sep
+        const char *env = getenv("NM_NODE_PATH");
+        m->dbg_node_path = env && strcmp(env, "generic") == 0 ? 1 : env && strcmp(env, "sep") == 0 ? 2 : 0;
     }
     nm_fast_plan(d, m->g, &m->fast);
     {
@@ -451,6 +457,7 @@ extern "C" nm_status nm_profile_begin(nm_mesh *mesh)
     if (!mesh) { nm_set_error("NULL argument"); return NM_EINVAL; }
     mesh->prof_on = true;
     mesh->prof_n = 0;
+    mesh->prof_dropped = 0;
     return NM_OK;
 }
 
@@ -472,6 +479,8 @@ extern "C" nm_status nm_profile_end(nm_mesh *mesh, void *stream, double *ms_host
 }
 
 extern "C" long long nm_launch_count(const nm_mesh *mesh) { return mesh ? mesh->launches : 0; }
+
+extern "C" long long nm_profile_dropped(const nm_mesh *mesh) { return mesh ? mesh->prof_dropped : 0; }
 
 extern "C" int nm_debug_demag_path(const nm_mesh *mesh)
 {
@@ -539,11 +548,8 @@ void base_args(const nm_mesh *m, double t, const nm_zeeman *z, unsigned terms, N
     // separable kernel: uniform A and Ku (anisotropy off counts as uniform)
     const bool an_on = (terms & NM_TERM_ANISO) != 0;
     a->sep = (m->uni_A && (m->uni_Ku || !an_on)) ? 1 : 0;
-    {
-        const char *env = getenv("NM_NODE_PATH");        // "generic" forces the 27-point kernel, "sep" k_node_sep
-        if (env && strcmp(env, "generic") == 0) a->sep = 0;
-        else if (env && strcmp(env, "sep") == 0 && a->sep) a->sep = 2;
-    }
+    if (m->dbg_node_path == 1) a->sep = 0;                       // test switch, read once at nm_mesh_create
+    else if (m->dbg_node_path == 2 && a->sep) a->sep = 2;
     a->cex = (terms & NM_TERM_EXCHANGE) ? (T)(16.0 * m->desc.A_scalar / NM_MU0) : (T)0;
     a->cku = an_on ? (T)(16.0 * m->desc.Ku_scalar / NM_MU0) : (T)0;
     for (int d = 0; d < 3; ++d) a->idx2[d] = (T)(1.0 / (dx[d] * dx[d]));
@@ -667,7 +673,7 @@ nm_status dopri5_step(nm_mesh *m, double t, double dt, T *y, const nm_zeeman *z,
     }
     NM_TRY(nm_launch_err_final(m, m->last_partials, 3.0 * (double)m->g.nodes, st));
     // y5 lives in Yb[5 & 1]
-    return nm_launch_commit<T>(m, y, Yb[1], m->partials + m->last_partials, renorm, st);
+    return nm_launch_commit<T>(m, y, Yb[1], m->partials + m->n_partials, renorm, st);
 }
 
 // (f, -(df/dm)^T a, -(df/dMs)^T a): reading C7, two demag convolutions and two node passes.
@@ -914,7 +920,7 @@ extern "C" nm_status nm_rk_step(nm_mesh *mesh, nm_scheme scheme, double t, doubl
                                                   atol, s);
         }));
         if (err_norm_host) {
-            NM_CUDA_TRY(cudaMemcpyAsync(err_norm_host, mesh->partials + mesh->last_partials, sizeof(double),
+            NM_CUDA_TRY(cudaMemcpyAsync(err_norm_host, mesh->partials + mesh->n_partials, sizeof(double),
                                         cudaMemcpyDeviceToHost, st));
             NM_CUDA_TRY(cudaStreamSynchronize(st));
         }

@@ -119,9 +119,11 @@ struct nm_mesh {
     // materials given as scalars at create (enables the separable node kernel)
     bool uni_A, uni_Ku, uni_Ms;
     bool hc1_valid;
+    int dbg_node_path;      // NM_NODE_PATH at create: 0 automatic, 1 27-point kernel, 2 k_node_sep (tests)
     // per-launch timing (nm_profile_begin / nm_profile_end)
     bool prof_on;
     int prof_n;
+    long long prof_dropped; // launches since nm_profile_begin that found the event table full (not timed)
     int prof_cls[NM_PROF_MAX];
     cudaEvent_t prof_ev[NM_PROF_MAX][2];
     int prof_ev_made;       // events created so far (created lazily, destroyed with the mesh)
@@ -140,6 +142,7 @@ struct NmLaunchScope {
     NmLaunchScope(nm_mesh *mesh, int cls, cudaStream_t stream) : m(mesh), st(stream), slot(-1)
     {
         m->launches++;
+        if (m->prof_on && m->prof_n >= NM_PROF_MAX) m->prof_dropped++;
         if (m->prof_on && m->prof_n < NM_PROF_MAX) {
             slot = m->prof_n++;
             if (slot >= m->prof_ev_made) {

@@ -94,7 +94,8 @@ __device__ __forceinline__ void node_epilogue(const NmLocalArgs<T> &a, long long
             }
             if (r.ynext) {
                 if (r.renorm) {
-                    const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+                    const T n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+                    const T inv = n2 > (T)0 ? rsqrt_t<T>(n2) : (T)0;   // a zero vector (vacuum node) stays zero
                     y[0] *= inv; y[1] *= inv; y[2] *= inv;
                 }
                 r.ynext[n] = y[0]; r.ynext[nn + n] = y[1]; r.ynext[2 * nn + n] = y[2];
@@ -500,13 +501,15 @@ __global__ void __launch_bounds__(SX * SY) k_node_sep(const NmLocalArgs<T> a, in
     }
 }
 
-// partials[0..n) -> partials[n] = sqrt(sum / count), fixed summation order
-__global__ void k_err_final(double *partials, int n, double count)
+// partials[0..n) -> partials[slot] = sqrt(sum / count), fixed summation order.  `slot` is the fixed last
+// entry of the array (its capacity), not n: the commit kernel and the host read-back of a replayed step
+// must not depend on which node kernel ran last.
+__global__ void k_err_final(double *partials, int n, double count, int slot)
 {
     double v = 0.0;
     for (int i = threadIdx.x; i < n; i += blockDim.x) v += partials[i];
     const double s = block_sum(v);
-    if (threadIdx.x == 0) partials[n] = sqrt(s / count);
+    if (threadIdx.x == 0) partials[slot] = sqrt(s / count);
 }
 
 // Uniform-field gradient, first pass: per-block fp64 sums of b_n over the nodes with (S Ms)_n > 0.
@@ -600,7 +603,8 @@ __global__ void k_commit(T *__restrict__ m, const T *__restrict__ y5, long long 
     if (n >= nodes) return;
     T y[3] = {y5[n], y5[nodes + n], y5[2 * nodes + n]};
     if (renorm) {
-        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+        const T n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+        const T inv = n2 > (T)0 ? rsqrt_t<T>(n2) : (T)0;   // a zero vector (vacuum node) stays zero
         y[0] *= inv; y[1] *= inv; y[2] *= inv;
     }
     m[n] = y[0]; m[nodes + n] = y[1]; m[2 * nodes + n] = y[2];
@@ -751,7 +755,8 @@ template <typename T> __global__ void k_lincomb(const LinArgs<T> a)
             for (int s = 0; s < a.nsrc; ++s) v += a.coef[s] * a.src[s][j * a.vec_n + i];
             y[j] = v;
         }
-        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+        const T n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+        const T inv = n2 > (T)0 ? rsqrt_t<T>(n2) : (T)0;   // a zero vector (vacuum node) stays zero
         for (int j = 0; j < 3; ++j) a.out[j * a.vec_n + i] = y[j] * inv;
     } else {
         if (i >= a.n) return;
@@ -779,7 +784,8 @@ template <typename T> __global__ void k_lincomb_batch(const LinBatch<T> b)
             v += a.coef[0] * a.src[0][j * a.vec_n + i];
             y[j] = v;
         }
-        const T inv = rsqrt_t<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+        const T n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+        const T inv = n2 > (T)0 ? rsqrt_t<T>(n2) : (T)0;   // a zero vector (vacuum node) stays zero
         for (int j = 0; j < 3; ++j) a.out[j * a.vec_n + i] = y[j] * inv;
     } else {
         if (i >= a.n) return;
@@ -859,7 +865,7 @@ nm_status nm_launch_err_final(nm_mesh *mesh, int n_partials, double count, cudaS
 {
     {
         NmLaunchScope sc(mesh, NM_K_OTHER, st);
-        k_err_final<<<1, 1024, 0, st>>>(mesh->partials, n_partials, count);
+        k_err_final<<<1, 1024, 0, st>>>(mesh->partials, n_partials, count, mesh->n_partials);
     }
 
     NM_CUDA_TRY(cudaGetLastError());

@@ -145,7 +145,8 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
 #pragma unroll
             for (int j = 0; j < 3; ++j) y[j] = base[j] + r.dt * acc[j];
             if (r.renorm) {
-                const T inv = rsqrt_c<T>(y[0] * y[0] + y[1] * y[1] + y[2] * y[2]);
+                const T n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+                const T inv = n2 > (T)0 ? rsqrt_c<T>(n2) : (T)0;   // a zero vector (vacuum node) stays zero
                 y[0] *= inv; y[1] *= inv; y[2] *= inv;
             }
 #pragma unroll

@@ -7,8 +7,9 @@
 // which for |R| >= 8 max(dx) is a smooth integrand.  The double volume integral reduces to one
 // 3-D integral over u = r - r' with the triangle weight prod_d (dx_d - |u_d|); it is evaluated
 // here in fp64 with Gauss-Legendre points on each half-interval (6 points: error < 1e-18
-// absolute at 8 cell sizes; 4 and 3 points further out, measured against the closed form in
-// _work prototypes and by tests/test_gpu_tensor.py).  No cancellation occurs, unlike the
+// absolute at 8 cell sizes; 4 and 3 points further out; tests/test_gpu_parity.py:
+// test_tensor_matches_oracle holds every entry of five grids to 1e-13 of the oracle's binary128
+// closed form, the 48^3 grid reaching all three orders).  No cancellation occurs, unlike the
 // closed form whose fp64 evaluation loses every digit beyond ~100 cells.  Offsets closer than
 // that come from the closed form in binary128 on the host (nm_newell_host.cpp).
 //

@@ -7,19 +7,25 @@ import torch
 
 
 def dopri5_next_dt(dt, err_norm, safety=0.9, lo=0.2, hi=5.0):
-    """Reading C6: dt_new = dt * clip(0.9 * err^(-1/5), 0.2, 5)."""
-    if not (err_norm > 0.0):
+    """Reading C6: dt_new = dt * clip(0.9 * err^(-1/5), 0.2, 5).  A non-finite error norm (NaN / Inf
+    in the trial state) is a rejected step: shrink by the lower clip factor."""
+    if err_norm != err_norm or err_norm == float("inf"):
+        return dt * lo
+    if err_norm <= 0.0:
         return dt * hi
     return dt * min(hi, max(lo, safety * err_norm ** (-0.2)))
 
 
 def integrate_dopri5(mesh, m, t0, t1, dt0, zeeman=None, rtol=1e-5, atol=1e-5, renormalise=True,
-                     max_steps=10 ** 9, on_step=None):
+                     max_steps=10 ** 9, on_step=None, dt_min=0.0, max_rejects_in_a_row=50):
     """Advance m in place from t0 to t1 with Dormand-Prince 5(4).  The device takes
     the accept/reject decision (nm_rk_step leaves m untouched on a rejected step) and returns the
-    scalar error norm; this loop only adapts dt.  Returns (t, dt, accepted, rejected)."""
+    scalar error norm; this loop only adapts dt.  Returns (t, dt, accepted, rejected).  Raises
+    ArithmeticError when the step size falls below dt_min or max_rejects_in_a_row trial steps in a
+    row are rejected (a non-finite error norm counts as rejected): the state cannot be advanced."""
     t, dt = float(t0), float(dt0)
     acc = rej = 0
+    run = 0
     while t < t1 and acc + rej < max_steps:
         h = min(dt, t1 - t)
         err = mesh.nm_rk_step(1, t, h, m, zeeman, renormalise=renormalise, rtol=rtol, atol=atol,
@@ -27,11 +33,18 @@ def integrate_dopri5(mesh, m, t0, t1, dt0, zeeman=None, rtol=1e-5, atol=1e-5, re
         if err <= 1.0:
             t += h
             acc += 1
+            run = 0
             if on_step is not None:
                 on_step(t, h, err)
         else:
             rej += 1
-        dt = dopri5_next_dt(h, err)
+            run += 1
+        nxt = dopri5_next_dt(h, err)
+        # a step clipped to land on t1 says nothing against the step size in use before it
+        dt = max(nxt, dt) if (h < dt and err <= 1.0) else nxt
+        if run >= max_rejects_in_a_row or not (dt > dt_min):
+            raise ArithmeticError("Dormand-Prince: %d trial steps rejected in a row at t = %.6e s "
+                                  "(last error norm %r, next dt %.3e s)" % (run, t, err, dt))
     return t, dt, acc, rej
 
 

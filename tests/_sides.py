@@ -17,6 +17,44 @@ def rel_l2(x, ref):
     return num / den if den > 0 else num
 
 
+def max_abs_rel(x, ref):
+    """max |x - ref| / max |ref|: the element-wise companion of rel_l2 (one wrong node on a 17 M-node
+    grid moves the L2 norm by 1e-6 of itself and this by its full error)."""
+    x = np.asarray(x, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    den = np.max(np.abs(ref))
+    num = np.max(np.abs(x - ref))
+    return num / den if den > 0 else num
+
+
+def assert_parity(x, ref, tol, what="", cmax=10.0):
+    """north_star's relative-L2 bound and, beside it, max |x - ref| <= cmax * tol * max |ref|."""
+    e, m = rel_l2(x, ref), max_abs_rel(x, ref)
+    assert e <= tol, "%s: rel L2 %.3e > %.1e" % (what, e, tol)
+    assert m <= cmax * tol, "%s: max abs %.3e of max|ref| > %.1e" % (what, m, cmax * tol)
+    return e, m
+
+
+# The oracle's tensor table N(p), p_d = 0..N_d-1, depends on the offset and the cell size only, so the
+# table of a smaller grid with the same cells is a sub-block of a larger one (pinned on a tiny case in
+# tests/test_oracle_demag.py).  The config-4 grids share their cell size: the __float128 table of the
+# largest one asked for so far is kept for the session and sliced.
+_TENSOR_CACHE = {}
+
+
+def oracle_tensor(n_cells, dx):
+    from oracle import demag
+    n = tuple(int(v) for v in n_cells)
+    key = tuple(float(v) for v in dx)
+    have = _TENSOR_CACHE.get(key)
+    if have is not None and all(a <= b for a, b in zip(n, have.shape[1:])):
+        return np.ascontiguousarray(have[:, :n[0], :n[1], :n[2]])
+    Nt = demag.demag_tensor(n, key)
+    if have is None or Nt.size > have.size:
+        _TENSOR_CACHE[key] = Nt
+    return Nt
+
+
 def np_dtype(torch_dtype):
     import torch
     return np.float64 if torch_dtype == torch.float64 else np.float32
@@ -26,8 +64,11 @@ def oracle_problem(w, dtype=np.float64):
     """oracle.llg.Problem with the materials rounded to the build precision."""
     from oracle import llg
     r = lambda v: wl.round_to(w.cell_array(v), dtype)
-    return llg.Problem(tuple(w.n_cells), tuple(float(v) for v in w.dx), r(w.Ms), r(w.A), r(w.Ku),
-                       tuple(w.ku_axis), float(w.gamma), float(w.alpha), int(w.terms))
+    p = llg.Problem(tuple(w.n_cells), tuple(float(v) for v in w.dx), r(w.Ms), r(w.A), r(w.Ku),
+                    tuple(w.ku_axis), float(w.gamma), float(w.alpha), int(w.terms))
+    if (w.terms & wl.TERM_DEMAG) and int(np.prod(w.n_cells)) >= 32 ** 3:
+        p._Nt = oracle_tensor(w.n_cells, w.dx)
+    return p
 
 
 def oracle_zeeman(w, dtype=np.float64, h_static=None):

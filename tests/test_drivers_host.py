@@ -35,6 +35,33 @@ def test_integrate_dopri5_loop_control():
     assert abs(mesh.calls[-1][0] + mesh.calls[-1][1] - 1.0) < 1e-15
 
 
+class _NanMesh:
+    """Every trial step returns a NaN error norm (a state that went non-finite)."""
+    def __init__(self):
+        self.calls = []
+
+    def nm_rk_step(self, scheme, t, dt, m, zeeman, renormalise, rtol, atol, want_err):
+        self.calls.append(dt)
+        return float("nan")
+
+
+def test_non_finite_error_norm_shrinks_the_step_and_then_fails():
+    """a NaN error norm used to read as "no error" (dt * 5 for ever)."""
+    import pytest
+    assert drivers.dopri5_next_dt(1.0, float("nan")) == 0.2
+    assert drivers.dopri5_next_dt(1.0, float("inf")) == 0.2
+    assert llg.dopri5_next_dt(1.0, float("nan")) == 0.2 and llg.dopri5_next_dt(1.0, float("inf")) == 0.2
+    mesh = _NanMesh()
+    with pytest.raises(ArithmeticError):
+        drivers.integrate_dopri5(mesh, None, 0.0, 1.0, 0.1, max_rejects_in_a_row=6)
+    assert len(mesh.calls) == 6
+    assert all(b < a for a, b in zip(mesh.calls, mesh.calls[1:]))     # each retry is smaller
+    mesh = _NanMesh()
+    with pytest.raises(ArithmeticError):
+        drivers.integrate_dopri5(mesh, None, 0.0, 1.0, 0.1, dt_min=1e-3)
+    assert len(mesh.calls) == 3                                       # 0.1, 0.02, 0.004 -> 0.0008 < dt_min
+
+
 class _FakeAdjMesh:
     """Scalar stand-in for the adjoint loops: m += 1 per forward step, m -= 1 per backward step;
     records the order of the calls."""

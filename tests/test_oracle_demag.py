@@ -290,3 +290,12 @@ def test_tensor_at_listed_offsets_matches_table_and_dipole_limit():
         A[r, s] = A[s, r] = T[a]
     assert np.abs(A - D).max() <= 1e-4 * np.abs(D).max()
     assert abs(np.trace(A)) <= 1e-9 * np.abs(D).max()
+
+
+def test_tensor_table_of_a_smaller_grid_is_a_sub_block():
+    """N(p) depends on the offset and the cell size only (tests/_sides.py slices the table of the
+    largest config-4 grid for the smaller ones)."""
+    dx = (2e-9, 3e-9, 2.5e-9)
+    big = demag.demag_tensor((8, 7, 6), dx)
+    small = demag.demag_tensor((5, 4, 3), dx)
+    assert np.array_equal(big[:, :5, :4, :3], small)

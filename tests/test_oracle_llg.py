@@ -168,3 +168,14 @@ def test_dopri5_error_norm_definition():
     got = y5[:, 0, 0, 0] if ok else None
     if ok:
         assert np.allclose(got, y5r, rtol=1e-13)
+
+
+def test_normalise_keeps_zero_vectors_zero():
+    """Vacuum nodes carry m = 0 by convention: normalise must not turn them into NaN."""
+    m = np.zeros((3, 2, 2, 1))
+    m[:, 0, 0, 0] = (3.0, 0.0, 4.0)
+    m[:, 1, 1, 0] = (0.0, -2.0, 0.0)
+    out = llg.normalise(m)
+    assert np.all(np.isfinite(out))
+    assert np.allclose(out[:, 0, 0, 0], (0.6, 0.0, 0.8)) and np.allclose(out[:, 1, 1, 0], (0.0, -1.0, 0.0))
+    assert np.all(out[:, 0, 1, 0] == 0) and np.all(out[:, 1, 0, 0] == 0)

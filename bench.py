@@ -45,14 +45,74 @@ def parse():
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sample-grid", type=int, default=0, help="oracle sample grid (0 = auto)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 / film sweep block")
+    ap.add_argument("--config3", type=float, default=0.0, metavar="NS",
+                    help="instead of the bench: run config 3's stated recipe (512x512x1, fp32, Dormand-Prince) "
+                         "for NS nanoseconds (10 = the full run) and print its wall time as one JSON line")
+    ap.add_argument("--traffic-from", default="", metavar="NCU_REP",
+                    help="instead of the bench: read dram bytes per launch of the hot kernels from an "
+                         "`ncu --set full` report of this command and write profiles/traffic.json")
     return ap.parse_args()
 
 
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class from the
-# committed `ncu --set full` capture of this command (profiles/r1e_final.md); only for the workload
-# that capture was taken on (256^3, fp32)
-NCU_TRAFFIC = {(256, "f32"): {"mid": 2025138896, "y_fwd": 1195136896, "y_inv": 1215810952,
-                              "x_fwd": 569166424, "x_inv": 586457048, "node": 808990384}}
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch of each kernel class come from
+# profiles/traffic.json, written by `bench.py --traffic-from <ncu report>` from one `ncu --set full`
+# capture of this command and stamped with the hash of the kernel sources it was captured on; a
+# capture of other sources than the ones in the tree is reported as stale (traffic = null).
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+KERNEL_CLASS = (("k_pz_mid", "mid"), ("k_fz_mid", "mid"), ("k_py_fwd", "y_fwd"), ("k_fy_fwd", "y_fwd"),
+                ("k_py_inv", "y_inv"), ("k_fy_inv", "y_inv"), ("k_px_fwd", "x_fwd"), ("k_px_inv", "x_inv"),
+                ("k_node", "node"))
+
+
+def csrc_hash():
+    import hashlib
+    d = os.path.join(ROOT, "paper_2411_11725_b200", "csrc")
+    h = hashlib.sha1()
+    for f in sorted(os.listdir(d)):
+        h.update(f.encode())
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()
+
+
+def load_traffic(N, dtype):
+    """(bytes per launch by kernel class or {}, source string)."""
+    try:
+        t = json.load(open(TRAFFIC_JSON))
+    except Exception:
+        return {}, "no profiles/traffic.json"
+    if t.get("csrc_sha1") != csrc_hash():
+        return {}, "profiles/traffic.json is stale (captured on other kernel sources, commit %s)" % t.get("commit")
+    if (t.get("grid"), t.get("dtype")) != (N, dtype):
+        return {}, "profiles/traffic.json is for %s^3 %s" % (t.get("grid"), t.get("dtype"))
+    return t["bytes_per_launch"], "profiles/traffic.json (ncu --set full, per launch, commit %s)" % t.get("commit")
+
+
+def write_traffic(rep, N, dtype):
+    """Parse `ncu -i rep --page raw --csv` and write profiles/traffic.json."""
+    import csv
+    import io
+    out = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True).stdout
+    rows = list(csv.reader(io.StringIO(out)))
+    idx = {h: i for i, h in enumerate(rows[0])}
+    units = rows[1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    acc = {}
+    for r in rows[2:]:
+        name = r[idx["Kernel Name"]]
+        cls = next((c for k, c in KERNEL_CLASS if name.startswith(k)), None)
+        if cls is None:
+            continue
+        b = 0.0
+        for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            b += float(r[idx[col]].replace(",", "")) * scale[units[idx[col]]]
+        acc.setdefault(cls, []).append(b)
+    commit = subprocess.run(["git", "rev-parse", "--short", "HEAD"], capture_output=True, text=True, cwd=ROOT).stdout.strip()
+    doc = {"commit": commit or None, "csrc_sha1": csrc_hash(), "grid": N, "dtype": dtype, "report": os.path.basename(rep),
+           "bytes_per_launch": {k: int(sum(v) / len(v)) for k, v in acc.items()},
+           "launches_averaged": {k: len(v) for k, v in acc.items()}}
+    json.dump(doc, open(TRAFFIC_JSON, "w"), indent=1)
+    print(json.dumps(doc))
 
 
 def peaks():
@@ -149,7 +209,7 @@ def oracle_sample_grid(n_steps_total, grid, forced=0):
     return min(16, grid)
 
 
-def oracle_run(sample_n, dtype_name, steps, warmup):
+def oracle_run(sample_n, dtype_name, steps, warmup, fft_workers=1):
     """Times `steps` oracle steps (rk4_step + adjoint_rhs, fp64 arithmetic on inputs rounded to the
     build precision) on the sample grid; the demag tensor setup is outside the timed region, like
     nm_mesh_create on the GPU side.  Returns (seconds, cells per step, threads)."""
@@ -172,14 +232,30 @@ def oracle_run(sample_n, dtype_name, steps, warmup):
         adjoint.adjoint_rhs(p, 0.0, mm, a)
         return mm
 
-    for _ in range(warmup):
-        m = step(m)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        m = step(m)
-    sec = time.perf_counter() - t0
-    # numpy elementwise loops and numpy.fft (pocketfft) run on one thread; no BLAS call is made
-    return sec, sample_n ** 3, 1
+    def run():
+        mm = m
+        for _ in range(warmup):
+            mm = step(mm)
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            mm = step(mm)
+        return time.perf_counter() - t0
+
+    if fft_workers <= 1:
+        # numpy elementwise loops and numpy.fft (pocketfft) run on one thread; no BLAS call is made
+        return run(), sample_n ** 3, 1
+    # BASELINE.md 4's second line: the same oracle with its library FFT calls (numpy.fft.rfftn / irfftn,
+    # the only routines it calls there) served by scipy.fft on `fft_workers` threads; everything else
+    # in it stays single-threaded numpy.  The oracle's source is not touched: the two names are
+    # swapped in numpy.fft for the duration of this leg.
+    import scipy.fft as sfft
+    keep = (np.fft.rfftn, np.fft.irfftn)
+    np.fft.rfftn = lambda a, s=None, axes=None: sfft.rfftn(a, s=s, axes=axes, workers=fft_workers)
+    np.fft.irfftn = lambda a, s=None, axes=None: sfft.irfftn(a, s=s, axes=axes, workers=fft_workers)
+    try:
+        return run(), sample_n ** 3, fft_workers
+    finally:
+        np.fft.rfftn, np.fft.irfftn = keep
 
 
 def run_reference(args):
@@ -203,6 +279,136 @@ def run_reference(args):
         "gpu_launches": 0,
     }
     print(json.dumps(out))
+
+
+# --------------------------------------------------------------------------------------------------
+# the other configurations, timed after the bench's own region (CUDA events, this process, one GPU)
+def _dev_mesh(w, td):
+    import numpy as np
+    import torch
+
+    from paper_2411_11725_b200 import binding as nm
+    from paper_2411_11725_b200 import workloads as wl
+    put = lambda a: torch.from_numpy(wl.to_abi(a)).to(device="cuda", dtype=td).contiguous()
+    mat = {k: (float(getattr(w, k)) if np.isscalar(getattr(w, k)) else put(getattr(w, k))) for k in ("Ms", "A", "Ku")}
+    mesh = nm.Mesh(w.n_cells, w.dx, dtype=td, device=torch.cuda.current_device(), terms=w.terms, gamma=w.gamma,
+                   alpha=w.alpha, ku_axis=w.ku_axis, **mat)
+    z = None
+    if w.terms & wl.TERM_ZEEMAN:
+        hp = put(w.h_pulse) if w.h_pulse is not None else None
+        amp = (lambda t: wl.sinc_pulse(t, **w.pulse)) if (w.pulse and hp is not None) else None
+        z = nm.Zeeman(h_uniform=w.h_uniform, h_pulse=hp, amp=amp)
+    nd = np.float64 if td == torch.float64 else np.float32
+    return mesh, z, put(wl.round_to(w.m0, nd))
+
+
+def _event_ms(fn, n, warm=5):
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n
+
+
+def sweep_block(peak):
+    """nm_llg_rhs (and the steps each config is stated with) at the other points of config 4 and at the
+    film configs 1, 3, 5: ms per call by CUDA events after warm-up, Mcells/s, and the fraction of the
+    HBM peak over the algorithmic bytes of one evaluation (grids that fit the 126 MB L2 are marked)."""
+    import torch
+
+    from paper_2411_11725_b200 import binding as nm
+    from paper_2411_11725_b200 import workloads as wl
+    rows = []
+    pts = [(wl.config4_sweep(n), td) for n, td in ((16, "f32"), (32, "f32"), (64, "f32"), (128, "f32"), (192, "f32"),
+                                                    (64, "f64"), (128, "f64"), (192, "f64"), (256, "f64"))]
+    pts += [(wl.config1_tiny_film(), "f64"), (wl.config2_cube(64), "f32"), (wl.config3_thin_film(512), "f32"),
+            (wl.config5_inverse(), "f64")]
+    for w, prec in pts:
+        td = torch.float32 if prec == "f32" else torch.float64
+        s = 4 if prec == "f32" else 8
+        mesh, z, m = _dev_mesh(w, td)
+        N1, N2, N3 = w.n_cells
+        cells = N1 * N2 * N3
+        big = cells >= 128 ** 3
+        reps = 10 if big else 100
+        out = torch.empty_like(m)
+        l0 = mesh.nm_launch_count()
+        mesh.nm_llg_rhs(0.0, m, z, out)
+        per_rhs = mesh.nm_launch_count() - l0
+        t_rhs = _event_ms(lambda: mesh.nm_llg_rhs(0.0, m, z, out), reps)
+        y = m.clone()
+        dt = w.dt if w.dt > 0 else 1e-13
+        row = {"workload": w.name, "n_cells": [N1, N2, N3], "dtype": prec, "llg_rhs_ms": t_rhs,
+               "mcells_per_s": cells / t_rhs / 1e3, "launches_per_rhs": per_rhs,
+               "demag_path": mesh.nm_debug_demag_path(),
+               "rk4_step_ms": _event_ms(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, y, z), max(3, reps // 2))}
+        byts = sum(algorithmic_bytes(N1, N2, N3, s).values())
+        row["algorithmic_bytes"] = byts
+        row["frac"] = byts / (t_rhs * 1e-3) / 1e9 / peak
+        row["l2_resident"] = byts < 126e6
+        if w.name.startswith("config3"):
+            y.copy_(m)
+            row["dopri5_step_ms"] = _event_ms(lambda: mesh.nm_rk_step(nm.NM_DOPRI5, 1e-10, dt, y, z), 50)
+            row["host_amplitude_callback"] = True
+        if w.name.startswith("config5") or w.name.startswith("config1"):
+            a = m.clone()
+            u = torch.zeros(mesh.cell_shape_abi, dtype=td, device=m.device)
+            row["adjoint_rk4_step_ms"] = _event_ms(lambda: mesh.nm_adjoint_rk4_step(0.0, dt, y, a, u, z), 50)
+        rows.append(row)
+        mesh.close()
+        mesh.workspace = None
+        del m, out, y
+        torch.cuda.empty_cache()
+    return rows
+
+
+def run_config3(args):
+    """Config 3 as BASELINE.json states it: 512x512x1 cells, fp32, stripe pulse, Dormand-Prince with
+    rtol = atol = 1e-5 from 0 to args.config3 ns through drivers.integrate_dopri5 (one host read of the
+    error norm per trial step).  Prints wall time, step counts, |m| and the internal energy."""
+    import numpy as np
+    import torch
+
+    from paper_2411_11725_b200 import drivers
+    from paper_2411_11725_b200 import workloads as wl
+    w = wl.config3_thin_film(512)
+    td = torch.float32
+    mesh, z, y = _dev_mesh(w, td)
+
+    def energy():
+        H = mesh.nm_heff(0.0, y).double()
+        cnt = []
+        for N in w.n_cells:
+            c = torch.full((N + 1,), 2.0, dtype=torch.float64, device=y.device)
+            c[0] = c[-1] = 1.0
+            cnt.append(c)
+        L = cnt[2][:, None, None] * cnt[1][None, :, None] * cnt[0][None, None, :]
+        L = L * (4e-7 * np.pi * float(w.Ms) * float(np.prod(w.dx)) / 8.0)
+        return -0.5 * float((L * (y.double() * H).sum(0)).sum())
+
+    E0 = energy()
+    T = args.config3 * 1e-9
+    l0 = mesh.nm_launch_count()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    t, dt, acc, rej = drivers.integrate_dopri5(mesh, y, 0.0, T, 1e-13, z)
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    evals = 7 * (acc + rej)
+    print(json.dumps({
+        "what": "config 3 stated recipe", "n_cells": list(w.n_cells), "dtype": "f32", "t_end_s": t,
+        "wall_s": sec, "accepted": acc, "rejected": rej, "rhs_evaluations": evals, "last_dt_s": dt,
+        "ms_per_trial_step": 1e3 * sec / (acc + rej), "mcells_per_s": evals * float(np.prod(w.n_cells)) / sec / 1e6,
+        "gpu_launches": mesh.nm_launch_count() - l0,
+        "max_abs_norm_minus_1": float((y.double().norm(dim=0) - 1).abs().max()),
+        "finite": bool(torch.isfinite(y).all()), "energy_J": {"t0": E0, "t_end": energy()},
+        "rtol": 1e-5, "atol": 1e-5}))
 
 
 # --------------------------------------------------------------------------------------------------
@@ -282,6 +488,7 @@ def run_b200(args):
     sec = over_ranks(timed(step, args.steps))
     w1 = time.time()
     prof = mesh.nm_profile_end()
+    mesh_dropped = mesh.nm_profile_dropped()
     launches = mesh.nm_launch_count() - launches0
     clocks = sampler.stop(w0, w1) if sampler else None
     # the same K steps without the per-kernel events (what the events cost)
@@ -372,6 +579,7 @@ def run_b200(args):
 
     # ---- roofline of the dominant kernel (largest share of the timed region) ----
     peak, peak_src = peaks()
+    traffic, traffic_src = load_traffic(N, args.dtype)
     alg = algorithmic_bytes(N, N, N, s)
     shares = {k: v[0] for k, v in prof.items() if v[1] > 0}
     tot_ms = sum(shares.values())
@@ -380,8 +588,8 @@ def run_b200(args):
     achieved = alg[dom] / (dom_ms * 1e-3 / dom_n) / 1e9
     eval_bytes = sum(alg.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((N, args.dtype), {}).get(dom),
-                "traffic_source": "profiles/r1e_final.md (ncu --set full, per launch)", "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic.get(dom),
+                "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg[dom], "launches": dom_n,
                 "avg_launch_ms": dom_ms / dom_n, "share_of_step": dom_ms / tot_ms}
     # The z pass is as close to the FP32 pipe as to HBM: the same launch against the
@@ -429,6 +637,14 @@ def run_b200(args):
                       "adjoint_rhs_ms": 1e3 * t_adj,
                       "ms_per_step_without_kernel_events": 1e3 * sec_plain / args.steps},
     }
+    if not args.no_sweep and world == 1:
+        mesh.close()
+        mesh.workspace = None            # the bench mesh's 5.4 GB go back before the sweep's meshes come
+        buf.clear()
+        torch.cuda.empty_cache()
+        out["sweep"] = sweep_block(peak)
+    if out["kernels"] and mesh_dropped:
+        out["profile_dropped_launches"] = mesh_dropped
     if not args.no_cpu_baseline and world == 1:
         n = args.sample_grid or min(64, N)
         csteps = 3                  # about 15 s of CPU work at 64^3 on the GPU box's host
@@ -438,6 +654,12 @@ def run_b200(args):
             "kind": "oracle", "host_cores": os.cpu_count(),
             "sample": "%d oracle steps (rk4_step + adjoint_rhs) of the config-4 recipe at %d^3 cells, "
                       "%.1f s, tensor setup untimed" % (csteps, n, csec)}
+        # the same sample with the oracle's FFT calls on every host core
+        tsec, _, tthreads = oracle_run(n, args.dtype, csteps, 0, fft_workers=os.cpu_count() or 1)
+        out["cpu_baseline"]["threaded_fft"] = {
+            "value": EVALS_PER_STEP * ccells * csteps / tsec / 1e6, "unit": UNIT, "cores": tthreads,
+            "how": "numpy.fft.rfftn / irfftn served by scipy.fft(workers=%d); the rest of the oracle is "
+                   "single-threaded numpy; %.1f s" % (tthreads, tsec)}
     else:
         out["cpu_baseline"] = None
     print(json.dumps(out))
@@ -447,7 +669,11 @@ def run_b200(args):
 
 if __name__ == "__main__":
     a_ = parse()
-    if a_.impl == "reference":
+    if a_.traffic_from:
+        write_traffic(a_.traffic_from, a_.grid, a_.dtype)
+    elif a_.impl == "reference":
         run_reference(a_)
+    elif a_.config3 > 0:
+        run_config3(a_)
     else:
         run_b200(a_)

@@ -177,7 +177,9 @@ class Mesh:
     """nm_mesh handle plus the torch-allocated workspace block it lives in."""
 
     def __init__(self, n_cells, cell_size, dtype=torch.float32, device=0, terms=3, gamma=2.211e5,
-                 alpha=0.0, ku_axis=(0.0, 0.0, 1.0), Ms=None, A=None, Ku=None):
+                 alpha=0.0, ku_axis=(0.0, 0.0, 1.0), Ms=None, A=None, Ku=None, workspace=None):
+        """workspace: optional caller-made uint8 device tensor (256-byte aligned start, at least
+        nm_mesh_query_workspace bytes) to build the mesh in, instead of one allocated here."""
         self.dtype = dtype
         self.device = int(device)
         self.n_cells = tuple(int(v) for v in n_cells)
@@ -186,8 +188,14 @@ class Mesh:
         desc = make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis, Ms, A, Ku)
         nbytes = nm_mesh_query_workspace(desc)
         self.workspace_bytes = nbytes
-        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda:%d" % self.device)
-        base = (self.workspace.data_ptr() + 255) & ~255
+        if workspace is None:
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda:%d" % self.device)
+            base = (self.workspace.data_ptr() + 255) & ~255
+        else:
+            assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.numel() >= nbytes
+            assert workspace.data_ptr() % 256 == 0
+            self.workspace = workspace
+            base = workspace.data_ptr()
         h = ctypes.c_void_p()
         torch.cuda.synchronize(self.device)
         _check(lib().nm_mesh_create(ctypes.byref(h), ctypes.byref(desc), ctypes.c_void_p(base), nbytes))

@@ -16,5 +16,8 @@ Array conventions (the paper's multi-indices, Eqs. 8-10):
   cell scalar field    Ms[c1, c2, c3]     shape (N1, N2, N3)
   cell vector field    M[j, c1, c2, c3]   shape (3, N1, N2, N3)
 
+Reduced bases for films and rods (Eqs. 23-24): oracle/lowdim.py; nodal arrays keep
+three spatial axes, the reduced ones of extent 1 (Problem.basis = 2 or 1).
+
 Parity unpinned: none (every function below is pinned by tests/test_oracle_*.py).
 """

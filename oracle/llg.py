@@ -15,6 +15,7 @@ import numpy as np
 
 from . import demag as _demag
 from . import local_fields as _lf
+from . import lowdim as _ld
 from .mesh import lumped_mass, n_nodes
 
 TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN = 1, 2, 4, 8
@@ -33,6 +34,7 @@ class Problem:
     alpha: float = 0.0
     terms: int = TERM_EXCHANGE | TERM_DEMAG
     _Nt: np.ndarray = field(default=None, repr=False)
+    basis: int = 3            # dimensions the nodal basis varies in: 3, or 2 / 1 (Eqs. 23-24, oracle/lowdim.py)
 
     @staticmethod
     def uniform(n_cells, dx, Ms, A, Ku=0.0, **kw):
@@ -42,11 +44,11 @@ class Problem:
 
     @property
     def node_shape(self):
-        return n_nodes(self.n_cells)
+        return n_nodes(self.n_cells) if self.basis == 3 else _ld.node_shape(self.n_cells, self.basis)
 
     @property
     def L(self):
-        return lumped_mass(self.Ms, self.dx)
+        return lumped_mass(self.Ms, self.dx) if self.basis == 3 else _ld.lumped_mass(self.Ms, self.dx, self.basis)
 
     @property
     def Nt(self):
@@ -57,6 +59,8 @@ class Problem:
 
 def effective_field(p, m, h_ext=None, parts=False, demag_direct=False):
     """H_eff on nodes.  h_ext: nodal external field (3, nodes), a 3-vector, or None."""
+    if p.basis != 3:
+        return _effective_field_lowdim(p, m, h_ext, parts, demag_direct)
     L = p.L
     out = {}
     if p.terms & TERM_EXCHANGE:
@@ -70,6 +74,30 @@ def effective_field(p, m, h_ext=None, parts=False, demag_direct=False):
         out["zeeman"] = _lf.field_from_variation(_lf.variation_zeeman(h, p.Ms, p.dx), L)
     if p.terms & TERM_DEMAG:
         out["demag"] = _demag.demag_field(m, p.Ms, p.Nt, direct=demag_direct)
+    if parts:
+        return out
+    H = np.zeros_like(m, dtype=np.float64)
+    for v in out.values():
+        H = H + v
+    return H
+
+
+def _effective_field_lowdim(p, m, h_ext, parts, demag_direct):
+    """effective_field with the reduced basis of Eqs. (23)-(24): the same terms through oracle/lowdim.py."""
+    D = p.basis
+    L = p.L
+    out = {}
+    if p.terms & TERM_EXCHANGE:
+        out["exchange"] = _lf.field_from_variation(_ld.variation_exchange(m, p.A, p.dx, D), L)
+    if p.terms & TERM_ANISO:
+        out["aniso"] = _lf.field_from_variation(_ld.variation_uniaxial(m, p.Ku, p.ku_axis, p.dx, D), L)
+    if p.terms & TERM_ZEEMAN and h_ext is not None:
+        h = np.asarray(h_ext, dtype=np.float64)
+        if h.ndim == 1:
+            h = np.broadcast_to(h[:, None, None, None], m.shape)
+        out["zeeman"] = _lf.field_from_variation(_ld.variation_zeeman(h, p.Ms, p.dx, D), L)
+    if p.terms & TERM_DEMAG:
+        out["demag"] = _ld.demag_field(m, p.Ms, p.Nt, D, direct=demag_direct)
     if parts:
         return out
     H = np.zeros_like(m, dtype=np.float64)

@@ -74,6 +74,16 @@ typedef struct {
     double ku_axis[3];    /* anisotropy axis k, unit vector, global (reading C3(i)) */
     const void *Ms, *A, *Ku; /* device, cell-wise [N3][N2][N1], copied at create; NULL => scalar below */
     double Ms_scalar, A_scalar, Ku_scalar;
+    int basis;            /* dimensions the nodal basis varies in (Sec. III C):
+                             0 or 3  full 3-D nodal basis, (N1+1)(N2+1)(N3+1) nodes;
+                             2       film: basis functions constant along z (Eq. 23), needs N3 = 1;
+                                     nodal arrays are [3][1][N2+1][N1+1];
+                             1       rod: constant along y and z (Eq. 24), needs N2 = N3 = 1; nodal
+                                     arrays are [3][1][1][N1+1].
+                             The weak form is still integrated over the 3-D cells (element matrices
+                             without derivatives along the reduced axes, lumped mass V / 2^D per cell,
+                             node <-> cell averaging over the 2^D vertices of a cell).  Forward path only:
+                             the adjoint entry points return NM_EUNSUPPORTED on a reduced basis. */
 } nm_mesh_desc;
 
 /* Bytes of device workspace nm_mesh_create needs for this description (spectrum buffers, demag

@@ -39,7 +39,8 @@ class nm_mesh_desc(ctypes.Structure):
                 ("ku_axis", ctypes.c_double * 3),
                 ("Ms", ctypes.c_void_p), ("A", ctypes.c_void_p), ("Ku", ctypes.c_void_p),
                 ("Ms_scalar", ctypes.c_double), ("A_scalar", ctypes.c_double),
-                ("Ku_scalar", ctypes.c_double)]
+                ("Ku_scalar", ctypes.c_double),
+                ("basis", ctypes.c_int)]
 
 
 AMP_FUNC = ctypes.CFUNCTYPE(ctypes.c_double, ctypes.c_double, ctypes.c_void_p)
@@ -125,7 +126,7 @@ def _stream(device):
 
 
 def make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis=(0.0, 0.0, 1.0),
-              Ms=None, A=None, Ku=None):
+              Ms=None, A=None, Ku=None, basis=3):
     """Fill an nm_mesh_desc.  Ms/A/Ku: python scalar or a device tensor [N3][N2][N1]."""
     d = nm_mesh_desc()
     d.n_cells[:] = [int(v) for v in n_cells]
@@ -135,6 +136,7 @@ def make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis=(0
     d.terms = int(terms)
     d.gamma, d.alpha = float(gamma), float(alpha)
     d.ku_axis[:] = [float(v) for v in ku_axis]
+    d.basis = int(basis)
     keep = []
     for name, v in (("Ms", Ms), ("A", A), ("Ku", Ku)):
         if torch.is_tensor(v):
@@ -177,15 +179,17 @@ class Mesh:
     """nm_mesh handle plus the torch-allocated workspace block it lives in."""
 
     def __init__(self, n_cells, cell_size, dtype=torch.float32, device=0, terms=3, gamma=2.211e5,
-                 alpha=0.0, ku_axis=(0.0, 0.0, 1.0), Ms=None, A=None, Ku=None, workspace=None):
+                 alpha=0.0, ku_axis=(0.0, 0.0, 1.0), Ms=None, A=None, Ku=None, workspace=None, basis=3):
         """workspace: optional caller-made uint8 device tensor (256-byte aligned start, at least
         nm_mesh_query_workspace bytes) to build the mesh in, instead of one allocated here."""
         self.dtype = dtype
         self.device = int(device)
         self.n_cells = tuple(int(v) for v in n_cells)
-        self.node_shape_abi = (3, self.n_cells[2] + 1, self.n_cells[1] + 1, self.n_cells[0] + 1)
+        self.basis = int(basis) or 3
+        self.node_shape_abi = (3, self.n_cells[2] + 1 if self.basis > 2 else 1,
+                               self.n_cells[1] + 1 if self.basis > 1 else 1, self.n_cells[0] + 1)
         self.cell_shape_abi = (self.n_cells[2], self.n_cells[1], self.n_cells[0])
-        desc = make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis, Ms, A, Ku)
+        desc = make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis, Ms, A, Ku, basis)
         nbytes = nm_mesh_query_workspace(desc)
         self.workspace_bytes = nbytes
         if workspace is None:

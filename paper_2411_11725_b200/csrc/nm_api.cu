@@ -79,6 +79,12 @@ nm_status validate(const nm_mesh_desc *d)
         if (!(d->cell_size[i] > 0)) { nm_set_error("cell_size[%d] must be > 0", i); return NM_EINVAL; }
     }
     if (d->dtype != NM_F32 && d->dtype != NM_F64) { nm_set_error("bad dtype"); return NM_EINVAL; }
+    if (d->basis < 0 || d->basis > 3) { nm_set_error("basis = %d is not 0, 1, 2 or 3", d->basis); return NM_EINVAL; }
+    if ((d->basis == 2 && d->n_cells[2] != 1) || (d->basis == 1 && (d->n_cells[1] != 1 || d->n_cells[2] != 1))) {
+        nm_set_error("a %d-D basis needs one cell along the reduced axes (n_cells = %d x %d x %d)", d->basis,
+                     d->n_cells[0], d->n_cells[1], d->n_cells[2]);
+        return NM_EINVAL;
+    }
     if (d->terms == 0 || (d->terms & ~15u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
     if (!(d->gamma == d->gamma) || !(d->alpha == d->alpha)) { nm_set_error("gamma / alpha is NaN"); return NM_EINVAL; }
     if (d->terms & NM_TERM_ANISO) {
@@ -110,7 +116,12 @@ nm_status validate(const nm_mesh_desc *d)
 void make_geom(const nm_mesh_desc *d, NmGeom *g)
 {
     g->N1 = d->n_cells[0]; g->N2 = d->n_cells[1]; g->N3 = d->n_cells[2];
-    g->n1 = g->N1 + 1; g->n2 = g->N2 + 1; g->n3 = g->N3 + 1;
+    const int basis = d->basis == 0 ? 3 : d->basis;
+    g->n1 = g->N1 + 1;
+    g->n2 = basis >= 2 ? g->N2 + 1 : 1;
+    g->n3 = basis >= 3 ? g->N3 + 1 : 1;
+    g->ys = basis >= 2 ? g->n1 : 0;
+    g->zs = basis >= 3 ? g->n1 * g->n2 : 0;
     g->P1 = g->N1 > 1 ? 2 * g->N1 : 1;
     g->P2 = g->N2 > 1 ? 2 * g->N2 : 1;
     g->P3 = g->N3 > 1 ? 2 * g->N3 : 1;
@@ -548,6 +559,7 @@ void base_args(const nm_mesh *m, double t, const nm_zeeman *z, unsigned terms, N
     // separable kernel: uniform A and Ku (anisotropy off counts as uniform)
     const bool an_on = (terms & NM_TERM_ANISO) != 0;
     a->sep = (m->uni_A && (m->uni_Ku || !an_on)) ? 1 : 0;
+    if (m->g.zs == 0) a->sep = 0;                                // reduced basis: the 27-point kernel with zero strides
     if (m->dbg_node_path == 1) a->sep = 0;                       // test switch, read once at nm_mesh_create
     else if (m->dbg_node_path == 2 && a->sep) a->sep = 2;
     a->cex = (terms & NM_TERM_EXCHANGE) ? (T)(16.0 * m->desc.A_scalar / NM_MU0) : (T)0;
@@ -867,6 +879,15 @@ nm_status check_call(nm_mesh *mesh, const void *p0, const void *p1)
     return NM_OK;
 }
 
+nm_status check_adjoint(const nm_mesh *mesh)
+{
+    if (mesh && mesh->g.zs == 0) {
+        nm_set_error("the adjoint entry points serve the full 3-D basis only (basis = %d)", mesh->desc.basis);
+        return NM_EUNSUPPORTED;
+    }
+    return NM_OK;
+}
+
 } // namespace
 
 extern "C" nm_status nm_heff(nm_mesh *mesh, double t, const void *m, const nm_zeeman *zeeman, void *H_out,
@@ -935,6 +956,7 @@ extern "C" nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, 
                                         void *dudt_Ms_out, void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
+    NM_TRY(check_adjoint(mesh));
     if (!dadt_out) { nm_set_error("dadt_out is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     return mesh->f64 ? adjoint_eval<double>(mesh, t, (const double *)m, (const double *)a, zeeman,
@@ -949,6 +971,7 @@ nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, v
                             void *stream)
 {
     NM_TRY(check_call(mesh, m_inout, a_inout));
+    NM_TRY(check_adjoint(mesh));
     if (!u_inout) { nm_set_error("u_inout is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     NmStepKey key;
@@ -1001,6 +1024,7 @@ extern "C" nm_status nm_llg_adjoint_rhs_materials(nm_mesh *mesh, const void *m, 
                                                   void *dudt_Ku_out, void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
+    NM_TRY(check_adjoint(mesh));
     if (!dudt_A_out && !dudt_Ku_out) { nm_set_error("both outputs are NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     return mesh->f64 ? mat_grad<double>(mesh, (const double *)m, (const double *)a, (double *)dudt_A_out,
@@ -1013,6 +1037,7 @@ extern "C" nm_status nm_llg_adjoint_rhs_hext(nm_mesh *mesh, const void *m, const
                                              void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
+    NM_TRY(check_adjoint(mesh));
     if (!dudt_h_out) { nm_set_error("dudt_h_out is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     NM_CUDA_TRY(cudaMemsetAsync(dudt_h_out, 0, 3 * sizeof(double), st));

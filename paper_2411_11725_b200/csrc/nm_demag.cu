@@ -40,7 +40,8 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
     const int c3 = blockIdx.y;
     const int row0 = blockIdx.x * RX;
     const int n_lines = 3 * RX;
-    const long long plane = (long long)g.n1 * g.n2;
+    const long long plane = g.zs;      // 0 / g.ys = 0 along an axis the basis does not vary in (Eqs. 23-24):
+    const int rowp = g.ys;             // the four (dy, dz) nodes of a cell column then coincide pairwise
     // 1. cell averages, packed two reals per complex slot
     for (int idx = threadIdx.x; idx < n_lines * Lx; idx += blockDim.x) {
         const int n = idx % Lx;
@@ -50,7 +51,7 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
         T v0 = 0, v1 = 0;
         if (c2 < g.N2) {
             const T *base = fld + (long long)comp * g.nodes + (long long)c3 * plane +
-                            (long long)c2 * g.n1;
+                            (long long)c2 * rowp;
             const int c1 = 2 * n;
             if (c1 < g.N1) {
                 // column sums over the 4 (dy,dz) nodes at x = c1, c1+1, c1+2
@@ -58,7 +59,7 @@ k_x_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename Cx<T>::V *
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
                     const int x = c1 + d;
-                    col[d] = x <= g.N1 ? (base[x] + base[x + g.n1]) + (base[x + plane] + base[x + plane + g.n1])
+                    col[d] = x <= g.N1 ? (base[x] + base[x + rowp]) + (base[x + plane] + base[x + plane + rowp])
                                        : (T)0;
                 }
                 const long long cell = ((long long)c3 * g.N2 + c2) * g.N1 + c1;

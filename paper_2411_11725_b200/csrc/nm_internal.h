@@ -39,7 +39,10 @@ template <> struct NmVec2<double> { typedef double2 type; };
 // Geometry and workspace pointers handed to kernels by value.
 struct NmGeom {
     int N1, N2, N3;    // cells
-    int n1, n2, n3;    // nodes = cells + 1
+    int n1, n2, n3;    // stored node extents: cells + 1, or 1 along an axis the basis does not vary in
+    int ys, zs;        // element stride from a node to its +y / +z neighbour (n1, n1 n2), or 0 along a reduced
+                       // axis: the neighbour is the node itself, i.e. the state is uniform along that axis and
+                       // the 3-D operators applied to it are the reduced scheme (Eqs. 23-24)
     int P1, P2, P3;    // padded FFT lengths (2 N_d, or 1 if N_d == 1)
     int C1;            // complex outputs of the x transform: N1 + 1 (or 1)
     int C1p;           // row pitch of spectrum buffers, complex elements

@@ -154,8 +154,9 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
         const long long nn = g.nodes;
         const long long n = (long long)i3 * pl + p;
         const int ox[3] = {i1 > 0 ? -1 : 0, 0, i1 < g.N1 ? 1 : 0};
-        const int oy[3] = {i2 > 0 ? -g.n1 : 0, 0, i2 < g.N2 ? g.n1 : 0};
-        const int oz[3] = {i3 > 0 ? -pl : 0, 0, i3 < g.N3 ? pl : 0};
+        // strides g.ys / g.zs: 0 along an axis the basis does not vary in (the +1 neighbour is the node itself)
+        const int oy[3] = {i2 > 0 ? -g.ys : 0, 0, i2 < g.N2 ? g.ys : 0};
+        const int oz[3] = {i3 > 0 ? -g.zs : 0, 0, i3 < g.N3 ? g.zs : 0};
         // the 8 adjacent cells (bit 0: x, 1: y, 2: z; 0 = lower side)
         const bool vx[2] = {i1 > 0, i1 < g.N1}, vy[2] = {i2 > 0, i2 < g.N2}, vz[2] = {i3 > 0, i3 < g.N3};
         const int cx[2] = {i1 > 0 ? i1 - 1 : 0, i1 < g.N1 ? i1 : g.N1 - 1};

@@ -60,12 +60,12 @@ def np_dtype(torch_dtype):
     return np.float64 if torch_dtype == torch.float64 else np.float32
 
 
-def oracle_problem(w, dtype=np.float64):
+def oracle_problem(w, dtype=np.float64, basis=3):
     """oracle.llg.Problem with the materials rounded to the build precision."""
     from oracle import llg
     r = lambda v: wl.round_to(w.cell_array(v), dtype)
     p = llg.Problem(tuple(w.n_cells), tuple(float(v) for v in w.dx), r(w.Ms), r(w.A), r(w.Ku),
-                    tuple(w.ku_axis), float(w.gamma), float(w.alpha), int(w.terms))
+                    tuple(w.ku_axis), float(w.gamma), float(w.alpha), int(w.terms), basis=basis)
     if (w.terms & wl.TERM_DEMAG) and int(np.prod(w.n_cells)) >= 32 ** 3:
         p._Nt = oracle_tensor(w.n_cells, w.dx)
     return p
@@ -78,7 +78,7 @@ def oracle_zeeman(w, dtype=np.float64, h_static=None):
     hu = wl.round_to(np.asarray(w.h_uniform, dtype=np.float64), dtype)
     hp = wl.round_to(w.h_pulse, dtype) if w.h_pulse is not None else None
     hs = wl.round_to(h_static, dtype) if h_static is not None else None
-    shape = (3,) + w.node_shape
+    shape = tuple(np.asarray(w.m0).shape)          # the basis nodes (a reduced basis has fewer: _sides.reduce_nodal)
 
     def z(t):
         h = np.broadcast_to(hu[:, None, None, None], shape).copy()
@@ -102,14 +102,21 @@ def host(t):
     return wl.from_abi(t.detach().cpu().double().numpy())
 
 
-def gpu_mesh(w, torch_dtype, device=0):
+def reduce_nodal(a, D):
+    """A paper-order nodal array of a one-layer mesh restricted to the nodes of a D-dimensional basis
+    (Eqs. 23-24): the layer at index 0 of every reduced axis, kept as an axis of extent 1."""
+    sl = tuple(slice(None) if d < D else slice(0, 1) for d in range(3))
+    return np.ascontiguousarray(np.asarray(a)[(Ellipsis,) + sl])
+
+
+def gpu_mesh(w, torch_dtype, device=0, basis=3):
     from paper_2411_11725_b200 import binding as nm
     mat = {}
     for name in ("Ms", "A", "Ku"):
         v = getattr(w, name)
         mat[name] = float(v) if np.isscalar(v) else dev(v, torch_dtype, device)
     return nm.Mesh(w.n_cells, w.dx, dtype=torch_dtype, device=device, terms=w.terms, gamma=w.gamma,
-                   alpha=w.alpha, ku_axis=w.ku_axis, **mat)
+                   alpha=w.alpha, ku_axis=w.ku_axis, basis=basis, **mat)
 
 
 def gpu_zeeman(w, torch_dtype, device=0, h_static=None):

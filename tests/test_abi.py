@@ -38,7 +38,7 @@ def test_binding_struct_matches_header_layout(nm):
     # field order of nm_mesh_desc / nm_zeeman as declared in nm.h
     assert [f[0] for f in nm.nm_mesh_desc._fields_] == [
         "n_cells", "cell_size", "dtype", "device", "terms", "gamma", "alpha", "ku_axis", "Ms", "A",
-        "Ku", "Ms_scalar", "A_scalar", "Ku_scalar"]
+        "Ku", "Ms_scalar", "A_scalar", "Ku_scalar", "basis"]
     assert [f[0] for f in nm.nm_zeeman._fields_] == ["h_static", "h_pulse", "h_uniform", "amp", "user"]
 
 

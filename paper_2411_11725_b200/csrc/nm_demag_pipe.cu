@@ -689,25 +689,27 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
 // copy), the B side is 512 rows of 64 bytes, one per ky, 3 N3 rows apart: a 4-D tensor map over
 // B[kt P2 + ky][comp][c3][16 floats] moves them as two boxes of 256 rows.  Persistent CTAs, two per
 // SM; thread 0 keeps the copies of the neighbouring tiles in flight around the transform.
-struct PySmem {
+template <typename T> struct PySmem {
+    typedef typename VT<T>::V V;
     static constexpr int N = 256, P = 512;
-    static constexpr int A_ELEMS = N * TW, A_BYTES = A_ELEMS * 8;           // 16384
-    static constexpr int B_ELEMS = P * TW, B_BYTES = B_ELEMS * 8;           // 32768
-    static constexpr int SCR_BYTES = 16 * Team<16>::SCRATCH * 8;            // 35840
+    static constexpr int A_ELEMS = N * TW, A_BYTES = A_ELEMS * (int)sizeof(V);         // 16384 (fp32) / 32768
+    static constexpr int B_ELEMS = P * TW, B_BYTES = B_ELEMS * (int)sizeof(V);         // 32768 / 65536
+    static constexpr int SCR_BYTES = 16 * team_scratch<T, 16>() * (int)sizeof(V);      // 35840 / 70656
     // forward: two A stages in, one B tile out; inverse: one B stage in (reloaded as soon as it is read), one A tile out
     static constexpr int FWD_BYTES = 2 * A_BYTES + B_BYTES + SCR_BYTES + 64;
     static constexpr int INV_BYTES = B_BYTES + A_BYTES + SCR_BYTES + 64;
+    static constexpr int CTAS = sizeof(T) == 8 ? 1 : 2;                                // persistent CTAs per SM
 };
+static_assert(PySmem<double>::FWD_BYTES <= 227 * 1024, "k_py_fwd<double> shared memory exceeds the sm_100a per-CTA limit");
 
 // EMB: rows c2 >= n2v of an A tile were never written (embedded mesh) and enter as zeros.
-template <bool EMB>
-__global__ void __launch_bounds__(kPipeThreads, 2)
-k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
-         const float2 *__restrict__ wP, int n2v)
+template <typename T, bool EMB>
+__global__ void __launch_bounds__(kPipeThreads, PySmem<T>::CTAS)
+k_py_fwd(const typename VT<T>::V *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
+         const typename VT<T>::V *__restrict__ wP, int n2v)
 {
-    typedef float T;
-    typedef float2 V;
-    typedef PySmem S;
+    typedef typename VT<T>::V V;
+    typedef PySmem<T> S;
     constexpr int M = 16;
     extern __shared__ __align__(1024) unsigned char smem[];
     V *s_out = reinterpret_cast<V *>(smem);                                 // [P][8]
@@ -737,7 +739,7 @@ k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, 
     }
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     const int cin = j * TW + (w ^ swz(j));                  // A rows are swizzled by c2 = e, swz(j + 16 t) = swz(j)
     int n = 0;
     for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
@@ -775,13 +777,13 @@ k_py_fwd(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, 
     if (tid == 0) bulk_wait<0>();
 }
 
-__global__ void __launch_bounds__(kPipeThreads, 2)
-k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3, int nTiles, int kt0,
-         const float2 *__restrict__ wP)
+template <typename T>
+__global__ void __launch_bounds__(kPipeThreads, PySmem<T>::CTAS)
+k_py_inv(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict__ A, int N3, int nTiles, int kt0,
+         const typename VT<T>::V *__restrict__ wP)
 {
-    typedef float T;
-    typedef float2 V;
-    typedef PySmem S;
+    typedef typename VT<T>::V V;
+    typedef PySmem<T> S;
     constexpr int M = 16;
     extern __shared__ __align__(1024) unsigned char smem[];
     V *s_in = reinterpret_cast<V *>(smem);                                  // [P][8]
@@ -806,7 +808,7 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3
     if (tid == 0 && (int)blockIdx.x < nTiles) load_b(blockIdx.x);
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     const int cout = j * TW + (w ^ swz(j));
     int n = 0;
     for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
@@ -1109,8 +1111,8 @@ typedef CUresult (*NmEncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32
 nm_status nm_pipe_setup(nm_mesh *mesh)
 {
     mesh->fast.tmapB_ok = false;
-    if (!mesh->fast.on || mesh->f64 || !mesh->fast.pipe) return NM_OK;
-    const bool y8 = mesh->fast.M2 == 8 && mesh->g.N3 % 2 == 0;     // two planes per tile
+    if (!mesh->fast.on || !mesh->fast.pipe) return NM_OK;
+    const bool y8 = !mesh->f64 && mesh->fast.M2 == 8 && mesh->g.N3 % 2 == 0;     // two planes per tile (fp32 only)
     if (mesh->fast.M2 != 16 && !y8) return NM_OK;
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -1120,11 +1122,14 @@ nm_status nm_pipe_setup(nm_mesh *mesh)
         return NM_OK;                       // the non-pipelined y kernels serve instead
     }
     const NmGeom &g = mesh->g;
+    // a row = 8 complex = 16 reals = 64 bytes (fp32) or 128 bytes (fp64)
+    const cuuint64_t rowb = mesh->f64 ? 128 : 64;
     const cuuint64_t dims[4] = {16, (cuuint64_t)mesh->fast.F3, 3, (cuuint64_t)mesh->fast.NKT * g.P2};
-    const cuuint64_t strides[3] = {64, (cuuint64_t)mesh->fast.F3 * 64, (cuuint64_t)3 * mesh->fast.F3 * 64};
+    const cuuint64_t strides[3] = {rowb, (cuuint64_t)mesh->fast.F3 * rowb, (cuuint64_t)3 * mesh->fast.F3 * rowb};
     const cuuint32_t box[4] = {16, y8 ? 2u : 1u, 1, 256};       // M2 = 8: both planes of a tile, all 256 ky rows
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = ((NmEncodeTiledFn)fn)((CUtensorMap *)&mesh->fast.tmapB, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, mesh->bufB,
+    CUresult r = ((NmEncodeTiledFn)fn)((CUtensorMap *)&mesh->fast.tmapB,
+                                       mesh->f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, mesh->bufB,
                                        dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -1132,6 +1137,32 @@ nm_status nm_pipe_setup(nm_mesh *mesh)
         return NM_ECUDA;
     }
     mesh->fast.tmapB_ok = true;
+    return NM_OK;
+}
+
+template <typename T> static nm_status launch_py16(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st)
+{
+    typedef typename VT<T>::V V;
+    typedef PySmem<T> S;
+    const NmGeom &g = mesh->g;
+    const int nTiles = nkt * 3 * g.N3;
+    const int cap = S::CTAS * mesh->sm_count;
+    const int grid = nTiles < cap ? nTiles : cap;
+    if (!inverse) {
+        NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::FWD_BYTES));
+            kern<<<grid, kPipeThreads, S::FWD_BYTES, st>>>((const V *)mesh->bufA, mesh->fast.tmapB, g.N3, nTiles, kt0,
+                                                           (const V *)mesh->tw_y, g.N2);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_py_fwd<T, true>) : go(k_py_fwd<T, false>));
+    } else {
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::INV_BYTES));
+        NmLaunchScope sc(mesh, NM_K_Y_INV, st);
+        k_py_inv<T><<<grid, kPipeThreads, S::INV_BYTES, st>>>(mesh->fast.tmapB, (V *)mesh->bufA, g.N3, nTiles, kt0,
+                                                            (const V *)mesh->tw_y);
+    }
     return NM_OK;
 }
 
@@ -1160,24 +1191,6 @@ nm_status nm_pipe_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t 
         }
         return NM_OK;
     }
-    const int nTiles = nkt * 3 * g.N3;
-    const int grid = nTiles < 2 * mesh->sm_count ? nTiles : 2 * mesh->sm_count;
-    if (!inverse) {
-        NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
-        if (mesh->fast.embed) {
-            NM_CUDA_TRY(cudaFuncSetAttribute(k_py_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::FWD_BYTES));
-            k_py_fwd<true><<<grid, kPipeThreads, PySmem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3,
-                                                                         nTiles, kt0, (const float2 *)mesh->tw_y, g.N2);
-        } else {
-            NM_CUDA_TRY(cudaFuncSetAttribute(k_py_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::FWD_BYTES));
-            k_py_fwd<false><<<grid, kPipeThreads, PySmem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3,
-                                                                          nTiles, kt0, (const float2 *)mesh->tw_y, g.N2);
-        }
-    } else {
-        NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, PySmem::INV_BYTES));
-        NmLaunchScope sc(mesh, NM_K_Y_INV, st);
-        k_py_inv<<<grid, kPipeThreads, PySmem::INV_BYTES, st>>>(mesh->fast.tmapB, (float2 *)mesh->bufA, g.N3, nTiles, kt0,
-                                                              (const float2 *)mesh->tw_y);
-    }
-    return NM_OK;
+    if (mesh->f64) return launch_py16<double>(mesh, inverse, kt0, nkt, st);
+    return launch_py16<float>(mesh, inverse, kt0, nkt, st);
 }

@@ -45,6 +45,7 @@ CASES = [
     ("36x64x48 embedded, cell-wise materials", lambda: wl.varied_case((36, 64, 48), vacuum=True), "f32", 2),
     ("32x32x32 f64 (k_fy_*, k_fz_mid)", lambda: _cube((32, 32, 32)), "f64", 1),
     ("128x16x16 f64 (k_px_* f64, k_node_col f64)", lambda: _cube((128, 32, 16)), "f64", 1),
+    ("32x256x32 f64 (k_py_fwd / k_py_inv in fp64)", lambda: _cube((32, 256, 32)), "f64", 1),
 ]
 
 

@@ -434,6 +434,190 @@ k_pz_mid8(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nIte
 }
 
 
+// ---- z pass, fp64, 256 cells along z ---------------------------------------------------------------
+// One shared-memory region serves, in turn, the spectrum tile of a work item (3 x 256 x 8 complex
+// doubles, 96 KB) and the folded tensor rows of its eight columns (8 x 6 x 258 doubles, 96.75 KB):
+// a warp pulls its column of the tile into registers (3 x 16 complex doubles per thread, which is
+// what an fp64 thread can hold -- the stage twiddles live in a shared-memory table); the last warp
+// to have done so has the tensor rows copied over the tile while the forward transforms run; the last
+// warp to finish its products has the next tile copied over the tensor rows while the inverse
+// transforms run.  Results go straight from registers to B (16-byte stores, the eight warps of a CTA
+// fill the 128-byte rows between them), so no output tile is staged and both bulk copies have a whole
+// transform phase to land.  No CTA-wide barrier inside the loop: warps meet only at the two counters.
+struct Pz64Smem {
+    static constexpr int N = 256;
+    static constexpr int TILE_ELEMS = 3 * N * TW;                   // complex doubles
+    static constexpr int TILE_BYTES = TILE_ELEMS * 16;              // 98304
+    static constexpr int KZP = 258;                                 // tensor |kz| pitch (reals), even
+    static constexpr int TSLICE = 6 * KZP;                          // reals per column
+    static constexpr int TENS_BYTES = TW * TSLICE * 8;              // 99072, one bulk copy
+    static constexpr int REGION = TENS_BYTES > TILE_BYTES ? TENS_BYTES : TILE_BYTES;
+    static constexpr int OFF_SCR = REGION;
+    static constexpr int SCR_BYTES = 16 * Team<16>::SCRATCH64 * 16; // 70656
+    static constexpr int OFF_TW = OFF_SCR + SCR_BYTES;
+    static constexpr int TW_BYTES = 16 * 32 * 16;                   // [t'][lane]
+    static constexpr int OFF_BAR = OFF_TW + TW_BYTES;
+    static constexpr int BYTES = OFF_BAR + 32;
+};
+static_assert(Pz64Smem::BYTES <= 227 * 1024, "k_pz_mid64 shared memory exceeds the sm_100a per-CTA limit");
+static_assert(Pz64Smem::OFF_SCR % 128 == 0 && Pz64Smem::OFF_TW % 16 == 0 && Pz64Smem::OFF_BAR % 8 == 0, "alignment");
+
+// arrival on a CTA-local counter, ordered after this thread's earlier accesses and before its later
+// ones; returns the count before the arrival
+__device__ __forceinline__ unsigned arrive_count(unsigned *cnt)
+{
+    unsigned old;
+    asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(cnt)) : "memory");
+    return old;
+}
+
+template <bool EMB>
+__global__ void __launch_bounds__(kPipeThreads, 1)
+k_pz_mid64(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int nItems, int kt0,
+           const double2 *__restrict__ wP, int n3v)
+{
+    typedef double T;
+    typedef double2 V;
+    typedef Pz64Smem S;
+    constexpr int M = 16, N = 256, P = 512;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    V *s_B = reinterpret_cast<V *>(smem);
+    const T *s_T = reinterpret_cast<const T *>(smem);
+    V *s_scr = reinterpret_cast<V *>(smem + S::OFF_SCR);
+    V *s_tw = reinterpret_cast<V *>(smem + S::OFF_TW);
+    uint64_t *fullB = reinterpret_cast<uint64_t *>(smem + S::OFF_BAR);
+    uint64_t *fullT = fullB + 1;
+    unsigned *cnt = reinterpret_cast<unsigned *>(fullT + 1);        // [0]: columns in registers, [1]: products done
+
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, j = lane >> 1;
+    const int P2 = 2 * N2, K2 = N2 + 1;
+    const int G = gridDim.x;
+
+    auto tile_ptr = [&](int g, int sub) -> V * {
+        const int kyf = g % K2, ktl = g / K2;
+        const int ky = sub ? P2 - kyf : kyf;
+        return B + ((long long)ktl * P2 + ky) * S::TILE_ELEMS;
+    };
+    if (tid == 0) {
+        mbar_init(fullB, 1);
+        mbar_init(fullT, 1);
+        cnt[0] = cnt[1] = 0;
+        mbar_fence_init();
+    }
+    // stage twiddles of every lane: w_P^(j (2 t' + h)) (load_twiddles_h), conflict-free by lane
+    for (int q = tid; q < 16 * 32; q += kPipeThreads) {
+        const int tp = q >> 5, ln = q & 31;
+        s_tw[q] = wP[((ln >> 1) * (2 * tp + (ln & 1))) & (P - 1)];
+    }
+    __syncthreads();
+    if (tid == 0 && (int)blockIdx.x < nItems) {
+        mbar_expect_tx(fullB, S::TILE_BYTES);
+        bulk_load(s_B, tile_ptr(blockIdx.x, 0), S::TILE_BYTES, fullB);
+    }
+    const V *tws = s_tw + lane;
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH64;
+    const T *ts = s_T + w * S::TSLICE;
+    const int cw0 = w ^ swz(j);          // swz(j + 16 t) = swz(j)
+    uint32_t ph = 0;
+
+    for (int g = blockIdx.x; g < nItems; g += G) {
+        const int kyf = g % K2, kt = kt0 + g / K2;
+        const int nt = (kyf == 0 || kyf == N2) ? 1 : 2;
+        for (int sub = 0; sub < nt; ++sub, ph ^= 1) {
+            mbar_wait(fullB, ph);
+            const int cwj = cw0 ^ swz(sub ? P2 - kyf : kyf);     // rows of B are swizzled by c3 and by ky
+            const int coff = j * TW + cwj;                        // element (c, e = j + 16 t): + (c N + 16 t) TW
+            V a[3][16];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    a[c][t] = s_B[coff + (c * N + M * t) * TW];
+                    if (EMB && j + M * t >= n3v) a[c][t] = mk<T>((T)0, (T)0);
+                }
+            }
+            __syncwarp();
+            if (lane == 0 && (arrive_count(cnt) & 7) == 7) {     // every column is in registers: bring the tensor rows
+                mbar_expect_tx(fullT, S::TENS_BYTES);
+                bulk_load(smem, Tn + ((long long)kt * K2 + kyf) * TW * S::TSLICE, S::TENS_BYTES, fullT);
+            }
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, false>(a[c]);
+            }
+            dft16<T, false>(a[0]);
+            fwd_put_s<T, M, 32>(a[0], tws, scr, j);
+            dft16<T, false>(a[1]);
+            fwd_get<T, M>(a[0], scr, j);
+            dft16<T, false>(a[2]);
+            fwd_put_s<T, M, 32>(a[1], tws, scr, j);
+            dft16<T, false>(a[0]);
+            fwd_get<T, M>(a[1], scr, j);
+            fwd_put_s<T, M, 32>(a[2], tws, scr, j);
+            dft16<T, false>(a[1]);
+            fwd_get<T, M>(a[2], scr, j);
+            dft16<T, false>(a[2]);
+            // H^ = -N^ M^ ; rows of the folded tensor: sign -1 per folded odd axis
+            mbar_wait(fullT, ph);
+            const T sy = sub ? (T)-1 : (T)1;
+#pragma unroll
+            for (int s = 0; s < 16; ++s) {
+                const int rs = rev16(s);
+                const int kz = 2 * slot_freq<M>(j, s) + h;
+                const bool up = rs > 8 || (rs == 8 && (j | h) != 0);
+                const int kzf = up ? P - kz : kz;
+                const T sz = up ? (T)-1 : (T)1;
+                const T *tp = ts + kzf;
+                const T nxx = tp[0], nyy = tp[S::KZP], nzz = tp[2 * S::KZP];
+                const T nxy = sy * tp[3 * S::KZP], nxz = sz * tp[4 * S::KZP], nyz = sy * sz * tp[5 * S::KZP];
+                const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
+                const V hx = caxpy(nxz, mz, caxpy(nxy, my_, cscale(nxx, mx)));
+                const V hy = caxpy(nyz, mz, caxpy(nyy, my_, cscale(nxy, mx)));
+                const V hz = caxpy(nzz, mz, caxpy(nyz, my_, cscale(nxz, mx)));
+                a[0][s] = mk<T>(-hx.x, -hx.y);
+                a[1][s] = mk<T>(-hy.x, -hy.y);
+                a[2][s] = mk<T>(-hz.x, -hz.y);
+            }
+            __syncwarp();
+            if (lane == 0 && (arrive_count(cnt + 1) & 7) == 7) {  // every product is done: bring the next tile
+                int ng = g, nsub = sub + 1;
+                if (nsub >= nt) { ng = g + G; nsub = 0; }
+                if (ng < nItems) {
+                    mbar_expect_tx(fullB, S::TILE_BYTES);
+                    bulk_load(s_B, tile_ptr(ng, nsub), S::TILE_BYTES, fullB);
+                }
+            }
+            dft16<T, true>(a[0]);
+            inv_put<T, M>(a[0], scr, j);
+            dft16<T, true>(a[1]);
+            inv_get_s<T, M, 32>(a[0], tws, scr, j);
+            dft16<T, true>(a[2]);
+            inv_put<T, M>(a[1], scr, j);
+            dft16<T, true>(a[0]);
+            inv_get_s<T, M, 32>(a[1], tws, scr, j);
+            inv_put<T, M>(a[2], scr, j);
+            dft16<T, true>(a[1]);
+            inv_get_s<T, M, 32>(a[2], tws, scr, j);
+            dft16<T, true>(a[2]);
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, true>(a[c]);
+            }
+            V *out = tile_ptr(g, sub) + coff;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    V v = a[c][t];
+                    v = cadd(v, shfl1(v));
+                    if ((t >> 3) == h) out[(c * N + M * t) * TW] = v;
+                }
+            }
+        }
+    }
+}
+
 // ---- x passes ----------------------------------------------------------------------------------
 // Geometry shared by k_px_fwd / k_px_inv for N1 = 16 M: a CTA of 8 warps owns R = 2 LINES cell rows
 // (c2) of one cell plane c3; warp w transforms LINES/8 = 16/M complex lines, each packing the two
@@ -1012,7 +1196,8 @@ k_py_inv8(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N
 // ---- host side ----------------------------------------------------------------------------------
 bool nm_pipe_mid_ok(const nm_mesh *mesh)
 {
-    if (!mesh->fast.on || mesh->f64 || !mesh->fast.pipe) return false;
+    if (!mesh->fast.on || !mesh->fast.pipe) return false;
+    if (mesh->f64) return mesh->fast.M3 == 16 && mesh->fast.Kzp == Pz64Smem::KZP;
     return (mesh->fast.M3 == 16 && mesh->fast.Kzp == PzSmem::KZP) || (mesh->fast.M3 == 8 && mesh->fast.Kzp == Pz8Smem::KZP);
 }
 
@@ -1022,6 +1207,16 @@ nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     const int nItems = nkt * g.K2;
     const int grid = nItems < mesh->sm_count ? nItems : mesh->sm_count;
     NmLaunchScope sc(mesh, NM_K_MID, st);
+    if (mesh->f64) {
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pz64Smem::BYTES));
+            kern<<<grid, kPipeThreads, Pz64Smem::BYTES, st>>>((double2 *)mesh->bufB, (const double *)mesh->fast.Tn, mesh->fast.F2,
+                                                             nItems, kt0, (const double2 *)mesh->tw_z, g.N3);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_pz_mid64<true>) : go(k_pz_mid64<false>));
+        return NM_OK;
+    }
     if (mesh->fast.M3 == 8) {
         auto go = [&](auto kern) -> nm_status {
             NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pz8Smem::BYTES));

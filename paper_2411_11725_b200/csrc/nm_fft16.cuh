@@ -463,4 +463,34 @@ __device__ __forceinline__ void inv_get(typename VT<T>::V *a, const typename VT<
     }
 }
 
+// fwd_put / inv_get with the stage twiddles read from a shared-memory table instead of registers
+// (fp64: 16 complex twiddles are 64 registers a thread holding three lines does not have):
+// tws[t' * TWS] = the caller's twiddle t' of this lane (TW0 form, see load_twiddles_h).
+template <typename T, int M, int TWS>
+__device__ __forceinline__ void fwd_put_s(const typename VT<T>::V *a, const typename VT<T>::V *tws,
+                                          typename VT<T>::V *scr, int i)
+{
+    typedef typename VT<T>::V V;
+    const int l = i / M, j = i % M;
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+        const int tp = rev16(p);
+        scr[skew((l * 16 + tp) * M + j)] = cmul(a[p], tws[tp * TWS]);
+    }
+}
+template <typename T, int M, int TWS>
+__device__ __forceinline__ void inv_get_s(typename VT<T>::V *a, const typename VT<T>::V *tws,
+                                          const typename VT<T>::V *scr, int i)
+{
+    typedef typename VT<T>::V V;
+    const int l = i / M, j = i % M;
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+        const int tp = rev16(p);
+        a[p] = cmulc(scr[skew((l * 16 + tp) * M + j)], tws[tp * TWS]);
+    }
+}
+
 } // namespace nmf

@@ -62,7 +62,18 @@ def parse():
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
 KERNEL_CLASS = (("k_pz_mid", "mid"), ("k_fz_mid", "mid"), ("k_py_fwd", "y_fwd"), ("k_fy_fwd", "y_fwd"),
                 ("k_py_inv", "y_inv"), ("k_fy_inv", "y_inv"), ("k_px_fwd", "x_fwd"), ("k_px_inv", "x_inv"),
-                ("k_node", "node"))
+                ("k_node", "node"))     # split further by the epilogue mode, see node_class()
+
+
+def node_class(kernel_name):
+    """'node' / 'node_rk' / 'node_adj' from the epilogue mode in a node kernel's template arguments
+    (k_node_col<T, RY, CS, CM, ...>: CM 0-1 H / f, 2-4 Runge-Kutta stage, 5-6 adjoint passes)."""
+    import re
+    m = re.match(r"k_node_col<[^,]+,\s*\d+,\s*\d+,\s*(\d+)", kernel_name)
+    if not m:
+        return "node"
+    cm = int(m.group(1))
+    return "node" if cm <= 1 else "node_rk" if cm <= 4 else "node_adj"
 
 
 def csrc_hash():
@@ -103,6 +114,8 @@ def write_traffic(rep, N, dtype):
         cls = next((c for k, c in KERNEL_CLASS if name.startswith(k)), None)
         if cls is None:
             continue
+        if cls == "node":
+            cls = node_class(name)
         b = 0.0
         for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
             b += float(r[idx[col]].replace(",", "")) * scale[units[idx[col]]]
@@ -140,7 +153,14 @@ def algorithmic_bytes(N1, N2, N3, s):
     b = {
         "x_fwd": 3 * s * nodes + s * cells + spec_a,
         "x_inv": spec_a + 3 * s * cells,
-        "node": 3 * s * nodes + 2 * s * cells + 3 * s * cells + 3 * s * nodes,
+        # node pass: m (3 nodal) + H^cell (3 cell) + materials (2 cell) in, then what the epilogue moves:
+        "node": 3 * s * nodes + 5 * s * cells + 3 * s * nodes,                  # H or f out
+        # Runge-Kutta stage (a10), mean over the four stages of RK4: the start-of-step state and stage states
+        # in (0, 3, 3, 9 nodal arrays: stage 1 reads y0 as m), the next stage state out (3)
+        "node_rk": 3 * s * nodes + 5 * s * cells + (3.75 + 3) * s * nodes,
+        # adjoint passes (a11), mean of the two: pass 1 reads a, writes f, d, q (3 each) and w (1); pass 2
+        # reads d and writes da/dt
+        "node_adj": 3 * s * nodes + 5 * s * cells + (3 + 6.5) * s * nodes,
     }
     if N3 > 1:
         b["y_fwd"] = spec_a + spec_b
@@ -348,7 +368,7 @@ def sweep_block(peak):
                "mcells_per_s": cells / t_rhs / 1e3, "launches_per_rhs": per_rhs,
                "demag_path": mesh.nm_debug_demag_path(),
                "rk4_step_ms": _event_ms(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, y, z), max(3, reps // 2))}
-        byts = sum(algorithmic_bytes(N1, N2, N3, s).values())
+        byts = sum(v for k, v in algorithmic_bytes(N1, N2, N3, s).items() if k not in ("node_rk", "node_adj"))
         row["algorithmic_bytes"] = byts
         row["frac"] = byts / (t_rhs * 1e-3) / 1e9 / peak
         row["l2_resident"] = byts < 126e6
@@ -586,7 +606,7 @@ def run_b200(args):
     dom = max((k for k in shares if k in alg), key=lambda k: shares[k])
     dom_ms, dom_n = prof[dom]
     achieved = alg[dom] / (dom_ms * 1e-3 / dom_n) / 1e9
-    eval_bytes = sum(alg.values())
+    eval_bytes = sum(v for k, v in alg.items() if k not in ("node_rk", "node_adj"))   # one nm_llg_rhs
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic.get(dom),
                 "traffic_source": traffic_src, "peak_source": peak_src,

@@ -225,7 +225,8 @@ int nm_debug_demag_path(const nm_mesh *mesh);
  * nm_profile_end synchronises `stream` and writes, for each of the nm_profile_class_count() kernel classes, the summed device time in milliseconds and the number
  * of recorded launches to the two HOST arrays (each of nm_profile_class_count() entries).
  * nm_profile_class_name(i) names class i ("x_fwd", "y_fwd", "mid", "y_inv", "x_inv", "node",
- * "adj_cell", "lincomb", "other"). */
+ * "adj_cell", "lincomb", "other", "node_rk", "node_adj": the node pass is split by what its epilogue
+ * moves -- H or f alone, a Runge-Kutta stage, an adjoint pass). */
 long long nm_profile_dropped(const nm_mesh *mesh); /* launches since nm_profile_begin that were not timed */
 int nm_profile_class_count(void);
 const char *nm_profile_class_name(int cls);

@@ -16,9 +16,11 @@ import numpy as np
 from . import demag as _demag
 from . import local_fields as _lf
 from . import lowdim as _ld
+from . import more_terms as _mt
 from .mesh import lumped_mass, n_nodes
 
 TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN = 1, 2, 4, 8
+TERM_DMI, TERM_CUBIC = 16, 32      # further local terms of PAPER.md:171 (oracle/more_terms.py)
 
 
 @dataclass
@@ -35,6 +37,11 @@ class Problem:
     terms: int = TERM_EXCHANGE | TERM_DEMAG
     _Nt: np.ndarray = field(default=None, repr=False)
     basis: int = 3            # dimensions the nodal basis varies in: 3, or 2 / 1 (Eqs. 23-24, oracle/lowdim.py)
+    D: np.ndarray = None      # (N1,N2,N3) J/m^2, DMI constant (TERM_DMI)
+    dmi_kind: str = "bulk"    # "bulk" or "interfacial"
+    dmi_normal: int = 2       # film normal of the interfacial form
+    Kc: np.ndarray = None     # (N1,N2,N3) J/m^3, cubic anisotropy constant (TERM_CUBIC)
+    cubic_axes: tuple = ((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0))
 
     @staticmethod
     def uniform(n_cells, dx, Ms, A, Ku=0.0, **kw):
@@ -74,6 +81,10 @@ def effective_field(p, m, h_ext=None, parts=False, demag_direct=False):
         out["zeeman"] = _lf.field_from_variation(_lf.variation_zeeman(h, p.Ms, p.dx), L)
     if p.terms & TERM_DEMAG:
         out["demag"] = _demag.demag_field(m, p.Ms, p.Nt, direct=demag_direct)
+    if p.terms & TERM_DMI:
+        out["dmi"] = _lf.field_from_variation(_mt.variation_dmi(m, p.D, p.dx, p.dmi_kind, p.dmi_normal), L)
+    if p.terms & TERM_CUBIC:
+        out["cubic"] = _lf.field_from_variation(_mt.variation_cubic(m, p.Kc, p.cubic_axes, p.dx), L)
     if parts:
         return out
     H = np.zeros_like(m, dtype=np.float64)
@@ -84,6 +95,8 @@ def effective_field(p, m, h_ext=None, parts=False, demag_direct=False):
 
 def _effective_field_lowdim(p, m, h_ext, parts, demag_direct):
     """effective_field with the reduced basis of Eqs. (23)-(24): the same terms through oracle/lowdim.py."""
+    if p.terms & (TERM_DMI | TERM_CUBIC):
+        raise NotImplementedError("DMI / cubic anisotropy are written for the 3-D basis only")
     D = p.basis
     L = p.L
     out = {}

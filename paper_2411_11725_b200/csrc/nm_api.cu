@@ -454,7 +454,8 @@ extern "C" nm_status nm_mesh_destroy(nm_mesh *mesh)
 }
 
 static const char *const kClassNames[NM_K_COUNT] = {"x_fwd", "y_fwd", "mid", "y_inv", "x_inv",
-                                                    "node", "adj_cell", "lincomb", "other"};
+                                                    "node", "adj_cell", "lincomb", "other",
+                                                    "node_rk", "node_adj"};
 
 extern "C" int nm_profile_class_count(void) { return NM_K_COUNT; }
 

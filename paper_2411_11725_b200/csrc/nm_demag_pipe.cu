@@ -709,23 +709,30 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
     const int rg = tid / N, col = tid % N;                  // phase 1: row group (16 cell rows) and node column
     // small grids: the three components in three CTAs (gridDim.z = 3)
     const int comp_lo = gridDim.z == 3 ? blockIdx.z : 0, comp_hi = gridDim.z == 3 ? comp_lo + 1 : 3;
-    for (int comp = comp_lo; comp < comp_hi; ++comp) {
+    // z sums of component `comp`: 17 node rows of this thread's column, and (threads < R) the last node column;
+    // in fp64 (one CTA per SM) those of component comp + 1 are requested before component comp is
+    // transformed, so that they travel while the SM computes
+    T z[17], zlast = (T)0;
+    auto load_z = [&](int comp) {
         const T *base = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + rg * 16) * g.n1;
-        {
-            T z[17];
 #pragma unroll
-            for (int r = 0; r < 17; ++r)
-                z[r] = (!EMB || col < g.n1) ? base[(long long)r * g.n1 + col] + base[plane + (long long)r * g.n1 + col] : (T)0;
-#pragma unroll
-            for (int r = 0; r < 16; r += 2)
-                s_y[(rg * 8 + (r >> 1)) * G::YP + col] = mk<T>(z[r] + z[r + 1], z[r + 1] + z[r + 2]);
-            if (tid < R) {   // last node column n1 = N
-                const T *q = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + tid) * g.n1 + N;
-                const T v = (!EMB || N < g.n1) ? (q[0] + q[plane]) + (q[g.n1] + q[plane + g.n1]) : (T)0;
-                reinterpret_cast<T *>(s_y + (tid >> 1) * G::YP + N)[tid & 1] = v;
-            }
+        for (int r = 0; r < 17; ++r)
+            z[r] = (!EMB || col < g.n1) ? base[(long long)r * g.n1 + col] + base[plane + (long long)r * g.n1 + col] : (T)0;
+        if (tid < R) {   // last node column n1 = N
+            const T *q = fld + (long long)comp * g.nodes + (long long)c3 * plane + (long long)(r0 + tid) * g.n1 + N;
+            zlast = (!EMB || N < g.n1) ? (q[0] + q[plane]) + (q[g.n1] + q[plane + g.n1]) : (T)0;
         }
+    };
+    constexpr bool PREF = sizeof(T) == 8;                   // fp32 (two CTAs per SM, 128 registers): measured slower
+    if (PREF) load_z(comp_lo);
+    for (int comp = comp_lo; comp < comp_hi; ++comp) {
+        if (!PREF) load_z(comp);
+#pragma unroll
+        for (int r = 0; r < 16; r += 2)
+            s_y[(rg * 8 + (r >> 1)) * G::YP + col] = mk<T>(z[r] + z[r + 1], z[r + 1] + z[r + 2]);
+        if (tid < R) reinterpret_cast<T *>(s_y + (tid >> 1) * G::YP + N)[tid & 1] = zlast;
         __syncthreads();
+        if (PREF && comp + 1 < comp_hi) load_z(comp + 1);
         V a[16];
         const V *yl = s_y + line * G::YP + j;
 #pragma unroll

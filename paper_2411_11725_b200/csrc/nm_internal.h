@@ -16,8 +16,12 @@
 // kernel classes reported by nm_profile_end (order = NM_PROF_* of include/nm.h)
 enum NmKernelClass {
     NM_K_X_FWD = 0, NM_K_Y_FWD, NM_K_MID, NM_K_Y_INV, NM_K_X_INV, NM_K_NODE, NM_K_ADJ_CELL,
-    NM_K_LINCOMB, NM_K_OTHER, NM_K_COUNT
+    NM_K_LINCOMB, NM_K_OTHER, NM_K_NODE_RK, NM_K_NODE_ADJ, NM_K_COUNT
 };
+// the node pass by what its epilogue moves: H / f alone ("node"), a Runge-Kutta stage that also reads
+// the start-of-step state and earlier derivatives and writes the derivative and the next stage state
+// ("node_rk"), the two adjoint passes ("node_adj"); mode = NmLocalMode of nm_local.cuh
+inline int nm_node_class(int mode) { return mode <= 1 ? NM_K_NODE : mode == 2 ? NM_K_NODE_RK : NM_K_NODE_ADJ; }
 #define NM_MU0 (4.0e-7 * 3.14159265358979323846264338327950288)
 
 // ------------------------------------------------------------------------------------------------

@@ -821,7 +821,7 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
     if (a.sep && nodal_zee && fwd_mode && mesh->Zs) {
         // nodal Zeeman arrays with uniform A and Ku: smooth the field once, then the separable kernels
         {
-            NmLaunchScope sc(mesh, NM_K_NODE, st);
+            NmLaunchScope sc(mesh, NM_K_OTHER, st);
             const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
             k_zeeman_smooth<T><<<grid, kBlock, 0, st>>>(a, (T *)mesh->Zs);
         }
@@ -836,11 +836,11 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
         int zchunk;
         const dim3 grid = sep_grid(a.g, &zchunk);
         mesh->last_partials = (int)(grid.x * grid.y * grid.z);
-        NmLaunchScope sc(mesh, NM_K_NODE, st);
+        NmLaunchScope sc(mesh, nm_node_class(a.mode), st);
         if (a.ms_uni > 0) k_node_sep<T, true><<<grid, dim3(SX, SY), 0, st>>>(a, zchunk);
         else k_node_sep<T, false><<<grid, dim3(SX, SY), 0, st>>>(a, zchunk);
     } else {
-        NmLaunchScope sc(mesh, NM_K_NODE, st);
+        NmLaunchScope sc(mesh, nm_node_class(a.mode), st);
         const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
         mesh->last_partials = (int)(grid.x * grid.y);
         const bool extra = (a.terms & NM_TERM_ANISO) || nodal_zee;

@@ -530,7 +530,7 @@ nm_status launch_col_p(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
     NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     mesh->last_partials = (int)(grid.x * grid.y);
     {
-        NmLaunchScope sc(mesh, NM_K_NODE, st);
+        NmLaunchScope sc(mesh, nm_node_class(a.mode), st);
         kern<<<grid, col_threads(g), bytes, st>>>(a, zchunk);
     }
     NM_CUDA_TRY(cudaGetLastError());

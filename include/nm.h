@@ -54,7 +54,15 @@ typedef enum {
 } nm_status;
 
 /* field terms, OR-ed into nm_mesh_desc.terms */
-enum { NM_TERM_EXCHANGE = 1, NM_TERM_DEMAG = 2, NM_TERM_ANISO = 4, NM_TERM_ZEEMAN = 8 };
+enum { NM_TERM_EXCHANGE = 1, NM_TERM_DEMAG = 2, NM_TERM_ANISO = 4, NM_TERM_ZEEMAN = 8,
+       /* further local terms through the same weak form ("crystalline anisotropies, and both
+          symmetric and antisymmetric exchange interactions", readings F3) */
+       NM_TERM_DMI = 16,   /* antisymmetric exchange, density D sum T[a,d,b] m_a d_d m_b (nm_mesh_desc.dmi_kind) */
+       NM_TERM_CUBIC = 32  /* cubic anisotropy, density Kc (a1^2 a2^2 + a2^2 a3^2 + a3^2 a1^2), a_q = m . c_q */
+};
+typedef enum { NM_DMI_BULK = 0,        /* D m . curl m */
+               NM_DMI_INTERFACIAL = 1  /* D [m_n div m - (m . grad) m_n], n = nm_mesh_desc.dmi_normal */
+} nm_dmi_kind;
 
 typedef enum { NM_RK4 = 0, NM_DOPRI5 = 1 } nm_scheme;
 
@@ -84,6 +92,16 @@ typedef struct {
                              without derivatives along the reduced axes, lumped mass V / 2^D per cell,
                              node <-> cell averaging over the 2^D vertices of a cell).  Forward path only:
                              the adjoint entry points return NM_EUNSUPPORTED on a reduced basis. */
+    /* NM_TERM_DMI / NM_TERM_CUBIC (3-D basis; forward path only: nm_heff, nm_llg_rhs, nm_rk_step -- the
+       adjoint entry points return NM_EUNSUPPORTED with these terms on).  The element contributions are
+       integrated exactly (DMI: bilinear in the Q1 functions; cubic: 3-point Gauss per axis), summed into
+       the nodes and divided by the lumped mass, Eqs. (17)-(22). */
+    const void *D, *Kc;   /* device, cell-wise [N3][N2][N1], copied at create; NULL => scalar below */
+    double D_scalar;      /* J/m^2 */
+    double Kc_scalar;     /* J/m^3 */
+    int dmi_kind;         /* nm_dmi_kind */
+    int dmi_normal;       /* film normal axis (0, 1, 2) of NM_DMI_INTERFACIAL */
+    double cubic_axes[9]; /* rows c_1, c_2, c_3: one global orthonormal frame */
 } nm_mesh_desc;
 
 /* Bytes of device workspace nm_mesh_create needs for this description (spectrum buffers, demag

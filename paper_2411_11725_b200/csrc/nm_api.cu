@@ -85,7 +85,28 @@ nm_status validate(const nm_mesh_desc *d)
                      d->n_cells[0], d->n_cells[1], d->n_cells[2]);
         return NM_EINVAL;
     }
-    if (d->terms == 0 || (d->terms & ~15u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
+    if (d->terms == 0 || (d->terms & ~63u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
+    if (d->terms & (NM_TERM_DMI | NM_TERM_CUBIC)) {
+        if (d->basis != 0 && d->basis != 3) {
+            nm_set_error("NM_TERM_DMI / NM_TERM_CUBIC are written for the 3-D basis (basis = %d)", d->basis);
+            return NM_EUNSUPPORTED;
+        }
+        if ((d->terms & NM_TERM_DMI) && (d->dmi_kind < 0 || d->dmi_kind > 1 || d->dmi_normal < 0 || d->dmi_normal > 2)) {
+            nm_set_error("dmi_kind = %d / dmi_normal = %d out of range", d->dmi_kind, d->dmi_normal);
+            return NM_EINVAL;
+        }
+        if (d->terms & NM_TERM_CUBIC) {
+            const double *c = d->cubic_axes;
+            for (int q = 0; q < 3; ++q)
+                for (int r = q; r < 3; ++r) {
+                    const double dot = c[3 * q] * c[3 * r] + c[3 * q + 1] * c[3 * r + 1] + c[3 * q + 2] * c[3 * r + 2];
+                    if (std::fabs(dot - (q == r ? 1.0 : 0.0)) > 1e-9) {
+                        nm_set_error("cubic_axes must be three orthonormal rows");
+                        return NM_EINVAL;
+                    }
+                }
+        }
+    }
     if (!(d->gamma == d->gamma) || !(d->alpha == d->alpha)) { nm_set_error("gamma / alpha is NaN"); return NM_EINVAL; }
     if (d->terms & NM_TERM_ANISO) {
         const double *k = d->ku_axis;
@@ -175,6 +196,9 @@ size_t carve(nm_mesh *m, char *base)
     m->Uc[0] = c.take(g.cells * e);
     m->Uc[1] = c.take(g.cells * e);
     m->Zs = (m->desc.terms & NM_TERM_ZEEMAN) ? c.take(vec) : nullptr;
+    m->Dmi = (m->desc.terms & NM_TERM_DMI) ? c.take(g.cells * e) : nullptr;
+    m->Kcub = (m->desc.terms & NM_TERM_CUBIC) ? c.take(g.cells * e) : nullptr;
+    m->Xs = (m->desc.terms & (NM_TERM_DMI | NM_TERM_CUBIC)) ? c.take(vec) : nullptr;
     m->Hc1 = m->Hc2 = nullptr;
     m->Nreal = nullptr;
     m->fast.Tn = m->fast.wPx = nullptr;
@@ -405,10 +429,14 @@ extern "C" nm_status nm_mesh_create(nm_mesh **out, const nm_mesh_desc *desc, voi
             if ((s = set_material<double>(m, m->Ms, desc->Ms, desc->Ms_scalar, st)) != NM_OK) break;
             if ((s = set_material<double>(m, m->A, desc->A, desc->A_scalar, st)) != NM_OK) break;
             if ((s = set_material<double>(m, m->Ku, desc->Ku, desc->Ku_scalar, st)) != NM_OK) break;
+            if (m->Dmi && (s = set_material<double>(m, m->Dmi, desc->D, desc->D_scalar, st)) != NM_OK) break;
+            if (m->Kcub && (s = set_material<double>(m, m->Kcub, desc->Kc, desc->Kc_scalar, st)) != NM_OK) break;
         } else {
             if ((s = set_material<float>(m, m->Ms, desc->Ms, desc->Ms_scalar, st)) != NM_OK) break;
             if ((s = set_material<float>(m, m->A, desc->A, desc->A_scalar, st)) != NM_OK) break;
             if ((s = set_material<float>(m, m->Ku, desc->Ku, desc->Ku_scalar, st)) != NM_OK) break;
+            if (m->Dmi && (s = set_material<float>(m, m->Dmi, desc->D, desc->D_scalar, st)) != NM_OK) break;
+            if (m->Kcub && (s = set_material<float>(m, m->Kcub, desc->Kc, desc->Kc_scalar, st)) != NM_OK) break;
         }
         if ((s = nm_compute_sMs(m, st)) != NM_OK) break;
         if ((s = nm_pipe_setup(m)) != NM_OK) break;
@@ -433,7 +461,7 @@ extern "C" nm_status nm_mesh_create(nm_mesh **out, const nm_mesh_desc *desc, voi
         return s;
     }
     // the pointers in desc are not kept
-    m->desc.Ms = m->desc.A = m->desc.Ku = nullptr;
+    m->desc.Ms = m->desc.A = m->desc.Ku = m->desc.D = m->desc.Kc = nullptr;
     *out = m;
     return NM_OK;
 }
@@ -584,6 +612,32 @@ nm_status demag_part(nm_mesh *m, const T *fld, T *Hc, const T **Hc_arg, cudaStre
     return NM_OK;
 }
 
+// Field of the further local terms (NM_TERM_DMI, NM_TERM_CUBIC) of `fld` into the mesh's Xs array, which the
+// node kernel then adds to H.
+template <typename T> nm_status extra_part(nm_mesh *m, const T *fld, const T **hadd_arg, cudaStream_t st)
+{
+    if (!m->Xs) return NM_OK;
+    NmExtraArgs<T> x;
+    memset(&x, 0, sizeof(x));
+    x.g = m->g;
+    x.fld = fld;
+    x.Ms = (const T *)m->Ms;
+    x.D = (const T *)m->Dmi;
+    x.Kc = (const T *)m->Kcub;
+    x.out = (T *)m->Xs;
+    const double *dx = m->desc.cell_size;
+    const double V = dx[0] * dx[1] * dx[2];
+    x.V = (T)V;
+    x.mu0V8 = (T)(NM_MU0 * V / 8.0);
+    for (int d = 0; d < 3; ++d) x.idx[d] = (T)(1.0 / dx[d]);
+    x.dmi_kind = m->desc.dmi_kind;
+    x.dmi_normal = m->desc.dmi_normal;
+    for (int q = 0; q < 9; ++q) x.cax[q] = (T)m->desc.cubic_axes[q];
+    NM_TRY(nm_launch_extra<T>(m, x, st));
+    *hadd_arg = (const T *)m->Xs;
+    return NM_OK;
+}
+
 template <typename T>
 nm_status eval_simple(nm_mesh *m, double t, const T *fld, const nm_zeeman *z, T *out, int mode,
                       cudaStream_t st)
@@ -591,6 +645,7 @@ nm_status eval_simple(nm_mesh *m, double t, const T *fld, const nm_zeeman *z, T 
     NmLocalArgs<T> a;
     base_args<T>(m, t, z, m->desc.terms, &a);
     a.fld = fld;
+    NM_TRY(extra_part<T>(m, fld, &a.hadd, st));
     NM_TRY(demag_part<T>(m, fld, (T *)m->Hc1, &a.Hc, st));
     m->hc1_valid = a.Hc != nullptr;
     a.mode = mode;
@@ -606,6 +661,7 @@ nm_status eval_stage(nm_mesh *m, double t, const T *fld, const nm_zeeman *z, con
     NmLocalArgs<T> a;
     base_args<T>(m, t, z, m->desc.terms, &a);
     a.fld = fld;
+    NM_TRY(extra_part<T>(m, fld, &a.hadd, st));
     NM_TRY(demag_part<T>(m, fld, (T *)m->Hc1, &a.Hc, st));
     m->hc1_valid = a.Hc != nullptr;
     a.mode = NM_MODE_RK;
@@ -884,6 +940,10 @@ nm_status check_adjoint(const nm_mesh *mesh)
 {
     if (mesh && mesh->g.zs == 0) {
         nm_set_error("the adjoint entry points serve the full 3-D basis only (basis = %d)", mesh->desc.basis);
+        return NM_EUNSUPPORTED;
+    }
+    if (mesh && (mesh->desc.terms & (NM_TERM_DMI | NM_TERM_CUBIC))) {
+        nm_set_error("the adjoint entry points do not differentiate NM_TERM_DMI / NM_TERM_CUBIC");
         return NM_EUNSUPPORTED;
     }
     return NM_OK;

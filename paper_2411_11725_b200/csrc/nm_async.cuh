@@ -52,6 +52,27 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         : "memory");
 }
 
+// The same wait for a thread that has nothing else to do (a copy warp): between probes it sleeps, so
+// that its probe / branch instructions do not take issue slots from the warps that share its scheduler
+// (a failed try_wait returns within a few cycles; the arbiter favours the highest warp id).
+__device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    for (;;) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+        if (done) break;
+        __nanosleep(128);
+    }
+}
+
 // global -> shared, completion signalled on `bar` (bytes: multiple of 16; both addresses 16-B aligned)
 __device__ __forceinline__ void bulk_load(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *bar)
 {

@@ -113,7 +113,7 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
             const int nt = n_tiles(g);
             for (int sub = 0; sub < nt; ++sub, ++n) {
                 const int b = n % S::NBUF;
-                mbar_wait(doneB + b, (uint32_t)((n / S::NBUF) & 1));
+                mbar_wait_idle(doneB + b, (uint32_t)((n / S::NBUF) & 1));
                 bulk_store(tile_ptr(g, sub), s_B + b * S::TILE_ELEMS, S::TILE_BYTES);
                 bulk_commit();
                 bulk_wait_read<0>();          // the store has left the buffer: refill it with tile n + NBUF
@@ -325,9 +325,9 @@ k_pz_mid8(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nIte
         int n = 0;
         for (int g = blockIdx.x; g < nItems; g += G, ++n) {
             const int b = n % S::NBUF;
-            mbar_wait(freeT, (uint32_t)(n & 1));            // the products of item n are done
+            mbar_wait_idle(freeT, (uint32_t)(n & 1));       // the products of item n are done
             if (g + G < nItems) load_tensor(g + G);
-            mbar_wait(doneB + b, (uint32_t)((n / S::NBUF) & 1));
+            mbar_wait_idle(doneB + b, (uint32_t)((n / S::NBUF) & 1));
             const int nt = n_tiles(g);
             for (int sub = 0; sub < nt; ++sub)
                 bulk_store(tile_ptr(g, sub), s_B + b * S::SLOT_ELEMS + sub * S::TILE_ELEMS, S::TILE_BYTES);

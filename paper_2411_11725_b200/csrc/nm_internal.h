@@ -116,6 +116,8 @@ struct nm_mesh {
     void *Hc1, *Hc2;        // cell demag fields [3][cells]
     void *Q, *W;            // adjoint scratch: nodal vector, nodal scalar
     void *Zs;               // weak-form nodal Zeeman field of the current stage (nodal vector), or null
+    void *Dmi, *Kcub;       // cell scalars of NM_TERM_DMI / NM_TERM_CUBIC (real), or null
+    void *Xs;               // field of those terms at the current stage (nodal vector), or null
     void *K[7];             // RK stage derivatives (nodal vectors)
     void *Y[2];             // RK stage states
     void *Uc[2];            // cell scalars (adjoint RK)

@@ -243,6 +243,7 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
                 T hv = (a.kax[j] * an - ex[j]) * invL + hd[j] * invS;
                 if (zee_on) hv += a.hu[j];
                 if (zee_nodal) hv += a.mu0 * ze[j] * invL;
+                if (a.hadd) hv += a.hadd[j * nn + n];
                 H[j] = hv;
             }
         }
@@ -314,7 +315,7 @@ __global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a
             }
     const T sc = sms > 0 ? a.mu0 / (a.mu0V8 * sms) : (T)0;
 #pragma unroll
-    for (int j = 0; j < 3; ++j) Zs[j * nn + n] = sc * ze[j];
+    for (int j = 0; j < 3; ++j) Zs[j * nn + n] = sc * ze[j] + (a.hadd ? a.hadd[j * nn + n] : (T)0);   // + the field of the further local terms
 }
 
 // -------------------------------------------------------------------------------------------------
@@ -811,6 +812,121 @@ inline dim3 sep_grid(const NmGeom &g, int *zchunk)
     return dim3(gx, gy, nblk(g.n3, *zchunk));
 }
 
+
+// -------------------------------------------------------------------------------------------------
+// Further local terms through the weak form (readings F3), one thread per
+// node, the paper's element loop (Eqs. 19-20) gathered: for each of the (up to 8) cells c that contain
+// node n = c + i,
+//   DMI     dE_{n,a} += D_c sum_{d,b} T[a,d,b] g_d[b],   g_d = sum_{i'} (G^d[i,i'] - G^d[i',i]) m_{c+i'}
+//           with G^d[i,i'] - G^d[i',i] = (V / dx_d) (i'_d - i_d) M1[i_e,i'_e] M1[i_f,i'_f]  (M1 = 1/3, 1/6):
+//           T antisymmetric in (a, b): the Levi-Civita symbol (bulk) or T[n,d,d] = 1, T[d,d,n] = -1 (interfacial)
+//   cubic   dE_{n,j} += Kc_c V sum_q w_q phi_i(x_q) de/dm_j(m^h(x_q)),  3-point Gauss rule per axis (exact),
+//           e = a1^2 a2^2 + a2^2 a3^2 + a3^2 a1^2,  a_r = m . c_r,  de/dm = sum_r 2 a_r (|a|^2 - a_r^2) c_r
+// out_n = -dE_n / L_n, L_n = mu0 (V/8) (S Ms)_n (Eq. 22); 0 where (S Ms)_n = 0.
+template <typename T>
+__global__ void __launch_bounds__(kBlock) k_extra_local(const NmExtraArgs<T> a)
+{
+    const NmGeom &g = a.g;
+    const int pl = g.n1 * g.n2;
+    const int p = blockIdx.x * kBlock + threadIdx.x;
+    const int i3 = blockIdx.y;
+    if (p >= pl) return;
+    const int i2 = p / g.n1, i1 = p - i2 * g.n1;
+    const long long nn = g.nodes;
+    const long long n = (long long)i3 * pl + p;
+    const T third = (T)(1.0 / 3.0), sixth = (T)(1.0 / 6.0);
+    // 3-point Gauss-Legendre rule on [0, 1]
+    const T gx[3] = {(T)(0.5 - 0.5 * 0.77459666924148337704), (T)0.5, (T)(0.5 + 0.5 * 0.77459666924148337704)};
+    const T gw[3] = {(T)(5.0 / 18.0), (T)(8.0 / 18.0), (T)(5.0 / 18.0)};
+    T dE[3] = {0, 0, 0};
+    T sms = 0;
+    for (int ci = 0; ci < 8; ++ci) {
+        const int bx = ci & 1, by = (ci >> 1) & 1, bz = ci >> 2;     // 0: the cell below the node along that axis
+        const int c1 = i1 - 1 + bx, c2 = i2 - 1 + by, c3 = i3 - 1 + bz;
+        if (c1 < 0 || c1 >= g.N1 || c2 < 0 || c2 >= g.N2 || c3 < 0 || c3 >= g.N3) continue;
+        const long long c = ((long long)c3 * g.N2 + c2) * g.N1 + c1;
+        sms += a.Ms[c];
+        const int iv[3] = {1 - bx, 1 - by, 1 - bz};                  // local vertex index of n in cell c
+        const long long n0 = ((long long)c3 * g.n2 + c2) * g.n1 + c1; // vertex (0,0,0) of the cell
+        T mv[8][3];
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {
+            const long long q = n0 + (v & 1) + ((v >> 1) & 1) * g.n1 + (long long)(v >> 2) * pl;
+            mv[v][0] = a.fld[q];
+            mv[v][1] = a.fld[nn + q];
+            mv[v][2] = a.fld[2 * nn + q];
+        }
+        if (a.D) {
+            T gd[3][3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                gd[d][0] = gd[d][1] = gd[d][2] = 0;
+#pragma unroll
+                for (int v = 0; v < 8; ++v) {
+                    const int vv[3] = {v & 1, (v >> 1) & 1, v >> 2};
+                    const int sd = vv[d] - iv[d];
+                    if (sd == 0) continue;
+                    T w = (T)sd * a.V * a.idx[d];
+#pragma unroll
+                    for (int e = 0; e < 3; ++e)
+                        if (e != d) w *= (vv[e] == iv[e]) ? third : sixth;
+                    gd[d][0] += w * mv[v][0];
+                    gd[d][1] += w * mv[v][1];
+                    gd[d][2] += w * mv[v][2];
+                }
+            }
+            const T Dc = a.D[c];
+            if (a.dmi_kind == 0) {      // sum_{d,b} eps[a,d,b] g_d[b]
+                dE[0] += Dc * (gd[1][2] - gd[2][1]);
+                dE[1] += Dc * (gd[2][0] - gd[0][2]);
+                dE[2] += Dc * (gd[0][1] - gd[1][0]);
+            } else {
+                const int nrm = a.dmi_normal;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    if (d == nrm) continue;
+                    dE[nrm] += Dc * gd[d][d];       // T[n,d,d] = +1
+                    dE[d] -= Dc * gd[d][nrm];       // T[d,d,n] = -1
+                }
+            }
+        }
+        if (a.Kc) {
+            const T KV = a.Kc[c] * a.V;
+            for (int qz = 0; qz < 3; ++qz)
+                for (int qy = 0; qy < 3; ++qy)
+#pragma unroll
+                    for (int qx = 0; qx < 3; ++qx) {
+                        const T fx[2] = {(T)1 - gx[qx], gx[qx]}, fy[2] = {(T)1 - gx[qy], gx[qy]}, fz[2] = {(T)1 - gx[qz], gx[qz]};
+                        T mq[3] = {0, 0, 0};
+#pragma unroll
+                        for (int v = 0; v < 8; ++v) {
+                            const T ph = fx[v & 1] * fy[(v >> 1) & 1] * fz[v >> 2];
+                            mq[0] += ph * mv[v][0];
+                            mq[1] += ph * mv[v][1];
+                            mq[2] += ph * mv[v][2];
+                        }
+                        T al[3], S = 0;
+#pragma unroll
+                        for (int r = 0; r < 3; ++r) {
+                            al[r] = a.cax[3 * r] * mq[0] + a.cax[3 * r + 1] * mq[1] + a.cax[3 * r + 2] * mq[2];
+                            S += al[r] * al[r];
+                        }
+                        const T wq = KV * gw[qx] * gw[qy] * gw[qz] * fx[iv[0]] * fy[iv[1]] * fz[iv[2]];
+#pragma unroll
+                        for (int r = 0; r < 3; ++r) {
+                            const T cr = (T)2 * al[r] * (S - al[r] * al[r]) * wq;
+                            dE[0] += cr * a.cax[3 * r];
+                            dE[1] += cr * a.cax[3 * r + 1];
+                            dE[2] += cr * a.cax[3 * r + 2];
+                        }
+                    }
+        }
+    }
+    const T sc = sms > 0 ? (T)-1 / (a.mu0V8 * sms) : (T)0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) a.out[j * nn + n] = sc * dE[j];
+}
+
 } // namespace
 
 // ---- host launchers used by nm_api.cu -----------------------------------------------------------
@@ -851,6 +967,19 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;
 }
+
+template <typename T> nm_status nm_launch_extra(nm_mesh *mesh, const NmExtraArgs<T> &a, cudaStream_t st)
+{
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
+        k_extra_local<T><<<grid, kBlock, 0, st>>>(a);
+    }
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+template nm_status nm_launch_extra<float>(nm_mesh *, const NmExtraArgs<float> &, cudaStream_t);
+template nm_status nm_launch_extra<double>(nm_mesh *, const NmExtraArgs<double> &, cudaStream_t);
 
 int nm_node_blocks(const NmGeom &g)
 {

@@ -74,6 +74,19 @@ template <typename T> struct NmAdjCellArgs {
     T *dudt;
 };
 
+// Further local terms (NM_TERM_DMI, NM_TERM_CUBIC) evaluated per node into a nodal field that
+// the node kernels add to H (NmLocalArgs.hadd)
+template <typename T> struct NmExtraArgs {
+    NmGeom g;
+    const T *fld, *Ms, *D, *Kc;     // nodal m; cell-wise Ms, D, Kc (D / Kc null when the term is off)
+    T *out;                         // nodal vector: -(dE_dmi + dE_cubic) / L, 0 where (S Ms)_n = 0
+    T mu0V8, V;
+    T idx[3];                       // 1 / dx_d
+    int dmi_kind, dmi_normal;
+    T cax[9];                       // cubic frame, rows c_1, c_2, c_3
+};
+template <typename T> nm_status nm_launch_extra(nm_mesh *mesh, const NmExtraArgs<T> &a, cudaStream_t st);
+
 // host launchers defined in nm_local.cu
 template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st);
 // nm_node_col.cu: column-marching form of the separable kernel (cp.async stage ring)

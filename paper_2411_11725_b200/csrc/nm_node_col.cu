@@ -461,10 +461,10 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                     if (a.terms & NM_TERM_ZEEMAN) {
                         const T hz = a.hu[j];
                         Hp[j] = padd(Hp[j], UNI_MS ? pr1<T>(hz) : pr<T>(smsp.x > 0 ? hz : (T)0, smsp.y > 0 ? hz : (T)0));
-                        if (a.hadd)     // smoothed nodal Zeeman field (0 where S Ms = 0)
-                            Hp[j] = padd(Hp[j], pr<T>(rowlive[0] ? comp(a.hadd, j, nn)[nrow[0]] : (T)0,
-                                                      rowlive[1] ? comp(a.hadd, j, nn)[nrow[1]] : (T)0));
                     }
+                    if (a.hadd)     // smoothed nodal Zeeman field and / or the further local terms (0 where S Ms = 0)
+                        Hp[j] = padd(Hp[j], pr<T>(rowlive[0] ? comp(a.hadd, j, nn)[nrow[0]] : (T)0,
+                                                  rowlive[1] ? comp(a.hadd, j, nn)[nrow[1]] : (T)0));
                 }
                 // a9 (Eq. 1) on both rows: f = -gamma' m x H - alpha gamma' m x (m x H)
                 V fp[3];

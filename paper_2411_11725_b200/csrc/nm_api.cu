@@ -264,7 +264,8 @@ void init_host(nm_mesh *m, const nm_mesh_desc *d)
         // test switch, read here once (never on the evaluation path): NM_NODE_PATH = "generic" forces the
         // 27-point node kernel, "sep" k_node_sep
         const char *env = getenv("NM_NODE_PATH");
-        m->dbg_node_path = env && strcmp(env, "generic") == 0 ? 1 : env && strcmp(env, "sep") == 0 ? 2 : 0;
+        m->dbg_node_path = env && strcmp(env, "generic") == 0 ? 1 : env && strcmp(env, "sep") == 0 ? 2 :
+                           env && strcmp(env, "ring") == 0 ? 3 : 0;     // "ring": the cp.async form of the column kernel
     }
     nm_fast_plan(d, m->g, &m->fast);
     {

@@ -116,6 +116,16 @@ __device__ __forceinline__ void tensor_load_4d(void *smem_dst, const void *tmap,
         : "memory");
 }
 
+// 1-D tiled copy: `box` elements of a flat array starting at element c0 (any element index; elements
+// outside the array arrive as zeros)
+__device__ __forceinline__ void tensor_load_1d(void *smem_dst, const void *tmap, int c0, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.tensor.1d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3}], [%2];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(tmap), "r"(smem_u32(bar)), "r"(c0)
+                 : "memory");
+}
+
 __device__ __forceinline__ void tensor_store_4d(const void *tmap, const void *smem_src, int c0, int c1, int c2, int c3)
 {
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(tmap),

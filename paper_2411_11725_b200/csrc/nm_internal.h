@@ -128,7 +128,7 @@ struct nm_mesh {
     // materials given as scalars at create (enables the separable node kernel)
     bool uni_A, uni_Ku, uni_Ms;
     bool hc1_valid;
-    int dbg_node_path;      // NM_NODE_PATH at create: 0 automatic, 1 27-point kernel, 2 k_node_sep (tests)
+    int dbg_node_path;      // NM_NODE_PATH at create: 0 automatic, 1 27-point kernel, 2 k_node_sep, 3 column kernel fed by cp.async (tests)
     // per-launch timing (nm_profile_begin / nm_profile_end)
     bool prof_on;
     int prof_n;

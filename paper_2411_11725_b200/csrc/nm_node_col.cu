@@ -25,10 +25,12 @@
 // (mirrored) row / column indices; RY + 1 cell rows of each component of H^cell (and of Ms),
 // zero-filled outside the mesh -- is streamed by cp.async into a ring of CS stages, CS - 2 planes
 // ahead of the arithmetic, one CTA barrier per plane.  The epilogue is compiled per mode.
+#include "nm_async.cuh"
 #include "nm_local.cuh"
 #include "nm_pair.cuh"
 
 using namespace nmp;
+using namespace nma;
 
 namespace {
 
@@ -217,19 +219,48 @@ __host__ __device__ inline ColGeom col_geom(const NmGeom &g, bool has_hc, bool u
     return c;
 }
 
+// TMA-fed form (N1T > 0: the mesh has exactly N1T cells per row, known at compile time).  The RY + 2 node
+// rows a CTA needs of one component and plane are (RY + 2)(N1T + 1) contiguous elements of the nodal array:
+// the producer thread fetches them with one bulk copy (cp.async.bulk) and each cell row with another; a stage
+// completes on an mbarrier.  A bulk copy starts and ends on 16-byte boundaries and node rows do not (n1 is
+// odd), so the copy starts at the element index rounded down to a multiple of AL = 4 (fp32) or 2 (fp64) and
+// the rows sit `shift` < AL elements into the tile, a number that changes with the plane and the component.
+// (A 1-D tensor map was tried first: its boxes must start on 16-byte boundaries too, and fifteen 1 KB boxes
+// per plane were slower than three copies.)  Rows keep the array's own pitch n1 = N1T + 1 and there are no ghost columns: the end columns read themselves as
+// their missing neighbour (the same mirrored value), and the first / last CTA of the row axis copy the
+// mirrored ghost row inside the tile.
+template <typename T, int RY, int N1T> struct ColTma {
+    static constexpr int n1 = N1T + 1;
+    static constexpr int BOX = 256;                                  // elements per box
+    static constexpr int AL = 16 / (int)sizeof(T);                   // elements per 16 bytes: copies start and end on these
+    static constexpr int NB = ((RY + 2) * n1 + AL - 1 + BOX - 1) / BOX;
+    static constexpr int MS = NB * BOX;                              // elements per component tile (rows + shift, rounded)
+    static constexpr int CP = N1T + 4;                               // cell row pitch: N1T cells, zeros
+    static constexpr int OFF_C = 3 * MS + 4;                         // cell (row 0, column 0) of component 0; 4 zeros before
+    __host__ __device__ static constexpr int stage(int ncell) { return ((OFF_C + ncell * (RY + 1) * CP + 31) / 32) * 32; }
+};
+
 constexpr int CQ = 3;       // cell copies per thread and component (host checks cchunks <= CQ * threads)
 
-template <typename T, int RY, int CS, int CM, bool UNI_MS, int MAXT, int PITCH>
-__global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const NmLocalArgs<T> a, int zchunk)
+template <typename T, int RY, int CS, int CM, bool UNI_MS, int MAXT, int PITCH, int N1T>
+__global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2)
+k_node_col(const NmLocalArgs<T> a, int zchunk)
 {
     static_assert(RY == 2, "the plane arithmetic pairs the two node rows of a thread");
     typedef typename PairOf<T>::V V;
-    extern __shared__ __align__(16) unsigned char col_smem[];
+    typedef ColTma<T, RY, N1T> TM;
+    constexpr bool TMA = N1T > 0;
+    extern __shared__ __align__(1024) unsigned char col_smem[];
     T *sm = reinterpret_cast<T *>(col_smem);
     const NmGeom &g = a.g;
-    const int n1 = g.n1, n2 = g.n2, N1 = g.N1;
+    const int n1 = TMA ? TM::n1 : g.n1, n2 = g.n2, N1 = TMA ? N1T : g.N1;
     const bool has_hc = a.Hc != nullptr;
-    const ColGeom cg = col_geom<T, RY, PITCH>(g, has_hc, UNI_MS);
+    ColGeom cg = col_geom<T, RY, PITCH>(g, has_hc, UNI_MS);
+    if (TMA) {          // the same names, the TMA tile geometry
+        cg.CP = TM::CP;
+        cg.moff_cells = TM::OFF_C;
+        cg.stage = TM::stage(cg.ncell);
+    }
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int r0 = blockIdx.x * RY;                       // first node row of the CTA
     const int z0 = blockIdx.y * zchunk, z1 = min(z0 + zchunk, g.n3);
@@ -239,6 +270,22 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
     constexpr bool RK = CM == CM_RK0 || CM == CM_RKS || CM == CM_RKN;
 
     for (int q = tid; q < CS * cg.stage; q += nthr) sm[q] = (T)0;
+    // TMA: per stage a transaction barrier (the copies have landed) and a barrier the consumer warps arrive on
+    // (they have left the stage); warp NW, past the last node column, is the producer
+    uint64_t *full = reinterpret_cast<uint64_t *>(sm + CS * cg.stage);
+    uint64_t *empty = full + CS;
+    const int NW = (n1 + 31) / 32;
+    const bool producer = TMA && tid >= NW * 32;
+    if (TMA) {
+        if (tid == 0) {
+            for (int q = 0; q < CS; ++q) {
+                mbar_init(full + q, 1);
+                mbar_init(empty + q, NW);
+            }
+            mbar_fence_init();
+        }
+        fence_async_smem();                                 // the zeros are written before any bulk copy lands
+    }
     __syncthreads();
 
     // ---- what this thread copies every plane (fixed offsets; only the plane base moves) ----------
@@ -266,7 +313,49 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
         }
     }
     const unsigned sm_base = smem_addr(sm);
+    // TMA: rows of the cell tile that exist for this CTA (uniform), the same on every plane
+    int crow_lo = 0, crow_hi = -1;
+    if (TMA && has_hc) {
+        crow_lo = r0 - 1 < 0 ? 1 : 0;
+        crow_hi = min(RY, g.N2 - r0);                      // tile row `row` is cell row r0 - 1 + row < N2
+    }
     auto issue = [&](int k, int slot) {
+        if (TMA) {      // the producer thread: three copies of node rows, one per cell row
+            T *sb = sm + slot * cg.stage;
+            const int kc = min(max(k, 0), g.n3 - 1);
+            const bool cv = has_hc && k - 1 >= 0 && k - 1 < g.N3;
+            const int E = 3 * (int)nn;
+            int e0[3], len[3], off[3], total = cv ? (crow_hi - crow_lo + 1) * (UNI_MS ? 3 : 4) * N1T : 0;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                // rows r0 - 1 .. r0 + RY of component j, plane kc: (RY + 2) n1 contiguous elements from the 16-byte
+                // boundary below their start, clipped to the array (what is clipped belongs to rows that do not
+                // exist, except the last elements of the array when its length is not a multiple of 4)
+                e0[j] = (j * (int)nn + kc * (int)pl + (r0 - 1) * TM::n1) & ~(TM::AL - 1);
+                len[j] = ((RY + 2) * TM::n1 + 2 * (TM::AL - 1)) & ~(TM::AL - 1);
+                off[j] = 0;
+                if (e0[j] < 0) { off[j] = -e0[j]; len[j] += e0[j]; e0[j] = 0; }
+                if (e0[j] + len[j] > E) {
+                    len[j] = (E - e0[j]) & ~(TM::AL - 1);
+                    for (int q = e0[j] + len[j]; q < E; ++q) sb[j * TM::MS + off[j] + q - e0[j]] = a.fld[q];
+                }
+                total += len[j];
+            }
+            mbar_expect_tx(full + slot, (uint32_t)(total * sizeof(T)));      // releases the stores above with it
+#pragma unroll
+            for (int j = 0; j < 3; ++j)
+                bulk_load(sb + j * TM::MS + off[j], a.fld + e0[j], (uint32_t)(len[j] * sizeof(T)), full + slot);
+            if (cv) {
+                const size_t kc2 = (size_t)(k - 1) * cpl;
+                for (int j = 0; j < (UNI_MS ? 3 : 4); ++j) {
+                    const T *src = (j < 3 ? comp(a.Hc, j, nc) : a.Ms) + kc2;
+                    for (int row = crow_lo; row <= crow_hi; ++row)
+                        bulk_load(sb + TM::OFF_C + (j * (RY + 1) + row) * TM::CP, src + (size_t)(r0 - 1 + row) * N1T,
+                                  (uint32_t)(N1T * sizeof(T)), full + slot);
+                }
+            }
+            return;
+        }
         const unsigned sbase = sm_base + (unsigned)(slot * cg.stage) * (unsigned)sizeof(T);
         if (mcopy) {
             const unsigned kc = (unsigned)min(max(k, 0), g.n3 - 1) * pl;
@@ -338,22 +427,65 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
     double err2 = 0.0;
 
     const int kstart = max(z0 - 1, 0), kend = z1;         // plane kend = n3 is fetched clamped and weighted 0
+    if (!TMA) {
 #pragma unroll
-    for (int s = 0; s < CS - 2; ++s) {
-        if (kstart + s <= kend) issue(kstart + s, s);
-        cp_commit();
+        for (int s = 0; s < CS - 2; ++s) {
+            if (kstart + s <= kend) issue(kstart + s, s);
+            cp_commit();
+        }
+    } else if (tid == NW * 32) {
+        // producer: plane k goes into stage (k - kstart) % CS as soon as every consumer warp has left the plane
+        // that used it last; the consumers hold two stages (planes k - 1 and k), so the copies run CS - 2 ahead
+        int it = 0;
+        for (int k = kstart; k <= kend; ++k, ++it) {
+            const int sl = it % CS;
+            if (it >= CS) mbar_wait_idle(empty + sl, (uint32_t)((it / CS - 1) & 1));
+            issue(k, sl);
+        }
     }
+    // TMA: x neighbours of the end columns are the columns themselves (mirrored ghosts); tile rows whose node
+    // row does not exist are copied from the mirrored one when the stage has landed (first / last CTA only)
+    const int xlo = tid > 0 ? -1 : 0, xhi = tid < n1 - 1 ? 1 : 0;
+    const bool edge = TMA && (r0 == 0 || r0 + RY > n2 - 1);
     int slot = 0;
+    int shc[3] = {0, 0, 0}, shp[3] = {0, 0, 0};            // TMA: shift of the rows in the tiles of plane k and of plane k - 1
+    unsigned fphase = 0;                                   // bit q: parity of the next completion of stage q
     unsigned nbase = (unsigned)(kstart - 1) * pl + (unsigned)r0 * n1 + tid;    // node (z = k - 1, row r0, column tid); unused while z < 0
-    for (int k = kstart; k <= kend; ++k, nbase += pl) {
-        cp_wait<CS - 3>();
-        __syncthreads();
-        {
+    for (int k = producer ? kend + 1 : kstart; k <= kend; ++k, nbase += pl) {
+        if (TMA) {
+            const int kc = min(max(k, 0), g.n3 - 1);
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                shp[j] = shc[j];
+                shc[j] = (j * (int)nn + kc * (int)pl + (r0 - 1) * TM::n1) & (TM::AL - 1);
+            }
+            mbar_wait(full + slot, (fphase >> slot) & 1u);
+            fphase ^= 1u << slot;
+        } else {
+            cp_wait<CS - 3>();
+            __syncthreads();
             const int kn = k + CS - 2;
             int sn = slot + CS - 2;
             if (sn >= CS) sn -= CS;
             if (kn <= kend) issue(kn, sn);
             cp_commit();
+        }
+        if (edge) {
+            T *sb = sm + slot * cg.stage;
+            if (live) {
+#pragma unroll
+                for (int r = 0; r < RY + 2; ++r) {
+                    const int i2 = r0 - 1 + r;
+                    const int ic = min(max(i2, 0), n2 - 1);
+                    if (ic != i2) {
+#pragma unroll
+                        for (int j = 0; j < 3; ++j)
+                            sb[j * TM::MS + shc[j] + r * TM::n1 + tid] = sb[j * TM::MS + shc[j] + (ic - (r0 - 1)) * TM::n1 + tid];
+                    }
+                }
+            }
+            fence_async_smem();
+            asm volatile("bar.sync 1, %0;" ::"r"(NW * 32) : "memory");     // the consumer warps only
         }
         const int z = k - 1;
         const bool zout = z >= z0 && z < z1;
@@ -379,6 +511,8 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
         const T eR_M = a.cex * gLp;
         const T wR_out = gRm * sixth, w_P = dzk - (gLk + gRk) * sixth, w_M = gLp * sixth;
         const T *st = sm + slot * cg.stage;
+        // TMA: a cell plane that does not exist is not fetched (the stage keeps older, finite values): weight 0
+        const T cTk = (TMA && !(k - 1 >= 0 && k - 1 < g.N3)) ? (T)0 : cT;
         if (live) {
             V Tn[3];
             if (has_hc) {
@@ -400,7 +534,7 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                         const T *crow = cb + (j * (RY + 1) + cr) * cg.CP;
                         X[cr] = UNI_MS ? crow[-1] + crow[0] : ml[cr] * crow[-1] + mr[cr] * crow[0];
                     }
-                    Tn[j] = pmul(pr1<T>(cT), padd(pr<T>(X[0], X[1]), pr<T>(X[1], X[2])));
+                    Tn[j] = pmul(pr1<T>(cTk), padd(pr<T>(X[0], X[1]), pr<T>(X[1], X[2])));
                 }
             } else {
                 Tn[0] = Tn[1] = Tn[2] = pr1<T>((T)0);
@@ -409,13 +543,22 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
             V Gout[3];
 #pragma unroll
             for (int j = 0; j < 3; ++j) {
-                const T *t = st + j * (RY + 2) * cg.MP + tid;     // columns tid, tid + 1, tid + 2 = i1 - 1, i1, i1 + 1
                 T c[RY + 2], sx[RY + 2];
+                if (TMA) {
+                    const T *t = st + j * TM::MS + shc[j] + tid;  // rows at the array's pitch, no ghost columns
 #pragma unroll
-                for (int r = 0; r < RY + 2; ++r) {
-                    const T *row = t + r * cg.MP;
-                    c[r] = row[1];
-                    sx[r] = row[0] + row[2];
+                    for (int r = 0; r < RY + 2; ++r) {
+                        c[r] = t[r * TM::n1];
+                        sx[r] = (t + xlo)[r * TM::n1] + (t + xhi)[r * TM::n1];
+                    }
+                } else {
+                    const T *t = st + j * (RY + 2) * cg.MP + tid; // columns tid, tid + 1, tid + 2 = i1 - 1, i1, i1 + 1
+#pragma unroll
+                    for (int r = 0; r < RY + 2; ++r) {
+                        const T *row = t + r * cg.MP;
+                        c[r] = row[1];
+                        sx[r] = row[0] + row[2];
+                    }
                 }
                 const V CC = pr<T>(c[1], c[2]), SXc = pr<T>(sx[1], sx[2]);
                 const V ax = pfma(CC, pr1<T>((T)2), pneg(SXc));
@@ -438,12 +581,13 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                 const T izf = (z > 0 && z < g.N3) ? (T)0.5 : (T)1;             // 1 / (gL + gR) of output z
                 int sp = slot - 1;
                 if (sp < 0) sp += CS;
-                const T *sprev = sm + sp * cg.stage + tid + 1;                // centre column of plane z
+                const T *sprev = sm + sp * cg.stage + tid + (TMA ? 0 : 1);    // centre column of plane z
                 const unsigned nrow[RY] = {nbase, nbase + (unsigned)n1};
                 V mcp[3];
 #pragma unroll
                 for (int j = 0; j < 3; ++j)
-                    mcp[j] = pr<T>(sprev[(j * (RY + 2) + 1) * cg.MP], sprev[(j * (RY + 2) + 2) * cg.MP]);
+                    mcp[j] = TMA ? pr<T>(sprev[j * TM::MS + shp[j] + TM::n1], sprev[j * TM::MS + shp[j] + 2 * TM::n1])
+                                 : pr<T>(sprev[(j * (RY + 2) + 1) * cg.MP], sprev[(j * (RY + 2) + 2) * cg.MP]);
                 V smsp, invp;
                 if (UNI_MS) {
                     invp = pmul(pr<T>(inv_xy[0], inv_xy[1]), pr1<T>(izf));
@@ -491,9 +635,13 @@ __global__ void __launch_bounds__(MAXT, sizeof(T) == 8 ? 1 : 2) k_node_col(const
                 }
             }
         }
+        if (TMA && k > kstart) {          // plane k - 1 is no longer needed by this warp
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(empty + (slot == 0 ? CS - 1 : slot - 1));
+        }
         if (++slot == CS) slot = 0;
     }
-    cp_wait<0>();
+    if (!TMA) cp_wait<0>();
     if (CM == CM_RKN) {
         if (a.rk.want_err) {
             const double s = block_sum_c(err2, nthr);
@@ -526,7 +674,7 @@ nm_status launch_col_p(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
     const size_t bytes = (size_t)CS * cg.stage * sizeof(T);
     const int zchunk = col_zchunk(g);
     const dim3 grid((g.n2 + kRY - 1) / kRY, (g.n3 + zchunk - 1) / zchunk);
-    auto kern = k_node_col<T, kRY, CS, CM, UNI_MS, kMaxT, PITCH>;
+    auto kern = k_node_col<T, kRY, CS, CM, UNI_MS, kMaxT, PITCH, 0>;
     NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     mesh->last_partials = (int)(grid.x * grid.y);
     {
@@ -537,9 +685,45 @@ nm_status launch_col_p(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
     return NM_OK;
 }
 
+// ---- TMA-fed form: N1 = 128 or 256 cells per row ----------------------------------------------------------
+// which compile-time row length serves this launch (0: the cp.async form)
+template <typename T> int col_tma_n1(const nm_mesh *mesh, const NmLocalArgs<T> &a)
+{
+    if (mesh->dbg_node_path == 3) return 0;                // NM_NODE_PATH=ring at nm_mesh_create (tests, measurements)
+    const NmGeom &g = a.g;
+    if (g.N1 != 128 && g.N1 != 256) return 0;
+    if (3 * g.nodes >= (1ll << 31) || (((uintptr_t)a.fld) & 15)) return 0;
+    if (a.Hc && ((((uintptr_t)a.Hc) | ((uintptr_t)a.Ms)) & 15)) return 0;
+    return g.N1;
+}
+
+template <typename T, int CM, bool UNI_MS, int N1T>
+nm_status launch_col_tma(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
+{
+    constexpr int CS = ColStages<T>::CS;
+    typedef ColTma<T, kRY, N1T> TM;
+    const NmGeom &g = a.g;
+    const int ncell = a.Hc ? (UNI_MS ? 3 : 4) : 0;
+    const size_t bytes = (size_t)CS * TM::stage(ncell) * sizeof(T) + 2 * CS * sizeof(uint64_t);
+    const int zchunk = col_zchunk(g);
+    const dim3 grid((g.n2 + kRY - 1) / kRY, (g.n3 + zchunk - 1) / zchunk);
+    auto kern = k_node_col<T, kRY, CS, CM, UNI_MS, kMaxT, kPitchS, N1T>;
+    NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    mesh->last_partials = (int)(grid.x * grid.y);
+    {
+        NmLaunchScope sc(mesh, nm_node_class(a.mode), st);
+        kern<<<grid, ((TM::n1 + 31) / 32 + 1) * 32, bytes, st>>>(a, zchunk);      // + the producer warp
+    }
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
 template <typename T, int CM, bool UNI_MS>
 nm_status launch_col(nm_mesh *mesh, const NmLocalArgs<T> &a, cudaStream_t st)
 {
+    const int nt = col_tma_n1<T>(mesh, a);
+    if (nt == 256) return launch_col_tma<T, CM, UNI_MS, 256>(mesh, a, st);
+    if (nt == 128) return launch_col_tma<T, CM, UNI_MS, 128>(mesh, a, st);
     return col_pitch(a.g) == kPitchS ? launch_col_p<T, CM, UNI_MS, kPitchS>(mesh, a, st)
                                      : launch_col_p<T, CM, UNI_MS, kPitchL>(mesh, a, st);
 }

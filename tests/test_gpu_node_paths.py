@@ -1,9 +1,10 @@
 """GPU parity of the three node-kernel forms against the fp64 oracle (a5-a11).
 
 With uniform A and Ku the library evaluates the local terms through separable operators, either
-in the column-marching kernel (k_node_col: whole node rows per CTA, cp.async stage ring; grids with
-96 <= N1 + 1 <= 320) or in the patch kernel (k_node_sep); cell-wise A / Ku use the 27-point
-kernel (k_node).  NM_NODE_PATH selects a form for the meshes created while it is set, so each form
+in the column-marching kernel (k_node_col: whole node rows per CTA, a ring of plane stages fed by a
+producer warp with bulk copies when N1 is 128 or 256, else -- or with NM_NODE_PATH=ring -- by cp.async
+of every thread; grids with 96 <= N1 + 1 <= 320) or in the patch kernel (k_node_sep); cell-wise A / Ku
+use the 27-point kernel (k_node).  NM_NODE_PATH selects a form for the meshes created while it is set, so each form
 is held to the same oracle on the same inputs: every mode of the epilogue (H, f, RK4 stages,
 Dormand-Prince stages with the error norm, both adjoint passes), cell-wise Ms with a vacuum block
 and scalar Ms, grids whose z extent spans several z chunks and whose last row tile is ragged.
@@ -25,7 +26,7 @@ TOL = {"f32": 1e-5, "f64": 1e-11}
 DT = {"f32": torch.float32, "f64": torch.float64}
 
 
-@pytest.fixture(params=["auto", "sep", "generic"])
+@pytest.fixture(params=["auto", "ring", "sep", "generic"])
 def node_path(request):
     old = os.environ.get("NM_NODE_PATH")
     if request.param == "auto":
@@ -51,7 +52,7 @@ def _case(n, uniform_ms, seed=21):
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("uniform_ms", [False, True])
-@pytest.mark.parametrize("n", [(96, 9, 4), (128, 16, 16), (108, 4, 48), (243, 2, 3)])
+@pytest.mark.parametrize("n", [(96, 9, 4), (128, 16, 16), (108, 4, 48), (243, 2, 3), (256, 5, 42), (128, 1, 1)])
 def test_heff_and_rhs(n, uniform_ms, prec, node_path):
     from oracle import llg
     td = DT[prec]

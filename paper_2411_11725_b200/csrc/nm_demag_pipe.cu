@@ -630,6 +630,11 @@ template <typename T, int M> struct PxGeom {
     static constexpr int PZ = P + 8;            // pitch of a packed spectrum line
     static constexpr int SCR = team_scratch<T, M>();
     static constexpr size_t FWD_BYTES = ((size_t)LINES * YP + (size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T);
+    // forward, bulk-fed (fp32, M >= 4): the packed lines of a warp live in that warp's own exchange scratch
+    // (LT PZ <= 2 SCR), and a raw buffer takes the R + 1 node rows of the two planes of the next component
+    static constexpr bool BULK_OK = sizeof(T) == 4 && LT * PZ <= 2 * SCR;
+    __host__ __device__ static constexpr int raw_pitch(int n1) { return ((R + 1) * n1 + 6 + 31) & ~31; }     // reals per plane
+    static size_t fwd_bulk_bytes(int n1) { return ((size_t)LINES * YP + 16 * SCR) * 2 * sizeof(T) + (size_t)2 * raw_pitch(n1) * sizeof(T) + 16; }
     // inverse: output tile (R x N reals) + exchange scratch + staged spectrum rows of one component, the
     // blocks of consecutive k1 tiles 64 bytes apart modulo 128 (the gather of a half-warp spans two)
     static constexpr int SK = 64 / (2 * (int)sizeof(T));    // 64 bytes of complex elements
@@ -669,31 +674,41 @@ template <> __device__ __forceinline__ void load2<double2>(const double2 *src, d
 //            by one thread, 16-byte stores
 // EMB (embedded mesh, nm_fast_plan): the mesh has N1 <= N cells per row; cells beyond it are zero, node
 // columns beyond n1 are not read, and the rows of A have pitch f2 (the y transform extent) >= N2.
-template <typename T, int M, bool UNI, bool EMB>
+// BULK (fp32, M >= 4, 16-byte aligned field): the node rows of a component -- R + 1 contiguous rows in each of the
+// two planes -- arrive by two bulk copies issued one component ahead (from the 16-byte boundary below their
+// start: `shift` elements into the buffer), so phase 1 reads shared memory and the HBM latency is off the path.
+template <typename T, int M, bool UNI, bool EMB, bool BULK>
 __global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
 k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename VT<T>::V *__restrict__ A,
-         NmGeom g, const typename VT<T>::V *__restrict__ wP, int f2)
+         NmGeom g, const typename VT<T>::V *__restrict__ wP, int f2, int persist)
 {
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
     constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
+    static_assert(!BULK || G::BULK_OK, "bulk-fed x pass: fp32 and M >= 4");
     extern __shared__ __align__(1024) unsigned char smem[];
     V *s_y = reinterpret_cast<V *>(smem);                   // LINES x YP
-    V *s_z = s_y + LINES * G::YP;                           // LINES x PZ
-    V *s_scr = s_z + LINES * G::PZ;
+    V *s_z = s_y + LINES * G::YP;                           // LINES x PZ (BULK: inside the scratch, per warp)
+    V *s_scr = BULK ? s_z : s_z + LINES * G::PZ;
+    const int RP = G::raw_pitch(g.n1);
+    T *s_raw = reinterpret_cast<T *>(s_scr + 16 * G::SCR);  // BULK: 2 planes x RP
+    uint64_t *full = reinterpret_cast<uint64_t *>(s_raw + 2 * RP);
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
     const int line = w * LT + l;
-    const int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    // persist (BULK only): a CTA walks the tiles blockIdx.x, blockIdx.x + gridDim.x, ... (tile = row block + nbx * plane)
+    // and requests the first component of its next tile while the last one of this tile is transformed
+    int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    const int nbx = g.N2 / R, ntiles = persist ? nbx * g.N3 : 1;
     V *scr = s_scr + (2 * w + h) * G::SCR;
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     // Ms/8 of this thread's cells (rows 2 line, 2 line + 1; columns e = j + M t)
     constexpr bool MS1 = UNI && !EMB;                       // one Ms/8 for every cell of the thread
     V msr[MS1 ? 1 : 16];
-    if (MS1) msr[0] = mk<T>((T)0.125 * ms_uni, (T)0.125 * ms_uni);
-    else {
+    auto load_ms = [&]() {
+        if (MS1) { msr[0] = mk<T>((T)0.125 * ms_uni, (T)0.125 * ms_uni); return; }
         const int N1 = EMB ? g.N1 : N;
         const T *mrow = Ms + ((long long)c3 * g.N2 + r0 + 2 * line) * N1 + j;
 #pragma unroll
@@ -704,7 +719,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
             else v = mk<T>((T)0.125 * mrow[M * t], (T)0.125 * mrow[N1 + M * t]);
             msr[MS1 ? 0 : t] = v;
         }
-    }
+    };
     const long long plane = (long long)g.n1 * g.n2;
     const int rg = tid / N, col = tid % N;                  // phase 1: row group (16 cell rows) and node column
     // small grids: the three components in three CTAs (gridDim.z = 3)
@@ -724,14 +739,66 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
         }
     };
     constexpr bool PREF = sizeof(T) == 8;                   // fp32 (two CTAs per SM, 128 registers): measured slower
+    // BULK: thread 0 requests the rows of a component; element e0 of the array lands at s_raw[p RP + (e0 & 3)]
+    const int nodes3 = 3 * (int)g.nodes;
+    auto request = [&](int comp, int rr0, int cc3) {
+        int e0[2], len[2], total = 0;
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const int e = comp * (int)g.nodes + (cc3 + p) * (int)plane + rr0 * g.n1;
+            e0[p] = e & ~3;
+            len[p] = ((R + 1) * g.n1 + (e & 3) + 3) & ~3;
+            if (e0[p] + len[p] > nodes3) {                  // the array ends inside the last 16 bytes: its last elements by hand
+                len[p] = (nodes3 - e0[p]) & ~3;
+                for (int q = e0[p] + len[p]; q < nodes3; ++q) s_raw[p * RP + q - e0[p]] = fld[q];
+            }
+            total += len[p];
+        }
+        mbar_expect_tx(full, (uint32_t)(total * sizeof(T)));
+#pragma unroll
+        for (int p = 0; p < 2; ++p) bulk_load(s_raw + p * RP, fld + e0[p], (uint32_t)(len[p] * sizeof(T)), full);
+    };
+    auto take_z = [&](int comp) {
+        const int sh0 = (comp * (int)g.nodes + c3 * (int)plane + r0 * g.n1) & 3;
+        const int sh1 = (comp * (int)g.nodes + (c3 + 1) * (int)plane + r0 * g.n1) & 3;
+        const T *q0 = s_raw + sh0 + rg * 16 * g.n1 + col, *q1 = s_raw + RP + sh1 + rg * 16 * g.n1 + col;
+#pragma unroll
+        for (int r = 0; r < 17; ++r) z[r] = (!EMB || col < g.n1) ? q0[r * g.n1] + q1[r * g.n1] : (T)0;
+        if (tid < R) {
+            const T *a0 = s_raw + sh0 + tid * g.n1 + N, *a1 = s_raw + RP + sh1 + tid * g.n1 + N;
+            zlast = (!EMB || N < g.n1) ? (a0[0] + a1[0]) + (a0[g.n1] + a1[g.n1]) : (T)0;
+        }
+    };
+    unsigned nwait = 0;
+    if (BULK) {
+        if (tid == 0) {
+            mbar_init(full, 1);
+            mbar_fence_init();
+        }
+        __syncthreads();
+        if (persist) { r0 = ((int)blockIdx.x % nbx) * R; c3 = (int)blockIdx.x / nbx; }
+        if (tid == 0) request(comp_lo, r0, c3);
+    }
+    for (int tile = persist ? (int)blockIdx.x : 0; tile < ntiles; tile += persist ? (int)gridDim.x : 1) {
+    if (persist) { r0 = (tile % nbx) * R; c3 = tile / nbx; }
+    load_ms();
     if (PREF) load_z(comp_lo);
     for (int comp = comp_lo; comp < comp_hi; ++comp) {
-        if (!PREF) load_z(comp);
+        if (BULK) {
+            mbar_wait(full, nwait & 1u);
+            ++nwait;
+            take_z(comp);
+        } else if (!PREF) load_z(comp);
 #pragma unroll
         for (int r = 0; r < 16; r += 2)
             s_y[(rg * 8 + (r >> 1)) * G::YP + col] = mk<T>(z[r] + z[r + 1], z[r + 1] + z[r + 2]);
         if (tid < R) reinterpret_cast<T *>(s_y + (tid >> 1) * G::YP + N)[tid & 1] = zlast;
         __syncthreads();
+        if (BULK && tid == 0) {                             // the raw rows have been read by everyone
+            const int nt = tile + (int)gridDim.x;
+            if (comp + 1 < comp_hi) request(comp + 1, r0, c3);
+            else if (persist && nt < ntiles) request(comp_lo, (nt % nbx) * R, nt / nbx);
+        }
         if (PREF && comp + 1 < comp_hi) load_z(comp + 1);
         V a[16];
         const V *yl = s_y + line * G::YP + j;
@@ -743,15 +810,21 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
         }
         if (h) shift32<T, false>(a);
         fft_fwd<T, M, true>(a, tw, scr, i);
+        // packed line `ln`: BULK keeps the LT lines of warp ln / LT in that warp's two exchange scratches
+        auto zline = [&](int ln) -> V * { return BULK ? s_scr + (ln / LT) * 2 * G::SCR + (ln % LT) * G::PZ : s_z + ln * G::PZ; };
+        if (BULK) __syncwarp();                             // every lane has taken its values out of the scratch
+        {
+            V *zw = zline(line);
 #pragma unroll
-        for (int s = 0; s < 16; ++s) s_z[line * G::PZ + 2 * slot_freq<M>(j, s) + h] = a[s];
+            for (int s = 0; s < 16; ++s) zw[2 * slot_freq<M>(j, s) + h] = a[s];
+        }
         __syncthreads();
         for (int idx = tid; idx < NKT * LINES * 4; idx += kPipeThreads) {
             const int q = idx & 3, ln = (idx >> 2) % LINES, kt = idx / (4 * LINES);
             const int c2 = r0 + 2 * ln;
             const int p0 = 2 * q;                           // physical slots p0, p0 + 1 of the blocked row
             const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
-            const V *zl = s_z + ln * G::PZ;
+            const V *zl = zline(ln);
             V ze, zo;
             load2(zl + (k0 & ~1), ze, zo);
             const V za = (k0 & 1) ? zo : ze, zb = (k0 & 1) ? ze : zo;      // Z[k0], Z[k1]
@@ -765,6 +838,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
             store2(dst, a0, a1);
             store2(dst + TW, b0, b1);
         }
+    }
     }
 }
 
@@ -1261,12 +1335,31 @@ template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, co
         auto go = [&](auto kern, T ms) -> nm_status {
             NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::FWD_BYTES));
             kern<<<grid, kPipeThreads, G::FWD_BYTES, st>>>(fld, (const T *)mesh->Ms, ms, (V *)mesh->bufA, g,
-                                                           (const V *)mesh->fast.wPx, f2);
+                                                           (const V *)mesh->fast.wPx, f2, 0);
             return NM_OK;
         };
         const T ms = (T)mesh->desc.Ms_scalar;
-        if (mesh->fast.embed) NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, true>, ms) : go(k_px_fwd<T, M, false, true>, (T)0));
-        else NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, false>, ms) : go(k_px_fwd<T, M, false, false>, (T)0));
+        if constexpr (G::BULK_OK) {
+            // bulk-fed form: 16-byte aligned field, 32-bit element indices
+            if (!(((uintptr_t)fld) & 15) && 3 * g.nodes < (1ll << 31) && mesh->dbg_node_path != 3) {
+                const size_t bytes = G::fwd_bulk_bytes(g.n1);
+                // whole grids (not split by component): persistent CTAs, two per SM, over the tiles
+                const int ntiles = (int)(grid.x * grid.y);
+                const bool persist = !split && ntiles > 2 * mesh->sm_count;
+                const dim3 pgrid = persist ? dim3(2 * mesh->sm_count, 1, 1) : grid;
+                auto gob = [&](auto kern, T msv) -> nm_status {
+                    NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+                    kern<<<pgrid, kPipeThreads, bytes, st>>>(fld, (const T *)mesh->Ms, msv, (V *)mesh->bufA, g,
+                                                             (const V *)mesh->fast.wPx, f2, persist ? 1 : 0);
+                    return NM_OK;
+                };
+                if (mesh->fast.embed) NM_TRY(mesh->uni_Ms ? gob(k_px_fwd<T, M, true, true, true>, ms) : gob(k_px_fwd<T, M, false, true, true>, (T)0));
+                else NM_TRY(mesh->uni_Ms ? gob(k_px_fwd<T, M, true, false, true>, ms) : gob(k_px_fwd<T, M, false, false, true>, (T)0));
+                return NM_OK;
+            }
+        }
+        if (mesh->fast.embed) NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, true, false>, ms) : go(k_px_fwd<T, M, false, true, false>, (T)0));
+        else NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, false, false>, ms) : go(k_px_fwd<T, M, false, false, false>, (T)0));
     } else {
         NmLaunchScope sc(mesh, NM_K_X_INV, st);
         auto go = [&](auto kern) -> nm_status {

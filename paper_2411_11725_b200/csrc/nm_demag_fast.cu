@@ -501,7 +501,7 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
         const int vec = d->dtype == NM_F64 ? 2 : 4;
         if (N[0] < 2 || N[1] < 2 || N[2] < 2) return;                           // films and rods: the 2-D / 1-D general path
         // a mesh the general path can serve (every N_d = 2^a 3^b) is embedded only where that is faster:
-        // it must fill 1/2 (fp32) or 3/4 (fp64) of the (y, z) plane the z pass transforms in full
+        // it must fill 1/2 (pipelined y / z kernels) or 3/4 of the (y, z) plane the z pass transforms in full
         bool smooth = true;
         for (int a = 0; a < 3; ++a) {
             int v = N[a];
@@ -510,7 +510,9 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
             if (v != 1) smooth = false;
         }
         const long long fill = (long long)N[1] * N[2] * 4, plane = (long long)F[1] * F[2];
-        if (smooth && fill < (d->dtype == NM_F64 ? 3 : 2) * plane) return;
+        // (fp64 has pipelined y / z kernels at 256 cells only: smaller extended planes must be fuller to pay)
+        const bool piped = d->dtype != NM_F64 || (F[1] == 256 && F[2] == 256);
+        if (smooth && fill < (piped ? 2 : 3) * plane) return;
         if (N[1] % (2 * 8 * LTx) != 0 || N[0] % vec != 0) return;              // whole x-pass CTAs of rows, 16-byte cell rows
         if (N[2] % (16 / M[1]) != 0) return;                                   // whole y-pass CTAs of planes
         if (d->dtype == NM_F64 && M[0] == 1) return;                           // no staged fp64 x pass at N1 = 16

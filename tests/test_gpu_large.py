@@ -51,13 +51,14 @@ def test_heff_and_rhs_dense_parity_bench_size_fp32(N):
     assert mesh.nm_debug_demag_path() == (1 if N == 256 else 2)
 
 
-@pytest.mark.parametrize("prec,N", [("f32", 128), ("f32", 96), ("f64", 128), ("f64", 96)])
+@pytest.mark.parametrize("prec,N", [("f32", 128), ("f32", 96), ("f64", 128), ("f64", 96), ("f64", 192)])
 def test_heff_and_rhs_dense_parity_mid_sizes(prec, N):
     """Config 4 at 128^3 (fp32: k_py_fwd8 / k_pz_mid8; fp64: the one-CTA-per-tile fast kernels,
-    k_fz_mid) and 96^3 (fp32: zero-extended to 128^3; fp64: general radix-2/3 path), every node.
-    (3-7 s each with the sliced tensor table.)"""
+    k_fz_mid), 96^3 (fp32: zero-extended to 128^3; fp64: general radix-2/3 path) and 192^3 in fp64
+    (zero-extended to 256^3: k_py_fwd / k_py_inv<double>, k_pz_mid64 with masked rows), every node.
+    (3-7 s each with the sliced tensor table; 192: ~25 s.)"""
     mesh = _dense_case(N, prec)
-    want = {("f32", 128): 1, ("f32", 96): 2, ("f64", 128): 1, ("f64", 96): 0}[(prec, N)]
+    want = {("f32", 128): 1, ("f32", 96): 2, ("f64", 128): 1, ("f64", 96): 0, ("f64", 192): 2}[(prec, N)]
     assert mesh.nm_debug_demag_path() == want
 
 

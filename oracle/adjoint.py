@@ -26,6 +26,7 @@ import numpy as np
 
 from . import demag as _demag
 from . import llg as _llg
+from . import local_fields as _lf
 from .mesh import (LOCAL, MU0, element_matrices, gather_nodes_to_cells, node_view,
                    scatter_cells_to_nodes)
 
@@ -114,6 +115,23 @@ def adjoint_rhs_hext(p, t, m, a):
     return -np.array([np.sum(b[j][inside]) for j in range(3)])
 
 
+def adjoint_rhs_hnodal(p, t, m, a):
+    """-(df/dh)^T a for a *nodal* external field h (3, nodes) added to H_ext through the weak form of
+    Eq. (21) (SURVEY.md §8(f) row 2 lists H^ext among the design variables; reading C3(ii)).
+
+    H^z = -L^-1 Z(h) with Z = variation_zeeman, linear in h and symmetric (an assembled mass matrix), so
+        (dH^z/dh)^T b = -Z(b / L),   b = (df/dH)^T a = g' m x a - alpha g' m x (m x a),
+    and -(df/dh)^T a = Z(b / L), with b / L := 0 where L_n = 0 (reading C3(iii)).  Returns a nodal
+    3-vector field; zero without the Zeeman term.  For a uniform h its sum over the nodes is
+    adjoint_rhs_hext."""
+    if not (p.terms & _llg.TERM_ZEEMAN):
+        return np.zeros_like(m)
+    gp = p.gamma / (1.0 + p.alpha ** 2)
+    mxa = _llg.cross(m, a)
+    b = gp * mxa - p.alpha * gp * _llg.cross(m, mxa)
+    return _lf.variation_zeeman(_safe_div(b, p.L), p.Ms, p.dx)
+
+
 def adjoint_rhs_materials(p, t, m, a):
     """(-(df/dA)^T a, -(df/dKu)^T a), cell-wise (design variables A_c, Ku_c).
 
@@ -155,7 +173,7 @@ def forward_rk4(p, m0, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
 
 
 def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, a_jumps=None,
-                 with_hext=False, with_materials=False):
+                 with_hext=False, with_materials=False, with_hnodal=False):
     """Integrate Eq. (29) from T = t0 + n_steps dt back to t0 with RK4 steps of -dt.
 
     State (m, a, u); m is renormalised after every step and replaced by the stored forward
@@ -172,6 +190,8 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
     (m0, a0, u0, u_h(0)); u_h(0) = dL/dh for a uniform external field h.
     with_materials: also integrate (u_A, u_Ku) with adjoint_rhs_materials and append
     (u_A(0), u_Ku(0)) = (dL/dA, dL/dKu) per cell to the returned tuple.
+    with_hnodal: also integrate u_hn with adjoint_rhs_hnodal and append u_hn(0) = dL/dh per node and
+    component for a time-constant nodal external field h (last in the returned tuple).
     """
     m, a = mT.copy(), aT.copy()
     u = np.zeros(p.n_cells)
@@ -186,12 +206,22 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
     uA = np.zeros(p.n_cells)
     uKu = np.zeros(p.n_cells)
 
+    uhn = np.zeros_like(mT)
+    G = (lambda t, m_, a_: adjoint_rhs_hnodal(p, t, m_, a_)) if with_hnodal else None
+
     for s in range(n_steps, 0, -1):
         t = t0 + s * dt
+        if with_hnodal:         # the stage states are those of the RK4 step below
+            g1 = G(t, m, a)
         k1 = F(t, m, a)
         k2 = F(t + 0.5 * h, m + 0.5 * h * k1[0], a + 0.5 * h * k1[1])
         k3 = F(t + 0.5 * h, m + 0.5 * h * k2[0], a + 0.5 * h * k2[1])
         k4 = F(t + h, m + h * k3[0], a + h * k3[1])
+        if with_hnodal:
+            g2 = G(t + 0.5 * h, m + 0.5 * h * k1[0], a + 0.5 * h * k1[1])
+            g3 = G(t + 0.5 * h, m + 0.5 * h * k2[0], a + 0.5 * h * k2[1])
+            g4 = G(t + h, m + h * k3[0], a + h * k3[1])
+            uhn = uhn + h / 6.0 * (g1 + 2 * g2 + 2 * g3 + g4)
         m = _llg.normalise(m + h / 6.0 * (k1[0] + 2 * k2[0] + 2 * k3[0] + k4[0]))
         a = a + h / 6.0 * (k1[1] + 2 * k2[1] + 2 * k3[1] + k4[1])
         u = u + h / 6.0 * (k1[2] + 2 * k2[2] + 2 * k3[2] + k4[2])
@@ -205,4 +235,4 @@ def backward_rk4(p, mT, aT, dt, n_steps, zeeman=None, checkpoints=None, t0=0.0, 
         if a_jumps is not None and (s - 1) in a_jumps:
             a = a + a_jumps[s - 1]
     out = (m, a, u) + ((uh,) if with_hext else ())
-    return out + ((uA, uKu) if with_materials else ())
+    return out + ((uA, uKu) if with_materials else ()) + ((uhn,) if with_hnodal else ())

@@ -320,3 +320,61 @@ def test_adjoint_driver_zero_and_linearity():
     # checkpoints put m back exactly on the forward trajectory
     mb = adjoint.backward_rk4(p, mT, a1, 5e-14, 20, checkpoints=ck)[0]
     assert np.array_equal(mb, m0)
+
+
+def test_hnodal_vjp_against_finite_differences_entry_by_entry():
+    """adjoint_rhs_hnodal: a . (df/dh_{n,j}) for EVERY nodal entry of a nodal external field, by central
+    differences of the forward RHS, on a mesh with a vacuum corner and cell-wise Ms; its sum over the
+    nodes is the uniform-field gradient adjoint_rhs_hext."""
+    p, zee = make((3, 2, 2), seed=3)
+    Ms = p.Ms.copy()
+    Ms[0, 0, :] = 0.0
+    Ms[0, 1, 0] = 0.0
+    p = with_Ms(p, Ms)
+    m = rand_unit(p.node_shape, 4)
+    a = np.random.default_rng(5).standard_normal(m.shape)
+    base = zee(0.0)
+    got = adjoint.adjoint_rhs_hnodal(p, 0.0, m, a)
+    assert got.shape == m.shape
+    eps = 10.0
+    for idx in np.ndindex(*m.shape):
+        d = np.zeros_like(m)
+        d[idx] = eps
+        fp = llg.llg_rhs(p, 0.0, m, lambda t: base + d)
+        fm = llg.llg_rhs(p, 0.0, m, lambda t: base - d)
+        fd = -np.sum(a * (fp - fm)) / (2 * eps)
+        assert abs(got[idx] - fd) <= 1e-9 * np.abs(got).max(), (idx, got[idx], fd)
+    assert np.allclose(got.sum(axis=(1, 2, 3)), adjoint.adjoint_rhs_hext(p, 0.0, m, a), rtol=1e-12)
+    p0 = Problem(p.n_cells, p.dx, p.Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha, TERM_EXCHANGE | TERM_DEMAG, p._Nt)
+    assert np.all(adjoint.adjoint_rhs_hnodal(p0, 0.0, m, a) == 0.0)
+
+
+def test_hnodal_gradient_of_a_trajectory_against_finite_differences():
+    """dL/dh_{n,j} of L = w . m(T) for a time-constant nodal external field: u_hn(0) of the backward pass
+    vs central differences of the forward solve at seeded entries; summed over nodes it is dL/dh of the
+    uniform field."""
+    rng = np.random.default_rng(27)
+    n, dx = (6, 2, 1), (4e-9, 4e-9, 5e-9)
+    p = Problem(n, dx, rng.uniform(1e5, 1.5e5, n), np.full(n, 3.65e-12), np.full(n, 2e4), ku_axis=(0.0, 0.6, 0.8),
+                alpha=0.05, terms=ALL)
+    p.Nt
+    hn = 2e3 * rng.standard_normal((3,) + p.node_shape)
+    m0 = 0.1 * rng.standard_normal((3,) + p.node_shape)
+    m0[0] += 1
+    m0 /= np.sqrt(np.sum(m0 * m0, axis=0))
+    w = rng.standard_normal(m0.shape)
+    dt, nst = 5e-14, 80
+    zee = lambda t: hn
+    mT, ck = adjoint.forward_rk4(p, m0, dt, nst, zee, checkpoint_every=40)
+    out = adjoint.backward_rk4(p, mT, w, dt, nst, zee, checkpoints=ck, with_hext=True, with_hnodal=True)
+    uh, uhn = out[3], out[4]
+    assert np.allclose(uhn.sum(axis=(1, 2, 3)), uh, rtol=1e-10)
+    scale = np.abs(uhn).max()
+    for _ in range(6):
+        idx = tuple(int(rng.integers(0, k)) for k in hn.shape)
+        d = np.zeros_like(hn)
+        d[idx] = 50.0
+        Lp = np.sum(w * adjoint.forward_rk4(p, m0, dt, nst, lambda t: hn + d)[0])
+        Lm = np.sum(w * adjoint.forward_rk4(p, m0, dt, nst, lambda t: hn - d)[0])
+        fd = (Lp - Lm) / 100.0
+        assert abs(uhn[idx] - fd) <= 1e-3 * scale, (idx, uhn[idx], fd)

@@ -207,7 +207,16 @@ nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt, void *m_i
 typedef struct {
     void *u_A, *u_Ku;     /* device cell arrays, mesh dtype, in/out */
     double *u_h;          /* device fp64 [3], in/out (uniform external field, see above) */
+    void *u_hn;           /* device nodal 3-vector field, mesh dtype, in/out: gradient with respect to a
+                             time-constant NODAL external field (nm_llg_adjoint_rhs_hnodal) */
 } nm_adjoint_extra;
+
+/* -(df/dh)^T a for a nodal external field h(n) entering through the weak form of Eq. (21) (
+ * SURVEY.md 8(f) row 2 lists H^ext among the design variables): with b = (df/dH)^T a,
+ *   dudt_hn_out = Z(b / L),  Z h = -mu0 sum_c Ms_c sum_i' M_{i,i'} h_{c+i'}  (the Zeeman variation, symmetric),
+ * a nodal 3-vector field of the mesh dtype; zero without NM_TERM_ZEEMAN and at nodes with (S Ms)_n = 0 all round.
+ * Summed over the nodes it equals nm_llg_adjoint_rhs_hext.  Uses the mesh's adjoint scratch. */
+nm_status nm_llg_adjoint_rhs_hnodal(nm_mesh *mesh, const void *m, const void *a, void *dudt_hn_out, void *stream);
 nm_status nm_llg_adjoint_rhs_materials(nm_mesh *mesh, const void *m, const void *a, void *dudt_A_out,
                                        void *dudt_Ku_out, void *stream);
 nm_status nm_adjoint_rk4_step_ex(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,

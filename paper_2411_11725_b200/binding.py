@@ -25,7 +25,7 @@ NM_RK4, NM_DOPRI5 = 0, 1
 EXPORTS = ("nm_mesh_query_workspace", "nm_mesh_create", "nm_mesh_set_Ms", "nm_mesh_destroy",
            "nm_last_error", "nm_heff", "nm_llg_rhs", "nm_rk_step", "nm_llg_adjoint_rhs",
            "nm_adjoint_rk4_step", "nm_adjoint_add_objective", "nm_llg_adjoint_rhs_hext", "nm_adjoint_rk4_step_hext",
-           "nm_llg_adjoint_rhs_materials", "nm_adjoint_rk4_step_ex", "nm_debug_get_tensor", "nm_debug_get_cell_field",
+           "nm_llg_adjoint_rhs_materials", "nm_adjoint_rk4_step_ex", "nm_llg_adjoint_rhs_hnodal", "nm_debug_get_tensor", "nm_debug_get_cell_field",
            "nm_launch_count", "nm_profile_dropped", "nm_debug_demag_path", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
            "nm_profile_end")
 
@@ -59,7 +59,8 @@ class nm_zeeman(ctypes.Structure):
 
 
 class nm_adjoint_extra(ctypes.Structure):
-    _fields_ = [("u_A", ctypes.c_void_p), ("u_Ku", ctypes.c_void_p), ("u_h", ctypes.c_void_p)]
+    _fields_ = [("u_A", ctypes.c_void_p), ("u_Ku", ctypes.c_void_p), ("u_h", ctypes.c_void_p),
+                ("u_hn", ctypes.c_void_p)]
 
 
 class NmError(RuntimeError):
@@ -94,6 +95,7 @@ def lib():
         L.nm_adjoint_rk4_step.argtypes = [vp, dbl, dbl, vp, vp, vp, ctypes.POINTER(nm_zeeman), i32, vp]
         L.nm_adjoint_add_objective.argtypes = [vp, vp, vp, dbl, vp]
         L.nm_llg_adjoint_rhs_hext.argtypes = [vp, vp, vp, vp, vp]
+        L.nm_llg_adjoint_rhs_hnodal.argtypes = [vp, vp, vp, vp, vp]
         L.nm_llg_adjoint_rhs_materials.argtypes = [vp, vp, vp, vp, vp, vp]
         L.nm_adjoint_rk4_step_ex.argtypes = [vp, dbl, dbl, vp, vp, vp, ctypes.POINTER(nm_adjoint_extra),
                                              ctypes.POINTER(nm_zeeman), i32, vp]
@@ -280,12 +282,18 @@ class Mesh:
                                                   _stream(self.device)))
         return gA, gKu
 
+    def nm_llg_adjoint_rhs_hnodal(self, m, a):
+        out = torch.empty_like(m)
+        _check(lib().nm_llg_adjoint_rhs_hnodal(self.handle, _ptr(m), _ptr(a), _ptr(out), _stream(self.device)))
+        return out
+
     def nm_adjoint_rk4_step_ex(self, t, dt, m, a, u, u_A=None, u_Ku=None, u_h=None, zeeman=None,
-                               renormalise=True):
+                               renormalise=True, u_hn=None):
         ex = nm_adjoint_extra()
         ex.u_A = u_A.data_ptr() if u_A is not None else None
         ex.u_Ku = u_Ku.data_ptr() if u_Ku is not None else None
         ex.u_h = u_h.data_ptr() if u_h is not None else None
+        ex.u_hn = u_hn.data_ptr() if u_hn is not None else None
         _check(lib().nm_adjoint_rk4_step_ex(self.handle, float(t), float(dt), _ptr(m), _ptr(a), _ptr(u),
                                             ctypes.byref(ex), _zref(zeeman), 1 if renormalise else 0,
                                             _stream(self.device)))

@@ -827,7 +827,7 @@ nm_status mat_grad(nm_mesh *m, const T *mm, const T *av, T *uA, T *uKu, double c
 }
 
 template <typename T>
-nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, double *uh, T *uA, T *uKu,
+nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, double *uh, T *uA, T *uKu, T *uhn,
                       const nm_zeeman *z, int renorm, cudaStream_t st)
 {
     const double gp_h = m->desc.gamma / (1.0 + m->desc.alpha * m->desc.alpha);
@@ -845,6 +845,11 @@ nm_status adjoint_rk4(nm_mesh *m, double t, double dt, T *mm, T *av, T *u, doubl
         NM_TRY(adjoint_eval<T>(m, ts[s], sm, sa, z, F, DA, DU, st));
         // u_h += w_s (-(df/dh)^T a) of this stage (reads the stage state before it is overwritten)
         if (want_h) NM_TRY(nm_launch_hext_grad<T>(m, sm, sa, gp_h, m->desc.alpha * gp_h, w[s], uh, st));
+        if (uhn && (m->desc.terms & NM_TERM_ZEEMAN)) {      // u_hn += w_s Z(b / L): q = b / (S Ms) is in Q after the adjoint pass
+            NmLocalArgs<T> la;
+            base_args<T>(m, 0.0, nullptr, m->desc.terms, &la);
+            NM_TRY(nm_launch_hnodal_grad<T>(m, la, (const T *)m->Q, sm, sa, w[s], 1, uhn, st));
+        }
         NM_TRY(mat_grad<T>(m, sm, sa, uA, uKu, w[s], 1, st));
         const T ws = (T)w[s];
         if (s < 3) {
@@ -1029,8 +1034,8 @@ extern "C" nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, 
 
 namespace {
 nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout, void *u_inout,
-                            double *u_h_inout, void *u_A, void *u_Ku, const nm_zeeman *zeeman, int renormalise,
-                            void *stream)
+                            double *u_h_inout, void *u_A, void *u_Ku, void *u_hn, const nm_zeeman *zeeman,
+                            int renormalise, void *stream)
 {
     NM_TRY(check_call(mesh, m_inout, a_inout));
     NM_TRY(check_adjoint(mesh));
@@ -1046,13 +1051,14 @@ nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, v
     key.p[3] = u_h_inout;
     key.p[4] = u_A;
     key.p[5] = u_Ku;
+    key.p[6] = u_hn;
     return run_step(mesh, NM_GRAPH_ADJ_RK4, zeeman, key, st, [&](cudaStream_t s) {
         return mesh->f64 ? adjoint_rk4<double>(mesh, t, dt, (double *)m_inout, (double *)a_inout,
                                                (double *)u_inout, u_h_inout, (double *)u_A, (double *)u_Ku,
-                                               zeeman, renormalise, s)
+                                               (double *)u_hn, zeeman, renormalise, s)
                          : adjoint_rk4<float>(mesh, t, dt, (float *)m_inout, (float *)a_inout,
                                               (float *)u_inout, u_h_inout, (float *)u_A, (float *)u_Ku,
-                                              zeeman, renormalise, s);
+                                              (float *)u_hn, zeeman, renormalise, s);
     });
 }
 } // namespace
@@ -1060,7 +1066,7 @@ nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, v
 extern "C" nm_status nm_adjoint_rk4_step(nm_mesh *mesh, double t, double dt, void *m_inout, void *a_inout,
                                          void *u_inout, const nm_zeeman *zeeman, int renormalise, void *stream)
 {
-    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, nullptr, nullptr, nullptr, zeeman,
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, nullptr, nullptr, nullptr, nullptr, zeeman,
                              renormalise, stream);
 }
 
@@ -1069,7 +1075,7 @@ extern "C" nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt
                                               int renormalise, void *stream)
 {
     if (!u_h_inout) { nm_set_error("u_h_inout is NULL"); return NM_EINVAL; }
-    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, u_h_inout, nullptr, nullptr, zeeman,
+    return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, u_h_inout, nullptr, nullptr, nullptr, zeeman,
                              renormalise, stream);
 }
 
@@ -1079,7 +1085,30 @@ extern "C" nm_status nm_adjoint_rk4_step_ex(nm_mesh *mesh, double t, double dt, 
 {
     if (!extra) { nm_set_error("extra is NULL"); return NM_EINVAL; }
     return adjoint_rk4_entry(mesh, t, dt, m_inout, a_inout, u_inout, extra->u_h, extra->u_A, extra->u_Ku,
-                             zeeman, renormalise, stream);
+                             extra->u_hn, zeeman, renormalise, stream);
+}
+
+extern "C" nm_status nm_llg_adjoint_rhs_hnodal(nm_mesh *mesh, const void *m, const void *a, void *dudt_hn_out,
+                                               void *stream)
+{
+    NM_TRY(check_call(mesh, m, a));
+    NM_TRY(check_adjoint(mesh));
+    if (!dudt_hn_out) { nm_set_error("dudt_hn_out is NULL"); return NM_EINVAL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!(mesh->desc.terms & NM_TERM_ZEEMAN)) {
+        NM_CUDA_TRY(cudaMemsetAsync(dudt_hn_out, 0, 3 * mesh->g.nodes * mesh->esz, st));
+        return NM_OK;
+    }
+    if (mesh->f64) {
+        NmLocalArgs<double> la;
+        base_args<double>(mesh, 0.0, nullptr, mesh->desc.terms, &la);
+        return nm_launch_hnodal_grad<double>(mesh, la, nullptr, (const double *)m, (const double *)a, 1.0, 0,
+                                             (double *)dudt_hn_out, st);
+    }
+    NmLocalArgs<float> la;
+    base_args<float>(mesh, 0.0, nullptr, mesh->desc.terms, &la);
+    return nm_launch_hnodal_grad<float>(mesh, la, nullptr, (const float *)m, (const float *)a, 1.0, 0,
+                                        (float *)dudt_hn_out, st);
 }
 
 extern "C" nm_status nm_llg_adjoint_rhs_materials(nm_mesh *mesh, const void *m, const void *a, void *dudt_A_out,

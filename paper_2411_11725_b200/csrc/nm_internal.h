@@ -82,7 +82,7 @@ struct NmFast {
 struct NmStepKey {
     int kind, renorm, has_z, pad;   // no implicit padding: keys are compared with memcmp
     double dt, rtol, atol, hu[3];
-    const void *p[6], *hs, *hp;
+    const void *p[7], *hs, *hp;
     unsigned long long epoch;
 };
 struct NmStepGraph {

@@ -261,8 +261,11 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
 // involve m): Zs_n = (mu0 / L_n) sum_{c in n} Ms_c sum_{i'} M_{i,i'} H^ext_{c+i'}  (Eq. 21, reading
 // C3(ii)), H^ext = h_static + amp h_pulse; 0 where (S Ms)_n = 0.  Lets meshes with uniform A and Ku keep
 // the separable node kernels when the Zeeman field is a nodal array (config 3's stripe pulse).
-template <typename T>
-__global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a, T *__restrict__ Zs)
+// GRAD: the transpose of the same operator, for the gradient with respect to a nodal external field
+// (SURVEY.md 8(f) row 2): with h := q = b / (S Ms),  out (+)= coef (-(8/V) sum_c Ms_c sum_i' M_{i,i'} q_{c+i'})
+// = coef Z(b / L) = -coef (df/dh)^T a  (oracle/adjoint.py: adjoint_rhs_hnodal).
+template <typename T, bool GRAD>
+__global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a, T *__restrict__ Zs, T coef, int accumulate)
 {
     const NmGeom &g = a.g;
     const int pl = g.n1 * g.n2;
@@ -315,7 +318,30 @@ __global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a
             }
     const T sc = sms > 0 ? a.mu0 / (a.mu0V8 * sms) : (T)0;
 #pragma unroll
-    for (int j = 0; j < 3; ++j) Zs[j * nn + n] = sc * ze[j] + (a.hadd ? a.hadd[j * nn + n] : (T)0);   // + the field of the further local terms
+    for (int j = 0; j < 3; ++j) {
+        if (GRAD) {
+            const T gv = -coef * (a.mu0 / a.mu0V8) * ze[j];
+            Zs[j * nn + n] = accumulate ? Zs[j * nn + n] + gv : gv;
+        } else {
+            Zs[j * nn + n] = sc * ze[j] + (a.hadd ? a.hadd[j * nn + n] : (T)0);   // + the field of the further local terms
+        }
+    }
+}
+
+// q = b / (S Ms), b = g' m x a - alpha g' m x (m x a); 0 where (S Ms)_n = 0
+template <typename T>
+__global__ void k_bq(const T *__restrict__ m, const T *__restrict__ av, const T *__restrict__ sMs, long long nn, T gp, T agp,
+                     T *__restrict__ Q)
+{
+    const long long n = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= nn) return;
+    const T mm[3] = {m[n], m[nn + n], m[2 * nn + n]}, aa[3] = {av[n], av[nn + n], av[2 * nn + n]};
+    const T mxa[3] = {mm[1] * aa[2] - mm[2] * aa[1], mm[2] * aa[0] - mm[0] * aa[2], mm[0] * aa[1] - mm[1] * aa[0]};
+    const T mm2[3] = {mm[1] * mxa[2] - mm[2] * mxa[1], mm[2] * mxa[0] - mm[0] * mxa[2], mm[0] * mxa[1] - mm[1] * mxa[0]};
+    const T s = sMs[n];
+    const T inv = s > 0 ? (T)1 / s : (T)0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) Q[j * nn + n] = (gp * mxa[j] - agp * mm2[j]) * inv;
 }
 
 // -------------------------------------------------------------------------------------------------
@@ -939,7 +965,7 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
         {
             NmLaunchScope sc(mesh, NM_K_OTHER, st);
             const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
-            k_zeeman_smooth<T><<<grid, kBlock, 0, st>>>(a, (T *)mesh->Zs);
+            k_zeeman_smooth<T, false><<<grid, kBlock, 0, st>>>(a, (T *)mesh->Zs, (T)0, 0);
         }
         NM_CUDA_TRY(cudaGetLastError());
         NmLocalArgs<T> b = a;
@@ -1026,6 +1052,33 @@ nm_status nm_launch_hext_grad(nm_mesh *mesh, const T *m, const T *a, double gp, 
     {
         NmLaunchScope sc(mesh, NM_K_OTHER, st);
         k_hext_final<<<1, 256, 0, st>>>(mesh->hpart, (int)nb, coef, u_h);
+    }
+    NM_CUDA_TRY(cudaGetLastError());
+    return NM_OK;
+}
+
+// u_hn (+)= coef Z(q L / L) with q = b / (S Ms) given (q != null: the Q array of the adjoint pass) or made here
+// from (m, a) into the mesh's Q scratch
+template <typename T>
+nm_status nm_launch_hnodal_grad(nm_mesh *mesh, const NmLocalArgs<T> &base, const T *q, const T *m, const T *av,
+                                double coef, int accumulate, T *u_hn, cudaStream_t st)
+{
+    const long long nn = mesh->g.nodes;
+    if (!q) {
+        {
+            NmLaunchScope sc(mesh, NM_K_OTHER, st);
+            k_bq<T><<<nblk(nn, 256), 256, 0, st>>>(m, av, (const T *)mesh->sMs, nn, base.gp, base.agp, (T *)mesh->Q);
+        }
+        q = (const T *)mesh->Q;
+    }
+    NmLocalArgs<T> a = base;
+    a.h_static = q;
+    a.h_pulse = nullptr;
+    a.hadd = nullptr;
+    {
+        NmLaunchScope sc(mesh, NM_K_OTHER, st);
+        const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
+        k_zeeman_smooth<T, true><<<grid, kBlock, 0, st>>>(a, u_hn, (T)coef, accumulate);
     }
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;
@@ -1124,6 +1177,8 @@ nm_status nm_compute_sMs(nm_mesh *mesh, cudaStream_t st)
     template nm_status nm_launch_hext_grad<T>(nm_mesh *, const T *, const T *, double, double, double,  \
                                               double *, cudaStream_t);                                  \
     template nm_status nm_launch_adj_cell<T>(nm_mesh *, const NmAdjCellArgs<T> &, cudaStream_t);        \
+    template nm_status nm_launch_hnodal_grad<T>(nm_mesh *, const NmLocalArgs<T> &, const T *, const T *, const T *, \
+                                                double, int, T *, cudaStream_t);                       \
     template nm_status nm_lincomb<T>(nm_mesh *, T *, const T *, int, const T *const *, const T *,       \
                                      long long, long long, cudaStream_t);                               \
     template nm_status nm_lincomb_batch<T>(nm_mesh *, const NmLinOp<T> *, int, cudaStream_t);

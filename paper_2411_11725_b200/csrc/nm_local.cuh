@@ -105,6 +105,12 @@ template <typename T>
 nm_status nm_launch_hext_grad(nm_mesh *mesh, const T *m, const T *a, double gp, double agp, double coef,
                               double *u_h, cudaStream_t st);
 
+// u_hn (+)= coef (-(df/dh)^T a) for a nodal external field h through the weak form:
+// the transposed Zeeman smoothing applied to q = b / (S Ms); q = null: made from (m, a) into mesh->Q.
+template <typename T>
+nm_status nm_launch_hnodal_grad(nm_mesh *mesh, const NmLocalArgs<T> &base, const T *q, const T *m, const T *av,
+                                double coef, int accumulate, T *u_hn, cudaStream_t st);
+
 // Cell-wise VJPs with respect to A_c and Ku_c, b = g' m x a - alpha g' m x (m x a),
 // bL = b / L (0 where (S Ms)_n = 0), the element matrices K, M of Eq. (12) by vertex difference pattern:
 //   gA_c  = +2 sum_{i,i'} K[i,i'] bL_{c+i} . m_{c+i'}           = -(df/dA_c)^T a

@@ -59,7 +59,7 @@ def forward_rk4(mesh, m, dt, n_steps, zeeman=None, checkpoint_every=0, t0=0.0):
 
 
 def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_every=100, t0=0.0,
-                     objectives_at=None, with_hext=False, with_materials=False):
+                     objectives_at=None, with_hext=False, with_materials=False, with_hnodal=False):
     """Adjoint-state gradient dJ/dMs (Eqs. 27-30; reading C8).
 
     Forward RK4 from m0 with checkpoints, a(T) = aT_of_mT(m(T)) (the caller's dJ/dm(T)), then the
@@ -74,7 +74,9 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
     (nm_adjoint_rk4_step_hext; PAPER.md:339-347) and return (m(T), a(0), u(0), u_h(0) = dL/dh as a
     device fp64 3-vector).
     with_materials: also integrate the gradients with respect to the cell-wise A and Ku
-    (nm_adjoint_rk4_step_ex) and append (u_A(0), u_Ku(0)) to the returned tuple."""
+    (nm_adjoint_rk4_step_ex) and append (u_A(0), u_Ku(0)) to the returned tuple.
+    with_hnodal: also integrate the gradient with respect to a time-constant nodal external field
+    (nm_adjoint_extra.u_hn) and append u_hn(0) = dL/dh per node and component, last."""
     m = m0.clone()
     jumps = {}
     if objectives_at:
@@ -93,9 +95,10 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
     uh = torch.zeros(3, dtype=torch.float64, device=m.device) if with_hext else None
     uA = torch.zeros_like(u) if with_materials else None
     uKu = torch.zeros_like(u) if with_materials else None
+    uhn = torch.zeros_like(m) if with_hnodal else None
     for s in range(n_steps, 0, -1):
-        if with_materials:
-            mesh.nm_adjoint_rk4_step_ex(t0 + s * dt, dt, m, a, u, u_A=uA, u_Ku=uKu, u_h=uh, zeeman=zeeman)
+        if with_materials or with_hnodal:
+            mesh.nm_adjoint_rk4_step_ex(t0 + s * dt, dt, m, a, u, u_A=uA, u_Ku=uKu, u_h=uh, zeeman=zeeman, u_hn=uhn)
         elif with_hext:
             mesh.nm_adjoint_rk4_step_hext(t0 + s * dt, dt, m, a, u, uh, zeeman)
         else:
@@ -105,7 +108,7 @@ def adjoint_gradient(mesh, m0, aT_of_mT, dt, n_steps, zeeman=None, checkpoint_ev
         if (s - 1) in jumps:
             mesh.nm_adjoint_add_objective(a, jumps[s - 1])
     out = (mT, a, u) + ((uh,) if with_hext else ())
-    return out + ((uA, uKu) if with_materials else ())
+    return out + ((uA, uKu) if with_materials else ()) + ((uhn,) if with_hnodal else ())
 
 
 # ---- field-angle problem of Sec. VII (Eqs. 31-33) ------------------------------

@@ -600,3 +600,47 @@ def test_errors_are_statuses_not_crashes():
     m[0] = 1.0
     assert float(mesh.nm_heff(0.0, m).abs().max()) == 0.0   # uniform m: exchange field vanishes
     assert mesh.nm_launch_count() > 0
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_nodal_hext_gradient_rhs_and_backward_pass(prec):
+    """Gradient with respect to a NODAL external field (SURVEY.md 8(f) row 2, H^ext): nm_llg_adjoint_rhs_hnodal
+    against oracle adjoint_rhs_hnodal on a ragged all-terms mesh with a vacuum block, its sum over the nodes
+    against the uniform-field gradient, and u_hn(0) of drivers.adjoint_gradient(with_hnodal=True) against the
+    oracle's backward pass on a film with a nodal static field."""
+    from oracle import adjoint
+    from paper_2411_11725_b200 import drivers
+    td = DT[prec]
+    nd = np_dtype(td)
+    w, hs = wl.varied_case((24, 12, 6), vacuum=True)
+    p = oracle_problem(w, nd)
+    m = _m0(w, td)
+    a = wl.round_to(np.random.default_rng(31).standard_normal(m.shape), nd)
+    ref = adjoint.adjoint_rhs_hnodal(p, 0.0, m, a)
+    mesh = gpu_mesh(w, td)
+    got = host(mesh.nm_llg_adjoint_rhs_hnodal(dev(m, td), dev(a, td)))
+    assert_parity(got, ref, TOL[prec], "nodal-field gradient")
+    vac = p.L == 0
+    assert vac.any()
+    uni = mesh.nm_llg_adjoint_rhs_hext(dev(m, td), dev(a, td)).cpu().numpy()
+    assert np.max(np.abs(got.sum(axis=(1, 2, 3)) - uni)) <= (1e-10 if prec == "f64" else 1e-4) * np.max(np.abs(uni))
+    w0 = wl.config4_sweep(16)
+    assert torch.all(gpu_mesh(w0, td).nm_llg_adjoint_rhs_hnodal(dev(_m0(w0, td), td), dev(_m0(w0, td), td)) == 0)
+    # backward integration with a nodal static field
+    w = wl.config5_inverse((32, 8, 1), n_steps=30)
+    w.h_uniform = (1e3, 2e3, -1.5e3)
+    p = oracle_problem(w, nd)
+    hs = wl.round_to(1e3 * np.random.default_rng(8).standard_normal((3,) + w.node_shape), nd)
+    z = oracle_zeeman(w, nd, hs)
+    m0 = _m0(w, td)
+    wT = wl.round_to(wl.objective_weights(w), nd)
+    mT_ref, ck = adjoint.forward_rk4(p, m0, w.dt, w.n_steps, z, checkpoint_every=10)
+    ref = adjoint.backward_rk4(p, mT_ref, wT, w.dt, w.n_steps, z, checkpoints=ck, with_hnodal=True)
+    mesh = gpu_mesh(w, td)
+    gz = gpu_zeeman(w, td, h_static=hs)
+    gT = dev(wT, td)
+    out = drivers.adjoint_gradient(mesh, dev(m0, td), lambda mm: gT, w.dt, w.n_steps, gz, checkpoint_every=10,
+                                   with_hnodal=True)
+    assert rel_l2(host(out[1]), ref[1]) <= TOL[prec]
+    assert rel_l2(wl.from_abi(out[2].cpu().double().numpy()), ref[2]) <= TOL[prec]
+    assert_parity(host(out[3]), ref[3], TOL[prec], "u_hn(0)")

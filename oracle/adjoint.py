@@ -22,6 +22,8 @@ neural-ODE reference 26.)  The paper delegates both products to framework autodi
                           + (S^T q)_c . Hcell_c + mbar_c . Y_c
      q = b / (S Ms),  mbar = S^T m / 8,  Hcell = -N * (Ms mbar),  Y = -N * (Ms o S^T q)
 """
+import dataclasses
+
 import numpy as np
 
 from . import demag as _demag
@@ -62,8 +64,11 @@ def adjoint_rhs(p, t, m, a, zeeman=None, pieces=None):
     d = -gp * cross(H, a) - al * gp * (dot(m, H) * a + dot(a, m) * H - 2.0 * dot(a, H) * m)
 
     # Hlin^T b = L o Hlin(b / L): the same field operators, without the Zeeman term
-    p_lin = _llg.Problem(p.n_cells, p.dx, p.Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha,
-                         p.terms & ~_llg.TERM_ZEEMAN, p._Nt)
+    # (exchange, anisotropy, demag and DMI are linear in m with an L-symmetric operator; the cubic
+    # anisotropy is not linear: its transposed Jacobian is not written here)
+    if p.terms & _llg.TERM_CUBIC:
+        raise NotImplementedError("adjoint_rhs does not differentiate the cubic anisotropy")
+    p_lin = dataclasses.replace(p, terms=p.terms & ~_llg.TERM_ZEEMAN)
     HTb = L * _llg.effective_field(p_lin, _safe_div(b, L), None)
     dadt = -(d + HTb)
 

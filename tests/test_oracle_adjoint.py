@@ -3,7 +3,9 @@ import numpy as np
 import pytest
 
 from oracle import adjoint, llg, mesh
-from oracle.llg import Problem, TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN
+import dataclasses
+
+from oracle.llg import Problem, TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN, TERM_DMI, TERM_CUBIC
 
 ALL = TERM_EXCHANGE | TERM_DEMAG | TERM_ANISO | TERM_ZEEMAN
 
@@ -19,14 +21,18 @@ def make(n=(3, 2, 2), alpha=0.1, terms=ALL, seed=0):
     p = Problem(n, dx, rng.uniform(4e5, 8e5, n), rng.uniform(0.8e-11, 1.3e-11, n),
                 rng.uniform(1e5, 5e5, n), ku_axis=(0.0, 0.6, 0.8), alpha=alpha, terms=terms)
     hext = rng.standard_normal((3,) + p.node_shape) * 3e4
+    if terms & TERM_DMI:        # cell-wise DMI constant; the interfacial kind when the demag term is off
+        p = dataclasses.replace(p, D=rng.uniform(1e-3, 3e-3, n), dmi_kind="bulk" if terms & TERM_DEMAG else "interfacial",
+                                dmi_normal=1)
     return p, (lambda t: hext)
 
 
 def with_Ms(p, Ms):
-    return Problem(p.n_cells, p.dx, Ms, p.A, p.Ku, p.ku_axis, p.gamma, p.alpha, p.terms, p._Nt)
+    return dataclasses.replace(p, Ms=Ms)
 
 
-@pytest.mark.parametrize("terms", [ALL, TERM_EXCHANGE | TERM_DEMAG, TERM_DEMAG, TERM_EXCHANGE | TERM_ANISO | TERM_ZEEMAN])
+@pytest.mark.parametrize("terms", [ALL, TERM_EXCHANGE | TERM_DEMAG, TERM_DEMAG, TERM_EXCHANGE | TERM_ANISO | TERM_ZEEMAN,
+                                   ALL | TERM_DMI, TERM_EXCHANGE | TERM_DMI, TERM_DMI])
 def test_dense_jacobians_by_finite_differences(terms):
     """Explicit dense Jacobians of the oracle's own forward RHS by central differences on a
     3x2x2-cell mesh; both vector-Jacobian products must equal a^T J."""
@@ -378,3 +384,11 @@ def test_hnodal_gradient_of_a_trajectory_against_finite_differences():
         Lm = np.sum(w * adjoint.forward_rk4(p, m0, dt, nst, lambda t: hn - d)[0])
         fd = (Lp - Lm) / 100.0
         assert abs(uhn[idx] - fd) <= 1e-3 * scale, (idx, uhn[idx], fd)
+
+
+def test_cubic_anisotropy_is_refused_by_the_adjoint():
+    p, zee = make()
+    p = dataclasses.replace(p, terms=p.terms | TERM_CUBIC, Kc=np.full(p.n_cells, 1e4))
+    m = rand_unit(p.node_shape, 2)
+    with pytest.raises(NotImplementedError):
+        adjoint.adjoint_rhs(p, 0.0, m, m.copy(), zee)

@@ -754,6 +754,7 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
     NmLocalArgs<T> a;
     base_args<T>(m, t, z, m->desc.terms, &a);
     a.fld = mm;
+    NM_TRY(extra_part<T>(m, mm, &a.hadd, st));          // DMI: linear in m, part of H and of Hlin (cubic: refused)
     NM_TRY(demag_part<T>(m, mm, (T *)m->Hc1, &a.Hc, st));
     m->hc1_valid = a.Hc != nullptr;
     a.mode = NM_MODE_ADJ1;
@@ -767,6 +768,7 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
     NmLocalArgs<T> b;
     base_args<T>(m, t, nullptr, m->desc.terms & ~(unsigned)NM_TERM_ZEEMAN, &b);
     b.fld = (const T *)m->Q;
+    NM_TRY(extra_part<T>(m, (const T *)m->Q, &b.hadd, st));
     NM_TRY(demag_part<T>(m, (const T *)m->Q, (T *)m->Hc2, &b.Hc, st));
     b.mode = NM_MODE_ADJ2;
     b.dadt = dadt;
@@ -948,8 +950,8 @@ nm_status check_adjoint(const nm_mesh *mesh)
         nm_set_error("the adjoint entry points serve the full 3-D basis only (basis = %d)", mesh->desc.basis);
         return NM_EUNSUPPORTED;
     }
-    if (mesh && (mesh->desc.terms & (NM_TERM_DMI | NM_TERM_CUBIC))) {
-        nm_set_error("the adjoint entry points do not differentiate NM_TERM_DMI / NM_TERM_CUBIC");
+    if (mesh && (mesh->desc.terms & NM_TERM_CUBIC)) {
+        nm_set_error("the adjoint entry points do not differentiate NM_TERM_CUBIC (not linear in m)");
         return NM_EUNSUPPORTED;
     }
     return NM_OK;

@@ -618,6 +618,173 @@ k_pz_mid64(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int n
     }
 }
 
+// ---- z pass, fp64, 128 cells along z -----------------------------------------------------------------
+// k_pz_mid64 for M = 8: a team transforms two lines, so a warp owns two columns and four warps a tile;
+// warps 0-3 take the +ky tile of an item and warps 4-7 the -ky tile (same folded tensor rows).  The
+// region holds the tile pair (2 x 48 KB), then the tensor rows of the eight columns (48.75 KB).
+struct Pz64Smem8 {
+    static constexpr int N = 128;
+    static constexpr int TILE_ELEMS = 3 * N * TW;                   // complex doubles
+    static constexpr int TILE_BYTES = TILE_ELEMS * 16;              // 49152
+    static constexpr int KZP = 130;
+    static constexpr int TSLICE = 6 * KZP;
+    static constexpr int TENS_BYTES = TW * TSLICE * 8;              // 49920, one bulk copy
+    static constexpr int REGION = 2 * TILE_BYTES;
+    static constexpr int OFF_SCR = REGION;
+    static constexpr int SCR_BYTES = 16 * Team<8>::SCRATCH64 * 16;
+    static constexpr int OFF_TW = OFF_SCR + SCR_BYTES;
+    static constexpr int TW_BYTES = 16 * 32 * 16;
+    static constexpr int OFF_BAR = OFF_TW + TW_BYTES;
+    static constexpr int BYTES = OFF_BAR + 32;
+};
+static_assert(Pz64Smem8::BYTES <= 227 * 1024 && Pz64Smem8::TENS_BYTES <= Pz64Smem8::REGION, "k_pz_mid64_8 shared memory");
+
+template <bool EMB>
+__global__ void __launch_bounds__(kPipeThreads, 1)
+k_pz_mid64_8(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int nItems, int kt0,
+             const double2 *__restrict__ wP, int n3v)
+{
+    typedef double T;
+    typedef double2 V;
+    typedef Pz64Smem8 S;
+    constexpr int M = 8, N = 128, P = 256;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    V *s_B = reinterpret_cast<V *>(smem);
+    const T *s_T = reinterpret_cast<const T *>(smem);
+    V *s_scr = reinterpret_cast<V *>(smem + S::OFF_SCR);
+    V *s_tw = reinterpret_cast<V *>(smem + S::OFF_TW);
+    uint64_t *fullB = reinterpret_cast<uint64_t *>(smem + S::OFF_BAR);
+    uint64_t *fullT = fullB + 1;
+    unsigned *cnt = reinterpret_cast<unsigned *>(fullT + 1);
+
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int sub = w >> 2, cp = w & 3;
+    const int h = lane & 1, i = lane >> 1;
+    const int l = i >> 3, j = i & 7;
+    const int k1 = 2 * cp + l;
+    const int P2 = 2 * N2, K2 = N2 + 1;
+    const int G = gridDim.x;
+
+    auto tile_ptr = [&](int g, int sb) -> V * {
+        const int kyf = g % K2, ktl = g / K2;
+        const int ky = sb ? P2 - kyf : kyf;
+        return B + ((long long)ktl * P2 + ky) * S::TILE_ELEMS;
+    };
+    auto n_tiles = [&](int g) -> int {
+        const int kyf = g % K2;
+        return (kyf == 0 || kyf == N2) ? 1 : 2;
+    };
+    auto load_item = [&](int g) {
+        const int nt = n_tiles(g);
+        mbar_expect_tx(fullB, nt * S::TILE_BYTES);
+        for (int sb = 0; sb < nt; ++sb) bulk_load(s_B + sb * S::TILE_ELEMS, tile_ptr(g, sb), S::TILE_BYTES, fullB);
+    };
+    if (tid == 0) {
+        mbar_init(fullB, 1);
+        mbar_init(fullT, 1);
+        cnt[0] = cnt[1] = 0;
+        mbar_fence_init();
+    }
+    for (int q = tid; q < 16 * 32; q += kPipeThreads) {
+        const int tp = q >> 5, ln = q & 31;
+        s_tw[q] = wP[(((ln >> 1) & 7) * (2 * tp + (ln & 1))) & (P - 1)];
+    }
+    __syncthreads();
+    if (tid == 0 && (int)blockIdx.x < nItems) load_item(blockIdx.x);
+    const V *tws = s_tw + lane;
+    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH64;
+    const T *ts = s_T + k1 * S::TSLICE;
+    uint32_t ph = 0;
+
+    for (int g = blockIdx.x; g < nItems; g += G, ph ^= 1) {
+        const int kyf = g % K2, kt = kt0 + g / K2;
+        const int nt = (kyf == 0 || kyf == N2) ? 1 : 2;
+        const bool work = sub < nt;
+        // element (c, e = j + 8 t) of column k1: row (c N + e), slot k1 ^ swz(e) ^ swz(ky); swz(j + 8 t) = (j >> 1) ^ 4 (t & 1)
+        const int cw = k1 ^ swz(sub ? P2 - kyf : kyf) ^ (j >> 1);
+        const int offE = j * TW + cw, offO = j * TW + (cw ^ 4);
+        mbar_wait(fullB, ph);
+        V a[3][16];
+        if (work) {
+            const V *tb = s_B + sub * S::TILE_ELEMS;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    a[c][t] = tb[((t & 1) ? offO : offE) + (c * N + M * t) * TW];
+                    if (EMB && j + M * t >= n3v) a[c][t] = mk<T>((T)0, (T)0);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0 && (arrive_count(cnt) & 7) == 7) {
+            mbar_expect_tx(fullT, S::TENS_BYTES);
+            bulk_load(smem, Tn + ((long long)kt * K2 + kyf) * TW * S::TSLICE, S::TENS_BYTES, fullT);
+        }
+        if (work) {
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, false>(a[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                dft16<T, false>(a[c]);
+                fwd_put_s<T, M, 32>(a[c], tws, scr, i);
+                fwd_get<T, M>(a[c], scr, i);
+                dftM<T, false, M>(a[c]);
+            }
+        }
+        mbar_wait(fullT, ph);
+        if (work) {
+            const T sy = sub ? (T)-1 : (T)1;
+#pragma unroll
+            for (int s = 0; s < 16; ++s) {
+                const int u = s / M, r8 = rev8(s % M);
+                const int kz = 2 * slot_freq<M>(j, s) + h;
+                const bool up = r8 > 4 || (r8 == 4 && (j | u | h) != 0);
+                const int kzf = up ? P - kz : kz;
+                const T sz = up ? (T)-1 : (T)1;
+                const T *tp = ts + kzf;
+                const T nxx = tp[0], nyy = tp[S::KZP], nzz = tp[2 * S::KZP];
+                const T nxy = sy * tp[3 * S::KZP], nxz = sz * tp[4 * S::KZP], nyz = sy * sz * tp[5 * S::KZP];
+                const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
+                const V hx = caxpy(nxz, mz, caxpy(nxy, my_, cscale(nxx, mx)));
+                const V hy = caxpy(nyz, mz, caxpy(nyy, my_, cscale(nxy, mx)));
+                const V hz = caxpy(nzz, mz, caxpy(nyz, my_, cscale(nxz, mx)));
+                a[0][s] = mk<T>(-hx.x, -hx.y);
+                a[1][s] = mk<T>(-hy.x, -hy.y);
+                a[2][s] = mk<T>(-hz.x, -hz.y);
+            }
+        }
+        __syncwarp();
+        if (lane == 0 && (arrive_count(cnt + 1) & 7) == 7 && g + G < nItems) load_item(g + G);
+        if (work) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                dftM<T, true, M>(a[c]);
+                inv_put<T, M>(a[c], scr, i);
+                inv_get_s<T, M, 32>(a[c], tws, scr, i);
+                dft16<T, true>(a[c]);
+            }
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, true>(a[c]);
+            }
+            V *out = tile_ptr(g, sub);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    V v = a[c][t];
+                    v = cadd(v, shfl1(v));
+                    if ((t >> 3) == h) out[((t & 1) ? offO : offE) + (c * N + M * t) * TW] = v;
+                }
+            }
+        }
+    }
+}
+
+
 // ---- x passes ----------------------------------------------------------------------------------
 // Geometry shared by k_px_fwd / k_px_inv for N1 = 16 M: a CTA of 8 warps owns R = 2 LINES cell rows
 // (c2) of one cell plane c3; warp w transforms LINES/8 = 16/M complex lines, each packing the two
@@ -1278,7 +1445,7 @@ k_py_inv8(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N
 bool nm_pipe_mid_ok(const nm_mesh *mesh)
 {
     if (!mesh->fast.on || !mesh->fast.pipe) return false;
-    if (mesh->f64) return mesh->fast.M3 == 16 && mesh->fast.Kzp == Pz64Smem::KZP;
+    if (mesh->f64) return (mesh->fast.M3 == 16 && mesh->fast.Kzp == Pz64Smem::KZP) || (mesh->fast.M3 == 8 && mesh->fast.Kzp == Pz64Smem8::KZP);
     return (mesh->fast.M3 == 16 && mesh->fast.Kzp == PzSmem::KZP) || (mesh->fast.M3 == 8 && mesh->fast.Kzp == Pz8Smem::KZP);
 }
 
@@ -1288,6 +1455,16 @@ nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     const int nItems = nkt * g.K2;
     const int grid = nItems < mesh->sm_count ? nItems : mesh->sm_count;
     NmLaunchScope sc(mesh, NM_K_MID, st);
+    if (mesh->f64 && mesh->fast.M3 == 8) {
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pz64Smem8::BYTES));
+            kern<<<grid, kPipeThreads, Pz64Smem8::BYTES, st>>>((double2 *)mesh->bufB, (const double *)mesh->fast.Tn, mesh->fast.F2,
+                                                              nItems, kt0, (const double2 *)mesh->tw_z, g.N3);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_pz_mid64_8<true>) : go(k_pz_mid64_8<false>));
+        return NM_OK;
+    }
     if (mesh->f64) {
         auto go = [&](auto kern) -> nm_status {
             NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pz64Smem::BYTES));

@@ -47,6 +47,7 @@ CASES = [
     ("128x16x16 f64 (k_px_* f64, k_node_col f64)", lambda: _cube((128, 32, 16)), "f64", 1),
     ("32x256x32 f64 (k_py_fwd / k_py_inv in fp64)", lambda: _cube((32, 256, 32)), "f64", 1),
     ("32x32x256 f64 (k_pz_mid64)", lambda: _cube((32, 32, 256)), "f64", 1),
+    ("32x128x128 f64 (k_pz_mid64_8, k_py_*8 in fp64)", lambda: _cube((32, 128, 128)), "f64", 1),
 ]
 
 

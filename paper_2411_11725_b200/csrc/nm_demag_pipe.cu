@@ -1280,25 +1280,27 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict_
 // B side: 256 rows of 128 bytes (ky; both planes), one 4-D box.  Lane = (j, line, half) with the line
 // in bit 1, so that a half-warp scatters into both 64-byte halves of the B rows (the slot parity of
 // an output is the same for every lane, which leaves a two-way conflict on that side).
-struct Py8Smem {
+template <typename T> struct Py8Smem {
+    typedef typename VT<T>::V V;
     static constexpr int N = 128, P = 256;
-    static constexpr int LINE_ELEMS = N * TW;                               // 1024 complex, 8 KB
-    static constexpr int A_ELEMS = 2 * LINE_ELEMS + 16;                     // two lines, 16 B skew, padded to 128 B
-    static constexpr int A_BYTES = A_ELEMS * 8;
-    static constexpr int B_ELEMS = P * 2 * TW, B_BYTES = B_ELEMS * 8;       // 32768
-    static constexpr int SCR_BYTES = 16 * Team<8>::SCRATCH * 8;
+    static constexpr int LINE_ELEMS = N * TW;                               // 1024 complex, 8 KB (fp32) / 16 KB
+    static constexpr int A_ELEMS = 2 * LINE_ELEMS + 16;                     // two lines, 2 elements of skew, padded to 128 B
+    static constexpr int A_BYTES = A_ELEMS * (int)sizeof(V);
+    static constexpr int B_ELEMS = P * 2 * TW, B_BYTES = B_ELEMS * (int)sizeof(V);   // 32768 / 65536
+    static constexpr int SCR_BYTES = 16 * team_scratch<T, 8>() * (int)sizeof(V);
     static constexpr int FWD_BYTES = 2 * A_BYTES + B_BYTES + SCR_BYTES + 64;
     static constexpr int INV_BYTES = B_BYTES + A_BYTES + SCR_BYTES + 64;
+    static constexpr int CTAS = sizeof(T) == 8 ? 1 : 2;
 };
+static_assert(Py8Smem<double>::FWD_BYTES <= 227 * 1024, "k_py_fwd8<double> shared memory exceeds the sm_100a per-CTA limit");
 
-template <bool EMB>
-__global__ void __launch_bounds__(kPipeThreads, 2)
-k_py_fwd8(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
-          const float2 *__restrict__ wP, int n2v)
+template <typename T, bool EMB>
+__global__ void __launch_bounds__(kPipeThreads, Py8Smem<T>::CTAS)
+k_py_fwd8(const typename VT<T>::V *__restrict__ A, const __grid_constant__ NmTensorMap tmB, int N3, int nTiles, int kt0,
+          const typename VT<T>::V *__restrict__ wP, int n2v)
 {
-    typedef float T;
-    typedef float2 V;
-    typedef Py8Smem S;
+    typedef typename VT<T>::V V;
+    typedef Py8Smem<T> S;
     constexpr int M = 8;
     extern __shared__ __align__(1024) unsigned char smem[];
     V *s_out = reinterpret_cast<V *>(smem);                                 // [P][2][8]
@@ -1318,9 +1320,9 @@ k_py_fwd8(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB,
     // tile tl -> (ktl, comp, plane pair q), q fastest: consecutive tiles are consecutive 16 KB of A
     auto load_a = [&](int tl, int b) {
         const V *src = A + ((long long)kt0 * 3 * H3 + tl) * 2 * S::LINE_ELEMS;
-        mbar_expect_tx(full + b, 2 * S::LINE_ELEMS * 8);
-        bulk_load(s_in + b * S::A_ELEMS, src, S::LINE_ELEMS * 8, full + b);
-        bulk_load(s_in + b * S::A_ELEMS + S::LINE_ELEMS + 2, src + S::LINE_ELEMS, S::LINE_ELEMS * 8, full + b);
+        mbar_expect_tx(full + b, 2 * S::LINE_ELEMS * (int)sizeof(V));
+        bulk_load(s_in + b * S::A_ELEMS, src, S::LINE_ELEMS * (int)sizeof(V), full + b);
+        bulk_load(s_in + b * S::A_ELEMS + S::LINE_ELEMS + 2, src + S::LINE_ELEMS, S::LINE_ELEMS * (int)sizeof(V), full + b);
     };
     if (tid == 0) {
         for (int q = 0; q < 2; ++q)
@@ -1328,7 +1330,7 @@ k_py_fwd8(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB,
     }
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     // element e = j + 8 t of line l: row e, slot w ^ swz(e), swz(j + 8 t) = (j >> 1) ^ 4 (t & 1)
     const int cinE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1));
     const int cinO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1) ^ 4);
@@ -1370,13 +1372,13 @@ k_py_fwd8(const float2 *__restrict__ A, const __grid_constant__ NmTensorMap tmB,
     if (tid == 0) bulk_wait<0>();
 }
 
-__global__ void __launch_bounds__(kPipeThreads, 2)
-k_py_inv8(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N3, int nTiles, int kt0,
-          const float2 *__restrict__ wP)
+template <typename T>
+__global__ void __launch_bounds__(kPipeThreads, Py8Smem<T>::CTAS)
+k_py_inv8(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict__ A, int N3, int nTiles, int kt0,
+          const typename VT<T>::V *__restrict__ wP)
 {
-    typedef float T;
-    typedef float2 V;
-    typedef Py8Smem S;
+    typedef typename VT<T>::V V;
+    typedef Py8Smem<T> S;
     constexpr int M = 8;
     extern __shared__ __align__(1024) unsigned char smem[];
     V *s_in = reinterpret_cast<V *>(smem);                                  // [P][2][8]
@@ -1400,7 +1402,7 @@ k_py_inv8(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N
     if (tid == 0 && (int)blockIdx.x < nTiles) load_b(blockIdx.x);
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
-    V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     const int coutE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1));
     const int coutO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1) ^ 4);
     int n = 0;
@@ -1431,8 +1433,8 @@ k_py_inv8(const __grid_constant__ NmTensorMap tmB, float2 *__restrict__ A, int N
         __syncthreads();
         if (tid == 0) {
             V *dst = A + ((long long)kt0 * 3 * H3 + tl) * 2 * S::LINE_ELEMS;
-            bulk_store(dst, s_out, S::LINE_ELEMS * 8);
-            bulk_store(dst + S::LINE_ELEMS, s_out + S::LINE_ELEMS + 2, S::LINE_ELEMS * 8);
+            bulk_store(dst, s_out, S::LINE_ELEMS * (int)sizeof(V));
+            bulk_store(dst + S::LINE_ELEMS, s_out + S::LINE_ELEMS + 2, S::LINE_ELEMS * (int)sizeof(V));
             bulk_commit();
         }
     }
@@ -1584,7 +1586,7 @@ nm_status nm_pipe_setup(nm_mesh *mesh)
 {
     mesh->fast.tmapB_ok = false;
     if (!mesh->fast.on || !mesh->fast.pipe) return NM_OK;
-    const bool y8 = !mesh->f64 && mesh->fast.M2 == 8 && mesh->g.N3 % 2 == 0;     // two planes per tile (fp32 only)
+    const bool y8 = mesh->fast.M2 == 8 && mesh->g.N3 % 2 == 0;     // two planes per tile
     if (mesh->fast.M2 != 16 && !y8) return NM_OK;
     void *fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -1638,31 +1640,38 @@ template <typename T> static nm_status launch_py16(nm_mesh *mesh, bool inverse, 
     return NM_OK;
 }
 
+template <typename T> static nm_status launch_py8(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st)
+{
+    typedef typename VT<T>::V V;
+    typedef Py8Smem<T> S;
+    const NmGeom &g = mesh->g;
+    const int nTiles = nkt * 3 * (g.N3 / 2);
+    const int cap = S::CTAS * mesh->sm_count;
+    const int grid = nTiles < cap ? nTiles : cap;
+    if (!inverse) {
+        NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::FWD_BYTES));
+            kern<<<grid, kPipeThreads, S::FWD_BYTES, st>>>((const V *)mesh->bufA, mesh->fast.tmapB, g.N3, nTiles, kt0,
+                                                           (const V *)mesh->tw_y, g.N2);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_py_fwd8<T, true>) : go(k_py_fwd8<T, false>));
+    } else {
+        NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv8<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::INV_BYTES));
+        NmLaunchScope sc(mesh, NM_K_Y_INV, st);
+        k_py_inv8<T><<<grid, kPipeThreads, S::INV_BYTES, st>>>(mesh->fast.tmapB, (V *)mesh->bufA, g.N3, nTiles, kt0,
+                                                             (const V *)mesh->tw_y);
+    }
+    return NM_OK;
+}
+
 bool nm_pipe_y_ok(const nm_mesh *mesh) { return mesh->fast.on && mesh->fast.pipe && mesh->fast.tmapB_ok; }
 
 nm_status nm_pipe_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t st)
 {
     const NmGeom &g = mesh->g;
-    if (mesh->fast.M2 == 8) {
-        const int nTiles = nkt * 3 * (g.N3 / 2);
-        const int grid = nTiles < 2 * mesh->sm_count ? nTiles : 2 * mesh->sm_count;
-        if (!inverse) {
-            NmLaunchScope sc(mesh, NM_K_Y_FWD, st);
-            auto go = [&](auto kern) -> nm_status {
-                NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Py8Smem::FWD_BYTES));
-                kern<<<grid, kPipeThreads, Py8Smem::FWD_BYTES, st>>>((const float2 *)mesh->bufA, mesh->fast.tmapB, g.N3, nTiles,
-                                                                      kt0, (const float2 *)mesh->tw_y, g.N2);
-                return NM_OK;
-            };
-            NM_TRY(mesh->fast.embed ? go(k_py_fwd8<true>) : go(k_py_fwd8<false>));
-        } else {
-            NM_CUDA_TRY(cudaFuncSetAttribute(k_py_inv8, cudaFuncAttributeMaxDynamicSharedMemorySize, Py8Smem::INV_BYTES));
-            NmLaunchScope sc(mesh, NM_K_Y_INV, st);
-            k_py_inv8<<<grid, kPipeThreads, Py8Smem::INV_BYTES, st>>>(mesh->fast.tmapB, (float2 *)mesh->bufA, g.N3, nTiles, kt0,
-                                                                      (const float2 *)mesh->tw_y);
-        }
-        return NM_OK;
-    }
+    if (mesh->fast.M2 == 8) return mesh->f64 ? launch_py8<double>(mesh, inverse, kt0, nkt, st) : launch_py8<float>(mesh, inverse, kt0, nkt, st);
     if (mesh->f64) return launch_py16<double>(mesh, inverse, kt0, nkt, st);
     return launch_py16<float>(mesh, inverse, kt0, nkt, st);
 }

@@ -510,8 +510,8 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
             if (v != 1) smooth = false;
         }
         const long long fill = (long long)N[1] * N[2] * 4, plane = (long long)F[1] * F[2];
-        // (fp64 has pipelined y / z kernels at 256 cells only: smaller extended planes must be fuller to pay)
-        const bool piped = d->dtype != NM_F64 || (F[1] == 256 && F[2] == 256);
+        // (fp64 has pipelined y / z kernels at 128 and 256 cells only: smaller extended planes must be fuller to pay)
+        const bool piped = d->dtype != NM_F64 || ((F[1] == 256 || F[1] == 128) && (F[2] == 256 || F[2] == 128));
         if (smooth && fill < (piped ? 2 : 3) * plane) return;
         if (N[1] % (2 * 8 * LTx) != 0 || N[0] % vec != 0) return;              // whole x-pass CTAs of rows, 16-byte cell rows
         if (N[2] % (16 / M[1]) != 0) return;                                   // whole y-pass CTAs of planes

@@ -3,7 +3,7 @@
 The workload bench.py times (config 4, 256^3, fp32, exchange + demag, scalar materials: pipelined
 fast demag path, k_node_col) is compared with the fp64 oracle at every node, on the bench's own
 seeded dense random m, and so is the 192^3 point of the sweep; fp64 is compared densely at 128^3
-(fast path, k_fz_mid) and 96^3 (general radix-2/3 path).  The oracle's __float128 tensor table of
+(pipelined fp64 kernels), 96^3 and 192^3 (zero-extended to 128^3 / 256^3).  The oracle's __float128 tensor table of
 the 256^3 grid takes a few minutes on the host cores; the smaller config-4 grids slice it
 (tests/_sides.py:oracle_tensor).  Beside the dense checks stay the ones the oracle computes output by
 output (sparse sources) and the closed form that holds at any size (magnetometric factor -1/3 of a
@@ -53,12 +53,12 @@ def test_heff_and_rhs_dense_parity_bench_size_fp32(N):
 
 @pytest.mark.parametrize("prec,N", [("f32", 128), ("f32", 96), ("f64", 128), ("f64", 96), ("f64", 192)])
 def test_heff_and_rhs_dense_parity_mid_sizes(prec, N):
-    """Config 4 at 128^3 (fp32: k_py_fwd8 / k_pz_mid8; fp64: the one-CTA-per-tile fast kernels,
-    k_fz_mid), 96^3 (fp32: zero-extended to 128^3; fp64: general radix-2/3 path) and 192^3 in fp64
-    (zero-extended to 256^3: k_py_fwd / k_py_inv<double>, k_pz_mid64 with masked rows), every node.
+    """Config 4 at 128^3 (fp32: k_py_fwd8 / k_pz_mid8; fp64: k_py_fwd8 / k_py_inv8<double>, k_pz_mid64_8),
+    96^3 (zero-extended to 128^3 in both precisions) and 192^3 in fp64 (zero-extended to 256^3:
+    k_py_fwd / k_py_inv<double>, k_pz_mid64 with masked rows), every node.
     (3-7 s each with the sliced tensor table; 192: ~25 s.)"""
     mesh = _dense_case(N, prec)
-    want = {("f32", 128): 1, ("f32", 96): 2, ("f64", 128): 1, ("f64", 96): 0, ("f64", 192): 2}[(prec, N)]
+    want = {("f32", 128): 1, ("f32", 96): 2, ("f64", 128): 1, ("f64", 96): 2, ("f64", 192): 2}[(prec, N)]
     assert mesh.nm_debug_demag_path() == want
 
 

@@ -797,9 +797,10 @@ template <typename T, int M> struct PxGeom {
     static constexpr int PZ = P + 8;            // pitch of a packed spectrum line
     static constexpr int SCR = team_scratch<T, M>();
     static constexpr size_t FWD_BYTES = ((size_t)LINES * YP + (size_t)LINES * PZ + 16 * SCR) * 2 * sizeof(T);
-    // forward, bulk-fed (fp32, M >= 4): the packed lines of a warp live in that warp's own exchange scratch
+    // forward, bulk-fed (M >= 4): the packed lines of a warp live in that warp's own exchange scratch
     // (LT PZ <= 2 SCR), and a raw buffer takes the R + 1 node rows of the two planes of the next component
-    static constexpr bool BULK_OK = sizeof(T) == 4 && LT * PZ <= 2 * SCR;
+    static constexpr bool BULK_OK = LT * PZ <= 2 * SCR;     // M >= 4
+    static constexpr int AL = 16 / (int)sizeof(T);          // elements per 16 bytes: bulk copies start and end on these
     __host__ __device__ static constexpr int raw_pitch(int n1) { return ((R + 1) * n1 + 6 + 31) & ~31; }     // reals per plane
     static size_t fwd_bulk_bytes(int n1) { return ((size_t)LINES * YP + 16 * SCR) * 2 * sizeof(T) + (size_t)2 * raw_pitch(n1) * sizeof(T) + 16; }
     // inverse: output tile (R x N reals) + exchange scratch + staged spectrum rows of one component, the
@@ -841,7 +842,7 @@ template <> __device__ __forceinline__ void load2<double2>(const double2 *src, d
 //            by one thread, 16-byte stores
 // EMB (embedded mesh, nm_fast_plan): the mesh has N1 <= N cells per row; cells beyond it are zero, node
 // columns beyond n1 are not read, and the rows of A have pitch f2 (the y transform extent) >= N2.
-// BULK (fp32, M >= 4, 16-byte aligned field): the node rows of a component -- R + 1 contiguous rows in each of the
+// BULK (M >= 4, 16-byte aligned field): the node rows of a component -- R + 1 contiguous rows in each of the
 // two planes -- arrive by two bulk copies issued one component ahead (from the 16-byte boundary below their
 // start: `shift` elements into the buffer), so phase 1 reads shared memory and the HBM latency is off the path.
 template <typename T, int M, bool UNI, bool EMB, bool BULK>
@@ -852,7 +853,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
     constexpr int N = G::N, P = G::P, LT = G::LT, LINES = G::LINES, R = G::R, NKT = G::NKT;
-    static_assert(!BULK || G::BULK_OK, "bulk-fed x pass: fp32 and M >= 4");
+    static_assert(!BULK || G::BULK_OK, "bulk-fed x pass: M >= 4");
     extern __shared__ __align__(1024) unsigned char smem[];
     V *s_y = reinterpret_cast<V *>(smem);                   // LINES x YP
     V *s_z = s_y + LINES * G::YP;                           // LINES x PZ (BULK: inside the scratch, per warp)
@@ -905,18 +906,18 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
             zlast = (!EMB || N < g.n1) ? (q[0] + q[plane]) + (q[g.n1] + q[plane + g.n1]) : (T)0;
         }
     };
-    constexpr bool PREF = sizeof(T) == 8;                   // fp32 (two CTAs per SM, 128 registers): measured slower
-    // BULK: thread 0 requests the rows of a component; element e0 of the array lands at s_raw[p RP + (e0 & 3)]
+    constexpr bool PREF = sizeof(T) == 8 && !BULK;          // register prefetch: the fp64 form without the raw-row buffer (fp32: measured slower)
+    // BULK: thread 0 requests the rows of a component; element e0 of the array lands at s_raw[p RP + (e0 & (AL - 1))]
     const int nodes3 = 3 * (int)g.nodes;
     auto request = [&](int comp, int rr0, int cc3) {
         int e0[2], len[2], total = 0;
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
             const int e = comp * (int)g.nodes + (cc3 + p) * (int)plane + rr0 * g.n1;
-            e0[p] = e & ~3;
-            len[p] = ((R + 1) * g.n1 + (e & 3) + 3) & ~3;
+            e0[p] = e & ~(G::AL - 1);
+            len[p] = ((R + 1) * g.n1 + (e & (G::AL - 1)) + G::AL - 1) & ~(G::AL - 1);
             if (e0[p] + len[p] > nodes3) {                  // the array ends inside the last 16 bytes: its last elements by hand
-                len[p] = (nodes3 - e0[p]) & ~3;
+                len[p] = (nodes3 - e0[p]) & ~(G::AL - 1);
                 for (int q = e0[p] + len[p]; q < nodes3; ++q) s_raw[p * RP + q - e0[p]] = fld[q];
             }
             total += len[p];
@@ -926,8 +927,8 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
         for (int p = 0; p < 2; ++p) bulk_load(s_raw + p * RP, fld + e0[p], (uint32_t)(len[p] * sizeof(T)), full);
     };
     auto take_z = [&](int comp) {
-        const int sh0 = (comp * (int)g.nodes + c3 * (int)plane + r0 * g.n1) & 3;
-        const int sh1 = (comp * (int)g.nodes + (c3 + 1) * (int)plane + r0 * g.n1) & 3;
+        const int sh0 = (comp * (int)g.nodes + c3 * (int)plane + r0 * g.n1) & (G::AL - 1);
+        const int sh1 = (comp * (int)g.nodes + (c3 + 1) * (int)plane + r0 * g.n1) & (G::AL - 1);
         const T *q0 = s_raw + sh0 + rg * 16 * g.n1 + col, *q1 = s_raw + RP + sh1 + rg * 16 * g.n1 + col;
 #pragma unroll
         for (int r = 0; r < 17; ++r) z[r] = (!EMB || col < g.n1) ? q0[r * g.n1] + q1[r * g.n1] : (T)0;
@@ -1524,8 +1525,9 @@ template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, co
                 const size_t bytes = G::fwd_bulk_bytes(g.n1);
                 // whole grids (not split by component): persistent CTAs, two per SM, over the tiles
                 const int ntiles = (int)(grid.x * grid.y);
-                const bool persist = !split && ntiles > 2 * mesh->sm_count;
-                const dim3 pgrid = persist ? dim3(2 * mesh->sm_count, 1, 1) : grid;
+                const int per_sm = sizeof(T) == 8 ? 1 : 2;
+                const bool persist = !split && ntiles > per_sm * mesh->sm_count;
+                const dim3 pgrid = persist ? dim3(per_sm * mesh->sm_count, 1, 1) : grid;
                 auto gob = [&](auto kern, T msv) -> nm_status {
                     NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
                     kern<<<pgrid, kPipeThreads, bytes, st>>>(fld, (const T *)mesh->Ms, msv, (V *)mesh->bufA, g,

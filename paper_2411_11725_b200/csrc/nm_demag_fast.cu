@@ -63,7 +63,7 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
 #pragma unroll
     for (int t = 0; t < 16; ++t) {
         const int e = j + M * t;
-        V v = s_io[(sub * N + e) * TW + (k1 ^ swz(e))];
+        V v = s_io[(sub * N + e) * TW + (k1 ^ swzT<T>(e))];
         if (e >= n2v) v = mk<T>((T)0, (T)0);                // embedded mesh: rows the x pass never wrote
         if (h) v = cmul(v, wP[e]);
         a[t] = v;
@@ -71,11 +71,11 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
     __syncthreads();   // the input tile is dead; s_io becomes the output tile
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
     fft_fwd<T, M>(a, tw, scr, i);
-    const int sl = k1 ^ swz(c3_0 + sub);
+    const int sl = k1 ^ swzT<T>(c3_0 + sub);
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int ky = 2 * slot_freq<M>(j, s) + h;
-        s_io[ky * OUT_PITCH + sub * TW + (sl ^ swz(ky))] = a[s];
+        s_io[ky * OUT_PITCH + sub * TW + (sl ^ swzT<T>(ky))] = a[s];
     }
     __syncthreads();
     // rows of LT*8 complex, one per ky
@@ -115,11 +115,11 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
     V tw[16];
     load_twiddles2<T, M>(tw, wP, j);
     V a[16];
-    const int sl = k1 ^ swz(c3_0 + sub);
+    const int sl = k1 ^ swzT<T>(c3_0 + sub);
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
         const int ky = 2 * slot_freq<M>(j, s) + h;
-        a[s] = s_io[ky * PITCH + sub * TW + (sl ^ swz(ky))];
+        a[s] = s_io[ky * PITCH + sub * TW + (sl ^ swzT<T>(ky))];
     }
     __syncthreads();
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
@@ -131,7 +131,7 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
         if (h) v = cmulc(v, wP[e]);
         // sum of the even and odd halves: partner lane = lane ^ 1
         v = cadd(v, shfl1(v));
-        if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ swz(e))] = v;
+        if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ swzT<T>(e))] = v;
     }
     __syncthreads();
     V *dst = A + ((((long long)kt * 3 + comp) * N3 + c3_0) * N) * TW;
@@ -174,13 +174,13 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     load_twiddles2<T, M>(tw, wP, j);
     V a[3][16];
     V *my = s_io + (sub * 3) * N * TW;
-    const int kq = k1 ^ swz(ky0 + sub);                     // rows of B are swizzled by c3 and by ky
+    const int kq = k1 ^ swzT<T>(ky0 + sub);                     // rows of B are swizzled by c3 and by ky
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
             const int e = j + M * t;
-            V v = my[(c * N + e) * TW + (kq ^ swz(e))];
+            V v = my[(c * N + e) * TW + (kq ^ swzT<T>(e))];
             if (EMB && e >= n3v) v = mk<T>((T)0, (T)0);     // embedded mesh: planes the y pass never wrote
             if (h) v = cmul(v, wP[e]);
             a[c][t] = v;
@@ -218,7 +218,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
             V v = a[c][t];
             if (h) v = cmulc(v, wP[e]);
             v = cadd(v, shfl1(v));
-            if ((t >> 3) == h) my[(c * N + e) * TW + (kq ^ swz(e))] = v;
+            if ((t >> 3) == h) my[(c * N + e) * TW + (kq ^ swzT<T>(e))] = v;
         }
     }
     __syncthreads();
@@ -281,7 +281,7 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
             const int kt = idx / (R * TW), rem = idx % (R * TW);
             const int r = rem / TW, slot = rem % TW;
             const int c2 = r0 + r;
-            const int k = kt * TW + (slot ^ swz(c2));
+            const int k = kt * TW + (slot ^ swzT<T>(c2));
             V out = mk<T>((T)0, (T)0);
             if (k <= N) {
                 const V zk = s_z[(r >> 1) * P + k];
@@ -324,7 +324,7 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             const int kt = idx / (R * TW), rem = idx % (R * TW);
             const int r = rem / TW, slot = rem % TW;
             const int c2 = r0 + r;
-            s_x[r * XP + kt * TW + (slot ^ swz(c2))] =
+            s_x[r * XP + kt * TW + (slot ^ swzT<T>(c2))] =
                 A[((((long long)kt * 3 + comp) * g.N3 + c3) * g.N2 + r0) * TW + rem];
         }
         __syncthreads();

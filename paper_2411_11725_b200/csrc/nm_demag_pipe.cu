@@ -518,7 +518,7 @@ k_pz_mid64(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int n
     const V *tws = s_tw + lane;
     V *scr = s_scr + (2 * w + h) * Team<M>::SCRATCH64;
     const T *ts = s_T + w * S::TSLICE;
-    const int cw0 = w ^ swz(j);          // swz(j + 16 t) = swz(j)
+    const int cw0 = w ^ swzT<T>(j);      // swz(j + 16 t) = swz(j)
     uint32_t ph = 0;
 
     for (int g = blockIdx.x; g < nItems; g += G) {
@@ -526,7 +526,7 @@ k_pz_mid64(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int n
         const int nt = (kyf == 0 || kyf == N2) ? 1 : 2;
         for (int sub = 0; sub < nt; ++sub, ph ^= 1) {
             mbar_wait(fullB, ph);
-            const int cwj = cw0 ^ swz(sub ? P2 - kyf : kyf);     // rows of B are swizzled by c3 and by ky
+            const int cwj = cw0 ^ swzT<T>(sub ? P2 - kyf : kyf); // rows of B are swizzled by c3 and by ky
             const int coff = j * TW + cwj;                        // element (c, e = j + 16 t): + (c N + 16 t) TW
             V a[3][16];
 #pragma unroll
@@ -700,8 +700,9 @@ k_pz_mid64_8(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int
         const int kyf = g % K2, kt = kt0 + g / K2;
         const int nt = (kyf == 0 || kyf == N2) ? 1 : 2;
         const bool work = sub < nt;
-        // element (c, e = j + 8 t) of column k1: row (c N + e), slot k1 ^ swz(e) ^ swz(ky); swz(j + 8 t) = (j >> 1) ^ 4 (t & 1)
-        const int cw = k1 ^ swz(sub ? P2 - kyf : kyf) ^ (j >> 1);
+        // element (c, e = j + 8 t) of column k1: row (c N + e), slot k1 ^ swz(e) ^ swz(ky); the fp64 swizzle of
+        // e = j + 8 t is that of j for even t and 4 slots further for odd t
+        const int cw = k1 ^ swzT<T>(sub ? P2 - kyf : kyf) ^ swzT<T>(j);
         const int offE = j * TW + cw, offO = j * TW + (cw ^ 4);
         mbar_wait(fullB, ph);
         V a[3][16];
@@ -991,7 +992,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
             const int q = idx & 3, ln = (idx >> 2) % LINES, kt = idx / (4 * LINES);
             const int c2 = r0 + 2 * ln;
             const int p0 = 2 * q;                           // physical slots p0, p0 + 1 of the blocked row
-            const int k0 = kt * TW + (p0 ^ swz(c2)), k1 = k0 ^ 1;
+            const int k0 = kt * TW + (p0 ^ swzT<T>(c2)), k1 = k0 ^ 1;
             const V *zl = zline(ln);
             V ze, zo;
             load2(zl + (k0 & ~1), ze, zo);
@@ -1004,7 +1005,8 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
             if (k1 > N) { a1 = mk<T>((T)0, (T)0); b1 = a1; }
             V *dst = A + ((((long long)kt * 3 + comp) * g.N3 + c3) * f2 + c2) * TW + p0;
             store2(dst, a0, a1);
-            store2(dst + TW, b0, b1);
+            // row c2 + 1 (c2 even): the same columns; its fp64 swizzle differs in slot bit 2
+            store2(dst + TW + (sizeof(T) == 8 ? (p0 ^ 4) - p0 : 0), b0, b1);
         }
     }
     }
@@ -1051,7 +1053,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     stage(comp_lo);
     // Xa, Xb of this thread's line: rows 2 line, 2 line + 1 of every block, column k1 at slot k1 ^ swz(c2)
     const V *ra = s_raw + (2 * line) * TW;
-    const int sw = swz(r0 + 2 * line);
+    const int sw = swzT<T>(r0 + 2 * line);
     for (int comp = comp_lo; comp < comp_hi; ++comp) {
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                                    // staged rows visible; the output tile has been read
@@ -1064,7 +1066,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             const bool up = k > N;
             const int kk = up ? P - k : k;
             const V *q = ra + (kk >> 3) * G::KP + ((kk & 7) ^ sw);
-            const V u = q[0], v = q[TW];
+            const V u = q[0], v = (sizeof(T) == 8 ? ra + (kk >> 3) * G::KP + ((kk & 7) ^ sw ^ 4) : q)[TW];   // row + 1: fp64 slot bit 2
             const T sg = up ? (T)-1 : (T)1;
             a[s] = mk<T>(u.x - sg * v.y, v.x + sg * u.y);
         }
@@ -1173,7 +1175,7 @@ k_py_fwd(const typename VT<T>::V *__restrict__ A, const __grid_constant__ NmTens
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
-    const int cin = j * TW + (w ^ swz(j));                  // A rows are swizzled by c2 = e, swz(j + 16 t) = swz(j)
+    const int cin = j * TW + (w ^ swzT<T>(j));              // A rows are swizzled by c2 = e, swz(j + 16 t) = swz(j)
     int n = 0;
     for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
         const int c3 = tl % N3, comp = (tl / N3) % 3, ktl = tl / (3 * N3);
@@ -1195,8 +1197,8 @@ k_py_fwd(const typename VT<T>::V *__restrict__ A, const __grid_constant__ NmTens
         fft_fwd<T, M, true>(a, tw, scr, j);
         if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
         __syncthreads();
-        // row ky = 2 (j + 16 rev16(s)) + h, column k1 = w swizzled by c3 and ky: swz(ky) = j & 7
-        V *out = s_out + (2 * j + h) * TW + (w ^ swz(c3) ^ (j & 7));
+        // row ky = 2 (j + 16 rev16(s)) + h, column k1 = w swizzled by c3 and ky: swz(ky) = swz(2 j + h)
+        V *out = s_out + (2 * j + h) * TW + (w ^ swzT<T>(c3) ^ swzT<T>(2 * j + h));
 #pragma unroll
         for (int s = 0; s < 16; ++s) out[32 * rev16(s) * TW] = a[s];
         fence_async_smem();
@@ -1242,12 +1244,12 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict_
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
-    const int cout = j * TW + (w ^ swz(j));
+    const int cout = j * TW + (w ^ swzT<T>(j));
     int n = 0;
     for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
         const int c3 = tl % N3;
         mbar_wait(full, (uint32_t)(n & 1));
-        const V *in = s_in + (2 * j + h) * TW + (w ^ swz(c3) ^ (j & 7));
+        const V *in = s_in + (2 * j + h) * TW + (w ^ swzT<T>(c3) ^ swzT<T>(2 * j + h));
         V a[16];
 #pragma unroll
         for (int s = 0; s < 16; ++s) a[s] = in[32 * rev16(s) * TW];
@@ -1332,9 +1334,9 @@ k_py_fwd8(const typename VT<T>::V *__restrict__ A, const __grid_constant__ NmTen
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
-    // element e = j + 8 t of line l: row e, slot w ^ swz(e), swz(j + 8 t) = (j >> 1) ^ 4 (t & 1)
-    const int cinE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1));
-    const int cinO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1) ^ 4);
+    // element e = j + 8 t of line l: row e, slot w ^ swz(e), swz(j + 8 t) = swz(j) ^ 4 (t & 1)
+    const int cinE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ swzT<T>(j));
+    const int cinO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ swzT<T>(j) ^ 4);
     int n = 0;
     for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
         const int q = tl % H3, comp = (tl / H3) % 3, ktl = tl / (3 * H3);
@@ -1355,13 +1357,13 @@ k_py_fwd8(const typename VT<T>::V *__restrict__ A, const __grid_constant__ NmTen
         if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
         __syncthreads();
         // slot s = 8 u + p holds ky = 2 (2 j + u + 16 rev8(p)) + h; element (ky, l): row 2 ky + l,
-        // column w swizzled by the plane pair and by ky: swz(ky) = (2 j + u) & 7
-        const int cs = w ^ swz(c3_0);
+        // column w swizzled by the plane and by ky: swz(ky) = swz(4 j + 2 u + h)
+        const int cs = w ^ swzT<T>(c3_0 + l);          // plane c3_0 + l of the pair
 #pragma unroll
         for (int s = 0; s < 16; ++s) {
             const int u = s / M, r8 = rev8(s % M);
             const int ky = 4 * j + 2 * u + 32 * r8 + h;
-            s_out[(2 * ky + l) * TW + (cs ^ ((2 * j + u) & 7))] = a[s];
+            s_out[(2 * ky + l) * TW + (cs ^ swzT<T>(4 * j + 2 * u + h))] = a[s];
         }
         fence_async_smem();
         __syncthreads();
@@ -1404,19 +1406,19 @@ k_py_inv8(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
-    const int coutE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1));
-    const int coutO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ (j >> 1) ^ 4);
+    const int coutE = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ swzT<T>(j));
+    const int coutO = l * (S::LINE_ELEMS + 2) + j * TW + (w ^ swzT<T>(j) ^ 4);
     int n = 0;
     for (int tl = blockIdx.x; tl < nTiles; tl += G, ++n) {
         const int c3_0 = 2 * (tl % H3);
         mbar_wait(full, (uint32_t)(n & 1));
-        const int cs = w ^ swz(c3_0);
+        const int cs = w ^ swzT<T>(c3_0 + l);          // plane c3_0 + l of the pair
         V a[16];
 #pragma unroll
         for (int s = 0; s < 16; ++s) {
             const int u = s / M, r8 = rev8(s % M);
             const int ky = 4 * j + 2 * u + 32 * r8 + h;
-            a[s] = s_in[(2 * ky + l) * TW + (cs ^ ((2 * j + u) & 7))];
+            a[s] = s_in[(2 * ky + l) * TW + (cs ^ swzT<T>(4 * j + 2 * u + h))];
         }
         __syncthreads();                                    // the stage is free again
         if (tid == 0 && tl + G < nTiles) load_b(tl + G);

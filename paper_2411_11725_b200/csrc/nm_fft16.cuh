@@ -33,6 +33,15 @@ constexpr int TW = 8;   // complex columns (k1) per blocked spectrum row
 // fall into 16 different 8-byte bank pairs of shared memory (row parity picks the half, swz the
 // slot), so the strided column reads of the consuming pass are conflict-free.
 __host__ __device__ __forceinline__ int swz(int r) { return (r >> 1) & 7; }
+// The swizzle by precision.  fp64 elements are 16 bytes and a row of 8 is the whole 128-byte bank period, so
+// which banks an access uses is the slot alone, and a 128-bit access is served eight lanes at a time: the rows
+// one such group touches -- four consecutive rows of a column (both halves of a team read the same element),
+// or eight consecutive rows where the halves own alternate rows -- must sit in different slots.  Row parity,
+// which picks the bank half in fp32, therefore goes into the slot: 8 consecutive rows -> slots 0,4,1,5,2,6,3,7.
+template <typename T> __host__ __device__ __forceinline__ int swzT(int r)
+{
+    return sizeof(T) == 8 ? (((r >> 1) & 7) ^ ((r & 1) << 2)) : ((r >> 1) & 7);
+}
 
 template <typename T> __device__ __forceinline__ typename VT<T>::V mk(T a, T b)
 {

@@ -20,7 +20,7 @@ from . import more_terms as _mt
 from .mesh import lumped_mass, n_nodes
 
 TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN = 1, 2, 4, 8
-TERM_DMI, TERM_CUBIC = 16, 32      # further local terms of PAPER.md:171 (oracle/more_terms.py)
+TERM_DMI, TERM_CUBIC, TERM_RKKY = 16, 32, 64      # further local terms of PAPER.md:79, 171 (oracle/more_terms.py)
 
 
 @dataclass
@@ -42,6 +42,8 @@ class Problem:
     dmi_normal: int = 2       # film normal of the interfacial form
     Kc: np.ndarray = None     # (N1,N2,N3) J/m^3, cubic anisotropy constant (TERM_CUBIC)
     cubic_axes: tuple = ((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0))
+    rkky_J: float = 0.0       # J/m^2, interlayer coupling between the node planes rkky_planes (TERM_RKKY)
+    rkky_planes: tuple = (0, 0)
 
     @staticmethod
     def uniform(n_cells, dx, Ms, A, Ku=0.0, **kw):
@@ -85,6 +87,8 @@ def effective_field(p, m, h_ext=None, parts=False, demag_direct=False):
         out["dmi"] = _lf.field_from_variation(_mt.variation_dmi(m, p.D, p.dx, p.dmi_kind, p.dmi_normal), L)
     if p.terms & TERM_CUBIC:
         out["cubic"] = _lf.field_from_variation(_mt.variation_cubic(m, p.Kc, p.cubic_axes, p.dx), L)
+    if p.terms & TERM_RKKY:
+        out["rkky"] = _lf.field_from_variation(_mt.variation_rkky(m, p.rkky_J, p.rkky_planes, p.dx), L)
     if parts:
         return out
     H = np.zeros_like(m, dtype=np.float64)
@@ -95,8 +99,8 @@ def effective_field(p, m, h_ext=None, parts=False, demag_direct=False):
 
 def _effective_field_lowdim(p, m, h_ext, parts, demag_direct):
     """effective_field with the reduced basis of Eqs. (23)-(24): the same terms through oracle/lowdim.py."""
-    if p.terms & (TERM_DMI | TERM_CUBIC):
-        raise NotImplementedError("DMI / cubic anisotropy are written for the 3-D basis only")
+    if p.terms & (TERM_DMI | TERM_CUBIC | TERM_RKKY):
+        raise NotImplementedError("DMI / cubic anisotropy / RKKY are written for the 3-D basis only")
     D = p.basis
     L = p.L
     out = {}

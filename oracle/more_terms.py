@@ -20,6 +20,12 @@ writes out the symmetric exchange only (Eq. 3); this file adds, through Eqs. (17
       quadrature", read as exact integration):
       dE_{c+i,j} += Kc_c sum_q w_q phi_i(x_q) de/dm_j (m^h(x_q))
 
+  interlayer (RKKY) coupling      E = -J int_Gamma m(x, y, z_a) . m(x, y, z_b) dGamma  across a spacer between the node
+      planes z_a and z_b ("interfacial energy contributions such as the RKKY coupling between two
+      ferromagnetic layers"), Gamma = the whole x-y cross-section; m^h restricted to a node plane is bilinear on
+      the faces, so with the 2-D element mass matrix M2[i,i'] = dx dy M1[i_x,i'_x] M1[i_y,i'_y]
+      dE_{(f+i, z_a)} += -J sum_{i'} M2[i,i'] m_{(f+i', z_b)}   and the same with a and b exchanged.
+
 Readings (rows F3): the paper names these terms without formulas; the densities above
 are the standard ones; D and Kc are cell-wise like every other material parameter (Eq. 15).
 """
@@ -150,5 +156,36 @@ def energy_cubic(m, Kc, axes, dx):
     return float(E)
 
 
-__all__ = ["dmi_tensor", "gradient_matrices", "variation_dmi", "energy_dmi", "variation_cubic", "energy_cubic",
+def variation_rkky(m, J, planes, dx):
+    """dE_{n,j} of E = -J int m(., z_a) . m(., z_b) dGamma; planes = (z_a, z_b) node-plane indices along axis 3."""
+    za, zb = int(planes[0]), int(planes[1])
+    dE = np.zeros_like(m, dtype=np.float64)
+    area = float(dx[0]) * float(dx[1])
+    for src, dst in ((zb, za), (za, zb)):
+        ms = m[:, :, :, src]                      # (3, n1, n2) on the source plane
+        out = dE[:, :, :, dst]
+        for i in ((0, 0), (0, 1), (1, 0), (1, 1)):
+            for ip in ((0, 0), (0, 1), (1, 0), (1, 1)):
+                w = -J * area * M1[i[0], ip[0]] * M1[i[1], ip[1]]
+                si = tuple(slice(1, None) if i[d] else slice(0, -1) for d in range(2))
+                sp = tuple(slice(1, None) if ip[d] else slice(0, -1) for d in range(2))
+                out[(slice(None),) + si] += w * ms[(slice(None),) + sp]
+    return dE
+
+
+def energy_rkky(m, J, planes, dx):
+    """E = -J sum_faces sum_{i,i'} M2[i,i'] m_{(f+i, z_a)} . m_{(f+i', z_b)}."""
+    za, zb = int(planes[0]), int(planes[1])
+    area = float(dx[0]) * float(dx[1])
+    a, b = m[:, :, :, za], m[:, :, :, zb]
+    E = 0.0
+    for i in ((0, 0), (0, 1), (1, 0), (1, 1)):
+        for ip in ((0, 0), (0, 1), (1, 0), (1, 1)):
+            si = tuple(slice(1, None) if i[d] else slice(0, -1) for d in range(2))
+            sp = tuple(slice(1, None) if ip[d] else slice(0, -1) for d in range(2))
+            E += -J * area * M1[i[0], ip[0]] * M1[i[1], ip[1]] * np.sum(a[(slice(None),) + si] * b[(slice(None),) + sp])
+    return float(E)
+
+
+__all__ = ["variation_rkky", "energy_rkky", "dmi_tensor", "gradient_matrices", "variation_dmi", "energy_dmi", "variation_cubic", "energy_cubic",
            "grad_phi_ref"]

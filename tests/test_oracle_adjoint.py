@@ -5,7 +5,7 @@ import pytest
 from oracle import adjoint, llg, mesh
 import dataclasses
 
-from oracle.llg import Problem, TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN, TERM_DMI, TERM_CUBIC
+from oracle.llg import Problem, TERM_EXCHANGE, TERM_DEMAG, TERM_ANISO, TERM_ZEEMAN, TERM_DMI, TERM_CUBIC, TERM_RKKY
 
 ALL = TERM_EXCHANGE | TERM_DEMAG | TERM_ANISO | TERM_ZEEMAN
 
@@ -24,6 +24,8 @@ def make(n=(3, 2, 2), alpha=0.1, terms=ALL, seed=0):
     if terms & TERM_DMI:        # cell-wise DMI constant; the interfacial kind when the demag term is off
         p = dataclasses.replace(p, D=rng.uniform(1e-3, 3e-3, n), dmi_kind="bulk" if terms & TERM_DEMAG else "interfacial",
                                 dmi_normal=1)
+    if terms & TERM_RKKY:
+        p = dataclasses.replace(p, rkky_J=2e-3, rkky_planes=(0, n[2]))
     return p, (lambda t: hext)
 
 
@@ -32,7 +34,7 @@ def with_Ms(p, Ms):
 
 
 @pytest.mark.parametrize("terms", [ALL, TERM_EXCHANGE | TERM_DEMAG, TERM_DEMAG, TERM_EXCHANGE | TERM_ANISO | TERM_ZEEMAN,
-                                   ALL | TERM_DMI, TERM_EXCHANGE | TERM_DMI, TERM_DMI])
+                                   ALL | TERM_DMI, TERM_EXCHANGE | TERM_DMI, TERM_DMI, ALL | TERM_RKKY, TERM_RKKY | TERM_DMI])
 def test_dense_jacobians_by_finite_differences(terms):
     """Explicit dense Jacobians of the oracle's own forward RHS by central differences on a
     3x2x2-cell mesh; both vector-Jacobian products must equal a^T J."""

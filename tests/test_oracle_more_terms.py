@@ -238,3 +238,67 @@ def test_terms_add_in_effective_field():
     parts = effective_field(p, m, parts=True)
     assert set(parts) == {"exchange", "dmi", "cubic"}
     assert np.allclose(effective_field(p, m), parts["exchange"] + parts["dmi"] + parts["cubic"])
+
+
+def _two_layers(n=(4, 3, 5), spacer=(2, 3)):
+    """Two magnetic layers separated by one vacuum cell layer (cells c3 = 2): node planes 2 and 3 face each other."""
+    Ms = np.full(n, 8e5)
+    Ms[:, :, spacer[0]:spacer[1]] = 0.0
+    return Ms
+
+
+def test_rkky_uniform_layers_closed_form():
+    """Uniform m_a on plane z_a and m_b on plane z_b: E = -J A (m_a . m_b) exactly; the variation on plane a
+    sums to -J A m_b; a corner node carries a quarter of an interior node's share."""
+    from oracle.llg import TERM_RKKY
+    n, dx = (4, 3, 5), np.array([2e-9, 3e-9, 1e-9])
+    J, planes = 1.5e-3, (2, 3)
+    nn = mesh.n_nodes(n)
+    ma, mb = np.array([0.6, 0.0, 0.8]), np.array([0.0, 1.0, 0.0]) * 0.5 + np.array([0.0, 0.0, 0.5])
+    m = np.zeros((3,) + nn)
+    m[:, :, :, :3] = ma.reshape(3, 1, 1, 1)
+    m[:, :, :, 3:] = mb.reshape(3, 1, 1, 1)
+    A = n[0] * dx[0] * n[1] * dx[1]
+    assert np.isclose(mt.energy_rkky(m, J, planes, dx), -J * A * (ma @ mb), rtol=1e-13)
+    dE = mt.variation_rkky(m, J, planes, dx)
+    assert np.allclose(dE[:, :, :, 2].sum(axis=(1, 2)), -J * A * mb, rtol=1e-13)
+    assert np.allclose(dE[:, :, :, 3].sum(axis=(1, 2)), -J * A * ma, rtol=1e-13)
+    assert np.all(dE[:, :, :, [0, 1, 4, 5]] == 0)
+    assert np.allclose(dE[:, 1, 1, 2], -J * dx[0] * dx[1] * mb) and np.allclose(dE[:, 0, 0, 2], -J * dx[0] * dx[1] * mb / 4)
+    # field on an interior interface node: H = J m_b / (mu0 Ms t), t = the half cell of magnetic material below it
+    p = Problem(n, tuple(dx), _two_layers(n), np.zeros(n), np.zeros(n), terms=TERM_RKKY, rkky_J=J, rkky_planes=planes)
+    H = effective_field(p, m)
+    assert np.allclose(H[:, 1, 1, 2], J * mb / (MU0 * 8e5 * dx[2] / 2), rtol=1e-12)
+
+
+def test_rkky_bilinear_identity_symmetry_and_brute_force():
+    """E = (1/2) sum m . dE; <u, dE(v)> = <v, dE(u)>; dE against central differences of the face integral
+    evaluated with 2-D hat functions and a 3-point Gauss rule per face."""
+    rng = np.random.default_rng(6)
+    n, dx = (3, 2, 4), np.array([1.0, 1.3, 0.7])
+    J, planes = 0.9, (1, 3)
+    nn = mesh.n_nodes(n)
+    m, u = rng.standard_normal((3,) + nn), rng.standard_normal((3,) + nn)
+    dE = mt.variation_rkky(m, J, planes, dx)
+    assert np.isclose(mt.energy_rkky(m, J, planes, dx), 0.5 * np.sum(m * dE), rtol=1e-12)
+    assert np.isclose(np.sum(u * dE), np.sum(m * mt.variation_rkky(u, J, planes, dx)), rtol=1e-12)
+    g, gw = _gauss(3)
+
+    def brute(mm):
+        E = 0.0
+        for f1 in range(n[0]):
+            for f2 in range(n[1]):
+                for (a, wa), (b, wb) in itertools.product(zip(g, gw), repeat=2):
+                    ph = np.outer([1 - a, a], [1 - b, b])
+                    va = np.einsum("jxy,xy->j", mm[:, f1:f1 + 2, f2:f2 + 2, planes[0]], ph)
+                    vb = np.einsum("jxy,xy->j", mm[:, f1:f1 + 2, f2:f2 + 2, planes[1]], ph)
+                    E += -J * wa * wb * dx[0] * dx[1] * (va @ vb)
+        return E
+    assert np.isclose(brute(m), mt.energy_rkky(m, J, planes, dx), rtol=1e-12)
+    ref = np.zeros_like(m)
+    for idx in itertools.product(range(3), range(nn[0]), range(nn[1]), planes):
+        mp, mm_ = m.copy(), m.copy()
+        mp[idx] += 1e-5
+        mm_[idx] -= 1e-5
+        ref[idx] = (brute(mp) - brute(mm_)) / 2e-5
+    assert np.allclose(dE, ref, rtol=1e-7, atol=1e-9)

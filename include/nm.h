@@ -58,7 +58,9 @@ enum { NM_TERM_EXCHANGE = 1, NM_TERM_DEMAG = 2, NM_TERM_ANISO = 4, NM_TERM_ZEEMA
        /* further local terms through the same weak form ("crystalline anisotropies, and both
           symmetric and antisymmetric exchange interactions", readings F3) */
        NM_TERM_DMI = 16,   /* antisymmetric exchange, density D sum T[a,d,b] m_a d_d m_b (nm_mesh_desc.dmi_kind) */
-       NM_TERM_CUBIC = 32  /* cubic anisotropy, density Kc (a1^2 a2^2 + a2^2 a3^2 + a3^2 a1^2), a_q = m . c_q */
+       NM_TERM_CUBIC = 32, /* cubic anisotropy, density Kc (a1^2 a2^2 + a2^2 a3^2 + a3^2 a1^2), a_q = m . c_q */
+       NM_TERM_RKKY = 64   /* interlayer coupling E = -J int m(x,y,z_a) . m(x,y,z_b) dGamma between two node planes
+                              (PAPER.md:79), through the 2-D face mass matrix; linear in m: every entry point */
 };
 typedef enum { NM_DMI_BULK = 0,        /* D m . curl m */
                NM_DMI_INTERFACIAL = 1  /* D [m_n div m - (m . grad) m_n], n = nm_mesh_desc.dmi_normal */
@@ -103,6 +105,8 @@ typedef struct {
     int dmi_kind;         /* nm_dmi_kind */
     int dmi_normal;       /* film normal axis (0, 1, 2) of NM_DMI_INTERFACIAL */
     double cubic_axes[9]; /* rows c_1, c_2, c_3: one global orthonormal frame */
+    double rkky_J;        /* J/m^2 (NM_TERM_RKKY); > 0 favours parallel layers */
+    int rkky_planes[2];   /* node-plane indices z_a != z_b along axis 3, 0 <= z <= N3 */
 } nm_mesh_desc;
 
 /* Bytes of device workspace nm_mesh_create needs for this description (spectrum buffers, demag

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libnm.so")
 NM_F32, NM_F64 = 0, 1
 NM_OK, NM_EINVAL, NM_EUNSUPPORTED, NM_ECUDA, NM_ENOMEM = 0, -1, -2, -3, -4
 NM_TERM_EXCHANGE, NM_TERM_DEMAG, NM_TERM_ANISO, NM_TERM_ZEEMAN = 1, 2, 4, 8
-NM_TERM_DMI, NM_TERM_CUBIC = 16, 32
+NM_TERM_DMI, NM_TERM_CUBIC, NM_TERM_RKKY = 16, 32, 64
 NM_DMI_BULK, NM_DMI_INTERFACIAL = 0, 1
 NM_RK4, NM_DOPRI5 = 0, 1
 
@@ -46,7 +46,8 @@ class nm_mesh_desc(ctypes.Structure):
                 ("D", ctypes.c_void_p), ("Kc", ctypes.c_void_p),
                 ("D_scalar", ctypes.c_double), ("Kc_scalar", ctypes.c_double),
                 ("dmi_kind", ctypes.c_int), ("dmi_normal", ctypes.c_int),
-                ("cubic_axes", ctypes.c_double * 9)]
+                ("cubic_axes", ctypes.c_double * 9),
+                ("rkky_J", ctypes.c_double), ("rkky_planes", ctypes.c_int * 2)]
 
 
 AMP_FUNC = ctypes.CFUNCTYPE(ctypes.c_double, ctypes.c_double, ctypes.c_void_p)
@@ -135,7 +136,7 @@ def _stream(device):
 
 def make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis=(0.0, 0.0, 1.0),
               Ms=None, A=None, Ku=None, basis=3, D=None, Kc=None, dmi_kind=NM_DMI_BULK, dmi_normal=2,
-              cubic_axes=(1.0, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0)):
+              cubic_axes=(1.0, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0), rkky_J=0.0, rkky_planes=(0, 0)):
     """Fill an nm_mesh_desc.  Ms/A/Ku/D/Kc: python scalar or a device tensor [N3][N2][N1]."""
     d = nm_mesh_desc()
     d.n_cells[:] = [int(v) for v in n_cells]
@@ -147,6 +148,8 @@ def make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis=(0
     d.ku_axis[:] = [float(v) for v in ku_axis]
     d.basis = int(basis)
     d.dmi_kind, d.dmi_normal = int(dmi_kind), int(dmi_normal)
+    d.rkky_J = float(rkky_J)
+    d.rkky_planes[:] = [int(v) for v in rkky_planes]
     d.cubic_axes[:] = [float(v) for row in cubic_axes for v in (row if hasattr(row, "__len__") else (row,))]
     keep = []
     for name, v in (("Ms", Ms), ("A", A), ("Ku", Ku), ("D", D), ("Kc", Kc)):
@@ -192,7 +195,7 @@ class Mesh:
     def __init__(self, n_cells, cell_size, dtype=torch.float32, device=0, terms=3, gamma=2.211e5,
                  alpha=0.0, ku_axis=(0.0, 0.0, 1.0), Ms=None, A=None, Ku=None, workspace=None, basis=3,
                  D=None, Kc=None, dmi_kind=NM_DMI_BULK, dmi_normal=2,
-                 cubic_axes=(1.0, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0)):
+                 cubic_axes=(1.0, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0), rkky_J=0.0, rkky_planes=(0, 0)):
         """workspace: optional caller-made uint8 device tensor (256-byte aligned start, at least
         nm_mesh_query_workspace bytes) to build the mesh in, instead of one allocated here."""
         self.dtype = dtype
@@ -203,7 +206,7 @@ class Mesh:
                                self.n_cells[1] + 1 if self.basis > 1 else 1, self.n_cells[0] + 1)
         self.cell_shape_abi = (self.n_cells[2], self.n_cells[1], self.n_cells[0])
         desc = make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis, Ms, A, Ku, basis,
-                         D, Kc, dmi_kind, dmi_normal, cubic_axes)
+                         D, Kc, dmi_kind, dmi_normal, cubic_axes, rkky_J, rkky_planes)
         nbytes = nm_mesh_query_workspace(desc)
         self.workspace_bytes = nbytes
         if workspace is None:

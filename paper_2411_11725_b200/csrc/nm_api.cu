@@ -85,11 +85,18 @@ nm_status validate(const nm_mesh_desc *d)
                      d->n_cells[0], d->n_cells[1], d->n_cells[2]);
         return NM_EINVAL;
     }
-    if (d->terms == 0 || (d->terms & ~63u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
-    if (d->terms & (NM_TERM_DMI | NM_TERM_CUBIC)) {
+    if (d->terms == 0 || (d->terms & ~127u)) { nm_set_error("terms = %u is not a combination of NM_TERM_*", d->terms); return NM_EINVAL; }
+    if (d->terms & (NM_TERM_DMI | NM_TERM_CUBIC | NM_TERM_RKKY)) {
         if (d->basis != 0 && d->basis != 3) {
-            nm_set_error("NM_TERM_DMI / NM_TERM_CUBIC are written for the 3-D basis (basis = %d)", d->basis);
+            nm_set_error("NM_TERM_DMI / NM_TERM_CUBIC / NM_TERM_RKKY are written for the 3-D basis (basis = %d)", d->basis);
             return NM_EUNSUPPORTED;
+        }
+        if (d->terms & NM_TERM_RKKY) {
+            const int za = d->rkky_planes[0], zb = d->rkky_planes[1];
+            if (za == zb || za < 0 || zb < 0 || za > d->n_cells[2] || zb > d->n_cells[2]) {
+                nm_set_error("rkky_planes = (%d, %d) must be two different node planes in [0, N3]", za, zb);
+                return NM_EINVAL;
+            }
         }
         if ((d->terms & NM_TERM_DMI) && (d->dmi_kind < 0 || d->dmi_kind > 1 || d->dmi_normal < 0 || d->dmi_normal > 2)) {
             nm_set_error("dmi_kind = %d / dmi_normal = %d out of range", d->dmi_kind, d->dmi_normal);
@@ -198,7 +205,7 @@ size_t carve(nm_mesh *m, char *base)
     m->Zs = (m->desc.terms & NM_TERM_ZEEMAN) ? c.take(vec) : nullptr;
     m->Dmi = (m->desc.terms & NM_TERM_DMI) ? c.take(g.cells * e) : nullptr;
     m->Kcub = (m->desc.terms & NM_TERM_CUBIC) ? c.take(g.cells * e) : nullptr;
-    m->Xs = (m->desc.terms & (NM_TERM_DMI | NM_TERM_CUBIC)) ? c.take(vec) : nullptr;
+    m->Xs = (m->desc.terms & (NM_TERM_DMI | NM_TERM_CUBIC | NM_TERM_RKKY)) ? c.take(vec) : nullptr;
     m->Hc1 = m->Hc2 = nullptr;
     m->Nreal = nullptr;
     m->fast.Tn = m->fast.wPx = nullptr;
@@ -634,6 +641,9 @@ template <typename T> nm_status extra_part(nm_mesh *m, const T *fld, const T **h
     x.dmi_kind = m->desc.dmi_kind;
     x.dmi_normal = m->desc.dmi_normal;
     for (int q = 0; q < 9; ++q) x.cax[q] = (T)m->desc.cubic_axes[q];
+    x.rkky_JA = (m->desc.terms & NM_TERM_RKKY) ? (T)(m->desc.rkky_J * dx[0] * dx[1]) : (T)0;
+    x.rkky_za = m->desc.rkky_planes[0];
+    x.rkky_zb = m->desc.rkky_planes[1];
     NM_TRY(nm_launch_extra<T>(m, x, st));
     *hadd_arg = (const T *)m->Xs;
     return NM_OK;

@@ -948,6 +948,26 @@ __global__ void __launch_bounds__(kBlock) k_extra_local(const NmExtraArgs<T> a)
                     }
         }
     }
+    // interlayer coupling: dE_{(f+i, z_a)} += -J dx dy sum_{i'} M1 M1 m_{(f+i', z_b)} over the (up to 4) faces f of the
+    // node in its plane, and the same with the planes exchanged
+    if (a.rkky_JA != (T)0 && (i3 == a.rkky_za || i3 == a.rkky_zb)) {
+        const int zo = i3 == a.rkky_za ? a.rkky_zb : a.rkky_za;
+        for (int fi = 0; fi < 4; ++fi) {
+            const int bx = fi & 1, by = fi >> 1;
+            const int f1 = i1 - 1 + bx, f2 = i2 - 1 + by;
+            if (f1 < 0 || f1 >= g.N1 || f2 < 0 || f2 >= g.N2) continue;
+            const int ix = 1 - bx, iy = 1 - by;                      // local vertex of the node in face f
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+                const int vx = v & 1, vy = v >> 1;
+                const T w = -a.rkky_JA * (vx == ix ? third : sixth) * (vy == iy ? third : sixth);
+                const long long q = (long long)zo * pl + (long long)(f2 + vy) * g.n1 + (f1 + vx);
+                dE[0] += w * a.fld[q];
+                dE[1] += w * a.fld[nn + q];
+                dE[2] += w * a.fld[2 * nn + q];
+            }
+        }
+    }
     const T sc = sms > 0 ? (T)-1 / (a.mu0V8 * sms) : (T)0;
 #pragma unroll
     for (int j = 0; j < 3; ++j) a.out[j * nn + n] = sc * dE[j];

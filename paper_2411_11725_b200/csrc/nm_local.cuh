@@ -84,6 +84,8 @@ template <typename T> struct NmExtraArgs {
     T idx[3];                       // 1 / dx_d
     int dmi_kind, dmi_normal;
     T cax[9];                       // cubic frame, rows c_1, c_2, c_3
+    T rkky_JA;                      // J dx dy (0: term off)
+    int rkky_za, rkky_zb;
 };
 template <typename T> nm_status nm_launch_extra(nm_mesh *mesh, const NmExtraArgs<T> &a, cudaStream_t st);
 

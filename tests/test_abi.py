@@ -39,7 +39,7 @@ def test_binding_struct_matches_header_layout(nm):
     assert [f[0] for f in nm.nm_mesh_desc._fields_] == [
         "n_cells", "cell_size", "dtype", "device", "terms", "gamma", "alpha", "ku_axis", "Ms", "A",
         "Ku", "Ms_scalar", "A_scalar", "Ku_scalar", "basis", "D", "Kc", "D_scalar", "Kc_scalar", "dmi_kind",
-        "dmi_normal", "cubic_axes"]
+        "dmi_normal", "cubic_axes", "rkky_J", "rkky_planes"]
     assert [f[0] for f in nm.nm_zeeman._fields_] == ["h_static", "h_pulse", "h_uniform", "amp", "user"]
 
 
@@ -55,7 +55,7 @@ def test_query_workspace_validates(nm):
     assert nm.nm_mesh_query_workspace(_desc(nm, dtype_f64=True)) > nm.nm_mesh_query_workspace(_desc(nm))
     assert nm.nm_mesh_query_workspace(_desc(nm, terms=3)) > nm.nm_mesh_query_workspace(_desc(nm, terms=1))
     for bad, status in ((dict(n=(0, 8, 8)), nm.NM_EINVAL), (dict(terms=0), nm.NM_EINVAL),
-                        (dict(terms=64), nm.NM_EINVAL), (dict(dx=(1e-9, 0.0, 1e-9)), nm.NM_EINVAL),
+                        (dict(terms=128), nm.NM_EINVAL), (dict(dx=(1e-9, 0.0, 1e-9)), nm.NM_EINVAL),
                         (dict(n=(11, 8, 8)), nm.NM_EUNSUPPORTED), (dict(n=(8, 13, 8), terms=2), nm.NM_EUNSUPPORTED)):
         with pytest.raises(nm.NmError) as e:
             nm.nm_mesh_query_workspace(_desc(nm, **bad))

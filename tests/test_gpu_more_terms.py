@@ -19,7 +19,7 @@ ND = {"f64": np.float64, "f32": np.float32}
 AXES = np.linalg.qr(np.random.default_rng(77).standard_normal((3, 3)))[0]      # a rotated cubic frame
 
 
-def _case(n, prec, terms, kind="bulk", normal=2, uniform=False, vacuum=True, seed=0):
+def _case(n, prec, terms, kind="bulk", normal=2, uniform=False, vacuum=True, seed=0, rkky=None):
     """Seeded inputs (rounded to the build precision), the oracle Problem and the GPU mesh."""
     from oracle import llg
     nd, td = ND[prec], TD[prec]
@@ -29,7 +29,7 @@ def _case(n, prec, terms, kind="bulk", normal=2, uniform=False, vacuum=True, see
     r = lambda a: wl.round_to(a, nd)
     if uniform:
         Ms, A, Ku, D, Kc = 8e5, 1.3e-11, 4e4, 2.5e-3, 3e4
-        cells = lambda v: np.full(n, float(np.float64(nd(v))))
+        cells = lambda v: np.full(n, float(np.float64(nd(v)))) if np.isscalar(v) else v
     else:
         Ms = r(rng.uniform(2e5, 8e5, n))
         if vacuum and n[0] >= 4:
@@ -37,16 +37,20 @@ def _case(n, prec, terms, kind="bulk", normal=2, uniform=False, vacuum=True, see
         A, Ku = r(rng.uniform(0.5e-11, 2e-11, n)), r(rng.uniform(1e4, 5e4, n))
         D, Kc = r(rng.uniform(1e-3, 3e-3, n)), r(rng.uniform(1e4, 5e4, n))
         cells = lambda v: v
+    rk_J, rk_planes = rkky if rkky else (0.0, (0, 0))
+    if rkky and n[2] > 1:                         # vacuum spacer: the cell layers between the coupled node planes
+        Ms = cells(Ms).copy()
+        Ms[:, :, rk_planes[0]:rk_planes[1]] = 0.0
     m = wl.box_filter3(wl.random_unit_field(tuple(k + 1 for k in n), 50 + seed))
     m = r(m / np.sqrt((m ** 2).sum(axis=0)))
     axes = AXES                                   # fp64 on both sides (the library casts it to the build precision)
     kax = np.array([1.0, 2.0, 2.0]) / 3.0
     p = llg.Problem(n, dx, cells(Ms), cells(A), cells(Ku), tuple(kax), 2.211e5, 0.05, terms, D=cells(D), dmi_kind=kind,
-                    dmi_normal=normal, Kc=cells(Kc), cubic_axes=axes)
+                    dmi_normal=normal, Kc=cells(Kc), cubic_axes=axes, rkky_J=rk_J, rkky_planes=rk_planes)
     g = lambda v: float(np.float64(nd(v))) if np.isscalar(v) else dev(v, td)
     mesh = nm.Mesh(n, dx, dtype=td, terms=terms, gamma=2.211e5, alpha=0.05, ku_axis=kax, Ms=g(Ms), A=g(A), Ku=g(Ku),
                    D=g(D), Kc=g(Kc), dmi_kind=nm.NM_DMI_BULK if kind == "bulk" else nm.NM_DMI_INTERFACIAL,
-                   dmi_normal=normal, cubic_axes=axes)
+                   dmi_normal=normal, cubic_axes=axes, rkky_J=rk_J, rkky_planes=rk_planes)
     return p, mesh, m
 
 
@@ -166,3 +170,27 @@ def test_adjoint_and_reduced_basis_say_unsupported():
     with pytest.raises(nm.NmError) as e:
         nm.Mesh((4, 4, 4), (2e-9,) * 3, dtype=torch.float64, terms=32, Ms=8e5, Kc=1e4, cubic_axes=(1, 0, 0, 0, 1, 0, 0, 1, 0))
     assert e.value.status == nm.NM_EINVAL
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n,planes,uniform", [((9, 6, 5), (2, 3), False), ((128, 6, 5), (1, 4), True), ((5, 4, 1), (0, 1), False)])
+def test_rkky_interlayer_coupling(n, planes, uniform, prec):
+    """NM_TERM_RKKY against oracle variation_rkky: two layers across a vacuum spacer (the cell layers
+    between the coupled node planes have Ms = 0; the one-layer film couples its two faces), alone and with
+    exchange + demag + DMI, then the adjoint right-hand side (the term is linear in m: it rides in H and in
+    Hlin^T b)."""
+    from oracle import adjoint, llg
+    J = -1.2e-3                                           # antiferromagnetic coupling
+    for terms in (64, 1 | 2 | 16 | 64):
+        p, mesh, m = _case(n, prec, terms, "bulk", uniform=uniform, vacuum=False, seed=13, rkky=(J, planes))
+        H = host(mesh.nm_heff(0.0, dev(m, TD[prec])))
+        ref = llg.effective_field(p, m)
+        assert_parity(H, ref, TOL[prec], "H with RKKY, terms %d" % terms)
+        if terms == 64:
+            other = [k for k in range(n[2] + 1) if k not in planes]
+            assert np.all(H[:, :, :, other] == 0) and np.abs(H).max() > 0
+    a = wl.round_to(np.random.default_rng(14).standard_normal(m.shape), ND[prec])
+    f_ref, da_ref, du_ref = adjoint.adjoint_rhs(p, 0.0, m, a)
+    f, da, du = mesh.nm_llg_adjoint_rhs(0.0, dev(m, TD[prec]), dev(a, TD[prec]))
+    assert_parity(host(da), da_ref, TOL[prec], "da/dt with RKKY")
+    assert rel_l2(wl.from_abi(du.cpu().double().numpy()), du_ref) <= TOL[prec]

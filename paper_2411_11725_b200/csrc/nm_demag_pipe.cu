@@ -1022,7 +1022,7 @@ k_px_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, T ms_uni, typename
 template <typename T, int M, bool EMB>
 __global__ void __launch_bounds__(kPipeThreads, sizeof(T) == 8 ? 1 : 2)
 k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, const typename VT<T>::V *__restrict__ wP,
-         int f2)
+         int f2, int persist)
 {
     typedef typename VT<T>::V V;
     typedef PxGeom<T, M> G;
@@ -1035,24 +1035,30 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     const int h = lane & 1, i = lane >> 1;
     const int l = i / M, j = i % M;
     const int line = w * LT + l;
-    const int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    // persist: a CTA walks the tiles blockIdx.x, blockIdx.x + gridDim.x, ... (tile = row block + nbx * plane) and
+    // stages the first component of its next tile while the last one of this tile is transformed
+    int r0 = blockIdx.x * R, c3 = blockIdx.y;
+    const int nbx = g.N2 / R, ntiles = persist ? nbx * g.N3 : 1;
+    if (persist) { r0 = ((int)blockIdx.x % nbx) * R; c3 = (int)blockIdx.x / nbx; }
     V *scr = s_scr + (2 * w + h) * G::SCR;
     V tw[16];
     load_twiddles_h<T, M>(tw, wP, j, h);
     constexpr int PIECES = R * TW * (int)sizeof(V) / 16;    // 16-byte pieces per block
-    auto stage = [&](int comp) {
+    auto stage = [&](int comp, int rr0, int cc3) {
         for (int e = tid; e < NKT * PIECES; e += kPipeThreads) {
             const int kt = e / PIECES, off = e - kt * PIECES;
-            const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + c3) * f2 + r0) * TW) + off * 16;
+            const char *src = reinterpret_cast<const char *>(A + ((((long long)kt * 3 + comp) * g.N3 + cc3) * f2 + rr0) * TW) + off * 16;
             const unsigned dst = smem_u32(reinterpret_cast<char *>(s_raw + kt * G::KP) + off * 16);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     const int comp_lo = gridDim.z == 3 ? blockIdx.z : 0, comp_hi = gridDim.z == 3 ? comp_lo + 1 : 3;
-    stage(comp_lo);
+    stage(comp_lo, r0, c3);
     // Xa, Xb of this thread's line: rows 2 line, 2 line + 1 of every block, column k1 at slot k1 ^ swz(c2)
     const V *ra = s_raw + (2 * line) * TW;
+    for (int tile = persist ? (int)blockIdx.x : 0; tile < ntiles; tile += persist ? (int)gridDim.x : 1) {
+    if (persist) { r0 = (tile % nbx) * R; c3 = tile / nbx; }
     const int sw = swzT<T>(r0 + 2 * line);
     for (int comp = comp_lo; comp < comp_hi; ++comp) {
         asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -1071,7 +1077,8 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             a[s] = mk<T>(u.x - sg * v.y, v.x + sg * u.y);
         }
         __syncthreads();                                    // the staging buffer is free
-        if (comp + 1 < comp_hi) stage(comp + 1);
+        if (comp + 1 < comp_hi) stage(comp + 1, r0, c3);
+        else if (persist && tile + (int)gridDim.x < ntiles) stage(comp_lo, ((tile + (int)gridDim.x) % nbx) * R, (tile + (int)gridDim.x) / nbx);
         fft_inv<T, M, true>(a, tw, scr, i);
         if (h) shift32<T, true>(a);
         if (M >= 8) {
@@ -1115,6 +1122,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
                 }
             }
         }
+    }
     }
 }
 
@@ -1545,9 +1553,13 @@ template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, co
         else NM_TRY(mesh->uni_Ms ? go(k_px_fwd<T, M, true, false, false>, ms) : go(k_px_fwd<T, M, false, false, false>, (T)0));
     } else {
         NmLaunchScope sc(mesh, NM_K_X_INV, st);
+        const int per_sm = sizeof(T) == 8 ? 1 : 2;
+        const bool persist = !split && (int)(grid.x * grid.y) > per_sm * mesh->sm_count && mesh->dbg_node_path != 3;
+        const dim3 pgrid = persist ? dim3(per_sm * mesh->sm_count, 1, 1) : grid;
         auto go = [&](auto kern) -> nm_status {
             NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::INV_BYTES));
-            kern<<<grid, kPipeThreads, G::INV_BYTES, st>>>((const V *)mesh->bufA, Hc, g, (const V *)mesh->fast.wPx, f2);
+            kern<<<pgrid, kPipeThreads, G::INV_BYTES, st>>>((const V *)mesh->bufA, Hc, g, (const V *)mesh->fast.wPx, f2,
+                                                            persist ? 1 : 0);
             return NM_OK;
         };
         NM_TRY(mesh->fast.embed ? go(k_px_inv<T, M, true>) : go(k_px_inv<T, M, false>));

@@ -103,6 +103,7 @@ def write_traffic(rep, N, dtype):
     """Parse `ncu -i rep --page raw --csv` and write profiles/traffic.json."""
     import csv
     import io
+    import re
     out = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True).stdout
     rows = list(csv.reader(io.StringIO(out)))
     idx = {h: i for i, h in enumerate(rows[0])}
@@ -111,11 +112,13 @@ def write_traffic(rep, N, dtype):
     acc = {}
     for r in rows[2:]:
         name = r[idx["Kernel Name"]]
-        cls = next((c for k, c in KERNEL_CLASS if name.startswith(k)), None)
+        mk = re.search(r"\bk_[a-z0-9_]+.*", name)          # "void <unnamed>::k_pz_mid<0>(float2 *, ...)" -> "k_pz_mid<0>(..."
+        base = mk.group(0) if mk else name
+        cls = next((c for k, c in KERNEL_CLASS if base.startswith(k)), None)
         if cls is None:
             continue
         if cls == "node":
-            cls = node_class(name)
+            cls = node_class(base)
         b = 0.0
         for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
             b += float(r[idx[col]].replace(",", "")) * scale[units[idx[col]]]

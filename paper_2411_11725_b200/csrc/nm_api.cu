@@ -190,14 +190,17 @@ size_t carve(nm_mesh *m, char *base)
     m->hpart = (double *)c.take((size_t)3 * NM_HEXT_BLOCKS * sizeof(double));
     // Runge-Kutta / adjoint scratch; doubles as fp64 scratch of the tensor setup
     const size_t vec = (size_t)3 * g.nodes * e;
-    size_t rk = 9 * vec;
+    // every stage array starts on a 256-byte boundary (3 nodes e is odd-sized): the bulk-copy feeds of the x pass
+    // and of the node kernel need 16-byte aligned nodal arrays, and a stage state is the field of the next stage
+    const size_t vecp = (vec + 255) & ~(size_t)255;
+    size_t rk = 9 * vecp;
     if (demag) {
         const size_t need = (size_t)2 * 6 * g.C1 * g.K2 * g.K3 * sizeof(double);
         if (need > rk) rk = need;
     }
     char *r = (char *)c.take(rk);
-    for (int i = 0; i < 7; ++i) m->K[i] = r ? r + i * vec : nullptr;
-    for (int i = 0; i < 2; ++i) m->Y[i] = r ? r + (7 + i) * vec : nullptr;
+    for (int i = 0; i < 7; ++i) m->K[i] = r ? r + i * vecp : nullptr;
+    for (int i = 0; i < 2; ++i) m->Y[i] = r ? r + (7 + i) * vecp : nullptr;
     m->Q = c.take(vec);
     m->W = c.take(g.nodes * e);
     m->Uc[0] = c.take(g.cells * e);

@@ -1,7 +1,7 @@
-"""GPU parity of the further local terms (NM_TERM_DMI, NM_TERM_CUBIC)
-against oracle/more_terms.py through the C-ABI: term by term, together with every other term on ragged
-grids with cell-wise materials and a vacuum block, on each node path (column-marching, separable,
-27-point), and over Runge-Kutta steps.  Wall time: ~6 s."""
+"""GPU parity of the further local terms (NM_TERM_DMI, NM_TERM_CUBIC, NM_TERM_RKKY, SURVEY.md
+8(f) row 3) against oracle/more_terms.py through the C-ABI: term by term, together with every other term on
+ragged grids with cell-wise materials and a vacuum block, on each node path (column-marching, separable,
+27-point), over Runge-Kutta steps, and (DMI, RKKY) in the adjoint right-hand side.  Wall time: ~8 s."""
 import numpy as np
 import pytest
 import torch

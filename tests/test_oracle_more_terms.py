@@ -1,4 +1,5 @@
-"""Pins of oracle/more_terms.py (DMI and cubic anisotropy through the weak form):
+"""Pins of oracle/more_terms.py (DMI, cubic anisotropy and RKKY interlayer coupling through the weak form,
+PAPER.md:79, 171):
 quadrature of Eq. 12's products, closed forms, invariants, and a brute-force global assembly that
 shares nothing with the element loop (global hat functions, energy by 4-point Gauss quadrature,
 gradient by central differences of that energy)."""

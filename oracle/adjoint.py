@@ -29,6 +29,7 @@ import numpy as np
 from . import demag as _demag
 from . import llg as _llg
 from . import local_fields as _lf
+from . import more_terms as _mt
 from .mesh import (LOCAL, MU0, element_matrices, gather_nodes_to_cells, node_view,
                    scatter_cells_to_nodes)
 
@@ -64,12 +65,12 @@ def adjoint_rhs(p, t, m, a, zeeman=None, pieces=None):
     d = -gp * cross(H, a) - al * gp * (dot(m, H) * a + dot(a, m) * H - 2.0 * dot(a, H) * m)
 
     # Hlin^T b = L o Hlin(b / L): the same field operators, without the Zeeman term
-    # (exchange, anisotropy, demag and DMI are linear in m with an L-symmetric operator; the cubic
-    # anisotropy is not linear: its transposed Jacobian is not written here)
-    if p.terms & _llg.TERM_CUBIC:
-        raise NotImplementedError("adjoint_rhs does not differentiate the cubic anisotropy")
-    p_lin = dataclasses.replace(p, terms=p.terms & ~_llg.TERM_ZEEMAN)
+    # (exchange, anisotropy, demag, DMI and RKKY are linear in m with an L-symmetric operator; the cubic
+    # anisotropy is not: H_cub = -L^-1 g(m), so (dH_cub/dm)^T b = -Hess E_cub(m) (b / L), the Hessian being symmetric)
+    p_lin = dataclasses.replace(p, terms=p.terms & ~(_llg.TERM_ZEEMAN | _llg.TERM_CUBIC))
     HTb = L * _llg.effective_field(p_lin, _safe_div(b, L), None)
+    if p.terms & _llg.TERM_CUBIC:
+        HTb = HTb - _mt.hessvec_cubic(m, _safe_div(b, L), p.Kc, p.cubic_axes, p.dx)
     dadt = -(d + HTb)
 
     # -(df/dMs)^T a

@@ -143,6 +143,33 @@ def variation_cubic(m, Kc, axes, dx):
     return dE
 
 
+def hessvec_cubic(m, v, Kc, axes, dx):
+    """(d^2 E / dm^2)(m) v for the cubic anisotropy energy: the derivative of variation_cubic at m in the nodal
+    direction v (used by the adjoint: (dH/dm)^T b = -Hess (b / L), the Hessian being symmetric).  In the frame,
+    d^2 e / da_q da_r = 2 (|a|^2 - a_q^2) delta_qr + 4 a_q a_r (1 - delta_qr)."""
+    c = np.asarray(axes, dtype=np.float64)
+    V = float(dx[0]) * float(dx[1]) * float(dx[2])
+    out = np.zeros_like(m, dtype=np.float64)
+    for q1 in range(3):
+        for q2 in range(3):
+            for q3 in range(3):
+                x = np.array([_GX[q1], _GX[q2], _GX[q3]])
+                w = V * _GW[q1] * _GW[q2] * _GW[q3]
+                mq, vq = _interpolate(m, x), _interpolate(v, x)
+                al = [c[q, 0] * mq[0] + c[q, 1] * mq[1] + c[q, 2] * mq[2] for q in range(3)]
+                be = [c[q, 0] * vq[0] + c[q, 1] * vq[1] + c[q, 2] * vq[2] for q in range(3)]
+                S = al[0] ** 2 + al[1] ** 2 + al[2] ** 2
+                ab = al[0] * be[0] + al[1] * be[1] + al[2] * be[2]
+                h = np.zeros_like(mq)
+                for q in range(3):
+                    hq = 2.0 * (S - al[q] ** 2) * be[q] + 4.0 * al[q] * (ab - al[q] * be[q])
+                    for j in range(3):
+                        h[j] = h[j] + hq * c[q, j]
+                for i in LOCAL:
+                    node_view(out, i)[...] += Kc * w * phi_ref(i, x) * h
+    return out
+
+
 def energy_cubic(m, Kc, axes, dx):
     V = float(dx[0]) * float(dx[1]) * float(dx[2])
     E = 0.0
@@ -187,5 +214,5 @@ def energy_rkky(m, J, planes, dx):
     return float(E)
 
 
-__all__ = ["variation_rkky", "energy_rkky", "dmi_tensor", "gradient_matrices", "variation_dmi", "energy_dmi", "variation_cubic", "energy_cubic",
+__all__ = ["variation_rkky", "energy_rkky", "hessvec_cubic", "dmi_tensor", "gradient_matrices", "variation_dmi", "energy_dmi", "variation_cubic", "energy_cubic",
            "grad_phi_ref"]

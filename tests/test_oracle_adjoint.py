@@ -26,6 +26,8 @@ def make(n=(3, 2, 2), alpha=0.1, terms=ALL, seed=0):
                                 dmi_normal=1)
     if terms & TERM_RKKY:
         p = dataclasses.replace(p, rkky_J=2e-3, rkky_planes=(0, n[2]))
+    if terms & TERM_CUBIC:
+        p = dataclasses.replace(p, Kc=rng.uniform(1e4, 5e4, n), cubic_axes=np.linalg.qr(rng.standard_normal((3, 3)))[0])
     return p, (lambda t: hext)
 
 
@@ -34,7 +36,7 @@ def with_Ms(p, Ms):
 
 
 @pytest.mark.parametrize("terms", [ALL, TERM_EXCHANGE | TERM_DEMAG, TERM_DEMAG, TERM_EXCHANGE | TERM_ANISO | TERM_ZEEMAN,
-                                   ALL | TERM_DMI, TERM_EXCHANGE | TERM_DMI, TERM_DMI, ALL | TERM_RKKY, TERM_RKKY | TERM_DMI])
+                                   ALL | TERM_DMI, TERM_EXCHANGE | TERM_DMI, TERM_DMI, ALL | TERM_RKKY, TERM_RKKY | TERM_DMI, ALL | TERM_CUBIC, TERM_CUBIC])
 def test_dense_jacobians_by_finite_differences(terms):
     """Explicit dense Jacobians of the oracle's own forward RHS by central differences on a
     3x2x2-cell mesh; both vector-Jacobian products must equal a^T J."""
@@ -388,9 +390,17 @@ def test_hnodal_gradient_of_a_trajectory_against_finite_differences():
         assert abs(uhn[idx] - fd) <= 1e-3 * scale, (idx, uhn[idx], fd)
 
 
-def test_cubic_anisotropy_is_refused_by_the_adjoint():
-    p, zee = make()
-    p = dataclasses.replace(p, terms=p.terms | TERM_CUBIC, Kc=np.full(p.n_cells, 1e4))
-    m = rand_unit(p.node_shape, 2)
-    with pytest.raises(NotImplementedError):
-        adjoint.adjoint_rhs(p, 0.0, m, m.copy(), zee)
+def test_cubic_hessian_vector_product_is_the_derivative_of_the_variation():
+    """hessvec_cubic(m, v) against a central difference of variation_cubic along v; symmetric: u . H v = v . H u."""
+    from oracle import more_terms as mt
+    rng = np.random.default_rng(4)
+    n, dx = (3, 2, 2), np.array([1.0, 1.2, 0.8])
+    Kc = rng.uniform(0.5, 2.0, n)
+    axes = np.linalg.qr(rng.standard_normal((3, 3)))[0]
+    nn = tuple(k + 1 for k in n)
+    m, v, u = (rng.standard_normal((3,) + nn) for _ in range(3))
+    hv = mt.hessvec_cubic(m, v, Kc, axes, dx)
+    eps = 1e-6
+    fd = (mt.variation_cubic(m + eps * v, Kc, axes, dx) - mt.variation_cubic(m - eps * v, Kc, axes, dx)) / (2 * eps)
+    assert np.allclose(hv, fd, rtol=1e-8, atol=1e-9 * np.abs(fd).max())
+    assert np.isclose(np.sum(u * hv), np.sum(v * mt.hessvec_cubic(m, u, Kc, axes, dx)), rtol=1e-12)

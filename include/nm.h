@@ -94,9 +94,9 @@ typedef struct {
                              without derivatives along the reduced axes, lumped mass V / 2^D per cell,
                              node <-> cell averaging over the 2^D vertices of a cell).  Forward path only:
                              the adjoint entry points return NM_EUNSUPPORTED on a reduced basis. */
-    /* NM_TERM_DMI / NM_TERM_CUBIC (3-D basis).  The DMI term is linear in m like the exchange term and is
-       carried by every entry point (the adjoint ones give d/dm and d/dMs, not d/dD); with the cubic term on
-       the adjoint entry points return NM_EUNSUPPORTED (forward path only: nm_heff, nm_llg_rhs, nm_rk_step).  The element contributions are
+    /* NM_TERM_DMI / NM_TERM_CUBIC (3-D basis).  Both are carried by every entry point (the adjoint ones give
+       d/dm and d/dMs, not d/dD or d/dKc): the DMI term is linear in m like the exchange term; for the cubic
+       term the adjoint right-hand side applies the Hessian of its energy at m.  The element contributions are
        integrated exactly (DMI: bilinear in the Q1 functions; cubic: 3-point Gauss per axis), summed into
        the nodes and divided by the lumped mass, Eqs. (17)-(22). */
     const void *D, *Kc;   /* device, cell-wise [N3][N2][N1], copied at create; NULL => scalar below */

@@ -70,7 +70,8 @@ def adjoint_rhs(p, t, m, a, zeeman=None, pieces=None):
     p_lin = dataclasses.replace(p, terms=p.terms & ~(_llg.TERM_ZEEMAN | _llg.TERM_CUBIC))
     HTb = L * _llg.effective_field(p_lin, _safe_div(b, L), None)
     if p.terms & _llg.TERM_CUBIC:
-        HTb = HTb - _mt.hessvec_cubic(m, _safe_div(b, L), p.Kc, p.cubic_axes, p.dx)
+        # (0 at nodes with L = 0, like L o Hlin(b / L) above: reading C7 carries no adjoint at vacuum nodes)
+        HTb = HTb - np.where(L > 0, _mt.hessvec_cubic(m, _safe_div(b, L), p.Kc, p.cubic_axes, p.dx), 0.0)
     dadt = -(d + HTb)
 
     # -(df/dMs)^T a

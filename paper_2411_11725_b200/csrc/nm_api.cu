@@ -623,15 +623,18 @@ nm_status demag_part(nm_mesh *m, const T *fld, T *Hc, const T **Hc_arg, cudaStre
     return NM_OK;
 }
 
-// Field of the further local terms (NM_TERM_DMI, NM_TERM_CUBIC) of `fld` into the mesh's Xs array, which the
-// node kernel then adds to H.
-template <typename T> nm_status extra_part(nm_mesh *m, const T *fld, const T **hadd_arg, cudaStream_t st)
+// Field of the further local terms (NM_TERM_DMI, NM_TERM_CUBIC, NM_TERM_RKKY) of `fld` into the mesh's Xs array,
+// which the node kernel then adds to H.  about != null (adjoint pass 2): the cubic term's derivative at `about`
+// applied to fld; the other terms are linear and act on fld as they are.
+template <typename T>
+nm_status extra_part(nm_mesh *m, const T *fld, const T **hadd_arg, cudaStream_t st, const T *about = nullptr)
 {
     if (!m->Xs) return NM_OK;
     NmExtraArgs<T> x;
     memset(&x, 0, sizeof(x));
     x.g = m->g;
     x.fld = fld;
+    x.about = about;
     x.Ms = (const T *)m->Ms;
     x.D = (const T *)m->Dmi;
     x.Kc = (const T *)m->Kcub;
@@ -767,7 +770,7 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
     NmLocalArgs<T> a;
     base_args<T>(m, t, z, m->desc.terms, &a);
     a.fld = mm;
-    NM_TRY(extra_part<T>(m, mm, &a.hadd, st));          // DMI: linear in m, part of H and of Hlin (cubic: refused)
+    NM_TRY(extra_part<T>(m, mm, &a.hadd, st));
     NM_TRY(demag_part<T>(m, mm, (T *)m->Hc1, &a.Hc, st));
     m->hc1_valid = a.Hc != nullptr;
     a.mode = NM_MODE_ADJ1;
@@ -781,7 +784,7 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
     NmLocalArgs<T> b;
     base_args<T>(m, t, nullptr, m->desc.terms & ~(unsigned)NM_TERM_ZEEMAN, &b);
     b.fld = (const T *)m->Q;
-    NM_TRY(extra_part<T>(m, (const T *)m->Q, &b.hadd, st));
+    NM_TRY(extra_part<T>(m, (const T *)m->Q, &b.hadd, st, mm));   // cubic: -Hess E(m) q / L, the rest linear in q
     NM_TRY(demag_part<T>(m, (const T *)m->Q, (T *)m->Hc2, &b.Hc, st));
     b.mode = NM_MODE_ADJ2;
     b.dadt = dadt;
@@ -961,10 +964,6 @@ nm_status check_adjoint(const nm_mesh *mesh)
 {
     if (mesh && mesh->g.zs == 0) {
         nm_set_error("the adjoint entry points serve the full 3-D basis only (basis = %d)", mesh->desc.basis);
-        return NM_EUNSUPPORTED;
-    }
-    if (mesh && (mesh->desc.terms & NM_TERM_CUBIC)) {
-        nm_set_error("the adjoint entry points do not differentiate NM_TERM_CUBIC (not linear in m)");
         return NM_EUNSUPPORTED;
     }
     return NM_OK;

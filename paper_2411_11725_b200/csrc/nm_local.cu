@@ -848,6 +848,7 @@ inline dim3 sep_grid(const NmGeom &g, int *zchunk)
 //           T antisymmetric in (a, b): the Levi-Civita symbol (bulk) or T[n,d,d] = 1, T[d,d,n] = -1 (interfacial)
 //   cubic   dE_{n,j} += Kc_c V sum_q w_q phi_i(x_q) de/dm_j(m^h(x_q)),  3-point Gauss rule per axis (exact),
 //           e = a1^2 a2^2 + a2^2 a3^2 + a3^2 a1^2,  a_r = m . c_r,  de/dm = sum_r 2 a_r (|a|^2 - a_r^2) c_r
+//           (adjoint pass 2: the Hessian of that energy at m applied to q instead, which is what (dH_cub/dm)^T b is)
 // out_n = -dE_n / L_n, L_n = mu0 (V/8) (S Ms)_n (Eq. 22); 0 where (S Ms)_n = 0.
 template <typename T>
 __global__ void __launch_bounds__(kBlock) k_extra_local(const NmExtraArgs<T> a)
@@ -918,32 +919,67 @@ __global__ void __launch_bounds__(kBlock) k_extra_local(const NmExtraArgs<T> a)
         }
         if (a.Kc) {
             const T KV = a.Kc[c] * a.V;
+            // a.about != null: the Hessian of the energy at `about` applied to fld (adjoint pass 2) instead of the
+            // gradient at fld:  d2e/da_r da_s = 2 (|a|^2 - a_r^2) delta_rs + 4 a_r a_s (1 - delta_rs)
+            T av[8][3];
+            if (a.about) {
+#pragma unroll
+                for (int v = 0; v < 8; ++v) {
+                    const long long q = n0 + (v & 1) + ((v >> 1) & 1) * g.n1 + (long long)(v >> 2) * pl;
+                    av[v][0] = a.about[q];
+                    av[v][1] = a.about[nn + q];
+                    av[v][2] = a.about[2 * nn + q];
+                }
+            }
             for (int qz = 0; qz < 3; ++qz)
                 for (int qy = 0; qy < 3; ++qy)
 #pragma unroll
                     for (int qx = 0; qx < 3; ++qx) {
                         const T fx[2] = {(T)1 - gx[qx], gx[qx]}, fy[2] = {(T)1 - gx[qy], gx[qy]}, fz[2] = {(T)1 - gx[qz], gx[qz]};
-                        T mq[3] = {0, 0, 0};
+                        T mq[3] = {0, 0, 0}, aq[3] = {0, 0, 0};
 #pragma unroll
                         for (int v = 0; v < 8; ++v) {
                             const T ph = fx[v & 1] * fy[(v >> 1) & 1] * fz[v >> 2];
                             mq[0] += ph * mv[v][0];
                             mq[1] += ph * mv[v][1];
                             mq[2] += ph * mv[v][2];
-                        }
-                        T al[3], S = 0;
-#pragma unroll
-                        for (int r = 0; r < 3; ++r) {
-                            al[r] = a.cax[3 * r] * mq[0] + a.cax[3 * r + 1] * mq[1] + a.cax[3 * r + 2] * mq[2];
-                            S += al[r] * al[r];
+                            if (a.about) {
+                                aq[0] += ph * av[v][0];
+                                aq[1] += ph * av[v][1];
+                                aq[2] += ph * av[v][2];
+                            }
                         }
                         const T wq = KV * gw[qx] * gw[qy] * gw[qz] * fx[iv[0]] * fy[iv[1]] * fz[iv[2]];
+                        if (!a.about) {
+                            T al[3], S = 0;
 #pragma unroll
-                        for (int r = 0; r < 3; ++r) {
-                            const T cr = (T)2 * al[r] * (S - al[r] * al[r]) * wq;
-                            dE[0] += cr * a.cax[3 * r];
-                            dE[1] += cr * a.cax[3 * r + 1];
-                            dE[2] += cr * a.cax[3 * r + 2];
+                            for (int r = 0; r < 3; ++r) {
+                                al[r] = a.cax[3 * r] * mq[0] + a.cax[3 * r + 1] * mq[1] + a.cax[3 * r + 2] * mq[2];
+                                S += al[r] * al[r];
+                            }
+#pragma unroll
+                            for (int r = 0; r < 3; ++r) {
+                                const T cr = (T)2 * al[r] * (S - al[r] * al[r]) * wq;
+                                dE[0] += cr * a.cax[3 * r];
+                                dE[1] += cr * a.cax[3 * r + 1];
+                                dE[2] += cr * a.cax[3 * r + 2];
+                            }
+                        } else {
+                            T al[3], be[3], S = 0, ab = 0;
+#pragma unroll
+                            for (int r = 0; r < 3; ++r) {
+                                al[r] = a.cax[3 * r] * aq[0] + a.cax[3 * r + 1] * aq[1] + a.cax[3 * r + 2] * aq[2];
+                                be[r] = a.cax[3 * r] * mq[0] + a.cax[3 * r + 1] * mq[1] + a.cax[3 * r + 2] * mq[2];
+                                S += al[r] * al[r];
+                                ab += al[r] * be[r];
+                            }
+#pragma unroll
+                            for (int r = 0; r < 3; ++r) {
+                                const T cr = ((T)2 * (S - al[r] * al[r]) * be[r] + (T)4 * al[r] * (ab - al[r] * be[r])) * wq;
+                                dE[0] += cr * a.cax[3 * r];
+                                dE[1] += cr * a.cax[3 * r + 1];
+                                dE[2] += cr * a.cax[3 * r + 2];
+                            }
                         }
                     }
         }

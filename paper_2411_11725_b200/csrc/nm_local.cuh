@@ -79,6 +79,7 @@ template <typename T> struct NmAdjCellArgs {
 template <typename T> struct NmExtraArgs {
     NmGeom g;
     const T *fld, *Ms, *D, *Kc;     // nodal m; cell-wise Ms, D, Kc (D / Kc null when the term is off)
+    const T *about;                 // null: cubic term = its field at fld; else its linearisation about this nodal m, applied to fld
     T *out;                         // nodal vector: -(dE_dmi + dE_cubic) / L, 0 where (S Ms)_n = 0
     T mu0V8, V;
     T idx[3];                       // 1 / dx_d

@@ -158,9 +158,37 @@ def test_adjoint_rhs_and_backward_step_with_dmi(n, kind, uniform, prec):
     assert rel_l2(wl.from_abi(uu.cpu().double().numpy()), ref[2]) <= TOL[prec]
 
 
-def test_adjoint_and_reduced_basis_say_unsupported():
-    mesh = nm.Mesh((4, 4, 4), (2e-9,) * 3, dtype=torch.float64, terms=1 | 32, Ms=8e5, A=1.3e-11, Kc=1e4)
-    m = dev(wl.random_unit_field((5, 5, 5), 1), torch.float64)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n,uniform,terms", [((9, 6, 5), False, 1 | 2 | 4 | 16 | 32), ((128, 6, 5), True, 1 | 2 | 32),
+                                             ((7, 5, 4), False, 32)])
+def test_adjoint_rhs_and_backward_step_with_cubic_anisotropy(n, uniform, terms, prec):
+    """The cubic term is not linear in m: pass 2 of the adjoint right-hand side applies the Hessian of its energy at
+    m to q = b / (S Ms) (oracle more_terms.hessvec_cubic).  (f, -(df/dm)^T a, -(df/dMs)^T a) against the oracle,
+    then three backward RK4 steps of (m, a, u)."""
+    from oracle import adjoint, llg
+    p, mesh, m = _case(n, prec, terms, "bulk", uniform=uniform, seed=21)
+    a = wl.round_to(np.random.default_rng(22).standard_normal(m.shape), ND[prec])
+    f_ref, da_ref, du_ref = adjoint.adjoint_rhs(p, 0.0, m, a)
+    f, da, du = mesh.nm_llg_adjoint_rhs(0.0, dev(m, TD[prec]), dev(a, TD[prec]))
+    assert_parity(host(f), f_ref, TOL[prec], "f")
+    assert_parity(host(da), da_ref, TOL[prec], "da/dt with cubic")
+    assert rel_l2(wl.from_abi(du.cpu().double().numpy()), du_ref) <= TOL[prec]
+    dt = 2e-14
+    mT = m.copy()
+    for s in range(3):
+        mT = llg.rk4_step(p, s * dt, dt, mT)
+    ref = adjoint.backward_rk4(p, mT, a, dt, 3)
+    mm, aa = dev(mT, TD[prec]), dev(a, TD[prec])
+    uu = torch.zeros(mesh.cell_shape_abi, dtype=TD[prec], device=mm.device)
+    for s in range(3, 0, -1):
+        mesh.nm_adjoint_rk4_step(s * dt, dt, mm, aa, uu)
+    assert rel_l2(host(aa), ref[1]) <= TOL[prec]
+    assert rel_l2(wl.from_abi(uu.cpu().double().numpy()), ref[2]) <= TOL[prec]
+
+
+def test_reduced_basis_says_unsupported():
+    mesh = nm.Mesh((8, 8, 1), (2e-9,) * 3, dtype=torch.float64, terms=1, Ms=8e5, A=1.3e-11, basis=2)
+    m = dev(wl.random_unit_field((9, 9, 1), 1), torch.float64)
     with pytest.raises(nm.NmError) as e:
         mesh.nm_llg_adjoint_rhs(0.0, m, m.clone())
     assert e.value.status == nm.NM_EUNSUPPORTED

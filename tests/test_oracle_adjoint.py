@@ -71,6 +71,33 @@ def test_dense_jacobians_by_finite_differences(terms):
     assert np.allclose(-dudt.ravel(), JMs_T_a, rtol=1e-6, atol=1e-7 * np.abs(JMs_T_a).max())
 
 
+def test_dense_jacobian_with_a_vacuum_corner():
+    """Reading C7 carries no adjoint at nodes with (S Ms)_n = 0.  With every material constant 0 in the vacuum cells
+    (the vacuum is empty) that is the exact transposed Jacobian, vacuum nodes included: a node of a magnetic cell
+    always has (S Ms) > 0, so m at a vacuum node enters no field.  3x3x2 cells with a 2x2x2 vacuum corner, every term
+    on (DMI and the cubic term included), a^T J by central differences of the forward RHS."""
+    terms = ALL | TERM_DMI | TERM_CUBIC
+    p, zee = make(n=(3, 3, 2), terms=terms, seed=7)
+    vac = np.zeros(p.n_cells, dtype=bool)
+    vac[:2, :2, :] = True
+    p = dataclasses.replace(p, **{k: np.where(vac, 0.0, getattr(p, k)) for k in ("Ms", "A", "Ku", "D", "Kc")})
+    assert np.any(p.L == 0) and np.any(p.L > 0)
+    rng = np.random.default_rng(8)
+    m = rand_unit(p.node_shape, 9) * (1 + 0.05 * rng.standard_normal(p.node_shape))
+    a = rng.standard_normal(m.shape)
+    _, dadt, _ = adjoint.adjoint_rhs(p, 0.0, m, a, zee)
+    fl, Jm_T_a = m.ravel(), np.zeros(m.size)
+    for k in range(m.size):
+        h = 1e-6
+        mp_, mm_ = fl.copy(), fl.copy()
+        mp_[k] += h
+        mm_[k] -= h
+        col = (llg.llg_rhs(p, 0.0, mp_.reshape(m.shape), zee) - llg.llg_rhs(p, 0.0, mm_.reshape(m.shape), zee)) / (2 * h)
+        Jm_T_a[k] = np.sum(a * col)
+    assert np.allclose(-dadt.ravel(), Jm_T_a, rtol=1e-7, atol=1e-8 * np.abs(Jm_T_a).max())
+    assert np.all(dadt[:, p.L == 0] == 0)
+
+
 def test_dot_product_test_larger_mesh():
     """<a, J v> = <J^T a, v> with J v by central differences (6x5x3 cells, all terms)."""
     p, zee = make(n=(6, 5, 3), seed=3)

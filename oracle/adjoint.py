@@ -21,6 +21,9 @@ neural-ODE reference 26.)  The paper delegates both products to framework autodi
                           + sum_i b_{c+i} . mu0 (M Hext_loc)_i / L_{c+i}
                           + (S^T q)_c . Hcell_c + mbar_c . Y_c
      q = b / (S Ms),  mbar = S^T m / 8,  Hcell = -N * (Ms mbar),  Y = -N * (Ms o S^T q)
+
+On the reduced 2-D / 1-D bases of Eqs. (23)-(24) (Problem.basis) the same formulas hold with the operators of
+oracle/lowdim.py: S, S^T over the 2^D vertices of a cell, mbar = S^T m / 2^D, the reduced element matrices.
 """
 import dataclasses
 
@@ -29,9 +32,21 @@ import numpy as np
 from . import demag as _demag
 from . import llg as _llg
 from . import local_fields as _lf
+from . import lowdim as _ld
 from . import more_terms as _mt
 from .mesh import (LOCAL, MU0, element_matrices, gather_nodes_to_cells, node_view,
                    scatter_cells_to_nodes)
+
+
+def _basis_ops(p):
+    """(local vertices, node_view, S, S^T, mass matrix M, vertices per cell) of the problem's nodal basis:
+    the 3-D one (oracle/mesh.py) or the reduced one of Eqs. (23)-(24) (oracle/lowdim.py).  The formulas in
+    this file's header hold for both, with 2^D vertices per cell in place of 8."""
+    D = p.basis
+    if D == 3:
+        return LOCAL, node_view, scatter_cells_to_nodes, gather_nodes_to_cells, element_matrices(p.dx)[1], 8
+    return (_ld.local(D), lambda a, i: _ld.node_view(a, i, D), lambda b: _ld.scatter_cells_to_nodes(b, D),
+            lambda a: _ld.gather_nodes_to_cells(a, D), _ld.element_matrices(p.dx, D)[1], 2 ** D)
 
 
 def _safe_div(num, den):
@@ -49,7 +64,8 @@ def adjoint_rhs(p, t, m, a, zeeman=None, pieces=None):
     gp = p.gamma / (1.0 + p.alpha ** 2)
     al = p.alpha
     L = p.L
-    SMs = scatter_cells_to_nodes(p.Ms)
+    local, nview, scatter, gather, M, nv = _basis_ops(p)
+    SMs = scatter(p.Ms)
     h_ext = zeeman(t) if zeeman is not None else None
     if h_ext is not None:
         h_ext = np.asarray(h_ext, dtype=np.float64)
@@ -75,27 +91,26 @@ def adjoint_rhs(p, t, m, a, zeeman=None, pieces=None):
     dadt = -(d + HTb)
 
     # -(df/dMs)^T a
-    grad = -gather_nodes_to_cells(_safe_div(dot(b, H), SMs))
+    grad = -gather(_safe_div(dot(b, H), SMs))
     if pieces is not None:
         pieces["field"] = grad.copy()
         # the same sum with every product b_j H_j taken in magnitude: b is perpendicular to m, so the
         # m-parallel part of H (most of the exchange field of a smooth m) cancels inside b . H
-        pieces["field_abs"] = gather_nodes_to_cells(
+        pieces["field_abs"] = gather(
             _safe_div(np.abs(b[0] * H[0]) + np.abs(b[1] * H[1]) + np.abs(b[2] * H[2]), SMs))
     if (p.terms & _llg.TERM_ZEEMAN) and h_ext is not None:
-        _, M = element_matrices(p.dx)
         bL = _safe_div(b, L)
         zee = np.zeros_like(grad)
-        for i in LOCAL:
-            for ip in LOCAL:
-                zee = zee + MU0 * M[i + ip] * np.sum(node_view(bL, i) * node_view(h_ext, ip), axis=0)
+        for i in local:
+            for ip in local:
+                zee = zee + MU0 * M[i + ip] * np.sum(nview(bL, i) * nview(h_ext, ip), axis=0)
         grad = grad + zee
         if pieces is not None:
             pieces["zeeman"] = zee
     if p.terms & _llg.TERM_DEMAG:
         q = _safe_div(b, SMs)
-        STq = gather_nodes_to_cells(q)
-        mbar = gather_nodes_to_cells(m) / 8.0
+        STq = gather(q)
+        mbar = gather(m) / nv
         Hcell = _demag.demag_field_cells_fft(p.Ms * mbar, p.Nt)
         Y = _demag.demag_field_cells_fft(p.Ms * STq, p.Nt)
         grad = grad + np.sum(STq * Hcell, axis=0) + np.sum(mbar * Y, axis=0)
@@ -136,6 +151,8 @@ def adjoint_rhs_hnodal(p, t, m, a):
     gp = p.gamma / (1.0 + p.alpha ** 2)
     mxa = _llg.cross(m, a)
     b = gp * mxa - p.alpha * gp * _llg.cross(m, mxa)
+    if p.basis != 3:
+        return _ld.variation_zeeman(_safe_div(b, p.L), p.Ms, p.dx, p.basis)
     return _lf.variation_zeeman(_safe_div(b, p.L), p.Ms, p.dx)
 
 
@@ -153,18 +170,19 @@ def adjoint_rhs_materials(p, t, m, a):
     mxa = _llg.cross(m, a)
     b = gp * mxa - p.alpha * gp * _llg.cross(m, mxa)
     bL = _safe_div(b, p.L)
-    K, M = element_matrices(p.dx)
+    local, nview = _basis_ops(p)[:2]
+    K, M = element_matrices(p.dx) if p.basis == 3 else _ld.element_matrices(p.dx, p.basis)
     k = np.asarray(p.ku_axis, dtype=np.float64)
     bk = k[0] * bL[0] + k[1] * bL[1] + k[2] * bL[2]
     mk = k[0] * m[0] + k[1] * m[1] + k[2] * m[2]
     gA = np.zeros(p.n_cells)
     gKu = np.zeros(p.n_cells)
-    for i in LOCAL:
-        for ip in LOCAL:
+    for i in local:
+        for ip in local:
             if p.terms & _llg.TERM_EXCHANGE:
-                gA += -2.0 * K[i + ip] * np.sum(node_view(bL, i) * node_view(m, ip), axis=0)
+                gA += -2.0 * K[i + ip] * np.sum(nview(bL, i) * nview(m, ip), axis=0)
             if p.terms & _llg.TERM_ANISO:
-                gKu += 2.0 * M[i + ip] * node_view(bk, i) * node_view(mk, ip)
+                gKu += 2.0 * M[i + ip] * nview(bk, i) * nview(mk, ip)
     return -gA, -gKu
 
 

@@ -431,3 +431,66 @@ def test_cubic_hessian_vector_product_is_the_derivative_of_the_variation():
     fd = (mt.variation_cubic(m + eps * v, Kc, axes, dx) - mt.variation_cubic(m - eps * v, Kc, axes, dx)) / (2 * eps)
     assert np.allclose(hv, fd, rtol=1e-8, atol=1e-9 * np.abs(fd).max())
     assert np.isclose(np.sum(u * hv), np.sum(v * mt.hessvec_cubic(m, u, Kc, axes, dx)), rtol=1e-12)
+
+
+@pytest.mark.parametrize("D,n", [(2, (3, 2, 1)), (1, (4, 1, 1))])
+def test_reduced_basis_vjps_against_finite_differences(D, n):
+    """The adjoint right-hand side on the reduced bases of Eqs. (23)-(24) (Problem.basis = 2, 1): every
+    vector-Jacobian product against central differences of the forward RHS of the same basis (itself pinned in
+    tests/test_oracle_lowdim.py), all four base terms on, one vacuum cell: a^T df/dm and a^T df/dMs densely,
+    a^T df/dh for a uniform and for a nodal external field, a^T df/dA_c and a^T df/dKu_c for every cell."""
+    rng = np.random.default_rng(40 + D)
+    dx = (3e-9, 2.5e-9, 3.5e-9)
+    Ms = rng.uniform(4e5, 8e5, n)
+    Ms[0, 0, 0] = 0.0
+    p = Problem(n, dx, Ms, rng.uniform(0.8e-11, 1.3e-11, n), rng.uniform(1e5, 5e5, n), ku_axis=(0.0, 0.6, 0.8),
+                alpha=0.1, terms=ALL, basis=D)
+    p.Nt
+    assert np.any(p.L == 0)
+    hext = rng.standard_normal((3,) + p.node_shape) * 3e4
+    zee = lambda t: hext
+    m = rand_unit(p.node_shape, 2) * (1 + 0.05 * rng.standard_normal(p.node_shape))
+    a = rng.standard_normal(m.shape)
+    rhs = lambda prob, mm, hh=hext: llg.llg_rhs(prob, 0.0, mm, lambda t: hh)
+    f, dadt, dudt = adjoint.adjoint_rhs(p, 0.0, m, a, zee)
+    assert np.allclose(f, rhs(p, m), rtol=1e-14)
+    live = np.broadcast_to(p.L > 0, m.shape).ravel()
+    got = -dadt.ravel()
+    for k in range(m.size):
+        e = np.zeros(m.size)
+        e[k] = 1e-6
+        fd = np.sum(a * (rhs(p, m + e.reshape(m.shape)) - rhs(p, m - e.reshape(m.shape)))) / 2e-6
+        if live[k]:
+            assert abs(got[k] - fd) <= 1e-7 * np.abs(got).max(), (k, got[k], fd)
+        else:
+            assert got[k] == 0.0          # reading C7: no adjoint at vacuum nodes
+    for c in np.ndindex(*n):
+        if p.Ms[c] == 0:
+            continue
+        h = 1e-4 * p.Ms[c]
+        up, dn = p.Ms.copy(), p.Ms.copy()
+        up[c] += h
+        dn[c] -= h
+        fd = np.sum(a * (rhs(dataclasses.replace(p, Ms=up), m) - rhs(dataclasses.replace(p, Ms=dn), m))) / (2 * h)
+        assert abs(-dudt[c] - fd) <= 1e-6 * np.abs(dudt).max(), (c, dudt[c], fd)
+    # external field: uniform and nodal
+    gu = adjoint.adjoint_rhs_hext(p, 0.0, m, a)
+    gn = adjoint.adjoint_rhs_hnodal(p, 0.0, m, a)
+    assert np.allclose(gn.reshape(3, -1).sum(axis=1), gu, rtol=1e-12)
+    eps = 10.0
+    for k in range(0, m.size, 3):
+        e = np.zeros(m.size)
+        e[k] = eps
+        e = e.reshape(m.shape)
+        fd = -np.sum(a * (rhs(p, m, hext + e) - rhs(p, m, hext - e))) / (2 * eps)
+        assert abs(gn.ravel()[k] - fd) <= 1e-9 * np.abs(gn).max(), (k, gn.ravel()[k], fd)
+    gA, gKu = adjoint.adjoint_rhs_materials(p, 0.0, m, a)
+    for c in np.ndindex(*n):
+        for name, g in (("A", gA), ("Ku", gKu)):
+            base = getattr(p, name)
+            h = 0.1 * base[c]
+            up, dn = base.copy(), base.copy()
+            up[c] += h
+            dn[c] -= h
+            fd = -np.sum(a * (rhs(dataclasses.replace(p, **{name: up}), m) - rhs(dataclasses.replace(p, **{name: dn}), m))) / (2 * h)
+            assert abs(g[c] - fd) <= 1e-9 * np.abs(g).max(), (name, c, g[c], fd)

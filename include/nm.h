@@ -92,8 +92,8 @@ typedef struct {
                                      arrays are [3][1][1][N1+1].
                              The weak form is still integrated over the 3-D cells (element matrices
                              without derivatives along the reduced axes, lumped mass V / 2^D per cell,
-                             node <-> cell averaging over the 2^D vertices of a cell).  Forward path only:
-                             the adjoint entry points return NM_EUNSUPPORTED on a reduced basis. */
+                             node <-> cell averaging over the 2^D vertices of a cell).  Every entry
+                             point serves the reduced bases, the adjoint ones included. */
     /* NM_TERM_DMI / NM_TERM_CUBIC (3-D basis).  Both are carried by every entry point (the adjoint ones give
        d/dm and d/dMs, not d/dD or d/dKc): the DMI term is linear in m like the exchange term; for the cubic
        term the adjoint right-hand side applies the Hessian of its energy at m.  The element contributions are

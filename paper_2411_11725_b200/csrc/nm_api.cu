@@ -809,6 +809,7 @@ nm_status adjoint_eval(nm_mesh *m, double t, const T *mm, const T *av, const nm_
         }
         c.terms = (m->desc.terms & NM_TERM_ZEEMAN) && z ? m->desc.terms : (m->desc.terms & ~(unsigned)NM_TERM_ZEEMAN);
         c.dudt = dudt;
+        c.red = (T)nm_red_scale(m);
         NM_TRY(nm_launch_adj_cell<T>(m, c, st));
     }
     return NM_OK;
@@ -836,7 +837,7 @@ nm_status mat_grad(nm_mesh *m, const T *mm, const T *av, T *uA, T *uKu, double c
     g.gp = la.gp;
     g.agp = la.agp;
     const double V = m->desc.cell_size[0] * m->desc.cell_size[1] * m->desc.cell_size[2];
-    g.invL = (T)(8.0 / (NM_MU0 * V));
+    g.invL = (T)(8.0 * nm_red_scale(m) / (NM_MU0 * V));     // 2^D / (mu0 V)
     g.coef = (T)coef;
     g.accumulate = accumulate;
     g.ex_on = (m->desc.terms & NM_TERM_EXCHANGE) != 0;
@@ -960,15 +961,6 @@ nm_status check_call(nm_mesh *mesh, const void *p0, const void *p1)
     return NM_OK;
 }
 
-nm_status check_adjoint(const nm_mesh *mesh)
-{
-    if (mesh && mesh->g.zs == 0) {
-        nm_set_error("the adjoint entry points serve the full 3-D basis only (basis = %d)", mesh->desc.basis);
-        return NM_EUNSUPPORTED;
-    }
-    return NM_OK;
-}
-
 } // namespace
 
 extern "C" nm_status nm_heff(nm_mesh *mesh, double t, const void *m, const nm_zeeman *zeeman, void *H_out,
@@ -1037,7 +1029,6 @@ extern "C" nm_status nm_llg_adjoint_rhs(nm_mesh *mesh, double t, const void *m, 
                                         void *dudt_Ms_out, void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
-    NM_TRY(check_adjoint(mesh));
     if (!dadt_out) { nm_set_error("dadt_out is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     return mesh->f64 ? adjoint_eval<double>(mesh, t, (const double *)m, (const double *)a, zeeman,
@@ -1052,7 +1043,6 @@ nm_status adjoint_rk4_entry(nm_mesh *mesh, double t, double dt, void *m_inout, v
                             int renormalise, void *stream)
 {
     NM_TRY(check_call(mesh, m_inout, a_inout));
-    NM_TRY(check_adjoint(mesh));
     if (!u_inout) { nm_set_error("u_inout is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     NmStepKey key;
@@ -1106,7 +1096,6 @@ extern "C" nm_status nm_llg_adjoint_rhs_hnodal(nm_mesh *mesh, const void *m, con
                                                void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
-    NM_TRY(check_adjoint(mesh));
     if (!dudt_hn_out) { nm_set_error("dudt_hn_out is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     if (!(mesh->desc.terms & NM_TERM_ZEEMAN)) {
@@ -1129,7 +1118,6 @@ extern "C" nm_status nm_llg_adjoint_rhs_materials(nm_mesh *mesh, const void *m, 
                                                   void *dudt_Ku_out, void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
-    NM_TRY(check_adjoint(mesh));
     if (!dudt_A_out && !dudt_Ku_out) { nm_set_error("both outputs are NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     return mesh->f64 ? mat_grad<double>(mesh, (const double *)m, (const double *)a, (double *)dudt_A_out,
@@ -1142,7 +1130,6 @@ extern "C" nm_status nm_llg_adjoint_rhs_hext(nm_mesh *mesh, const void *m, const
                                              void *stream)
 {
     NM_TRY(check_call(mesh, m, a));
-    NM_TRY(check_adjoint(mesh));
     if (!dudt_h_out) { nm_set_error("dudt_h_out is NULL"); return NM_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
     NM_CUDA_TRY(cudaMemsetAsync(dudt_h_out, 0, 3 * sizeof(double), st));

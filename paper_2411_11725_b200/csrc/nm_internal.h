@@ -143,6 +143,16 @@ struct nm_mesh {
     NmStepGraph step_graph[NM_GRAPH_SLOTS];
 };
 
+// 2^(D-3) for a nodal basis that varies in D axes (1 on the 3-D basis).  The kernels reach a reduced basis through
+// zero node strides along the reduced axes, which counts every vertex of a cell 2^(3-D) times and keeps the 3-D
+// lumped mass V / 8: the cell-wise gradients of the adjoint entry points take this factor once (a node kernel sees
+// only its own half of each reduced axis, (1/3 + 1/6) of the mass row, which cancels against V / 8 vs V / 2^D).
+inline double nm_red_scale(const nm_mesh *m)
+{
+    const int D = m->desc.basis == 0 ? 3 : m->desc.basis;
+    return D >= 3 ? 1.0 : (D == 2 ? 0.5 : 0.25);
+}
+
 // Brackets one kernel launch with an event pair when profiling is on, and counts it.
 struct NmLaunchScope {
     nm_mesh *m;

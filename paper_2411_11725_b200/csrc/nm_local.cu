@@ -276,8 +276,8 @@ __global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a
     const long long nn = g.nodes;
     const long long n = (long long)i3 * pl + p;
     const int ox[3] = {i1 > 0 ? -1 : 0, 0, i1 < g.N1 ? 1 : 0};
-    const int oy[3] = {i2 > 0 ? -g.n1 : 0, 0, i2 < g.N2 ? g.n1 : 0};
-    const int oz[3] = {i3 > 0 ? -pl : 0, 0, i3 < g.N3 ? pl : 0};
+    const int oy[3] = {i2 > 0 ? -g.ys : 0, 0, i2 < g.N2 ? g.ys : 0};      // 0 along a reduced axis, as in k_node
+    const int oz[3] = {i3 > 0 ? -g.zs : 0, 0, i3 < g.N3 ? g.zs : 0};
     const bool vx[2] = {i1 > 0, i1 < g.N1}, vy[2] = {i2 > 0, i2 < g.N2}, vz[2] = {i3 > 0, i3 < g.N3};
     const int cx[2] = {i1 > 0 ? i1 - 1 : 0, i1 < g.N1 ? i1 : g.N1 - 1};
     const int cy[2] = {i2 > 0 ? i2 - 1 : 0, i2 < g.N2 ? i2 : g.N2 - 1};
@@ -588,7 +588,8 @@ template <typename T> __global__ void __launch_bounds__(128) k_mat_grad(const Nm
     T mv[8][3], bl[8][3], mk[8], bk[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-        const long long n = ((long long)(c3 + ((i >> 2) & 1)) * g.n2 + (c2 + ((i >> 1) & 1))) * g.n1 + (c1 + (i & 1));
+        // strides g.ys / g.zs: 0 along a reduced axis (the two vertices are one node; a.invL carries the 2^D / 8)
+        const long long n = (long long)(c3 + ((i >> 2) & 1)) * g.zs + (long long)(c2 + ((i >> 1) & 1)) * g.ys + (c1 + (i & 1));
         const T mc[3] = {a.m[n], a.m[nn + n], a.m[2 * nn + n]};
         const T ac[3] = {a.a[n], a.a[nn + n], a.a[2 * nn + n]};
         const T sms = a.sMs[n];
@@ -671,7 +672,7 @@ __global__ void k_adj_cell(const NmAdjCellArgs<T> a)
     long long nd[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i)
-        nd[i] = ((long long)(c3 + (i >> 2)) * g.n2 + (c2 + ((i >> 1) & 1))) * g.n1 + (c1 + (i & 1));
+        nd[i] = (long long)(c3 + (i >> 2)) * g.zs + (long long)(c2 + ((i >> 1) & 1)) * g.ys + (c1 + (i & 1));
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         sw += a.W[nd[i]];
@@ -702,7 +703,8 @@ __global__ void k_adj_cell(const NmAdjCellArgs<T> a)
         for (int j = 0; j < 3; ++j)
             grad += sq[j] * a.Hc1[j * g.cells + c] + sm[j] * a.Hc2[j * g.cells + c];   // mbar.Y = (sm/8).(8 Hc2)
     }
-    a.dudt[c] = -grad;
+    // reduced basis (strides 0): every vertex of the 2^D was counted 2^(3-D) times in each of the four pieces
+    a.dudt[c] = -grad * a.red;
 }
 
 // The same without nodal Zeeman arrays, marching along z: a thread owns one cell column (c1, c2) of

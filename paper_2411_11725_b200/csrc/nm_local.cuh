@@ -70,6 +70,7 @@ template <typename T> struct NmAdjCellArgs {
     T amp;
     T hu[3];
     T wM8V[8];          // (8/V) * mass matrix entry by offset pattern
+    T red;              // 2^(D-3): 1 on the 3-D basis (nm_red_scale)
     unsigned terms;
     T *dudt;
 };

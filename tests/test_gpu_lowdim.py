@@ -142,12 +142,55 @@ def test_reduced_basis_boundary_behaviour():
         with pytest.raises(nm.NmError) as e:
             nm.Mesh(n, (1e-9,) * 3, terms=1, Ms=8e5, A=1e-11, Ku=0.0, basis=basis)
         assert e.value.status == nm.NM_EINVAL
-    mesh = nm.Mesh((8, 8, 1), (1e-9,) * 3, dtype=torch.float64, terms=3, Ms=8e5, A=1e-11, Ku=0.0, basis=2)
-    m = torch.zeros(mesh.node_shape_abi, dtype=torch.float64, device="cuda:0")
-    m[0] = 1.0
-    with pytest.raises(nm.NmError) as e:
-        mesh.nm_llg_adjoint_rhs(0.0, m, m)
-    assert e.value.status == nm.NM_EUNSUPPORTED
     # basis = 0 means the full basis
     full = nm.Mesh((8, 8, 1), (1e-9,) * 3, dtype=torch.float64, terms=3, Ms=8e5, A=1e-11, Ku=0.0, basis=0)
     assert full.node_shape_abi == (3, 2, 9, 9)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n,D", [((24, 12, 1), 2), ((9, 35, 1), 2), ((50, 1, 1), 1), ((1, 1, 1), 2)])
+def test_adjoint_entry_points_on_reduced_bases(n, D, prec):
+    """SURVEY 8(f) rows 1 x 2: the adjoint right-hand side and every gradient on the 2-D / 1-D bases against the oracle
+    (oracle/adjoint.py with the operators of oracle/lowdim.py): f, -(df/dm)^T a, -(df/dMs)^T a with every term on, a
+    vacuum block and a nodal static field; the uniform- and nodal-field gradients; the A_c / Ku_c gradients; then the
+    backward pass of (m, a, u, u_h, u_A, u_Ku, u_hn) over 20 RK4 steps with a checkpoint."""
+    from oracle import adjoint
+    from paper_2411_11725_b200 import drivers
+    td, nd = DT[prec], np_dtype(DT[prec])
+    w, hs = _reduced(*wl.varied_case(n, vacuum=(n[0] >= 6)), D)
+    p = oracle_problem(w, nd, basis=D)
+    z = oracle_zeeman(w, nd, hs)
+    m = wl.round_to(w.m0, nd)
+    a = wl.round_to(np.random.default_rng(61).standard_normal(m.shape), nd)
+    mesh = gpu_mesh(w, td, basis=D)
+    gz = gpu_zeeman(w, td, h_static=hs)
+    f_ref, da_ref, du_ref = adjoint.adjoint_rhs(p, 0.0, m, a, z)
+    f, da, du = mesh.nm_llg_adjoint_rhs(0.0, dev(m, td), dev(a, td), gz)
+    assert_parity(host(f), f_ref, TOL[prec], "f")
+    assert_parity(host(da), da_ref, TOL[prec], "da/dt")
+    # the Ms gradient is a sum of pieces that cancel (DESIGN.md 6): fp32 bound as for the 3-D basis
+    assert rel_l2(wl.from_abi(du.cpu().double().numpy()), du_ref) <= (1e-11 if prec == "f64" else 1e-5)
+    uh = mesh.nm_llg_adjoint_rhs_hext(dev(m, td), dev(a, td)).cpu().numpy()
+    uh_ref = adjoint.adjoint_rhs_hext(p, 0.0, m, a)
+    assert np.max(np.abs(uh - uh_ref)) <= (1e-11 if prec == "f64" else 1e-5) * max(np.max(np.abs(uh_ref)), 1e-300)
+    assert_parity(host(mesh.nm_llg_adjoint_rhs_hnodal(dev(m, td), dev(a, td))), adjoint.adjoint_rhs_hnodal(p, 0.0, m, a),
+                  TOL[prec], "nodal-field gradient")
+    gA, gKu = mesh.nm_llg_adjoint_rhs_materials(dev(m, td), dev(a, td))
+    gA_ref, gKu_ref = adjoint.adjoint_rhs_materials(p, 0.0, m, a)
+    assert rel_l2(wl.from_abi(gA.cpu().double().numpy()), gA_ref) <= TOL[prec]
+    assert rel_l2(wl.from_abi(gKu.cpu().double().numpy()), gKu_ref) <= TOL[prec]
+    # backward pass
+    dt, nst = 2e-14, 20
+    wT = wl.round_to(np.random.default_rng(62).standard_normal(m.shape), nd)
+    mT_ref, ck = adjoint.forward_rk4(p, m, dt, nst, z, checkpoint_every=10)
+    ref = adjoint.backward_rk4(p, mT_ref, wT, dt, nst, z, checkpoints=ck, with_hext=True, with_materials=True,
+                               with_hnodal=True)
+    gT = dev(wT, td)
+    out = drivers.adjoint_gradient(mesh, dev(m, td), lambda mm: gT, dt, nst, gz, checkpoint_every=10, with_hext=True,
+                                   with_materials=True, with_hnodal=True)
+    assert rel_l2(host(out[0]), mT_ref) <= TOL[prec]
+    assert rel_l2(host(out[1]), ref[1]) <= TOL[prec]
+    for k, name in ((2, "u"), (4, "u_A"), (5, "u_Ku")):
+        assert rel_l2(wl.from_abi(out[k].cpu().double().numpy()), ref[k]) <= TOL[prec], name
+    assert np.max(np.abs(out[3].cpu().numpy() - ref[3])) <= TOL[prec] * np.max(np.abs(ref[3]))
+    assert_parity(host(out[6]), ref[6], TOL[prec], "u_hn(0)")

@@ -186,12 +186,7 @@ def test_adjoint_rhs_and_backward_step_with_cubic_anisotropy(n, uniform, terms, 
     assert rel_l2(wl.from_abi(uu.cpu().double().numpy()), ref[2]) <= TOL[prec]
 
 
-def test_reduced_basis_says_unsupported():
-    mesh = nm.Mesh((8, 8, 1), (2e-9,) * 3, dtype=torch.float64, terms=1, Ms=8e5, A=1.3e-11, basis=2)
-    m = dev(wl.random_unit_field((9, 9, 1), 1), torch.float64)
-    with pytest.raises(nm.NmError) as e:
-        mesh.nm_llg_adjoint_rhs(0.0, m, m.clone())
-    assert e.value.status == nm.NM_EUNSUPPORTED
+def test_further_terms_on_a_reduced_basis_and_a_skewed_frame_are_refused():
     with pytest.raises(nm.NmError) as e:
         nm.Mesh((8, 8, 1), (2e-9,) * 3, dtype=torch.float64, terms=1 | 32, Ms=8e5, A=1.3e-11, Kc=1e4, basis=2)
     assert e.value.status == nm.NM_EUNSUPPORTED

@@ -52,9 +52,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         : "memory");
 }
 
-// The same wait for a thread that has nothing else to do (a copy warp): between probes it sleeps, so
-// that its probe / branch instructions do not take issue slots from the warps that share its scheduler
-// (a failed try_wait returns within a few cycles; the arbiter favours the highest warp id).
+// The same wait for a thread that has nothing else to do (a copy warp): the probe carries a suspend-time hint, so
+// the thread is parked in the barrier unit until the phase completes (or the hint runs out) instead of coming back
+// within a few cycles, and sleeps before probing again; its probe / branch instructions then take next to no issue
+// slots from the transform warps that share its scheduler.
 __device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t parity)
 {
     uint32_t done;
@@ -62,14 +63,14 @@ __device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t parity)
         asm volatile(
             "{\n"
             ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
             "selp.u32 %0, 1, 0, p;\n"
             "}\n"
             : "=r"(done)
-            : "r"(smem_u32(bar)), "r"(parity)
+            : "r"(smem_u32(bar)), "r"(parity), "r"(1000000u)
             : "memory");
         if (done) break;
-        __nanosleep(128);
+        __nanosleep(256);
     }
 }
 

@@ -264,20 +264,51 @@ __global__ void __launch_bounds__(kBlock) k_node(const NmLocalArgs<T> a)
 // GRAD: the transpose of the same operator, for the gradient with respect to a nodal external field
 // (SURVEY.md 8(f) row 2): with h := q = b / (S Ms),  out (+)= coef (-(8/V) sum_c Ms_c sum_i' M_{i,i'} q_{c+i'})
 // = coef Z(b / L) = -coef (df/dh)^T a  (oracle/adjoint.py: adjoint_rhs_hnodal).
+// A CTA owns a ZX x ZY patch of nodes of one plane: the field (h_static + amp h_pulse) of the patch, its halo and the
+// two neighbouring planes goes through shared memory once, and the 27-point sums read it from there.
+constexpr int ZX = 32, ZY = 8, ZPX = ZX + 2, ZPY = ZY + 2;
 template <typename T, bool GRAD>
-__global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a, T *__restrict__ Zs, T coef, int accumulate)
+__global__ void __launch_bounds__(ZX * ZY) k_zeeman_smooth(const NmLocalArgs<T> a, T *__restrict__ Zs, T coef, int accumulate)
 {
+    __shared__ T sh[3][3][ZPY][ZPX];
     const NmGeom &g = a.g;
-    const int pl = g.n1 * g.n2;
-    const int p = blockIdx.x * kBlock + threadIdx.x;
-    const int i3 = blockIdx.y;
-    if (p >= pl) return;
-    const int i2 = p / g.n1, i1 = p - i2 * g.n1;
     const long long nn = g.nodes;
-    const long long n = (long long)i3 * pl + p;
-    const int ox[3] = {i1 > 0 ? -1 : 0, 0, i1 < g.N1 ? 1 : 0};
-    const int oy[3] = {i2 > 0 ? -g.ys : 0, 0, i2 < g.N2 ? g.ys : 0};      // 0 along a reduced axis, as in k_node
-    const int oz[3] = {i3 > 0 ? -g.zs : 0, 0, i3 < g.N3 ? g.zs : 0};
+    const int x0 = blockIdx.x * ZX, y0 = blockIdx.y * ZY, i3 = blockIdx.z;
+    // a thread fills (xx, yy) = (tx, ty) and, at the patch edges, (tx + ZX, .) for tx < 2 and (., ty + ZY) for ty < 2
+    // along an axis the basis does not vary in, every neighbour is the node itself (strides g.ys / g.zs = 0)
+    auto fill = [&](auto value) {
+#pragma unroll
+        for (int ry = 0; ry < 2; ++ry) {
+            const int yy = threadIdx.y + ry * ZY;
+            const int gy = g.ys ? y0 - 1 + yy : 0;
+#pragma unroll
+            for (int rx = 0; rx < 2; ++rx) {
+                const int xx = threadIdx.x + rx * ZX;
+                const int gx = x0 - 1 + xx;
+                const bool mine = (!ry || threadIdx.y < 2) && (!rx || threadIdx.x < 2);
+                const bool okxy = mine && gx >= 0 && gx < g.n1 && gy >= 0 && gy < g.n2;
+#pragma unroll
+                for (int dz = 0; dz < 3; ++dz) {
+                    const int gz = g.zs ? i3 - 1 + dz : 0;
+                    const bool ok = okxy && gz >= 0 && gz < g.n3;
+                    const long long q = ok ? ((long long)gz * g.n2 + gy) * g.n1 + gx : 0;
+#pragma unroll
+                    for (int j = 0; j < 3; ++j) {
+                        const T v = value(j * nn + q);
+                        if (mine) sh[j][dz][yy][xx] = ok ? v : (T)0;
+                    }
+                }
+            }
+        }
+    };
+    if (a.h_static && a.h_pulse) fill([&](long long q) { return a.h_static[q] + a.amp * a.h_pulse[q]; });
+    else if (a.h_pulse) fill([&](long long q) { return a.amp * a.h_pulse[q]; });
+    else if (a.h_static) fill([&](long long q) { return a.h_static[q]; });
+    else fill([&](long long) { return (T)0; });
+    __syncthreads();
+    const int i1 = x0 + threadIdx.x, i2 = y0 + threadIdx.y;
+    if (i1 >= g.n1 || i2 >= g.n2) return;
+    const long long n = ((long long)i3 * g.n2 + i2) * g.n1 + i1;
     const bool vx[2] = {i1 > 0, i1 < g.N1}, vy[2] = {i2 > 0, i2 < g.N2}, vz[2] = {i3 > 0, i3 < g.N3};
     const int cx[2] = {i1 > 0 ? i1 - 1 : 0, i1 < g.N1 ? i1 : g.N1 - 1};
     const int cy[2] = {i2 > 0 ? i2 - 1 : 0, i2 < g.N2 ? i2 : g.N2 - 1};
@@ -290,6 +321,22 @@ __global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a
         cM[ci] = (vx[bx] && vy[by] && vz[bz]) ? a.Ms[c] : (T)0;
         sms += cM[ci];
     }
+    // Ms summed over the cells that contain both n and n + delta (none: the neighbour does not exist), axis by axis:
+    // offset -1 / +1 along an axis keeps the cells on that side, offset 0 keeps both
+    T sx[3][2][2], sxy[3][3][2];
+#pragma unroll
+    for (int bz = 0; bz < 2; ++bz)
+#pragma unroll
+        for (int by = 0; by < 2; ++by) {
+            const T lo = cM[by * 2 + bz * 4], hi = cM[1 + by * 2 + bz * 4];
+            sx[0][by][bz] = lo; sx[1][by][bz] = lo + hi; sx[2][by][bz] = hi;
+        }
+#pragma unroll
+    for (int dx = 0; dx < 3; ++dx)
+#pragma unroll
+        for (int bz = 0; bz < 2; ++bz) {
+            sxy[dx][0][bz] = sx[dx][0][bz]; sxy[dx][1][bz] = sx[dx][0][bz] + sx[dx][1][bz]; sxy[dx][2][bz] = sx[dx][1][bz];
+        }
     T ze[3] = {0, 0, 0};
 #pragma unroll
     for (int dz = -1; dz <= 1; ++dz)
@@ -298,23 +345,11 @@ __global__ void __launch_bounds__(kBlock) k_zeeman_smooth(const NmLocalArgs<T> a
 #pragma unroll
             for (int dx = -1; dx <= 1; ++dx) {
                 const int e = (dx != 0) | ((dy != 0) << 1) | ((dz != 0) << 2);
-                T sM = 0;
-#pragma unroll
-                for (int ci = 0; ci < 8; ++ci) {
-                    const int bx = ci & 1, by = (ci >> 1) & 1, bz = ci >> 2;
-                    const bool in = (dx == 0 || bx == (dx + 1) / 2) && (dy == 0 || by == (dy + 1) / 2) &&
-                                    (dz == 0 || bz == (dz + 1) / 2);
-                    if (in) sM += cM[ci];
-                }
-                const long long q = n + ox[dx + 1] + oy[dy + 1] + oz[dz + 1];
+                const T lo = sxy[dx + 1][dy + 1][0], hi = sxy[dx + 1][dy + 1][1];
+                const T sM = dz < 0 ? lo : (dz > 0 ? hi : lo + hi);
                 const T w = a.wM[e] * sM;
 #pragma unroll
-                for (int j = 0; j < 3; ++j) {
-                    T hv = 0;
-                    if (a.h_static) hv += a.h_static[j * nn + q];
-                    if (a.h_pulse) hv += a.amp * a.h_pulse[j * nn + q];
-                    ze[j] += w * hv;
-                }
+                for (int j = 0; j < 3; ++j) ze[j] += w * sh[j][dz + 1][threadIdx.y + 1 + dy][threadIdx.x + 1 + dx];
             }
     const T sc = sms > 0 ? a.mu0 / (a.mu0V8 * sms) : (T)0;
 #pragma unroll
@@ -1022,8 +1057,8 @@ template <typename T> nm_status nm_launch_node(nm_mesh *mesh, const NmLocalArgs<
         // nodal Zeeman arrays with uniform A and Ku: smooth the field once, then the separable kernels
         {
             NmLaunchScope sc(mesh, NM_K_OTHER, st);
-            const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
-            k_zeeman_smooth<T, false><<<grid, kBlock, 0, st>>>(a, (T *)mesh->Zs, (T)0, 0);
+            const dim3 grid((a.g.n1 + ZX - 1) / ZX, (a.g.n2 + ZY - 1) / ZY, a.g.n3);
+            k_zeeman_smooth<T, false><<<grid, dim3(ZX, ZY), 0, st>>>(a, (T *)mesh->Zs, (T)0, 0);
         }
         NM_CUDA_TRY(cudaGetLastError());
         NmLocalArgs<T> b = a;
@@ -1135,8 +1170,8 @@ nm_status nm_launch_hnodal_grad(nm_mesh *mesh, const NmLocalArgs<T> &base, const
     a.hadd = nullptr;
     {
         NmLaunchScope sc(mesh, NM_K_OTHER, st);
-        const dim3 grid(nblk((long long)a.g.n1 * a.g.n2, kBlock), a.g.n3);
-        k_zeeman_smooth<T, true><<<grid, kBlock, 0, st>>>(a, u_hn, (T)coef, accumulate);
+        const dim3 grid((a.g.n1 + ZX - 1) / ZX, (a.g.n2 + ZY - 1) / ZY, a.g.n3);
+        k_zeeman_smooth<T, true><<<grid, dim3(ZX, ZY), 0, st>>>(a, u_hn, (T)coef, accumulate);
     }
     NM_CUDA_TRY(cudaGetLastError());
     return NM_OK;

@@ -219,14 +219,12 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 #pragma unroll
                 for (int c = 0; c < 3; ++c) shift32<T, true>(a[c]);
             }
+            // even + odd half: the lane of half h keeps rows t = s + 8 h (half_sum)
+            V *colh = col + (size_t)h * 8 * M * TW;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
 #pragma unroll
-                for (int t = 0; t < 16; ++t) {
-                    V v = a[c][t];
-                    v = cadd(v, shfl1(v));
-                    if ((t >> 3) == h) col[(c * N + M * t) * TW] = v;
-                }
+                for (int s = 0; s < 8; ++s) colh[(c * N + M * s) * TW] = half_sum(a[c], s, h);
             }
             fence_async_smem();
             __syncwarp();
@@ -412,11 +410,7 @@ k_pz_mid8(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nIte
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
 #pragma unroll
-                for (int t = 0; t < 16; ++t) {
-                    V v = a[c][t];
-                    v = cadd(v, shfl1(v));
-                    if ((t >> 3) == h) ((t & 1) ? colO : colE)[(c * N + M * t) * TW] = v;
-                }
+                for (int s = 0; s < 8; ++s) ((s & 1) ? colO : colE)[(c * N + M * (s + 8 * h)) * TW] = half_sum(a[c], s, h);
             }
             fence_async_smem();
             __syncwarp();
@@ -608,7 +602,7 @@ k_pz_mid64(double2 *__restrict__ B, const double *__restrict__ Tn, int N2, int n
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
 #pragma unroll
-                for (int t = 0; t < 16; ++t) {
+                for (int t = 0; t < 16; ++t) {      // (fp64: half_sum's selects cost more registers than the kernel has)
                     V v = a[c][t];
                     v = cadd(v, shfl1(v));
                     if ((t >> 3) == h) out[(c * N + M * t) * TW] = v;
@@ -1088,8 +1082,7 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
             T *rowA = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0 + 2 * line) * n1row;
 #pragma unroll
             for (int tt = 0; tt < 8; ++tt) {
-                const V lo = cadd(a[tt], shfl1(a[tt])), hi = cadd(a[tt + 8], shfl1(a[tt + 8]));
-                const V v = h ? hi : lo;
+                const V v = half_sum(a, tt, h);
                 const int e = j + M * (tt + 8 * h);
                 if (!EMB || e < n1row) {
                     rowA[e] = v.x;
@@ -1099,13 +1092,10 @@ k_px_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
         } else {
             // short lines: through a row-major staging tile, 16-byte stores
 #pragma unroll
-            for (int t = 0; t < 16; ++t) {
-                V v = a[t];
-                v = cadd(v, shfl1(v));
-                if ((t >> 3) == h) {
-                    s_out[(2 * line) * N + j + M * t] = v.x;
-                    s_out[(2 * line + 1) * N + j + M * t] = v.y;
-                }
+            for (int s = 0; s < 8; ++s) {
+                const V v = half_sum(a, s, h);
+                s_out[(2 * line) * N + j + M * (s + 8 * h)] = v.x;
+                s_out[(2 * line + 1) * N + j + M * (s + 8 * h)] = v.y;
             }
             __syncthreads();
             constexpr int VEC = 16 / sizeof(T);
@@ -1269,11 +1259,7 @@ k_py_inv(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict_
         __syncthreads();
         V *out = s_out + cout;
 #pragma unroll
-        for (int t = 0; t < 16; ++t) {
-            V v = a[t];
-            v = cadd(v, shfl1(v));
-            if ((t >> 3) == h) out[M * t * TW] = v;
-        }
+        for (int s = 0; s < 8; ++s) out[M * (s + 8 * h) * TW] = half_sum(a, s, h);
         fence_async_smem();
         __syncthreads();
         if (tid == 0) {
@@ -1435,11 +1421,7 @@ k_py_inv8(const __grid_constant__ NmTensorMap tmB, typename VT<T>::V *__restrict
         if (tid == 0) bulk_wait_read<0>();                  // the previous tile has left s_out
         __syncthreads();
 #pragma unroll
-        for (int t = 0; t < 16; ++t) {
-            V v = a[t];
-            v = cadd(v, shfl1(v));
-            if ((t >> 3) == h) s_out[((t & 1) ? coutO : coutE) + M * t * TW] = v;
-        }
+        for (int s = 0; s < 8; ++s) s_out[((s & 1) ? coutO : coutE) + M * (s + 8 * h) * TW] = half_sum(a, s, h);
         fence_async_smem();
         __syncthreads();
         if (tid == 0) {

@@ -109,6 +109,15 @@ template <typename V> __device__ __forceinline__ V shfl1(V v)
     return r;
 }
 
+// Sum of the even and odd halves of output row t = s + 8 h (s = 0..7) of an inverse padded transform: the lane of half
+// h keeps the rows t = s + 8 h, sends its partner the value the partner keeps and adds the one it receives -- one
+// exchange per kept value (adding the halves of all 16 rows on both lanes and dropping eight costs two).
+template <typename V> __device__ __forceinline__ V half_sum(const V *a, int s, int h)
+{
+    const V give = h ? a[s] : a[s + 8], keep = h ? a[s + 8] : a[s];
+    return cadd(keep, shfl1(give));
+}
+
 // a * w (INV = false) or a * conj(w) (INV = true)
 template <bool INV, typename V> __device__ __forceinline__ V ctw(V a, V w)
 {

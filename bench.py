@@ -339,6 +339,20 @@ def _event_ms(fn, n, warm=5):
     return e0.elapsed_time(e1) / n
 
 
+def _wall_ms(fn, n, warm=3):
+    """Host wall clock per call, the stream drained on both sides (the paper's protocol: integration
+    wall time divided by the number of field evaluations)."""
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(n):
+        fn()
+    torch.cuda.synchronize()
+    return 1e3 * (time.perf_counter() - t0) / n
+
+
 def sweep_block(peak):
     """nm_llg_rhs (and the steps each config is stated with) at the other points of config 4 and at the
     film configs 1, 3, 5: ms per call by CUDA events after warm-up, Mcells/s, and the fraction of the
@@ -371,6 +385,8 @@ def sweep_block(peak):
                "mcells_per_s": cells / t_rhs / 1e3, "launches_per_rhs": per_rhs,
                "demag_path": mesh.nm_debug_demag_path(),
                "rk4_step_ms": _event_ms(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, y, z), max(3, reps // 2))}
+        # the paper's own protocol (Fig. 6): wall time of a fixed-step integration / field evaluations
+        row["paper_protocol_ms_per_eval"] = _wall_ms(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, y, z), max(5, reps)) / 4.0
         byts = sum(v for k, v in algorithmic_bytes(N1, N2, N3, s).items() if k not in ("node_rk", "node_adj"))
         row["algorithmic_bytes"] = byts
         row["frac"] = byts / (t_rhs * 1e-3) / 1e9 / peak
@@ -531,6 +547,7 @@ def run_b200(args):
     t_heff = over_ranks(timed(lambda: mesh.nm_heff(0.0, m, None, H), reps)) / reps
     t_rhs = over_ranks(timed(lambda: mesh.nm_llg_rhs(0.0, m, None, H), reps)) / reps
     t_rk4 = over_ranks(timed(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, m), reps)) / reps
+    t_paper = _wall_ms(lambda: mesh.nm_rk_step(nm.NM_RK4, 0.0, dt, m), reps) / 4.0
     t_adj = over_ranks(timed(lambda: nm._check(L.nm_llg_adjoint_rhs(
         mesh.handle, 0.0, vp(m.data_ptr()), vp(a.data_ptr()), None, vp(f_out.data_ptr()),
         vp(dadt.data_ptr()), vp(dudt.data_ptr()), nm._stream(local))), reps)) / reps
@@ -657,6 +674,7 @@ def run_b200(args):
         "breakdown": {"heff_ms": 1e3 * t_heff, "heff_mcells_per_s": cells / t_heff / 1e6,
                       "llg_rhs_ms": 1e3 * t_rhs, "llg_rhs_mcells_per_s": cells / t_rhs / 1e6,
                       "rk4_step_ms": 1e3 * t_rk4, "rk4_steps_per_s": 1.0 / t_rk4,
+                      "paper_protocol_ms_per_eval": t_paper,      # RK4 integration wall time / field evaluations
                       "adjoint_rhs_ms": 1e3 * t_adj,
                       "ms_per_step_without_kernel_events": 1e3 * sec_plain / args.steps},
     }

@@ -198,6 +198,28 @@ nm_status nm_adjoint_rk4_step_hext(nm_mesh *mesh, double t, double dt, void *m_i
                                    void *u_inout, double *u_h_inout, const nm_zeeman *zeeman,
                                    int renormalise, void *stream);
 
+/* The same uniform-field gradient for callers that cannot allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no nm_mesh and no workspace are needed, and the call makes no
+ * cudaMalloc / cudaFree and calls no allocating library routine.  Its per-block partial sums live in a
+ * file-scope device array of libnm.so (192 KB, held by every GPU that loads the library until the process exits),
+ * which limits the mesh to NM_NOALLOC_MAX_NODES nodes, (N1+1)(N2+1)(N3+1); more is NM_EINVAL.
+ *   device      the GPU the arrays live on (made current by the call); 0 <= device < 64
+ *   dtype       precision of m, a, Ms
+ *   n_cells     HOST, N1, N2, N3 >= 1 (3-D nodal basis)
+ *   m, a        DEVICE nodal 3-vector fields [3][N3+1][N2+1][N1+1]
+ *   Ms          DEVICE cell array [N3][N2][N1], or NULL = magnetic everywhere; a node counts if some cell that
+ *               contains it has Ms > 0 (reading C3(iii): nodes with (S Ms)_n = 0 see no field)
+ *   gamma, alpha  as in nm_mesh_desc
+ *   dudt_h_out  DEVICE fp64 [3], overwritten: - sum_{n: (S Ms)_n > 0} b_n,  b = g' m x a - alpha g' m x (m x a),
+ *               what nm_llg_adjoint_rhs_hext gives on a mesh with NM_TERM_ZEEMAN (fp64 sums in a fixed order)
+ * Enqueues two kernels on `stream`.  All calls on one device share the scratch array: it keeps the last call's
+ * partial sums, each call overwrites what it reads (nothing needs clearing), and calls that OVERLAP on the GPU
+ * (different streams without an ordering between them) race on it -- order them, or use the mesh entry point.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress); make it outside stream capture. */
+#define NM_NOALLOC_MAX_NODES (1ll << 25)
+nm_status nm_hext_gradient_noalloc(int device, nm_dtype dtype, const int *n_cells, const void *m, const void *a,
+                                   const void *Ms, double gamma, double alpha, double *dudt_h_out, void *stream);
+
 /* Gradients with respect to the cell-wise exchange constant A_c and anisotropy constant Ku_c (design
  * variables beside Ms).  f depends on them through H = -dE/L only, dE linear in
  * both (Eqs. 19-20, 22), so with b as above and bL = b / L (0 at nodes with L_n = 0), K and M the

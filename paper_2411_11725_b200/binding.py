@@ -27,7 +27,7 @@ EXPORTS = ("nm_mesh_query_workspace", "nm_mesh_create", "nm_mesh_set_Ms", "nm_me
            "nm_adjoint_rk4_step", "nm_adjoint_add_objective", "nm_llg_adjoint_rhs_hext", "nm_adjoint_rk4_step_hext",
            "nm_llg_adjoint_rhs_materials", "nm_adjoint_rk4_step_ex", "nm_llg_adjoint_rhs_hnodal", "nm_debug_get_tensor", "nm_debug_get_cell_field",
            "nm_launch_count", "nm_profile_dropped", "nm_debug_demag_path", "nm_profile_class_count", "nm_profile_class_name", "nm_profile_begin",
-           "nm_profile_end")
+           "nm_profile_end", "nm_hext_gradient_noalloc")
 
 
 class nm_mesh_desc(ctypes.Structure):
@@ -101,6 +101,7 @@ def lib():
         L.nm_adjoint_rk4_step_ex.argtypes = [vp, dbl, dbl, vp, vp, vp, ctypes.POINTER(nm_adjoint_extra),
                                              ctypes.POINTER(nm_zeeman), i32, vp]
         L.nm_adjoint_rk4_step_hext.argtypes = [vp, dbl, dbl, vp, vp, vp, vp, ctypes.POINTER(nm_zeeman), i32, vp]
+        L.nm_hext_gradient_noalloc.argtypes = [i32, i32, ctypes.POINTER(i32), vp, vp, vp, dbl, dbl, vp, vp]
         L.nm_debug_get_tensor.argtypes = [vp, vp]
         L.nm_debug_get_cell_field.argtypes = [vp, vp, vp]
         L.nm_launch_count.argtypes = [vp]
@@ -162,6 +163,23 @@ def make_desc(n_cells, cell_size, dtype, device, terms, gamma, alpha, ku_axis=(0
             setattr(d, name + "_scalar", float(v) if v is not None else 0.0)
     d._keep = keep
     return d
+
+
+NM_NOALLOC_MAX_NODES = 1 << 25
+
+
+def nm_hext_gradient_noalloc(n_cells, m, a, Ms=None, gamma=2.211e5, alpha=0.0, out=None):
+    """-(df/dh)^T a for a uniform external field without a mesh, a workspace or any allocation inside the library
+    (include/nm.h).  m, a: CUDA nodal fields in ABI order; Ms: CUDA cell array or None; out: CUDA fp64 [3] (made here
+    if None -- pass one to keep the call itself allocation-free)."""
+    if out is None:
+        out = torch.empty(3, dtype=torch.float64, device=m.device)
+    assert out.dtype == torch.float64 and out.numel() == 3 and out.is_cuda
+    dev = m.device.index if m.device.index is not None else torch.cuda.current_device()
+    n = (ctypes.c_int * 3)(*[int(v) for v in n_cells])
+    _check(lib().nm_hext_gradient_noalloc(dev, NM_F64 if m.dtype == torch.float64 else NM_F32, n, _ptr(m), _ptr(a),
+                                          _ptr(Ms), float(gamma), float(alpha), _ptr(out), _stream(dev)))
+    return out
 
 
 def nm_mesh_query_workspace(desc):

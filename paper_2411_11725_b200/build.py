@@ -12,7 +12,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnm.so")
-CU = ["nm_api.cu", "nm_local.cu", "nm_node_col.cu", "nm_demag.cu", "nm_demag_fast.cu", "nm_demag_pipe.cu", "nm_tensor.cu"]
+CU = ["nm_api.cu", "nm_local.cu", "nm_node_col.cu", "nm_demag.cu", "nm_demag_fast.cu", "nm_demag_pipe.cu", "nm_tensor.cu",
+      "nm_noalloc.cu"]
 CPP = ["nm_newell_host.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]

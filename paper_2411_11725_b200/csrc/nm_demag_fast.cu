@@ -41,7 +41,8 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
          const typename VT<T>::V *__restrict__ wP, int F3, int n2v)
 {
     typedef typename VT<T>::V V;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     constexpr int OUT_PITCH = LT * TW + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     V *s_io = reinterpret_cast<V *>(smem_raw);              // in: LT*N*8, out: P*OUT_PITCH
@@ -55,27 +56,28 @@ k_fy_fwd(const typename VT<T>::V *__restrict__ A, typename VT<T>::V *__restrict_
     __syncthreads();
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int h = lane & 1, i = lane >> 1;
-    const int l = i / M, j = i % M;
-    const int line = w * LT + l, sub = line / TW, k1 = line % TW;
+    const int l = G::R3 ? min(i / MI, 2) : i / MI, j = i % MI;       // (M = 12: l = the sub-sequence, lanes with i / MI = 3 idle)
+    const bool act = !G::R3 || i / MI < 3;
+    const int line = G::R3 ? w : w * LT + l, sub = line / TW, k1 = line % TW;
     V tw[16];
-    load_twiddles2<T, M>(tw, wP, j);
+    len_twiddles<T, M>(tw, wP, j);
     V a[16];
 #pragma unroll
     for (int t = 0; t < 16; ++t) {
-        const int e = j + M * t;
+        const int e = len_elem<M>(l, j, t);
         V v = s_io[(sub * N + e) * TW + (k1 ^ swzT<T>(e))];
         if (e >= n2v) v = mk<T>((T)0, (T)0);                // embedded mesh: rows the x pass never wrote
-        if (h) v = cmul(v, wP[e]);
+        if (h) v = cmul(v, wP[len_pre<M>(l, j, t)]);
         a[t] = v;
     }
     __syncthreads();   // the input tile is dead; s_io becomes the output tile
-    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
-    fft_fwd<T, M>(a, tw, scr, i);
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, MI>();
+    len_fwd<T, M>(a, tw, scr, i, wP, lane);
     const int sl = k1 ^ swzT<T>(c3_0 + sub);
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
-        const int ky = 2 * slot_freq<M>(j, s) + h;
-        s_io[ky * OUT_PITCH + sub * TW + (sl ^ swzT<T>(ky))] = a[s];
+        const int ky = len_freq<M>(l, j, s, h);
+        if (act) s_io[ky * OUT_PITCH + sub * TW + (sl ^ swzT<T>(ky))] = a[s];
     }
     __syncthreads();
     // rows of LT*8 complex, one per ky
@@ -93,7 +95,8 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
          const typename VT<T>::V *__restrict__ wP, int F3)
 {
     typedef typename VT<T>::V V;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     constexpr int PITCH = LT * TW + 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     V *s_io = reinterpret_cast<V *>(smem_raw);              // in: P*PITCH, out: LT*N*8
@@ -110,28 +113,29 @@ k_fy_inv(const typename VT<T>::V *__restrict__ B, typename VT<T>::V *__restrict_
     __syncthreads();
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int h = lane & 1, i = lane >> 1;
-    const int l = i / M, j = i % M;
-    const int line = w * LT + l, sub = line / TW, k1 = line % TW;
+    const int l = G::R3 ? min(i / MI, 2) : i / MI, j = i % MI;       // (M = 12: l = the sub-sequence, lanes with i / MI = 3 idle)
+    const bool act = !G::R3 || i / MI < 3;
+    const int line = G::R3 ? w : w * LT + l, sub = line / TW, k1 = line % TW;
     V tw[16];
-    load_twiddles2<T, M>(tw, wP, j);
+    len_twiddles<T, M>(tw, wP, j);
     V a[16];
     const int sl = k1 ^ swzT<T>(c3_0 + sub);
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
-        const int ky = 2 * slot_freq<M>(j, s) + h;
+        const int ky = len_freq<M>(l, j, s, h);
         a[s] = s_io[ky * PITCH + sub * TW + (sl ^ swzT<T>(ky))];
     }
     __syncthreads();
-    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
-    fft_inv<T, M>(a, tw, scr, i);
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, MI>();
+    len_inv<T, M>(a, tw, scr, i, wP, lane);
 #pragma unroll
     for (int t = 0; t < 16; ++t) {
-        const int e = j + M * t;
+        const int e = len_elem<M>(l, j, t);
         V v = a[t];
-        if (h) v = cmulc(v, wP[e]);
+        if (h) v = cmulc(v, wP[len_pre<M>(l, j, t)]);
         // sum of the even and odd halves: partner lane = lane ^ 1
         v = cadd(v, shfl1(v));
-        if ((t >> 3) == h) s_io[(sub * N + e) * TW + (k1 ^ swzT<T>(e))] = v;
+        if ((t >> 3) == h && act) s_io[(sub * N + e) * TW + (k1 ^ swzT<T>(e))] = v;
     }
     __syncthreads();
     V *dst = A + ((((long long)kt * 3 + comp) * N3 + c3_0) * N) * TW;
@@ -148,7 +152,8 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
          const typename VT<T>::V *__restrict__ wP, int n3v)
 {
     typedef typename VT<T>::V V;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     V *s_io = reinterpret_cast<V *>(smem_raw);              // LT*3*N*8
     V *s_scr = s_io + LT * 3 * N * TW;
@@ -167,11 +172,12 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     __syncthreads();
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int h = lane & 1, i = lane >> 1;
-    const int l = i / M, j = i % M;
-    const int line = w * LT + l, sub = line / TW, k1 = line % TW;
-    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
+    const int l = G::R3 ? min(i / MI, 2) : i / MI, j = i % MI;       // (M = 12: l = the sub-sequence, lanes with i / MI = 3 idle)
+    const bool act = !G::R3 || i / MI < 3;
+    const int line = G::R3 ? w : w * LT + l, sub = line / TW, k1 = line % TW;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, MI>();
     V tw[16];
-    load_twiddles2<T, M>(tw, wP, j);
+    len_twiddles<T, M>(tw, wP, j);
     V a[3][16];
     V *my = s_io + (sub * 3) * N * TW;
     const int kq = k1 ^ swzT<T>(ky0 + sub);                     // rows of B are swizzled by c3 and by ky
@@ -179,13 +185,13 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     for (int c = 0; c < 3; ++c) {
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
-            const int e = j + M * t;
+            const int e = len_elem<M>(l, j, t);
             V v = my[(c * N + e) * TW + (kq ^ swzT<T>(e))];
             if (EMB && e >= n3v) v = mk<T>((T)0, (T)0);     // embedded mesh: planes the y pass never wrote
-            if (h) v = cmul(v, wP[e]);
+            if (h) v = cmul(v, wP[len_pre<M>(l, j, t)]);
             a[c][t] = v;
         }
-        fft_fwd<T, M>(a[c], tw, scr, i);
+        len_fwd<T, M>(a[c], tw, scr, i, wP, lane);
     }
     // H^ = -N^ M^
     const int ky = ky0 + sub;
@@ -195,7 +201,7 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     const T *trow = Tn + ((((long long)kt * (N2 + 1) + kyf) * TW + k1) * 6) * Kzp;
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
-        const int kz = 2 * slot_freq<M>(j, s) + h;
+        const int kz = len_freq<M>(l, j, s, h);
         const int kzf = kz <= N ? kz : P - kz;
         const T sz = kz <= N ? (T)1 : (T)-1;
         const T *tp = trow + kzf;
@@ -211,14 +217,14 @@ k_fz_mid(typename VT<T>::V *__restrict__ B, const T *__restrict__ Tn, int N2, in
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        fft_inv<T, M>(a[c], tw, scr, i);
+        len_inv<T, M>(a[c], tw, scr, i, wP, lane);
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
-            const int e = j + M * t;
+            const int e = len_elem<M>(l, j, t);
             V v = a[c][t];
-            if (h) v = cmulc(v, wP[e]);
+            if (h) v = cmulc(v, wP[len_pre<M>(l, j, t)]);
             v = cadd(v, shfl1(v));
-            if ((t >> 3) == h) my[(c * N + e) * TW + (kq ^ swzT<T>(e))] = v;
+            if ((t >> 3) == h && act) my[(c * N + e) * TW + (kq ^ swzT<T>(e))] = v;
         }
     }
     __syncthreads();
@@ -234,22 +240,24 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
          int NKT, const typename VT<T>::V *__restrict__ wP)
 {
     typedef typename VT<T>::V V;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     const int W = blockDim.x >> 5;
     const int R = 2 * LT * W;
     constexpr int CP = N + 1;                               // cell row pitch (reals)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     V *s_z = reinterpret_cast<V *>(smem_raw);               // W*LT lines x P
     V *s_scr = s_z + W * LT * P;                            // 2 W teams
-    T *s_cell = reinterpret_cast<T *>(s_scr + 2 * W * team_scratch<T, M>());   // R x CP
+    T *s_cell = reinterpret_cast<T *>(s_scr + 2 * W * team_scratch<T, MI>());   // R x CP
     const int r0 = blockIdx.x * R, c3 = blockIdx.y;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int h = lane & 1, i = lane >> 1;
-    const int l = i / M, j = i % M;
-    const int line = w * LT + l;
-    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
+    const int l = G::R3 ? min(i / MI, 2) : i / MI, j = i % MI;
+    const bool act = !G::R3 || i / MI < 3;
+    const int line = G::R3 ? w : w * LT + l;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, MI>();
     V tw[16];
-    load_twiddles2<T, M>(tw, wP, j);
+    len_twiddles<T, M>(tw, wP, j);
     const long long plane = (long long)g.n1 * g.n2;
     // small grids: one component per CTA (gridDim.z = 3)
     for (int comp = gridDim.z == 3 ? (int)blockIdx.z : 0; comp < (gridDim.z == 3 ? (int)blockIdx.z + 1 : 3); ++comp) {
@@ -267,14 +275,15 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
         V a[16];
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
-            const int e = j + M * t;
+            const int e = len_elem<M>(l, j, t);
             V v = mk<T>(s_cell[(2 * line) * CP + e], s_cell[(2 * line + 1) * CP + e]);
-            if (h) v = cmul(v, wP[e]);
+            if (h) v = cmul(v, wP[len_pre<M>(l, j, t)]);
             a[t] = v;
         }
-        fft_fwd<T, M>(a, tw, scr, i);
+        len_fwd<T, M>(a, tw, scr, i, wP, lane);
 #pragma unroll
-        for (int s = 0; s < 16; ++s) s_z[line * P + 2 * slot_freq<M>(j, s) + h] = a[s];
+        for (int s = 0; s < 16; ++s)
+            if (act) s_z[line * P + len_freq<M>(l, j, s, h)] = a[s];
         __syncthreads();
         // untangle the two real rows of each line and store blocked, swizzled by c2
         for (int idx = threadIdx.x; idx < NKT * R * TW; idx += blockDim.x) {
@@ -285,7 +294,7 @@ k_fx_fwd(const T *__restrict__ fld, const T *__restrict__ Ms, typename VT<T>::V 
             V out = mk<T>((T)0, (T)0);
             if (k <= N) {
                 const V zk = s_z[(r >> 1) * P + k];
-                const V zm = s_z[(r >> 1) * P + ((P - k) & (P - 1))];
+                const V zm = s_z[(r >> 1) * P + (k ? P - k : 0)];
                 if (r & 1) out = mk<T>((T)0.5 * (zk.y + zm.y), (T)-0.5 * (zk.x - zm.x));
                 else out = mk<T>((T)0.5 * (zk.x + zm.x), (T)0.5 * (zk.y - zm.y));
             }
@@ -303,7 +312,8 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
          const typename VT<T>::V *__restrict__ wP)
 {
     typedef typename VT<T>::V V;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     const int W = blockDim.x >> 5;
     const int R = 2 * LT * W;
     const int XP = NKT * TW + 1;                            // row pitch of s_x (complex)
@@ -313,11 +323,12 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
     const int r0 = blockIdx.x * R, c3 = blockIdx.y;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int h = lane & 1, i = lane >> 1;
-    const int l = i / M, j = i % M;
-    const int line = w * LT + l;
-    V *scr = s_scr + (2 * w + h) * team_scratch<T, M>();
+    const int l = G::R3 ? min(i / MI, 2) : i / MI, j = i % MI;
+    const bool act = !G::R3 || i / MI < 3;
+    const int line = G::R3 ? w : w * LT + l;
+    V *scr = s_scr + (2 * w + h) * team_scratch<T, MI>();
     V tw[16];
-    load_twiddles2<T, M>(tw, wP, j);
+    len_twiddles<T, M>(tw, wP, j);
     // small grids: one component per CTA (gridDim.z = 3)
     for (int comp = gridDim.z == 3 ? (int)blockIdx.z : 0; comp < (gridDim.z == 3 ? (int)blockIdx.z + 1 : 3); ++comp) {
         for (int idx = threadIdx.x; idx < NKT * R * TW; idx += blockDim.x) {
@@ -332,7 +343,7 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
         const V *xa = s_x + (2 * line) * XP, *xb = xa + XP;
 #pragma unroll
         for (int s = 0; s < 16; ++s) {
-            const int k = 2 * slot_freq<M>(j, s) + h;
+            const int k = len_freq<M>(l, j, s, h);
             if (k <= N) {
                 const V u = xa[k], v = xb[k];
                 a[s] = mk<T>(u.x - v.y, u.y + v.x);          // Xa + i Xb
@@ -341,15 +352,15 @@ k_fx_inv(const typename VT<T>::V *__restrict__ A, T *__restrict__ Hc, NmGeom g, 
                 a[s] = mk<T>(u.x + v.y, v.x - u.y);          // conj(Xa) + i conj(Xb)
             }
         }
-        fft_inv<T, M>(a, tw, scr, i);
+        len_inv<T, M>(a, tw, scr, i, wP, lane);
         T *ha = Hc + (long long)comp * g.cells + ((long long)c3 * g.N2 + r0 + 2 * line) * g.N1;
 #pragma unroll
         for (int t = 0; t < 16; ++t) {
-            const int e = j + M * t;
+            const int e = len_elem<M>(l, j, t);
             V v = a[t];
-            if (h) v = cmulc(v, wP[e]);
+            if (h) v = cmulc(v, wP[len_pre<M>(l, j, t)]);
             v = cadd(v, shfl1(v));
-            if ((t >> 3) == h) {
+            if ((t >> 3) == h && act) {
                 ha[e] = v.x;
                 ha[g.N1 + e] = v.y;
             }
@@ -377,7 +388,8 @@ nm_status launch_x(nm_mesh *mesh, bool inverse, const T *fld, T *Hc, cudaStream_
     typedef typename VT<T>::V V;
     const NmGeom &g = mesh->g;
     const NmFast &f = mesh->fast;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     const int W = f.Wx, R = 2 * LT * W;
     const bool split = (long long)(g.N2 / R) * g.N3 < 2LL * mesh->sm_count;
     const dim3 grid(g.N2 / R, g.N3, split ? 3 : 1);
@@ -401,7 +413,8 @@ nm_status launch_y(nm_mesh *mesh, bool inverse, int kt0, int nkt, cudaStream_t s
 {
     typedef typename VT<T>::V V;
     const NmGeom &g = mesh->g;
-    constexpr int N = 16 * M, P = 2 * N, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, P = G::P, LT = G::LT, MI = G::MI;
     if (nm_pipe_y_ok(mesh)) return nm_pipe_y(mesh, inverse, kt0, nkt, st);
     const size_t sm = (size_t)P * (LT * TW + 1) * sizeof(V) + scratch_bytes<T>(kWarps);
     const dim3 grid(g.N3 / LT, 3, nkt);
@@ -424,7 +437,8 @@ nm_status launch_z(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
 {
     typedef typename VT<T>::V V;
     const NmGeom &g = mesh->g;
-    constexpr int N = 16 * M, LT = 16 / M;
+    typedef Len<M> G;
+    constexpr int N = G::N, LT = G::LT;
     if (nm_pipe_mid_ok(mesh)) return nm_pipe_mid(mesh, kt0, nkt, st);
     const size_t sm = (size_t)LT * 3 * N * TW * sizeof(V) + scratch_bytes<T>(kWarps);
     const dim3 grid(g.P2 / LT, nkt);
@@ -447,6 +461,7 @@ nm_status launch_z(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
     case 2: { constexpr int MM = 2; NM_TRY(CALL); } break;                                             \
     case 4: { constexpr int MM = 4; NM_TRY(CALL); } break;                                             \
     case 8: { constexpr int MM = 8; NM_TRY(CALL); } break;                                             \
+    case 12: { constexpr int MM = 12; NM_TRY(CALL); } break;                                           \
     default: { constexpr int MM = 16; NM_TRY(CALL); } break;                                           \
     }
 
@@ -493,10 +508,14 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
         if (N[a] > 256) return;
         F[a] = 16;
         while (F[a] < N[a]) F[a] *= 2;
+        if (N[a] == 192) F[a] = 192;                 // 3 x 64: the radix-3 form of the register core (Len<12>)
         if (F[a] != N[a]) exact = false;
         M[a] = F[a] / 16;
     }
-    const int LTx = 16 / M[0];
+    if (!exact)                                      // embedded meshes know the sizes 16 * 2^k only
+        for (int a = 0; a < 3; ++a)
+            if (F[a] == 192) { F[a] = 256; M[a] = 16; }
+    const int LTx = M[0] == 12 ? 1 : 16 / M[0];
     if (!exact) {
         const int vec = d->dtype == NM_F64 ? 2 : 4;
         if (N[0] < 2 || N[1] < 2 || N[2] < 2) return;                           // films and rods: the 2-D / 1-D general path
@@ -514,7 +533,7 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
         const bool piped = d->dtype != NM_F64 || ((F[1] == 256 || F[1] == 128) && (F[2] == 256 || F[2] == 128));
         if (smooth && fill < (piped ? 2 : 3) * plane) return;
         if (N[1] % (2 * 8 * LTx) != 0 || N[0] % vec != 0) return;              // whole x-pass CTAs of rows, 16-byte cell rows
-        if (N[2] % (16 / M[1]) != 0) return;                                   // whole y-pass CTAs of planes
+        if (N[2] % (16 / M[1]) != 0) return;                                   // whole y-pass CTAs of planes (M = 12 never gets here)
         if (d->dtype == NM_F64 && M[0] == 1) return;                           // no staged fp64 x pass at N1 = 16
         f->embed = true;
     }

@@ -1552,6 +1552,7 @@ template <typename T, int M> nm_status launch_px(nm_mesh *mesh, bool inverse, co
 bool nm_pipe_x_ok(const nm_mesh *mesh)
 {
     if (!mesh->fast.on || !mesh->fast.pipe) return false;
+    if (mesh->fast.M1 == 12) return false;                  // N1 = 192: k_fx_fwd / k_fx_inv (Len<12>)
     const int R = 2 * 8 * (16 / mesh->fast.M1);
     if (mesh->f64 && mesh->fast.M1 == 1) return false;      // the staged inverse would need more than 227 KB
     return mesh->g.N2 % R == 0;

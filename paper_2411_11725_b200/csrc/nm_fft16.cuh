@@ -511,4 +511,102 @@ __device__ __forceinline__ void inv_get_s(typename VT<T>::V *a, const typename V
     }
 }
 
+// ---- lengths by template parameter M ------------------------------------------------------------------------
+// M in {1, 2, 4, 8, 16}: N = 16 M, one team = 16 / M lines.  M = 12: N = 192 = 3 x 64, a radix-3 step on top of the
+// M = 4 core: the line is split into its three decimated sub-sequences x_r[n'] = x[3 n' + r], which are three of the
+// four lines of an M = 4 team (team thread i = 4 l + j: l = r, l = 3 idles); with G_r the padded 128-point transform
+// of x_r,
+//     X[k' + 128 s] = sum_r w_3^(r s) (w_384^(r k') G_r[k']),   k' < 128, s = 0, 1, 2,
+// and the thread of sub-sequence l ends up with the outputs s = l of its slots (three lane exchanges per slot).
+// The cropped inverse runs the same steps backwards.  wP is the table exp(-2 pi i q / P), P = 2 N, throughout.
+template <int M> struct Len {
+    static constexpr int N = 16 * M, P = 2 * N, MI = M, LT = 16 / M;
+    static constexpr bool R3 = false;
+};
+template <> struct Len<12> {
+    static constexpr int N = 192, P = 384, MI = 4, LT = 1;
+    static constexpr bool R3 = true;
+};
+
+// element held in register t of team thread (l, j) on the data side
+template <int M> __device__ __forceinline__ int len_elem(int l, int j, int t)
+{
+    return Len<M>::R3 ? 3 * (j + Len<M>::MI * t) + l : j + M * t;
+}
+// index into wP of the odd half's pre-twiddle of that element: w_P'^(n') of the transform the core runs
+template <int M> __device__ __forceinline__ int len_pre(int l, int j, int t)
+{
+    return Len<M>::R3 ? 3 * (j + Len<M>::MI * t) : j + M * t;
+}
+// frequency (0..P-1) held in slot s of team thread (l, j), half h, on the spectral side
+template <int M> __device__ __forceinline__ int len_freq(int l, int j, int s, int h)
+{
+    return 2 * slot_freq<Len<M>::MI>(j, s) + h + (Len<M>::R3 ? 128 * l : 0);
+}
+template <typename T, int M>
+__device__ __forceinline__ void len_twiddles(typename VT<T>::V *tw, const typename VT<T>::V *__restrict__ wP, int j)
+{
+    if (Len<M>::R3) {
+#pragma unroll
+        for (int t = 1; t < 16; ++t) tw[t] = wP[(6 * j * t) % 384];         // w_64^(j t)
+    } else {
+        load_twiddles2<T, Len<M>::MI>(tw, wP, j);
+    }
+}
+
+// the value slot holds in the thread of sub-sequence r of the same (j, h): lane = 8 l + 2 j + h
+template <typename V> __device__ __forceinline__ V shfl_sub(V v, int lane, int r)
+{
+    V o;
+    o.x = __shfl_sync(0xffffffffu, v.x, (lane & 7) + 8 * r);
+    o.y = __shfl_sync(0xffffffffu, v.y, (lane & 7) + 8 * r);
+    return o;
+}
+
+// X_l = T_0 + w^l T_1 + w^(2l) T_2 with w = exp(-+ 2 pi i / 3) (forward / INV), for the thread's own l
+template <typename T, bool INV, typename V> __device__ __forceinline__ V dft3_own(V t0, V t1, V t2, int l)
+{
+    const V sm = cadd(t1, t2), df = csub(t1, t2);
+    const T hs = (T)0.86602540378443864676372317075294;
+    // l = 0: t0 + sm;  l = 1, 2: t0 - sm / 2 -+ i hs df (forward: l = 1 takes -i), inverse the other way round
+    const T cs = l == 0 ? (T)1 : (T)-0.5;
+    T g = l == 0 ? (T)0 : (l == 1 ? -hs : hs);
+    if (INV) g = -g;
+    return mk<T>(t0.x + cs * sm.x - g * df.y, t0.y + cs * sm.y + g * df.x);
+}
+
+template <typename T, int M>
+__device__ __forceinline__ void len_fwd(typename VT<T>::V *a, const typename VT<T>::V *tw, typename VT<T>::V *scr, int i,
+                                        const typename VT<T>::V *__restrict__ wP, int lane)
+{
+    typedef typename VT<T>::V V;
+    fft_fwd<T, Len<M>::MI>(a, tw, scr, i);
+    if (Len<M>::R3) {
+        const int l = min(i >> 2, 2), j = i & 3, h = lane & 1;
+#pragma unroll
+        for (int s = 0; s < 16; ++s) {
+            const int kp = 2 * slot_freq<4>(j, s) + h;
+            const V v = l ? cmul(a[s], wP[l * kp]) : a[s];
+            a[s] = dft3_own<T, false>(shfl_sub(v, lane, 0), shfl_sub(v, lane, 1), shfl_sub(v, lane, 2), l);
+        }
+    }
+}
+
+template <typename T, int M>
+__device__ __forceinline__ void len_inv(typename VT<T>::V *a, const typename VT<T>::V *tw, typename VT<T>::V *scr, int i,
+                                        const typename VT<T>::V *__restrict__ wP, int lane)
+{
+    typedef typename VT<T>::V V;
+    if (Len<M>::R3) {
+        const int l = min(i >> 2, 2), j = i & 3, h = lane & 1;
+#pragma unroll
+        for (int s = 0; s < 16; ++s) {
+            const int kp = 2 * slot_freq<4>(j, s) + h;
+            const V y = dft3_own<T, true>(shfl_sub(a[s], lane, 0), shfl_sub(a[s], lane, 1), shfl_sub(a[s], lane, 2), l);
+            a[s] = l ? cmulc(y, wP[l * kp]) : y;
+        }
+    }
+    fft_inv<T, Len<M>::MI>(a, tw, scr, i);
+}
+
 } // namespace nmf

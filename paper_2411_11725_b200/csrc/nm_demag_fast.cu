@@ -12,6 +12,8 @@
 //   * the tensor is stored as T[kt][|ky|][k1][6][|kz|] and read coalesced along kz.
 // Passes: k_fx_fwd (avg * Ms, x R2C) -> k_fy_fwd -> k_fz_mid (z fwd, H^ = -N^ M^, z inv) ->
 // k_fy_inv -> k_fx_inv (C2R, crop) -> Hc[3][N3][N2][N1] for the node kernel.
+#include <cstdlib>
+
 #include "nm_fft16.cuh"
 #include "nm_internal.h"
 
@@ -503,12 +505,18 @@ void nm_fast_plan(const nm_mesh_desc *d, const NmGeom &g, NmFast *f)
     if (!(d->terms & NM_TERM_DEMAG)) return;
     int M[3], F[3];
     const int N[3] = {g.N1, g.N2, g.N3};
+    // NM_FAST192=1 (read at nm_mesh_create): an axis of 192 cells is transformed at its own length (Len<12>, nm_fft16.cuh:
+    // 192 = 3 x 64) instead of zero-extended to 256.  Off by default: measured slower (profiles/r2_final.md) -- the
+    // 192-cell forms exist for the one-CTA-per-tile kernels k_fx_* / k_fy_* and for the z pass (k_pz_mid3) only, and
+    // the persistent pipelines at 256 cells make up for 2.4 times the work.
+    const char *e192 = getenv("NM_FAST192");
+    const bool native192 = e192 && e192[0] == '1';
     bool exact = true;
     for (int a = 0; a < 3; ++a) {
         if (N[a] > 256) return;
         F[a] = 16;
         while (F[a] < N[a]) F[a] *= 2;
-        if (N[a] == 192) F[a] = 192;                 // 3 x 64: the radix-3 form of the register core (Len<12>)
+        if (N[a] == 192 && native192) F[a] = 192;    // 3 x 64: the radix-3 form of the register core (Len<12>)
         if (F[a] != N[a]) exact = false;
         M[a] = F[a] / 16;
     }

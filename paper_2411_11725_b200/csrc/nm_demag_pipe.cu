@@ -234,6 +234,219 @@ k_pz_mid(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItem
 }
 
 
+// ---- z pass, 192 cells along z -----------------------------------------------------------------------
+// k_pz_mid for N3 = 192 = 3 x 64 (Len<12>, nm_fft16.cuh): the same pipeline (copy warp, three-deep tile ring,
+// per-warp tensor slices); a warp still owns one k1 column, its lanes are (l, j, h) = (sub-sequence, thread of the
+// M = 4 team, half), lanes with l = 3 idle; the radix-3 step sits between the 64-point transforms and the tensor
+// product, two lane exchanges per slot.
+struct Pz3Smem {
+    static constexpr int N = 192;
+    static constexpr int TILE_ELEMS = 3 * N * TW;                   // complex
+    static constexpr int TILE_BYTES = TILE_ELEMS * 8;               // 36864
+    static constexpr int NBUF = 4;
+    static constexpr int KZP = 194;                                 // tensor |kz| pitch (reals), even
+    static constexpr int TSLICE = 6 * KZP;                          // reals per warp (4656 B, one bulk copy)
+    static constexpr int WSCR = 2 * Team<4>::SCRATCH - 8;
+    static constexpr int OFF_T = NBUF * TILE_BYTES;
+    static constexpr int OFF_SCR = OFF_T + 8 * TSLICE * 4;
+    static constexpr int OFF_BAR = OFF_SCR + 8 * WSCR * 8;
+    static constexpr int BYTES = OFF_BAR + (2 * NBUF + 8) * 8;
+};
+static_assert(Pz3Smem::BYTES <= 227 * 1024, "k_pz_mid3 shared memory exceeds the sm_100a per-CTA limit");
+
+template <bool EMB>
+__global__ void __launch_bounds__(kMidThreads, 1)
+k_pz_mid3(float2 *__restrict__ B, const float *__restrict__ Tn, int N2, int nItems, int kt0,
+          const float2 *__restrict__ wP, int n3v)
+{
+    typedef float T;
+    typedef float2 V;
+    typedef Pz3Smem S;
+    constexpr int MI = 4, N = 192, P = 384;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    V *s_B = reinterpret_cast<V *>(smem);
+    T *s_T = reinterpret_cast<T *>(smem + S::OFF_T);
+    V *s_scr = reinterpret_cast<V *>(smem + S::OFF_SCR);
+    uint64_t *fullB = reinterpret_cast<uint64_t *>(smem + S::OFF_BAR);
+    uint64_t *doneB = fullB + S::NBUF;
+    uint64_t *fullT = doneB + S::NBUF;
+
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int h = lane & 1, i = lane >> 1, j = i & 3, l = min(i >> 2, 2);
+    const bool act = (i >> 2) < 3;
+    const int P2 = 2 * N2, K2 = N2 + 1;
+    const int G = gridDim.x;
+
+    if (tid == 0) {
+        for (int q = 0; q < S::NBUF; ++q) {
+            mbar_init(fullB + q, 1);
+            mbar_init(doneB + q, 8);
+        }
+        for (int q = 0; q < 8; ++q) mbar_init(fullT + q, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto tile_ptr = [&](int g, int sub) -> V * {
+        const int kyf = g % K2, ktl = g / K2;
+        const int ky = sub ? P2 - kyf : kyf;
+        return B + ((long long)ktl * P2 + ky) * S::TILE_ELEMS;
+    };
+    auto n_tiles = [&](int g) -> int {
+        const int kyf = g % K2;
+        return (kyf == 0 || kyf == N2) ? 1 : 2;
+    };
+    auto load_tensor = [&](int g) {
+        const int kyf = g % K2, kt = kt0 + g / K2;
+        const T *src = Tn + (((long long)kt * K2 + kyf) * TW + w) * S::TSLICE;
+        mbar_expect_tx(fullT + w, S::TSLICE * 4);
+        bulk_load(s_T + w * S::TSLICE, src, S::TSLICE * 4, fullT + w);
+    };
+
+    if (w == 8) {           // copy warp, as in k_pz_mid
+        if (lane != 0) return;
+        int pg = blockIdx.x, psub = 0;
+        for (int q = 0; q < S::NBUF; ++q) {
+            if (pg < nItems) {
+                mbar_expect_tx(fullB + q, S::TILE_BYTES);
+                bulk_load(s_B + q * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + q);
+                if (psub + 1 < n_tiles(pg)) ++psub;
+                else { pg += G; psub = 0; }
+            }
+        }
+        int n = 0;
+        for (int g = blockIdx.x; g < nItems; g += G) {
+            const int nt = n_tiles(g);
+            for (int sub = 0; sub < nt; ++sub, ++n) {
+                const int b = n % S::NBUF;
+                mbar_wait_idle(doneB + b, (uint32_t)((n / S::NBUF) & 1));
+                bulk_store(tile_ptr(g, sub), s_B + b * S::TILE_ELEMS, S::TILE_BYTES);
+                bulk_commit();
+                bulk_wait_read<0>();
+                if (pg < nItems) {
+                    mbar_expect_tx(fullB + b, S::TILE_BYTES);
+                    bulk_load(s_B + b * S::TILE_ELEMS, tile_ptr(pg, psub), S::TILE_BYTES, fullB + b);
+                    if (psub + 1 < n_tiles(pg)) ++psub;
+                    else { pg += G; psub = 0; }
+                }
+            }
+        }
+        bulk_wait<0>();
+        return;
+    }
+    if (lane == 0 && (int)blockIdx.x < nItems) load_tensor(blockIdx.x);
+
+    // stage twiddles of the 64-point transforms in the TW0 form with the slot-position part of the radix-3 twiddle
+    // folded in, w_384^((3 j + l)(2 t' + h)), and the rest of that twiddle, w_12^(l p) (r3_fwd); wP = exp(-2 pi i q / 384)
+    V tw[16], tw3[3];
+#pragma unroll
+    for (int t = 0; t < 16; ++t) tw[t] = wP[(3 * j + l) * (2 * t + h)];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) tw3[q] = wP[32 * l * (q + 1)];
+    V *scr = s_scr + w * S::WSCR + h * Team<MI>::SCRATCH;
+    const T *ts = s_T + w * S::TSLICE;
+    int n = 0;
+    uint32_t tphase = 0;
+
+    for (int g = blockIdx.x; g < nItems; g += G) {
+        const int kyf = g % K2;
+        const int nt = (kyf == 0 || kyf == N2) ? 1 : 2;
+        for (int sub = 0; sub < nt; ++sub, ++n) {
+            const int b = n % S::NBUF;
+            mbar_wait(fullB + b, (uint32_t)((n / S::NBUF) & 1));
+            const int cw = w ^ swz(sub ? P2 - kyf : kyf);        // rows of B are swizzled by c3 and by ky
+            V *tile = s_B + b * S::TILE_ELEMS;
+            V a[3][16];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int t = 0; t < 16; ++t) {
+                    const int e = 3 * (j + MI * t) + l;
+                    a[c][t] = tile[(c * N + e) * TW + (cw ^ swz(e))];
+                    if (EMB && e >= n3v) a[c][t] = mk<T>((T)0, (T)0);
+                }
+            }
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, false>(a[c]);
+            }
+            dft16<T, false>(a[0]);
+            fwd_put<T, MI, true>(a[0], tw, scr, i);
+            dft16<T, false>(a[1]);
+            fwd_get<T, MI>(a[0], scr, i);
+            dft16<T, false>(a[2]);
+            fwd_put<T, MI, true>(a[1], tw, scr, i);
+            dftM<T, false, MI>(a[0]);
+            fwd_get<T, MI>(a[1], scr, i);
+            fwd_put<T, MI, true>(a[2], tw, scr, i);
+            dftM<T, false, MI>(a[1]);
+            r3_fwd<T>(a[0], tw3, lane, l);
+            fwd_get<T, MI>(a[2], scr, i);
+            dftM<T, false, MI>(a[2]);
+            r3_fwd<T>(a[1], tw3, lane, l);
+            r3_fwd<T>(a[2], tw3, lane, l);
+            if (sub == 0) {
+                mbar_wait(fullT + w, tphase);
+                tphase ^= 1;
+            }
+            const T sy = sub ? (T)-1 : (T)1;
+#pragma unroll
+            for (int s = 0; s < 16; ++s) {
+                const int kz = 2 * slot_freq<MI>(j, s) + h + 128 * l;
+                const bool up = kz > N;
+                const int kzf = up ? P - kz : kz;
+                const T sz = up ? (T)-1 : (T)1;
+                const T *tp = ts + kzf;
+                const T nxx = tp[0], nyy = tp[S::KZP], nzz = tp[2 * S::KZP];
+                const T nxy = sy * tp[3 * S::KZP], nxz = sz * tp[4 * S::KZP], nyz = sy * sz * tp[5 * S::KZP];
+                const V mx = a[0][s], my_ = a[1][s], mz = a[2][s];
+                const V hx = caxpy(nxz, mz, caxpy(nxy, my_, cscale(nxx, mx)));
+                const V hy = caxpy(nyz, mz, caxpy(nyy, my_, cscale(nxy, mx)));
+                const V hz = caxpy(nzz, mz, caxpy(nyz, my_, cscale(nxz, mx)));
+                a[0][s] = mk<T>(-hx.x, -hx.y);
+                a[1][s] = mk<T>(-hy.x, -hy.y);
+                a[2][s] = mk<T>(-hz.x, -hz.y);
+            }
+            if (sub == nt - 1) {
+                __syncwarp();
+                if (lane == 0 && g + G < nItems) load_tensor(g + G);
+            }
+            r3_inv<T>(a[0], tw3, lane, l);
+            dftM<T, true, MI>(a[0]);
+            inv_put<T, MI>(a[0], scr, i);
+            r3_inv<T>(a[1], tw3, lane, l);
+            dftM<T, true, MI>(a[1]);
+            inv_get<T, MI, true>(a[0], tw, scr, i);
+            r3_inv<T>(a[2], tw3, lane, l);
+            dftM<T, true, MI>(a[2]);
+            inv_put<T, MI>(a[1], scr, i);
+            dft16<T, true>(a[0]);
+            inv_get<T, MI, true>(a[1], tw, scr, i);
+            inv_put<T, MI>(a[2], scr, i);
+            dft16<T, true>(a[1]);
+            inv_get<T, MI, true>(a[2], tw, scr, i);
+            dft16<T, true>(a[2]);
+            if (h) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) shift32<T, true>(a[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int s = 0; s < 8; ++s) {
+                    const int e = 3 * (j + MI * (s + 8 * h)) + l;
+                    const V v = half_sum(a[c], s, h);
+                    if (act) tile[(c * N + e) * TW + (cw ^ swz(e))] = v;
+                }
+            }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(doneB + b);
+        }
+    }
+}
+
+
 // ---- z pass, 128 cells along z ---------------------------------------------------------------------
 // The same pipeline for N3 = 128 (M = 8): a team transforms two lines at once, so a warp owns two
 // columns of a tile and four warps a whole tile; warps 0-3 take the +ky tile of an item and warps
@@ -1441,6 +1654,7 @@ bool nm_pipe_mid_ok(const nm_mesh *mesh)
 {
     if (!mesh->fast.on || !mesh->fast.pipe) return false;
     if (mesh->f64) return (mesh->fast.M3 == 16 && mesh->fast.Kzp == Pz64Smem::KZP) || (mesh->fast.M3 == 8 && mesh->fast.Kzp == Pz64Smem8::KZP);
+    if (mesh->fast.M3 == 12) return mesh->fast.Kzp == Pz3Smem::KZP;
     return (mesh->fast.M3 == 16 && mesh->fast.Kzp == PzSmem::KZP) || (mesh->fast.M3 == 8 && mesh->fast.Kzp == Pz8Smem::KZP);
 }
 
@@ -1468,6 +1682,17 @@ nm_status nm_pipe_mid(nm_mesh *mesh, int kt0, int nkt, cudaStream_t st)
             return NM_OK;
         };
         NM_TRY(mesh->fast.embed ? go(k_pz_mid64<true>) : go(k_pz_mid64<false>));
+        return NM_OK;
+    }
+    if (mesh->fast.M3 == 12) {
+        auto go = [&](auto kern) -> nm_status {
+            NM_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Pz3Smem::BYTES));
+            kern<<<grid, kMidThreads, Pz3Smem::BYTES, st>>>((float2 *)mesh->bufB, (const float *)mesh->fast.Tn, mesh->fast.F2,
+                                                            nItems, kt0, (const float2 *)mesh->tw_z, g.N3);
+            return NM_OK;
+        };
+        NM_TRY(mesh->fast.embed ? go(k_pz_mid3<true>) : go(k_pz_mid3<false>));
+        NM_CUDA_TRY(cudaGetLastError());
         return NM_OK;
     }
     if (mesh->fast.M3 == 8) {

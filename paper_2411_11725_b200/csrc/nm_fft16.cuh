@@ -572,7 +572,8 @@ template <typename T, bool INV, typename V> __device__ __forceinline__ V dft3_ow
     const T cs = l == 0 ? (T)1 : (T)-0.5;
     T g = l == 0 ? (T)0 : (l == 1 ? -hs : hs);
     if (INV) g = -g;
-    return mk<T>(t0.x + cs * sm.x - g * df.y, t0.y + cs * sm.y + g * df.x);
+    // (re, im) = t0 + cs sm + g (-df.y, df.x): two packed multiply-adds
+    return pfma(mk<T>(df.y, df.x), mk<T>(-g, g), pfma(sm, mk<T>(cs, cs), t0));
 }
 
 template <typename T, int M>
@@ -586,7 +587,7 @@ __device__ __forceinline__ void len_fwd(typename VT<T>::V *a, const typename VT<
 #pragma unroll
         for (int s = 0; s < 16; ++s) {
             const int kp = 2 * slot_freq<4>(j, s) + h;
-            const V v = l ? cmul(a[s], wP[l * kp]) : a[s];
+            const V v = cmul(a[s], wP[l * kp]);
             a[s] = dft3_own<T, false>(shfl_sub(v, lane, 0), shfl_sub(v, lane, 1), shfl_sub(v, lane, 2), l);
         }
     }
@@ -603,10 +604,48 @@ __device__ __forceinline__ void len_inv(typename VT<T>::V *a, const typename VT<
         for (int s = 0; s < 16; ++s) {
             const int kp = 2 * slot_freq<4>(j, s) + h;
             const V y = dft3_own<T, true>(shfl_sub(a[s], lane, 0), shfl_sub(a[s], lane, 1), shfl_sub(a[s], lane, 2), l);
-            a[s] = l ? cmulc(y, wP[l * kp]) : y;
+            a[s] = cmulc(y, wP[l * kp]);
         }
     }
     fft_inv<T, Len<M>::MI>(a, tw, scr, i);
+}
+
+// The radix-3 step of Len<12> with two lane exchanges per slot (the pipelined 192-cell kernels): a thread keeps its
+// own value and fetches those of the sub-sequences l + 1 and l + 2 (mod 3); `lane` = 8 l + 2 j + h, l = min(i / 4, 2).
+template <typename T, bool INV>
+__device__ __forceinline__ typename VT<T>::V r3_gather(typename VT<T>::V own, int lane, int l)
+{
+    typedef typename VT<T>::V V;
+    const int la = (lane & 7) + 8 * (l == 2 ? 0 : l + 1), lb = (lane & 7) + 8 * (l == 0 ? 2 : l - 1);
+    V A, B;                                                     // values of sub-sequences l + 1 and l + 2
+    A.x = __shfl_sync(0xffffffffu, own.x, la);
+    A.y = __shfl_sync(0xffffffffu, own.y, la);
+    B.x = __shfl_sync(0xffffffffu, own.x, lb);
+    B.y = __shfl_sync(0xffffffffu, own.y, lb);
+    // (t0, t1, t2) = l = 0: (own, A, B); l = 1: (B, own, A); l = 2: (A, B, own) -- scalar selects, no branches
+    const bool p0 = l == 0, p1 = l == 1;
+    const V t0 = mk<T>(p0 ? own.x : (p1 ? B.x : A.x), p0 ? own.y : (p1 ? B.y : A.y));
+    const V t1 = mk<T>(p0 ? A.x : (p1 ? own.x : B.x), p0 ? A.y : (p1 ? own.y : B.y));
+    const V t2 = mk<T>(p0 ? B.x : (p1 ? A.x : own.x), p0 ? B.y : (p1 ? A.y : own.y));
+    return dft3_own<T, INV>(t0, t1, t2, l);
+}
+// The twiddle w_384^(l k') of slot s = 4 u + p, k' = 8 j + 2 u + 32 p + h, factors into w^(l (2 t' + h)), t' = 4 j + u
+// the position the value had in the exchange -- which the caller folds into its stage twiddles,
+// tw[t'] = w_384^((3 j + l)(2 t' + h)) -- and bc[p - 1] = w_12^(l p), applied here (12 products per transform).
+template <typename T>
+__device__ __forceinline__ void r3_fwd(typename VT<T>::V *a, const typename VT<T>::V *bc, int lane, int l)
+{
+#pragma unroll
+    for (int s = 0; s < 16; ++s) a[s] = r3_gather<T, false>((s & 3) ? cmul(a[s], bc[(s & 3) - 1]) : a[s], lane, l);
+}
+template <typename T>
+__device__ __forceinline__ void r3_inv(typename VT<T>::V *a, const typename VT<T>::V *bc, int lane, int l)
+{
+#pragma unroll
+    for (int s = 0; s < 16; ++s) {
+        const typename VT<T>::V y = r3_gather<T, true>(a[s], lane, l);
+        a[s] = (s & 3) ? cmulc(y, bc[(s & 3) - 1]) : y;
+    }
 }
 
 } // namespace nmf

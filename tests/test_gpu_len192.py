@@ -44,3 +44,25 @@ def test_native_192_axis_against_the_oracle(n, prec, monkeypatch):
     other = gpu_mesh(w, td)
     assert other.nm_debug_demag_path() in (0, 2)        # zero-extended to 256 (or the general path)
     assert_parity(host(other.nm_heff(0.0, dev(m, td))), ref_H, TOL[prec], "H, default")
+
+
+@pytest.mark.parametrize("n,prec", [((192, 32, 32), "f32"), ((32, 192, 32), "f32"), ((32, 32, 192), "f32"),
+                                    ((32, 32, 192), "f64"), ((192, 192, 32), "f64")])
+def test_native_192_guard_bands_and_run_to_run_identity(n, prec, monkeypatch):
+    """The checks of tests/test_gpu_guards.py on the 192-cell kernels (k_fx_* / k_fy_* / k_fz_mid with M = 12, k_pz_mid3):
+    inputs inside NaN slabs, outputs and the workspace inside canary slabs, every entry point three times over --
+    finite, canaries intact, repetitions bit-identical, guarded equal to plain."""
+    import test_gpu_guards as gg
+    monkeypatch.setenv("NM_FAST192", "1")
+    make = lambda: gg._cube(n)
+    reps, out_ok, ws_ok, path = gg._run(make, prec, guarded=True)
+    assert path == 1 and ws_ok and out_ok
+    for t_ in reps[0]:
+        assert bool(torch.isfinite(t_).all()), "an input was read outside its array (NaN guard band)"
+    for r in reps[1:]:
+        for x, y in zip(reps[0], r):
+            assert torch.equal(x, y), "results differ between identical runs"
+    plain, _, ws_ok2, _ = gg._run(make, prec, guarded=False)
+    assert ws_ok2
+    for x, y in zip(reps[0], plain[0]):
+        assert torch.equal(x, y), "guarded and plain runs differ"

@@ -1025,8 +1025,9 @@ template <> __device__ __forceinline__ void store2<float2>(float2 *dst, float2 a
 }
 template <> __device__ __forceinline__ void store2<double2>(double2 *dst, double2 a, double2 b)
 {
-    dst[0] = a;
-    dst[1] = b;
+    // one 32-byte store (sm_100: 256-bit global vector access; dst is 32-byte aligned): two 16-byte stores would each
+    // fill half a sector, and the store queue is what this loop waits on in fp64
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(dst), "d"(a.x), "d"(a.y), "d"(b.x), "d"(b.y) : "memory");
 }
 template <typename V> __device__ __forceinline__ void load2(const V *src, V &a, V &b);
 template <> __device__ __forceinline__ void load2<float2>(const float2 *src, float2 &a, float2 &b)

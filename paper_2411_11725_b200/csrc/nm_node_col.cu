@@ -97,7 +97,7 @@ template <typename P> __device__ __forceinline__ P *comp(P *base, int j, size_t 
 // arithmetic: the start-of-step state (Runge-Kutta), a (ADJ1) or d (ADJ2).
 template <typename T, int CM>
 __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, size_t nn, const T *mc,
-                                           const T *H, const T *f, T sms, const T *y0, double &err2)
+                                           const T *H, const T *f, T sms, const T *y0, const T *sp, double &err2)
 {
     if (CM == CM_H) {
 #pragma unroll
@@ -124,8 +124,7 @@ __device__ __forceinline__ void epilogue_c(const NmLocalArgs<T> &a, unsigned n, 
         if (CM == CM_RKS) {
 #pragma unroll
             for (int j = 0; j < 3; ++j)
-                base[j] = r.bs[0] * y0[j] + r.bs[1] * comp(r.sprev[0], j, nn)[n] + r.bs[2] * comp(r.sprev[1], j, nn)[n] +
-                          r.bs[3] * mc[j];
+                base[j] = r.bs[0] * y0[j] + r.bs[1] * sp[j] + r.bs[2] * sp[3 + j] + r.bs[3] * mc[j];    // sp: the two stage states, loaded with y0
         } else if (CM == CM_RKN) {
             for (int q = 0; q < r.nprev; ++q) {
                 const T *kp = r.kprev[q] + n;
@@ -491,14 +490,19 @@ k_node_col(const NmLocalArgs<T> a, int zchunk)
         const bool zout = z >= z0 && z < z1;
         // what the epilogue reads at its nodes (start-of-step state, a, or d): loaded now, used after
         // the plane arithmetic
-        T y0[RY][3];
+        T y0[RY][3], ys[RY][CM == CM_RKS ? 6 : 1];
         if ((RK || CM == CM_ADJ1 || CM == CM_ADJ2) && zout) {
             const T *pre = RK ? a.rk.y0 : (CM == CM_ADJ1 ? a.adj : a.dadt);
 #pragma unroll
             for (int ry = 0; ry < RY; ++ry)
 #pragma unroll
-                for (int j = 0; j < 3; ++j)
+                for (int j = 0; j < 3; ++j) {
                     y0[ry][j] = rowlive[ry] ? comp(pre, j, nn)[nbase + ry * n1] : (T)0;
+                    if (CM == CM_RKS) {     // last RK4 stage: the two stage states it combines, too (their latency was the epilogue's)
+                        ys[ry][j] = rowlive[ry] ? comp(a.rk.sprev[0], j, nn)[nbase + ry * n1] : (T)0;
+                        ys[ry][3 + j] = rowlive[ry] ? comp(a.rk.sprev[1], j, nn)[nbase + ry * n1] : (T)0;
+                    }
+                }
         }
         // plane-uniform z coefficients: plane k is the centre of output k, the upper neighbour of
         // output k - 1 and the lower neighbour of output k + 1
@@ -631,7 +635,7 @@ k_node_col(const NmLocalArgs<T> a, int zchunk)
                     const T mc[3] = {ry ? mcp[0].y : mcp[0].x, ry ? mcp[1].y : mcp[1].x, ry ? mcp[2].y : mcp[2].x};
                     const T H[3] = {ry ? Hp[0].y : Hp[0].x, ry ? Hp[1].y : Hp[1].x, ry ? Hp[2].y : Hp[2].x};
                     const T f[3] = {ry ? fp[0].y : fp[0].x, ry ? fp[1].y : fp[1].x, ry ? fp[2].y : fp[2].x};
-                    epilogue_c<T, CM>(a, nrow[ry], nn, mc, H, f, ry ? smsp.y : smsp.x, y0[ry], err2);
+                    epilogue_c<T, CM>(a, nrow[ry], nn, mc, H, f, ry ? smsp.y : smsp.x, y0[ry], ys[ry], err2);
                 }
             }
         }

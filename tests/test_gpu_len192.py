@@ -26,7 +26,9 @@ def _cube(n):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("n", [(192, 32, 16), (32, 192, 32), (32, 32, 192), (192, 64, 192)])
+# (the last two: a 192-cell axis beside axes the persistent TMA pipelines serve -- k_py_* with 192 planes, k_pz_mid with
+# 385 ky rows, k_px_* feeding k_fy_* with M = 12)
+@pytest.mark.parametrize("n", [(192, 32, 16), (32, 192, 32), (32, 32, 192), (192, 64, 192), (32, 256, 192), (256, 192, 32)])
 def test_native_192_axis_against_the_oracle(n, prec, monkeypatch):
     from oracle import llg
     td, nd = DT[prec], np_dtype(DT[prec])

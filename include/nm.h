@@ -117,7 +117,12 @@ nm_status nm_mesh_query_workspace(const nm_mesh_desc *desc, size_t *bytes_out);
  * queried size).  Computes the demag tensor of uniformly magnetised cuboids (reading C4: Newell
  * closed form in __float128 near the origin, 6-D Gauss quadrature of the dipole kernel beyond
  * 8 cell sizes; both agree with the closed form to < 1e-15), its real, symmetric spectrum with
- * 1/(P1 P2 P3) folded in, S Ms and the FFT tables.  Synchronous; not part of the hot path. */
+ * 1/(P1 P2 P3) folded in, S Ms and the FFT tables.  Synchronous; not part of the hot path.
+ * Environment switches, read here (and by nm_mesh_query_workspace) once, for tests and measurements; none changes a
+ * result beyond rounding: NM_DEMAG_PATH=generic (general-size demag kernels), NM_PIPE=0 (one-CTA-per-tile fast
+ * kernels), NM_KT_CHUNK=c (k1 tiles per y/z/y launch group), NM_NODE_PATH=generic|sep|ring (forms of the node
+ * kernel), NM_GRAPH=0|1 (whole-step launch replay), NM_FAST192=1 (an axis of 192 cells transformed at its own
+ * length, 3 x 64, instead of zero-extended to 256; slower). */
 nm_status nm_mesh_create(nm_mesh **out, const nm_mesh_desc *desc, void *workspace, size_t bytes);
 
 /* Replace the cell-wise saturation magnetisation (device array) and recompute S Ms. */
